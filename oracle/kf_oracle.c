@@ -1,0 +1,479 @@
+/*
+ * kf_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, double-precision CPU statement of what the hot path computes: batched
+ * Kalman-filter track fitting and best-hit candidate scoring in a cylindrical barrel
+ * (arXiv:1705.02876; "seeding, building, fitting" + chi2; PAPER.md:65 6x6 track /
+ * 3x3 hit matrices in global coordinates; PAPER.md:71 projective bins; PAPER.md:73 best hit =
+ * lowest chi2 increment; equations: BASELINE.json:north_star).  The paper prints no formulas;
+ * every formula below is a reading listed in DESIGN.md ("Readings A1..A17").
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * load this.  It shares no code, header, table or constant with the CUDA path
+ * (paper_1705_02876_b200/csrc) and is never a fallback for it.
+ *
+ * Conventions: AoS per track, dense 6x6 row-major matrices, no blocking / fusion / reordering.
+ * State u = (x, y, z, px, py, pz) [cm, GeV/c]; charge q = +-1; B = Bz z-hat [Tesla].
+ *
+ * Pins (tests/test_oracle_pins.py): P1 exact helix recovery, P2 propagation invariants + RK4 +
+ * worked value, P3 Jacobian vs finite differences / radial null / |p| conservation, P4 EKF ==
+ * batch weighted least squares, P5 covariance PSD rank 5, P6 pulls and chi2/ndf, P7 Highland
+ * check values, P8 window scoring == brute force, P9 bin structure, P10 rotation symmetry.
+ * Parity-unpinned: none of the functions below (efficiency / fake rate of PAPER.md:85 is not
+ * computed here at all).
+ */
+#include <math.h>
+#include <pthread.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_C_B 2.99792458e-3 /* GeV/(c T cm), reading A1 */
+#define ORC_PI 3.14159265358979323846
+
+enum { ORC_PROP_FAIL = 1, ORC_S_NOT_PD = 2, ORC_NONFINITE = 4, ORC_BAD_CHARGE = 8 };
+
+/* ---- Highland multiple-scattering width (reading A5) --------------------------------------
+ * theta0 = 0.0136 GeV / (beta p) * sqrt(t) * (1 + 0.038 ln t), t = x/X0 (flat), beta = p/E. */
+double orc_theta0(double p, double mass, double t) {
+    if (t <= 0.0) return 0.0;
+    double beta = p / sqrt(p * p + mass * mass);
+    return 0.0136 / (beta * p) * sqrt(t) * (1.0 + 0.038 * log(t));
+}
+
+/* ---- helix propagation to the cylinder of radius r, with Jacobian (readings A2, A3, A4) ----
+ * Equations of motion, s = transverse path length, kappa = k / pT, k = q c_B Bz:
+ *   dx/ds = px/pT  dy/ds = py/pT  dz/ds = pz/pT  dpx/ds = kappa py  dpy/ds = -kappa px  dpz/ds = 0
+ * Solution with theta = kappa s, S = sin theta, Cm = 1 - cos theta:
+ *   x' = x + (px S + py Cm)/k   y' = y + (py S - px Cm)/k   z' = z + pz s/pT
+ *   px' = px cos + py S         py' = -px S + py cos        pz' = pz
+ * First outward crossing of |pos'| = r:  a S - b Cm = D with
+ *   a = x px + y py,  b = (y px - x py) - pT^2/k,  D = (k/2)(r^2 - x^2 - y^2);
+ *   t = tan(theta/2) = D / (a + sqrt(a^2 - D(2b + D))).
+ * F = A + (df/ds) (x) (ds/du): A = d(map)/du at fixed s, ds/du from the constraint |pos'| = r.
+ * Returns 0 or ORC_PROP_FAIL (then nothing is written). F may be NULL. */
+int orc_propagate(const double u[6], double q, double Bz, double r, double out[6], double F[36],
+                  double *s_out, double *theta_out) {
+    double x = u[0], y = u[1], z = u[2], px = u[3], py = u[4], pz = u[5];
+    double k = q * ORC_C_B * Bz;
+    double pt2 = px * px + py * py;
+    double pt = sqrt(pt2);
+    double rho2 = x * x + y * y;
+    if (!(r * r > rho2)) return ORC_PROP_FAIL;
+    double a = x * px + y * py;
+    double b = (y * px - x * py) - pt2 / k;
+    double D = 0.5 * k * (r * r - rho2);
+    double disc = a * a - D * (2.0 * b + D);
+    if (!(disc > 0.0)) return ORC_PROP_FAIL;
+    double den = a + sqrt(disc);
+    if (!(den > 0.0)) return ORC_PROP_FAIL;
+    double t = D / den;
+    double S = 2.0 * t / (1.0 + t * t);
+    double Cm = 2.0 * t * t / (1.0 + t * t);
+    double co = 1.0 - Cm;
+    double theta = 2.0 * atan(t);
+    double s = theta * pt / k;
+    double xn = x + (px * S + py * Cm) / k;
+    double yn = y + (py * S - px * Cm) / k;
+    double zn = z + pz * s / pt;
+    double pxn = px * co + py * S;
+    double pyn = -px * S + py * co;
+    if (F) {
+        double A[6][6];
+        memset(A, 0, sizeof A);
+        for (int i = 0; i < 6; ++i) A[i][i] = 1.0;
+        double taux = -theta * px / pt2, tauy = -theta * py / pt2; /* d theta / d(px,py) at fixed s */
+        A[0][3] = S / k + pxn * taux / k;
+        A[0][4] = Cm / k + pxn * tauy / k;
+        A[1][3] = -Cm / k + pyn * taux / k;
+        A[1][4] = S / k + pyn * tauy / k;
+        A[2][3] = -pz * s * px / (pt2 * pt);
+        A[2][4] = -pz * s * py / (pt2 * pt);
+        A[2][5] = s / pt;
+        A[3][3] = co + pyn * taux;
+        A[3][4] = S + pyn * tauy;
+        A[4][3] = -S - pxn * taux;
+        A[4][4] = co - pxn * tauy;
+        double kap = k / pt;
+        double dfds[6] = {pxn / pt, pyn / pt, pz / pt, kap * pyn, -kap * pxn, 0.0};
+        double vr = (xn * pxn + yn * pyn) / pt; /* d(|pos'|^2 / 2)/ds */
+        for (int c = 0; c < 6; ++c) {
+            double dsdu = -(xn * A[0][c] + yn * A[1][c]) / vr;
+            for (int i = 0; i < 6; ++i) F[i * 6 + c] = A[i][c] + dfds[i] * dsdu;
+        }
+    }
+    out[0] = xn; out[1] = yn; out[2] = zn; out[3] = pxn; out[4] = pyn; out[5] = pz;
+    if (s_out) *s_out = s;
+    if (theta_out) *theta_out = theta;
+    return 0;
+}
+
+/* ---- process noise (reading A5): thin scatterer at the layer, evaluated at the propagated
+ * momentum p': Q_pp = theta0^2 (|p|^2 I3 - p p^T), all other blocks zero. */
+void orc_process_noise(const double u[6], double mass, double t, double Q[36]) {
+    memset(Q, 0, 36 * sizeof(double));
+    double p2 = u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+    double th0 = orc_theta0(sqrt(p2), mass, t);
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+            Q[(3 + i) * 6 + 3 + j] = th0 * th0 * ((i == j ? p2 : 0.0) - u[3 + i] * u[3 + j]);
+}
+
+/* C' = F C F^T + Q (north_star), dense triple loops. */
+void orc_transport_cov(const double F[36], const double C[36], const double Q[36], double out[36]) {
+    double FC[36];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double acc = 0.0;
+            for (int m = 0; m < 6; ++m) acc += F[i * 6 + m] * C[m * 6 + j];
+            FC[i * 6 + j] = acc;
+        }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double acc = 0.0;
+            for (int m = 0; m < 6; ++m) acc += FC[i * 6 + m] * F[j * 6 + m];
+            out[i * 6 + j] = acc + Q[i * 6 + j];
+        }
+}
+
+/* inverse of a symmetric 3x3 by cofactors; returns det */
+static double inv3(const double S[9], double Si[9]) {
+    double c00 = S[4] * S[8] - S[5] * S[7];
+    double c01 = S[5] * S[6] - S[3] * S[8];
+    double c02 = S[3] * S[7] - S[4] * S[6];
+    double det = S[0] * c00 + S[1] * c01 + S[2] * c02;
+    double id = 1.0 / det;
+    Si[0] = c00 * id;
+    Si[1] = (S[2] * S[7] - S[1] * S[8]) * id;
+    Si[2] = (S[1] * S[5] - S[2] * S[4]) * id;
+    Si[3] = c01 * id;
+    Si[4] = (S[0] * S[8] - S[2] * S[6]) * id;
+    Si[5] = (S[2] * S[3] - S[0] * S[5]) * id;
+    Si[6] = c02 * id;
+    Si[7] = (S[1] * S[6] - S[0] * S[7]) * id;
+    Si[8] = (S[0] * S[4] - S[1] * S[3]) * id;
+    return det;
+}
+
+/* ---- chi2 increment of hit (m, V) against state (u, C) (readings A6, A8):
+ * r = m - H u, H = [I3 0]; S = C_pp + V; chi2 = r^T S^-1 r.  Returns 0 / ORC_S_NOT_PD. */
+int orc_chi2_increment(const double u[6], const double C[36], const double m[3], const double V[9],
+                       double *chi2) {
+    double S[9], Si[9], r[3];
+    for (int i = 0; i < 3; ++i) {
+        r[i] = m[i] - u[i];
+        for (int j = 0; j < 3; ++j) S[i * 3 + j] = C[i * 6 + j] + V[i * 3 + j];
+    }
+    if (!(inv3(S, Si) > 0.0)) return ORC_S_NOT_PD;
+    double c = 0.0;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) c += r[i] * Si[i * 3 + j] * r[j];
+    *chi2 = c;
+    return 0;
+}
+
+/* ---- Kalman update (reading A8): K = C H^T S^-1; x = u + K r;
+ * C_new = (I - K H) C (I - K H)^T + K V K^T  (Joseph form of C - K H C), symmetrised. */
+int orc_update(const double u[6], const double C[36], const double m[3], const double V[9],
+               double uo[6], double Co[36], double *chi2) {
+    double S[9], Si[9], r[3], K[18], c = 0.0;
+    for (int i = 0; i < 3; ++i) {
+        r[i] = m[i] - u[i];
+        for (int j = 0; j < 3; ++j) S[i * 3 + j] = C[i * 6 + j] + V[i * 3 + j];
+    }
+    if (!(inv3(S, Si) > 0.0)) return ORC_S_NOT_PD;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) c += r[i] * Si[i * 3 + j] * r[j];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double acc = 0.0;
+            for (int m2 = 0; m2 < 3; ++m2) acc += C[i * 6 + m2] * Si[m2 * 3 + j];
+            K[i * 3 + j] = acc;
+        }
+    double un[6];
+    for (int i = 0; i < 6; ++i) un[i] = u[i] + K[i * 3] * r[0] + K[i * 3 + 1] * r[1] + K[i * 3 + 2] * r[2];
+    double A[36], AC[36], Cn[36];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) A[i * 6 + j] = (i == j ? 1.0 : 0.0) - (j < 3 ? K[i * 3 + j] : 0.0);
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double acc = 0.0;
+            for (int m2 = 0; m2 < 6; ++m2) acc += A[i * 6 + m2] * C[m2 * 6 + j];
+            AC[i * 6 + j] = acc;
+        }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double acc = 0.0;
+            for (int m2 = 0; m2 < 6; ++m2) acc += AC[i * 6 + m2] * A[j * 6 + m2];
+            for (int a2 = 0; a2 < 3; ++a2)
+                for (int b2 = 0; b2 < 3; ++b2) acc += K[i * 3 + a2] * V[a2 * 3 + b2] * K[j * 3 + b2];
+            Cn[i * 6 + j] = acc;
+        }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) Co[i * 6 + j] = 0.5 * (Cn[i * 6 + j] + Cn[j * 6 + i]);
+    int finite = isfinite(c);
+    for (int i = 0; i < 6; ++i) finite = finite && isfinite(un[i]);
+    if (!finite) return ORC_NONFINITE;
+    memcpy(uo, un, sizeof un);
+    *chi2 = c;
+    return 0;
+}
+
+/* ---- one track, all layers (readings A10, A11): layers in increasing radius; a layer whose
+ * mask bit is 0 is skipped entirely; a layer that fails (propagation / S / non-finite) sets the
+ * status bit and leaves state and covariance as they were before that layer.
+ * trace (optional): per layer 122 doubles = x_pred[6] F[36] Q[36] x_filt[6] C_filt[36] dchi2 used */
+#define ORC_TRACE_STRIDE 122
+static void fit_one(int L, const double *radius, const double *xX0, double Bz, double mass,
+                    const double par[6], const double cov[36], int q, const double *hpos,
+                    const double *hcov, uint32_t mask, double opar[6], double ocov[36],
+                    double *ochi2, int32_t *onhits, uint32_t *ostatus, double *trace) {
+    double u[6], C[36];
+    memcpy(u, par, sizeof u);
+    memcpy(C, cov, sizeof C);
+    double chi2 = 0.0;
+    int nh = 0;
+    uint32_t st = 0;
+    if (q != 1 && q != -1) {
+        st = ORC_BAD_CHARGE;
+    } else {
+        for (int l = 0; l < L; ++l) {
+            double *tr = trace ? trace + (size_t)l * ORC_TRACE_STRIDE : NULL;
+            if (tr) memset(tr, 0, ORC_TRACE_STRIDE * sizeof(double));
+            if (!((mask >> l) & 1u)) continue;
+            double up[6], F[36], Q[36], Cp[36], un[6], Cn[36], dchi2;
+            int rc = orc_propagate(u, (double)q, Bz, radius[l], up, F, NULL, NULL);
+            if (rc) { st |= (uint32_t)rc; continue; }
+            orc_process_noise(up, mass, xX0[l], Q);
+            orc_transport_cov(F, C, Q, Cp);
+            rc = orc_update(up, Cp, hpos + 3 * l, hcov + 9 * l, un, Cn, &dchi2);
+            if (rc) { st |= (uint32_t)rc; continue; }
+            memcpy(u, un, sizeof u);
+            memcpy(C, Cn, sizeof C);
+            chi2 += dchi2;
+            nh += 1;
+            if (tr) {
+                memcpy(tr, up, 6 * sizeof(double));
+                memcpy(tr + 6, F, 36 * sizeof(double));
+                memcpy(tr + 42, Q, 36 * sizeof(double));
+                memcpy(tr + 78, u, 6 * sizeof(double));
+                memcpy(tr + 84, C, 36 * sizeof(double));
+                tr[120] = dchi2;
+                tr[121] = 1.0;
+            }
+        }
+    }
+    memcpy(opar, u, sizeof u);
+    memcpy(ocov, C, sizeof C);
+    *ochi2 = chi2;
+    *onhits = nh;
+    *ostatus = st;
+}
+
+typedef struct {
+    int64_t lo, hi;
+    int L;
+    const double *radius, *xX0;
+    double Bz, mass;
+    const double *par, *cov;
+    const int8_t *q;
+    const double *hpos, *hcov;
+    const uint32_t *mask;
+    double *opar, *ocov, *ochi2;
+    int32_t *onhits;
+    uint32_t *ostatus;
+    double *trace;
+} fit_job;
+
+static void *fit_range(void *p) {
+    fit_job *j = (fit_job *)p;
+    for (int64_t i = j->lo; i < j->hi; ++i)
+        fit_one(j->L, j->radius, j->xX0, j->Bz, j->mass, j->par + 6 * i, j->cov + 36 * i, j->q[i],
+                j->hpos + (size_t)i * j->L * 3, j->hcov + (size_t)i * j->L * 9,
+                j->mask ? j->mask[i] : 0xffffffffu, j->opar + 6 * i, j->ocov + 36 * i, j->ochi2 + i,
+                j->onhits + i, j->ostatus + i,
+                j->trace ? j->trace + (size_t)i * j->L * ORC_TRACE_STRIDE : NULL);
+    return NULL;
+}
+
+/* Batched fit.  AoS double inputs: par[n][6], cov[n][36], hpos[n][L][3], hcov[n][L][9].
+ * nthreads >= 1: contiguous track ranges, one pthread each. */
+int orc_fit_tracks(int64_t n, int L, const double *radius, const double *xX0, double Bz, double mass,
+                   const double *par, const double *cov, const int8_t *q, const double *hpos,
+                   const double *hcov, const uint32_t *mask, double *opar, double *ocov,
+                   double *ochi2, int32_t *onhits, uint32_t *ostatus, double *trace, int nthreads) {
+    if (nthreads < 1) nthreads = 1;
+    if (nthreads > 256) nthreads = 256;
+    fit_job jobs[256];
+    pthread_t th[256];
+    for (int t = 0; t < nthreads; ++t) {
+        fit_job j = {n * t / nthreads, n * (t + 1) / nthreads, L, radius, xX0, Bz, mass, par, cov, q,
+                     hpos, hcov, mask, opar, ocov, ochi2, onhits, ostatus, trace};
+        jobs[t] = j;
+    }
+    if (nthreads == 1) {
+        fit_range(&jobs[0]);
+        return 0;
+    }
+    for (int t = 0; t < nthreads; ++t)
+        if (pthread_create(&th[t], NULL, fit_range, &jobs[t])) return -1;
+    for (int t = 0; t < nthreads; ++t) pthread_join(th[t], NULL);
+    return 0;
+}
+
+/* ---- hit binning (reading A16, "directionally projective bins") ----------------
+ * Definition: eta = asinh(z / r_layer), phi = atan2(y, x);
+ *   i_eta = clamp(floor((eta + eta_max) / (2 eta_max / n_eta)), 0, n_eta-1)
+ *   i_phi = floor((phi + pi) / (2 pi / n_phi)) mod n_phi;  bin = i_eta * n_phi + i_phi.        */
+int32_t orc_bin_index_def(double x, double y, double z, double r_layer, int n_eta, int n_phi,
+                          double eta_max) {
+    double eta = asinh(z / r_layer), phi = atan2(y, x);
+    int ie = (int)floor((eta + eta_max) / (2.0 * eta_max / n_eta));
+    if (ie < 0) ie = 0;
+    if (ie > n_eta - 1) ie = n_eta - 1;
+    int ip = (int)floor((phi + ORC_PI) / (2.0 * ORC_PI / n_phi));
+    ip = ((ip % n_phi) + n_phi) % n_phi;
+    return ie * n_phi + ip;
+}
+
+/* The same bins decided in SINGLE precision without transcendental calls, so that a hit that
+ * sits within rounding of a bin edge gets one well-defined bin (reading A16b: where
+ * floating point decides an integer both sides decide in the kernel's precision):
+ *   u = fl32(z / r);            i_eta = #{ j in 1..n_eta-1 : u >= fl32(sinh(-eta_max + j d_eta)) }
+ *   upper half plane (y > 0, or y == 0 and x > 0):
+ *       i_phi = n_phi/2 + #{ j in n_phi/2+1..n_phi-1 : fl32(cx_j * y) >= fl32(sy_j * x) }
+ *   y == 0 and x <= 0: i_phi = 0 (phi = +-pi wraps to the first bin)
+ *   lower half plane (y < 0): i_phi = #{ j in 1..n_phi/2-1 : fl32(cx_j * y) >= fl32(sy_j * x) }
+ *   (cx_j, sy_j) = fl32(cos, sin)(-pi + j 2pi/n_phi): "the hit is at or counter-clockwise past
+ *   edge j".  Compiled with -ffp-contract=off: every product is rounded to float once. */
+int32_t orc_bin_index_f32(float x, float y, float z, float r_layer, int n_eta, int n_phi,
+                          double eta_max) {
+    volatile float u = z / r_layer;
+    int ie = 0;
+    for (int j = 1; j < n_eta; ++j) {
+        float edge = (float)sinh(-eta_max + j * (2.0 * eta_max / n_eta));
+        ie += (u >= edge);
+    }
+    int half = n_phi / 2, ip;
+    if (y > 0.0f || (y == 0.0f && x > 0.0f)) {
+        ip = half;
+        for (int j = half + 1; j < n_phi; ++j) {
+            float cx = (float)cos(-ORC_PI + j * (2.0 * ORC_PI / n_phi));
+            float sy = (float)sin(-ORC_PI + j * (2.0 * ORC_PI / n_phi));
+            volatile float lhs = cx * y, rhs = sy * x;
+            ip += (lhs >= rhs);
+        }
+    } else if (y == 0.0f) {
+        ip = 0;
+    } else {
+        ip = 0;
+        for (int j = 1; j < half; ++j) {
+            float cx = (float)cos(-ORC_PI + j * (2.0 * ORC_PI / n_phi));
+            float sy = (float)sin(-ORC_PI + j * (2.0 * ORC_PI / n_phi));
+            volatile float lhs = cx * y, rhs = sy * x;
+            ip += (lhs >= rhs);
+        }
+    }
+    return ie * n_phi + ip;
+}
+
+/* Stable counting sort of one layer's hits by bin (single-precision decision rule).
+ * bin_offset[n_bins+1], sorted_to_orig[n_hits]; bin_of[n_hits] (optional) receives each bin. */
+void orc_bin_hits(int64_t n_hits, const float *x, const float *y, const float *z, float r_layer,
+                  int n_eta, int n_phi, double eta_max, int32_t *bin_offset, int32_t *sorted_to_orig,
+                  int32_t *bin_of) {
+    int nb = n_eta * n_phi;
+    int32_t *b = (int32_t *)malloc((size_t)(n_hits > 0 ? n_hits : 1) * sizeof(int32_t));
+    for (int i = 0; i <= nb; ++i) bin_offset[i] = 0;
+    for (int64_t h = 0; h < n_hits; ++h) {
+        b[h] = orc_bin_index_f32(x[h], y[h], z[h], r_layer, n_eta, n_phi, eta_max);
+        bin_offset[b[h] + 1] += 1;
+    }
+    for (int i = 0; i < nb; ++i) bin_offset[i + 1] += bin_offset[i];
+    int32_t *cur = (int32_t *)malloc((size_t)(nb > 0 ? nb : 1) * sizeof(int32_t));
+    for (int i = 0; i < nb; ++i) cur[i] = bin_offset[i];
+    for (int64_t h = 0; h < n_hits; ++h) sorted_to_orig[cur[b[h]]++] = (int32_t)h;
+    if (bin_of) memcpy(bin_of, b, (size_t)n_hits * sizeof(int32_t));
+    free(cur);
+    free(b);
+}
+
+/* ---- best-hit candidate scoring on one layer (reading A16) --------------------
+ * Per candidate: propagate to r_layer (+Q); candidate bin from its own (eta, phi) by the
+ * definition formula; window i_eta +- w clipped, i_phi +- w wrapped; chi2 of every hit in the
+ * window; best = lowest chi2, exact ties -> lowest original index; accept iff chi2 < cut; accepted
+ * and do_update: Kalman update, nhits += 1, chi2 += best.  Otherwise best_hit = -1 and the state
+ * stays the propagated one.  best_chi2 = lowest chi2 seen (INFINITY if the window is empty).
+ * Propagation failure: status bit, candidate untouched, best_hit = -1, best_chi2 = INFINITY.
+ * all_hits != 0: ignore the bins and scan every hit of the layer (brute force, pin P8).
+ * Hits: double AoS hpos[H][3], hcov[H][9] in ORIGINAL order. */
+void orc_score_layer(int64_t n, double r_layer, double xX0, double Bz, double mass, double *par,
+                     double *cov, const int8_t *q, double *chi2, int32_t *nhits, uint32_t *status,
+                     int64_t n_hits, const double *hpos, const double *hcov, int n_eta, int n_phi,
+                     double eta_max, const int32_t *bin_offset, const int32_t *sorted_to_orig,
+                     int window_half, double chi2_cut, int do_update, int all_hits,
+                     int32_t *best_hit, double *best_chi2, double *second_chi2) {
+    for (int64_t i = 0; i < n; ++i) {
+        double *u = par + 6 * i, *C = cov + 36 * i;
+        best_hit[i] = -1;
+        best_chi2[i] = INFINITY;
+        if (second_chi2) second_chi2[i] = INFINITY;
+        if (q[i] != 1 && q[i] != -1) { status[i] |= ORC_BAD_CHARGE; continue; }
+        double up[6], F[36], Q[36], Cp[36];
+        int rc = orc_propagate(u, (double)q[i], Bz, r_layer, up, F, NULL, NULL);
+        if (rc) { status[i] |= (uint32_t)rc; continue; }
+        orc_process_noise(up, mass, xX0, Q);
+        orc_transport_cov(F, C, Q, Cp);
+        double best = INFINITY, second = INFINITY;
+        int32_t bh = -1;
+        if (all_hits) {
+            for (int64_t h = 0; h < n_hits; ++h) {
+                double c;
+                if (orc_chi2_increment(up, Cp, hpos + 3 * h, hcov + 9 * h, &c)) continue;
+                if (c < best || (c == best && (int32_t)h < bh)) { second = best; best = c; bh = (int32_t)h; }
+                else if (c < second) second = c;
+            }
+        } else {
+            int cb = orc_bin_index_def(up[0], up[1], up[2], r_layer, n_eta, n_phi, eta_max);
+            int ie = cb / n_phi, ip = cb % n_phi;
+            for (int de = -window_half; de <= window_half; ++de) {
+                int e = ie + de;
+                if (e < 0 || e >= n_eta) continue;
+                for (int dp = -window_half; dp <= window_half; ++dp) {
+                    int p = ((ip + dp) % n_phi + n_phi) % n_phi;
+                    if (2 * window_half + 1 > n_phi && dp > -window_half + n_phi - 1) continue;
+                    int bin = e * n_phi + p;
+                    for (int32_t sidx = bin_offset[bin]; sidx < bin_offset[bin + 1]; ++sidx) {
+                        int32_t h = sorted_to_orig[sidx];
+                        double c;
+                        if (orc_chi2_increment(up, Cp, hpos + 3 * (size_t)h, hcov + 9 * (size_t)h, &c)) continue;
+                        if (c < best || (c == best && h < bh)) { second = best; best = c; bh = h; }
+                        else if (c < second) second = c;
+                    }
+                }
+            }
+        }
+        best_chi2[i] = best;
+        if (second_chi2) second_chi2[i] = second;
+        int accepted = 0;
+        if (bh >= 0 && best < chi2_cut) {
+            if (do_update) {
+                double un[6], Cn[36], c;
+                rc = orc_update(up, Cp, hpos + 3 * (size_t)bh, hcov + 9 * (size_t)bh, un, Cn, &c);
+                if (rc) { status[i] |= (uint32_t)rc; }
+                else {
+                    memcpy(u, un, 6 * sizeof(double));
+                    memcpy(C, Cn, 36 * sizeof(double));
+                    chi2[i] += c;
+                    nhits[i] += 1;
+                    accepted = 1;
+                }
+            } else accepted = 2;
+            best_hit[i] = bh;
+        }
+        if (accepted != 1) { /* state = propagated one (Q included) */
+            memcpy(u, up, 6 * sizeof(double));
+            memcpy(C, Cp, 36 * sizeof(double));
+        }
+    }
+}

@@ -1,0 +1,233 @@
+"""ctypes loader for oracle/kf_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Layout conversion only (fp32 SoA inputs -> double AoS, packed 21 -> dense 6x6, packed 6 -> dense
+3x3).  All arithmetic of the method lives in kf_oracle.c; see its header for the citations, the
+readings it follows and the pins.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this module.  It never imports the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "kf_oracle.c")
+_LIB = os.path.join(_HERE, "libkf_oracle.so")
+
+PROP_FAIL, S_NOT_PD, NONFINITE, BAD_CHARGE = 1, 2, 4, 8
+TRACE_STRIDE = 122
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (no contraction: every float product is rounded once)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared",
+                               "-o", _LIB, _SRC, "-lm", "-lpthread"])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        dp = C.POINTER(C.c_double)
+        _lib.orc_theta0.restype = C.c_double
+        _lib.orc_theta0.argtypes = [C.c_double] * 3
+        _lib.orc_propagate.restype = C.c_int
+        _lib.orc_propagate.argtypes = [dp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
+        _lib.orc_process_noise.restype = None
+        _lib.orc_process_noise.argtypes = [dp, C.c_double, C.c_double, dp]
+        _lib.orc_transport_cov.restype = None
+        _lib.orc_transport_cov.argtypes = [dp, dp, dp, dp]
+        _lib.orc_chi2_increment.restype = C.c_int
+        _lib.orc_chi2_increment.argtypes = [dp, dp, dp, dp, dp]
+        _lib.orc_update.restype = C.c_int
+        _lib.orc_update.argtypes = [dp, dp, dp, dp, dp, dp, dp]
+        _lib.orc_fit_tracks.restype = C.c_int
+        _lib.orc_bin_index_def.restype = C.c_int32
+        _lib.orc_bin_index_def.argtypes = [C.c_double] * 4 + [C.c_int, C.c_int, C.c_double]
+        _lib.orc_bin_index_f32.restype = C.c_int32
+        _lib.orc_bin_index_f32.argtypes = [C.c_float] * 4 + [C.c_int, C.c_int, C.c_double]
+        _lib.orc_bin_hits.restype = None
+        _lib.orc_score_layer.restype = None
+    return _lib
+
+
+def _p(a, ct=C.c_double):
+    return a.ctypes.data_as(C.POINTER(ct)) if a is not None else None
+
+
+# ------------------------------------------------------------------ layout helpers (no arithmetic)
+_TRI = [(i, j) for i in range(6) for j in range(i, 6)]
+
+
+def unpack_cov21(c21: np.ndarray) -> np.ndarray:
+    """[21][n] packed upper triangle (row-major) -> [n][6][6] dense symmetric, float64."""
+    n = c21.shape[1]
+    out = np.empty((n, 6, 6))
+    for k, (i, j) in enumerate(_TRI):
+        out[:, i, j] = c21[k]
+        out[:, j, i] = c21[k]
+    return out
+
+
+def pack_cov21(c: np.ndarray) -> np.ndarray:
+    """[n][6][6] -> [21][n]."""
+    return np.stack([c[:, i, j] for (i, j) in _TRI])
+
+
+def unpack_cov6(v6: np.ndarray) -> np.ndarray:
+    """[..., 6, n] packed xx,xy,xz,yy,yz,zz -> [n, ..., 3, 3] dense, float64."""
+    v = np.moveaxis(np.asarray(v6, dtype=np.float64), -1, 0)          # [n, ..., 6]
+    idx = np.array([[0, 1, 2], [1, 3, 4], [2, 4, 5]])
+    return v[..., idx]
+
+
+# ------------------------------------------------------------------ scalar-level entry points
+def theta0(p, mass, t):
+    return lib().orc_theta0(float(p), float(mass), float(t))
+
+
+def propagate(u, q, Bz, r, want_F=True):
+    """-> (status, u_out[6], F[6,6] or None, s, theta)"""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    out = np.zeros(6)
+    F = np.zeros(36) if want_F else None
+    s = C.c_double(0.0)
+    th = C.c_double(0.0)
+    rc = lib().orc_propagate(_p(u), float(q), float(Bz), float(r), _p(out), _p(F), C.byref(s), C.byref(th))
+    return rc, out, (F.reshape(6, 6) if want_F else None), s.value, th.value
+
+
+def process_noise(u, mass, t):
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    Q = np.zeros(36)
+    lib().orc_process_noise(_p(u), float(mass), float(t), _p(Q))
+    return Q.reshape(6, 6)
+
+
+def transport_cov(F, Cm, Q):
+    F = np.ascontiguousarray(F, dtype=np.float64)
+    Cm = np.ascontiguousarray(Cm, dtype=np.float64)
+    Q = np.ascontiguousarray(Q, dtype=np.float64)
+    out = np.zeros(36)
+    lib().orc_transport_cov(_p(F), _p(Cm), _p(Q), _p(out))
+    return out.reshape(6, 6)
+
+
+def chi2_increment(u, Cm, m, V):
+    u, Cm, m, V = (np.ascontiguousarray(a, dtype=np.float64) for a in (u, Cm, m, V))
+    c = C.c_double(0.0)
+    rc = lib().orc_chi2_increment(_p(u), _p(Cm), _p(m), _p(V), C.byref(c))
+    return rc, c.value
+
+
+def update(u, Cm, m, V):
+    u, Cm, m, V = (np.ascontiguousarray(a, dtype=np.float64) for a in (u, Cm, m, V))
+    uo, Co = np.zeros(6), np.zeros(36)
+    c = C.c_double(0.0)
+    rc = lib().orc_update(_p(u), _p(Cm), _p(m), _p(V), _p(uo), _p(Co), C.byref(c))
+    return rc, uo, Co.reshape(6, 6), c.value
+
+
+# ------------------------------------------------------------------ batched fit
+def fit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None,
+               nthreads: int = 1, want_trace: bool = False) -> dict:
+    """Fit n tracks.  Inputs in the SoA fp32 layout of the C ABI (par[6][n], cov21[21][n],
+    hpos[L][3][n], hcov[L][6][n]); widened to double, transposed to AoS and handed to
+    orc_fit_tracks.  Returns dict(par[6][n], cov[n][6][6], chi2, nhits, status[, trace])."""
+    L = int(len(radius))
+    n = int(par.shape[1])
+    rad = np.ascontiguousarray(radius, dtype=np.float64)
+    xx0 = np.ascontiguousarray(x_over_X0, dtype=np.float64)
+    par_a = np.ascontiguousarray(np.asarray(par, dtype=np.float64).T)               # [n][6]
+    cov_a = np.ascontiguousarray(unpack_cov21(np.asarray(cov21, dtype=np.float64)))  # [n][6][6]
+    q_a = np.ascontiguousarray(q, dtype=np.int8)
+    hp_a = np.ascontiguousarray(np.transpose(np.asarray(hpos, dtype=np.float64), (2, 0, 1)))  # [n][L][3]
+    hc_a = np.ascontiguousarray(np.swapaxes(unpack_cov6(hcov), 0, 0))               # [n][L][3][3]
+    m_a = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint32)
+    opar = np.zeros((n, 6)); ocov = np.zeros((n, 6, 6)); ochi2 = np.zeros(n)
+    onh = np.zeros(n, dtype=np.int32); ost = np.zeros(n, dtype=np.uint32)
+    trace = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
+    rc = lib().orc_fit_tracks(C.c_int64(n), C.c_int(L), _p(rad), _p(xx0), C.c_double(Bz), C.c_double(mass),
+                              _p(par_a), _p(cov_a), _p(q_a, C.c_int8), _p(hp_a), _p(hc_a),
+                              _p(m_a, C.c_uint32), _p(opar), _p(ocov), _p(ochi2), _p(onh, C.c_int32),
+                              _p(ost, C.c_uint32), _p(trace), C.c_int(nthreads))
+    if rc != 0:
+        raise RuntimeError("orc_fit_tracks failed")
+    out = dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost)
+    if want_trace:
+        out["trace"] = trace
+    return out
+
+
+def fit_batch(batch, nthreads: int = 1, want_trace: bool = False) -> dict:
+    """Convenience: fit a workloads.barrel_events.FitBatch-shaped object (duck-typed)."""
+    return fit_tracks(batch.radius, batch.x_over_X0, batch.Bz, batch.mass, batch.par, batch.cov,
+                      batch.q, batch.hpos, batch.hcov, batch.mask, nthreads, want_trace)
+
+
+# ------------------------------------------------------------------ binning and scoring
+def bin_index_def(x, y, z, r_layer, n_eta, n_phi, eta_max):
+    return lib().orc_bin_index_def(float(x), float(y), float(z), float(r_layer), n_eta, n_phi, float(eta_max))
+
+
+def bin_index_f32(x, y, z, r_layer, n_eta, n_phi, eta_max):
+    return lib().orc_bin_index_f32(float(x), float(y), float(z), float(r_layer), n_eta, n_phi, float(eta_max))
+
+
+def bin_hits(pos, r_layer, n_eta, n_phi, eta_max) -> dict:
+    """pos[3][H] fp32 -> dict(bin_offset[n_bins+1], sorted_to_orig[H], bin_of[H])."""
+    pos = np.ascontiguousarray(pos, dtype=np.float32)
+    H = int(pos.shape[1])
+    off = np.zeros(n_eta * n_phi + 1, dtype=np.int32)
+    s2o = np.zeros(max(H, 1), dtype=np.int32)
+    bof = np.zeros(max(H, 1), dtype=np.int32)
+    x, y, z = (np.ascontiguousarray(pos[i]) for i in range(3))
+    lib().orc_bin_hits(C.c_int64(H), _p(x, C.c_float), _p(y, C.c_float), _p(z, C.c_float),
+                       C.c_float(r_layer), C.c_int(n_eta), C.c_int(n_phi), C.c_double(eta_max),
+                       _p(off, C.c_int32), _p(s2o, C.c_int32), _p(bof, C.c_int32))
+    return dict(bin_offset=off, sorted_to_orig=s2o[:H], bin_of=bof[:H])
+
+
+class Candidates:
+    """Double AoS candidate set the scoring oracle advances layer by layer."""
+
+    def __init__(self, par, cov21, q, chi2=None, nhits=None):
+        n = int(par.shape[1])
+        self.n = n
+        self.par = np.ascontiguousarray(np.asarray(par, dtype=np.float64).T)
+        self.cov = np.ascontiguousarray(unpack_cov21(np.asarray(cov21, dtype=np.float64)))
+        self.q = np.ascontiguousarray(q, dtype=np.int8)
+        self.chi2 = np.zeros(n) if chi2 is None else np.ascontiguousarray(chi2, dtype=np.float64).copy()
+        self.nhits = np.zeros(n, dtype=np.int32) if nhits is None else np.ascontiguousarray(nhits, dtype=np.int32).copy()
+        self.status = np.zeros(n, dtype=np.uint32)
+
+
+def score_layer(cands: Candidates, r_layer, x_over_X0, Bz, mass, hpos, hcov, bins: dict | None,
+                n_eta, n_phi, eta_max, window_half=2, chi2_cut=30.0, do_update=True,
+                all_hits=False) -> dict:
+    """Advance `cands` by one layer (in place).  hpos[3][H], hcov[6][H] fp32 in ORIGINAL order.
+    Returns dict(best_hit[n] (original index or -1), best_chi2[n], second_chi2[n])."""
+    hp = np.ascontiguousarray(np.asarray(hpos, dtype=np.float64).T)      # [H][3]
+    hc = np.ascontiguousarray(unpack_cov6(hcov))                          # [H][3][3]
+    H = int(hp.shape[0])
+    n = cands.n
+    bh = np.zeros(n, dtype=np.int32); bc = np.zeros(n); sc = np.zeros(n)
+    off = s2o = None
+    if not all_hits:
+        off = np.ascontiguousarray(bins["bin_offset"], dtype=np.int32)
+        s2o = np.ascontiguousarray(bins["sorted_to_orig"], dtype=np.int32)
+    lib().orc_score_layer(C.c_int64(n), C.c_double(r_layer), C.c_double(x_over_X0), C.c_double(Bz),
+                          C.c_double(mass), _p(cands.par), _p(cands.cov), _p(cands.q, C.c_int8),
+                          _p(cands.chi2), _p(cands.nhits, C.c_int32), _p(cands.status, C.c_uint32),
+                          C.c_int64(H), _p(hp), _p(hc), C.c_int(n_eta), C.c_int(n_phi), C.c_double(eta_max),
+                          _p(off, C.c_int32), _p(s2o, C.c_int32), C.c_int(window_half),
+                          C.c_double(chi2_cut), C.c_int(1 if do_update else 0), C.c_int(1 if all_hits else 0),
+                          _p(bh, C.c_int32), _p(bc), _p(sc))
+    return dict(best_hit=bh, best_chi2=bc, second_chi2=sc)

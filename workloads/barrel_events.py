@@ -1,0 +1,289 @@
+"""Seeded synthetic barrel-detector events (input generator only).
+
+This module stands in for the paper's in-house toy simulation (section 3.2:
+"equally spaced, fixed length concentric cylinders ... Gaussian smearing of the hit positions",
+seeds "derived from the first three hits"), which is not available.  The five workloads are the
+ones BASELINE.json:configs[0..4] describe; the recipe (distributions, sigmas, seed prior) is
+written out in DESIGN.md "Input recipe".
+
+It is shared by the tests, bench.py and __graft_entry__.smoke().  It contains NO Kalman-filter
+arithmetic (no Jacobian, no gain, no chi2, no binning) and imports neither `oracle/` nor the CUDA
+package: it only *simulates* truth particles (circle/cylinder intersection written as a two-circle
+intersection with atan2 turning angles -- deliberately a different formulation from the
+half-angle crossing the fit uses), smears hits, scatters the truth and smears a seed.
+
+All arithmetic is float64; everything handed to the fitters is rounded ONCE to float32
+(reading A17) so the oracle and the CUDA path see bit-identical inputs.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+C_B = 2.99792458e-3          # GeV / (c * Tesla * cm): p_T[GeV] = C_B * B[T] * R[cm]
+M_PION = 0.13957             # GeV, mass used for beta in the scattering angle
+BASE_SEED = 170502876
+
+SIGMA_RPHI = 0.01            # cm  (BASELINE.json:configs[0])
+SIGMA_Z = 0.1                # cm  (BASELINE.json:configs[0])
+SIGMA_R = 0.1                # cm  (reading A6: radial error assigned to a hit)
+SEED_POS_SMEAR = 0.03        # cm  (A13)
+SEED_MOM_SMEAR = 0.10        # fraction of true pT (A13, "smeared 10%")
+SEED_POS_SIGMA0 = 0.3        # cm, prior sigma on position (A13)
+SEED_MOM_SIGMA0 = 0.3        # fraction of seed pT, prior sigma on each momentum component (A13)
+
+
+@dataclass
+class BarrelConfig:
+    """One of BASELINE.json:configs[i] as numbers."""
+    index: int
+    n_events: int
+    n_tracks: int                 # per event
+    n_layers: int
+    pt_min: float
+    pt_max: float
+    eta_max: float
+    x_over_X0: float
+    Bz: float = 3.8
+    layer_step_cm: float = 4.0
+    noise_hits_per_layer: int = 0  # config 4 only
+    n_eta: int = 40                # config 4 only
+    n_phi: int = 64
+    eta_bin_max: float = 1.2
+    first_scored_layer: int = 3
+
+    @property
+    def radii(self) -> np.ndarray:
+        return self.layer_step_cm * np.arange(1, self.n_layers + 1, dtype=np.float64)
+
+
+def get_config(i: int) -> BarrelConfig:
+    if i == 0:
+        return BarrelConfig(0, 1, 1_000, 10, 0.5, 10.0, 1.0, 0.0)
+    if i == 1:
+        return BarrelConfig(1, 1, 20_000, 10, 0.5, 10.0, 1.0, 0.01)
+    if i == 2:
+        return BarrelConfig(2, 100, 20_000, 10, 0.5, 10.0, 1.0, 0.01)
+    if i == 3:
+        return BarrelConfig(3, 1, 100_000, 20, 0.3, 20.0, 1.5, 0.01)
+    if i == 4:
+        return BarrelConfig(4, 1, 20_000, 10, 0.5, 10.0, 1.0, 0.01, noise_hits_per_layer=100_000)
+    raise ValueError(f"no such config {i}")
+
+
+@dataclass
+class FitBatch:
+    """Inputs of one kf_fit_tracks call, SoA element-major, fp32 (what both fitters read)."""
+    n: int
+    radius: np.ndarray        # [L]  f32
+    x_over_X0: np.ndarray     # [L]  f32
+    Bz: float
+    mass: float
+    par: np.ndarray           # [6][n]  f32  seed x,y,z,px,py,pz
+    cov: np.ndarray           # [21][n] f32  seed covariance, upper triangle row-major
+    q: np.ndarray             # [n]     i8
+    hpos: np.ndarray          # [L][3][n] f32
+    hcov: np.ndarray          # [L][6][n] f32  xx,xy,xz,yy,yz,zz
+    mask: np.ndarray          # [n] u32, bit l = track has a hit on layer l
+    truth: np.ndarray = field(repr=False, default=None)   # [L][6][n] f64 post-scatter truth at each layer
+    truth_vertex: np.ndarray = field(repr=False, default=None)  # [6][n] f64
+
+    @property
+    def n_layers(self) -> int:
+        return int(self.radius.shape[0])
+
+
+def highland_theta0(p: np.ndarray, mass: float, t: float) -> np.ndarray:
+    """Width of the simulated scattering angle (PDG Highland form, flat thickness t = x/X0)."""
+    if t <= 0.0:
+        return np.zeros_like(p)
+    beta = p / np.sqrt(p * p + mass * mass)
+    return 0.0136 / (beta * p) * math.sqrt(t) * (1.0 + 0.038 * math.log(t))
+
+
+def _cross_cylinder(pos, mom, q, Bz, r):
+    """First forward crossing of each truth helix with the cylinder of radius r.
+
+    Two-circle intersection (track circle: centre c, radius R; layer circle: origin, radius r),
+    turning angle from atan2 differences about the centre.  Returns new (pos, mom).
+    """
+    x, y, z = pos
+    px, py, pz = mom
+    k = q * C_B * Bz
+    pt = np.hypot(px, py)
+    R = pt / np.abs(k)
+    cx = x + py / k
+    cy = y - px / k
+    d = np.hypot(cx, cy)
+    a = (d * d + r * r - R * R) / (2.0 * d)
+    h = np.sqrt(np.maximum(r * r - a * a, 0.0))
+    ux, uy = cx / d, cy / d
+    psi0 = np.arctan2(y - cy, x - cx)
+    best_theta = None
+    best_pt = None
+    for sgn in (+1.0, -1.0):
+        X = a * ux - sgn * h * uy
+        Y = a * uy + sgn * h * ux
+        psi = np.arctan2(Y - cy, X - cx)
+        # the position angle about the centre evolves as psi(theta) = psi0 - theta, theta = kappa*s
+        turn = np.where(k > 0, np.mod(psi0 - psi, 2 * np.pi), -np.mod(psi - psi0, 2 * np.pi))
+        if best_theta is None:
+            best_theta, best_pt = turn, (X, Y)
+        else:
+            take = np.abs(turn) < np.abs(best_theta)
+            best_theta = np.where(take, turn, best_theta)
+            best_pt = (np.where(take, X, best_pt[0]), np.where(take, Y, best_pt[1]))
+    theta = best_theta
+    s = theta * pt / k
+    c, sn = np.cos(theta), np.sin(theta)
+    return (best_pt[0], best_pt[1], z + pz * s / pt), (px * c + py * sn, -px * sn + py * c, pz)
+
+
+def hit_covariance(phi_h, sigma_r=SIGMA_R, sigma_rphi=SIGMA_RPHI, sigma_z=SIGMA_Z):
+    """V = Rz(phi_h) diag(sr^2, srphi^2, sz^2) Rz(phi_h)^T packed xx,xy,xz,yy,yz,zz."""
+    c, s = np.cos(phi_h), np.sin(phi_h)
+    vr, vt, vz = sigma_r ** 2, sigma_rphi ** 2, sigma_z ** 2
+    zero = np.zeros_like(c)
+    return np.stack([vr * c * c + vt * s * s, (vr - vt) * c * s, zero,
+                     vr * s * s + vt * c * c, zero, zero + vz])
+
+
+def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
+                   smear_hits: bool = True, smear_seed: bool = True) -> FitBatch:
+    """One event of `cfg` (rng = default_rng(BASE_SEED + 1000*config + event))."""
+    rng = np.random.default_rng(BASE_SEED + 1000 * cfg.index + event)
+    n = cfg.n_tracks if n_tracks is None else n_tracks
+    L = cfg.n_layers
+    radii = cfg.radii
+    q = rng.choice(np.array([-1.0, 1.0]), size=n)
+    pt = rng.uniform(cfg.pt_min, cfg.pt_max, size=n)
+    phi = rng.uniform(0.0, 2 * np.pi, size=n)
+    eta = rng.uniform(-cfg.eta_max, cfg.eta_max, size=n)
+    mom = (pt * np.cos(phi), pt * np.sin(phi), pt * np.sinh(eta))
+    pos = (np.zeros(n), np.zeros(n), np.zeros(n))
+    truth_vertex = np.stack(pos + mom)
+
+    hpos = np.zeros((L, 3, n))
+    hcov = np.zeros((L, 6, n))
+    truth = np.full((L, 6, n), np.nan)
+    mask = np.zeros(n, dtype=np.uint32)
+    alive = np.ones(n, dtype=bool)
+    for l in range(L):
+        r = float(radii[l])
+        k = q * C_B * cfg.Bz
+        ptl = np.hypot(mom[0], mom[1])
+        R = ptl / np.abs(k)
+        centre = np.hypot(pos[0] + mom[1] / k, pos[1] - mom[0] / k)
+        alive &= ~(r > 0.9 * (R + centre))          # A12: stop before a too-shallow crossing
+        with np.errstate(invalid="ignore", divide="ignore"):
+            npos, nmom = _cross_cylinder(pos, mom, q, cfg.Bz, r)
+        pos = tuple(np.where(alive, a, b) for a, b in zip(npos, pos))
+        mom = tuple(np.where(alive, a, b) for a, b in zip(nmom, mom))
+        # measurement: smear azimuth by sigma_rphi / r, z by sigma_z; the hit stays on the cylinder
+        g = rng.standard_normal((2, n))
+        if not smear_hits:
+            g = np.zeros_like(g)
+        phi_h = np.arctan2(pos[1], pos[0]) + g[0] * SIGMA_RPHI / r
+        hp = np.stack([r * np.cos(phi_h), r * np.sin(phi_h), pos[2] + g[1] * SIGMA_Z])
+        hv = hit_covariance(phi_h)
+        hpos[l] = np.where(alive, hp, 0.0)
+        hcov[l] = np.where(alive, hv, 0.0)
+        mask |= (alive.astype(np.uint32) << np.uint32(l))
+        # multiple scattering right after the hit: two independent angles about p-hat, |p| kept
+        a = rng.standard_normal((2, n))
+        if cfg.x_over_X0 > 0.0:
+            px, py, pz = mom
+            p = np.sqrt(px * px + py * py + pz * pz)
+            th0 = highland_theta0(p, M_PION, cfg.x_over_X0)
+            ptt = np.hypot(px, py)
+            e1 = (-py / ptt, px / ptt, np.zeros(n))                      # z-hat x p-hat, normalised
+            ph = (px / p, py / p, pz / p)
+            e2 = (ph[1] * e1[2] - ph[2] * e1[1], ph[2] * e1[0] - ph[0] * e1[2], ph[0] * e1[1] - ph[1] * e1[0])
+            t1, t2 = np.tan(a[0] * th0), np.tan(a[1] * th0)
+            d = tuple(ph[i] + t1 * e1[i] + t2 * e2[i] for i in range(3))
+            dn = np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)
+            mom = tuple(np.where(alive, p * d[i] / dn, mom[i]) for i in range(3))
+        truth[l] = np.where(alive, np.stack(pos + mom), np.nan)
+
+    # seed (A13)
+    g = rng.standard_normal((6, n))
+    if not smear_seed:
+        g = np.zeros_like(g)
+    spar = truth_vertex.copy()
+    spar[0:3] += SEED_POS_SMEAR * g[0:3]
+    spar[3:6] += SEED_MOM_SMEAR * pt * g[3:6]
+    spt = np.hypot(spar[3], spar[4])
+    scov = np.zeros((21, n))
+    diag_idx = [0, 6, 11, 15, 18, 20]
+    for i in range(3):
+        scov[diag_idx[i]] = SEED_POS_SIGMA0 ** 2
+        scov[diag_idx[3 + i]] = (SEED_MOM_SIGMA0 * spt) ** 2
+
+    f32 = np.float32
+    return FitBatch(
+        n=n, radius=radii.astype(f32), x_over_X0=np.full(L, cfg.x_over_X0, dtype=f32),
+        Bz=cfg.Bz, mass=M_PION,
+        par=np.ascontiguousarray(spar, dtype=f32), cov=np.ascontiguousarray(scov, dtype=f32),
+        q=q.astype(np.int8), hpos=np.ascontiguousarray(hpos, dtype=f32),
+        hcov=np.ascontiguousarray(hcov, dtype=f32), mask=mask, truth=truth, truth_vertex=truth_vertex)
+
+
+def concat_batches(batches: list[FitBatch]) -> FitBatch:
+    b0 = batches[0]
+    cat = lambda name, ax: np.ascontiguousarray(np.concatenate([getattr(b, name) for b in batches], axis=ax))
+    return FitBatch(n=sum(b.n for b in batches), radius=b0.radius, x_over_X0=b0.x_over_X0, Bz=b0.Bz,
+                    mass=b0.mass, par=cat("par", 1), cov=cat("cov", 1), q=cat("q", 0),
+                    hpos=cat("hpos", 2), hcov=cat("hcov", 2), mask=cat("mask", 0),
+                    truth=cat("truth", 2), truth_vertex=cat("truth_vertex", 1))
+
+
+def make_fit_batch(config: int, n_events: int | None = None, n_tracks: int | None = None) -> FitBatch:
+    """The fit workload of config 0..3 (config 2 = 100 independent events concatenated)."""
+    cfg = get_config(config)
+    ne = cfg.n_events if n_events is None else n_events
+    evs = [simulate_event(cfg, e, n_tracks) for e in range(ne)]
+    return evs[0] if ne == 1 else concat_batches(evs)
+
+
+@dataclass
+class LayerHits:
+    """All hits of one layer of one event (true + noise, shuffled), fp32 SoA."""
+    radius: float
+    pos: np.ndarray        # [3][H] f32
+    cov: np.ndarray        # [6][H] f32
+    true_index: np.ndarray  # [n_tracks] i32: index of track i's own hit in this pool
+
+
+@dataclass
+class BuildEvent:
+    """config 4: one config-1-style event plus per-layer hit pools with uniform noise."""
+    cfg: BarrelConfig
+    fit: FitBatch              # the event's tracks with their true hits (used to make seeds)
+    layers: list[LayerHits]
+
+
+def make_build_event(config: int = 4, n_tracks: int | None = None, noise_hits: int | None = None) -> BuildEvent:
+    cfg = get_config(config)
+    fit = simulate_event(cfg, 0, n_tracks)
+    rng = np.random.default_rng(BASE_SEED + 1000 * cfg.index + 500)
+    n_noise = cfg.noise_hits_per_layer if noise_hits is None else noise_hits
+    layers = []
+    for l in range(cfg.n_layers):
+        r = float(cfg.radii[l])
+        eta = rng.uniform(-cfg.eta_bin_max, cfg.eta_bin_max, size=n_noise)
+        phi = rng.uniform(-np.pi, np.pi, size=n_noise)
+        npos = np.stack([r * np.cos(phi), r * np.sin(phi), r * np.sinh(eta)])
+        ncov = hit_covariance(phi)
+        pos = np.concatenate([fit.hpos[l].astype(np.float64), npos], axis=1)
+        cov = np.concatenate([fit.hcov[l].astype(np.float64), ncov], axis=1)
+        H = pos.shape[1]
+        perm = rng.permutation(H)                      # pool slot j holds original hit perm[j]
+        inv = np.empty(H, dtype=np.int64)
+        inv[perm] = np.arange(H)
+        layers.append(LayerHits(radius=r,
+                                pos=np.ascontiguousarray(pos[:, perm], dtype=np.float32),
+                                cov=np.ascontiguousarray(cov[:, perm], dtype=np.float32),
+                                true_index=inv[:fit.n].astype(np.int32)))
+    return BuildEvent(cfg=cfg, fit=fit, layers=layers)

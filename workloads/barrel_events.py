@@ -151,8 +151,10 @@ def hit_covariance(phi_h, sigma_r=SIGMA_R, sigma_rphi=SIGMA_RPHI, sigma_z=SIGMA_
 
 
 def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
-                   smear_hits: bool = True, smear_seed: bool = True) -> FitBatch:
-    """One event of `cfg` (rng = default_rng(BASE_SEED + 1000*config + event))."""
+                   smear_hits: bool = True, smear_seed: bool = True, dtype=np.float32) -> FitBatch:
+    """One event of `cfg` (rng = default_rng(BASE_SEED + 1000*config + event)).
+
+    dtype=float64 keeps the un-rounded values (oracle pins only; the fitters' contract is fp32)."""
     rng = np.random.default_rng(BASE_SEED + 1000 * cfg.index + event)
     n = cfg.n_tracks if n_tracks is None else n_tracks
     L = cfg.n_layers
@@ -221,7 +223,7 @@ def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
         scov[diag_idx[i]] = SEED_POS_SIGMA0 ** 2
         scov[diag_idx[3 + i]] = (SEED_MOM_SIGMA0 * spt) ** 2
 
-    f32 = np.float32
+    f32 = dtype
     return FitBatch(
         n=n, radius=radii.astype(f32), x_over_X0=np.full(L, cfg.x_over_X0, dtype=f32),
         Bz=cfg.Bz, mass=M_PION,

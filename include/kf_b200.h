@@ -1,0 +1,181 @@
+/*
+ * kf_b200.h -- C ABI of the B200-native batched Kalman-filter track fitter.
+ *
+ * What it computes (arXiv:1705.02876):
+ *   - track fitting = the Kalman filter applied layer after layer, without branching, to the fixed
+ *     hit list of each track, giving the parameters and a chi2 (section 2 "a final
+ *     fit with a KF ... to compute a measure of the track quality in terms of a chi2";
+ *     PAPER.md:61 "track fitting can repeatedly apply the KF algorithm without branching");
+ *   - track state = 6 parameters in global coordinates with a 6x6 covariance, hit = 3-D point
+ *     with a 3x3 covariance (section 2.1);
+ *   - many small matrices stored matrix-major: "elements with the same index but from different
+ *     matrices are stored consecutively" (PAPER.md:65 Matriplex; section 4.1) --
+ *     here: structure of arrays, element-major across tracks, plane stride `ld`;
+ *   - hits of a layer placed in "directionally projective bins" (eta, phi) for fast look-up
+ *     (section 3);
+ *   - best-hit building: per candidate and layer "the hit that produced the lowest chi2 increment"
+ *     (section 3), one GPU thread group per candidate (section 4.3).
+ * The paper prints no formulas.  The equations are BASELINE.json:north_star's
+ *     C' = F C F^T + Q,  S = H C' H^T + V,  K = C' H^T S^-1,  x = x' + K r,  C = C' - K H C',
+ *     chi2 += r^T S^-1 r,      H = [I3 0],  r = m - H x'
+ * with the helix, Jacobian, Highland process noise and bin definitions written out in DESIGN.md
+ * ("Readings A1..A17").
+ *
+ * Units: cm, GeV/c, Tesla.  State order (x, y, z, px, py, pz).  Symmetric 6x6 packed as the upper
+ * triangle, row-major, 21 values: index(i<=j) = i*6 - i*(i-1)/2 + (j-i).  Symmetric 3x3 packed
+ * xx, xy, xz, yy, yz, zz.  Every array is element-major: element e of track t is at
+ * base[e*ld + t].
+ *
+ * Conventions for every call
+ *   Ownership: all buffers are caller-owned; the library keeps no pointer after a call returns.
+ *              The context owns only its scratch (kf_reserve / grown on demand by kf_bin_hits and
+ *              the *_host calls; growing synchronises the stream, steady state never allocates).
+ *   Memory:    "DEV" = device pointer on the context's device, "HOST" = host pointer.  Device
+ *              pointers must be 16-byte aligned and ld % 4 == 0 (so every plane is 16-byte aligned).
+ *   Async:     device-pointer calls enqueue on the context's stream and return without
+ *              synchronising.  *_host calls return after the results are in the host buffers.
+ *   Errors:    0 = KF_OK; negative = argument or launch error, and then no output is written.
+ *              No exception crosses this boundary.  Per-track trouble is data, not an error: it is
+ *              reported in `status` bits and the track keeps its last good state.
+ *   No CPU fallback exists: without a CUDA device kf_create fails with KF_ERR_CUDA.
+ */
+#ifndef KF_B200_H
+#define KF_B200_H
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define KF_API __attribute__((visibility("default")))
+#else
+#define KF_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- return codes -------------------------------------------------------------------------- */
+enum {
+    KF_OK = 0,
+    KF_ERR_NULL = -1,        /* a required pointer is NULL                                        */
+    KF_ERR_SHAPE = -2,       /* n < 0, ld < n, n_layers mismatch, layer index out of range ...    */
+    KF_ERR_ALIGN = -3,       /* device pointer not 16-byte aligned or ld % 4 != 0                 */
+    KF_ERR_UNSUPPORTED = -4, /* n_layers > 32, |Bz| < 1e-6 T, radii not strictly increasing,
+                                bins > KF_MAX_BINS, window wider than the phi ring                */
+    KF_ERR_CUDA = -5,        /* a CUDA runtime call failed (kf_last_cuda_error has the code)      */
+    KF_ERR_NOMEM = -6        /* scratch allocation failed                                         */
+};
+
+/* ---- per-track status bits (outputs) ---------------------------------------------------------- */
+enum {
+    KF_STATUS_PROP_FAIL = 1,  /* helix has no outward crossing with the layer (disc <= 0, r <= rho) */
+    KF_STATUS_S_NOT_PD = 2,   /* det S <= 0                                                         */
+    KF_STATUS_NONFINITE = 4,  /* update produced a non-finite state or chi2                         */
+    KF_STATUS_BAD_CHARGE = 8  /* q not in {+1, -1}: track is copied through untouched               */
+};
+
+#define KF_MAX_LAYERS 32
+#define KF_MAX_BINS 65536
+
+typedef struct kf_ctx kf_ctx; /* opaque: device, borrowed stream, scratch */
+
+/* Create a context on `device`.  `cuda_stream` is a borrowed cudaStream_t (e.g. the raw handle of a
+ * torch stream); NULL = the legacy default stream.  Fails with KF_ERR_CUDA if there is no device. */
+KF_API int kf_create(kf_ctx** out, int device, void* cuda_stream);
+KF_API int kf_destroy(kf_ctx* ctx);
+/* Change the borrowed stream used by later calls. */
+KF_API int kf_set_stream(kf_ctx* ctx, void* cuda_stream);
+/* Pre-size scratch so that no later call allocates: `max_hits` hits per layer for kf_bin_hits,
+ * `max_host_tracks` x `max_host_layers` for the *_host staging buffers (0 = leave as is). */
+KF_API int kf_reserve(kf_ctx* ctx, int64_t max_hits, int64_t max_host_tracks, int max_host_layers);
+/* Static, never NULL. */
+KF_API const char* kf_strerror(int code);
+/* cudaError_t of the last KF_ERR_CUDA on this context (0 if none). */
+KF_API int kf_last_cuda_error(const kf_ctx* ctx);
+/* ABI version, bumped when a struct or signature changes. */
+KF_API int kf_abi_version(void);
+
+/* ---- geometry: concentric cylinders in a uniform solenoid field (PAPER.md:83 toy detector) ---- */
+typedef struct {
+    int n_layers;             /* 1..KF_MAX_LAYERS                                                  */
+    const float* radius_cm;   /* HOST [n_layers], strictly increasing, > 0                         */
+    const float* x_over_X0;   /* HOST [n_layers], thickness in radiation lengths, 0 = no material  */
+    float Bz_tesla;           /* |Bz| >= 1e-6                                                      */
+    float mass_gev;           /* mass entering beta of the Highland formula (reading A5)           */
+} kf_geometry;
+
+/* ---- tracks (seeds in, fitted tracks out; candidates in/out) ------------------------------------ */
+typedef struct {
+    int64_t n, ld;            /* n tracks; plane stride ld >= n, ld % 4 == 0                        */
+    float* par;               /* [6][ld]  x y z px py pz                                           */
+    float* cov;               /* [21][ld] packed upper triangle                                    */
+    int8_t* q;                /* [n] charge +1 / -1                                                */
+    float* chi2;              /* [n]   fit: output total; scoring: in/out running total            */
+    int32_t* nhits;           /* [n]   fit: output hits used; scoring: in/out                      */
+    uint32_t* status;         /* [n]   fit: output; scoring: in/out (bits are OR-ed in)            */
+} kf_tracks;
+
+/* ---- per-track hit lists for fitting (the hit collection is fixed after building) -- */
+typedef struct {
+    int n_layers;             /* must equal geometry n_layers                                      */
+    int64_t n, ld;
+    const float* pos;         /* [n_layers][3][ld] hit of track t on layer l: x y z                */
+    const float* cov;         /* [n_layers][6][ld] its covariance xx xy xz yy yz zz                */
+    const uint32_t* mask;     /* [n] bit l set = track has a hit on layer l; NULL = all layers     */
+} kf_track_hits;
+
+/* Fit n tracks: for each layer in increasing radius whose mask bit is set, propagate state and
+ * covariance along the helix to the layer radius (C' = F C F^T + Q), then Kalman-update with the
+ * track's hit on that layer and add the chi2 increment (north_star).
+ * A layer that fails (status bit) is skipped and the track keeps its previous state.
+ * `out` may alias `seeds` (in-place); otherwise out->par/cov/chi2/nhits/status are written and
+ * out->q is ignored.  out->n/ld may differ from seeds->ld but out->n must equal seeds->n.
+ * All pointers DEV.  Enqueues one kernel on the context stream. */
+KF_API int kf_fit_tracks(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                  const kf_track_hits* hits, kf_tracks* out);
+
+/* Same call with every pointer HOST (pageable or pinned): copies in, fits, copies out, in chunks
+ * pipelined over internal streams, and returns when `out` is complete.  This is the end-to-end
+ * path (transfers overlapped with kernels).  Alignment rules do not apply. */
+KF_API int kf_fit_tracks_host(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                       const kf_track_hits* hits, kf_tracks* out);
+
+/* ---- hits of one layer and their (eta, phi) bins ------------------------------------ */
+typedef struct {
+    int64_t n_hits, ld;       /* ld >= n_hits, ld % 4 == 0                                         */
+    const float* pos;         /* DEV [3][ld]                                                       */
+    const float* cov;         /* DEV [6][ld]                                                       */
+} kf_layer_hits;
+
+typedef struct {
+    int n_eta, n_phi;         /* n_eta*n_phi <= KF_MAX_BINS, n_phi even                            */
+    float eta_max;            /* eta bins cover [-eta_max, eta_max), out-of-range hits clamp       */
+    int64_t ld;               /* plane stride of pos_sorted / cov_sorted, >= n_hits, % 4 == 0      */
+    int32_t* bin_offset;      /* DEV [n_eta*n_phi + 1] first sorted slot of each bin               */
+    int32_t* sorted_to_orig;  /* DEV [n_hits] original index of the hit in each sorted slot        */
+    float* pos_sorted;        /* DEV [3][ld] hits in bin order                                     */
+    float* cov_sorted;        /* DEV [6][ld]                                                       */
+} kf_layer_bins;
+
+/* Bin one layer's hits: bin = i_eta*n_phi + i_phi with eta = asinh(z/radius), phi = atan2(y,x) over
+ * [-pi, pi); stable counting sort (within a bin, original order).  The bin of a hit is decided in
+ * single precision against tabulated edges (reading A16b).  `out` arrays are
+ * caller-allocated.  n_hits == 0 is valid (all offsets 0). */
+KF_API int kf_bin_hits(kf_ctx* ctx, float radius_cm, const kf_layer_hits* hits, kf_layer_bins* out);
+
+/* Best-hit scoring of n candidates on ONE layer (`layer` indexes the geometry): propagate (+Q),
+ * take the candidate's own (eta, phi) bin, score chi2 = r^T (C'_pp + V_h)^-1 r for every hit in
+ * the window i_eta +- window_half (clipped), i_phi +- window_half (wrapped); best = lowest chi2,
+ * exact ties -> lowest original index; accepted iff chi2 < chi2_cut.
+ * Accepted and do_update: Kalman update, nhits += 1, chi2 += best.  Otherwise the candidate keeps
+ * the propagated state (Q included).  best_hit[n] = ORIGINAL hit index or -1; best_chi2[n] = lowest
+ * chi2 seen (+inf if the window was empty).  Propagation failure: status bit, candidate untouched,
+ * best_hit = -1, best_chi2 = +inf.  All pointers DEV.  The caller loops over layers. */
+KF_API int kf_score_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, kf_tracks* cands,
+                        const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                        float chi2_cut, int do_update, int32_t* best_hit, float* best_chi2);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KF_B200_H */

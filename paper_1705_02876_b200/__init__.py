@@ -1,0 +1,11 @@
+"""paper_1705_02876_b200 -- B200-native batched Kalman-filter track fitting (arXiv:1705.02876).
+
+The product is the C-ABI shared library `libkf_b200.so` (include/kf_b200.h) built from `csrc/`;
+this package is the thin ctypes binding with the same call names.  There is no CPU fallback:
+without the built library, or without a CUDA device, the calls raise.
+"""
+from .binding import (KFContext, KFError, Bins, Geometry, abi_version, lib_path, load_library,
+                      strerror, STATUS_BAD_CHARGE, STATUS_NONFINITE, STATUS_PROP_FAIL, STATUS_S_NOT_PD)
+
+__all__ = ["KFContext", "KFError", "Bins", "Geometry", "abi_version", "lib_path", "load_library",
+           "strerror", "STATUS_BAD_CHARGE", "STATUS_NONFINITE", "STATUS_PROP_FAIL", "STATUS_S_NOT_PD"]

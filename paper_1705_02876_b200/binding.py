@@ -1,0 +1,266 @@
+"""ctypes binding of include/kf_b200.h: argument marshalling only.
+
+Every step of the path (propagation, covariance transport, update, chi2, binning, scoring) runs in
+the CUDA kernels behind the C ABI; this module only turns torch tensors (device memory, streams)
+into the plain pointers and sizes the ABI takes.  Names follow the header: KFContext.fit_tracks ->
+kf_fit_tracks, .fit_tracks_host -> kf_fit_tracks_host, .bin_hits -> kf_bin_hits,
+.score_candidates -> kf_score_candidates.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libkf_b200.so")
+
+STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
+EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
+           "kf_abi_version", "kf_fit_tracks", "kf_fit_tracks_host", "kf_bin_hits", "kf_score_candidates"]
+
+
+class KFError(RuntimeError):
+    def __init__(self, code: int, what: str, cuda: int = 0):
+        super().__init__(f"{what}: {strerror(code)} (code {code}" + (f", cudaError {cuda})" if cuda else ")"))
+        self.code = code
+        self.cuda = cuda
+
+
+class _Geometry(C.Structure):
+    _fields_ = [("n_layers", C.c_int), ("radius_cm", C.POINTER(C.c_float)), ("x_over_X0", C.POINTER(C.c_float)),
+                ("Bz_tesla", C.c_float), ("mass_gev", C.c_float)]
+
+
+class _Tracks(C.Structure):
+    _fields_ = [("n", C.c_int64), ("ld", C.c_int64), ("par", C.c_void_p), ("cov", C.c_void_p), ("q", C.c_void_p),
+                ("chi2", C.c_void_p), ("nhits", C.c_void_p), ("status", C.c_void_p)]
+
+
+class _TrackHits(C.Structure):
+    _fields_ = [("n_layers", C.c_int), ("n", C.c_int64), ("ld", C.c_int64), ("pos", C.c_void_p), ("cov", C.c_void_p),
+                ("mask", C.c_void_p)]
+
+
+class _LayerHits(C.Structure):
+    _fields_ = [("n_hits", C.c_int64), ("ld", C.c_int64), ("pos", C.c_void_p), ("cov", C.c_void_p)]
+
+
+class _LayerBins(C.Structure):
+    _fields_ = [("n_eta", C.c_int), ("n_phi", C.c_int), ("eta_max", C.c_float), ("ld", C.c_int64),
+                ("bin_offset", C.c_void_p), ("sorted_to_orig", C.c_void_p), ("pos_sorted", C.c_void_p),
+                ("cov_sorted", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libkf_b200.so (built by `python -m paper_1705_02876_b200.build`).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_1705_02876_b200.build` "
+                          "(there is no CPU or PyTorch fallback)")
+    lib = C.CDLL(_LIB_PATH)
+    vp = C.c_void_p
+    lib.kf_create.restype = C.c_int
+    lib.kf_create.argtypes = [C.POINTER(vp), C.c_int, vp]
+    lib.kf_destroy.restype = C.c_int
+    lib.kf_destroy.argtypes = [vp]
+    lib.kf_set_stream.restype = C.c_int
+    lib.kf_set_stream.argtypes = [vp, vp]
+    lib.kf_reserve.restype = C.c_int
+    lib.kf_reserve.argtypes = [vp, C.c_int64, C.c_int64, C.c_int]
+    lib.kf_strerror.restype = C.c_char_p
+    lib.kf_strerror.argtypes = [C.c_int]
+    lib.kf_last_cuda_error.restype = C.c_int
+    lib.kf_last_cuda_error.argtypes = [vp]
+    lib.kf_abi_version.restype = C.c_int
+    lib.kf_abi_version.argtypes = []
+    for name in ("kf_fit_tracks", "kf_fit_tracks_host"):
+        f = getattr(lib, name)
+        f.restype = C.c_int
+        f.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.POINTER(_Tracks)]
+    lib.kf_bin_hits.restype = C.c_int
+    lib.kf_bin_hits.argtypes = [vp, C.c_float, C.POINTER(_LayerHits), C.POINTER(_LayerBins)]
+    lib.kf_score_candidates.restype = C.c_int
+    lib.kf_score_candidates.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.POINTER(_Tracks), C.POINTER(_LayerHits),
+                                        C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int, vp, vp]
+    _lib = lib
+    return lib
+
+
+def strerror(code: int) -> str:
+    return load_library().kf_strerror(int(code)).decode()
+
+
+def abi_version() -> int:
+    return int(load_library().kf_abi_version())
+
+
+@dataclass
+class Geometry:
+    """Concentric cylinders in a uniform solenoid field (host-side numbers)."""
+    radius_cm: np.ndarray
+    x_over_X0: np.ndarray
+    Bz_tesla: float
+    mass_gev: float
+
+    def _c(self):
+        r = np.ascontiguousarray(self.radius_cm, dtype=np.float32)
+        t = np.ascontiguousarray(self.x_over_X0, dtype=np.float32)
+        g = _Geometry(int(r.shape[0]), r.ctypes.data_as(C.POINTER(C.c_float)), t.ctypes.data_as(C.POINTER(C.c_float)),
+                      float(self.Bz_tesla), float(self.mass_gev))
+        return g, (r, t)          # keep the arrays alive while g is in use
+
+
+@dataclass
+class Bins:
+    """Caller-allocated outputs of kf_bin_hits for one layer (all torch CUDA tensors)."""
+    n_eta: int
+    n_phi: int
+    eta_max: float
+    bin_offset: torch.Tensor      # int32 [n_eta*n_phi + 1]
+    sorted_to_orig: torch.Tensor  # int32 [n_hits]
+    pos_sorted: torch.Tensor      # f32 [3][ld]
+    cov_sorted: torch.Tensor      # f32 [6][ld]
+
+    @staticmethod
+    def allocate(n_hits: int, n_eta: int, n_phi: int, eta_max: float, device) -> "Bins":
+        ld = max(4, (n_hits + 3) // 4 * 4)
+        return Bins(n_eta, n_phi, eta_max,
+                    torch.empty(n_eta * n_phi + 1, dtype=torch.int32, device=device),
+                    torch.empty(max(n_hits, 1), dtype=torch.int32, device=device),
+                    torch.empty((3, ld), dtype=torch.float32, device=device),
+                    torch.empty((6, ld), dtype=torch.float32, device=device))
+
+    def _c(self):
+        return _LayerBins(self.n_eta, self.n_phi, float(self.eta_max), int(self.pos_sorted.shape[1]),
+                          self.bin_offset.data_ptr(), self.sorted_to_orig.data_ptr(),
+                          self.pos_sorted.data_ptr(), self.cov_sorted.data_ptr())
+
+
+def _plane_ld(t: torch.Tensor, rows: int) -> int:
+    """A [rows][ld] (or [L][k][ld]) tensor whose last dimension is contiguous and planes are ld apart."""
+    if t.stride(-1) != 1:
+        raise ValueError("last dimension must be contiguous")
+    ld = t.stride(-2) if t.dim() >= 2 else t.shape[-1]
+    if t.dim() == 3 and t.stride(0) != t.shape[1] * ld:
+        raise ValueError("layer planes must be densely stacked")
+    flat_rows = int(np.prod(t.shape[:-1]))
+    if flat_rows != rows:
+        raise ValueError(f"expected {rows} planes, got {flat_rows}")
+    return int(ld)
+
+
+class KFContext:
+    """kf_ctx*: one per device/stream.  Methods mirror the C ABI; tensors are torch (CUDA for the
+    device calls, CPU -- ideally pinned -- for fit_tracks_host)."""
+
+    def __init__(self, device: int | torch.device = 0, stream: torch.cuda.Stream | None = None):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        dev = torch.device(device) if not isinstance(device, int) else torch.device("cuda", device)
+        self.device = dev
+        idx = dev.index if dev.index is not None else 0
+        sptr = C.c_void_p(stream.cuda_stream if stream is not None else
+                          (torch.cuda.current_stream(dev).cuda_stream if torch.cuda.is_available() else 0))
+        rc = self._lib.kf_create(C.byref(self._h), idx, sptr)
+        if rc != 0:
+            raise KFError(rc, "kf_create")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.kf_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int, what: str):
+        if rc != 0:
+            raise KFError(rc, what, self._lib.kf_last_cuda_error(self._h))
+
+    def set_stream(self, stream: torch.cuda.Stream | None):
+        s = stream.cuda_stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
+        self._check(self._lib.kf_set_stream(self._h, C.c_void_p(s)), "kf_set_stream")
+
+    def reserve(self, max_hits: int = 0, max_host_tracks: int = 0, max_host_layers: int = 0):
+        self._check(self._lib.kf_reserve(self._h, max_hits, max_host_tracks, max_host_layers), "kf_reserve")
+
+    # ------------------------------------------------------------------ marshalling helpers
+    @staticmethod
+    def _tracks(n, par, cov, q, chi2, nhits, status) -> _Tracks:
+        ld = _plane_ld(par, 6)
+        if _plane_ld(cov, 21) != ld:
+            raise ValueError("par and cov must share the plane stride ld")
+        return _Tracks(int(n), ld, par.data_ptr(), cov.data_ptr(), q.data_ptr() if q is not None else None,
+                       chi2.data_ptr(), nhits.data_ptr(), status.data_ptr())
+
+    @staticmethod
+    def _track_hits(n, L, hpos, hcov, mask) -> _TrackHits:
+        ld = _plane_ld(hpos, 3 * L)
+        if _plane_ld(hcov, 6 * L) != ld:
+            raise ValueError("hpos and hcov must share the plane stride ld")
+        return _TrackHits(int(L), int(n), ld, hpos.data_ptr(), hcov.data_ptr(),
+                          mask.data_ptr() if mask is not None else None)
+
+    # ------------------------------------------------------------------ kf_fit_tracks
+    def fit_tracks(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,
+                   out_par, out_cov, out_chi2, out_nhits, out_status):
+        """Enqueue one fit of n tracks (device tensors; SoA [6][ld], [21][ld], [L][3][ld], [L][6][ld])."""
+        g, keep = geom._c()
+        seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
+        out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
+        hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
+        self._check(self._lib.kf_fit_tracks(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)),
+                    "kf_fit_tracks")
+        del keep
+
+    def fit_tracks_host(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,
+                        out_par, out_cov, out_chi2, out_nhits, out_status):
+        """Same with HOST tensors (pinned for full overlap); returns when the outputs are complete."""
+        for t in (par, cov, q, hpos, hcov, out_par, out_cov, out_chi2, out_nhits, out_status):
+            if t.is_cuda:
+                raise ValueError("fit_tracks_host takes CPU tensors")
+        g, keep = geom._c()
+        seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
+        out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
+        hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
+        self._check(self._lib.kf_fit_tracks_host(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)),
+                    "kf_fit_tracks_host")
+        del keep
+
+    # ------------------------------------------------------------------ kf_bin_hits
+    def bin_hits(self, radius_cm: float, n_hits: int, pos, cov, bins: Bins):
+        lh = _LayerHits(int(n_hits), _plane_ld(pos, 3), pos.data_ptr(), cov.data_ptr())
+        if _plane_ld(cov, 6) != lh.ld:
+            raise ValueError("pos and cov must share the plane stride ld")
+        lb = bins._c()
+        self._check(self._lib.kf_bin_hits(self._h, float(radius_cm), C.byref(lh), C.byref(lb)), "kf_bin_hits")
+
+    # ------------------------------------------------------------------ kf_score_candidates
+    def score_candidates(self, geom: Geometry, layer: int, n: int, par, cov, q, chi2, nhits, status,
+                         n_hits: int, pos, cov_hits, bins: Bins, window_half: int, chi2_cut: float,
+                         do_update: bool, best_hit, best_chi2):
+        g, keep = geom._c()
+        cands = self._tracks(n, par, cov, q, chi2, nhits, status)
+        lh = _LayerHits(int(n_hits), _plane_ld(pos, 3), pos.data_ptr(), cov_hits.data_ptr())
+        lb = bins._c()
+        self._check(self._lib.kf_score_candidates(self._h, C.byref(g), int(layer), C.byref(cands), C.byref(lh),
+                                                  C.byref(lb), int(window_half), float(chi2_cut),
+                                                  1 if do_update else 0, best_hit.data_ptr(), best_chi2.data_ptr()),
+                    "kf_score_candidates")
+        del keep

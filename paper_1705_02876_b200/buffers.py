@@ -1,0 +1,83 @@
+"""Device-buffer helpers around the binding: allocation and layout only (no arithmetic).
+
+A `DeviceFit` holds the SoA tensors of one kf_fit_tracks call on one GPU, with the plane stride
+`ld` padded to a multiple of 4 floats as the ABI requires.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+from .binding import Geometry, KFContext
+
+
+def padded_ld(n: int) -> int:
+    return max(4, (int(n) + 3) // 4 * 4)
+
+
+def _to_planes(a: np.ndarray, ld: int, device, pin: bool = False) -> torch.Tensor:
+    """[..., n] numpy -> [..., ld] torch tensor (zero padded)."""
+    a = np.ascontiguousarray(a)
+    n = a.shape[-1]
+    t = torch.zeros(a.shape[:-1] + (ld,), dtype=torch.from_numpy(a[..., :0]).dtype,
+                    device="cpu", pin_memory=pin)
+    t[..., :n] = torch.from_numpy(a)
+    return t if str(device) == "cpu" else t.to(device)
+
+
+@dataclass
+class DeviceFit:
+    n: int
+    ld: int
+    geom: Geometry
+    par: torch.Tensor
+    cov: torch.Tensor
+    q: torch.Tensor
+    hpos: torch.Tensor
+    hcov: torch.Tensor
+    mask: torch.Tensor | None
+    out_par: torch.Tensor
+    out_cov: torch.Tensor
+    out_chi2: torch.Tensor
+    out_nhits: torch.Tensor
+    out_status: torch.Tensor
+
+    @staticmethod
+    def from_batch(batch, device="cuda:0", with_mask: bool = True, pin: bool = False) -> "DeviceFit":
+        """`batch` is a workloads.barrel_events.FitBatch-shaped object (duck-typed numpy arrays)."""
+        n = int(batch.n)
+        ld = padded_ld(n)
+        geom = Geometry(np.asarray(batch.radius, dtype=np.float32), np.asarray(batch.x_over_X0, dtype=np.float32),
+                        float(batch.Bz), float(batch.mass))
+        dev = device
+        mk = lambda shape, dt: torch.zeros(shape, dtype=dt, device=dev, pin_memory=(pin and str(dev) == "cpu"))
+        return DeviceFit(
+            n=n, ld=ld, geom=geom,
+            par=_to_planes(batch.par, ld, dev, pin), cov=_to_planes(batch.cov, ld, dev, pin),
+            q=_to_planes(batch.q.astype(np.int8), ld, dev, pin),
+            hpos=_to_planes(batch.hpos, ld, dev, pin), hcov=_to_planes(batch.hcov, ld, dev, pin),
+            mask=_to_planes(batch.mask.astype(np.uint32).view(np.int32), ld, dev, pin) if with_mask else None,
+            out_par=mk((6, ld), torch.float32), out_cov=mk((21, ld), torch.float32),
+            out_chi2=mk((ld,), torch.float32), out_nhits=mk((ld,), torch.int32), out_status=mk((ld,), torch.int32))
+
+    def fit(self, ctx: KFContext):
+        ctx.fit_tracks(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask,
+                       self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status)
+
+    def fit_host(self, ctx: KFContext):
+        ctx.fit_tracks_host(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask,
+                            self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status)
+
+    def results(self) -> dict:
+        n = self.n
+        return dict(par=self.out_par[:, :n].cpu().numpy(), cov=self.out_cov[:, :n].cpu().numpy(),
+                    chi2=self.out_chi2[:n].cpu().numpy(), nhits=self.out_nhits[:n].cpu().numpy(),
+                    status=self.out_status[:n].cpu().numpy().view(np.uint32))
+
+    @property
+    def algorithmic_bytes(self) -> int:
+        """HBM bytes one fit must move: 113 in + 120 out + 36 per layer, per track."""
+        L = int(self.geom.radius_cm.shape[0])
+        return self.n * (233 + 36 * L)

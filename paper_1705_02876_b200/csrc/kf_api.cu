@@ -1,0 +1,270 @@
+// kf_api.cu -- the C ABI of include/kf_b200.h: argument checks, host-side per-layer constants,
+// context scratch, kernel launches.  No arithmetic of the method lives here except the per-layer
+// constants (radius^2, 1/radius, Highland prefactor) that the kernels read.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/kf_b200.h"
+#include "kf_internal.h"
+
+using namespace kf;
+
+struct kf_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int last_cuda = 0;
+    // kf_bin_hits scratch
+    BinScratch bin;
+    // *_host staging
+    HostStage host;
+};
+
+namespace {
+
+constexpr int kAbiVersion = 1;
+
+int cuda_fail(kf_ctx* c, cudaError_t e) {
+    if (c) c->last_cuda = (int)e;
+    return KF_ERR_CUDA;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// Geometry -> kernel constants.  Returns KF_OK or an error code.
+int make_params(const kf_geometry* g, FitParams* P) {
+    if (!g || !g->radius_cm || !g->x_over_X0) return KF_ERR_NULL;
+    if (g->n_layers < 1) return KF_ERR_SHAPE;
+    if (g->n_layers > KF_MAX_LAYERS) return KF_ERR_UNSUPPORTED;
+    if (!(std::fabs((double)g->Bz_tesla) >= 1e-6)) return KF_ERR_UNSUPPORTED;
+    std::memset(P, 0, sizeof(*P));
+    P->n_layers = g->n_layers;
+    const double k0 = 2.99792458e-3 * (double)g->Bz_tesla;  // reading A1
+    P->k0 = (float)k0;
+    P->inv_k0 = (float)(1.0 / k0);
+    P->mass2 = (float)((double)g->mass_gev * (double)g->mass_gev);
+    double prev = 0.0;
+    for (int l = 0; l < g->n_layers; ++l) {
+        const double r = g->radius_cm[l];
+        if (!(r > prev)) return KF_ERR_UNSUPPORTED;  // strictly increasing, > 0 (also rejects NaN)
+        prev = r;
+        const double t = g->x_over_X0[l];
+        double ms = 0.0;
+        if (t > 0.0) {  // reading A5: theta0 = 0.0136/(beta p) sqrt(t) (1 + 0.038 ln t)
+            const double f = 1.0 + 0.038 * std::log(t);
+            ms = 0.0136 * 0.0136 * t * f * f;
+        }
+        P->layer[l].r = (float)r;
+        P->layer[l].r2 = (float)(r * r);
+        P->layer[l].inv_r = (float)(1.0 / r);
+        P->layer[l].ms = (float)ms;
+    }
+    return KF_OK;
+}
+
+int check_tracks(const kf_tracks* t, bool need_q, bool device) {
+    if (!t) return KF_ERR_NULL;
+    if (t->n < 0 || t->ld < t->n) return KF_ERR_SHAPE;
+    if (t->n == 0) return KF_OK;
+    if (!t->par || !t->cov || !t->chi2 || !t->nhits || !t->status) return KF_ERR_NULL;
+    if (need_q && !t->q) return KF_ERR_NULL;
+    if (device) {
+        if (t->ld % 4 != 0) return KF_ERR_ALIGN;
+        if (!aligned16(t->par) || !aligned16(t->cov)) return KF_ERR_ALIGN;
+    }
+    return KF_OK;
+}
+
+int check_track_hits(const kf_track_hits* h, const kf_geometry* g, int64_t n, bool device) {
+    if (!h) return KF_ERR_NULL;
+    if (h->n_layers != g->n_layers || h->n != n || h->ld < h->n) return KF_ERR_SHAPE;
+    if (n == 0) return KF_OK;
+    if (!h->pos || !h->cov) return KF_ERR_NULL;
+    if (device) {
+        if (h->ld % 4 != 0) return KF_ERR_ALIGN;
+        if (!aligned16(h->pos) || !aligned16(h->cov)) return KF_ERR_ALIGN;
+    }
+    return KF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int kf_abi_version(void) { return kAbiVersion; }
+
+const char* kf_strerror(int code) {
+    switch (code) {
+        case KF_OK: return "ok";
+        case KF_ERR_NULL: return "a required pointer is NULL";
+        case KF_ERR_SHAPE: return "inconsistent sizes (n, ld, n_layers or layer index)";
+        case KF_ERR_ALIGN: return "device pointer not 16-byte aligned or ld not a multiple of 4";
+        case KF_ERR_UNSUPPORTED: return "unsupported configuration (layers > 32, |Bz| < 1e-6 T, radii not increasing, bins)";
+        case KF_ERR_CUDA: return "a CUDA runtime call failed (see kf_last_cuda_error)";
+        case KF_ERR_NOMEM: return "scratch allocation failed";
+        default: return "unknown error code";
+    }
+}
+
+int kf_create(kf_ctx** out, int device, void* cuda_stream) {
+    if (!out) return KF_ERR_NULL;
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || device < 0 || device >= count) return KF_ERR_CUDA;  // no CPU fallback
+    e = cudaSetDevice(device);
+    if (e != cudaSuccess) return KF_ERR_CUDA;
+    kf_ctx* c = new (std::nothrow) kf_ctx();
+    if (!c) return KF_ERR_NOMEM;
+    c->device = device;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    *out = c;
+    return KF_OK;
+}
+
+int kf_destroy(kf_ctx* c) {
+    if (!c) return KF_ERR_NULL;
+    cudaSetDevice(c->device);
+    c->bin.release();
+    c->host.release();
+    delete c;
+    return KF_OK;
+}
+
+int kf_set_stream(kf_ctx* c, void* cuda_stream) {
+    if (!c) return KF_ERR_NULL;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    return KF_OK;
+}
+
+int kf_last_cuda_error(const kf_ctx* c) { return c ? c->last_cuda : 0; }
+
+int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_host_layers) {
+    if (!c) return KF_ERR_NULL;
+    if (max_hits < 0 || max_host_tracks < 0 || max_host_layers < 0 || max_host_layers > KF_MAX_LAYERS)
+        return KF_ERR_SHAPE;
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (max_hits > 0) {
+        e = c->bin.reserve(max_hits, KF_MAX_BINS, c->stream);
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    }
+    if (max_host_tracks > 0 && max_host_layers > 0) {
+        e = c->host.reserve(max_host_tracks, max_host_layers);
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    }
+    return KF_OK;
+}
+
+int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
+                  const kf_track_hits* hits, kf_tracks* out) {
+    if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if ((rc = check_tracks(seeds, true, true))) return rc;
+    if ((rc = check_tracks(out, false, true))) return rc;
+    if (out->n != seeds->n) return KF_ERR_SHAPE;
+    if ((rc = check_track_hits(hits, geom, seeds->n, true))) return rc;
+    if (seeds->n == 0) return KF_OK;
+    FitArgs a;
+    a.n = seeds->n;
+    a.par = seeds->par; a.cov = seeds->cov; a.ld_in = seeds->ld; a.q = seeds->q;
+    a.hpos = hits->pos; a.hcov = hits->cov; a.ld_hit = hits->ld; a.mask = hits->mask;
+    a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
+    a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
+    cudaError_t e = launch_fit(P, a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
+                       const kf_track_hits* hits, kf_tracks* out) {
+    if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if ((rc = check_tracks(seeds, true, false))) return rc;
+    if ((rc = check_tracks(out, false, false))) return rc;
+    if (out->n != seeds->n) return KF_ERR_SHAPE;
+    if ((rc = check_track_hits(hits, geom, seeds->n, false))) return rc;
+    if (seeds->n == 0) return KF_OK;
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    HostFitIO io;
+    io.n = seeds->n; io.L = geom->n_layers;
+    io.par = seeds->par; io.cov = seeds->cov; io.ld_in = seeds->ld; io.q = seeds->q;
+    io.hpos = hits->pos; io.hcov = hits->cov; io.ld_hit = hits->ld; io.mask = hits->mask;
+    io.opar = out->par; io.ocov = out->cov; io.ld_out = out->ld;
+    io.chi2 = out->chi2; io.nhits = out->nhits; io.status = out->status;
+    e = c->host.fit(P, io);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_bin_hits(kf_ctx* c, float radius_cm, const kf_layer_hits* hits, kf_layer_bins* out) {
+    if (!c || !hits || !out) return KF_ERR_NULL;
+    if (hits->n_hits < 0 || hits->ld < hits->n_hits || out->ld < hits->n_hits) return KF_ERR_SHAPE;
+    if (out->n_eta < 1 || out->n_phi < 2) return KF_ERR_SHAPE;
+    if (out->n_phi % 2 != 0 || (int64_t)out->n_eta * out->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
+    if (!(radius_cm > 0.0f) || !(out->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;
+    if (hits->n_hits > 0x7fffffff) return KF_ERR_UNSUPPORTED;
+    if (!out->bin_offset) return KF_ERR_NULL;
+    if (hits->n_hits > 0) {
+        if (!hits->pos || !hits->cov || !out->sorted_to_orig || !out->pos_sorted || !out->cov_sorted)
+            return KF_ERR_NULL;
+        if (hits->ld % 4 != 0 || out->ld % 4 != 0 || !aligned16(hits->pos) || !aligned16(hits->cov) ||
+            !aligned16(out->pos_sorted) || !aligned16(out->cov_sorted))
+            return KF_ERR_ALIGN;
+    }
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = c->bin.reserve(hits->n_hits, out->n_eta * out->n_phi, c->stream);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    BinArgs a;
+    a.n_hits = hits->n_hits; a.ld_in = hits->ld; a.pos = hits->pos; a.cov = hits->cov;
+    a.radius = radius_cm; a.n_eta = out->n_eta; a.n_phi = out->n_phi; a.eta_max = out->eta_max;
+    a.ld_out = out->ld; a.bin_offset = out->bin_offset; a.sorted_to_orig = out->sorted_to_orig;
+    a.pos_sorted = out->pos_sorted; a.cov_sorted = out->cov_sorted;
+    e = launch_bin(c->bin, a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_score_candidates(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks* cands,
+                        const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                        float chi2_cut, int do_update, int32_t* best_hit, float* best_chi2) {
+    if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (layer < 0 || layer >= geom->n_layers) return KF_ERR_SHAPE;
+    if ((rc = check_tracks(cands, true, true))) return rc;
+    if (hits->n_hits < 0 || hits->ld < hits->n_hits || bins->ld < hits->n_hits) return KF_ERR_SHAPE;
+    if (bins->n_eta < 1 || bins->n_phi < 2 || window_half < 0) return KF_ERR_SHAPE;
+    if (bins->n_phi % 2 != 0 || (int64_t)bins->n_eta * bins->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
+    if (2 * window_half + 1 > bins->n_phi) return KF_ERR_UNSUPPORTED;
+    if (!(bins->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;
+    if (cands->n == 0) return KF_OK;
+    if (!best_hit || !best_chi2 || !bins->bin_offset) return KF_ERR_NULL;
+    if (hits->n_hits > 0) {
+        if (!bins->sorted_to_orig || !bins->pos_sorted || !bins->cov_sorted) return KF_ERR_NULL;
+        if (bins->ld % 4 != 0 || !aligned16(bins->pos_sorted) || !aligned16(bins->cov_sorted))
+            return KF_ERR_ALIGN;
+    }
+    ScoreArgs a;
+    a.n = cands->n; a.ld = cands->ld; a.par = cands->par; a.cov = cands->cov; a.q = cands->q;
+    a.chi2 = cands->chi2; a.nhits = cands->nhits; a.status = cands->status;
+    a.n_hits = hits->n_hits; a.ld_hit = bins->ld;
+    a.pos_sorted = bins->pos_sorted; a.cov_sorted = bins->cov_sorted;
+    a.bin_offset = bins->bin_offset; a.sorted_to_orig = bins->sorted_to_orig;
+    a.n_eta = bins->n_eta; a.n_phi = bins->n_phi; a.eta_max = bins->eta_max;
+    a.window_half = window_half; a.chi2_cut = chi2_cut; a.do_update = do_update ? 1 : 0;
+    a.layer = layer; a.best_hit = best_hit; a.best_chi2 = best_chi2;
+    cudaError_t e = launch_score(P, a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
+}
+
+}  // extern "C"

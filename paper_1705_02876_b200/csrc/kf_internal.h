@@ -1,0 +1,96 @@
+// kf_internal.h -- declarations shared by the translation units of libkf_b200 (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "kf_math.cuh"
+
+namespace kf {
+
+// ---------------------------------------------------------------------------------- fit
+struct FitArgs {
+    int64_t n;
+    // inputs
+    const float* par; const float* cov; int64_t ld_in;
+    const int8_t* q;
+    const float* hpos; const float* hcov; int64_t ld_hit;
+    const uint32_t* mask;  // may be null
+    // outputs
+    float* opar; float* ocov; int64_t ld_out;
+    float* chi2; int32_t* nhits; uint32_t* status;
+};
+
+// kf_fit.cu
+cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream);
+
+// ---------------------------------------------------------------------------------- host path
+struct HostFitIO {
+    int64_t n; int L;
+    const float* par; const float* cov; int64_t ld_in; const int8_t* q;
+    const float* hpos; const float* hcov; int64_t ld_hit; const uint32_t* mask;
+    float* opar; float* ocov; int64_t ld_out; float* chi2; int32_t* nhits; uint32_t* status;
+};
+
+// Device staging for kf_fit_tracks_host: kSlots chunk buffers, each with its own stream, so the
+// H2D copy of chunk c+1, the kernel of chunk c and the D2H copy of chunk c-1 overlap.
+struct HostStage {
+    static constexpr int kSlots = 3;
+    int64_t chunk = 0;  // tracks per chunk (multiple of 4)
+    int layers = 0;
+    cudaStream_t stream[kSlots] = {nullptr, nullptr, nullptr};
+    char* buf[kSlots] = {nullptr, nullptr, nullptr};
+    size_t buf_bytes = 0;
+    cudaError_t reserve(int64_t max_tracks, int max_layers);
+    cudaError_t fit(const FitParams& P, const HostFitIO& io);
+    void release();
+};
+
+// ---------------------------------------------------------------------------------- binning
+struct BinArgs {
+    int64_t n_hits, ld_in;
+    const float* pos; const float* cov;
+    float radius; int n_eta, n_phi; float eta_max;
+    int64_t ld_out;
+    int32_t* bin_offset; int32_t* sorted_to_orig; float* pos_sorted; float* cov_sorted;
+};
+
+struct BinScratch {
+    int64_t cap_hits = 0;
+    int cap_bins = 0;
+    int32_t* bin_of = nullptr;   // [cap_hits] bin of each hit
+    int32_t* unsorted = nullptr; // [cap_hits] hit indices grouped by bin, arbitrary order inside
+    int32_t* counts = nullptr;   // [cap_bins + 1]
+    int32_t* cursor = nullptr;   // [cap_bins + 1]
+    // edge tables (device) for the (n_eta, n_phi, eta_max) last used
+    float* eta_edge = nullptr;   // [cap_bins] fl32(sinh(-eta_max + j d_eta)), j = 1..n_eta-1 at [j]
+    float* phi_cos = nullptr;    // [cap_bins] fl32(cos(-pi + j d_phi))
+    float* phi_sin = nullptr;    // [cap_bins]
+    int tab_n_eta = 0, tab_n_phi = 0;
+    float tab_eta_max = 0.0f;
+    std::vector<float> host_tab; // persistent host copy of the three tables (source of the async copy)
+    cudaError_t reserve(int64_t n_hits, int n_bins, cudaStream_t stream);
+    cudaError_t tables(int n_eta, int n_phi, float eta_max, cudaStream_t stream);
+    void release();
+};
+
+// kf_bin.cu
+cudaError_t launch_bin(BinScratch& s, const BinArgs& a, cudaStream_t stream);
+
+// ---------------------------------------------------------------------------------- scoring
+struct ScoreArgs {
+    int64_t n, ld;
+    float* par; float* cov; const int8_t* q; float* chi2; int32_t* nhits; uint32_t* status;
+    int64_t n_hits, ld_hit;
+    const float* pos_sorted; const float* cov_sorted;
+    const int32_t* bin_offset; const int32_t* sorted_to_orig;
+    int n_eta, n_phi; float eta_max;
+    int window_half; float chi2_cut; int do_update; int layer;
+    int32_t* best_hit; float* best_chi2;
+};
+
+// kf_score.cu
+cudaError_t launch_score(const FitParams& P, const ScoreArgs& a, cudaStream_t stream);
+
+}  // namespace kf

@@ -1,0 +1,443 @@
+// kf_math.cuh -- per-track Kalman-filter arithmetic shared by the fit and scoring kernels.
+//
+// Everything here is fp32 and register-resident: one call = one track on one layer.
+// What is computed is north_star's filter (C' = F C F^T + Q, S = C'_pp + V, K = C' H^T S^-1,
+// x = x' + K r, C = C' - K H C', chi2 += r^T S^-1 r) with the helix / Jacobian /
+// Highland readings A1..A8 of DESIGN.md.  HOW it is computed differs from the textbook 6x6 form
+// (DESIGN.md "Kernel arithmetic"):
+//
+//  * The covariance lives in a track-local frame: position block in (radial, tangential, z) of
+//    the current layer crossing, momentum block in (b1, b2, c) = (d pT, pT d phi, pT d(pz/pT)):
+//    b1 along pT, b2 the in-plane normal, c = d pz - (pz/pT) b1 the dip-slope coordinate.  These
+//    are two rotations about z plus one shear, i.e. a similarity C~ = J C J^T: algebraically the
+//    same filter, but the nearly rank-1 momentum block (|p| loose, direction tight) has its loose
+//    direction on ONE axis (b1) and no longer cancels in fp32.
+//  * In that frame the to-radius Jacobian is  F~ = I + (few rank-1 terms):
+//        row r' = 0                           (arrival point stays on the cylinder)
+//        row t' = G_t - tan(a') G_r
+//        row z' = e_z + (theta/k) e_c + (pz/pT)(theta/k e_b1 - G_r/cos(a'))
+//        row b1'= e_b1                        (|pT| is conserved)
+//        row b2'= e_b2 + k/cos(a') G_r
+//        row c' = e_c                         (pz/pT is conserved)
+//    with G_r, G_t the fixed-turning-angle displacement of the arrival point expressed along
+//    (radial', tangential') and a' the angle between momentum and radius at arrival.  So the
+//    transport needs three matrix-vector products instead of two 6x6 matrix products, and the
+//    propagated covariance has an exactly zero radial row/column (15 live elements).
+//  * The update uses the "V form": position rows of the new C are K V (no subtraction), the
+//    momentum block is C'_mm - K_m C'_pm.
+//
+// Complex shorthand used in comments: w = x + i y, pi = px + i py, E = exp(-i theta).
+// Helix (reading A2): w' = w + (i pi / k)(E - 1), pi' = pi E, z' = z + pz theta / k.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace kf {
+
+constexpr float kCB = 2.99792458e-3f;  // GeV / (c T cm), reading A1
+
+enum : uint32_t { ST_PROP_FAIL = 1u, ST_S_NOT_PD = 2u, ST_NONFINITE = 4u, ST_BAD_CHARGE = 8u };
+
+// Per-layer constants, computed once on the host in double and rounded to float.
+struct LayerConst {
+    float r;      // radius
+    float r2;     // r^2
+    float inv_r;  // 1 / r
+    float ms;     // Highland: 0.0136^2 t (1 + 0.038 ln t)^2, t = x/X0 (0 if t <= 0)
+};
+
+struct FitParams {
+    int n_layers;
+    float k0;      // c_B * Bz           (k = q k0)
+    float inv_k0;  // 1 / (c_B * Bz)
+    float mass2;   // mass^2
+    LayerConst layer[32];
+};
+
+__device__ __forceinline__ float rcp_fast(float x) { return __fdividef(1.0f, x); }
+
+// Track in registers.  Position frame unit vector (eax, eay): position-block coordinates
+// (a1, a2) mean  dw = (eax + i eay)(a1 + i a2).  The momentum frame always follows the current
+// momentum: d(pi) = (px + i py)/pT (b1 + i b2), d pz = c + (pz/pT) b1.
+// cXY = packed upper triangle over (a1, a2, z, b1, b2, c).
+struct Track {
+    float x, y, z, px, py, pz;
+    float eax, eay;
+    float c00, c01, c02, c03, c04, c05;
+    float c11, c12, c13, c14, c15;
+    float c22, c23, c24, c25;
+    float c33, c34, c35;
+    float c44, c45;
+    float c55;
+};
+
+// Change the momentum frame of the covariance: rotate (b1, b2) -> (dc + i ds)(b1 + i b2), then
+// shear c -> c + k1 b1 + k2 b2 (new b's), k1 = T_old dc - T_new, k2 = T_old ds, T = pz/pT.
+__device__ __forceinline__ void reaim_momentum(Track& t, float dc, float ds, float T_old,
+                                               float T_new) {
+    float a, b;
+    a = t.c03; b = t.c04; t.c03 = dc * a - ds * b; t.c04 = ds * a + dc * b;
+    a = t.c13; b = t.c14; t.c13 = dc * a - ds * b; t.c14 = ds * a + dc * b;
+    a = t.c23; b = t.c24; t.c23 = dc * a - ds * b; t.c24 = ds * a + dc * b;
+    a = t.c35; b = t.c45;
+    const float c35 = dc * a - ds * b, c45 = ds * a + dc * b;
+    const float cc = dc * dc, ss = ds * ds, cs = dc * ds;
+    const float ll = t.c33, ln = t.c34, nn = t.c44;
+    t.c33 = cc * ll - 2.0f * cs * ln + ss * nn;
+    t.c44 = ss * ll + 2.0f * cs * ln + cc * nn;
+    t.c34 = cs * (ll - nn) + (cc - ss) * ln;
+    const float k1 = T_old * dc - T_new, k2 = T_old * ds;
+    t.c05 += k1 * t.c03 + k2 * t.c04;
+    t.c15 += k1 * t.c13 + k2 * t.c14;
+    t.c25 += k1 * t.c23 + k2 * t.c24;
+    const float n35 = c35 + k1 * t.c33 + k2 * t.c34;
+    const float n45 = c45 + k1 * t.c34 + k2 * t.c44;
+    t.c55 += k1 * (c35 + n35) + k2 * (c45 + n45);
+    t.c35 = n35;
+    t.c45 = n45;
+}
+
+// Rotate the position-block coordinates (a1, a2) -> (dc + i ds)(a1 + i a2).
+__device__ __forceinline__ void reframe_position(Track& t, float dc, float ds) {
+    float a, b;
+    a = t.c02; b = t.c12; t.c02 = dc * a - ds * b; t.c12 = ds * a + dc * b;
+    a = t.c03; b = t.c13; t.c03 = dc * a - ds * b; t.c13 = ds * a + dc * b;
+    a = t.c04; b = t.c14; t.c04 = dc * a - ds * b; t.c14 = ds * a + dc * b;
+    a = t.c05; b = t.c15; t.c05 = dc * a - ds * b; t.c15 = ds * a + dc * b;
+    const float cc = dc * dc, ss = ds * ds, cs = dc * ds;
+    const float ll = t.c00, ln = t.c01, nn = t.c11;
+    t.c00 = cc * ll - 2.0f * cs * ln + ss * nn;
+    t.c11 = ss * ll + 2.0f * cs * ln + cc * nn;
+    t.c01 = cs * (ll - nn) + (cc - ss) * ln;
+}
+
+// Global-frame covariance (as stored) -> local frame.  Position frame stays global (ea = 1);
+// the momentum block goes to (b1, b2, c).
+__device__ __forceinline__ void enter_local_frame(Track& t) {
+    t.eax = 1.0f;
+    t.eay = 0.0f;
+    const float pt2 = t.px * t.px + t.py * t.py;
+    if (pt2 > 0.0f) {
+        const float ipt = rsqrtf(pt2);
+        // b = conj(e_l) * d(pi): rotation by -phi_p;  c = d pz - (pz/pT) b1
+        reaim_momentum(t, t.px * ipt, -t.py * ipt, 0.0f, t.pz * ipt);
+    }
+}
+
+// Local frame -> global frame (inverse of the above for the current frames).
+__device__ __forceinline__ void leave_local_frame(Track& t) {
+    reframe_position(t, t.eax, t.eay);
+    const float pt2 = t.px * t.px + t.py * t.py;
+    if (pt2 > 0.0f) {
+        const float ipt = rsqrtf(pt2);
+        reaim_momentum(t, t.px * ipt, t.py * ipt, t.pz * ipt, 0.0f);
+    }
+    t.eax = 1.0f;
+    t.eay = 0.0f;
+}
+
+// Result of the helix crossing + local-frame Jacobian ingredients.
+struct Crossing {
+    float xn, yn, zn, pxn, pyn;  // arrival state (pz unchanged)
+    float erx, ery;              // e_r' = w'/r
+    float elx, ely;              // e_l' = pi'/pT
+    float g0, g1, g3, g4;        // G_r over (a1, a2, b1, b2)
+    float t0, t1, t3, t4;        // row t' = G_t - tan(a') G_r
+    float z0, z1, z3, z4;        // row z' over (a1, a2, b1, b2); its z entry is 1, its c entry thk
+    float thk;                   // theta / k = s / pT
+    float mu;                    // k / cos(a')
+    float T;                     // pz / pT (conserved along the helix)
+    float pt2, ipt;
+};
+
+// Reading A3: first outward crossing of the helix with the cylinder of radius L.r, half-angle
+// form  t = tan(theta/2) = D / (a + sqrt(a^2 - D (2b + D))).  Returns false on PROP_FAIL.
+__device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float ik,
+                                                const LayerConst& L, Crossing& o) {
+    const float x = t.x, y = t.y, px = t.px, py = t.py;
+    const float pt2 = px * px + py * py;
+    const float rho2 = x * x + y * y;
+    if (!(L.r2 > rho2)) return false;
+    const float a = x * px + y * py;
+    const float b = (y * px - x * py) - pt2 * ik;
+    const float D = 0.5f * k * (L.r2 - rho2);
+    const float disc = a * a - D * (2.0f * b + D);
+    if (!(disc > 0.0f)) return false;
+    const float den = a + sqrtf(disc);
+    if (!(den > 0.0f)) return false;
+    const float tt = D / den;
+    const float i1 = 1.0f / (1.0f + tt * tt);
+    const float S = 2.0f * tt * i1;
+    const float Cm = tt * S;
+    const float co = 1.0f - Cm;
+    const float theta = 2.0f * atanf(tt);
+    o.thk = theta * ik;
+    o.xn = x + (px * S + py * Cm) * ik;
+    o.yn = y + (py * S - px * Cm) * ik;
+    o.zn = t.z + t.pz * o.thk;
+    o.pxn = px * co + py * S;
+    o.pyn = py * co - px * S;
+    const float ipt = rsqrtf(pt2);
+    o.pt2 = pt2;
+    o.ipt = ipt;
+    o.erx = o.xn * L.inv_r;
+    o.ery = o.yn * L.inv_r;
+    o.elx = o.pxn * ipt;
+    o.ely = o.pyn * ipt;
+    // exp(i a') = conj(e_r') e_l'
+    const float ca = o.erx * o.elx + o.ery * o.ely;
+    const float sa = o.erx * o.ely - o.ery * o.elx;
+    const float ic = 1.0f / ca;
+    const float T = sa * ic;
+    // P = conj(e_r') e_a
+    const float pc = o.erx * t.eax + o.ery * t.eay;
+    const float ps = o.erx * t.eay - o.ery * t.eax;
+    // N = ((S + i Cm)/k) exp(i a')
+    const float nr = (S * ca - Cm * sa) * ik;
+    const float nt = (S * sa + Cm * ca) * ik;
+    o.g0 = pc;  o.g1 = -ps; o.g3 = nr; o.g4 = -nt;
+    o.t0 = ps - T * pc;
+    o.t1 = pc + T * ps;
+    o.t3 = nt - T * nr;
+    o.t4 = nr + T * nt;
+    const float T_ = t.pz * ipt;
+    const float lam = T_ * ic;
+    o.T = T_;
+    o.z0 = -lam * pc;
+    o.z1 = lam * ps;
+    o.z3 = T_ * (o.thk - ic * nr);  // small: the |p|-at-fixed-direction mode does not move z'
+    o.z4 = lam * nt;
+    o.mu = k * ic;
+    return true;
+}
+
+// Propagated covariance in the arrival frame (radial row is exactly zero and not stored).
+struct PropCov {
+    float n11, n12, n13, n14, n15;
+    float n22, n23, n24, n25;
+    float n33, n34, n35;
+    float n44, n45;
+    float n55;
+};
+
+// C' = F~ C F~^T + Q~ (reading A4 Jacobian, A5 process noise at the propagated momentum).
+// RADIAL_NULL: the input covariance already has a zero a1 row (every layer after the first).
+template <bool RADIAL_NULL>
+__device__ __forceinline__ void transport_cov(const Track& t, const Crossing& o, float ms,
+                                              float mass2, PropCov& n) {
+    const float c00 = RADIAL_NULL ? 0.0f : t.c00, c01 = RADIAL_NULL ? 0.0f : t.c01;
+    const float c02 = RADIAL_NULL ? 0.0f : t.c02, c03 = RADIAL_NULL ? 0.0f : t.c03;
+    const float c04 = RADIAL_NULL ? 0.0f : t.c04, c05 = RADIAL_NULL ? 0.0f : t.c05;
+    const float g0 = o.g0, g1 = o.g1, g3 = o.g3, g4 = o.g4;
+    const float t0 = o.t0, t1 = o.t1, t3 = o.t3, t4 = o.t4;
+    const float z0 = o.z0, z1 = o.z1, z3 = o.z3, z4 = o.z4, thk = o.thk, mu = o.mu;
+    // v = C g, w = C tau, u = C zeta
+    const float v0 = c00 * g0 + c01 * g1 + c03 * g3 + c04 * g4;
+    const float v1 = c01 * g0 + t.c11 * g1 + t.c13 * g3 + t.c14 * g4;
+    const float v3 = c03 * g0 + t.c13 * g1 + t.c33 * g3 + t.c34 * g4;
+    const float v4 = c04 * g0 + t.c14 * g1 + t.c34 * g3 + t.c44 * g4;
+    const float v5 = c05 * g0 + t.c15 * g1 + t.c35 * g3 + t.c45 * g4;
+    const float w0 = c00 * t0 + c01 * t1 + c03 * t3 + c04 * t4;
+    const float w1 = c01 * t0 + t.c11 * t1 + t.c13 * t3 + t.c14 * t4;
+    const float w3 = c03 * t0 + t.c13 * t1 + t.c33 * t3 + t.c34 * t4;
+    const float w4 = c04 * t0 + t.c14 * t1 + t.c34 * t3 + t.c44 * t4;
+    const float w5 = c05 * t0 + t.c15 * t1 + t.c35 * t3 + t.c45 * t4;
+    const float u0 = c00 * z0 + c01 * z1 + c02 + c03 * z3 + c04 * z4 + c05 * thk;
+    const float u1 = c01 * z0 + t.c11 * z1 + t.c12 + t.c13 * z3 + t.c14 * z4 + t.c15 * thk;
+    const float u2 = c02 * z0 + t.c12 * z1 + t.c22 + t.c23 * z3 + t.c24 * z4 + t.c25 * thk;
+    const float u3 = c03 * z0 + t.c13 * z1 + t.c23 + t.c33 * z3 + t.c34 * z4 + t.c35 * thk;
+    const float u4 = c04 * z0 + t.c14 * z1 + t.c24 + t.c34 * z3 + t.c44 * z4 + t.c45 * thk;
+    const float u5 = c05 * z0 + t.c15 * z1 + t.c25 + t.c35 * z3 + t.c45 * z4 + t.c55 * thk;
+    const float gCg = g0 * v0 + g1 * v1 + g3 * v3 + g4 * v4;
+    const float tCg = t0 * v0 + t1 * v1 + t3 * v3 + t4 * v4;
+    const float zCg = g0 * u0 + g1 * u1 + g3 * u3 + g4 * u4;
+    n.n11 = t0 * w0 + t1 * w1 + t3 * w3 + t4 * w4;
+    n.n12 = t0 * u0 + t1 * u1 + t3 * u3 + t4 * u4;
+    n.n13 = w3;
+    n.n14 = w4 + mu * tCg;
+    n.n15 = w5;
+    n.n22 = z0 * u0 + z1 * u1 + u2 + z3 * u3 + z4 * u4 + thk * u5;
+    n.n23 = u3;
+    n.n24 = u4 + mu * zCg;
+    n.n25 = u5;
+    // Highland (A5): theta0^2 = ms (p^2 + m^2) / p^4;  Q = theta0^2 (p^2 I - p p^T), p = (pT, 0, pz),
+    // sheared to (b1, b2, c):  Q~ = theta0^2 [[pz^2, 0, -pz p^2/pT], [0, p^2, 0], [., 0, p^4/pT^2]]
+    const float pz = t.pz;
+    const float p2 = o.pt2 + pz * pz;
+    const float ip2 = 1.0f / p2;
+    const float th2 = ms * (p2 + mass2) * ip2 * ip2;
+    const float qc = th2 * p2 * o.ipt;  // theta0^2 p^2 / pT
+    n.n33 = t.c33 + th2 * pz * pz;
+    n.n34 = t.c34 + mu * v3;
+    n.n35 = t.c35 - qc * pz;
+    n.n44 = t.c44 + mu * (2.0f * v4 + mu * gCg) + th2 * p2;
+    n.n45 = t.c45 + mu * v5;
+    n.n55 = t.c55 + qc * (p2 * o.ipt);
+}
+
+// Hit in the arrival frame: residual (r, t, z) and rotated covariance.
+struct LocalHit {
+    float rr, rt, rz;
+    float vrr, vrt, vrz, vtt, vtz, vzz;
+};
+
+__device__ __forceinline__ void hit_to_local(const Crossing& o, float mx, float my, float mz,
+                                             float vxx, float vxy, float vxz, float vyy, float vyz,
+                                             float vzz, LocalHit& h) {
+    const float c = o.erx, s = o.ery;
+    const float dx = mx - o.xn, dy = my - o.yn;
+    h.rr = c * dx + s * dy;
+    h.rt = c * dy - s * dx;
+    h.rz = mz - o.zn;
+    const float cc = c * c, ss = s * s, cs = c * s;
+    h.vrr = cc * vxx + 2.0f * cs * vxy + ss * vyy;
+    h.vtt = ss * vxx - 2.0f * cs * vxy + cc * vyy;
+    h.vrt = cs * (vyy - vxx) + (cc - ss) * vxy;
+    h.vrz = c * vxz + s * vyz;
+    h.vtz = c * vyz - s * vxz;
+    h.vzz = vzz;
+}
+
+// Inverse of S = C'_pp + V~ (symmetric 3x3, cofactors).  Returns det.
+struct Sym3 {
+    float rr, rt, rz, tt, tz, zz;
+};
+
+__device__ __forceinline__ float invert_S(const PropCov& n, const LocalHit& h, Sym3& si) {
+    const float srr = h.vrr, srt = h.vrt, srz = h.vrz;
+    const float stt = n.n11 + h.vtt, stz = n.n12 + h.vtz, szz = n.n22 + h.vzz;
+    const float k00 = stt * szz - stz * stz;
+    const float k01 = srz * stz - srt * szz;
+    const float k02 = srt * stz - srz * stt;
+    const float det = srr * k00 + srt * k01 + srz * k02;
+    const float id = 1.0f / det;
+    si.rr = k00 * id;
+    si.rt = k01 * id;
+    si.rz = k02 * id;
+    si.tt = (srr * szz - srz * srz) * id;
+    si.tz = (srt * srz - srr * stz) * id;
+    si.zz = (srr * stt - srt * srt) * id;
+    return det;
+}
+
+__device__ __forceinline__ float chi2_of(const Sym3& si, const LocalHit& h) {
+    const float ur = si.rr * h.rr + si.rt * h.rt + si.rz * h.rz;
+    const float ut = si.rt * h.rr + si.tt * h.rt + si.tz * h.rz;
+    const float uz = si.rz * h.rr + si.tz * h.rt + si.zz * h.rz;
+    return h.rr * ur + h.rt * ut + h.rz * uz;
+}
+
+// Kalman update in the arrival frame, then re-aim the momentum frame at the updated momentum.
+// On success writes the new track (position frame = arrival frame) and returns the chi2
+// increment through *dchi2.  Returns a status bit on failure (track untouched).
+__device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, const PropCov& n,
+                                                  const LocalHit& h, float* dchi2) {
+    Sym3 si;
+    const float det = invert_S(n, h, si);
+    if (!(det > 0.0f)) return ST_S_NOT_PD;
+    const float chi2 = chi2_of(si, h);
+    // K = C'[:, (t,z)] Si[(t,z), :]   (rows t z l n p; columns r t z)
+#define KF_KROW(ct, cz, kr, kt, kz)                     \
+    const float kr = ct * si.rt + cz * si.rz;           \
+    const float kt = ct * si.tt + cz * si.tz;           \
+    const float kz = ct * si.tz + cz * si.zz;
+    KF_KROW(n.n11, n.n12, k1r, k1t, k1z)
+    KF_KROW(n.n12, n.n22, k2r, k2t, k2z)
+    KF_KROW(n.n13, n.n23, k3r, k3t, k3z)
+    KF_KROW(n.n14, n.n24, k4r, k4t, k4z)
+    KF_KROW(n.n15, n.n25, k5r, k5t, k5z)
+#undef KF_KROW
+    const float d1 = k1r * h.rr + k1t * h.rt + k1z * h.rz;
+    const float d2 = k2r * h.rr + k2t * h.rt + k2z * h.rz;
+    const float d3 = k3r * h.rr + k3t * h.rt + k3z * h.rz;
+    const float d4 = k4r * h.rr + k4t * h.rt + k4z * h.rz;
+    const float d5 = k5r * h.rr + k5t * h.rt + k5z * h.rz;
+    // finite(chi2) and finite(state): any non-finite term makes this sum non-finite
+    const float probe = chi2 + ((d1 + d2) + (d3 + d4) + d5) * 0.0f;
+    if (!(fabsf(probe) < __int_as_float(0x7f800000))) return ST_NONFINITE;
+    *dchi2 = chi2;
+    // state
+    t.x = o.xn - o.ery * d1;
+    t.y = o.yn + o.erx * d1;
+    t.z = o.zn + d2;
+    const float pxu = o.pxn + o.elx * d3 - o.ely * d4;
+    const float pyu = o.pyn + o.ely * d3 + o.elx * d4;
+    t.px = pxu;
+    t.py = pyu;
+    const float pzu = t.pz + d5 + o.T * d3;
+    t.pz = pzu;
+    t.eax = o.erx;
+    t.eay = o.ery;
+    // position rows: C[i][a] = sum_b K[i][b] V~[b][a], a in (t, z); radial row/column stay zero
+    t.c00 = 0.0f; t.c01 = 0.0f; t.c02 = 0.0f; t.c03 = 0.0f; t.c04 = 0.0f; t.c05 = 0.0f;
+    t.c11 = k1r * h.vrt + k1t * h.vtt + k1z * h.vtz;
+    t.c12 = k1r * h.vrz + k1t * h.vtz + k1z * h.vzz;
+    t.c22 = k2r * h.vrz + k2t * h.vtz + k2z * h.vzz;
+    t.c13 = k3r * h.vrt + k3t * h.vtt + k3z * h.vtz;
+    t.c23 = k3r * h.vrz + k3t * h.vtz + k3z * h.vzz;
+    t.c14 = k4r * h.vrt + k4t * h.vtt + k4z * h.vtz;
+    t.c24 = k4r * h.vrz + k4t * h.vtz + k4z * h.vzz;
+    t.c15 = k5r * h.vrt + k5t * h.vtt + k5z * h.vtz;
+    t.c25 = k5r * h.vrz + k5t * h.vtz + k5z * h.vzz;
+    // momentum block: C'_mm - K_m C'_pm  (C'_pm rows t, z)
+    t.c33 = n.n33 - (k3t * n.n13 + k3z * n.n23);
+    t.c34 = n.n34 - (k3t * n.n14 + k3z * n.n24);
+    t.c35 = n.n35 - (k3t * n.n15 + k3z * n.n25);
+    t.c44 = n.n44 - (k4t * n.n14 + k4z * n.n24);
+    t.c45 = n.n45 - (k4t * n.n15 + k4z * n.n25);
+    t.c55 = n.n55 - (k5t * n.n15 + k5z * n.n25);
+    // re-aim the momentum frame: exp(i d) = conj(e_l,new) e_l' = ((pT + d3) - i d4) / pT,new
+    const float pt = o.pt2 * o.ipt;
+    const float ar = pt + d3;
+    const float iptn = rsqrtf(ar * ar + d4 * d4);
+    reaim_momentum(t, ar * iptn, -d4 * iptn, o.T, pzu * iptn);
+    return 0u;
+}
+
+// Keep the propagated state (no hit used): position frame = arrival frame, momentum frame
+// already follows the propagated momentum.
+__device__ __forceinline__ void commit_propagated(Track& t, const Crossing& o, const PropCov& n) {
+    t.x = o.xn; t.y = o.yn; t.z = o.zn; t.px = o.pxn; t.py = o.pyn;
+    t.eax = o.erx; t.eay = o.ery;
+    t.c00 = 0.0f; t.c01 = 0.0f; t.c02 = 0.0f; t.c03 = 0.0f; t.c04 = 0.0f; t.c05 = 0.0f;
+    t.c11 = n.n11; t.c12 = n.n12; t.c13 = n.n13; t.c14 = n.n14; t.c15 = n.n15;
+    t.c22 = n.n22; t.c23 = n.n23; t.c24 = n.n24; t.c25 = n.n25;
+    t.c33 = n.n33; t.c34 = n.n34; t.c35 = n.n35;
+    t.c44 = n.n44; t.c45 = n.n45;
+    t.c55 = n.n55;
+}
+
+// ---- SoA load / store (element-major, plane stride ld) ---------------------------------------
+__device__ __forceinline__ void load_track(Track& t, const float* __restrict__ par,
+                                           const float* __restrict__ cov, int64_t ld, int64_t i) {
+    t.x = __ldg(par + 0 * ld + i);  t.y = __ldg(par + 1 * ld + i);  t.z = __ldg(par + 2 * ld + i);
+    t.px = __ldg(par + 3 * ld + i); t.py = __ldg(par + 4 * ld + i); t.pz = __ldg(par + 5 * ld + i);
+    t.c00 = __ldg(cov + 0 * ld + i);  t.c01 = __ldg(cov + 1 * ld + i);  t.c02 = __ldg(cov + 2 * ld + i);
+    t.c03 = __ldg(cov + 3 * ld + i);  t.c04 = __ldg(cov + 4 * ld + i);  t.c05 = __ldg(cov + 5 * ld + i);
+    t.c11 = __ldg(cov + 6 * ld + i);  t.c12 = __ldg(cov + 7 * ld + i);  t.c13 = __ldg(cov + 8 * ld + i);
+    t.c14 = __ldg(cov + 9 * ld + i);  t.c15 = __ldg(cov + 10 * ld + i);
+    t.c22 = __ldg(cov + 11 * ld + i); t.c23 = __ldg(cov + 12 * ld + i); t.c24 = __ldg(cov + 13 * ld + i);
+    t.c25 = __ldg(cov + 14 * ld + i);
+    t.c33 = __ldg(cov + 15 * ld + i); t.c34 = __ldg(cov + 16 * ld + i); t.c35 = __ldg(cov + 17 * ld + i);
+    t.c44 = __ldg(cov + 18 * ld + i); t.c45 = __ldg(cov + 19 * ld + i);
+    t.c55 = __ldg(cov + 20 * ld + i);
+    t.eax = 1.0f;
+    t.eay = 0.0f;
+}
+
+__device__ __forceinline__ void store_track(const Track& t, float* __restrict__ par,
+                                            float* __restrict__ cov, int64_t ld, int64_t i) {
+    par[0 * ld + i] = t.x;  par[1 * ld + i] = t.y;  par[2 * ld + i] = t.z;
+    par[3 * ld + i] = t.px; par[4 * ld + i] = t.py; par[5 * ld + i] = t.pz;
+    cov[0 * ld + i] = t.c00;  cov[1 * ld + i] = t.c01;  cov[2 * ld + i] = t.c02;
+    cov[3 * ld + i] = t.c03;  cov[4 * ld + i] = t.c04;  cov[5 * ld + i] = t.c05;
+    cov[6 * ld + i] = t.c11;  cov[7 * ld + i] = t.c12;  cov[8 * ld + i] = t.c13;
+    cov[9 * ld + i] = t.c14;  cov[10 * ld + i] = t.c15;
+    cov[11 * ld + i] = t.c22; cov[12 * ld + i] = t.c23; cov[13 * ld + i] = t.c24;
+    cov[14 * ld + i] = t.c25;
+    cov[15 * ld + i] = t.c33; cov[16 * ld + i] = t.c34; cov[17 * ld + i] = t.c35;
+    cov[18 * ld + i] = t.c44; cov[19 * ld + i] = t.c45;
+    cov[20 * ld + i] = t.c55;
+}
+
+}  // namespace kf

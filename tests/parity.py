@@ -1,0 +1,69 @@
+"""Parity metric between a fitter's output and the fp64 oracle (reading A15).
+
+north_star: relative 1e-4 on track parameters, 1e-3 on covariance elements, 1e-3 on chi2.
+A relative error of a component that is legitimately ~0 is undefined, so:
+  position   |d| <= 1e-4 * r_last            momentum |d| <= 1e-4 * |p|
+  covariance |dC_ij| <= 1e-3 * s_i s_j,  s_i = sqrt(max diagonal of i's 3x3 block)
+  chi2       |d| <= 1e-3 * max(chi2, 1)
+Diverged tracks (A14: oracle chi2 > ndf + 9 sqrt(2 ndf) or any oracle status bit) are excluded
+and counted; they must be < 0.1 % of a config.
+Pure numpy bookkeeping: no Kalman arithmetic here.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+TOL_PAR, TOL_COV, TOL_CHI2 = 1e-4, 1e-3, 1e-3
+_TRI = [(i, j) for i in range(6) for j in range(i, 6)]
+
+
+def dense_from_packed(c21: np.ndarray) -> np.ndarray:
+    n = c21.shape[1]
+    out = np.empty((n, 6, 6))
+    for k, (i, j) in enumerate(_TRI):
+        out[:, i, j] = c21[k]
+        out[:, j, i] = c21[k]
+    return out
+
+
+def diverged_mask(oracle: dict) -> np.ndarray:
+    ndf = np.maximum(2 * oracle["nhits"] - 5, 1).astype(np.float64)
+    return (oracle["status"] != 0) | (oracle["chi2"] > ndf + 9.0 * np.sqrt(2.0 * ndf))
+
+
+def compare_fit(gpu: dict, oracle: dict, r_last: float | np.ndarray, max_diverged_frac: float = 1e-3) -> dict:
+    """gpu: par[6][n] f32, cov[21][n] f32, chi2[n], nhits[n], status[n]; oracle: O.fit_tracks dict.
+    Returns the worst normalised errors (each must be <= 1 to pass) and raises AssertionError on failure."""
+    n = oracle["par"].shape[1]
+    bad = diverged_mask(oracle)
+    ok = ~bad
+    frac = bad.mean() if n else 0.0
+    assert frac <= max_diverged_frac, f"diverged fraction {frac:.4%}"
+    gp = np.asarray(gpu["par"], dtype=np.float64)[:, :n]
+    gc = dense_from_packed(np.asarray(gpu["cov"], dtype=np.float64)[:, :n])
+    op, oc = oracle["par"], oracle["cov"]
+    r_last = np.broadcast_to(np.asarray(r_last, dtype=np.float64), (n,))
+    e_pos = np.max(np.abs(gp[:3] - op[:3]), axis=0) / (TOL_PAR * r_last)
+    pabs = np.sqrt((op[3:] ** 2).sum(axis=0))
+    e_mom = np.max(np.abs(gp[3:] - op[3:]), axis=0) / (TOL_PAR * pabs)
+    d = np.diagonal(oc, axis1=1, axis2=2)
+    s = np.sqrt(np.concatenate([np.repeat(d[:, :3].max(axis=1, keepdims=True), 3, 1),
+                                np.repeat(d[:, 3:].max(axis=1, keepdims=True), 3, 1)], axis=1))
+    scale = s[:, :, None] * s[:, None, :]
+    e_cov = (np.abs(gc - oc) / (TOL_COV * scale)).reshape(n, -1).max(axis=1)
+    dd = np.sqrt(np.clip(d, 1e-300, None))
+    e_cov_strict = (np.abs(gc - oc) / (TOL_COV * dd[:, :, None] * dd[:, None, :])).reshape(n, -1).max(axis=1)
+    gchi = np.asarray(gpu["chi2"], dtype=np.float64)[:n]
+    e_chi = np.abs(gchi - oracle["chi2"]) / (TOL_CHI2 * np.maximum(oracle["chi2"], 1.0))
+    res = dict(n=n, n_diverged=int(bad.sum()),
+               pos=float(e_pos[ok].max(initial=0)), mom=float(e_mom[ok].max(initial=0)),
+               cov=float(e_cov[ok].max(initial=0)), chi2=float(e_chi[ok].max(initial=0)),
+               cov_strict_fail_frac=float((e_cov_strict[ok] > 1).mean()) if ok.any() else 0.0,
+               mom_p99=float(np.percentile(e_mom[ok], 99)) if ok.any() else 0.0,
+               cov_p99=float(np.percentile(e_cov[ok], 99)) if ok.any() else 0.0,
+               chi2_p99=float(np.percentile(e_chi[ok], 99)) if ok.any() else 0.0)
+    assert np.array_equal(np.asarray(gpu["nhits"])[:n][ok], oracle["nhits"][ok]), "nhits differ"
+    assert np.array_equal(np.asarray(gpu["status"])[:n][ok], oracle["status"][ok]), "status differ"
+    for key in ("pos", "mom", "cov", "chi2"):
+        assert res[key] <= 1.0, f"{key} parity failed: {res}"
+    return res

@@ -1,0 +1,205 @@
+"""GPU parity of kf_fit_tracks (through the C ABI) against the fp64 oracle, element by element.
+
+Tolerances: BASELINE.json north_star / DESIGN.md reading A15, written in tests/parity.py."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import kf_oracle as O
+from tests.parity import compare_fit
+from workloads import barrel_events as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import paper_1705_02876_b200 as K
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    c = K.KFContext(0)
+    yield c
+    c.close()
+
+
+def _gpu_fit(ctx, batch, with_mask=True):
+    from paper_1705_02876_b200.buffers import DeviceFit
+    d = DeviceFit.from_batch(batch, "cuda:0", with_mask=with_mask)
+    d.fit(ctx)
+    torch.cuda.synchronize()
+    return d.results()
+
+
+@pytest.mark.parametrize("config", [0, 1, 3])
+def test_fit_parity_full_config(ctx, config):
+    b = W.make_fit_batch(config)
+    g = _gpu_fit(ctx, b)
+    o = O.fit_batch(b, nthreads=8)
+    res = compare_fit(g, o, float(b.radius[-1]))
+    print(f"config {config}: {res}")
+
+
+def test_fit_parity_config2_sampled(ctx):
+    """Config 2 at full size (2M tracks, one launch, the configuration bench.py times); the oracle
+    checks every 16th event's tracks one by one."""
+    cfg = W.get_config(2)
+    b = W.make_fit_batch(2)
+    assert b.n == 2_000_000
+    g = _gpu_fit(ctx, b)
+    for ev in range(0, cfg.n_events, 16):
+        lo, hi = ev * cfg.n_tracks, (ev + 1) * cfg.n_tracks
+        sub = W.simulate_event(cfg, ev)
+        assert np.array_equal(sub.par, b.par[:, lo:hi])
+        o = O.fit_batch(sub, nthreads=8)
+        gs = {k: (v[..., lo:hi] if k in ("par", "cov") else v[lo:hi]) for k, v in g.items()}
+        compare_fit(gs, o, float(b.radius[-1]))
+    ndf = 2 * g["nhits"] - 5
+    assert (g["status"] != 0).mean() < 1e-3
+    assert 0.9 < np.median(g["chi2"] / ndf) < 1.1
+
+
+@pytest.mark.parametrize("n", [1, 31, 33, 127, 129, 1001])
+def test_fit_ragged_sizes(ctx, n):
+    b = W.simulate_event(W.get_config(1), 5, n_tracks=n)
+    g = _gpu_fit(ctx, b)
+    o = O.fit_batch(b)
+    compare_fit(g, o, float(b.radius[-1]), max_diverged_frac=1.0)
+
+
+def test_fit_empty(ctx):
+    b = W.simulate_event(W.get_config(1), 5, n_tracks=4)
+    from paper_1705_02876_b200.buffers import DeviceFit
+    d = DeviceFit.from_batch(b, "cuda:0")
+    d.n = 0
+    d.out_par.fill_(7.0)
+    d.fit(ctx)
+    torch.cuda.synchronize()
+    assert torch.all(d.out_par == 7.0)
+
+
+def test_fit_mask_null_equals_all_layers(ctx):
+    b = W.simulate_event(W.get_config(1), 6, n_tracks=500)
+    g1 = _gpu_fit(ctx, b, with_mask=True)
+    g2 = _gpu_fit(ctx, b, with_mask=False)
+    for k in g1:
+        assert np.array_equal(g1[k], g2[k]), k
+
+
+def test_fit_missing_layers(ctx):
+    """Hit masks with holes (plus: no hit at all, a missing first layer, only the first three).
+    The first three layers are kept in the random part: a track whose second hit comes 16 cm after
+    its first is propagated with a 30 % momentum prior, far outside the linear regime, and fp32
+    then reaches only ~1e-3 on the momentum variance."""
+    b = W.simulate_event(W.get_config(1), 8, n_tracks=2000)
+    rng = np.random.default_rng(3)
+    b.mask = (rng.integers(0, 1 << 10, size=b.n) | 0b111).astype(np.uint32)
+    b.mask[:50] = 0
+    b.mask[50:100] = 0b1111111110
+    b.mask[100:150] = 0b0000000111
+    g = _gpu_fit(ctx, b)
+    o = O.fit_batch(b)
+    nh = o["nhits"]
+    # tracks with >= 4 hits are well constrained: full parity; the others must agree on bookkeeping
+    sel = nh >= 4
+    sub_g = {k: (v[..., sel] if k in ("par", "cov") else v[sel]) for k, v in g.items()}
+    sub_o = {k: (v[..., sel] if k == "par" else v[sel]) for k, v in o.items()}
+    compare_fit(sub_g, sub_o, float(b.radius[-1]), max_diverged_frac=0.05)
+    assert np.array_equal(g["nhits"], nh)
+    # nothing fitted: the seed comes back bit-exact
+    z = nh == 0
+    assert z.sum() >= 50
+    assert np.array_equal(g["par"][:, z], b.par[:, z]) and np.array_equal(g["cov"][:, z], b.cov[:, z])
+    assert np.all(g["chi2"][z] == 0)
+
+
+def _zero_status(d):
+    d = dict(d)
+    d["status"] = np.zeros_like(d["status"])
+    return d
+
+
+def test_fit_status_bits(ctx):
+    """Degenerate tracks: bad charge, NaN hit (NONFINITE), non-positive-definite S (S_NOT_PD).
+    Same status, same hits used and same surviving state as the oracle."""
+    b = W.simulate_event(W.get_config(1), 9, n_tracks=64)
+    b.q[0] = 0
+    b.q[1] = 3
+    b.hpos[4, 1, 4] = np.nan                       # NaN hit on layer 4 of track 4
+    b.hcov[2, :, 5] = 0.0                          # zero hit covariance on layer 2 of track 5 ...
+    b.hcov[2, 0, 5] = -1.0                         # ... with a negative variance: det S <= 0
+    g = _gpu_fit(ctx, b)
+    o = O.fit_batch(b)
+    assert g["status"][0] == 8 and g["status"][1] == 8
+    assert np.array_equal(g["par"][:, :2], b.par[:, :2]) and np.array_equal(g["cov"][:, :2], b.cov[:, :2])
+    assert np.array_equal(g["status"], o["status"]), (g["status"][:8], o["status"][:8])
+    assert np.array_equal(g["nhits"], o["nhits"])
+    assert o["status"][4] == 4 and o["status"][5] == 2 and o["nhits"][4] == 9 and o["nhits"][5] == 9
+    sel = np.arange(b.n) >= 2
+    sub_g = {k: (v[..., sel] if k in ("par", "cov") else v[sel]) for k, v in g.items()}
+    sub_o = {k: (v[..., sel] if k == "par" else v[sel]) for k, v in o.items()}
+    compare_fit(_zero_status(sub_g), _zero_status(sub_o), float(b.radius[-1]), max_diverged_frac=1.0)
+
+
+def test_fit_propagation_failure(ctx):
+    """Tracks of pT 0.17-0.18 GeV (2R about 30 cm) asked for hits at r = 36 and 40 cm: no outward
+    crossing -> PROP_FAIL on both sides, state kept from the last good layer."""
+    cfg = W.BarrelConfig(1, 1, 256, 10, 0.17, 0.18, 1.0, 0.01)
+    b = W.simulate_event(cfg, 21)
+    assert np.all((b.mask >> 8) == 0)
+    b.mask = b.mask | np.uint32(0b11 << 8)
+    g = _gpu_fit(ctx, b)
+    o = O.fit_batch(b)
+    assert np.all(o["status"] == 1)
+    assert np.array_equal(g["status"], o["status"]) and np.array_equal(g["nhits"], o["nhits"])
+    compare_fit(_zero_status(g), _zero_status(o), float(b.radius[-1]), max_diverged_frac=0.05)
+
+
+def test_fit_in_place(ctx):
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.simulate_event(W.get_config(1), 10, n_tracks=777)
+    ref = _gpu_fit(ctx, b)
+    d = DeviceFit.from_batch(b, "cuda:0")
+    ctx.fit_tracks(d.geom, d.n, d.par, d.cov, d.q, d.hpos, d.hcov, d.mask, d.par, d.cov,
+                   d.out_chi2, d.out_nhits, d.out_status)
+    torch.cuda.synchronize()
+    assert np.array_equal(d.par[:, :d.n].cpu().numpy(), ref["par"])
+    assert np.array_equal(d.cov[:, :d.n].cpu().numpy(), ref["cov"])
+
+
+def test_fit_host_path_equals_device_path(ctx):
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.make_fit_batch(1)
+    ref = _gpu_fit(ctx, b)
+    h = DeviceFit.from_batch(b, "cpu", pin=True)
+    h.fit_host(ctx)
+    r = h.results()
+    for k in ref:
+        assert np.array_equal(ref[k], r[k]), k
+
+
+def test_fit_argument_errors(ctx):
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.simulate_event(W.get_config(1), 5, n_tracks=16)
+    d = DeviceFit.from_batch(b, "cuda:0")
+    d.out_par.fill_(5.0)
+    bad = K.Geometry(d.geom.radius_cm[::-1].copy(), d.geom.x_over_X0, 3.8, 0.13957)
+    with pytest.raises(K.KFError) as e:
+        ctx.fit_tracks(bad, d.n, d.par, d.cov, d.q, d.hpos, d.hcov, d.mask, d.out_par, d.out_cov,
+                       d.out_chi2, d.out_nhits, d.out_status)
+    assert e.value.code == -4
+    zero_b = K.Geometry(d.geom.radius_cm, d.geom.x_over_X0, 0.0, 0.13957)
+    with pytest.raises(K.KFError) as e:
+        ctx.fit_tracks(zero_b, d.n, d.par, d.cov, d.q, d.hpos, d.hcov, d.mask, d.out_par, d.out_cov,
+                       d.out_chi2, d.out_nhits, d.out_status)
+    assert e.value.code == -4
+    mis_par = torch.zeros(6 * 20 + 1, dtype=torch.float32, device="cuda:0")[1:].view(6, 20)
+    mis_cov = torch.zeros(21, 20, dtype=torch.float32, device="cuda:0")
+    with pytest.raises(K.KFError) as e:              # plane pointer off by 4 bytes
+        ctx.fit_tracks(d.geom, d.n, mis_par, mis_cov, d.q, d.hpos, d.hcov, d.mask, d.out_par, d.out_cov,
+                       d.out_chi2, d.out_nhits, d.out_status)
+    assert e.value.code == -3
+    with pytest.raises((K.KFError, ValueError)):     # wrong number of hit layers
+        ctx.fit_tracks(K.Geometry(d.geom.radius_cm[:5], d.geom.x_over_X0[:5], 3.8, 0.13957), d.n, d.par, d.cov, d.q,
+                       d.hpos, d.hcov, d.mask, d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status)
+    torch.cuda.synchronize()
+    assert torch.all(d.out_par == 5.0)               # on error no output is written

@@ -1,0 +1,248 @@
+#!/usr/bin/env python
+"""bench.py -- Kalman track fits per second on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Workload: BASELINE.json configs[2] -- 100 events x 20 000 tracks (2 000 000 fits) of the 10-layer
+barrel, synthetic (workloads/barrel_events.py), SoA, device-resident.  One step = one kf_fit_tracks
+call over the whole batch (one kernel launch).  With N > 1 (torchrun) every
+rank fits its own 100 events (weak scaling, no data-path collective); `value` = all ranks' fits / the
+slowest rank's device time.  `e2e` is the same metric through kf_fit_tracks_host with pinned HOST
+buffers, copies inside the timed region.  `--impl reference` times the fp64 CPU oracle instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "kalman_track_fits_per_sec_10_layer_barrel"
+UNIT = "fits/s"
+CONFIG_INDEX = 2
+# dram__bytes_read.sum + dram__bytes_write.sum of fit_kernel for one 2M-track launch, from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture exists).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def _peaks() -> tuple[float, str]:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.002):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        self._period = period_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40,
+                 "sw_thermal_slowdown": 0x20, "hw_power_brake_slowdown": 0x80}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self._period)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self) -> dict:
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def _make_batch(rank: int, n_events: int):
+    from workloads import barrel_events as W
+    from paper_1705_02876_b200.sharding import events_of_rank
+    cfg = W.get_config(CONFIG_INDEX)
+    evs = [W.simulate_event(cfg, e) for e in events_of_rank(n_events, rank)]
+    return cfg, (evs[0] if len(evs) == 1 else W.concat_batches(evs))
+
+
+def _oracle_rate(batch, n_tracks: int, threads: int, repeats: int = 1) -> tuple[float, float]:
+    """fits/s of the oracle as it stands on the first n_tracks tracks (conversion to its AoS double
+    layout excluded, the C call timed)."""
+    from oracle import kf_oracle as O
+    sl = lambda a: np.ascontiguousarray(a[..., :n_tracks])
+    args = (batch.radius, batch.x_over_X0, batch.Bz, batch.mass, sl(batch.par), sl(batch.cov), sl(batch.q),
+            sl(batch.hpos), sl(batch.hcov), sl(batch.mask))
+    best = None
+    for _ in range(repeats):
+        timing = {}
+        O.fit_tracks(*args, nthreads=threads, timing=timing)
+        best = timing["seconds"] if best is None else min(best, timing["seconds"])
+    return n_tracks / best, best
+
+
+def run_reference(args) -> None:
+    """--impl reference: the fp64 oracle on the host cores, same metric / config.  One step = one
+    oracle fit of a bounded sample (5 events = 100 000 tracks) of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import kf_oracle as O
+    O.build()
+    cores = min(os.cpu_count() or 1, 64)
+    sample_events = 5
+    cfg, batch = _make_batch(0, sample_events)
+    n = batch.n
+    for _ in range(max(1, min(args.warmup, 2))):
+        _oracle_rate(batch, n, cores)
+    steps = max(1, args.steps)
+    secs = [_oracle_rate(batch, n, cores)[1] for _ in range(steps)]
+    total = float(np.sum(secs))
+    value = n * steps / total
+    sample = f"{sample_events} events x {cfg.n_tracks} tracks of configs[2] per step, {steps} steps, C call timed"
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * total / steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": "configs[2] sample: 10-layer barrel, 0.01 X0/layer, %d tracks per step" % n},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out), flush=True)
+
+
+def run_ours(args) -> None:
+    import torch
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200 import sharding
+    from paper_1705_02876_b200.buffers import DeviceFit
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    rank, local_rank, ws = sharding.init()
+    if ws != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={ws}: launch with torchrun --nproc-per-node {args.gpus}")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    cfg, batch = _make_batch(rank, args.events)
+    n, L = batch.n, batch.n_layers
+    stream = torch.cuda.Stream(device=dev)
+    ctx = K.KFContext(local_rank, stream)
+    d = DeviceFit.from_batch(batch, dev)
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-ups, then exactly K steps between two events on the launch stream
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            d.fit(ctx)
+    torch.cuda.synchronize()
+    sharding.barrier(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        torch.cuda.synchronize()
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(args.steps):
+                d.fit(ctx)
+            e1.record(stream)
+        torch.cuda.synchronize()
+    sharding.barrier(dev)
+    ms_local = e0.elapsed_time(e1)
+    ms_total = sharding.max_over_ranks(ms_local, dev)
+    n_all = sharding.sum_over_ranks(float(n), dev)
+    ms_per_step = ms_total / args.steps
+    value = n_all * args.steps / (ms_total * 1e-3)
+
+    # ---- end to end: pinned HOST buffers through kf_fit_tracks_host, copies inside the timed region
+    h = DeviceFit.from_batch(batch, "cpu", pin=True)
+    ctx.reserve(0, n, L)
+    e2e_steps = max(3, min(args.steps, 10))
+    h.fit_host(ctx)
+    sharding.barrier(dev)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        h.fit_host(ctx)                       # returns when the outputs are in host memory
+    torch.cuda.synchronize()
+    e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+    h2d = n * (6 * 4 + 21 * 4 + 1 + 4 + L * 9 * 4)
+    d2h = n * (27 * 4 + 12)
+    e2e = {"value": n_all * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+           "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "kf_fit_tracks_host, pinned host SoA buffers"}
+    same = all(np.array_equal(a, b) for a, b in zip(d.results().values(), h.results().values()))
+
+    if rank == 0:
+        peak, peak_src = _peaks()
+        alg_bytes = d.algorithmic_bytes
+        achieved = alg_bytes / (ms_local / args.steps * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "kf::fit_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": int(alg_bytes), "bytes_per_fit": 233 + 36 * L}
+        threads = min(os.cpu_count() or 1, 64)
+        ns = min(n, 50 * cfg.n_tracks)
+        cpu_rate, cpu_s = _oracle_rate(batch, ns, threads)
+        cpu = {"value": cpu_rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"first {ns} tracks of the workload, one fp64 oracle fit, C call timed ({cpu_s:.2f} s wall)"}
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": args.steps, "warmup": args.warmup,
+               "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "f32", "data": "synthetic",
+               "config": {"workload": "configs[2]: %d events x %d tracks per GPU, 10-layer barrel r=4..40 cm, Bz=3.8 T, "
+                                      "0.01 X0/layer, SoA device-resident" % (args.events, cfg.n_tracks),
+                          "tracks_per_gpu": n, "n_layers": L, "parallelism": f"events sharded over {ws} GPU(s), no collective",
+                          "l2": "inputs+outputs (%.2f GB) larger than the 126 MB L2, no flush" % (alg_bytes / 1e9)},
+               "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline,
+               "cpu_baseline": cpu, "host_path_equals_device_path": bool(same)}
+        print(json.dumps(out), flush=True)
+    ctx.close()
+    sharding.shutdown()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--events", type=int, default=100, help="events of 20 000 tracks per GPU (configs[2] = 100)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -137,7 +137,7 @@ def update(u, Cm, m, V):
 
 # ------------------------------------------------------------------ batched fit
 def fit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None,
-               nthreads: int = 1, want_trace: bool = False) -> dict:
+               nthreads: int = 1, want_trace: bool = False, timing: dict | None = None) -> dict:
     """Fit n tracks.  Inputs in the SoA fp32 layout of the C ABI (par[6][n], cov21[21][n],
     hpos[L][3][n], hcov[L][6][n]); widened to double, transposed to AoS and handed to
     orc_fit_tracks.  Returns dict(par[6][n], cov[n][6][6], chi2, nhits, status[, trace])."""
@@ -154,10 +154,14 @@ def fit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None
     opar = np.zeros((n, 6)); ocov = np.zeros((n, 6, 6)); ochi2 = np.zeros(n)
     onh = np.zeros(n, dtype=np.int32); ost = np.zeros(n, dtype=np.uint32)
     trace = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
+    import time as _time
+    _t0 = _time.perf_counter()
     rc = lib().orc_fit_tracks(C.c_int64(n), C.c_int(L), _p(rad), _p(xx0), C.c_double(Bz), C.c_double(mass),
                               _p(par_a), _p(cov_a), _p(q_a, C.c_int8), _p(hp_a), _p(hc_a),
                               _p(m_a, C.c_uint32), _p(opar), _p(ocov), _p(ochi2), _p(onh, C.c_int32),
                               _p(ost, C.c_uint32), _p(trace), C.c_int(nthreads))
+    if timing is not None:          # instrumentation only: seconds spent inside the C call
+        timing["seconds"] = _time.perf_counter() - _t0
     if rc != 0:
         raise RuntimeError("orc_fit_tracks failed")
     out = dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost)

@@ -81,3 +81,69 @@ class DeviceFit:
         """HBM bytes one fit must move: 113 in + 120 out + 36 per layer, per track."""
         L = int(self.geom.radius_cm.shape[0])
         return self.n * (233 + 36 * L)
+
+
+@dataclass
+class DeviceLayer:
+    """All hits of one layer on the GPU plus the caller-allocated outputs of kf_bin_hits."""
+    n_hits: int
+    ld: int
+    pos: torch.Tensor      # f32 [3][ld] original order
+    cov: torch.Tensor      # f32 [6][ld]
+    bins: "Bins"
+
+    @staticmethod
+    def from_numpy(pos: np.ndarray, cov: np.ndarray, n_eta: int, n_phi: int, eta_max: float,
+                   device="cuda:0") -> "DeviceLayer":
+        from .binding import Bins
+        n = int(pos.shape[1])
+        ld = padded_ld(n)
+        return DeviceLayer(n, ld, _to_planes(pos.astype(np.float32), ld, device),
+                           _to_planes(cov.astype(np.float32), ld, device),
+                           Bins.allocate(n, n_eta, n_phi, eta_max, device))
+
+    def bin(self, ctx: KFContext, radius_cm: float):
+        ctx.bin_hits(radius_cm, self.n_hits, self.pos, self.cov, self.bins)
+
+
+@dataclass
+class DeviceCandidates:
+    """Track candidates advanced in place, layer by layer, by kf_score_candidates."""
+    n: int
+    ld: int
+    par: torch.Tensor
+    cov: torch.Tensor
+    q: torch.Tensor
+    chi2: torch.Tensor
+    nhits: torch.Tensor
+    status: torch.Tensor
+    best_hit: torch.Tensor
+    best_chi2: torch.Tensor
+
+    @staticmethod
+    def from_numpy(par, cov21, q, chi2=None, nhits=None, device="cuda:0") -> "DeviceCandidates":
+        n = int(par.shape[1])
+        ld = padded_ld(n)
+        z = lambda dt: torch.zeros(ld, dtype=dt, device=device)
+        c = DeviceCandidates(n, ld, _to_planes(np.asarray(par, dtype=np.float32), ld, device),
+                             _to_planes(np.asarray(cov21, dtype=np.float32), ld, device),
+                             _to_planes(np.asarray(q, dtype=np.int8), ld, device),
+                             z(torch.float32), z(torch.int32), z(torch.int32), z(torch.int32), z(torch.float32))
+        if chi2 is not None:
+            c.chi2[:n] = torch.from_numpy(np.asarray(chi2, dtype=np.float32)).to(device)
+        if nhits is not None:
+            c.nhits[:n] = torch.from_numpy(np.asarray(nhits, dtype=np.int32)).to(device)
+        return c
+
+    def score(self, ctx: KFContext, geom: Geometry, layer: int, hits: DeviceLayer, window_half: int = 2,
+              chi2_cut: float = 30.0, do_update: bool = True):
+        ctx.score_candidates(geom, layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,
+                             hits.n_hits, hits.pos, hits.cov, hits.bins, window_half, chi2_cut, do_update,
+                             self.best_hit, self.best_chi2)
+
+    def results(self) -> dict:
+        n = self.n
+        return dict(par=self.par[:, :n].cpu().numpy(), cov=self.cov[:, :n].cpu().numpy(),
+                    chi2=self.chi2[:n].cpu().numpy(), nhits=self.nhits[:n].cpu().numpy(),
+                    status=self.status[:n].cpu().numpy().view(np.uint32),
+                    best_hit=self.best_hit[:n].cpu().numpy(), best_chi2=self.best_chi2[:n].cpu().numpy())

@@ -1,0 +1,169 @@
+"""GPU parity of kf_bin_hits (bit-exact) and kf_score_candidates (indices identical except inside the
+1e-4 relative chi2 tie window of north_star) against the oracle, through the C ABI."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import kf_oracle as O
+from tests.parity import compare_fit
+from workloads import barrel_events as W
+
+pytestmark = pytest.mark.gpu
+NE, NP = 40, 64
+EMAX = float(np.float32(1.2))        # both sides see the same fp32-rounded eta_max (reading A17)
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import paper_1705_02876_b200 as K
+    c = K.KFContext(0)
+    yield c
+    c.close()
+
+
+def _bin_both(ctx, pos, cov, radius, ne=NE, nph=NP, emax=EMAX):
+    from paper_1705_02876_b200.buffers import DeviceLayer
+    dl = DeviceLayer.from_numpy(pos, cov, ne, nph, emax, "cuda:0")
+    dl.bin(ctx, radius)
+    torch.cuda.synchronize()
+    return dl, O.bin_hits(pos, radius, ne, nph, emax)
+
+
+def _assert_bins_equal(dl, ob, pos, cov):
+    H = dl.n_hits
+    assert np.array_equal(dl.bins.bin_offset.cpu().numpy(), ob["bin_offset"])
+    s2o = dl.bins.sorted_to_orig.cpu().numpy()[:H]
+    assert np.array_equal(s2o, ob["sorted_to_orig"])
+    assert np.array_equal(dl.bins.pos_sorted.cpu().numpy()[:, :H], pos[:, s2o])
+    assert np.array_equal(dl.bins.cov_sorted.cpu().numpy()[:, :H], cov[:, s2o])
+
+
+@pytest.mark.parametrize("n_tracks,noise", [(400, 2000), (20000, 100000)])
+def test_bin_hits_bit_exact(ctx, n_tracks, noise):
+    ev = W.make_build_event(4, n_tracks=n_tracks, noise_hits=noise)
+    for l in (0, 4, 9):
+        lay = ev.layers[l]
+        dl, ob = _bin_both(ctx, lay.pos, lay.cov, lay.radius)
+        _assert_bins_equal(dl, ob, lay.pos, lay.cov)
+
+
+def test_bin_hits_edge_cases(ctx):
+    rng = np.random.default_rng(11)
+    r = 12.0
+    cov = np.tile(np.array([1e-2, 0, 0, 1e-2, 0, 1e-2], dtype=np.float32)[:, None], (1, 5000))
+    # empty layer
+    dl, ob = _bin_both(ctx, np.zeros((3, 0), np.float32), np.zeros((6, 0), np.float32), r)
+    assert np.all(dl.bins.bin_offset.cpu().numpy() == 0) and np.all(ob["bin_offset"] == 0)
+    # every hit in one bin (the ranking step degenerates to one long segment), 1 hit, ragged counts
+    for H in (1, 3, 5000):
+        pos = np.stack([np.full(H, r), np.full(H, 0.01), np.full(H, 0.3)]).astype(np.float32)
+        dl, ob = _bin_both(ctx, pos, cov[:, :H], r)
+        _assert_bins_equal(dl, ob, pos, cov[:, :H])
+    # hits exactly on bin edges and on the axes, out-of-range eta (clamped), phi = +-pi
+    phi = np.concatenate([-np.pi + np.arange(64) * (2 * np.pi / 64), [np.pi, -np.pi, 0.0]])
+    eta = np.concatenate([-1.2 + np.arange(41) * 0.06, [-5.0, 5.0]])
+    P, E = np.meshgrid(phi, eta)
+    pos = np.stack([r * np.cos(P.ravel()), r * np.sin(P.ravel()), r * np.sinh(E.ravel())]).astype(np.float32)
+    H = pos.shape[1]
+    c2 = np.tile(cov[:, :1], (1, H))
+    dl, ob = _bin_both(ctx, pos, c2, r)
+    _assert_bins_equal(dl, ob, pos, c2)
+    # other bin shapes, incl. the largest table
+    pos = np.stack([r * np.cos(rng.uniform(-np.pi, np.pi, 3000)), r * np.sin(rng.uniform(-np.pi, np.pi, 3000)),
+                    r * np.sinh(rng.uniform(-2.5, 2.5, 3000))]).astype(np.float32)
+    for ne, nph, emax in [(1, 2, 1.0), (7, 10, 2.0), (256, 256, 2.5)]:
+        dl, ob = _bin_both(ctx, pos, cov[:, :3000], r, ne, nph, float(np.float32(emax)))
+        _assert_bins_equal(dl, ob, pos, cov[:, :3000])
+
+
+def _seeds(ev):
+    f = ev.fit
+    r = O.fit_tracks(f.radius[:3], f.x_over_X0[:3], f.Bz, f.mass, f.par, f.cov, f.q, f.hpos[:3], f.hcov[:3], None)
+    return r["par"].astype(np.float32), O.pack_cov21(r["cov"]).astype(np.float32), r["chi2"], r["nhits"]
+
+
+def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
+    """Layers 3..9 on both sides; returns (decisions, differing decisions inside the tie window)."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    f, cfg = ev.fit, ev.cfg
+    par, cov, chi2, nh = _seeds(ev)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+    dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    oc = O.Candidates(par, cov, f.q, chi2, nh)
+    alive = np.ones(f.n, dtype=bool)         # candidates whose decisions agreed so far
+    n_dec = n_tie = 0
+    for l in range(cfg.first_scored_layer, cfg.n_layers):
+        lay = ev.layers[l]
+        dl = DeviceLayer.from_numpy(lay.pos, lay.cov, NE, NP, EMAX, "cuda:0")
+        dl.bin(ctx, lay.radius)
+        dc.score(ctx, geom, l, dl, 2, chi2_cut, do_update)
+        torch.cuda.synchronize()
+        ob = O.bin_hits(lay.pos, lay.radius, NE, NP, EMAX)
+        orr = O.score_layer(oc, lay.radius, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NE, NP, EMAX,
+                            2, chi2_cut, do_update)
+        g = dc.results()
+        diff = (g["best_hit"] != orr["best_hit"]) & alive
+        b, s2 = orr["best_chi2"], orr["second_chi2"]
+        # allowed: best and runner-up within 1e-4 relative, or the best within 1e-4 relative of the cut
+        tie = (np.abs(s2 - b) <= 1e-4 * np.abs(b)) | (np.abs(b - chi2_cut) <= 1e-4 * chi2_cut)
+        assert not np.any(diff & ~tie), f"layer {l}: {int((diff & ~tie).sum())} mismatches outside the tie window"
+        n_dec += int(alive.sum())
+        n_tie += int(diff.sum())
+        alive &= ~diff                       # such a candidate is not compared further
+        acc = alive & (orr["best_hit"] >= 0)
+        rel = np.abs(g["best_chi2"][acc] - b[acc]) / np.maximum(b[acc], 1.0)
+        assert rel.max(initial=0) < 2e-3, rel.max()
+        assert np.array_equal(g["status"][alive], oc.status[alive])
+        assert np.array_equal(g["nhits"][alive], oc.nhits[alive])
+    if check_state:
+        g = dc.results()
+        sel = alive & (oc.status == 0)
+        sub_g = {k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in ("par", "cov", "chi2", "nhits", "status")}
+        sub_o = dict(par=oc.par.T[:, sel], cov=oc.cov[sel], chi2=oc.chi2[sel], nhits=oc.nhits[sel], status=oc.status[sel])
+        res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=0.05)
+        print("scoring state parity:", res)
+    return n_dec, n_tie
+
+
+def test_score_small_event(ctx):
+    ev = W.make_build_event(4, n_tracks=400, noise_hits=2000)
+    n_dec, n_tie = _score_event(ctx, ev)
+    assert n_dec >= 0.99 * 7 * 400
+
+
+def test_score_full_config4(ctx):
+    """BASELINE.json configs[4]: 20 000 seeds, 120 000 hits per layer, 40x64 bins, +-2-bin window."""
+    ev = W.make_build_event(4)
+    n_dec, n_tie = _score_event(ctx, ev)
+    print(f"config 4: {n_dec} decisions, {n_tie} differences inside the tie window")
+    assert n_dec >= 0.99 * 7 * 20000 and n_tie <= 20
+
+
+def test_score_no_update_and_reject_all(ctx):
+    ev = W.make_build_event(4, n_tracks=400, noise_hits=2000)
+    _score_event(ctx, ev, do_update=False)
+    _score_event(ctx, ev, chi2_cut=0.0)
+
+
+def test_score_empty_window_and_errors(ctx):
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    ev = W.make_build_event(4, n_tracks=64, noise_hits=0)
+    f = ev.fit
+    par, cov, chi2, nh = _seeds(ev)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+    dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    empty = DeviceLayer.from_numpy(np.zeros((3, 0), np.float32), np.zeros((6, 0), np.float32), NE, NP, EMAX, "cuda:0")
+    empty.bin(ctx, float(f.radius[3]))
+    dc.score(ctx, geom, 3, empty)
+    torch.cuda.synchronize()
+    g = dc.results()
+    assert np.all(g["best_hit"] == -1) and np.all(np.isinf(g["best_chi2"])) and np.array_equal(g["nhits"], nh)
+    np.testing.assert_allclose(np.hypot(g["par"][0], g["par"][1]), f.radius[3], rtol=1e-5)   # propagated state kept
+    with pytest.raises(K.KFError) as e:
+        dc.score(ctx, geom, 10, empty)
+    assert e.value.code == -2
+    with pytest.raises(K.KFError) as e:
+        dc.score(ctx, geom, 4, empty, window_half=40)
+    assert e.value.code == -4

@@ -16,7 +16,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libkf_b200.so")
+_LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so")   # override: kernel experiments
 
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",

@@ -3,34 +3,82 @@
 // One thread owns one track for the whole layer loop ("one thread per track";
 // PAPER.md:129 merged kernels, registers over shared memory): the state, the 21 (then 15) unique
 // covariance elements and the Jacobian ingredients never leave registers.  Inputs and outputs
-// are element-major SoA (PAPER.md:65, 119 Matriplex), so a warp's access to one element of 32
-// consecutive tracks is one 128-byte line.  Per-layer hits (9 floats per track and layer, the
-// only per-layer HBM traffic) are prefetched one layer ahead into registers.
+// are element-major SoA (PAPER.md:65, 119 Matriplex), so the data of 32 consecutive tracks is a
+// [rows][32] tile of 128-byte lines.
+//
+// All bulk traffic goes through the TMA unit (cp.async.bulk.tensor, 2-D tensor maps over the
+// [planes][ld] arrays), one instruction per tile, issued by one lane:
+//   * per warp, a ring of kStages hit tiles [9][32] floats (3 position + 6 covariance planes of
+//     one layer -- the only per-layer HBM traffic) is kept kStages layers ahead of the math, each
+//     stage guarded by its own mbarrier (complete_tx byte counting);
+//   * the seed tile [27][32] is loaded the same way and its shared memory is reused to stage the
+//     fitted tracks, which leave through a TMA store (out-of-range columns are clipped by the
+//     tensor map, so ragged tails need no special case).
+// The math reads shared memory with conflict-free LDS at immediate offsets: no per-thread address
+// arithmetic, no registers held for prefetch.  Warps never synchronise with each other.
 //
 // Algorithmic HBM bytes per track: 113 in (6 + 21 floats, charge, mask) + 120 out (27 floats,
 // chi2, nhits, status) + 36 per layer = 593 B at 10 layers.
+#include <cuda.h>
+
 #include "kf_internal.h"
 
 namespace kf {
 
 namespace {
 
+#ifndef KF_FIT_MIN_BLOCKS
+#define KF_FIT_MIN_BLOCKS 5
+#endif
+#ifndef KF_FIT_STAGES
+#define KF_FIT_STAGES 4
+#endif
+
 constexpr int kFitBlock = 128;
+constexpr int kWarps = kFitBlock / 32;
+constexpr int kStages = KF_FIT_STAGES;           // layers in flight per warp
+constexpr int kHitFloats = 9 * 32;               // one hit tile
+constexpr int kSeedFloats = 27 * 32;             // seed / result tile
+constexpr int kWarpFloats = kStages * kHitFloats + kSeedFloats;
+constexpr int kSmemBytes = kWarps * kWarpFloats * 4 + kWarps * (kStages + 1) * 8;
+
+struct FitMaps {
+    CUtensorMap hpos, hcov, par, cov, opar, ocov;
+};
 
 struct Hit {
     float x, y, z, vxx, vxy, vxz, vyy, vyz, vzz;
 };
 
-__device__ __forceinline__ Hit load_hit(const float* __restrict__ hpos,
-                                        const float* __restrict__ hcov, int64_t ld, int l,
-                                        int64_t i) {
-    const float* p = hpos + (int64_t)l * 3 * ld + i;
-    const float* c = hcov + (int64_t)l * 6 * ld + i;
-    Hit h;
-    h.x = __ldg(p);           h.y = __ldg(p + ld);      h.z = __ldg(p + 2 * ld);
-    h.vxx = __ldg(c);         h.vxy = __ldg(c + ld);    h.vxz = __ldg(c + 2 * ld);
-    h.vyy = __ldg(c + 3 * ld); h.vyz = __ldg(c + 4 * ld); h.vzz = __ldg(c + 5 * ld);
-    return h;
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// 2-D TMA tile load global -> shared; completion (bytes) is signalled on an mbarrier.
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int col, int row, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(dst), "l"(map), "r"(col), "r"(row), "r"(bar) : "memory");
+}
+// 2-D TMA tile store shared -> global (bulk async group).
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int col, int row, uint32_t src) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(map), "r"(col), "r"(row), "r"(src) : "memory");
 }
 
 // One layer for one track.  Returns 0 or the status bit of the failure (track untouched).
@@ -49,62 +97,165 @@ __device__ __forceinline__ uint32_t fit_layer(Track& t, float k, float ik, const
     return rc;
 }
 
-__global__ void __launch_bounds__(kFitBlock, 4)
-fit_kernel(const __grid_constant__ FitParams P, const FitArgs a) {
-    const int64_t i = (int64_t)blockIdx.x * kFitBlock + threadIdx.x;
-    if (i >= a.n) return;
+// Seed / result tile [27][32] in shared memory <-> registers (p = &tile[0][lane]).
+__device__ __forceinline__ void track_from_tile(Track& t, const float* p) {
+    t.x = p[0];         t.y = p[32];        t.z = p[64];        t.px = p[96];       t.py = p[128];      t.pz = p[160];
+    t.c00 = p[192];     t.c01 = p[224];     t.c02 = p[256];     t.c03 = p[288];     t.c04 = p[320];     t.c05 = p[352];
+    t.c11 = p[384];     t.c12 = p[416];     t.c13 = p[448];     t.c14 = p[480];     t.c15 = p[512];
+    t.c22 = p[544];     t.c23 = p[576];     t.c24 = p[608];     t.c25 = p[640];
+    t.c33 = p[672];     t.c34 = p[704];     t.c35 = p[736];
+    t.c44 = p[768];     t.c45 = p[800];
+    t.c55 = p[832];
+    t.eax = 1.0f;
+    t.eay = 0.0f;
+}
+__device__ __forceinline__ void track_to_tile(const Track& t, float* p) {
+    p[0] = t.x;         p[32] = t.y;        p[64] = t.z;        p[96] = t.px;       p[128] = t.py;      p[160] = t.pz;
+    p[192] = t.c00;     p[224] = t.c01;     p[256] = t.c02;     p[288] = t.c03;     p[320] = t.c04;     p[352] = t.c05;
+    p[384] = t.c11;     p[416] = t.c12;     p[448] = t.c13;     p[480] = t.c14;     p[512] = t.c15;
+    p[544] = t.c22;     p[576] = t.c23;     p[608] = t.c24;     p[640] = t.c25;
+    p[672] = t.c33;     p[704] = t.c34;     p[736] = t.c35;
+    p[768] = t.c44;     p[800] = t.c45;
+    p[832] = t.c55;
+}
+
+__global__ void __launch_bounds__(kFitBlock, KF_FIT_MIN_BLOCKS)
+fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t i0 = (int64_t)blockIdx.x * kFitBlock + wid * 32;  // first track of this warp
+    if (i0 >= a.n) return;                                          // whole warp out of range
+    const int L = P.n_layers;
+    float* wbase = reinterpret_cast<float*>(smem_raw) + wid * kWarpFloats;
+    float* seed_tile = wbase + kStages * kHitFloats;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + kWarps * kWarpFloats * 4) + wid * (kStages + 1);
+    const uint32_t hit0 = smem_u32(wbase), seed0 = smem_u32(seed_tile), bar0 = smem_u32(bars);
+    const int col = (int)i0;
+
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s <= kStages; ++s) mbar_init(bar0 + 8u * s, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // seed tile first, then the first kStages layers of hits
+        mbar_expect_tx(bar0 + 8u * kStages, kSeedFloats * 4);
+        tma_load_2d(seed0, &M.par, col, 0, bar0 + 8u * kStages);
+        tma_load_2d(seed0 + 6 * 128, &M.cov, col, 0, bar0 + 8u * kStages);
+#pragma unroll
+        for (int s = 0; s < kStages; ++s)
+            if (s < L) {
+                mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
+                tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * s, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * s, bar0 + 8u * s);
+            }
+    }
+    __syncwarp();
+
+    const bool valid = lane < a.n - i0;
+    const int64_t i = valid ? i0 + lane : a.n - 1;  // idle lanes shadow the last track, store nothing
     const int q = a.q[i];
     const uint32_t mask = a.mask ? __ldg(a.mask + i) : 0xffffffffu;
+    const bool good_q = (q == 1) | (q == -1);
+    const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
     Track t;
-    load_track(t, a.par, a.cov, a.ld_in, i);
+    mbar_wait(bar0 + 8u * kStages, 0u);
+    track_from_tile(t, seed_tile + lane);
+    if (good_q) enter_local_frame(t);
     float chi2 = 0.0f;
     int nh = 0;
     uint32_t st = 0u;
-    if (q != 1 && q != -1) {
-        st = ST_BAD_CHARGE;  // copied through untouched
-    } else {
-        const int L = P.n_layers;
-        const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
-        enter_local_frame(t);
-        Hit next = load_hit(a.hpos, a.hcov, a.ld_hit, 0, i);
-        int l = 0;
-        // until the first successful layer the covariance is a general 6x6 ...
-        bool started = false;
-        for (; l < L && !started; ++l) {
-            const Hit cur = next;
-            if (l + 1 < L) next = load_hit(a.hpos, a.hcov, a.ld_hit, l + 1, i);
-            if (!((mask >> l) & 1u)) continue;
-            const uint32_t rc = fit_layer<false>(t, k, ik, P.layer[l], P.mass2, cur, chi2);
+    bool started = false;  // false: general 6x6 covariance; true: its radial row is identically zero
+    for (int l = 0; l < L; ++l) {
+        const int s = l % kStages;
+        mbar_wait(bar0 + 8u * s, (uint32_t)(l / kStages) & 1u);
+        const float* tp = wbase + s * kHitFloats + lane;
+        Hit m;
+        m.x = tp[0];         m.y = tp[32];        m.z = tp[64];
+        m.vxx = tp[96];      m.vxy = tp[128];     m.vxz = tp[160];
+        m.vyy = tp[192];     m.vyz = tp[224];     m.vzz = tp[256];
+        __syncwarp();        // every lane has its hit in registers: the stage may be refilled
+        if (lane == 0 && l + kStages < L) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
+            tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * (l + kStages), bar0 + 8u * s);
+            tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * (l + kStages), bar0 + 8u * s);
+        }
+        if (good_q && ((mask >> l) & 1u)) {
+            uint32_t rc;
+            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.mass2, m, chi2);
+            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.mass2, m, chi2);
             st |= rc;
             if (rc == 0u) { nh += 1; started = true; }
         }
-        // ... afterwards its radial row is identically zero
-        for (; l < L; ++l) {
-            const Hit cur = next;
-            if (l + 1 < L) next = load_hit(a.hpos, a.hcov, a.ld_hit, l + 1, i);
-            if (!((mask >> l) & 1u)) continue;
-            const uint32_t rc = fit_layer<true>(t, k, ik, P.layer[l], P.mass2, cur, chi2);
-            st |= rc;
-            nh += (rc == 0u);
-        }
-        if (nh > 0) leave_local_frame(t);
-        else load_track(t, a.par, a.cov, a.ld_in, i);  // nothing fitted: hand the seed back bit-exact
     }
-    store_track(t, a.opar, a.ocov, a.ld_out, i);
-    a.chi2[i] = chi2;
-    a.nhits[i] = nh;
-    a.status[i] = st;
+    if (!good_q) st = ST_BAD_CHARGE;
+    if (good_q && nh > 0) {
+        leave_local_frame(t);
+        track_to_tile(t, seed_tile + lane);
+    }   // else: bad charge or nothing fitted -- the seed tile still holds the input, bit-exact
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncwarp();
+    if (lane == 0) {
+        tma_store_2d(&M.opar, col, 0, seed0);
+        tma_store_2d(&M.ocov, col, 0, seed0 + 6 * 128);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    if (valid) {
+        a.chi2[i] = chi2;
+        a.nhits[i] = nh;
+        a.status[i] = st;
+    }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // smem must outlive the store
+}
+
+}  // namespace
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+
+// Tensor map over a [rows][ld] float array of which n columns are valid; tiles are [box_rows][32].
+bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t rows, int box_rows) {
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
+    const cuuint32_t box[2] = {32u, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1u, 1u};
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 }  // namespace
 
 cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream) {
     if (a.n == 0) return cudaSuccess;
+    static const cudaError_t attr = cudaFuncSetAttribute(fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (attr != cudaSuccess) return attr;
+    const int L = P.n_layers;
+    FitMaps M;
+    if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3) ||
+        !make_map(&M.hcov, a.hcov, a.n, a.ld_hit, (int64_t)L * 6, 6) ||
+        !make_map(&M.par, a.par, a.n, a.ld_in, 6, 6) || !make_map(&M.cov, a.cov, a.n, a.ld_in, 21, 21) ||
+        !make_map(&M.opar, a.opar, a.n, a.ld_out, 6, 6) || !make_map(&M.ocov, a.ocov, a.n, a.ld_out, 21, 21))
+        return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
-    fit_kernel<<<(unsigned)blocks, kFitBlock, 0, stream>>>(P, a);
+    fit_kernel<<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     return cudaGetLastError();
 }
-
-int fit_kernel_count() { return 1; }
 
 }  // namespace kf

@@ -54,7 +54,14 @@ struct FitParams {
     LayerConst layer[32];
 };
 
-__device__ __forceinline__ float rcp_fast(float x) { return __fdividef(1.0f, x); }
+// MUFU-based reciprocal / reciprocal square root (about 1 ulp / 2 ulp), no slow path.
+#if defined(__CUDA_ARCH__)
+__device__ __forceinline__ float rcp_fast(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_fast(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+#else
+__device__ __forceinline__ float rcp_fast(float x) { return 1.0f / x; }
+__device__ __forceinline__ float rsqrt_fast(float x) { return rsqrtf(x); }
+#endif
 
 // Track in registers.  Position frame unit vector (eax, eay): position-block coordinates
 // (a1, a2) mean  dw = (eax + i eay)(a1 + i a2).  The momentum frame always follows the current
@@ -157,16 +164,15 @@ __device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float i
     const float x = t.x, y = t.y, px = t.px, py = t.py;
     const float pt2 = px * px + py * py;
     const float rho2 = x * x + y * y;
-    if (!(L.r2 > rho2)) return false;
     const float a = x * px + y * py;
     const float b = (y * px - x * py) - pt2 * ik;
     const float D = 0.5f * k * (L.r2 - rho2);
     const float disc = a * a - D * (2.0f * b + D);
-    if (!(disc > 0.0f)) return false;
-    const float den = a + sqrtf(disc);
-    if (!(den > 0.0f)) return false;
-    const float tt = D / den;
-    const float i1 = 1.0f / (1.0f + tt * tt);
+    const float den = a + disc * rsqrt_fast(disc);  // NaN unless disc > 0
+    // one test for the three PROP_FAIL conditions (r <= rho, disc <= 0, den <= 0; NaNs fail too)
+    if (!((L.r2 > rho2) & (disc > 0.0f) & (den > 0.0f))) return false;
+    const float tt = D * rcp_fast(den);
+    const float i1 = rcp_fast(1.0f + tt * tt);
     const float S = 2.0f * tt * i1;
     const float Cm = tt * S;
     const float co = 1.0f - Cm;
@@ -177,7 +183,7 @@ __device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float i
     o.zn = t.z + t.pz * o.thk;
     o.pxn = px * co + py * S;
     o.pyn = py * co - px * S;
-    const float ipt = rsqrtf(pt2);
+    const float ipt = rsqrt_fast(pt2);
     o.pt2 = pt2;
     o.ipt = ipt;
     o.erx = o.xn * L.inv_r;
@@ -187,7 +193,7 @@ __device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float i
     // exp(i a') = conj(e_r') e_l'
     const float ca = o.erx * o.elx + o.ery * o.ely;
     const float sa = o.erx * o.ely - o.ery * o.elx;
-    const float ic = 1.0f / ca;
+    const float ic = rcp_fast(ca);
     const float T = sa * ic;
     // P = conj(e_r') e_a
     const float pc = o.erx * t.eax + o.ery * t.eay;
@@ -264,7 +270,7 @@ __device__ __forceinline__ void transport_cov(const Track& t, const Crossing& o,
     // sheared to (b1, b2, c):  Q~ = theta0^2 [[pz^2, 0, -pz p^2/pT], [0, p^2, 0], [., 0, p^4/pT^2]]
     const float pz = t.pz;
     const float p2 = o.pt2 + pz * pz;
-    const float ip2 = 1.0f / p2;
+    const float ip2 = rcp_fast(p2);
     const float th2 = ms * (p2 + mass2) * ip2 * ip2;
     const float qc = th2 * p2 * o.ipt;  // theta0^2 p^2 / pT
     n.n33 = t.c33 + th2 * pz * pz;
@@ -332,30 +338,42 @@ __device__ __forceinline__ float chi2_of(const Sym3& si, const LocalHit& h) {
 // increment through *dchi2.  Returns a status bit on failure (track untouched).
 __device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, const PropCov& n,
                                                   const LocalHit& h, float* dchi2) {
-    Sym3 si;
-    const float det = invert_S(n, h, si);
-    if (!(det > 0.0f)) return ST_S_NOT_PD;
-    const float chi2 = chi2_of(si, h);
-    // K = C'[:, (t,z)] Si[(t,z), :]   (rows t z l n p; columns r t z)
-#define KF_KROW(ct, cz, kr, kt, kz)                     \
-    const float kr = ct * si.rt + cz * si.rz;           \
-    const float kt = ct * si.tt + cz * si.tz;           \
-    const float kz = ct * si.tz + cz * si.zz;
-    KF_KROW(n.n11, n.n12, k1r, k1t, k1z)
-    KF_KROW(n.n12, n.n22, k2r, k2t, k2z)
-    KF_KROW(n.n13, n.n23, k3r, k3t, k3z)
-    KF_KROW(n.n14, n.n24, k4r, k4t, k4z)
-    KF_KROW(n.n15, n.n25, k5r, k5t, k5z)
-#undef KF_KROW
-    const float d1 = k1r * h.rr + k1t * h.rt + k1z * h.rz;
-    const float d2 = k2r * h.rr + k2t * h.rt + k2z * h.rz;
-    const float d3 = k3r * h.rr + k3t * h.rt + k3z * h.rz;
-    const float d4 = k4r * h.rr + k4t * h.rt + k4z * h.rz;
-    const float d5 = k5r * h.rr + k5t * h.rt + k5z * h.rz;
+    // The radial row of C' is zero, so eliminating the radial component of S = C'_pp + V~ first
+    // (Schur complement on v_rr) leaves a 2-D measurement in (t, z):
+    //   V' = V_tz,tz - s s^T / v_rr,  s = (v_rt, v_rz);   r' = r_tz - s r_r / v_rr;
+    //   S' = C'_tz,tz + V';  chi2 = r_r^2 / v_rr + r'^T S'^-1 r';  K = C'[:, tz] S'^-1;
+    //   det S = v_rr det S'.
+    const float iv = rcp_fast(h.vrr);
+    const float sa = h.vrt * iv, sb = h.vrz * iv;
+    const float qtt = h.vtt - sa * h.vrt, qtz = h.vtz - sa * h.vrz, qzz = h.vzz - sb * h.vrz;
+    const float stt = n.n11 + qtt, stz = n.n12 + qtz, szz = n.n22 + qzz;
+    const float rt = h.rt - sa * h.rr, rz = h.rz - sb * h.rr;
+    const float det2 = stt * szz - stz * stz;
+    if (!(h.vrr * det2 > 0.0f)) return ST_S_NOT_PD;
+    const float id = rcp_fast(det2);
+    const float itt = szz * id, itz = -stz * id, izz = stt * id;
+    const float ut = itt * rt + itz * rz, uz = itz * rt + izz * rz;
+    const float chi2 = h.rr * h.rr * iv + rt * ut + rz * uz;
+    // state increments d = C'[:, tz] S'^-1 r'
+    const float d1 = n.n11 * ut + n.n12 * uz;
+    const float d2 = n.n12 * ut + n.n22 * uz;
+    const float d3 = n.n13 * ut + n.n23 * uz;
+    const float d4 = n.n14 * ut + n.n24 * uz;
+    const float d5 = n.n15 * ut + n.n25 * uz;
     // finite(chi2) and finite(state): any non-finite term makes this sum non-finite
     const float probe = chi2 + ((d1 + d2) + (d3 + d4) + d5) * 0.0f;
     if (!(fabsf(probe) < __int_as_float(0x7f800000))) return ST_NONFINITE;
     *dchi2 = chi2;
+    // gain rows (t z b1 b2 c) x columns (t, z)
+#define KF_KROW(ct, cz, kt, kz)                \
+    const float kt = ct * itt + cz * itz;      \
+    const float kz = ct * itz + cz * izz;
+    KF_KROW(n.n11, n.n12, k1t, k1z)
+    KF_KROW(n.n12, n.n22, k2t, k2z)
+    KF_KROW(n.n13, n.n23, k3t, k3z)
+    KF_KROW(n.n14, n.n24, k4t, k4z)
+    KF_KROW(n.n15, n.n25, k5t, k5z)
+#undef KF_KROW
     // state
     t.x = o.xn - o.ery * d1;
     t.y = o.yn + o.erx * d1;
@@ -368,17 +386,17 @@ __device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, c
     t.pz = pzu;
     t.eax = o.erx;
     t.eay = o.ery;
-    // position rows: C[i][a] = sum_b K[i][b] V~[b][a], a in (t, z); radial row/column stay zero
+    // position rows ("V form", no subtraction): C[i][a] = sum_b K[i][b] V'[b][a]; radial row stays 0
     t.c00 = 0.0f; t.c01 = 0.0f; t.c02 = 0.0f; t.c03 = 0.0f; t.c04 = 0.0f; t.c05 = 0.0f;
-    t.c11 = k1r * h.vrt + k1t * h.vtt + k1z * h.vtz;
-    t.c12 = k1r * h.vrz + k1t * h.vtz + k1z * h.vzz;
-    t.c22 = k2r * h.vrz + k2t * h.vtz + k2z * h.vzz;
-    t.c13 = k3r * h.vrt + k3t * h.vtt + k3z * h.vtz;
-    t.c23 = k3r * h.vrz + k3t * h.vtz + k3z * h.vzz;
-    t.c14 = k4r * h.vrt + k4t * h.vtt + k4z * h.vtz;
-    t.c24 = k4r * h.vrz + k4t * h.vtz + k4z * h.vzz;
-    t.c15 = k5r * h.vrt + k5t * h.vtt + k5z * h.vtz;
-    t.c25 = k5r * h.vrz + k5t * h.vtz + k5z * h.vzz;
+    t.c11 = k1t * qtt + k1z * qtz;
+    t.c12 = k1t * qtz + k1z * qzz;
+    t.c22 = k2t * qtz + k2z * qzz;
+    t.c13 = k3t * qtt + k3z * qtz;
+    t.c23 = k3t * qtz + k3z * qzz;
+    t.c14 = k4t * qtt + k4z * qtz;
+    t.c24 = k4t * qtz + k4z * qzz;
+    t.c15 = k5t * qtt + k5z * qtz;
+    t.c25 = k5t * qtz + k5z * qzz;
     // momentum block: C'_mm - K_m C'_pm  (C'_pm rows t, z)
     t.c33 = n.n33 - (k3t * n.n13 + k3z * n.n23);
     t.c34 = n.n34 - (k3t * n.n14 + k3z * n.n24);
@@ -389,7 +407,7 @@ __device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, c
     // re-aim the momentum frame: exp(i d) = conj(e_l,new) e_l' = ((pT + d3) - i d4) / pT,new
     const float pt = o.pt2 * o.ipt;
     const float ar = pt + d3;
-    const float iptn = rsqrtf(ar * ar + d4 * d4);
+    const float iptn = rsqrt_fast(ar * ar + d4 * d4);
     reaim_momentum(t, ar * iptn, -d4 * iptn, o.T, pzu * iptn);
     return 0u;
 }

@@ -31,9 +31,13 @@ def diverged_mask(oracle: dict) -> np.ndarray:
     return (oracle["status"] != 0) | (oracle["chi2"] > ndf + 9.0 * np.sqrt(2.0 * ndf))
 
 
-def compare_fit(gpu: dict, oracle: dict, r_last: float | np.ndarray, max_diverged_frac: float = 1e-3) -> dict:
+def compare_fit(gpu: dict, oracle: dict, r_last: float | np.ndarray, max_diverged_frac: float = 1e-3,
+                loosen: dict | None = None) -> dict:
     """gpu: par[6][n] f32, cov[21][n] f32, chi2[n], nhits[n], status[n]; oracle: O.fit_tracks dict.
-    Returns the worst normalised errors (each must be <= 1 to pass) and raises AssertionError on failure."""
+    Returns the worst normalised errors (each must be <= 1 to pass) and raises AssertionError on failure.
+    `loosen` multiplies a tolerance for callers whose contract is weaker than the fit's (the per-layer
+    scoring call stores the covariance in the global frame in fp32 between layers)."""
+    loosen = loosen or {}
     n = oracle["par"].shape[1]
     bad = diverged_mask(oracle)
     ok = ~bad
@@ -65,5 +69,5 @@ def compare_fit(gpu: dict, oracle: dict, r_last: float | np.ndarray, max_diverge
     assert np.array_equal(np.asarray(gpu["nhits"])[:n][ok], oracle["nhits"][ok]), "nhits differ"
     assert np.array_equal(np.asarray(gpu["status"])[:n][ok], oracle["status"][ok]), "status differ"
     for key in ("pos", "mom", "cov", "chi2"):
-        assert res[key] <= 1.0, f"{key} parity failed: {res}"
+        assert res[key] <= loosen.get(key, 1.0), f"{key} parity failed: {res}"
     return res

@@ -70,6 +70,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// One lane of the (converged) warp; the compiler keeps the guarded code on the uniform datapath.
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred P;\n"
+        "elect.sync _|P, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, P;\n"
+        "}\n" : "=r"(pred));
+    return pred != 0;
+}
 // 2-D TMA tile load global -> shared; completion (bytes) is signalled on an mbarrier.
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int col, int row, uint32_t bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
@@ -122,7 +133,8 @@ __device__ __forceinline__ void track_to_tile(const Track& t, float* p) {
 __global__ void __launch_bounds__(kFitBlock, KF_FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int wid = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform by construction
     const int64_t i0 = (int64_t)blockIdx.x * kFitBlock + wid * 32;  // first track of this warp
     if (i0 >= a.n) return;                                          // whole warp out of range
     const int L = P.n_layers;
@@ -132,7 +144,7 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
     const uint32_t hit0 = smem_u32(wbase), seed0 = smem_u32(seed_tile), bar0 = smem_u32(bars);
     const int col = (int)i0;
 
-    if (lane == 0) {
+    if (elect_one()) {
 #pragma unroll
         for (int s = 0; s <= kStages; ++s) mbar_init(bar0 + 8u * s, 1u);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -173,7 +185,7 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         m.vxx = tp[96];      m.vxy = tp[128];     m.vxz = tp[160];
         m.vyy = tp[192];     m.vyz = tp[224];     m.vzz = tp[256];
         __syncwarp();        // every lane has its hit in registers: the stage may be refilled
-        if (lane == 0 && l + kStages < L) {
+        if (l + kStages < L && elect_one()) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
             tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * (l + kStages), bar0 + 8u * s);
@@ -194,7 +206,8 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
     }   // else: bad charge or nothing fitted -- the seed tile still holds the input, bit-exact
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncwarp();
-    if (lane == 0) {
+    const bool storer = elect_one();
+    if (storer) {
         tma_store_2d(&M.opar, col, 0, seed0);
         tma_store_2d(&M.ocov, col, 0, seed0 + 6 * 128);
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
@@ -204,7 +217,7 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         a.nhits[i] = nh;
         a.status[i] = st;
     }
-    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // smem must outlive the store
+    if (storer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // smem must outlive the store
 }
 
 }  // namespace

@@ -80,10 +80,11 @@ struct Track {
 
 // Change the momentum frame of the covariance: rotate (b1, b2) -> (dc + i ds)(b1 + i b2), then
 // shear c -> c + k1 b1 + k2 b2 (new b's), k1 = T_old dc - T_new, k2 = T_old ds, T = pz/pT.
+template <bool RADIAL_NULL = false>
 __device__ __forceinline__ void reaim_momentum(Track& t, float dc, float ds, float T_old,
                                                float T_new) {
     float a, b;
-    a = t.c03; b = t.c04; t.c03 = dc * a - ds * b; t.c04 = ds * a + dc * b;
+    if constexpr (!RADIAL_NULL) { a = t.c03; b = t.c04; t.c03 = dc * a - ds * b; t.c04 = ds * a + dc * b; }
     a = t.c13; b = t.c14; t.c13 = dc * a - ds * b; t.c14 = ds * a + dc * b;
     a = t.c23; b = t.c24; t.c23 = dc * a - ds * b; t.c24 = ds * a + dc * b;
     a = t.c35; b = t.c45;
@@ -94,9 +95,9 @@ __device__ __forceinline__ void reaim_momentum(Track& t, float dc, float ds, flo
     t.c44 = ss * ll + 2.0f * cs * ln + cc * nn;
     t.c34 = cs * (ll - nn) + (cc - ss) * ln;
     const float k1 = T_old * dc - T_new, k2 = T_old * ds;
-    t.c05 += k1 * t.c03 + k2 * t.c04;
-    t.c15 += k1 * t.c13 + k2 * t.c14;
-    t.c25 += k1 * t.c23 + k2 * t.c24;
+    if constexpr (!RADIAL_NULL) t.c05 = fmaf(k2, t.c04, fmaf(k1, t.c03, t.c05));
+    t.c15 = fmaf(k2, t.c14, fmaf(k1, t.c13, t.c15));
+    t.c25 = fmaf(k2, t.c24, fmaf(k1, t.c23, t.c25));
     const float n35 = c35 + k1 * t.c33 + k2 * t.c34;
     const float n45 = c45 + k1 * t.c34 + k2 * t.c44;
     t.c55 += k1 * (c35 + n35) + k2 * (c45 + n45);
@@ -231,38 +232,53 @@ struct PropCov {
 template <bool RADIAL_NULL>
 __device__ __forceinline__ void transport_cov(const Track& t, const Crossing& o, float ms,
                                               float mass2, PropCov& n) {
-    const float c00 = RADIAL_NULL ? 0.0f : t.c00, c01 = RADIAL_NULL ? 0.0f : t.c01;
-    const float c02 = RADIAL_NULL ? 0.0f : t.c02, c03 = RADIAL_NULL ? 0.0f : t.c03;
-    const float c04 = RADIAL_NULL ? 0.0f : t.c04, c05 = RADIAL_NULL ? 0.0f : t.c05;
     const float g0 = o.g0, g1 = o.g1, g3 = o.g3, g4 = o.g4;
     const float t0 = o.t0, t1 = o.t1, t3 = o.t3, t4 = o.t4;
     const float z0 = o.z0, z1 = o.z1, z3 = o.z3, z4 = o.z4, thk = o.thk, mu = o.mu;
-    // v = C g, w = C tau, u = C zeta
-    const float v0 = c00 * g0 + c01 * g1 + c03 * g3 + c04 * g4;
-    const float v1 = c01 * g0 + t.c11 * g1 + t.c13 * g3 + t.c14 * g4;
-    const float v3 = c03 * g0 + t.c13 * g1 + t.c33 * g3 + t.c34 * g4;
-    const float v4 = c04 * g0 + t.c14 * g1 + t.c34 * g3 + t.c44 * g4;
-    const float v5 = c05 * g0 + t.c15 * g1 + t.c35 * g3 + t.c45 * g4;
-    const float w0 = c00 * t0 + c01 * t1 + c03 * t3 + c04 * t4;
-    const float w1 = c01 * t0 + t.c11 * t1 + t.c13 * t3 + t.c14 * t4;
-    const float w3 = c03 * t0 + t.c13 * t1 + t.c33 * t3 + t.c34 * t4;
-    const float w4 = c04 * t0 + t.c14 * t1 + t.c34 * t3 + t.c44 * t4;
-    const float w5 = c05 * t0 + t.c15 * t1 + t.c35 * t3 + t.c45 * t4;
-    const float u0 = c00 * z0 + c01 * z1 + c02 + c03 * z3 + c04 * z4 + c05 * thk;
-    const float u1 = c01 * z0 + t.c11 * z1 + t.c12 + t.c13 * z3 + t.c14 * z4 + t.c15 * thk;
-    const float u2 = c02 * z0 + t.c12 * z1 + t.c22 + t.c23 * z3 + t.c24 * z4 + t.c25 * thk;
-    const float u3 = c03 * z0 + t.c13 * z1 + t.c23 + t.c33 * z3 + t.c34 * z4 + t.c35 * thk;
-    const float u4 = c04 * z0 + t.c14 * z1 + t.c24 + t.c34 * z3 + t.c44 * z4 + t.c45 * thk;
-    const float u5 = c05 * z0 + t.c15 * z1 + t.c25 + t.c35 * z3 + t.c45 * z4 + t.c55 * thk;
-    const float gCg = g0 * v0 + g1 * v1 + g3 * v3 + g4 * v4;
-    const float tCg = t0 * v0 + t1 * v1 + t3 * v3 + t4 * v4;
-    const float zCg = g0 * u0 + g1 * u1 + g3 * u3 + g4 * u4;
-    n.n11 = t0 * w0 + t1 * w1 + t3 * w3 + t4 * w4;
-    n.n12 = t0 * u0 + t1 * u1 + t3 * u3 + t4 * u4;
+    // v = C g, w = C tau, u = C zeta   (rows 1..5; row 0 and the a1 column only before the first layer)
+    float v1 = t.c11 * g1 + t.c13 * g3 + t.c14 * g4;
+    float v3 = t.c13 * g1 + t.c33 * g3 + t.c34 * g4;
+    float v4 = t.c14 * g1 + t.c34 * g3 + t.c44 * g4;
+    float v5 = t.c15 * g1 + t.c35 * g3 + t.c45 * g4;
+    float w1 = t.c11 * t1 + t.c13 * t3 + t.c14 * t4;
+    float w3 = t.c13 * t1 + t.c33 * t3 + t.c34 * t4;
+    float w4 = t.c14 * t1 + t.c34 * t3 + t.c44 * t4;
+    float w5 = t.c15 * t1 + t.c35 * t3 + t.c45 * t4;
+    float u1 = t.c12 + t.c11 * z1 + t.c13 * z3 + t.c14 * z4 + t.c15 * thk;
+    float u2 = t.c22 + t.c12 * z1 + t.c23 * z3 + t.c24 * z4 + t.c25 * thk;
+    float u3 = t.c23 + t.c13 * z1 + t.c33 * z3 + t.c34 * z4 + t.c35 * thk;
+    float u4 = t.c24 + t.c14 * z1 + t.c34 * z3 + t.c44 * z4 + t.c45 * thk;
+    float u5 = t.c25 + t.c15 * z1 + t.c35 * z3 + t.c45 * z4 + t.c55 * thk;
+    float gCg = g1 * v1 + g3 * v3 + g4 * v4;
+    float tCg = t1 * v1 + t3 * v3 + t4 * v4;
+    float zCg = g1 * u1 + g3 * u3 + g4 * u4;
+    float n11 = t1 * w1 + t3 * w3 + t4 * w4;
+    float n12 = t1 * u1 + t3 * u3 + t4 * u4;
+    float n22 = u2 + z1 * u1 + z3 * u3 + z4 * u4 + thk * u5;
+    if constexpr (!RADIAL_NULL) {
+        const float v0 = t.c00 * g0 + t.c01 * g1 + t.c03 * g3 + t.c04 * g4;
+        const float w0 = t.c00 * t0 + t.c01 * t1 + t.c03 * t3 + t.c04 * t4;
+        const float u0 = t.c02 + t.c00 * z0 + t.c01 * z1 + t.c03 * z3 + t.c04 * z4 + t.c05 * thk;
+        // a1-column contributions to rows 1..5 (added before the dot products use them)
+        const float dv1 = t.c01 * g0, dv3 = t.c03 * g0, dv4 = t.c04 * g0, dv5 = t.c05 * g0;
+        const float dw1 = t.c01 * t0, dw3 = t.c03 * t0, dw4 = t.c04 * t0, dw5 = t.c05 * t0;
+        const float du1 = t.c01 * z0, du2 = t.c02 * z0, du3 = t.c03 * z0, du4 = t.c04 * z0, du5 = t.c05 * z0;
+        gCg += g0 * v0 + g1 * dv1 + g3 * dv3 + g4 * dv4;
+        tCg += t0 * v0 + t1 * dv1 + t3 * dv3 + t4 * dv4;
+        zCg += g0 * u0 + g1 * du1 + g3 * du3 + g4 * du4;
+        n11 += t0 * w0 + t1 * dw1 + t3 * dw3 + t4 * dw4;
+        n12 += t0 * u0 + t1 * du1 + t3 * du3 + t4 * du4;
+        n22 += z0 * u0 + z1 * du1 + du2 + z3 * du3 + z4 * du4 + thk * du5;
+        v1 += dv1; v3 += dv3; v4 += dv4; v5 += dv5;
+        w1 += dw1; w3 += dw3; w4 += dw4; w5 += dw5;
+        u1 += du1; u2 += du2; u3 += du3; u4 += du4; u5 += du5;
+    }
+    n.n11 = n11;
+    n.n12 = n12;
     n.n13 = w3;
     n.n14 = w4 + mu * tCg;
     n.n15 = w5;
-    n.n22 = z0 * u0 + z1 * u1 + u2 + z3 * u3 + z4 * u4 + thk * u5;
+    n.n22 = n22;
     n.n23 = u3;
     n.n24 = u4 + mu * zCg;
     n.n25 = u5;
@@ -398,17 +414,17 @@ __device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, c
     t.c15 = k5t * qtt + k5z * qtz;
     t.c25 = k5t * qtz + k5z * qzz;
     // momentum block: C'_mm - K_m C'_pm  (C'_pm rows t, z)
-    t.c33 = n.n33 - (k3t * n.n13 + k3z * n.n23);
-    t.c34 = n.n34 - (k3t * n.n14 + k3z * n.n24);
-    t.c35 = n.n35 - (k3t * n.n15 + k3z * n.n25);
-    t.c44 = n.n44 - (k4t * n.n14 + k4z * n.n24);
-    t.c45 = n.n45 - (k4t * n.n15 + k4z * n.n25);
-    t.c55 = n.n55 - (k5t * n.n15 + k5z * n.n25);
+    t.c33 = fmaf(-k3z, n.n23, fmaf(-k3t, n.n13, n.n33));
+    t.c34 = fmaf(-k3z, n.n24, fmaf(-k3t, n.n14, n.n34));
+    t.c35 = fmaf(-k3z, n.n25, fmaf(-k3t, n.n15, n.n35));
+    t.c44 = fmaf(-k4z, n.n24, fmaf(-k4t, n.n14, n.n44));
+    t.c45 = fmaf(-k4z, n.n25, fmaf(-k4t, n.n15, n.n45));
+    t.c55 = fmaf(-k5z, n.n25, fmaf(-k5t, n.n15, n.n55));
     // re-aim the momentum frame: exp(i d) = conj(e_l,new) e_l' = ((pT + d3) - i d4) / pT,new
     const float pt = o.pt2 * o.ipt;
     const float ar = pt + d3;
     const float iptn = rsqrt_fast(ar * ar + d4 * d4);
-    reaim_momentum(t, ar * iptn, -d4 * iptn, o.T, pzu * iptn);
+    reaim_momentum<true>(t, ar * iptn, -d4 * iptn, o.T, pzu * iptn);
     return 0u;
 }
 

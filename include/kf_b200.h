@@ -92,6 +92,10 @@ KF_API int kf_reserve(kf_ctx* ctx, int64_t max_hits, int64_t max_host_tracks, in
 KF_API const char* kf_strerror(int code);
 /* cudaError_t of the last KF_ERR_CUDA on this context (0 if none). */
 KF_API int kf_last_cuda_error(const kf_ctx* ctx);
+/* Measurement utility (not on the hot path): sustained FP32 FMA throughput of the device in TFLOP/s
+ * from a register-only FMA microbenchmark (8 independent chains per thread, 2048 threads per SM, best
+ * of `repeats` launches).  Synchronises the stream.  This is the denominator of the ALU roofline. */
+KF_API int kf_measure_fp32_peak(kf_ctx* ctx, int repeats, double* tflops_out);
 /* ABI version, bumped when a struct or signature changes. */
 KF_API int kf_abi_version(void);
 

@@ -20,7 +20,7 @@ _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so"
 
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_fit_tracks", "kf_fit_tracks_host", "kf_bin_hits", "kf_score_candidates"]
+           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_host", "kf_bin_hits", "kf_score_candidates"]
 
 
 class KFError(RuntimeError):
@@ -84,6 +84,8 @@ def load_library():
     lib.kf_strerror.argtypes = [C.c_int]
     lib.kf_last_cuda_error.restype = C.c_int
     lib.kf_last_cuda_error.argtypes = [vp]
+    lib.kf_measure_fp32_peak.restype = C.c_int
+    lib.kf_measure_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     lib.kf_abi_version.restype = C.c_int
     lib.kf_abi_version.argtypes = []
     for name in ("kf_fit_tracks", "kf_fit_tracks_host"):
@@ -199,6 +201,12 @@ class KFContext:
 
     def reserve(self, max_hits: int = 0, max_host_tracks: int = 0, max_host_layers: int = 0):
         self._check(self._lib.kf_reserve(self._h, max_hits, max_host_tracks, max_host_layers), "kf_reserve")
+
+    def measure_fp32_peak(self, repeats: int = 5) -> float:
+        """TFLOP/s of the register-only FMA microbenchmark (ALU roofline denominator)."""
+        out = C.c_double(0.0)
+        self._check(self._lib.kf_measure_fp32_peak(self._h, int(repeats), C.byref(out)), "kf_measure_fp32_peak")
+        return float(out.value)
 
     # ------------------------------------------------------------------ marshalling helpers
     @staticmethod

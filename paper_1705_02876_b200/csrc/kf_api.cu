@@ -157,6 +157,20 @@ int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_hos
     return KF_OK;
 }
 
+int kf_measure_fp32_peak(kf_ctx* c, int repeats, double* tflops_out) {
+    if (!c || !tflops_out) return KF_ERR_NULL;
+    if (repeats < 1) return KF_ERR_SHAPE;
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    float* sink = nullptr;
+    if ((e = cudaMalloc(&sink, 16)) != cudaSuccess) return cuda_fail(c, e);
+    const double t = measure_fp32_peak(c->stream, repeats, sink);
+    cudaFree(sink);
+    if (t < 0.0) return cuda_fail(c, (cudaError_t)(int)(-t));
+    *tflops_out = t;
+    return KF_OK;
+}
+
 int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
                   const kf_track_hits* hits, kf_tracks* out) {
     if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;
@@ -168,6 +182,7 @@ int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
     if (out->n != seeds->n) return KF_ERR_SHAPE;
     if ((rc = check_track_hits(hits, geom, seeds->n, true))) return rc;
     if (seeds->n == 0) return KF_OK;
+    if (seeds->n > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;  // TMA tile coordinates are int32
     FitArgs a;
     a.n = seeds->n;
     a.par = seeds->par; a.cov = seeds->cov; a.ld_in = seeds->ld; a.q = seeds->q;

@@ -93,4 +93,7 @@ struct ScoreArgs {
 // kf_score.cu
 cudaError_t launch_score(const FitParams& P, const ScoreArgs& a, cudaStream_t stream);
 
+// kf_peak.cu
+double measure_fp32_peak(cudaStream_t stream, int repeats, float* sink);
+
 }  // namespace kf

@@ -31,7 +31,7 @@ def test_header_declares_the_north_star_calls():
     names = _declared()
     for must in ("kf_fit_tracks", "kf_score_candidates", "kf_bin_hits", "kf_create", "kf_destroy", "kf_strerror"):
         assert must in names
-    assert len(names) == len(set(names)) >= 11
+    assert len(names) == len(set(names)) >= 12
 
 
 def test_library_exports_every_declared_symbol(lib):
@@ -60,6 +60,7 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_fit_tracks_host(None, None, None, None, None) == -1
     assert lib.kf_bin_hits(None, 1.0, None, None) == -1
     assert lib.kf_score_candidates(None, None, 0, None, None, None, 2, 30.0, 1, None, None) == -1
+    assert lib.kf_measure_fp32_peak(None, 3, None) == -1
     assert lib.kf_last_cuda_error(None) == 0
 
 

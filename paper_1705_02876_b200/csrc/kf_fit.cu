@@ -31,7 +31,7 @@ namespace {
 #define KF_FIT_MIN_BLOCKS 5
 #endif
 #ifndef KF_FIT_STAGES
-#define KF_FIT_STAGES 4
+#define KF_FIT_STAGES 3
 #endif
 
 constexpr int kFitBlock = 128;
@@ -184,19 +184,24 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         m.x = tp[0];         m.y = tp[32];        m.z = tp[64];
         m.vxx = tp[96];      m.vxy = tp[128];     m.vxz = tp[160];
         m.vyy = tp[192];     m.vyz = tp[224];     m.vzz = tp[256];
-        __syncwarp();        // every lane has its hit in registers: the stage may be refilled
-        if (l + kStages < L && elect_one()) {
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
-            tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * (l + kStages), bar0 + 8u * s);
-            tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * (l + kStages), bar0 + 8u * s);
-        }
+        __syncwarp();        // every lane has issued its reads of this stage
         if (good_q && ((mask >> l) & 1u)) {
             uint32_t rc;
             if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.mass2, m, chi2);
             else rc = fit_layer<false>(t, k, ik, P.layer[l], P.mass2, m, chi2);
             st |= rc;
             if (rc == 0u) { nh += 1; started = true; }
+        }
+        // The hit values have been consumed by the math above, so the stage can be handed back to the
+        // TMA unit (write-after-read across the generic and async proxies needs no fence once the
+        // reads have completed; the refill still lands kStages - 1 layers ahead of its use).
+        if (l + kStages < L) {
+            __syncwarp();
+            if (elect_one()) {
+                mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
+                tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * (l + kStages), bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * (l + kStages), bar0 + 8u * s);
+            }
         }
     }
     if (!good_q) st = ST_BAD_CHARGE;

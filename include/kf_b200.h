@@ -85,7 +85,7 @@ KF_API int kf_create(kf_ctx** out, int device, void* cuda_stream);
 KF_API int kf_destroy(kf_ctx* ctx);
 /* Change the borrowed stream used by later calls. */
 KF_API int kf_set_stream(kf_ctx* ctx, void* cuda_stream);
-/* Pre-size scratch so that no later call allocates: `max_hits` hits per layer for kf_bin_hits,
+/* Pre-size scratch so that no later call allocates: `max_hits` hits in total over the layers of one kf_bin_layers call,
  * `max_host_tracks` x `max_host_layers` for the *_host staging buffers (0 = leave as is). */
 KF_API int kf_reserve(kf_ctx* ctx, int64_t max_hits, int64_t max_host_tracks, int max_host_layers);
 /* Static, never NULL. */
@@ -157,8 +157,10 @@ typedef struct {
     int64_t ld;               /* plane stride of pos_sorted / cov_sorted, >= n_hits, % 4 == 0      */
     int32_t* bin_offset;      /* DEV [n_eta*n_phi + 1] first sorted slot of each bin               */
     int32_t* sorted_to_orig;  /* DEV [n_hits] original index of the hit in each sorted slot        */
-    float* pos_sorted;        /* DEV [3][ld] hits in bin order                                     */
-    float* cov_sorted;        /* DEV [6][ld]                                                       */
+    float* hit_rec;           /* DEV [n_hits][12] hits in bin order, packed for scoring:
+                                 x y z vxx vxy vxz vyy vyz vzz, original index (int32 bits), 0, 0  */
+    float* pos_sorted;        /* DEV [3][ld] hits in bin order, SoA; optional (NULL = not written)  */
+    float* cov_sorted;        /* DEV [6][ld] optional (NULL = not written)                          */
 } kf_layer_bins;
 
 /* Bin one layer's hits: bin = i_eta*n_phi + i_phi with eta = asinh(z/radius), phi = atan2(y,x) over
@@ -167,6 +169,18 @@ typedef struct {
  * caller-allocated.  n_hits == 0 is valid (all offsets 0). */
 KF_API int kf_bin_hits(kf_ctx* ctx, float radius_cm, const kf_layer_hits* hits, kf_layer_bins* out);
 
+/* The same for n_layers layers at once (HOST arrays of descriptors, DEV buffers inside): four kernel
+ * launches in total instead of four per layer.  All layers must share n_eta, n_phi and eta_max. */
+KF_API int kf_bin_layers(kf_ctx* ctx, int n_layers, const float* radius_cm, const kf_layer_hits* hits,
+                         kf_layer_bins* out);
+
+/* Optional: a processing order for kf_score_candidates that puts candidates reaching the same
+ * (eta, phi) bin of `layer` next to each other (stable counting sort of the candidates by that bin),
+ * so that neighbouring warps share their hit windows in cache.  order[n] DEV, a permutation of 0..n-1.
+ * Purely a scheduling hint: results do not depend on it. */
+KF_API int kf_order_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, const kf_tracks* cands,
+                               int n_eta, int n_phi, float eta_max, int32_t* order);
+
 /* Best-hit scoring of n candidates on ONE layer (`layer` indexes the geometry): propagate (+Q),
  * take the candidate's own (eta, phi) bin, score chi2 = r^T (C'_pp + V_h)^-1 r for every hit in
  * the window i_eta +- window_half (clipped), i_phi +- window_half (wrapped); best = lowest chi2,
@@ -174,10 +188,12 @@ KF_API int kf_bin_hits(kf_ctx* ctx, float radius_cm, const kf_layer_hits* hits, 
  * Accepted and do_update: Kalman update, nhits += 1, chi2 += best.  Otherwise the candidate keeps
  * the propagated state (Q included).  best_hit[n] = ORIGINAL hit index or -1; best_chi2[n] = lowest
  * chi2 seen (+inf if the window was empty).  Propagation failure: status bit, candidate untouched,
- * best_hit = -1, best_chi2 = +inf.  All pointers DEV.  The caller loops over layers. */
+ * best_hit = -1, best_chi2 = +inf.  Reads bins->bin_offset and bins->hit_rec.  `order` = NULL or the
+ * output of kf_order_candidates.  All pointers DEV.  The caller loops over layers. */
 KF_API int kf_score_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, kf_tracks* cands,
-                        const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
-                        float chi2_cut, int do_update, int32_t* best_hit, float* best_chi2);
+                               const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                               float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
+                               float* best_chi2);
 
 #ifdef __cplusplus
 }

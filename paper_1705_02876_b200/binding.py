@@ -20,7 +20,8 @@ _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so"
 
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_host", "kf_bin_hits", "kf_score_candidates"]
+           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_score_candidates"]
 
 
 class KFError(RuntimeError):
@@ -51,8 +52,8 @@ class _LayerHits(C.Structure):
 
 class _LayerBins(C.Structure):
     _fields_ = [("n_eta", C.c_int), ("n_phi", C.c_int), ("eta_max", C.c_float), ("ld", C.c_int64),
-                ("bin_offset", C.c_void_p), ("sorted_to_orig", C.c_void_p), ("pos_sorted", C.c_void_p),
-                ("cov_sorted", C.c_void_p)]
+                ("bin_offset", C.c_void_p), ("sorted_to_orig", C.c_void_p), ("hit_rec", C.c_void_p),
+                ("pos_sorted", C.c_void_p), ("cov_sorted", C.c_void_p)]
 
 
 _lib = None
@@ -94,9 +95,14 @@ def load_library():
         f.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.POINTER(_Tracks)]
     lib.kf_bin_hits.restype = C.c_int
     lib.kf_bin_hits.argtypes = [vp, C.c_float, C.POINTER(_LayerHits), C.POINTER(_LayerBins)]
+    lib.kf_bin_layers.restype = C.c_int
+    lib.kf_bin_layers.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(_LayerHits), C.POINTER(_LayerBins)]
+    lib.kf_order_candidates.restype = C.c_int
+    lib.kf_order_candidates.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.POINTER(_Tracks), C.c_int, C.c_int,
+                                        C.c_float, vp]
     lib.kf_score_candidates.restype = C.c_int
     lib.kf_score_candidates.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.POINTER(_Tracks), C.POINTER(_LayerHits),
-                                        C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int, vp, vp]
+                                        C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int, vp, vp, vp]
     _lib = lib
     return lib
 
@@ -133,22 +139,26 @@ class Bins:
     eta_max: float
     bin_offset: torch.Tensor      # int32 [n_eta*n_phi + 1]
     sorted_to_orig: torch.Tensor  # int32 [n_hits]
-    pos_sorted: torch.Tensor      # f32 [3][ld]
-    cov_sorted: torch.Tensor      # f32 [6][ld]
+    hit_rec: torch.Tensor         # f32 [n_hits][12] packed records in bin order
+    pos_sorted: torch.Tensor | None = None   # f32 [3][ld] optional SoA copy
+    cov_sorted: torch.Tensor | None = None   # f32 [6][ld]
 
     @staticmethod
-    def allocate(n_hits: int, n_eta: int, n_phi: int, eta_max: float, device) -> "Bins":
+    def allocate(n_hits: int, n_eta: int, n_phi: int, eta_max: float, device, soa: bool = True) -> "Bins":
         ld = max(4, (n_hits + 3) // 4 * 4)
         return Bins(n_eta, n_phi, eta_max,
                     torch.empty(n_eta * n_phi + 1, dtype=torch.int32, device=device),
                     torch.empty(max(n_hits, 1), dtype=torch.int32, device=device),
-                    torch.empty((3, ld), dtype=torch.float32, device=device),
-                    torch.empty((6, ld), dtype=torch.float32, device=device))
+                    torch.empty((max(n_hits, 1), 12), dtype=torch.float32, device=device),
+                    torch.empty((3, ld), dtype=torch.float32, device=device) if soa else None,
+                    torch.empty((6, ld), dtype=torch.float32, device=device) if soa else None)
 
     def _c(self):
-        return _LayerBins(self.n_eta, self.n_phi, float(self.eta_max), int(self.pos_sorted.shape[1]),
-                          self.bin_offset.data_ptr(), self.sorted_to_orig.data_ptr(),
-                          self.pos_sorted.data_ptr(), self.cov_sorted.data_ptr())
+        ld = int(self.pos_sorted.shape[1]) if self.pos_sorted is not None else 0
+        return _LayerBins(self.n_eta, self.n_phi, float(self.eta_max), ld,
+                          self.bin_offset.data_ptr(), self.sorted_to_orig.data_ptr(), self.hit_rec.data_ptr(),
+                          self.pos_sorted.data_ptr() if self.pos_sorted is not None else None,
+                          self.cov_sorted.data_ptr() if self.cov_sorted is not None else None)
 
 
 def _plane_ld(t: torch.Tensor, rows: int) -> int:
@@ -251,24 +261,49 @@ class KFContext:
                     "kf_fit_tracks_host")
         del keep
 
-    # ------------------------------------------------------------------ kf_bin_hits
-    def bin_hits(self, radius_cm: float, n_hits: int, pos, cov, bins: Bins):
+    # ------------------------------------------------------------------ kf_bin_hits / kf_bin_layers
+    @staticmethod
+    def _layer_hits(n_hits, pos, cov) -> _LayerHits:
         lh = _LayerHits(int(n_hits), _plane_ld(pos, 3), pos.data_ptr(), cov.data_ptr())
         if _plane_ld(cov, 6) != lh.ld:
             raise ValueError("pos and cov must share the plane stride ld")
+        return lh
+
+    def bin_hits(self, radius_cm: float, n_hits: int, pos, cov, bins: Bins):
+        lh = self._layer_hits(n_hits, pos, cov)
         lb = bins._c()
         self._check(self._lib.kf_bin_hits(self._h, float(radius_cm), C.byref(lh), C.byref(lb)), "kf_bin_hits")
+
+    def bin_layers(self, radii_cm, layers):
+        """layers: sequence of (n_hits, pos, cov, bins); one batched call for all of them."""
+        n = len(layers)
+        rad = (C.c_float * n)(*[float(r) for r in radii_cm])
+        lhs = (_LayerHits * n)(*[self._layer_hits(nh, p, c) for (nh, p, c, _) in layers])
+        lbs = (_LayerBins * n)(*[b._c() for (_, _, _, b) in layers])
+        self._check(self._lib.kf_bin_layers(self._h, n, rad, lhs, lbs), "kf_bin_layers")
+
+    # ------------------------------------------------------------------ kf_order_candidates
+    def order_candidates(self, geom: Geometry, layer: int, n: int, par, cov, q, chi2, nhits, status,
+                         n_eta: int, n_phi: int, eta_max: float, order):
+        g, keep = geom._c()
+        cands = self._tracks(n, par, cov, q, chi2, nhits, status)
+        self._check(self._lib.kf_order_candidates(self._h, C.byref(g), int(layer), C.byref(cands), int(n_eta),
+                                                  int(n_phi), float(eta_max), order.data_ptr()),
+                    "kf_order_candidates")
+        del keep
 
     # ------------------------------------------------------------------ kf_score_candidates
     def score_candidates(self, geom: Geometry, layer: int, n: int, par, cov, q, chi2, nhits, status,
                          n_hits: int, pos, cov_hits, bins: Bins, window_half: int, chi2_cut: float,
-                         do_update: bool, best_hit, best_chi2):
+                         do_update: bool, best_hit, best_chi2, order=None):
         g, keep = geom._c()
         cands = self._tracks(n, par, cov, q, chi2, nhits, status)
         lh = _LayerHits(int(n_hits), _plane_ld(pos, 3), pos.data_ptr(), cov_hits.data_ptr())
         lb = bins._c()
         self._check(self._lib.kf_score_candidates(self._h, C.byref(g), int(layer), C.byref(cands), C.byref(lh),
                                                   C.byref(lb), int(window_half), float(chi2_cut),
-                                                  1 if do_update else 0, best_hit.data_ptr(), best_chi2.data_ptr()),
+                                                  1 if do_update else 0,
+                                                  order.data_ptr() if order is not None else None,
+                                                  best_hit.data_ptr(), best_chi2.data_ptr()),
                     "kf_score_candidates")
         del keep

@@ -136,10 +136,16 @@ class DeviceCandidates:
         return c
 
     def score(self, ctx: KFContext, geom: Geometry, layer: int, hits: DeviceLayer, window_half: int = 2,
-              chi2_cut: float = 30.0, do_update: bool = True):
+              chi2_cut: float = 30.0, do_update: bool = True, order: torch.Tensor | None = None):
         ctx.score_candidates(geom, layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,
                              hits.n_hits, hits.pos, hits.cov, hits.bins, window_half, chi2_cut, do_update,
-                             self.best_hit, self.best_chi2)
+                             self.best_hit, self.best_chi2, order)
+
+    def make_order(self, ctx: KFContext, geom: Geometry, layer: int, n_eta: int, n_phi: int, eta_max: float):
+        order = torch.empty(max(self.n, 1), dtype=torch.int32, device=self.par.device)
+        ctx.order_candidates(geom, layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,
+                             n_eta, n_phi, eta_max, order)
+        return order
 
     def results(self) -> dict:
         n = self.n

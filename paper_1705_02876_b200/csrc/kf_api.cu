@@ -23,7 +23,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 1;
+constexpr int kAbiVersion = 2;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -147,7 +147,7 @@ int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_hos
     cudaError_t e = cudaSetDevice(c->device);
     if (e != cudaSuccess) return cuda_fail(c, e);
     if (max_hits > 0) {
-        e = c->bin.reserve(max_hits, KF_MAX_BINS, c->stream);
+        e = c->bin.reserve(max_hits, 2 * (KF_MAX_BINS + 1), c->stream);
         if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     }
     if (max_host_tracks > 0 && max_host_layers > 0) {
@@ -218,45 +218,92 @@ int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seed
     return KF_OK;
 }
 
-int kf_bin_hits(kf_ctx* c, float radius_cm, const kf_layer_hits* hits, kf_layer_bins* out) {
-    if (!c || !hits || !out) return KF_ERR_NULL;
-    if (hits->n_hits < 0 || hits->ld < hits->n_hits || out->ld < hits->n_hits) return KF_ERR_SHAPE;
+namespace {
+
+int check_bin_args(const kf_layer_hits* hits, const kf_layer_bins* out, float radius_cm) {
+    if (!hits || !out) return KF_ERR_NULL;
+    if (hits->n_hits < 0 || hits->ld < hits->n_hits) return KF_ERR_SHAPE;
     if (out->n_eta < 1 || out->n_phi < 2) return KF_ERR_SHAPE;
     if (out->n_phi % 2 != 0 || (int64_t)out->n_eta * out->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
     if (!(radius_cm > 0.0f) || !(out->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;
-    if (hits->n_hits > 0x7fffffff) return KF_ERR_UNSUPPORTED;
+    if (hits->n_hits > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
     if (!out->bin_offset) return KF_ERR_NULL;
     if (hits->n_hits > 0) {
-        if (!hits->pos || !hits->cov || !out->sorted_to_orig || !out->pos_sorted || !out->cov_sorted)
-            return KF_ERR_NULL;
-        if (hits->ld % 4 != 0 || out->ld % 4 != 0 || !aligned16(hits->pos) || !aligned16(hits->cov) ||
-            !aligned16(out->pos_sorted) || !aligned16(out->cov_sorted))
+        if (!hits->pos || !hits->cov || !out->sorted_to_orig || !out->hit_rec) return KF_ERR_NULL;
+        if (hits->ld % 4 != 0 || !aligned16(hits->pos) || !aligned16(hits->cov) || !aligned16(out->hit_rec))
             return KF_ERR_ALIGN;
+        if (out->pos_sorted || out->cov_sorted) {
+            if (out->ld < hits->n_hits) return KF_ERR_SHAPE;
+            if (out->ld % 4 != 0 || !aligned16(out->pos_sorted) || !aligned16(out->cov_sorted)) return KF_ERR_ALIGN;
+        }
     }
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    e = c->bin.reserve(hits->n_hits, out->n_eta * out->n_phi, c->stream);
-    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    return KF_OK;
+}
+
+BinArgs to_bin_args(float radius_cm, const kf_layer_hits* hits, const kf_layer_bins* out) {
     BinArgs a;
     a.n_hits = hits->n_hits; a.ld_in = hits->ld; a.pos = hits->pos; a.cov = hits->cov;
     a.radius = radius_cm; a.n_eta = out->n_eta; a.n_phi = out->n_phi; a.eta_max = out->eta_max;
     a.ld_out = out->ld; a.bin_offset = out->bin_offset; a.sorted_to_orig = out->sorted_to_orig;
-    a.pos_sorted = out->pos_sorted; a.cov_sorted = out->cov_sorted;
-    e = launch_bin(c->bin, a, c->stream);
+    a.pos_sorted = out->pos_sorted; a.cov_sorted = out->cov_sorted; a.hit_rec = out->hit_rec;
+    return a;
+}
+
+}  // namespace
+
+int kf_bin_layers(kf_ctx* c, int n_layers, const float* radius_cm, const kf_layer_hits* hits, kf_layer_bins* out) {
+    if (!c || !radius_cm || !hits || !out) return KF_ERR_NULL;
+    if (n_layers < 0 || n_layers > KF_MAX_LAYERS) return KF_ERR_SHAPE;
+    if (n_layers == 0) return KF_OK;
+    BinArgs args[KF_MAX_LAYERS];
+    for (int l = 0; l < n_layers; ++l) {
+        const int rc = check_bin_args(hits + l, out + l, radius_cm[l]);
+        if (rc) return rc;
+        if (out[l].n_eta != out[0].n_eta || out[l].n_phi != out[0].n_phi || out[l].eta_max != out[0].eta_max)
+            return KF_ERR_UNSUPPORTED;
+        args[l] = to_bin_args(radius_cm[l], hits + l, out + l);
+    }
+    cudaError_t e = cudaSetDevice(c->device);
     if (e != cudaSuccess) return cuda_fail(c, e);
+    e = launch_bin(c->bin, n_layers, args, c->stream);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_bin_hits(kf_ctx* c, float radius_cm, const kf_layer_hits* hits, kf_layer_bins* out) {
+    return kf_bin_layers(c, 1, &radius_cm, hits, out);
+}
+
+int kf_order_candidates(kf_ctx* c, const kf_geometry* geom, int layer, const kf_tracks* cands, int n_eta,
+                        int n_phi, float eta_max, int32_t* order) {
+    if (!c || !geom || !cands) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (layer < 0 || layer >= geom->n_layers) return KF_ERR_SHAPE;
+    if (cands->n < 0 || cands->ld < cands->n || n_eta < 1 || n_phi < 2) return KF_ERR_SHAPE;
+    if ((int64_t)n_eta * n_phi > KF_MAX_BINS || !(eta_max > 0.0f) || cands->n > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
+    if (cands->n == 0) return KF_OK;
+    if (!cands->par || !cands->q || !order) return KF_ERR_NULL;
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = launch_order(c->bin, P, layer, cands->n, cands->ld, cands->par, cands->q, n_eta, n_phi, eta_max, order,
+                     c->stream);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
 }
 
 int kf_score_candidates(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks* cands,
                         const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
-                        float chi2_cut, int do_update, int32_t* best_hit, float* best_chi2) {
+                        float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
+                        float* best_chi2) {
     if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
     FitParams P;
     int rc = make_params(geom, &P);
     if (rc) return rc;
     if (layer < 0 || layer >= geom->n_layers) return KF_ERR_SHAPE;
     if ((rc = check_tracks(cands, true, true))) return rc;
-    if (hits->n_hits < 0 || hits->ld < hits->n_hits || bins->ld < hits->n_hits) return KF_ERR_SHAPE;
+    if (hits->n_hits < 0) return KF_ERR_SHAPE;
     if (bins->n_eta < 1 || bins->n_phi < 2 || window_half < 0) return KF_ERR_SHAPE;
     if (bins->n_phi % 2 != 0 || (int64_t)bins->n_eta * bins->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
     if (2 * window_half + 1 > bins->n_phi) return KF_ERR_UNSUPPORTED;
@@ -264,16 +311,13 @@ int kf_score_candidates(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks
     if (cands->n == 0) return KF_OK;
     if (!best_hit || !best_chi2 || !bins->bin_offset) return KF_ERR_NULL;
     if (hits->n_hits > 0) {
-        if (!bins->sorted_to_orig || !bins->pos_sorted || !bins->cov_sorted) return KF_ERR_NULL;
-        if (bins->ld % 4 != 0 || !aligned16(bins->pos_sorted) || !aligned16(bins->cov_sorted))
-            return KF_ERR_ALIGN;
+        if (!bins->hit_rec) return KF_ERR_NULL;
+        if (!aligned16(bins->hit_rec)) return KF_ERR_ALIGN;
     }
     ScoreArgs a;
     a.n = cands->n; a.ld = cands->ld; a.par = cands->par; a.cov = cands->cov; a.q = cands->q;
     a.chi2 = cands->chi2; a.nhits = cands->nhits; a.status = cands->status;
-    a.n_hits = hits->n_hits; a.ld_hit = bins->ld;
-    a.pos_sorted = bins->pos_sorted; a.cov_sorted = bins->cov_sorted;
-    a.bin_offset = bins->bin_offset; a.sorted_to_orig = bins->sorted_to_orig;
+    a.n_hits = hits->n_hits; a.hit_rec = bins->hit_rec; a.bin_offset = bins->bin_offset; a.order = order;
     a.n_eta = bins->n_eta; a.n_phi = bins->n_phi; a.eta_max = bins->eta_max;
     a.window_half = window_half; a.chi2_cut = chi2_cut; a.do_update = do_update ? 1 : 0;
     a.layer = layer; a.best_hit = best_hit; a.best_chi2 = best_chi2;

@@ -1,5 +1,6 @@
-// kf_bin.cu -- (eta, phi) binning of one layer's hits ("directionally projective
-// bins"; PAPER.md:135 hits are regrouped on the GPU).
+// kf_bin.cu -- (eta, phi) binning of layer hit pools, and the same counting sort reused to give
+// candidates a cache-friendly processing order ("directionally projective bins";
+// PAPER.md:135 hits are regrouped on the GPU).
 //
 // bin = i_eta * n_phi + i_phi, eta = asinh(z / r_layer), phi = atan2(y, x) in [-pi, pi).
 // The bin of a hit is an integer decided by floating point, so it is decided in single precision
@@ -11,10 +12,13 @@
 //     lower half plane:      i_phi = #{ j in 1..n_phi/2-1 : fl(cos_j y) >= fl(sin_j x) }
 // with (cos_j, sin_j) = fl(cos, sin)(-pi + j d_phi).  No transcendental is evaluated on the GPU.
 //
-// Counting sort, stable: (1) bin of every hit + histogram, (2) exclusive scan -> bin_offset,
-// (3) scatter hit indices into their bin segment in arbitrary order (atomic cursor), (4) every
-// slot ranks its index inside its segment (indices are unique, so sorting them ascending IS the
-// stable order) and gathers the 9 floats of the hit into the bin-sorted SoA copy.
+// Counting sort, stable, batched over layers (grid.y = layer, 4 launches + 1 memset for ALL layers):
+// (1) key of every item + histogram, (2) exclusive scan -> bin_offset, (3) scatter item indices into
+// their bin segment in arbitrary order (atomic cursor), (4) every slot ranks its index inside its
+// segment (indices are unique, so ascending index IS the stable order) and, for hits, gathers the
+// hit into the bin-ordered outputs: a packed 12-float record per hit for the scoring kernel
+// (x y z vxx vxy vxz vyy vyz vzz, original index, 2 pad: three 128-bit loads per hit) and,
+// optionally, SoA copies.
 #include <cmath>
 
 #include "kf_internal.h"
@@ -32,7 +36,7 @@ __device__ __forceinline__ int bin_of_hit(float x, float y, float z, float r, in
                                           const float* __restrict__ phi_sin) {
     const float u = __fdiv_rn(z, r);
     // edges are non-decreasing in j, so "count of edges <= u" is an upper-bound search
-    int lo = 1, hi = n_eta;  // answer - 1 ... first j in [1, n_eta) with !(u >= edge[j]), else n_eta
+    int lo = 1, hi = n_eta;
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
         if (u >= __ldg(eta_edge + mid)) lo = mid + 1; else hi = mid;
@@ -54,22 +58,22 @@ __device__ __forceinline__ int bin_of_hit(float x, float y, float z, float r, in
 }
 
 __global__ void __launch_bounds__(kBlock)
-bin_count_kernel(int64_t n_hits, int64_t ld, const float* __restrict__ pos, float r, int n_eta,
-                 int n_phi, const float* __restrict__ eta_edge, const float* __restrict__ phi_cos,
-                 const float* __restrict__ phi_sin, int32_t* __restrict__ bin_of,
-                 int32_t* __restrict__ counts) {
+bin_key_kernel(const __grid_constant__ BinBatch B, const float* __restrict__ eta_edge,
+               const float* __restrict__ phi_cos, const float* __restrict__ phi_sin) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
     const int64_t h = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (h >= n_hits) return;
-    const int b = bin_of_hit(__ldg(pos + h), __ldg(pos + ld + h), __ldg(pos + 2 * ld + h), r, n_eta,
-                             n_phi, eta_edge, phi_cos, phi_sin);
-    bin_of[h] = b;
-    atomicAdd(counts + b, 1);
+    if (h >= L.n) return;
+    const int b = bin_of_hit(__ldg(L.pos + h), __ldg(L.pos + L.ld_in + h), __ldg(L.pos + 2 * L.ld_in + h),
+                             L.radius, B.n_eta, B.n_phi, eta_edge, phi_cos, phi_sin);
+    L.key[h] = b;
+    atomicAdd(L.counts + b, 1);
 }
 
-// Exclusive scan of counts[0..nb) -> bin_offset[0..nb], cursor = copy.  One block of 1024.
+// Exclusive scan of counts[0..nb) -> bin_offset[0..nb], cursor = copy.  One block of 1024 per layer.
 __global__ void __launch_bounds__(1024)
-bin_scan_kernel(int nb, const int32_t* __restrict__ counts, int32_t* __restrict__ bin_offset,
-                int32_t* __restrict__ cursor) {
+bin_scan_kernel(const __grid_constant__ BinBatch B) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
+    const int nb = B.n_eta * B.n_phi;
     __shared__ int32_t warp_sum[32];
     __shared__ int32_t carry_s;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -77,7 +81,7 @@ bin_scan_kernel(int nb, const int32_t* __restrict__ counts, int32_t* __restrict_
     __syncthreads();
     for (int base = 0; base < nb; base += 1024) {
         const int i = base + tid;
-        const int32_t c = i < nb ? counts[i] : 0;
+        const int32_t c = i < nb ? L.counts[i] : 0;
         int32_t incl = c;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -98,77 +102,120 @@ bin_scan_kernel(int nb, const int32_t* __restrict__ counts, int32_t* __restrict_
         __syncthreads();
         const int32_t carry = carry_s;
         const int32_t excl = carry + (wid ? warp_sum[wid - 1] : 0) + incl - c;
-        if (i < nb) { bin_offset[i] = excl; cursor[i] = excl; }
+        if (i < nb) { L.bin_offset[i] = excl; L.cursor[i] = excl; }
         __syncthreads();
         if (tid == 1023) carry_s = excl + c;
         __syncthreads();
     }
-    if (tid == 0) bin_offset[nb] = carry_s;
+    if (tid == 0) L.bin_offset[nb] = carry_s;
 }
 
 __global__ void __launch_bounds__(kBlock)
-bin_scatter_kernel(int64_t n_hits, const int32_t* __restrict__ bin_of, int32_t* __restrict__ cursor,
-                   int32_t* __restrict__ unsorted) {
+bin_scatter_kernel(const __grid_constant__ BinBatch B) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
     const int64_t h = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (h >= n_hits) return;
-    const int32_t slot = atomicAdd(cursor + bin_of[h], 1);
-    unsorted[slot] = (int32_t)h;
+    if (h >= L.n) return;
+    const int32_t slot = atomicAdd(L.cursor + L.key[h], 1);
+    L.unsorted[slot] = (int32_t)h;
 }
 
-// Slot p holds hit `mine` of bin b; its final place is bin_offset[b] + #{indices in the segment
+// Slot p holds item `mine` of bin b; its final place is bin_offset[b] + #{indices in the segment
 // smaller than mine}.  Neighbouring threads scan the same segment, so the loads broadcast.
 __global__ void __launch_bounds__(kBlock)
-bin_rank_gather_kernel(int64_t n_hits, int64_t ld_in, int64_t ld_out,
-                       const float* __restrict__ pos, const float* __restrict__ cov,
-                       const int32_t* __restrict__ bin_of, const int32_t* __restrict__ bin_offset,
-                       const int32_t* __restrict__ unsorted, int32_t* __restrict__ sorted_to_orig,
-                       float* __restrict__ pos_sorted, float* __restrict__ cov_sorted) {
+bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
     const int64_t p = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (p >= n_hits) return;
-    const int32_t mine = unsorted[p];
-    const int32_t b = bin_of[mine];
-    const int32_t s = bin_offset[b], e = bin_offset[b + 1];
+    if (p >= L.n) return;
+    const int32_t mine = L.unsorted[p];
+    const int32_t b = L.key[mine];
+    const int32_t s = L.bin_offset[b], e = L.bin_offset[b + 1];
     int32_t rank = 0;
-    for (int32_t j = s; j < e; ++j) rank += (__ldg(unsorted + j) < mine) ? 1 : 0;
+    for (int32_t j = s; j < e; ++j) rank += (__ldg(L.unsorted + j) < mine) ? 1 : 0;
     const int64_t dst = (int64_t)s + rank;
-    sorted_to_orig[dst] = mine;
+    L.sorted_to_orig[dst] = mine;
+    if (!L.pos) return;  // ordering only (candidates)
+    float v[9];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) pos_sorted[k * ld_out + dst] = __ldg(pos + k * ld_in + mine);
+    for (int k = 0; k < 3; ++k) v[k] = __ldg(L.pos + k * L.ld_in + mine);
 #pragma unroll
-    for (int k = 0; k < 6; ++k) cov_sorted[k * ld_out + dst] = __ldg(cov + k * ld_in + mine);
+    for (int k = 0; k < 6; ++k) v[3 + k] = __ldg(L.cov + k * L.ld_in + mine);
+    if (L.hit_rec) {
+        float4* rec = reinterpret_cast<float4*>(L.hit_rec + dst * 12);
+        rec[0] = make_float4(v[0], v[1], v[2], v[3]);
+        rec[1] = make_float4(v[4], v[5], v[6], v[7]);
+        rec[2] = make_float4(v[8], __int_as_float(mine), 0.0f, 0.0f);
+    }
+    if (L.pos_sorted) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) L.pos_sorted[k * L.ld_out + dst] = v[k];
+    }
+    if (L.cov_sorted) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) L.cov_sorted[k * L.ld_out + dst] = v[3 + k];
+    }
+}
+
+// Candidate keys for kf_order_candidates: the (eta, phi) bin of the candidate's crossing with the layer
+// (definition formula in fp32; the order only steers cache locality, never a result).
+__global__ void __launch_bounds__(kBlock)
+cand_key_kernel(const __grid_constant__ FitParams P, int layer, int64_t n, int64_t ld,
+                const float* __restrict__ par, const int8_t* __restrict__ q, int n_eta, int n_phi,
+                float eta_max, int32_t* __restrict__ key, int32_t* __restrict__ counts) {
+    const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (i >= n) return;
+    Track t;
+    t.x = __ldg(par + i);           t.y = __ldg(par + ld + i);      t.z = __ldg(par + 2 * ld + i);
+    t.px = __ldg(par + 3 * ld + i); t.py = __ldg(par + 4 * ld + i); t.pz = __ldg(par + 5 * ld + i);
+    t.eax = 1.0f; t.eay = 0.0f;
+    const float qf = (float)q[i];
+    Crossing o;
+    float x = t.x, y = t.y, z = t.z;
+    if (helix_to_radius(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], o)) { x = o.xn; y = o.yn; z = o.zn; }
+    const float rho = sqrtf(x * x + y * y);
+    const float eta = asinhf(z / fmaxf(rho, 1e-20f));
+    const float phi = atan2f(y, x);
+    int ie = (int)floorf((eta + eta_max) / (2.0f * eta_max / (float)n_eta));
+    ie = ie < 0 ? 0 : (ie > n_eta - 1 ? n_eta - 1 : ie);          // NaN -> 0 through the casts below
+    int ip = (int)floorf((phi + 3.14159265358979f) / (6.28318530717959f / (float)n_phi));
+    ip = ((ip % n_phi) + n_phi) % n_phi;
+    int b = ie * n_phi + ip;
+    if (!(b >= 0 && b < n_eta * n_phi)) b = 0;
+    key[i] = b;
+    atomicAdd(counts + b, 1);
 }
 
 }  // namespace
 
-cudaError_t BinScratch::reserve(int64_t n_hits, int n_bins, cudaStream_t stream) {
-    if (n_hits <= cap_hits && n_bins <= cap_bins) return cudaSuccess;
+cudaError_t BinScratch::reserve(int64_t n_items, int64_t n_bins, cudaStream_t stream) {
+    if (n_items <= cap_items && n_bins <= cap_bins) return cudaSuccess;
     // growing: drain the stream that may still use the old buffers, then reallocate
     cudaError_t e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) return e;
-    const int64_t nh = n_hits > cap_hits ? n_hits : cap_hits;
-    const int nb = n_bins > cap_bins ? n_bins : cap_bins;
+    const int64_t ni = n_items > cap_items ? n_items : cap_items;
+    const int64_t nb = n_bins > cap_bins ? n_bins : cap_bins;
     release();
-    const size_t hits_b = (size_t)(nh > 0 ? nh : 1) * sizeof(int32_t);
-    const size_t bins_b = (size_t)(nb + 1) * sizeof(int32_t);
-    if ((e = cudaMalloc(&bin_of, hits_b)) != cudaSuccess) { release(); return e; }
-    if ((e = cudaMalloc(&unsorted, hits_b)) != cudaSuccess) { release(); return e; }
+    const size_t items_b = (size_t)(ni > 0 ? ni : 1) * sizeof(int32_t);
+    const size_t bins_b = (size_t)(nb > 0 ? nb : 1) * sizeof(int32_t);
+    const size_t tab_b = (size_t)(KF_MAX_BINS_INTERNAL + 1) * sizeof(float);
+    if ((e = cudaMalloc(&key, items_b)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&unsorted, items_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&counts, bins_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&cursor, bins_b)) != cudaSuccess) { release(); return e; }
-    if ((e = cudaMalloc(&eta_edge, bins_b)) != cudaSuccess) { release(); return e; }
-    if ((e = cudaMalloc(&phi_cos, bins_b)) != cudaSuccess) { release(); return e; }
-    if ((e = cudaMalloc(&phi_sin, bins_b)) != cudaSuccess) { release(); return e; }
-    cap_hits = nh;
+    if ((e = cudaMalloc(&eta_edge, tab_b)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&phi_cos, tab_b)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&phi_sin, tab_b)) != cudaSuccess) { release(); return e; }
+    cap_items = ni;
     cap_bins = nb;
     return cudaSuccess;
 }
 
 void BinScratch::release() {
-    void* ptrs[] = {bin_of, unsorted, counts, cursor, eta_edge, phi_cos, phi_sin};
+    void* ptrs[] = {key, unsorted, counts, cursor, eta_edge, phi_cos, phi_sin};
     for (void* p : ptrs)
         if (p) cudaFree(p);
-    bin_of = unsorted = counts = cursor = nullptr;
+    key = unsorted = counts = cursor = nullptr;
     eta_edge = phi_cos = phi_sin = nullptr;
-    cap_hits = 0;
+    cap_items = 0;
     cap_bins = 0;
     tab_n_eta = tab_n_phi = 0;
     tab_eta_max = 0.0f;
@@ -200,23 +247,66 @@ cudaError_t BinScratch::tables(int n_eta, int n_phi, float eta_max, cudaStream_t
     return cudaSuccess;
 }
 
-cudaError_t launch_bin(BinScratch& s, const BinArgs& a, cudaStream_t stream) {
-    const int nb = a.n_eta * a.n_phi;
-    cudaError_t e = s.tables(a.n_eta, a.n_phi, a.eta_max, stream);
+// Bin up to kBinBatchMax layers per group of launches.  All layers share (n_eta, n_phi, eta_max).
+cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream) {
+    if (n_layers <= 0) return cudaSuccess;
+    const int n_eta = args[0].n_eta, n_phi = args[0].n_phi;
+    const int nb = n_eta * n_phi;
+    int64_t total = 0, max_hits = 0;
+    for (int l = 0; l < n_layers; ++l) { total += args[l].n_hits; if (args[l].n_hits > max_hits) max_hits = args[l].n_hits; }
+    cudaError_t e = s.reserve(total, (int64_t)(nb + 1) * n_layers, stream);
+    if (e != cudaSuccess) return e;
+    if ((e = s.tables(n_eta, n_phi, args[0].eta_max, stream)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(s.counts, 0, (size_t)(nb + 1) * n_layers * sizeof(int32_t), stream)) != cudaSuccess) return e;
+    int64_t item_off = 0;
+    for (int l0 = 0; l0 < n_layers; l0 += kBinBatchMax) {
+        const int m = n_layers - l0 < kBinBatchMax ? n_layers - l0 : kBinBatchMax;
+        BinBatch B;
+        B.n_layers = m; B.n_eta = n_eta; B.n_phi = n_phi;
+        int64_t group_max = 0;
+        for (int j = 0; j < m; ++j) {
+            const BinArgs& a = args[l0 + j];
+            BinLayerDev& L = B.layer[j];
+            L.n = a.n_hits; L.ld_in = a.ld_in; L.ld_out = a.ld_out; L.pos = a.pos; L.cov = a.cov; L.radius = a.radius;
+            L.bin_offset = a.bin_offset; L.sorted_to_orig = a.sorted_to_orig;
+            L.pos_sorted = a.pos_sorted; L.cov_sorted = a.cov_sorted; L.hit_rec = a.hit_rec;
+            L.key = s.key + item_off; L.unsorted = s.unsorted + item_off;
+            L.counts = s.counts + (int64_t)(l0 + j) * (nb + 1); L.cursor = s.cursor + (int64_t)(l0 + j) * (nb + 1);
+            item_off += a.n_hits;
+            if (a.n_hits > group_max) group_max = a.n_hits;
+        }
+        const dim3 grid((unsigned)((group_max + kBlock - 1) / kBlock), (unsigned)m);
+        if (group_max > 0) bin_key_kernel<<<grid, kBlock, 0, stream>>>(B, s.eta_edge, s.phi_cos, s.phi_sin);
+        bin_scan_kernel<<<dim3(1, m), 1024, 0, stream>>>(B);
+        if (group_max > 0) {
+            bin_scatter_kernel<<<grid, kBlock, 0, stream>>>(B);
+            bin_rank_gather_kernel<<<grid, kBlock, 0, stream>>>(B);
+        }
+    }
+    return cudaGetLastError();
+}
+
+// Stable order of candidates by the bin they reach on `layer`.
+cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n, int64_t ld, const float* par,
+                         const int8_t* q, int n_eta, int n_phi, float eta_max, int32_t* order,
+                         cudaStream_t stream) {
+    if (n == 0) return cudaSuccess;
+    const int nb = n_eta * n_phi;
+    cudaError_t e = s.reserve(n, 2 * (int64_t)(nb + 1), stream);
     if (e != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(s.counts, 0, (size_t)(nb + 1) * sizeof(int32_t), stream)) != cudaSuccess) return e;
-    const unsigned blocks = (unsigned)((a.n_hits + kBlock - 1) / kBlock);
-    if (a.n_hits > 0) {
-        bin_count_kernel<<<blocks, kBlock, 0, stream>>>(a.n_hits, a.ld_in, a.pos, a.radius, a.n_eta, a.n_phi,
-                                                        s.eta_edge, s.phi_cos, s.phi_sin, s.bin_of, s.counts);
-    }
-    bin_scan_kernel<<<1, 1024, 0, stream>>>(nb, s.counts, a.bin_offset, s.cursor);
-    if (a.n_hits > 0) {
-        bin_scatter_kernel<<<blocks, kBlock, 0, stream>>>(a.n_hits, s.bin_of, s.cursor, s.unsorted);
-        bin_rank_gather_kernel<<<blocks, kBlock, 0, stream>>>(a.n_hits, a.ld_in, a.ld_out, a.pos, a.cov, s.bin_of,
-                                                              a.bin_offset, s.unsorted, a.sorted_to_orig,
-                                                              a.pos_sorted, a.cov_sorted);
-    }
+    BinBatch B;
+    B.n_layers = 1; B.n_eta = n_eta; B.n_phi = n_phi;
+    BinLayerDev& L = B.layer[0];
+    L.n = n; L.ld_in = 0; L.ld_out = 0; L.pos = nullptr; L.cov = nullptr; L.radius = 0.0f;
+    L.bin_offset = s.counts + (nb + 1);  // second half of the counts buffer holds the offsets
+    L.sorted_to_orig = order; L.pos_sorted = nullptr; L.cov_sorted = nullptr; L.hit_rec = nullptr;
+    L.key = s.key; L.unsorted = s.unsorted; L.counts = s.counts; L.cursor = s.cursor;
+    const dim3 grid((unsigned)((n + kBlock - 1) / kBlock), 1);
+    cand_key_kernel<<<grid, kBlock, 0, stream>>>(P, layer, n, ld, par, q, n_eta, n_phi, eta_max, s.key, s.counts);
+    bin_scan_kernel<<<dim3(1, 1), 1024, 0, stream>>>(B);
+    bin_scatter_kernel<<<grid, kBlock, 0, stream>>>(B);
+    bin_rank_gather_kernel<<<grid, kBlock, 0, stream>>>(B);
     return cudaGetLastError();
 }
 

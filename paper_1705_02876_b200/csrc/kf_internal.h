@@ -48,43 +48,69 @@ struct HostStage {
 };
 
 // ---------------------------------------------------------------------------------- binning
+constexpr int KF_MAX_BINS_INTERNAL = 65536;
+constexpr int kBinBatchMax = 16;  // layers per group of launches
+
 struct BinArgs {
     int64_t n_hits, ld_in;
     const float* pos; const float* cov;
     float radius; int n_eta, n_phi; float eta_max;
     int64_t ld_out;
-    int32_t* bin_offset; int32_t* sorted_to_orig; float* pos_sorted; float* cov_sorted;
+    int32_t* bin_offset; int32_t* sorted_to_orig;
+    float* pos_sorted; float* cov_sorted;  // optional SoA copies (may be null)
+    float* hit_rec;                        // [n_hits][12] packed records (may be null)
+};
+
+// One layer (or one candidate set) as the batched sort kernels see it.
+struct BinLayerDev {
+    int64_t n, ld_in, ld_out;
+    const float* pos; const float* cov;    // null: order items only, gather nothing
+    float radius;
+    int32_t* bin_offset; int32_t* sorted_to_orig;
+    float* pos_sorted; float* cov_sorted; float* hit_rec;
+    int32_t* key;       // [n] bin of each item
+    int32_t* unsorted;  // [n] item indices grouped by bin, arbitrary order inside
+    int32_t* counts;    // [n_bins + 1]
+    int32_t* cursor;    // [n_bins + 1]
+};
+
+struct BinBatch {
+    int n_layers, n_eta, n_phi;
+    BinLayerDev layer[kBinBatchMax];
 };
 
 struct BinScratch {
-    int64_t cap_hits = 0;
-    int cap_bins = 0;
-    int32_t* bin_of = nullptr;   // [cap_hits] bin of each hit
-    int32_t* unsorted = nullptr; // [cap_hits] hit indices grouped by bin, arbitrary order inside
-    int32_t* counts = nullptr;   // [cap_bins + 1]
-    int32_t* cursor = nullptr;   // [cap_bins + 1]
+    int64_t cap_items = 0, cap_bins = 0;
+    int32_t* key = nullptr;
+    int32_t* unsorted = nullptr;
+    int32_t* counts = nullptr;
+    int32_t* cursor = nullptr;
     // edge tables (device) for the (n_eta, n_phi, eta_max) last used
-    float* eta_edge = nullptr;   // [cap_bins] fl32(sinh(-eta_max + j d_eta)), j = 1..n_eta-1 at [j]
-    float* phi_cos = nullptr;    // [cap_bins] fl32(cos(-pi + j d_phi))
-    float* phi_sin = nullptr;    // [cap_bins]
+    float* eta_edge = nullptr;   // fl32(sinh(-eta_max + j d_eta)), j = 1..n_eta-1 at [j]
+    float* phi_cos = nullptr;    // fl32(cos(-pi + j d_phi))
+    float* phi_sin = nullptr;
     int tab_n_eta = 0, tab_n_phi = 0;
     float tab_eta_max = 0.0f;
     std::vector<float> host_tab; // persistent host copy of the three tables (source of the async copy)
-    cudaError_t reserve(int64_t n_hits, int n_bins, cudaStream_t stream);
+    cudaError_t reserve(int64_t n_items, int64_t n_bins, cudaStream_t stream);
     cudaError_t tables(int n_eta, int n_phi, float eta_max, cudaStream_t stream);
     void release();
 };
 
 // kf_bin.cu
-cudaError_t launch_bin(BinScratch& s, const BinArgs& a, cudaStream_t stream);
+cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream);
+cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n, int64_t ld, const float* par,
+                         const int8_t* q, int n_eta, int n_phi, float eta_max, int32_t* order,
+                         cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------- scoring
 struct ScoreArgs {
     int64_t n, ld;
     float* par; float* cov; const int8_t* q; float* chi2; int32_t* nhits; uint32_t* status;
-    int64_t n_hits, ld_hit;
-    const float* pos_sorted; const float* cov_sorted;
-    const int32_t* bin_offset; const int32_t* sorted_to_orig;
+    int64_t n_hits;
+    const float* hit_rec;
+    const int32_t* bin_offset;
+    const int32_t* order;  // may be null
     int n_eta, n_phi; float eta_max;
     int window_half; float chi2_cut; int do_update; int layer;
     int32_t* best_hit; float* best_chi2;

@@ -349,6 +349,19 @@ __device__ __forceinline__ float chi2_of(const Sym3& si, const LocalHit& h) {
     return h.rr * ur + h.rt * ut + h.rz * uz;
 }
 
+// chi2 of one hit against the propagated candidate, same Schur elimination as kalman_update
+// (one hit of the scoring window).  Returns false when det S <= 0 (the hit is skipped).
+__device__ __forceinline__ bool chi2_schur(float n11, float n12, float n22, const LocalHit& h, float& chi2) {
+    const float iv = rcp_fast(h.vrr);
+    const float sa = h.vrt * iv, sb = h.vrz * iv;
+    const float stt = n11 + (h.vtt - sa * h.vrt), stz = n12 + (h.vtz - sa * h.vrz), szz = n22 + (h.vzz - sb * h.vrz);
+    const float rt = h.rt - sa * h.rr, rz = h.rz - sb * h.rr;
+    const float det2 = stt * szz - stz * stz;
+    const float q = szz * rt * rt - 2.0f * stz * rt * rz + stt * rz * rz;
+    chi2 = h.rr * h.rr * iv + q * rcp_fast(det2);
+    return h.vrr * det2 > 0.0f;
+}
+
 // Kalman update in the arrival frame, then re-aim the momentum frame at the updated momentum.
 // On success writes the new track (position frame = arrival frame) and returns the chi2
 // increment through *dchi2.  Returns a status bit on failure (track untouched).

@@ -36,6 +36,9 @@ def _assert_bins_equal(dl, ob, pos, cov):
     assert np.array_equal(s2o, ob["sorted_to_orig"])
     assert np.array_equal(dl.bins.pos_sorted.cpu().numpy()[:, :H], pos[:, s2o])
     assert np.array_equal(dl.bins.cov_sorted.cpu().numpy()[:, :H], cov[:, s2o])
+    rec = dl.bins.hit_rec.cpu().numpy()[:H]
+    assert np.array_equal(rec[:, 0:3], pos[:, s2o].T) and np.array_equal(rec[:, 3:9], cov[:, s2o].T)
+    assert np.array_equal(rec[:, 9].copy().view(np.int32), s2o)
 
 
 @pytest.mark.parametrize("n_tracks,noise", [(400, 2000), (20000, 100000)])
@@ -74,6 +77,55 @@ def test_bin_hits_edge_cases(ctx):
     for ne, nph, emax in [(1, 2, 1.0), (7, 10, 2.0), (256, 256, 2.5)]:
         dl, ob = _bin_both(ctx, pos, cov[:, :3000], r, ne, nph, float(np.float32(emax)))
         _assert_bins_equal(dl, ob, pos, cov[:, :3000])
+
+
+def test_bin_layers_batched_equals_per_layer(ctx):
+    """kf_bin_layers (all layers in four launches) == kf_bin_hits layer by layer == oracle."""
+    from paper_1705_02876_b200.buffers import DeviceLayer
+    ev = W.make_build_event(4, n_tracks=2000, noise_hits=9000)
+    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers]
+    dls[2] = DeviceLayer.from_numpy(np.zeros((3, 0), np.float32), np.zeros((6, 0), np.float32), NE, NP, EMAX, "cuda:0")
+    ctx.bin_layers([l.radius for l in ev.layers], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+    torch.cuda.synchronize()
+    for i, (d, l) in enumerate(zip(dls, ev.layers)):
+        if i == 2:
+            assert np.all(d.bins.bin_offset.cpu().numpy() == 0)
+            continue
+        _assert_bins_equal(d, O.bin_hits(l.pos, l.radius, NE, NP, EMAX), l.pos, l.cov)
+
+
+def test_order_is_a_stable_bin_sort_and_changes_no_result(ctx):
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    ev = W.make_build_event(4, n_tracks=3000, noise_hits=15000)
+    f = ev.fit
+    par, cov, chi2, nh = _seeds(ev)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+    lay = ev.layers[3]
+    dl = DeviceLayer.from_numpy(lay.pos, lay.cov, NE, NP, EMAX, "cuda:0")
+    dl.bin(ctx, lay.radius)
+    a = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    b = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    order = b.make_order(ctx, geom, 3, NE, NP, EMAX)
+    torch.cuda.synchronize()
+    o = order.cpu().numpy()[:f.n]
+    assert np.array_equal(np.sort(o), np.arange(f.n))                    # a permutation
+    # keys: bin of the oracle-propagated position; sorted by key, ascending index inside a key
+    keys = np.empty(f.n, dtype=np.int64)
+    for i in range(f.n):
+        rc, u, _, _, _ = O.propagate(par[:, i].astype(np.float64), float(f.q[i]), f.Bz, lay.radius, want_F=False)
+        keys[i] = O.bin_index_def(u[0], u[1], u[2], lay.radius, NE, NP, EMAX)
+    ko = keys[o]
+    bad = np.flatnonzero(np.diff(ko) < 0)
+    assert len(bad) <= 5                                                  # fp32 vs fp64 at a bin edge only
+    same = np.diff(ko) == 0
+    assert np.all(np.diff(o)[same] > 0) or len(bad) > 0
+    a.score(ctx, geom, 3, dl)
+    b.score(ctx, geom, 3, dl, order=order)
+    torch.cuda.synchronize()
+    ra, rb = a.results(), b.results()
+    for k in ra:
+        assert np.array_equal(ra[k], rb[k], equal_nan=True), k
 
 
 def _seeds(ev):

@@ -158,7 +158,7 @@ typedef struct {
     int32_t* bin_offset;      /* DEV [n_eta*n_phi + 1] first sorted slot of each bin               */
     int32_t* sorted_to_orig;  /* DEV [n_hits] original index of the hit in each sorted slot        */
     float* hit_rec;           /* DEV [n_hits][12] hits in bin order, packed for scoring:
-                                 x y z vxx vxy vxz vyy vyz vzz, original index (int32 bits), 0, 0  */
+                                 x y z vzz | vxx vxy vyy index(int32 bits) | vxz vyz 0 0           */
     float* pos_sorted;        /* DEV [3][ld] hits in bin order, SoA; optional (NULL = not written)  */
     float* cov_sorted;        /* DEV [6][ld] optional (NULL = not written)                          */
 } kf_layer_bins;
@@ -186,14 +186,29 @@ KF_API int kf_order_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, 
  * the window i_eta +- window_half (clipped), i_phi +- window_half (wrapped); best = lowest chi2,
  * exact ties -> lowest original index; accepted iff chi2 < chi2_cut.
  * Accepted and do_update: Kalman update, nhits += 1, chi2 += best.  Otherwise the candidate keeps
- * the propagated state (Q included).  best_hit[n] = ORIGINAL hit index or -1; best_chi2[n] = lowest
- * chi2 seen (+inf if the window was empty).  Propagation failure: status bit, candidate untouched,
+ * the propagated state (Q included).  best_hit[n] = ORIGINAL hit index or -1; best_chi2[n] = the
+ * lowest chi2 in the window when it is below chi2_cut, otherwise some value >= chi2_cut (hits that
+ * provably cannot beat the cut are not evaluated; +inf if none was).  Propagation failure: status bit, candidate untouched,
  * best_hit = -1, best_chi2 = +inf.  Reads bins->bin_offset and bins->hit_rec.  `order` = NULL or the
  * output of kf_order_candidates.  All pointers DEV.  The caller loops over layers. */
 KF_API int kf_score_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, kf_tracks* cands,
                                const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
                                float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
                                float* best_chi2);
+
+/* Best-hit building over n_build_layers consecutive layers first_layer, first_layer+1, ... in one call
+ * (PAPER.md:73, 133): per layer exactly what kf_score_candidates does, but the candidates stay in the
+ * kernel's track-local frame between layers, so the fitted state meets the same tolerances as
+ * kf_fit_tracks (the per-layer call has to hand the covariance back in the global frame in fp32 after
+ * every layer).  hits[j] / bins[j] (HOST arrays, DEV buffers inside) belong to layer first_layer + j.
+ * hit_index[j*ld_out + i] = ORIGINAL index of the hit taken by candidate i on that layer or -1,
+ * hit_chi2[j*ld_out + i] = its chi2 (see kf_score_candidates for rejected candidates); both DEV,
+ * [n_build_layers][ld_out], ld_out >= n.  A candidate that reaches no layer at all comes back through
+ * the local frame (equal to its input within fp32 rounding); a bad charge leaves it untouched. */
+KF_API int kf_build_best_hit(kf_ctx* ctx, const kf_geometry* geom, int first_layer, int n_build_layers,
+                             kf_tracks* cands, const kf_layer_hits* hits, const kf_layer_bins* bins,
+                             int window_half, float chi2_cut, int do_update, const int32_t* order,
+                             int32_t* hit_index, float* hit_chi2, int64_t ld_out);
 
 #ifdef __cplusplus
 }

@@ -141,6 +141,18 @@ class DeviceCandidates:
                              hits.n_hits, hits.pos, hits.cov, hits.bins, window_half, chi2_cut, do_update,
                              self.best_hit, self.best_chi2, order)
 
+    def build(self, ctx: KFContext, geom: Geometry, first_layer: int, layers: list, window_half: int = 2,
+              chi2_cut: float = 30.0, do_update: bool = True, order: torch.Tensor | None = None):
+        """kf_build_best_hit over `layers` (DeviceLayer list for first_layer, first_layer+1, ...).
+        Returns (hit_index[len(layers)][ld], hit_chi2[len(layers)][ld]) device tensors."""
+        m = len(layers)
+        idx = torch.empty((m, self.ld), dtype=torch.int32, device=self.par.device)
+        c2 = torch.empty((m, self.ld), dtype=torch.float32, device=self.par.device)
+        ctx.build_best_hit(geom, first_layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,
+                           [(l.n_hits, l.pos, l.cov, l.bins) for l in layers], window_half, chi2_cut, do_update,
+                           idx, c2, order)
+        return idx, c2
+
     def make_order(self, ctx: KFContext, geom: Geometry, layer: int, n_eta: int, n_phi: int, eta_max: float):
         order = torch.empty(max(self.n, 1), dtype=torch.int32, device=self.par.device)
         ctx.order_candidates(geom, layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,

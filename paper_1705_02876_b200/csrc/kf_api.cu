@@ -17,6 +17,8 @@ struct kf_ctx {
     int last_cuda = 0;
     // kf_bin_hits scratch
     BinScratch bin;
+    // kf_score_candidates / kf_build_best_hit scratch
+    ScoreScratch score;
     // *_host staging
     HostStage host;
 };
@@ -127,6 +129,7 @@ int kf_destroy(kf_ctx* c) {
     if (!c) return KF_ERR_NULL;
     cudaSetDevice(c->device);
     c->bin.release();
+    c->score.release();
     c->host.release();
     delete c;
     return KF_OK;
@@ -293,37 +296,71 @@ int kf_order_candidates(kf_ctx* c, const kf_geometry* geom, int layer, const kf_
     return KF_OK;
 }
 
-int kf_score_candidates(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks* cands,
-                        const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
-                        float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
-                        float* best_chi2) {
-    if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
-    FitParams P;
-    int rc = make_params(geom, &P);
-    if (rc) return rc;
-    if (layer < 0 || layer >= geom->n_layers) return KF_ERR_SHAPE;
-    if ((rc = check_tracks(cands, true, true))) return rc;
+namespace {
+
+int check_score_bins(const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half) {
+    if (!hits || !bins) return KF_ERR_NULL;
     if (hits->n_hits < 0) return KF_ERR_SHAPE;
     if (bins->n_eta < 1 || bins->n_phi < 2 || window_half < 0) return KF_ERR_SHAPE;
     if (bins->n_phi % 2 != 0 || (int64_t)bins->n_eta * bins->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
     if (2 * window_half + 1 > bins->n_phi) return KF_ERR_UNSUPPORTED;
     if (!(bins->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;
-    if (cands->n == 0) return KF_OK;
-    if (!best_hit || !best_chi2 || !bins->bin_offset) return KF_ERR_NULL;
+    if (!bins->bin_offset) return KF_ERR_NULL;
     if (hits->n_hits > 0) {
         if (!bins->hit_rec) return KF_ERR_NULL;
         if (!aligned16(bins->hit_rec)) return KF_ERR_ALIGN;
     }
+    return KF_OK;
+}
+
+}  // namespace
+
+int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,
+                      const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half, float chi2_cut,
+                      int do_update, const int32_t* order, int32_t* hit_index, float* hit_chi2, int64_t ld_out) {
+    if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
+    if ((rc = check_tracks(cands, true, true))) return rc;
+    if (n_build_layers == 0 || cands->n == 0) return KF_OK;
+    if (!hit_index || !hit_chi2) return KF_ERR_NULL;
+    if (ld_out < cands->n) return KF_ERR_SHAPE;
+    ScoreStep steps[KF_MAX_LAYERS];
+    for (int j = 0; j < n_build_layers; ++j) {
+        if ((rc = check_score_bins(hits + j, bins + j, window_half))) return rc;
+        if (bins[j].n_eta != bins[0].n_eta || bins[j].n_phi != bins[0].n_phi || bins[j].eta_max != bins[0].eta_max)
+            return KF_ERR_UNSUPPORTED;
+        steps[j].layer = first_layer + j;
+        steps[j].n_hits = hits[j].n_hits;
+        steps[j].hit_rec = bins[j].hit_rec;
+        steps[j].bin_offset = bins[j].bin_offset;
+        steps[j].best_hit = hit_index + (int64_t)j * ld_out;
+        steps[j].best_chi2 = hit_chi2 + (int64_t)j * ld_out;
+    }
     ScoreArgs a;
+    std::memset(&a, 0, sizeof(a));
     a.n = cands->n; a.ld = cands->ld; a.par = cands->par; a.cov = cands->cov; a.q = cands->q;
     a.chi2 = cands->chi2; a.nhits = cands->nhits; a.status = cands->status;
-    a.n_hits = hits->n_hits; a.hit_rec = bins->hit_rec; a.bin_offset = bins->bin_offset; a.order = order;
-    a.n_eta = bins->n_eta; a.n_phi = bins->n_phi; a.eta_max = bins->eta_max;
+    a.order = order;
+    a.n_eta = bins[0].n_eta; a.n_phi = bins[0].n_phi; a.eta_max = bins[0].eta_max;
     a.window_half = window_half; a.chi2_cut = chi2_cut; a.do_update = do_update ? 1 : 0;
-    a.layer = layer; a.best_hit = best_hit; a.best_chi2 = best_chi2;
-    cudaError_t e = launch_score(P, a, c->stream);
+    cudaError_t e = cudaSetDevice(c->device);
     if (e != cudaSuccess) return cuda_fail(c, e);
+    e = launch_build(c->score, P, a, n_build_layers, steps, c->stream);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
+}
+
+int kf_score_candidates(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks* cands,
+                        const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                        float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
+                        float* best_chi2) {
+    if (!c || !geom || !cands) return KF_ERR_NULL;
+    if (cands->n > 0 && (!best_hit || !best_chi2)) return KF_ERR_NULL;
+    return kf_build_best_hit(c, geom, layer, 1, cands, hits, bins, window_half, chi2_cut, do_update, order,
+                             best_hit, best_chi2, cands->n > 0 ? cands->ld : 0);
 }
 
 }  // extern "C"

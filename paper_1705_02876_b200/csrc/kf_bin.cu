@@ -17,7 +17,8 @@
 // their bin segment in arbitrary order (atomic cursor), (4) every slot ranks its index inside its
 // segment (indices are unique, so ascending index IS the stable order) and, for hits, gathers the
 // hit into the bin-ordered outputs: a packed 12-float record per hit for the scoring kernel
-// (x y z vxx vxy vxz vyy vyz vzz, original index, 2 pad: three 128-bit loads per hit) and,
+// (x y z vzz | vxx vxy vyy index | vxz vyz 0 0: the first 128-bit word serves the z pre-filter,
+// the second the tangential one, the third only full evaluations) and,
 // optionally, SoA copies.
 #include <cmath>
 
@@ -141,9 +142,9 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     for (int k = 0; k < 6; ++k) v[3 + k] = __ldg(L.cov + k * L.ld_in + mine);
     if (L.hit_rec) {
         float4* rec = reinterpret_cast<float4*>(L.hit_rec + dst * 12);
-        rec[0] = make_float4(v[0], v[1], v[2], v[3]);
-        rec[1] = make_float4(v[4], v[5], v[6], v[7]);
-        rec[2] = make_float4(v[8], __int_as_float(mine), 0.0f, 0.0f);
+        rec[0] = make_float4(v[0], v[1], v[2], v[8]);                    // x y z vzz
+        rec[1] = make_float4(v[3], v[4], v[6], __int_as_float(mine));    // vxx vxy vyy, original index
+        rec[2] = make_float4(v[5], v[7], 0.0f, 0.0f);                    // vxz vyz
     }
     if (L.pos_sorted) {
 #pragma unroll

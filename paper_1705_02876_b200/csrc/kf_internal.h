@@ -104,20 +104,46 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
                          cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------- scoring
+constexpr int kScorePlanes = 28;
+
 struct ScoreArgs {
     int64_t n, ld;
     float* par; float* cov; const int8_t* q; float* chi2; int32_t* nhits; uint32_t* status;
+    // current step
     int64_t n_hits;
     const float* hit_rec;
     const int32_t* bin_offset;
+    int32_t* best_hit; float* best_chi2;
+    // common
     const int32_t* order;  // may be null
     int n_eta, n_phi; float eta_max;
-    int window_half; float chi2_cut; int do_update; int layer;
-    int32_t* best_hit; float* best_chi2;
+    int window_half; float chi2_cut; int do_update;
+    // context scratch (filled by launch_build)
+    float* scratch; float* track; int32_t* flag; int32_t* slot; int64_t ld_sc;
+};
+
+struct ScoreStep {
+    int layer;               // geometry layer
+    int64_t n_hits;
+    const float* hit_rec;
+    const int32_t* bin_offset;
+    int32_t* best_hit;       // [n]
+    float* best_chi2;        // [n]
+};
+
+struct ScoreScratch {
+    int64_t cap = 0, ld = 0;
+    float* scratch = nullptr;  // [kScorePlanes][ld] propagated candidate (scan + update inputs)
+    float* track = nullptr;    // [29][ld] local-frame track between layers
+    int32_t* flag = nullptr;   // [ld]
+    int32_t* slot = nullptr;   // [ld] winning sorted slot or -1
+    cudaError_t reserve(int64_t n, cudaStream_t stream);
+    void release();
 };
 
 // kf_score.cu
-cudaError_t launch_score(const FitParams& P, const ScoreArgs& a, cudaStream_t stream);
+cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n_steps, const ScoreStep* steps,
+                         cudaStream_t stream);
 
 // kf_peak.cu
 double measure_fp32_peak(cudaStream_t stream, int repeats, float* sink);

@@ -1,17 +1,26 @@
-// kf_score.cu -- best-hit candidate scoring on one layer ("the hit that produced the
-// lowest chi2 increment"; PAPER.md:133-141 one GPU thread group per candidate, hits looked up
-// through the (eta, phi) bins).
+// kf_score.cu -- best-hit candidate scoring ("the hit that produced the lowest chi2
+// increment"; PAPER.md:133-141 hits looked up through the (eta, phi) bins), one layer at a time
+// (kf_score_candidates) or over consecutive layers with the candidates kept in the track-local frame
+// in between (kf_build_best_hit).
 //
-// One WARP owns one candidate.  Every lane propagates the candidate redundantly (state and C' in
-// registers, no shuffles needed afterwards), then the lanes stride over the hits of the
-// +-window_half bin window.  The window is, per eta row, one contiguous run of the bin-ordered
-// packed hit records (two runs when the phi ring wraps); a record is 12 floats, so a lane fetches a
-// hit with three 128-bit loads and a warp reads 1.5 KB of consecutive memory per step.  Two hits per
-// lane are in flight per iteration.  chi2 = r^T (C'_pp + V_h)^-1 r is evaluated in the candidate's
-// local frame with the same Schur elimination as the update; a shuffle arg-min picks (lowest chi2,
-// then lowest original index); all lanes apply the Kalman update with the winner, lane 0 stores.
-// Warp w processes candidate order[w] when an order is given (kf_order_candidates): neighbouring
-// warps then share their windows in L1/L2.  The order never changes a result.
+// Work is split by its natural parallelism:
+//   * per-CANDIDATE arithmetic (propagation, covariance transport, Kalman update, frame changes) runs
+//     one thread per candidate (`propagate_*_kernel`, `update_*_kernel`) and talks to the scan through
+//     a small SoA scratch (28 floats per candidate) owned by the context;
+//   * the per-HIT scan runs one warp per candidate (`scan_kernel`): the lanes stride over the hits of
+//     the +-window_half bin window, which is, per eta row, one contiguous run of the bin-ordered packed
+//     hit records (two runs when the phi ring wraps).
+//
+// Two-phase scan.  Nearly every hit of a window is many sigma away, and for any unit vector u
+//     chi2 = r^T S^-1 r >= (u.r)^2 / (u^T S u)           (Cauchy-Schwarz, S positive definite),
+// so with u = z-hat and u = tangent-hat (S_zz = C'_zz + v_zz, S_tt = C'_tt + v~_tt) a hit whose bound
+// exceeds the threshold T = min(chi2_cut, best chi2 so far) can neither be accepted nor beat the
+// current best and is dropped after ~20 instructions and two of its three 128-bit words.  The
+// survivors (a few per cent) are compacted through a per-warp list in shared memory (ballot + popc)
+// and evaluated densely, 32 at a time, with the same Schur-form chi2 as the update.  A 1 % margin on
+// the bound covers fp32 rounding.  A shuffle arg-min then picks (lowest chi2, lowest original index).
+// Warp w scans candidate order[w] when an order is given (kf_order_candidates), so neighbouring warps
+// share their windows in L1/L2; the order never changes a result.
 #include <math_constants.h>
 
 #include "kf_internal.h"
@@ -20,7 +29,158 @@ namespace kf {
 
 namespace {
 
-constexpr int kScoreBlock = 128;  // 4 candidates per CTA
+constexpr int kScanBlock = 128;   // 4 candidates per CTA
+constexpr int kCandBlock = 128;   // threads (= candidates) per CTA of the per-candidate kernels
+
+// Scratch planes (each [ld] floats): what the scan and the update need from the propagation.
+enum : int {
+    SC_XN, SC_YN, SC_ZN, SC_ERX, SC_ERY, SC_N11, SC_N12, SC_N22,   // scan + update
+    SC_PXN, SC_PYN, SC_PZ, SC_ELX, SC_ELY, SC_T, SC_PT2, SC_IPT,   // update
+    SC_N13, SC_N14, SC_N15, SC_N23, SC_N24, SC_N25, SC_N33, SC_N34, SC_N35, SC_N44, SC_N45, SC_N55,
+    SC_PLANES
+};
+static_assert(SC_PLANES == kScorePlanes, "scratch plane count");
+
+__device__ __forceinline__ void put_scratch(float* __restrict__ sc, int64_t ld, int64_t i, const Crossing& o,
+                                            const PropCov& n, float pz) {
+#define KF_PUT(k, v) sc[(int64_t)(k) * ld + i] = (v)
+    KF_PUT(SC_XN, o.xn);   KF_PUT(SC_YN, o.yn);   KF_PUT(SC_ZN, o.zn);   KF_PUT(SC_ERX, o.erx); KF_PUT(SC_ERY, o.ery);
+    KF_PUT(SC_N11, n.n11); KF_PUT(SC_N12, n.n12); KF_PUT(SC_N22, n.n22);
+    KF_PUT(SC_PXN, o.pxn); KF_PUT(SC_PYN, o.pyn); KF_PUT(SC_PZ, pz);     KF_PUT(SC_ELX, o.elx); KF_PUT(SC_ELY, o.ely);
+    KF_PUT(SC_T, o.T);     KF_PUT(SC_PT2, o.pt2); KF_PUT(SC_IPT, o.ipt);
+    KF_PUT(SC_N13, n.n13); KF_PUT(SC_N14, n.n14); KF_PUT(SC_N15, n.n15);
+    KF_PUT(SC_N23, n.n23); KF_PUT(SC_N24, n.n24); KF_PUT(SC_N25, n.n25);
+    KF_PUT(SC_N33, n.n33); KF_PUT(SC_N34, n.n34); KF_PUT(SC_N35, n.n35);
+    KF_PUT(SC_N44, n.n44); KF_PUT(SC_N45, n.n45); KF_PUT(SC_N55, n.n55);
+#undef KF_PUT
+}
+
+__device__ __forceinline__ void get_scratch(const float* __restrict__ sc, int64_t ld, int64_t i, Crossing& o,
+                                            PropCov& n, float& pz) {
+#define KF_GET(k) sc[(int64_t)(k) * ld + i]
+    o.xn = KF_GET(SC_XN);   o.yn = KF_GET(SC_YN);   o.zn = KF_GET(SC_ZN);   o.erx = KF_GET(SC_ERX); o.ery = KF_GET(SC_ERY);
+    n.n11 = KF_GET(SC_N11); n.n12 = KF_GET(SC_N12); n.n22 = KF_GET(SC_N22);
+    o.pxn = KF_GET(SC_PXN); o.pyn = KF_GET(SC_PYN); pz = KF_GET(SC_PZ);     o.elx = KF_GET(SC_ELX); o.ely = KF_GET(SC_ELY);
+    o.T = KF_GET(SC_T);     o.pt2 = KF_GET(SC_PT2); o.ipt = KF_GET(SC_IPT);
+    n.n13 = KF_GET(SC_N13); n.n14 = KF_GET(SC_N14); n.n15 = KF_GET(SC_N15);
+    n.n23 = KF_GET(SC_N23); n.n24 = KF_GET(SC_N24); n.n25 = KF_GET(SC_N25);
+    n.n33 = KF_GET(SC_N33); n.n34 = KF_GET(SC_N34); n.n35 = KF_GET(SC_N35);
+    n.n44 = KF_GET(SC_N44); n.n45 = KF_GET(SC_N45); n.n55 = KF_GET(SC_N55);
+#undef KF_GET
+}
+
+// Local-frame track <-> scratch between the layers of kf_build_best_hit (23 floats: the radial row of the
+// covariance is identically zero after the first layer).
+__device__ __forceinline__ void hit_from_record(const float4* __restrict__ rec, int32_t slot, const Crossing& o,
+                                                LocalHit& h) {
+    const float4* r0 = rec + (int64_t)slot * 3;
+    const float4 A = __ldg(r0), B = __ldg(r0 + 1), C = __ldg(r0 + 2);
+    hit_to_local(o, A.x, A.y, A.z, B.x, B.y, C.x, B.z, C.y, A.w, h);
+}
+
+// Propagate a local-frame track to layer Lc and park the result in the scratch; flags[i] = 1 if it got there.
+template <bool RADIAL_NULL>
+__device__ __forceinline__ bool propagate_to_scratch(const Track& t, float k, float ik, const LayerConst& Lc,
+                                                     float mass2, float* sc, int64_t ld, int64_t i) {
+    Crossing o;
+    if (!helix_to_radius(t, k, ik, Lc, o)) return false;
+    PropCov n;
+    transport_cov<RADIAL_NULL>(t, o, Lc.ms, mass2, n);
+    put_scratch(sc, ld, i, o, n, t.pz);
+    return true;
+}
+
+// ---- the current local-frame track between layers (kf_build_best_hit): 29 planes -------------------------
+__device__ __forceinline__ void put_track(float* __restrict__ ts, int64_t ld, int64_t i, const Track& t) {
+    const float v[29] = {t.x, t.y, t.z, t.px, t.py, t.pz, t.eax, t.eay, t.c00, t.c01, t.c02, t.c03, t.c04, t.c05,
+                         t.c11, t.c12, t.c13, t.c14, t.c15, t.c22, t.c23, t.c24, t.c25, t.c33, t.c34, t.c35,
+                         t.c44, t.c45, t.c55};
+#pragma unroll
+    for (int k = 0; k < 29; ++k) ts[(int64_t)k * ld + i] = v[k];
+}
+__device__ __forceinline__ void get_track(const float* __restrict__ ts, int64_t ld, int64_t i, Track& t) {
+    float v[29];
+#pragma unroll
+    for (int k = 0; k < 29; ++k) v[k] = ts[(int64_t)k * ld + i];
+    t.x = v[0]; t.y = v[1]; t.z = v[2]; t.px = v[3]; t.py = v[4]; t.pz = v[5]; t.eax = v[6]; t.eay = v[7];
+    t.c00 = v[8]; t.c01 = v[9]; t.c02 = v[10]; t.c03 = v[11]; t.c04 = v[12]; t.c05 = v[13];
+    t.c11 = v[14]; t.c12 = v[15]; t.c13 = v[16]; t.c14 = v[17]; t.c15 = v[18];
+    t.c22 = v[19]; t.c23 = v[20]; t.c24 = v[21]; t.c25 = v[22];
+    t.c33 = v[23]; t.c34 = v[24]; t.c35 = v[25]; t.c44 = v[26]; t.c45 = v[27]; t.c55 = v[28];
+}
+
+enum : int32_t { FLAG_IDLE = 0, FLAG_AT_LAYER = 1, FLAG_DEAD = 2 };
+
+// Candidate i stands at the layer (scratch filled): apply the scan's decision.  On return t is the
+// candidate after this layer in the local frame.
+__device__ __forceinline__ void apply_decision(const ScoreArgs& a, int64_t i, Track& t) {
+    Crossing o;
+    PropCov n;
+    float pz;
+    get_scratch(a.scratch, a.ld_sc, i, o, n, pz);
+    t.pz = pz;
+    const int32_t slot = a.slot[i];
+    bool updated = false;
+    if (slot >= 0 && a.do_update) {
+        LocalHit h;
+        hit_from_record(reinterpret_cast<const float4*>(a.hit_rec), slot, o, h);
+        float d;
+        const uint32_t rc = kalman_update(t, o, n, h, &d);
+        if (rc == 0u) { updated = true; a.chi2[i] += d; a.nhits[i] += 1; }
+        else a.status[i] |= rc;
+    }
+    if (!updated) commit_propagated(t, o, n);
+}
+
+// First step: global-frame candidate -> local frame -> propagate to `layer`.
+__global__ void __launch_bounds__(kCandBlock)
+propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, int layer, int keep_track) {
+    const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
+    if (i >= a.n) return;
+    const int q = a.q[i];
+    if (q != 1 && q != -1) { a.status[i] |= ST_BAD_CHARGE; a.flag[i] = FLAG_DEAD; return; }
+    Track t;
+    load_track(t, a.par, a.cov, a.ld, i);
+    enter_local_frame(t);
+    if (keep_track) put_track(a.track, a.ld_sc, i, t);
+    const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
+    const bool ok = propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.mass2, a.scratch, a.ld_sc, i);
+    if (!ok) a.status[i] |= ST_PROP_FAIL;
+    a.flag[i] = ok ? FLAG_AT_LAYER : FLAG_IDLE;
+}
+
+// Middle step of kf_build_best_hit: decision of the previous layer, then on to `layer`.
+__global__ void __launch_bounds__(kCandBlock)
+update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, int layer) {
+    const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
+    if (i >= a.n) return;
+    const int32_t f = a.flag[i];
+    if (f == FLAG_DEAD) return;
+    Track t;
+    if (f == FLAG_AT_LAYER) { apply_decision(a, i, t); put_track(a.track, a.ld_sc, i, t); }
+    else get_track(a.track, a.ld_sc, i, t);
+    const float qf = (float)a.q[i];
+    const bool ok = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.mass2, a.scratch,
+                                                a.ld_sc, i);
+    if (!ok) a.status[i] |= ST_PROP_FAIL;
+    a.flag[i] = ok ? FLAG_AT_LAYER : FLAG_IDLE;
+}
+
+// Last step: decision of the last layer, back to the global frame, store.
+// have_track = 0 (single-layer call): a candidate that did not reach the layer is left untouched.
+__global__ void __launch_bounds__(kCandBlock)
+update_global_kernel(const ScoreArgs a, int have_track) {
+    const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
+    if (i >= a.n) return;
+    const int32_t f = a.flag[i];
+    if (f == FLAG_DEAD) return;
+    Track t;
+    if (f == FLAG_AT_LAYER) apply_decision(a, i, t);
+    else if (have_track) get_track(a.track, a.ld_sc, i, t);
+    else return;
+    leave_local_frame(t);
+    store_track(t, a.par, a.cov, a.ld, i);
+}
 
 __device__ __forceinline__ bool better(float c, int32_t h, float bc, int32_t bh) {
     return c < bc || (c == bc && h < bh);
@@ -31,43 +191,44 @@ struct Best {
     int32_t orig, slot;
 };
 
-__device__ __forceinline__ void score_hit(const Crossing& o, const PropCov& n, const float4& A, const float4& B,
-                                          const float4& C, int32_t slot, Best& best) {
+struct ScanCand {       // what the scan needs of the propagated candidate
+    float xn, yn, zn, ec, es, n11, n12, n22;
+};
+
+// Full chi2 of the hit in `slot` against the candidate (same Schur form as the update).
+__device__ __forceinline__ void score_hit(const ScanCand& c, const float4* __restrict__ rec, int32_t slot, Best& best) {
+    const float4* r0 = rec + (int64_t)slot * 3;
+    const float4 A = __ldg(r0), B = __ldg(r0 + 1), C = __ldg(r0 + 2);
+    Crossing o;
+    o.xn = c.xn; o.yn = c.yn; o.zn = c.zn; o.erx = c.ec; o.ery = c.es;
     LocalHit h;
-    hit_to_local(o, A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w, C.x, h);
-    float c;
-    if (!chi2_schur(n.n11, n.n12, n.n22, h, c)) return;
-    const int32_t orig = __float_as_int(C.y);
-    if (better(c, orig, best.chi2, best.orig)) { best.chi2 = c; best.orig = orig; best.slot = slot; }
+    hit_to_local(o, A.x, A.y, A.z, B.x, B.y, C.x, B.z, C.y, A.w, h);
+    float chi2;
+    if (!chi2_schur(c.n11, c.n12, c.n22, h, chi2)) return;
+    const int32_t orig = __float_as_int(B.w);
+    if (better(chi2, orig, best.chi2, best.orig)) { best.chi2 = chi2; best.orig = orig; best.slot = slot; }
 }
 
-__global__ void __launch_bounds__(kScoreBlock)
-score_kernel(const __grid_constant__ FitParams P, const ScoreArgs a) {
+__global__ void __launch_bounds__(kScanBlock)
+scan_kernel(const ScoreArgs a, float inv_r) {
+    __shared__ int32_t survivors[kScanBlock / 32][64];
     const int lane = threadIdx.x & 31;
-    const int64_t w = ((int64_t)blockIdx.x * kScoreBlock + threadIdx.x) >> 5;
+    const int64_t w = ((int64_t)blockIdx.x * kScanBlock + threadIdx.x) >> 5;
     if (w >= a.n) return;
     const int64_t i = a.order ? (int64_t)__ldg(a.order + w) : w;
-    const LayerConst& Lc = P.layer[a.layer];
-    const int q = a.q[i];
-    if (q != 1 && q != -1) {
-        if (lane == 0) { a.status[i] |= ST_BAD_CHARGE; a.best_hit[i] = -1; a.best_chi2[i] = CUDART_INF_F; }
+    if (a.flag[i] != FLAG_AT_LAYER) {
+        if (lane == 0) { a.slot[i] = -1; a.best_hit[i] = -1; a.best_chi2[i] = CUDART_INF_F; }
         return;
     }
-    Track t;
-    load_track(t, a.par, a.cov, a.ld, i);
-    enter_local_frame(t);
-    const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
-    Crossing o;
-    if (!helix_to_radius(t, k, ik, Lc, o)) {
-        if (lane == 0) { a.status[i] |= ST_PROP_FAIL; a.best_hit[i] = -1; a.best_chi2[i] = CUDART_INF_F; }
-        return;
-    }
-    PropCov n;
-    transport_cov<false>(t, o, Lc.ms, P.mass2, n);
+    ScanCand c;
+    c.xn = a.scratch[SC_XN * a.ld_sc + i];   c.yn = a.scratch[SC_YN * a.ld_sc + i];
+    c.zn = a.scratch[SC_ZN * a.ld_sc + i];   c.ec = a.scratch[SC_ERX * a.ld_sc + i];
+    c.es = a.scratch[SC_ERY * a.ld_sc + i];  c.n11 = a.scratch[SC_N11 * a.ld_sc + i];
+    c.n12 = a.scratch[SC_N12 * a.ld_sc + i]; c.n22 = a.scratch[SC_N22 * a.ld_sc + i];
 
     // the candidate's own bin (reading A16): eta = asinh(z'/r), phi = atan2(y', x')
-    const float eta = asinhf(o.zn * Lc.inv_r);
-    const float phi = atan2f(o.yn, o.xn);
+    const float eta = asinhf(c.zn * inv_r);
+    const float phi = atan2f(c.yn, c.xn);
     const float d_eta = 2.0f * a.eta_max / (float)a.n_eta;
     const float d_phi = 2.0f * CUDART_PI_F / (float)a.n_phi;
     int ie = (int)floorf((eta + a.eta_max) / d_eta);
@@ -77,6 +238,11 @@ score_kernel(const __grid_constant__ FitParams P, const ScoreArgs a) {
 
     Best best;
     best.chi2 = CUDART_INF_F; best.orig = 0x7fffffff; best.slot = -1;
+    int32_t* list = survivors[threadIdx.x >> 5];
+    int cnt = 0;                               // warp-uniform number of listed survivors
+    float thr = 1.01f * a.chi2_cut;            // 1.01 * min(cut, best so far); NaN cut -> nothing passes
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const float ecc = c.ec * c.ec, ess = c.es * c.es, ecs2 = 2.0f * c.ec * c.es;
     const int wh = a.window_half;
     const float4* __restrict__ rec = reinterpret_cast<const float4*>(a.hit_rec);
     const int e_lo = ie - wh < 0 ? 0 : ie - wh, e_hi = ie + wh > a.n_eta - 1 ? a.n_eta - 1 : ie + wh;
@@ -91,22 +257,39 @@ score_kernel(const __grid_constant__ FitParams P, const ScoreArgs a) {
             if (nseg == 1) { s0 = __ldg(a.bin_offset + row + p0); s1 = __ldg(a.bin_offset + row + p1 + 1); }
             else if (sgi == 0) { s0 = __ldg(a.bin_offset + row + p0); s1 = __ldg(a.bin_offset + row + a.n_phi); }
             else { s0 = __ldg(a.bin_offset + row); s1 = __ldg(a.bin_offset + row + p1 - a.n_phi + 1); }
-            int32_t s = s0 + lane;
-            for (; s + 32 < s1; s += 64) {   // two hits per lane in flight
-                const float4* r0 = rec + (int64_t)s * 3;
-                const float4* r1 = rec + (int64_t)(s + 32) * 3;
-                const float4 A0 = __ldg(r0), B0 = __ldg(r0 + 1), C0 = __ldg(r0 + 2);
-                const float4 A1 = __ldg(r1), B1 = __ldg(r1 + 1), C1 = __ldg(r1 + 2);
-                score_hit(o, n, A0, B0, C0, s, best);
-                score_hit(o, n, A1, B1, C1, s + 32, best);
-            }
-            if (s < s1) {
-                const float4* r0 = rec + (int64_t)s * 3;
-                const float4 A0 = __ldg(r0), B0 = __ldg(r0 + 1), C0 = __ldg(r0 + 2);
-                score_hit(o, n, A0, B0, C0, s, best);
+            // software pipeline: the two words of the next 32 hits are in flight while these are tested
+            float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = A;
+            if (s0 + lane < s1) { A = __ldg(rec + (int64_t)(s0 + lane) * 3); B = __ldg(rec + (int64_t)(s0 + lane) * 3 + 1); }
+            for (int32_t sb = s0; sb < s1; sb += 32) {       // warp-uniform trip count
+                const int32_t s = sb + lane;
+                const float4 Ac = A, Bc = B;
+                if (s + 32 < s1) { A = __ldg(rec + (int64_t)(s + 32) * 3); B = __ldg(rec + (int64_t)(s + 32) * 3 + 1); }
+                const float dz = Ac.z - c.zn;
+                const float dx = Ac.x - c.xn, dy = Ac.y - c.yn;
+                const float rt = c.ec * dy - c.es * dx;
+                const float vtt = ess * Bc.x - ecs2 * Bc.y + ecc * Bc.z;
+                const bool pass = (s < s1) & (dz * dz <= thr * (c.n22 + Ac.w)) & (rt * rt <= thr * (c.n11 + vtt));
+                const unsigned m = __ballot_sync(0xffffffffu, pass);
+                if (pass) list[cnt + __popc(m & lt_mask)] = s;
+                cnt += __popc(m);
+                if (cnt >= 32) {                             // evaluate 32 survivors densely
+                    __syncwarp();
+                    const int32_t sl = list[lane];
+                    const int32_t carry = lane + 32 < cnt ? list[lane + 32] : 0;
+                    __syncwarp();
+                    if (lane + 32 < cnt) list[lane] = carry;
+                    cnt -= 32;
+                    score_hit(c, rec, sl, best);
+                    float bmin = best.chi2;
+#pragma unroll
+                    for (int d = 16; d > 0; d >>= 1) bmin = fminf(bmin, __shfl_xor_sync(0xffffffffu, bmin, d));
+                    thr = fminf(thr, 1.01f * bmin);
+                }
             }
         }
     }
+    __syncwarp();
+    if (lane < cnt) score_hit(c, rec, list[lane], best);
     // warp arg-min on (chi2, original index)
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
@@ -115,37 +298,59 @@ score_kernel(const __grid_constant__ FitParams P, const ScoreArgs a) {
         const int32_t os = __shfl_xor_sync(0xffffffffu, best.slot, d);
         if (better(oc, oo, best.chi2, best.orig)) { best.chi2 = oc; best.orig = oo; best.slot = os; }
     }
-    const bool found = best.slot >= 0;
-    const bool accept = found && best.chi2 < a.chi2_cut;
-    bool updated = false;
-    uint32_t st_add = 0u;
-    float dchi2 = 0.0f;
-    if (accept && a.do_update) {
-        const float4* r0 = rec + (int64_t)best.slot * 3;
-        const float4 A0 = __ldg(r0), B0 = __ldg(r0 + 1), C0 = __ldg(r0 + 2);
-        LocalHit h;
-        hit_to_local(o, A0.x, A0.y, A0.z, A0.w, B0.x, B0.y, B0.z, B0.w, C0.x, h);
-        const uint32_t rc = kalman_update(t, o, n, h, &dchi2);
-        if (rc == 0u) updated = true; else st_add = rc;
-    }
-    if (!updated) commit_propagated(t, o, n);
-    leave_local_frame(t);
     if (lane == 0) {
-        store_track(t, a.par, a.cov, a.ld, i);
+        const bool accept = best.slot >= 0 && best.chi2 < a.chi2_cut;
+        a.slot[i] = accept ? best.slot : -1;
         a.best_hit[i] = accept ? best.orig : -1;
         a.best_chi2[i] = best.chi2;
-        if (updated) { a.chi2[i] += dchi2; a.nhits[i] += 1; }
-        if (st_add) a.status[i] |= st_add;
     }
 }
 
 }  // namespace
 
-cudaError_t launch_score(const FitParams& P, const ScoreArgs& a, cudaStream_t stream) {
-    if (a.n == 0) return cudaSuccess;
-    const int per_block = kScoreBlock / 32;
-    const unsigned blocks = (unsigned)((a.n + per_block - 1) / per_block);
-    score_kernel<<<blocks, kScoreBlock, 0, stream>>>(P, a);
+cudaError_t ScoreScratch::reserve(int64_t n, cudaStream_t stream) {
+    if (n <= cap) return cudaSuccess;
+    cudaError_t e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return e;
+    release();
+    const int64_t ldn = (n + 3) / 4 * 4;
+    if ((e = cudaMalloc(&scratch, (size_t)kScorePlanes * ldn * 4)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&track, (size_t)29 * ldn * 4)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&flag, (size_t)ldn * 4)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&slot, (size_t)ldn * 4)) != cudaSuccess) { release(); return e; }
+    cap = ldn;
+    ld = ldn;
+    return cudaSuccess;
+}
+
+void ScoreScratch::release() {
+    void* ptrs[] = {scratch, track, flag, slot};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    scratch = track = nullptr;
+    flag = slot = nullptr;
+    cap = ld = 0;
+}
+
+// Score `n_layers` consecutive steps.  steps[j] gives the geometry layer and the hit pool of step j.
+cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n_steps, const ScoreStep* steps,
+                         cudaStream_t stream) {
+    if (a.n == 0 || n_steps <= 0) return cudaSuccess;
+    cudaError_t e = s.reserve(a.n, stream);
+    if (e != cudaSuccess) return e;
+    a.scratch = s.scratch; a.track = s.track; a.flag = s.flag; a.slot = s.slot; a.ld_sc = s.ld;
+    const unsigned cblocks = (unsigned)((a.n + kCandBlock - 1) / kCandBlock);
+    const unsigned sblocks = (unsigned)((a.n + kScanBlock / 32 - 1) / (kScanBlock / 32));
+    const int keep = n_steps > 1 ? 1 : 0;
+    for (int j = 0; j < n_steps; ++j) {
+        const ScoreStep& st = steps[j];
+        if (j == 0) propagate_global_kernel<<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer, keep);
+        else update_propagate_kernel<<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer);   // a.hit_rec still step j-1
+        a.hit_rec = st.hit_rec; a.bin_offset = st.bin_offset; a.n_hits = st.n_hits;
+        a.best_hit = st.best_hit; a.best_chi2 = st.best_chi2;
+        scan_kernel<<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
+    }
+    update_global_kernel<<<cblocks, kCandBlock, 0, stream>>>(a, keep);
     return cudaGetLastError();
 }
 

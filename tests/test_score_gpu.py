@@ -37,8 +37,10 @@ def _assert_bins_equal(dl, ob, pos, cov):
     assert np.array_equal(dl.bins.pos_sorted.cpu().numpy()[:, :H], pos[:, s2o])
     assert np.array_equal(dl.bins.cov_sorted.cpu().numpy()[:, :H], cov[:, s2o])
     rec = dl.bins.hit_rec.cpu().numpy()[:H]
-    assert np.array_equal(rec[:, 0:3], pos[:, s2o].T) and np.array_equal(rec[:, 3:9], cov[:, s2o].T)
-    assert np.array_equal(rec[:, 9].copy().view(np.int32), s2o)
+    cs = cov[:, s2o].T                                      # xx xy xz yy yz zz
+    assert np.array_equal(rec[:, 0:3], pos[:, s2o].T) and np.array_equal(rec[:, 3], cs[:, 5])
+    assert np.array_equal(rec[:, 4:7], cs[:, [0, 1, 3]]) and np.array_equal(rec[:, 8:10], cs[:, [2, 4]])
+    assert np.array_equal(rec[:, 7].copy().view(np.int32), s2o)
 
 
 @pytest.mark.parametrize("n_tracks,noise", [(400, 2000), (20000, 100000)])
@@ -180,6 +182,63 @@ def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
         res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0, loosen=dict(cov=10.0, mom=3.0))
         print("scoring state parity:", res)
     return n_dec, n_tie
+
+
+def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0):
+    """kf_build_best_hit over layers 3..9 in one call vs the oracle's layer loop: decisions by north_star's
+    rule, final state at the FIT tolerances (the candidates never leave the local frame)."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    f, cfg = ev.fit, ev.cfg
+    par, cov, chi2, nh = _seeds(ev)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+    dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    L0 = cfg.first_scored_layer
+    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers[L0:]]
+    ctx.bin_layers([l.radius for l in ev.layers[L0:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+    order = dc.make_order(ctx, geom, L0, NE, NP, EMAX) if use_order else None
+    idx, c2 = dc.build(ctx, geom, L0, dls, 2, 30.0, True, order)
+    torch.cuda.synchronize()
+    idx, c2 = idx.cpu().numpy()[:, :f.n], c2.cpu().numpy()[:, :f.n]
+    oc = O.Candidates(par, cov, f.q, chi2, nh)
+    alive = np.ones(f.n, dtype=bool)
+    n_dec = n_tie = 0
+    for j, l in enumerate(range(L0, cfg.n_layers)):
+        lay = ev.layers[l]
+        ob = O.bin_hits(lay.pos, lay.radius, NE, NP, EMAX)
+        orr = O.score_layer(oc, lay.radius, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NE, NP, EMAX, 2, 30.0, True)
+        diff = (idx[j] != orr["best_hit"]) & alive
+        b, s2 = orr["best_chi2"], orr["second_chi2"]
+        tie = (np.abs(s2 - b) <= 1e-4 * np.abs(b)) | (np.abs(b - 30.0) <= 1e-4 * 30.0)
+        assert not np.any(diff & ~tie), f"layer {l}: {int((diff & ~tie).sum())} mismatches outside the tie window"
+        n_dec += int(alive.sum()); n_tie += int(diff.sum())
+        alive &= ~diff
+        acc = alive & (orr["best_hit"] >= 0)
+        assert (np.abs(c2[j][acc] - b[acc]) / np.maximum(b[acc], 1.0)).max(initial=0) < 2e-3
+    g = dc.results()
+    sel = alive & (oc.status == 0)
+    assert np.array_equal(g["status"][alive], oc.status[alive]) and np.array_equal(g["nhits"][alive], oc.nhits[alive])
+    sub_g = {k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in ("par", "cov", "chi2", "nhits", "status")}
+    sub_o = dict(par=oc.par.T[:, sel], cov=oc.cov[sel], chi2=oc.chi2[sel], nhits=oc.nhits[sel], status=oc.status[sel])
+    # north_star fixes only the hit decisions for scoring; the state is held to the fit tolerances, except
+    # that with 100 000 noise hits per layer some candidates take wrong hits with chi2 up to 30 and kink by
+    # many sigma, where both filters linearise far from the truth: covariance 3e-3 there (worst seen 1.4e-3)
+    res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0, loosen=dict(cov=cov_loosen))
+    print("fused building state parity:", res)
+    return n_dec, n_tie
+
+
+def test_build_best_hit_small_event(ctx):
+    ev = W.make_build_event(4, n_tracks=400, noise_hits=2000)
+    n_dec, _ = _build_event_fused(ctx, ev, use_order=False)
+    assert n_dec >= 0.99 * 7 * 400
+
+
+def test_build_best_hit_full_config4(ctx):
+    ev = W.make_build_event(4)
+    n_dec, n_tie = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0)
+    print(f"config 4 fused: {n_dec} decisions, {n_tie} differences inside the tie window")
+    assert n_dec >= 0.99 * 7 * 20000 and n_tie <= 20
 
 
 def test_score_small_event(ctx):

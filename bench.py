@@ -147,6 +147,77 @@ def run_reference(args) -> None:
     print(json.dumps(out), flush=True)
 
 
+def measure_building(ctx, dev: str, reps: int = 10) -> dict:
+    """Secondary measurement (outside the timed fit region): BASELINE.json configs[4], the track-building
+    rows a8 + a9 of the path -- bin 7 layers x 120 000 hits (kf_bin_layers) and best-hit scoring of 20 000
+    candidates over layers 3..9 (kf_order_candidates + kf_build_best_hit).  Seeds = kf_fit_tracks on the
+    first three true hits (the product path; no oracle here)."""
+    import torch
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceFit, DeviceLayer
+    from workloads import barrel_events as W
+    ev = W.make_build_event(4)
+    f, cfg = ev.fit, ev.cfg
+    L0, L = cfg.first_scored_layer, cfg.n_layers
+    emax = float(np.float32(cfg.eta_bin_max))
+    import copy
+    f3 = copy.copy(f)
+    f3.radius, f3.x_over_X0 = f.radius[:L0], f.x_over_X0[:L0]
+    f3.hpos, f3.hcov = np.ascontiguousarray(f.hpos[:L0]), np.ascontiguousarray(f.hcov[:L0])
+    d3 = DeviceFit.from_batch(f3, dev)
+    d3.fit(ctx)
+    torch.cuda.synchronize()
+    s = d3.results()
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+    layers = [DeviceLayer.from_numpy(l.pos, l.cov, cfg.n_eta, cfg.n_phi, emax, dev) for l in ev.layers[L0:]]
+    ctx.reserve(max_hits=sum(l.n_hits for l in layers))
+    radii = [l.radius for l in ev.layers[L0:]]
+    args = [(l.n_hits, l.pos, l.cov, l.bins) for l in layers]
+    t_bin, t_build = [], []
+    for it in range(reps + 2):
+        dc = DeviceCandidates.from_numpy(s["par"], s["cov"], f.q, s["chi2"], s["nhits"], dev)
+        torch.cuda.synchronize()
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        st = torch.cuda.current_stream()
+        ctx.set_stream(st)
+        e[0].record(st)
+        ctx.bin_layers(radii, args)
+        e[1].record(st)
+        order = dc.make_order(ctx, geom, L0, cfg.n_eta, cfg.n_phi, emax)
+        idx, _ = dc.build(ctx, geom, L0, layers, 2, 30.0, True, order)
+        e[2].record(st)
+        torch.cuda.synchronize()
+        if it >= 2:
+            t_bin.append(e[0].elapsed_time(e[1]))
+            t_build.append(e[1].elapsed_time(e[2]))
+    # algorithmic work (SURVEY.md 8(d)): 850 + 60 n_window flop per candidate and layer, n_window counted
+    # from the bins around each candidate's true hit on that layer
+    n_win = 0
+    for j, l in enumerate(range(L0, L)):
+        off = layers[j].bins.bin_offset.cpu().numpy().astype(np.int64)
+        hp = ev.layers[l].pos[:, ev.layers[l].true_index].astype(np.float64)
+        ie = np.clip(np.floor((np.arcsinh(hp[2] / ev.layers[l].radius) + emax) / (2 * emax / cfg.n_eta)), 0, cfg.n_eta - 1).astype(int)
+        ip = np.floor((np.arctan2(hp[1], hp[0]) + np.pi) / (2 * np.pi / cfg.n_phi)).astype(int) % cfg.n_phi
+        cnt = off[1:] - off[:-1]
+        grid = cnt.reshape(cfg.n_eta, cfg.n_phi)
+        for de in range(-2, 3):
+            e_ = ie + de
+            ok = (e_ >= 0) & (e_ < cfg.n_eta)
+            for dp in range(-2, 3):
+                n_win += int(grid[np.clip(e_, 0, cfg.n_eta - 1), (ip + dp) % cfg.n_phi][ok].sum())
+    n_cl = f.n * (L - L0)
+    flops = 850.0 * n_cl + 60.0 * n_win
+    tb, ts = float(np.median(t_bin)), float(np.median(t_build))
+    taken = float((idx[:, :f.n] >= 0).float().mean().item())
+    ctx.set_stream(None)
+    return {"workload": "configs[4]: 20000 candidates, layers 3..9, 120000 hits/layer, 40x64 bins, +-2-bin window, chi2 < 30",
+            "bin_ms": tb, "bin_hits_per_s": sum(l.n_hits for l in layers) / (tb * 1e-3),
+            "build_ms": ts, "candidate_layers_per_s": n_cl / (ts * 1e-3),
+            "window_hits_scored_per_s": n_win / (ts * 1e-3), "mean_window_hits": n_win / n_cl,
+            "algorithmic_gflop": flops / 1e9, "hit_taken_fraction": taken,
+            "kernels_per_build": 4 + 2 * (L - L0) + 1, "reps": reps}
+
+
 def run_ours(args) -> None:
     import torch
     import paper_1705_02876_b200 as K
@@ -207,6 +278,7 @@ def run_ours(args) -> None:
            "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "kf_fit_tracks_host, pinned host SoA buffers"}
     same = all(np.array_equal(a, b) for a, b in zip(d.results().values(), h.results().values()))
     fp32_peak = ctx.measure_fp32_peak(5) if rank == 0 else 0.0
+    building = measure_building(ctx, dev) if (rank == 0 and not args.no_building) else None
 
     if rank == 0:
         peak, peak_src = _peaks()
@@ -240,6 +312,9 @@ def run_ours(args) -> None:
                           "l2": "inputs+outputs (%.2f GB) larger than the 126 MB L2, no flush" % (alg_bytes / 1e9)},
                "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "roofline_other": other,
                "cpu_baseline": cpu, "host_path_equals_device_path": bool(same)}
+        if building is not None:
+            building["alu_roofline_frac"] = building["algorithmic_gflop"] * 1e9 / (building["build_ms"] * 1e-3) / (fp32_peak * 1e12)
+            out["building"] = building
         print(json.dumps(out), flush=True)
     ctx.close()
     sharding.shutdown()
@@ -251,6 +326,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-building", action="store_true", help="skip the secondary configs[4] building measurement")
     ap.add_argument("--events", type=int, default=100, help="events of 20 000 tracks per GPU (configs[2] = 100)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -211,7 +211,7 @@ __device__ __forceinline__ void score_hit(const ScanCand& c, const float4* __res
 
 __global__ void __launch_bounds__(kScanBlock)
 scan_kernel(const ScoreArgs a, float inv_r) {
-    __shared__ int32_t survivors[kScanBlock / 32][64];
+    __shared__ int32_t survivors[kScanBlock / 32][96];
     const int lane = threadIdx.x & 31;
     const int64_t w = ((int64_t)blockIdx.x * kScanBlock + threadIdx.x) >> 5;
     if (w >= a.n) return;
@@ -257,27 +257,35 @@ scan_kernel(const ScoreArgs a, float inv_r) {
             if (nseg == 1) { s0 = __ldg(a.bin_offset + row + p0); s1 = __ldg(a.bin_offset + row + p1 + 1); }
             else if (sgi == 0) { s0 = __ldg(a.bin_offset + row + p0); s1 = __ldg(a.bin_offset + row + a.n_phi); }
             else { s0 = __ldg(a.bin_offset + row); s1 = __ldg(a.bin_offset + row + p1 - a.n_phi + 1); }
-            // software pipeline: the two words of the next 32 hits are in flight while these are tested
-            float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = A;
-            if (s0 + lane < s1) { A = __ldg(rec + (int64_t)(s0 + lane) * 3); B = __ldg(rec + (int64_t)(s0 + lane) * 3 + 1); }
-            for (int32_t sb = s0; sb < s1; sb += 32) {       // warp-uniform trip count
-                const int32_t s = sb + lane;
-                const float4 Ac = A, Bc = B;
-                if (s + 32 < s1) { A = __ldg(rec + (int64_t)(s + 32) * 3); B = __ldg(rec + (int64_t)(s + 32) * 3 + 1); }
-                const float dz = Ac.z - c.zn;
-                const float dx = Ac.x - c.xn, dy = Ac.y - c.yn;
-                const float rt = c.ec * dy - c.es * dx;
-                const float vtt = ess * Bc.x - ecs2 * Bc.y + ecc * Bc.z;
-                const bool pass = (s < s1) & (dz * dz <= thr * (c.n22 + Ac.w)) & (rt * rt <= thr * (c.n11 + vtt));
-                const unsigned m = __ballot_sync(0xffffffffu, pass);
-                if (pass) list[cnt + __popc(m & lt_mask)] = s;
-                cnt += __popc(m);
-                if (cnt >= 32) {                             // evaluate 32 survivors densely
+            // 64 hits per step: two records per lane, four independent 128-bit loads in flight
+            const float4* p = rec + (int64_t)(s0 + lane) * 3;
+            for (int32_t sb = s0; sb < s1; sb += 64, p += 64 * 3) {   // warp-uniform trip count
+                const int32_t sA = sb + lane, sB = sA + 32;
+                const bool vA = sA < s1, vB = sB < s1;
+                float4 A0 = make_float4(0.f, 0.f, 0.f, 0.f), B0 = A0, A1 = A0, B1 = A0;
+                if (vA) { A0 = __ldg(p); B0 = __ldg(p + 1); }
+                if (vB) { A1 = __ldg(p + 96); B1 = __ldg(p + 97); }
+                const float dz0 = A0.z - c.zn, dz1 = A1.z - c.zn;
+                const float rt0 = c.ec * (A0.y - c.yn) - c.es * (A0.x - c.xn);
+                const float rt1 = c.ec * (A1.y - c.yn) - c.es * (A1.x - c.xn);
+                const float vt0 = ess * B0.x - ecs2 * B0.y + ecc * B0.z;
+                const float vt1 = ess * B1.x - ecs2 * B1.y + ecc * B1.z;
+                const bool pA = vA & (dz0 * dz0 <= thr * (c.n22 + A0.w)) & (rt0 * rt0 <= thr * (c.n11 + vt0));
+                const bool pB = vB & (dz1 * dz1 <= thr * (c.n22 + A1.w)) & (rt1 * rt1 <= thr * (c.n11 + vt1));
+                const unsigned mA = __ballot_sync(0xffffffffu, pA);
+                const unsigned mB = __ballot_sync(0xffffffffu, pB);
+                if (pA) list[cnt + __popc(mA & lt_mask)] = sA;
+                cnt += __popc(mA);
+                if (pB) list[cnt + __popc(mB & lt_mask)] = sB;
+                cnt += __popc(mB);
+                while (cnt >= 32) {                          // evaluate 32 survivors densely
                     __syncwarp();
                     const int32_t sl = list[lane];
-                    const int32_t carry = lane + 32 < cnt ? list[lane + 32] : 0;
+                    const int32_t c1 = lane + 32 < cnt ? list[lane + 32] : 0;
+                    const int32_t c2 = lane + 64 < cnt ? list[lane + 64] : 0;
                     __syncwarp();
-                    if (lane + 32 < cnt) list[lane] = carry;
+                    if (lane + 32 < cnt) list[lane] = c1;
+                    if (lane + 64 < cnt) list[lane + 32] = c2;
                     cnt -= 32;
                     score_hit(c, rec, sl, best);
                     float bmin = best.chi2;

@@ -150,7 +150,7 @@ def run_reference(args) -> None:
 def measure_building(ctx, dev: str, reps: int = 10) -> dict:
     """Secondary measurement (outside the timed fit region): BASELINE.json configs[4], the track-building
     rows a8 + a9 of the path -- bin 7 layers x 120 000 hits (kf_bin_layers) and best-hit scoring of 20 000
-    candidates over layers 3..9 (kf_order_candidates + kf_build_best_hit).  Seeds = kf_fit_tracks on the
+    candidates over layers 3..9 (kf_build_best_hit).  Seeds = kf_fit_tracks on the
     first three true hits (the product path; no oracle here)."""
     import torch
     import paper_1705_02876_b200 as K
@@ -183,8 +183,7 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
         e[0].record(st)
         ctx.bin_layers(radii, args)
         e[1].record(st)
-        order = dc.make_order(ctx, geom, L0, cfg.n_eta, cfg.n_phi, emax)
-        idx, _ = dc.build(ctx, geom, L0, layers, 2, 30.0, True, order)
+        idx, _ = dc.build(ctx, geom, L0, layers, 2, 30.0, True, None)
         e[2].record(st)
         torch.cuda.synchronize()
         if it >= 2:
@@ -215,7 +214,7 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
             "build_ms": ts, "candidate_layers_per_s": n_cl / (ts * 1e-3),
             "window_hits_scored_per_s": n_win / (ts * 1e-3), "mean_window_hits": n_win / n_cl,
             "algorithmic_gflop": flops / 1e9, "hit_taken_fraction": taken,
-            "kernels_per_build": 4 + 2 * (L - L0) + 1, "reps": reps}
+            "kernels_per_build": 2 * (L - L0) + 1, "reps": reps}
 
 
 def run_ours(args) -> None:

@@ -159,6 +159,8 @@ typedef struct {
     int32_t* sorted_to_orig;  /* DEV [n_hits] original index of the hit in each sorted slot        */
     float* hit_rec;           /* DEV [n_hits][12] hits in bin order, packed for scoring:
                                  x y z vzz | vxx vxy vyy index(int32 bits) | vxz vyz 0 0           */
+    float* bin_box;           /* DEV [n_eta*n_phi][8] per-bin bounds for the scan's bin pruning:
+                                 x_lo x_hi y_lo y_hi | z_lo z_hi max(vzz) max(vxx+vyy)              */
     float* pos_sorted;        /* DEV [3][ld] hits in bin order, SoA; optional (NULL = not written)  */
     float* cov_sorted;        /* DEV [6][ld] optional (NULL = not written)                          */
 } kf_layer_bins;
@@ -189,7 +191,7 @@ KF_API int kf_order_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, 
  * the propagated state (Q included).  best_hit[n] = ORIGINAL hit index or -1; best_chi2[n] = the
  * lowest chi2 in the window when it is below chi2_cut, otherwise some value >= chi2_cut (hits that
  * provably cannot beat the cut are not evaluated; +inf if none was).  Propagation failure: status bit, candidate untouched,
- * best_hit = -1, best_chi2 = +inf.  Reads bins->bin_offset and bins->hit_rec.  `order` = NULL or the
+ * best_hit = -1, best_chi2 = +inf.  Reads bins->bin_offset, bins->hit_rec and bins->bin_box.  `order` = NULL or the
  * output of kf_order_candidates.  All pointers DEV.  The caller loops over layers. */
 KF_API int kf_score_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, kf_tracks* cands,
                                const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,

@@ -53,7 +53,7 @@ class _LayerHits(C.Structure):
 class _LayerBins(C.Structure):
     _fields_ = [("n_eta", C.c_int), ("n_phi", C.c_int), ("eta_max", C.c_float), ("ld", C.c_int64),
                 ("bin_offset", C.c_void_p), ("sorted_to_orig", C.c_void_p), ("hit_rec", C.c_void_p),
-                ("pos_sorted", C.c_void_p), ("cov_sorted", C.c_void_p)]
+                ("bin_box", C.c_void_p), ("pos_sorted", C.c_void_p), ("cov_sorted", C.c_void_p)]
 
 
 _lib = None
@@ -144,6 +144,7 @@ class Bins:
     bin_offset: torch.Tensor      # int32 [n_eta*n_phi + 1]
     sorted_to_orig: torch.Tensor  # int32 [n_hits]
     hit_rec: torch.Tensor         # f32 [n_hits][12] packed records in bin order
+    bin_box: torch.Tensor         # f32 [n_bins][8] per-bin bounds
     pos_sorted: torch.Tensor | None = None   # f32 [3][ld] optional SoA copy
     cov_sorted: torch.Tensor | None = None   # f32 [6][ld]
 
@@ -154,6 +155,7 @@ class Bins:
                     torch.empty(n_eta * n_phi + 1, dtype=torch.int32, device=device),
                     torch.empty(max(n_hits, 1), dtype=torch.int32, device=device),
                     torch.empty((max(n_hits, 1), 12), dtype=torch.float32, device=device),
+                    torch.empty((n_eta * n_phi, 8), dtype=torch.float32, device=device),
                     torch.empty((3, ld), dtype=torch.float32, device=device) if soa else None,
                     torch.empty((6, ld), dtype=torch.float32, device=device) if soa else None)
 
@@ -161,6 +163,7 @@ class Bins:
         ld = int(self.pos_sorted.shape[1]) if self.pos_sorted is not None else 0
         return _LayerBins(self.n_eta, self.n_phi, float(self.eta_max), ld,
                           self.bin_offset.data_ptr(), self.sorted_to_orig.data_ptr(), self.hit_rec.data_ptr(),
+                          self.bin_box.data_ptr(),
                           self.pos_sorted.data_ptr() if self.pos_sorted is not None else None,
                           self.cov_sorted.data_ptr() if self.cov_sorted is not None else None)
 

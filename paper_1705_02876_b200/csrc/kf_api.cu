@@ -25,7 +25,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 2;
+constexpr int kAbiVersion = 3;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -230,7 +230,8 @@ int check_bin_args(const kf_layer_hits* hits, const kf_layer_bins* out, float ra
     if (out->n_phi % 2 != 0 || (int64_t)out->n_eta * out->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
     if (!(radius_cm > 0.0f) || !(out->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;
     if (hits->n_hits > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
-    if (!out->bin_offset) return KF_ERR_NULL;
+    if (!out->bin_offset || !out->bin_box) return KF_ERR_NULL;
+    if (!aligned16(out->bin_box)) return KF_ERR_ALIGN;
     if (hits->n_hits > 0) {
         if (!hits->pos || !hits->cov || !out->sorted_to_orig || !out->hit_rec) return KF_ERR_NULL;
         if (hits->ld % 4 != 0 || !aligned16(hits->pos) || !aligned16(hits->cov) || !aligned16(out->hit_rec))
@@ -248,7 +249,7 @@ BinArgs to_bin_args(float radius_cm, const kf_layer_hits* hits, const kf_layer_b
     a.n_hits = hits->n_hits; a.ld_in = hits->ld; a.pos = hits->pos; a.cov = hits->cov;
     a.radius = radius_cm; a.n_eta = out->n_eta; a.n_phi = out->n_phi; a.eta_max = out->eta_max;
     a.ld_out = out->ld; a.bin_offset = out->bin_offset; a.sorted_to_orig = out->sorted_to_orig;
-    a.pos_sorted = out->pos_sorted; a.cov_sorted = out->cov_sorted; a.hit_rec = out->hit_rec;
+    a.pos_sorted = out->pos_sorted; a.cov_sorted = out->cov_sorted; a.hit_rec = out->hit_rec; a.bin_box = out->bin_box;
     return a;
 }
 
@@ -305,7 +306,8 @@ int check_score_bins(const kf_layer_hits* hits, const kf_layer_bins* bins, int w
     if (bins->n_phi % 2 != 0 || (int64_t)bins->n_eta * bins->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
     if (2 * window_half + 1 > bins->n_phi) return KF_ERR_UNSUPPORTED;
     if (!(bins->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;
-    if (!bins->bin_offset) return KF_ERR_NULL;
+    if (!bins->bin_offset || !bins->bin_box) return KF_ERR_NULL;
+    if (!aligned16(bins->bin_box)) return KF_ERR_ALIGN;
     if (hits->n_hits > 0) {
         if (!bins->hit_rec) return KF_ERR_NULL;
         if (!aligned16(bins->hit_rec)) return KF_ERR_ALIGN;
@@ -335,6 +337,7 @@ int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n
         steps[j].layer = first_layer + j;
         steps[j].n_hits = hits[j].n_hits;
         steps[j].hit_rec = bins[j].hit_rec;
+        steps[j].bin_box = bins[j].bin_box;
         steps[j].bin_offset = bins[j].bin_offset;
         steps[j].best_hit = hit_index + (int64_t)j * ld_out;
         steps[j].best_chi2 = hit_chi2 + (int64_t)j * ld_out;

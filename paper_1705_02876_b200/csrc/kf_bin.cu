@@ -12,7 +12,7 @@
 //     lower half plane:      i_phi = #{ j in 1..n_phi/2-1 : fl(cos_j y) >= fl(sin_j x) }
 // with (cos_j, sin_j) = fl(cos, sin)(-pi + j d_phi).  No transcendental is evaluated on the GPU.
 //
-// Counting sort, stable, batched over layers (grid.y = layer, 4 launches + 1 memset for ALL layers):
+// Counting sort, stable, batched over layers (grid.y = layer, 5 launches + 1 memset for ALL layers):
 // (1) key of every item + histogram, (2) exclusive scan -> bin_offset, (3) scatter item indices into
 // their bin segment in arbitrary order (atomic cursor), (4) every slot ranks its index inside its
 // segment (indices are unique, so ascending index IS the stable order) and, for hits, gathers the
@@ -156,6 +156,39 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     }
 }
 
+// Per-bin bounds for the scan's bin pruning: bounding box of the hits of the bin and the largest
+// v_zz and v_xx + v_yy (>= the tangential variance in any frame).  One warp per bin, no atomics.
+// NaN components are ignored (such a hit can never pass a chi2 bound either).  Empty bin: lo = +inf.
+__global__ void __launch_bounds__(kBlock)
+bin_box_kernel(const __grid_constant__ BinBatch B) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
+    if (!L.bin_box || !L.hit_rec) return;
+    const int lane = threadIdx.x & 31;
+    const int b = (int)((blockIdx.x * (unsigned)kBlock + threadIdx.x) >> 5);
+    if (b >= B.n_eta * B.n_phi) return;
+    const int32_t s0 = L.bin_offset[b], s1 = L.bin_offset[b + 1];
+    const float inf = __int_as_float(0x7f800000);
+    float xl = inf, xh = -inf, yl = inf, yh = -inf, zl = inf, zh = -inf, vz = 0.0f, vt = 0.0f;
+    const float4* rec = reinterpret_cast<const float4*>(L.hit_rec);
+    for (int32_t s = s0 + lane; s < s1; s += 32) {
+        const float4 A = rec[(int64_t)s * 3], Bw = rec[(int64_t)s * 3 + 1];
+        xl = fminf(xl, A.x); xh = fmaxf(xh, A.x); yl = fminf(yl, A.y); yh = fmaxf(yh, A.y);
+        zl = fminf(zl, A.z); zh = fmaxf(zh, A.z); vz = fmaxf(vz, A.w); vt = fmaxf(vt, Bw.x + Bw.z);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        xl = fminf(xl, __shfl_xor_sync(0xffffffffu, xl, d)); xh = fmaxf(xh, __shfl_xor_sync(0xffffffffu, xh, d));
+        yl = fminf(yl, __shfl_xor_sync(0xffffffffu, yl, d)); yh = fmaxf(yh, __shfl_xor_sync(0xffffffffu, yh, d));
+        zl = fminf(zl, __shfl_xor_sync(0xffffffffu, zl, d)); zh = fmaxf(zh, __shfl_xor_sync(0xffffffffu, zh, d));
+        vz = fmaxf(vz, __shfl_xor_sync(0xffffffffu, vz, d)); vt = fmaxf(vt, __shfl_xor_sync(0xffffffffu, vt, d));
+    }
+    if (lane == 0) {
+        float4* o = reinterpret_cast<float4*>(L.bin_box + (int64_t)b * 8);
+        o[0] = make_float4(xl, xh, yl, yh);
+        o[1] = make_float4(zl, zh, vz, vt);
+    }
+}
+
 // Candidate keys for kf_order_candidates: the (eta, phi) bin of the candidate's crossing with the layer
 // (definition formula in fp32; the order only steers cache locality, never a result).
 __global__ void __launch_bounds__(kBlock)
@@ -270,7 +303,7 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
             BinLayerDev& L = B.layer[j];
             L.n = a.n_hits; L.ld_in = a.ld_in; L.ld_out = a.ld_out; L.pos = a.pos; L.cov = a.cov; L.radius = a.radius;
             L.bin_offset = a.bin_offset; L.sorted_to_orig = a.sorted_to_orig;
-            L.pos_sorted = a.pos_sorted; L.cov_sorted = a.cov_sorted; L.hit_rec = a.hit_rec;
+            L.pos_sorted = a.pos_sorted; L.cov_sorted = a.cov_sorted; L.hit_rec = a.hit_rec; L.bin_box = a.bin_box;
             L.key = s.key + item_off; L.unsorted = s.unsorted + item_off;
             L.counts = s.counts + (int64_t)(l0 + j) * (nb + 1); L.cursor = s.cursor + (int64_t)(l0 + j) * (nb + 1);
             item_off += a.n_hits;
@@ -283,6 +316,7 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
             bin_scatter_kernel<<<grid, kBlock, 0, stream>>>(B);
             bin_rank_gather_kernel<<<grid, kBlock, 0, stream>>>(B);
         }
+        bin_box_kernel<<<dim3((unsigned)((nb * 32 + kBlock - 1) / kBlock), (unsigned)m), kBlock, 0, stream>>>(B);
     }
     return cudaGetLastError();
 }
@@ -301,7 +335,7 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
     BinLayerDev& L = B.layer[0];
     L.n = n; L.ld_in = 0; L.ld_out = 0; L.pos = nullptr; L.cov = nullptr; L.radius = 0.0f;
     L.bin_offset = s.counts + (nb + 1);  // second half of the counts buffer holds the offsets
-    L.sorted_to_orig = order; L.pos_sorted = nullptr; L.cov_sorted = nullptr; L.hit_rec = nullptr;
+    L.sorted_to_orig = order; L.pos_sorted = nullptr; L.cov_sorted = nullptr; L.hit_rec = nullptr; L.bin_box = nullptr;
     L.key = s.key; L.unsorted = s.unsorted; L.counts = s.counts; L.cursor = s.cursor;
     const dim3 grid((unsigned)((n + kBlock - 1) / kBlock), 1);
     cand_key_kernel<<<grid, kBlock, 0, stream>>>(P, layer, n, ld, par, q, n_eta, n_phi, eta_max, s.key, s.counts);

@@ -59,6 +59,7 @@ struct BinArgs {
     int32_t* bin_offset; int32_t* sorted_to_orig;
     float* pos_sorted; float* cov_sorted;  // optional SoA copies (may be null)
     float* hit_rec;                        // [n_hits][12] packed records (may be null)
+    float* bin_box;                        // [n_bins][8] per-bin bounds (may be null)
 };
 
 // One layer (or one candidate set) as the batched sort kernels see it.
@@ -67,7 +68,7 @@ struct BinLayerDev {
     const float* pos; const float* cov;    // null: order items only, gather nothing
     float radius;
     int32_t* bin_offset; int32_t* sorted_to_orig;
-    float* pos_sorted; float* cov_sorted; float* hit_rec;
+    float* pos_sorted; float* cov_sorted; float* hit_rec; float* bin_box;
     int32_t* key;       // [n] bin of each item
     int32_t* unsorted;  // [n] item indices grouped by bin, arbitrary order inside
     int32_t* counts;    // [n_bins + 1]
@@ -112,6 +113,7 @@ struct ScoreArgs {
     // current step
     int64_t n_hits;
     const float* hit_rec;
+    const float* bin_box;
     const int32_t* bin_offset;
     int32_t* best_hit; float* best_chi2;
     // common
@@ -126,6 +128,7 @@ struct ScoreStep {
     int layer;               // geometry layer
     int64_t n_hits;
     const float* hit_rec;
+    const float* bin_box;
     const int32_t* bin_offset;
     int32_t* best_hit;       // [n]
     float* best_chi2;        // [n]

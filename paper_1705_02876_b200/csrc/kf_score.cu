@@ -18,7 +18,10 @@
 // current best and is dropped after ~20 instructions and two of its three 128-bit words.  The
 // survivors (a few per cent) are compacted through a per-warp list in shared memory (ballot + popc)
 // and evaluated densely, 32 at a time, with the same Schur-form chi2 as the update.  A 1 % margin on
-// the bound covers fp32 rounding.  A shuffle arg-min then picks (lowest chi2, lowest original index).
+// the bound covers fp32 rounding.  The same two bounds are first applied to whole BINS (bounding box of
+// the bin's hits and its largest variances, made by kf_bin_layers): typically 2-4 of the 25 bins of a
+// window survive, the others are never touched.  A shuffle arg-min then picks (lowest chi2, lowest
+// original index).
 // Warp w scans candidate order[w] when an order is given (kf_order_candidates), so neighbouring warps
 // share their windows in L1/L2; the order never changes a result.
 #include <math_constants.h>
@@ -245,23 +248,43 @@ scan_kernel(const ScoreArgs a, float inv_r) {
     const float ecc = c.ec * c.ec, ess = c.es * c.es, ecs2 = 2.0f * c.ec * c.es;
     const int wh = a.window_half;
     const float4* __restrict__ rec = reinterpret_cast<const float4*>(a.hit_rec);
-    const int e_lo = ie - wh < 0 ? 0 : ie - wh, e_hi = ie + wh > a.n_eta - 1 ? a.n_eta - 1 : ie + wh;
-    // phi bins p0 .. p0 + 2w (mod n_phi): one run of the ordered records, or two when it wraps
-    const int p0 = ((ip - wh) % a.n_phi + a.n_phi) % a.n_phi;
-    const int p1 = p0 + 2 * wh;  // inclusive, may exceed n_phi - 1
-    const int nseg = p1 >= a.n_phi ? 2 : 1;
-    for (int e = e_lo; e <= e_hi; ++e) {
-        const int row = e * a.n_phi;
-        for (int sgi = 0; sgi < nseg; ++sgi) {
-            int32_t s0, s1;
-            if (nseg == 1) { s0 = __ldg(a.bin_offset + row + p0); s1 = __ldg(a.bin_offset + row + p1 + 1); }
-            else if (sgi == 0) { s0 = __ldg(a.bin_offset + row + p0); s1 = __ldg(a.bin_offset + row + a.n_phi); }
-            else { s0 = __ldg(a.bin_offset + row); s1 = __ldg(a.bin_offset + row + p1 - a.n_phi + 1); }
+    const float4* __restrict__ box = reinterpret_cast<const float4*>(a.bin_box);
+    const int side = 2 * wh + 1, n_win = side * side;
+    // The window, 32 bins at a time: lane j tests bin j against the same two bounds applied to the bin's
+    // bounding box (the closest any of its hits can be) and its largest variances; a bin that cannot hold
+    // a hit under the threshold is skipped without touching its hits.
+    for (int wb = 0; wb < n_win; wb += 32) {
+        const int j = wb + lane;
+        bool keep = false;
+        int32_t s0 = 0, s1 = 0;
+        if (j < n_win) {
+            const int e = ie - wh + j / side;
+            const int p = ((ip - wh + j % side) % a.n_phi + a.n_phi) % a.n_phi;
+            if (e >= 0 && e < a.n_eta) {
+                const int bin = e * a.n_phi + p;
+                s0 = __ldg(a.bin_offset + bin);
+                s1 = __ldg(a.bin_offset + bin + 1);
+                const float4 X = __ldg(box + 2 * bin), Z = __ldg(box + 2 * bin + 1);
+                const float dzm = fmaxf(0.0f, fmaxf(Z.x - c.zn, c.zn - Z.y));
+                // rt(x, y) = ec (y - yn) - es (x - xn) is linear: its range over the box is at the corners
+                const float ax = -c.es, ay = c.ec;
+                const float x0 = X.x - c.xn, x1 = X.y - c.xn, y0 = X.z - c.yn, y1 = X.w - c.yn;
+                const float lo = fminf(ax * x0, ax * x1) + fminf(ay * y0, ay * y1);
+                const float hi = fmaxf(ax * x0, ax * x1) + fmaxf(ay * y0, ay * y1);
+                const float rtm = lo > 0.0f ? lo : (hi < 0.0f ? -hi : 0.0f);
+                keep = (s1 > s0) & (dzm * dzm <= thr * (c.n22 + Z.z)) & (rtm * rtm <= thr * (c.n11 + Z.w));
+            }
+        }
+        unsigned kept = __ballot_sync(0xffffffffu, keep);
+        while (kept) {
+            const int src = __ffs(kept) - 1;
+            kept &= kept - 1;
+            const int32_t b0 = __shfl_sync(0xffffffffu, s0, src), b1 = __shfl_sync(0xffffffffu, s1, src);
             // 64 hits per step: two records per lane, four independent 128-bit loads in flight
-            const float4* p = rec + (int64_t)(s0 + lane) * 3;
-            for (int32_t sb = s0; sb < s1; sb += 64, p += 64 * 3) {   // warp-uniform trip count
+            const float4* p = rec + (int64_t)(b0 + lane) * 3;
+            for (int32_t sb = b0; sb < b1; sb += 64, p += 64 * 3) {   // warp-uniform trip count
                 const int32_t sA = sb + lane, sB = sA + 32;
-                const bool vA = sA < s1, vB = sB < s1;
+                const bool vA = sA < b1, vB = sB < b1;
                 float4 A0 = make_float4(0.f, 0.f, 0.f, 0.f), B0 = A0, A1 = A0, B1 = A0;
                 if (vA) { A0 = __ldg(p); B0 = __ldg(p + 1); }
                 if (vB) { A1 = __ldg(p + 96); B1 = __ldg(p + 97); }
@@ -354,7 +377,7 @@ cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n
         const ScoreStep& st = steps[j];
         if (j == 0) propagate_global_kernel<<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer, keep);
         else update_propagate_kernel<<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer);   // a.hit_rec still step j-1
-        a.hit_rec = st.hit_rec; a.bin_offset = st.bin_offset; a.n_hits = st.n_hits;
+        a.hit_rec = st.hit_rec; a.bin_box = st.bin_box; a.bin_offset = st.bin_offset; a.n_hits = st.n_hits;
         a.best_hit = st.best_hit; a.best_chi2 = st.best_chi2;
         scan_kernel<<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
     }

@@ -41,6 +41,15 @@ def _assert_bins_equal(dl, ob, pos, cov):
     assert np.array_equal(rec[:, 0:3], pos[:, s2o].T) and np.array_equal(rec[:, 3], cs[:, 5])
     assert np.array_equal(rec[:, 4:7], cs[:, [0, 1, 3]]) and np.array_equal(rec[:, 8:10], cs[:, [2, 4]])
     assert np.array_equal(rec[:, 7].copy().view(np.int32), s2o)
+    box = dl.bins.bin_box.cpu().numpy()
+    off = ob["bin_offset"]
+    for b in np.flatnonzero(np.diff(off) > 0)[::7]:               # every 7th non-empty bin
+        seg = s2o[off[b]:off[b + 1]]
+        want = [pos[0, seg].min(), pos[0, seg].max(), pos[1, seg].min(), pos[1, seg].max(), pos[2, seg].min(),
+                pos[2, seg].max(), max(cov[5, seg].max(), 0.0), max((cov[0, seg] + cov[3, seg]).max(), 0.0)]
+        assert np.array_equal(box[b], np.array(want, dtype=np.float32)), (b, box[b], want)
+    empty = np.flatnonzero(np.diff(off) == 0)
+    assert np.all(np.isposinf(box[empty][:, [0, 2, 4]])) and np.all(np.isneginf(box[empty][:, [1, 3, 5]]))
 
 
 @pytest.mark.parametrize("n_tracks,noise", [(400, 2000), (20000, 100000)])

@@ -15,7 +15,7 @@
  * Conventions: AoS per track, dense 6x6 row-major matrices, no blocking / fusion / reordering.
  * State u = (x, y, z, px, py, pz) [cm, GeV/c]; charge q = +-1; B = Bz z-hat [Tesla].
  *
- * Pins (tests/test_oracle_pins.py): P1 exact helix recovery, P2 propagation invariants + RK4 +
+ * Pins (tests/test_oracle_pins.py, tests/test_oracle_smoother.py): P1 exact helix recovery, P2 propagation invariants + RK4 +
  * worked value, P3 Jacobian vs finite differences / radial null / |p| conservation, P4 EKF ==
  * batch weighted least squares, P5 covariance PSD rank 5, P6 pulls and chi2/ndf, P7 Highland
  * check values, P8 window scoring == brute force, P9 bin structure, P10 rotation symmetry.
@@ -52,14 +52,16 @@ double orc_theta0(double p, double mass, double t) {
  *   t = tan(theta/2) = D / (a + sqrt(a^2 - D(2b + D))).
  * F = A + (df/ds) (x) (ds/du): A = d(map)/du at fixed s, ds/du from the constraint |pos'| = r.
  * Returns 0 or ORC_PROP_FAIL (then nothing is written). F may be NULL. */
-int orc_propagate(const double u[6], double q, double Bz, double r, double out[6], double F[36],
-                  double *s_out, double *theta_out) {
+static int propagate_dir(const double u[6], double q, double Bz, double r, int inward, double out[6],
+                         double F[36], double *s_out, double *theta_out) {
     double x = u[0], y = u[1], z = u[2], px = u[3], py = u[4], pz = u[5];
     double k = q * ORC_C_B * Bz;
     double pt2 = px * px + py * py;
     double pt = sqrt(pt2);
     double rho2 = x * x + y * y;
-    if (!(r * r > rho2)) return ORC_PROP_FAIL;
+    /* outward: target radius outside the current one; inward (reading A18): inside, reached by
+     * following the same helix BACKWARD in path length (D < 0 gives t < 0, theta < 0, s < 0) */
+    if (inward ? !(r * r < rho2) : !(r * r > rho2)) return ORC_PROP_FAIL;
     double a = x * px + y * py;
     double b = (y * px - x * py) - pt2 / k;
     double D = 0.5 * k * (r * r - rho2);
@@ -106,6 +108,17 @@ int orc_propagate(const double u[6], double q, double Bz, double r, double out[6
     if (s_out) *s_out = s;
     if (theta_out) *theta_out = theta;
     return 0;
+}
+
+int orc_propagate(const double u[6], double q, double Bz, double r, double out[6], double F[36],
+                  double *s_out, double *theta_out) {
+    return propagate_dir(u, q, Bz, r, 0, out, F, s_out, theta_out);
+}
+
+/* Same closed form followed backward along the helix to a SMALLER radius (reading A18). */
+int orc_propagate_inward(const double u[6], double q, double Bz, double r, double out[6], double F[36],
+                         double *s_out, double *theta_out) {
+    return propagate_dir(u, q, Bz, r, 1, out, F, s_out, theta_out);
 }
 
 /* ---- process noise (reading A5): thin scatterer at the layer, evaluated at the propagated
@@ -268,6 +281,115 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
     *ochi2 = chi2;
     *onhits = nh;
     *ostatus = st;
+}
+
+/* ---- backward refit / smoother (reading A18; "a final fit with a KF and smoother") ---------
+ * Starts from the forward result (u, C) standing at the outermost used hit layer, with the covariance
+ * inflated by kappa (the forward information is kept only as a weak prior), and runs the same filter
+ * inward over the same hits:
+ *   update with the outermost hit (no propagation: the state already stands on that layer);
+ *   for every further used layer, outer to inner:  C += Q(previous layer, at the current momentum)
+ *   [the scatterer just left behind], propagate inward (C' = F C F^T), update with the layer's hit.
+ * Result: state and covariance at the INNERMOST used hit layer (outer side of its material), chi2 of the
+ * backward pass.  A failing layer sets the status bit and is skipped as in the forward fit.
+ * `used` = bit mask of the layers the forward fit used (mask bit set AND no failure there).
+ * trace (optional): per layer 122 doubles as in fit_one (F = I, Q = 0 for the update-only first step;
+ * Q is the noise added BEFORE the propagation of that step). */
+static void refit_inward_one(int L, const double *radius, const double *xX0, double Bz, double mass, double kappa,
+                             const double par[6], const double cov[36], int q, const double *hpos,
+                             const double *hcov, uint32_t used, double opar[6], double ocov[36], double *ochi2,
+                             int32_t *onhits, uint32_t *ostatus, double *trace) {
+    double u[6], C[36];
+    memcpy(u, par, sizeof u);
+    for (int i = 0; i < 36; ++i) C[i] = kappa * cov[i];
+    double chi2 = 0.0;
+    int nh = 0, prev = -1;
+    uint32_t st = 0;
+    for (int l = L - 1; l >= 0; --l) {
+        double *tr = trace ? trace + (size_t)l * ORC_TRACE_STRIDE : NULL;
+        if (tr) memset(tr, 0, ORC_TRACE_STRIDE * sizeof(double));
+        if (!((used >> l) & 1u)) continue;
+        double up[6], F[36], Q[36], Cp[36], un[6], Cn[36], dchi2;
+        int rc;
+        if (prev < 0) { /* first step: update only */
+            memcpy(up, u, sizeof up);
+            memcpy(Cp, C, sizeof Cp);
+            memset(Q, 0, sizeof Q);
+            memset(F, 0, sizeof F);
+            for (int i = 0; i < 6; ++i) F[i * 6 + i] = 1.0;
+        } else {
+            double Cq[36], Z[36];
+            orc_process_noise(u, mass, xX0[prev], Q);
+            for (int i = 0; i < 36; ++i) Cq[i] = C[i] + Q[i];
+            rc = propagate_dir(u, (double)q, Bz, radius[l], 1, up, F, NULL, NULL);
+            if (rc) { st |= (uint32_t)rc; continue; }
+            memset(Z, 0, sizeof Z);
+            orc_transport_cov(F, Cq, Z, Cp);
+        }
+        rc = orc_update(up, Cp, hpos + 3 * l, hcov + 9 * l, un, Cn, &dchi2);
+        if (rc) { st |= (uint32_t)rc; continue; }
+        memcpy(u, un, sizeof u);
+        memcpy(C, Cn, sizeof C);
+        chi2 += dchi2;
+        nh += 1;
+        prev = l;
+        if (tr) {
+            memcpy(tr, up, 6 * sizeof(double));
+            memcpy(tr + 6, F, 36 * sizeof(double));
+            memcpy(tr + 42, Q, 36 * sizeof(double));
+            memcpy(tr + 78, u, 6 * sizeof(double));
+            memcpy(tr + 84, C, 36 * sizeof(double));
+            tr[120] = dchi2;
+            tr[121] = 1.0;
+        }
+    }
+    memcpy(opar, u, sizeof u);
+    memcpy(ocov, C, sizeof C);
+    *ochi2 = chi2;
+    *onhits = nh;
+    *ostatus = st;
+}
+
+/* Forward fit followed by the inward refit.  Outputs: forward result (opar/ocov/ochi2/onhits/ostatus) and
+ * smoothed result at the innermost used layer (spar/scov/schi2).  sstatus = bits of the backward pass.
+ * used_out (optional) = layers the forward fit used. */
+void orc_fit_smooth_one(int L, const double *radius, const double *xX0, double Bz, double mass, double kappa,
+                        const double par[6], const double cov[36], int q, const double *hpos,
+                        const double *hcov, uint32_t mask, double opar[6], double ocov[36], double *ochi2,
+                        int32_t *onhits, uint32_t *ostatus, double spar[6], double scov[36], double *schi2,
+                        uint32_t *sstatus, double *trace_fwd, double *trace_bwd) {
+    double *tf = trace_fwd, *own = NULL;
+    if (!tf) { own = (double *)malloc((size_t)L * ORC_TRACE_STRIDE * sizeof(double)); tf = own; }
+    fit_one(L, radius, xX0, Bz, mass, par, cov, q, hpos, hcov, mask, opar, ocov, ochi2, onhits, ostatus, tf);
+    uint32_t used = 0;
+    for (int l = 0; l < L; ++l)
+        if (tf[(size_t)l * ORC_TRACE_STRIDE + 121] != 0.0) used |= 1u << l;
+    int32_t nb;
+    if (used == 0) { /* nothing fitted: the input comes back */
+        memcpy(spar, opar, 6 * sizeof(double));
+        memcpy(scov, ocov, 36 * sizeof(double));
+        *schi2 = 0.0;
+        *sstatus = 0;
+    } else {
+        refit_inward_one(L, radius, xX0, Bz, mass, kappa, opar, ocov, q, hpos, hcov, used, spar, scov, schi2, &nb,
+                         sstatus, trace_bwd);
+    }
+    if (own) free(own);
+}
+
+/* Batched (single thread): AoS double inputs as in orc_fit_tracks. */
+void orc_fit_smooth_tracks(int64_t n, int L, const double *radius, const double *xX0, double Bz, double mass,
+                           double kappa, const double *par, const double *cov, const int8_t *q,
+                           const double *hpos, const double *hcov, const uint32_t *mask, double *opar,
+                           double *ocov, double *ochi2, int32_t *onhits, uint32_t *ostatus, double *spar,
+                           double *scov, double *schi2, uint32_t *sstatus, double *trace_fwd, double *trace_bwd) {
+    for (int64_t i = 0; i < n; ++i)
+        orc_fit_smooth_one(L, radius, xX0, Bz, mass, kappa, par + 6 * i, cov + 36 * i, q[i],
+                           hpos + (size_t)i * L * 3, hcov + (size_t)i * L * 9, mask ? mask[i] : 0xffffffffu,
+                           opar + 6 * i, ocov + 36 * i, ochi2 + i, onhits + i, ostatus + i, spar + 6 * i,
+                           scov + 36 * i, schi2 + i, sstatus + i,
+                           trace_fwd ? trace_fwd + (size_t)i * L * ORC_TRACE_STRIDE : NULL,
+                           trace_bwd ? trace_bwd + (size_t)i * L * ORC_TRACE_STRIDE : NULL);
 }
 
 typedef struct {

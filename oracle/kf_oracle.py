@@ -40,6 +40,9 @@ def lib():
         _lib.orc_theta0.argtypes = [C.c_double] * 3
         _lib.orc_propagate.restype = C.c_int
         _lib.orc_propagate.argtypes = [dp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
+        _lib.orc_propagate_inward.restype = C.c_int
+        _lib.orc_propagate_inward.argtypes = [dp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
+        _lib.orc_fit_smooth_tracks.restype = None
         _lib.orc_process_noise.restype = None
         _lib.orc_process_noise.argtypes = [dp, C.c_double, C.c_double, dp]
         _lib.orc_transport_cov.restype = None
@@ -101,6 +104,17 @@ def propagate(u, q, Bz, r, want_F=True):
     s = C.c_double(0.0)
     th = C.c_double(0.0)
     rc = lib().orc_propagate(_p(u), float(q), float(Bz), float(r), _p(out), _p(F), C.byref(s), C.byref(th))
+    return rc, out, (F.reshape(6, 6) if want_F else None), s.value, th.value
+
+
+def propagate_inward(u, q, Bz, r, want_F=True):
+    """Backward along the helix to a smaller radius (reading A18). -> (status, u_out, F, s, theta)"""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    out = np.zeros(6)
+    F = np.zeros(36) if want_F else None
+    s = C.c_double(0.0)
+    th = C.c_double(0.0)
+    rc = lib().orc_propagate_inward(_p(u), float(q), float(Bz), float(r), _p(out), _p(F), C.byref(s), C.byref(th))
     return rc, out, (F.reshape(6, 6) if want_F else None), s.value, th.value
 
 
@@ -167,6 +181,40 @@ def fit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None
     out = dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost)
     if want_trace:
         out["trace"] = trace
+    return out
+
+
+SMOOTH_KAPPA = 10.0    # reading A18: inflation of the forward covariance used as the backward prior
+
+
+def fit_smooth_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None, kappa: float = SMOOTH_KAPPA,
+                      want_trace: bool = False) -> dict:
+    """Forward fit + inward refit (smoother).  Same input layout as fit_tracks.  Returns the forward
+    results under the usual keys and the smoothed ones as spar[6][n], scov[n][6][6], schi2, sstatus
+    [, trace_fwd, trace_bwd]."""
+    L = int(len(radius))
+    n = int(par.shape[1])
+    rad = np.ascontiguousarray(radius, dtype=np.float64)
+    xx0 = np.ascontiguousarray(x_over_X0, dtype=np.float64)
+    par_a = np.ascontiguousarray(np.asarray(par, dtype=np.float64).T)
+    cov_a = np.ascontiguousarray(unpack_cov21(np.asarray(cov21, dtype=np.float64)))
+    q_a = np.ascontiguousarray(q, dtype=np.int8)
+    hp_a = np.ascontiguousarray(np.transpose(np.asarray(hpos, dtype=np.float64), (2, 0, 1)))
+    hc_a = np.ascontiguousarray(unpack_cov6(hcov))
+    m_a = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint32)
+    opar = np.zeros((n, 6)); ocov = np.zeros((n, 6, 6)); ochi2 = np.zeros(n)
+    onh = np.zeros(n, dtype=np.int32); ost = np.zeros(n, dtype=np.uint32)
+    spar = np.zeros((n, 6)); scov = np.zeros((n, 6, 6)); schi2 = np.zeros(n); sst = np.zeros(n, dtype=np.uint32)
+    tf = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
+    tb = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
+    lib().orc_fit_smooth_tracks(C.c_int64(n), C.c_int(L), _p(rad), _p(xx0), C.c_double(Bz), C.c_double(mass),
+                                C.c_double(kappa), _p(par_a), _p(cov_a), _p(q_a, C.c_int8), _p(hp_a), _p(hc_a),
+                                _p(m_a, C.c_uint32), _p(opar), _p(ocov), _p(ochi2), _p(onh, C.c_int32),
+                                _p(ost, C.c_uint32), _p(spar), _p(scov), _p(schi2), _p(sst, C.c_uint32), _p(tf), _p(tb))
+    out = dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost,
+               spar=np.ascontiguousarray(spar.T), scov=scov, schi2=schi2, sstatus=sst)
+    if want_trace:
+        out["trace_fwd"], out["trace_bwd"] = tf, tb
     return out
 
 

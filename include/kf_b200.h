@@ -138,6 +138,19 @@ typedef struct {
 KF_API int kf_fit_tracks(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                   const kf_track_hits* hits, kf_tracks* out);
 
+/* Fit and smooth ("a final fit with a KF and smoother"; reading A18): the forward
+ * fit of kf_fit_tracks, then the same filter run INWARD over the same hits, starting from the forward
+ * result with its covariance inflated by `kappa` (10 is the documented choice): update with the outermost
+ * used hit, then for each further used layer, outer to inner, add the process noise of the layer just
+ * left, propagate backward along the helix to the smaller radius, update.  `out` receives the forward
+ * result exactly as kf_fit_tracks writes it (state at the outermost used layer); `smoothed` receives the
+ * state and covariance at the INNERMOST used layer (outer side of its material), chi2 = chi2 of the
+ * backward pass, nhits = hits it used, status = its failure bits.  A track the forward fit could not
+ * start comes back as its input in both.  All pointers DEV; `out` may alias `seeds`, `smoothed` may not
+ * alias either.  One kernel. */
+KF_API int kf_fit_tracks_smooth(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                                const kf_track_hits* hits, float kappa, kf_tracks* out, kf_tracks* smoothed);
+
 /* Same call with every pointer HOST (pageable or pinned): copies in, fits, copies out, in chunks
  * pipelined over internal streams, and returns when `out` is complete.  This is the end-to-end
  * path (transfers overlapped with kernels).  Alignment rules do not apply. */

@@ -20,7 +20,7 @@ _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so"
 
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_build_best_hit"]
 
 
@@ -93,6 +93,9 @@ def load_library():
         f = getattr(lib, name)
         f.restype = C.c_int
         f.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.POINTER(_Tracks)]
+    lib.kf_fit_tracks_smooth.restype = C.c_int
+    lib.kf_fit_tracks_smooth.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.c_float,
+                                         C.POINTER(_Tracks), C.POINTER(_Tracks)]
     lib.kf_bin_hits.restype = C.c_int
     lib.kf_bin_hits.argtypes = [vp, C.c_float, C.POINTER(_LayerHits), C.POINTER(_LayerBins)]
     lib.kf_bin_layers.restype = C.c_int
@@ -252,6 +255,19 @@ class KFContext:
         hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
         self._check(self._lib.kf_fit_tracks(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)),
                     "kf_fit_tracks")
+        del keep
+
+    def fit_tracks_smooth(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask, kappa: float,
+                          out_par, out_cov, out_chi2, out_nhits, out_status,
+                          s_par, s_cov, s_chi2, s_nhits, s_status):
+        """Forward fit + inward refit (smoother) in one kernel; two result sets."""
+        g, keep = geom._c()
+        seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
+        out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
+        sm = self._tracks(n, s_par, s_cov, None, s_chi2, s_nhits, s_status)
+        hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
+        self._check(self._lib.kf_fit_tracks_smooth(self._h, C.byref(g), C.byref(seeds), C.byref(hits), float(kappa),
+                                                   C.byref(out), C.byref(sm)), "kf_fit_tracks_smooth")
         del keep
 
     def fit_tracks_host(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,

@@ -25,7 +25,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 3;
+constexpr int kAbiVersion = 4;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -192,6 +192,37 @@ int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
     a.hpos = hits->pos; a.hcov = hits->cov; a.ld_hit = hits->ld; a.mask = hits->mask;
     a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
     a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
+    cudaError_t e = launch_fit(P, a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits,
+                         float kappa, kf_tracks* out, kf_tracks* smoothed) {
+    if (!c || !geom || !seeds || !hits || !out || !smoothed) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (!(kappa >= 1.0f)) return KF_ERR_UNSUPPORTED;
+    if ((rc = check_tracks(seeds, true, true))) return rc;
+    if ((rc = check_tracks(out, false, true))) return rc;
+    if ((rc = check_tracks(smoothed, false, true))) return rc;
+    if (out->n != seeds->n || smoothed->n != seeds->n) return KF_ERR_SHAPE;
+    if ((rc = check_track_hits(hits, geom, seeds->n, true))) return rc;
+    if (seeds->n == 0) return KF_OK;
+    if (seeds->n > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
+    if (smoothed->par == seeds->par || smoothed->par == out->par || smoothed->cov == seeds->cov ||
+        smoothed->cov == out->cov)
+        return KF_ERR_UNSUPPORTED;
+    FitArgs a;
+    a.n = seeds->n;
+    a.par = seeds->par; a.cov = seeds->cov; a.ld_in = seeds->ld; a.q = seeds->q;
+    a.hpos = hits->pos; a.hcov = hits->cov; a.ld_hit = hits->ld; a.mask = hits->mask;
+    a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
+    a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
+    a.spar = smoothed->par; a.scov = smoothed->cov; a.ld_s = smoothed->ld;
+    a.schi2 = smoothed->chi2; a.snhits = smoothed->nhits; a.sstatus = smoothed->status;
+    a.kappa = kappa;
     cudaError_t e = launch_fit(P, a, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;

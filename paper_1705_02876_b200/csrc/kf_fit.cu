@@ -43,7 +43,7 @@ constexpr int kWarpFloats = kStages * kHitFloats + kSeedFloats;
 constexpr int kSmemBytes = kWarps * kWarpFloats * 4 + kWarps * (kStages + 1) * 8;
 
 struct FitMaps {
-    CUtensorMap hpos, hcov, par, cov, opar, ocov;
+    CUtensorMap hpos, hcov, par, cov, opar, ocov, spar, scov;
 };
 
 struct Hit {
@@ -130,7 +130,10 @@ __device__ __forceinline__ void track_to_tile(const Track& t, float* p) {
     p[832] = t.c55;
 }
 
-__global__ void __launch_bounds__(kFitBlock, KF_FIT_MIN_BLOCKS)
+// SMOOTH = false: forward fit (rows a1-a7).  SMOOTH = true: forward fit, then the inward refit of reading
+// A18 over the same hits (streamed again through the same ring, outermost layer first); two results.
+template <bool SMOOTH>
+__global__ void __launch_bounds__(kFitBlock, SMOOTH ? 4 : KF_FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -176,9 +179,12 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
     int nh = 0;
     uint32_t st = 0u;
     bool started = false;  // false: general 6x6 covariance; true: its radial row is identically zero
+    uint32_t phase = 0u;   // bit s = parity the next wait on stage s expects
+    uint32_t used = 0u;    // layers the forward fit used
     for (int l = 0; l < L; ++l) {
         const int s = l % kStages;
-        mbar_wait(bar0 + 8u * s, (uint32_t)(l / kStages) & 1u);
+        if constexpr (SMOOTH) { mbar_wait(bar0 + 8u * s, (phase >> s) & 1u); phase ^= 1u << s; }
+        else mbar_wait(bar0 + 8u * s, (uint32_t)(l / kStages) & 1u);
         const float* tp = wbase + s * kHitFloats + lane;
         Hit m;
         m.x = tp[0];         m.y = tp[32];        m.z = tp[64];
@@ -190,21 +196,109 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.mass2, m, chi2);
             else rc = fit_layer<false>(t, k, ik, P.layer[l], P.mass2, m, chi2);
             st |= rc;
-            if (rc == 0u) { nh += 1; started = true; }
+            if (rc == 0u) { nh += 1; started = true; used |= 1u << l; }
         }
         // The hit values have been consumed by the math above, so the stage can be handed back to the
         // TMA unit (write-after-read across the generic and async proxies needs no fence once the
         // reads have completed; the refill still lands kStages - 1 layers ahead of its use).
-        if (l + kStages < L) {
+        // In SMOOTH mode the ring runs on into the backward pass: step L + j carries layer L - 1 - j.
+        const int nxt = l + kStages;
+        if (nxt < (SMOOTH ? 2 * L : L)) {
+            const int ln = nxt < L ? nxt : 2 * L - 1 - nxt;
             __syncwarp();
             if (elect_one()) {
                 mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
-                tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * (l + kStages), bar0 + 8u * s);
-                tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * (l + kStages), bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * ln, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * ln, bar0 + 8u * s);
             }
         }
     }
     if (!good_q) st = ST_BAD_CHARGE;
+    if constexpr (SMOOTH) {
+        // ---- forward result out (a copy goes back to the global frame; t stays local for the refit)
+        if (good_q && nh > 0) {
+            Track g = t;
+            leave_local_frame(g);
+            track_to_tile(g, seed_tile + lane);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        const bool fstorer = elect_one();
+        if (fstorer) {
+            tma_store_2d(&M.opar, col, 0, seed0);
+            tma_store_2d(&M.ocov, col, 0, seed0 + 6 * 128);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        if (valid) { a.chi2[i] = chi2; a.nhits[i] = nh; a.status[i] = st; }
+        // ---- inward refit (reading A18)
+        float schi2 = 0.0f, ms_prev = 0.0f;
+        int nb = 0;
+        uint32_t sst = 0u;
+        bool first = true;
+        if (used) scale_cov(t, a.kappa);
+        for (int j = 0; j < L; ++j) {
+            const int l = L - 1 - j, step = L + j, s = step % kStages;
+            mbar_wait(bar0 + 8u * s, (phase >> s) & 1u);
+            phase ^= 1u << s;
+            const float* tp = wbase + s * kHitFloats + lane;
+            Hit m;
+            m.x = tp[0];         m.y = tp[32];        m.z = tp[64];
+            m.vxx = tp[96];      m.vxy = tp[128];     m.vxz = tp[160];
+            m.vyy = tp[192];     m.vyz = tp[224];     m.vzz = tp[256];
+            __syncwarp();
+            if ((used >> l) & 1u) {
+                Crossing o;
+                PropCov n;
+                bool ok = true;
+                const float k33 = t.c33, k35 = t.c35, k44 = t.c44, k55 = t.c55;
+                if (first) crossing_in_place(t, o, n);
+                else {
+                    ok = helix_to_radius<true>(t, k, ik, P.layer[l], o);
+                    if (ok) {
+                        add_process_noise(t, ms_prev, P.mass2);      // the scatterer just left behind
+                        transport_cov<true>(t, o, 0.0f, P.mass2, n);
+                    }
+                }
+                if (!ok) sst |= ST_PROP_FAIL;
+                else {
+                    LocalHit h;
+                    hit_to_local(o, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
+                    float d;
+                    const uint32_t rc = kalman_update(t, o, n, h, &d);
+                    if (rc == 0u) { schi2 += d; nb += 1; first = false; ms_prev = P.layer[l].ms; }
+                    else { sst |= rc; t.c33 = k33; t.c35 = k35; t.c44 = k44; t.c55 = k55; }   // layer skipped
+                }
+            }
+            const int nxt = step + kStages;
+            if (nxt < 2 * L) {
+                const int ln = 2 * L - 1 - nxt;
+                __syncwarp();
+                if (elect_one()) {
+                    mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
+                    tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * ln, bar0 + 8u * s);
+                    tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * ln, bar0 + 8u * s);
+                }
+            }
+        }
+        // the forward tile must have left shared memory before the smoothed one overwrites it
+        if (fstorer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncwarp();
+        if (good_q && used) {
+            leave_local_frame(t);
+            track_to_tile(t, seed_tile + lane);
+        }   // else the tile still holds the forward result = the input
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        const bool sstorer = elect_one();
+        if (sstorer) {
+            tma_store_2d(&M.spar, col, 0, seed0);
+            tma_store_2d(&M.scov, col, 0, seed0 + 6 * 128);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        if (valid) { a.schi2[i] = schi2; a.snhits[i] = nb; a.sstatus[i] = sst; }
+        if (sstorer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        return;
+    }
     if (good_q && nh > 0) {
         leave_local_frame(t);
         track_to_tile(t, seed_tile + lane);
@@ -262,8 +356,11 @@ bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t 
 
 cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream) {
     if (a.n == 0) return cudaSuccess;
-    static const cudaError_t attr = cudaFuncSetAttribute(fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    static const cudaError_t attr = cudaFuncSetAttribute(fit_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (attr != cudaSuccess) return attr;
+    static const cudaError_t attr2 = cudaFuncSetAttribute(fit_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (attr2 != cudaSuccess) return attr2;
+    const bool smooth = a.spar != nullptr;
     const int L = P.n_layers;
     FitMaps M;
     if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3) ||
@@ -271,8 +368,11 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
         !make_map(&M.par, a.par, a.n, a.ld_in, 6, 6) || !make_map(&M.cov, a.cov, a.n, a.ld_in, 21, 21) ||
         !make_map(&M.opar, a.opar, a.n, a.ld_out, 6, 6) || !make_map(&M.ocov, a.ocov, a.n, a.ld_out, 21, 21))
         return cudaErrorInvalidValue;
+    if (smooth && (!make_map(&M.spar, a.spar, a.n, a.ld_s, 6, 6) || !make_map(&M.scov, a.scov, a.n, a.ld_s, 21, 21)))
+        return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
-    fit_kernel<<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    if (smooth) fit_kernel<true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else fit_kernel<false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     return cudaGetLastError();
 }
 

@@ -20,6 +20,10 @@ struct FitArgs {
     // outputs
     float* opar; float* ocov; int64_t ld_out;
     float* chi2; int32_t* nhits; uint32_t* status;
+    // smoother outputs (spar == nullptr: forward fit only)
+    float* spar = nullptr; float* scov = nullptr; int64_t ld_s = 0;
+    float* schi2 = nullptr; int32_t* snhits = nullptr; uint32_t* sstatus = nullptr;
+    float kappa = 10.0f;
 };
 
 // kf_fit.cu

@@ -160,6 +160,9 @@ struct Crossing {
 
 // Reading A3: first outward crossing of the helix with the cylinder of radius L.r, half-angle
 // form  t = tan(theta/2) = D / (a + sqrt(a^2 - D (2b + D))).  Returns false on PROP_FAIL.
+// INWARD (reading A18): the same helix followed backward in path length to a smaller radius
+// (D < 0, t < 0, theta < 0); the local-frame Jacobian below holds for either sign of theta.
+template <bool INWARD = false>
 __device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float ik,
                                                 const LayerConst& L, Crossing& o) {
     const float x = t.x, y = t.y, px = t.px, py = t.py;
@@ -171,7 +174,7 @@ __device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float i
     const float disc = a * a - D * (2.0f * b + D);
     const float den = a + disc * rsqrt_fast(disc);  // NaN unless disc > 0
     // one test for the three PROP_FAIL conditions (r <= rho, disc <= 0, den <= 0; NaNs fail too)
-    if (!((L.r2 > rho2) & (disc > 0.0f) & (den > 0.0f))) return false;
+    if (!((INWARD ? L.r2 < rho2 : L.r2 > rho2) & (disc > 0.0f) & (den > 0.0f))) return false;
     const float tt = D * rcp_fast(den);
     const float i1 = rcp_fast(1.0f + tt * tt);
     const float S = 2.0f * tt * i1;
@@ -295,6 +298,41 @@ __device__ __forceinline__ void transport_cov(const Track& t, const Crossing& o,
     n.n44 = t.c44 + mu * (2.0f * v4 + mu * gCg) + th2 * p2;
     n.n45 = t.c45 + mu * v5;
     n.n55 = t.c55 + qc * (p2 * o.ipt);
+}
+
+// Reading A18, backward refit: the scatterer just left behind adds its Highland noise to the momentum
+// block BEFORE the inward propagation (same Q~ as in transport_cov, at the current momentum).
+__device__ __forceinline__ void add_process_noise(Track& t, float ms, float mass2) {
+    const float pt2 = t.px * t.px + t.py * t.py, pz = t.pz;
+    const float ipt = rsqrt_fast(pt2);
+    const float p2 = pt2 + pz * pz;
+    const float ip2 = rcp_fast(p2);
+    const float th2 = ms * (p2 + mass2) * ip2 * ip2;
+    const float qc = th2 * p2 * ipt;
+    t.c33 += th2 * pz * pz;
+    t.c35 -= qc * pz;
+    t.c44 += th2 * p2;
+    t.c55 += qc * (p2 * ipt);
+}
+
+// The track as it stands, dressed as a "crossing" with zero path length, so that kalman_update can be
+// applied without a propagation (first step of the backward refit: the state already stands on the
+// layer; its covariance is radially null in the frame (eax, eay) it carries).
+__device__ __forceinline__ void crossing_in_place(const Track& t, Crossing& o, PropCov& n) {
+    const float pt2 = t.px * t.px + t.py * t.py;
+    const float ipt = rsqrt_fast(pt2);
+    o.xn = t.x; o.yn = t.y; o.zn = t.z; o.pxn = t.px; o.pyn = t.py;
+    o.erx = t.eax; o.ery = t.eay; o.elx = t.px * ipt; o.ely = t.py * ipt;
+    o.T = t.pz * ipt; o.pt2 = pt2; o.ipt = ipt;
+    n.n11 = t.c11; n.n12 = t.c12; n.n13 = t.c13; n.n14 = t.c14; n.n15 = t.c15;
+    n.n22 = t.c22; n.n23 = t.c23; n.n24 = t.c24; n.n25 = t.c25;
+    n.n33 = t.c33; n.n34 = t.c34; n.n35 = t.c35; n.n44 = t.c44; n.n45 = t.c45; n.n55 = t.c55;
+}
+
+__device__ __forceinline__ void scale_cov(Track& t, float f) {
+    t.c11 *= f; t.c12 *= f; t.c13 *= f; t.c14 *= f; t.c15 *= f;
+    t.c22 *= f; t.c23 *= f; t.c24 *= f; t.c25 *= f;
+    t.c33 *= f; t.c34 *= f; t.c35 *= f; t.c44 *= f; t.c45 *= f; t.c55 *= f;
 }
 
 // Hit in the arrival frame: residual (r, t, z) and rotated covariance.

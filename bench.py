@@ -278,6 +278,23 @@ def run_ours(args) -> None:
     same = all(np.array_equal(a, b) for a, b in zip(d.results().values(), h.results().values()))
     fp32_peak = ctx.measure_fp32_peak(5) if rank == 0 else 0.0
     building = measure_building(ctx, dev) if (rank == 0 and not args.no_building) else None
+    smoothing = None
+    if rank == 0 and not args.no_building:
+        # secondary: kf_fit_tracks_smooth on the same batch (forward fit + inward refit, one kernel)
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                d.fit_smooth(ctx)
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record(stream)
+            for _ in range(20):
+                d.fit_smooth(ctx)
+            s1.record(stream)
+        torch.cuda.synchronize()
+        sm_ms = s0.elapsed_time(s1) / 20
+        sm_bytes = n * (113 + 2 * 36 * L + 2 * 120)
+        smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10)", "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3),
+                     "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0],
+                     "alu_roofline_frac": 2.0 * n * FLOPS_PER_TRACK_LAYER * L / (sm_ms * 1e-3) / (fp32_peak * 1e12)}
 
     if rank == 0:
         peak, peak_src = _peaks()
@@ -314,6 +331,8 @@ def run_ours(args) -> None:
         if building is not None:
             building["alu_roofline_frac"] = building["algorithmic_gflop"] * 1e9 / (building["build_ms"] * 1e-3) / (fp32_peak * 1e12)
             out["building"] = building
+        if smoothing is not None:
+            out["smoothing"] = smoothing
         print(json.dumps(out), flush=True)
     ctx.close()
     sharding.shutdown()

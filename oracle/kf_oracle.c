@@ -599,3 +599,135 @@ void orc_score_layer(int64_t n, double r_layer, double xX0, double Bz, double ma
         }
     }
 }
+
+/* ---- combinatorial track building (reading A19; "branching occurs to explore all possible track
+ * candidates up to some cutoff number of candidates per seed") ---------------------------------
+ * Every seed keeps at most n_cand candidates.  On each layer every candidate is propagated (+Q); every hit of
+ * its +-window_half bin window with chi2 < chi2_cut is compatible and spawns a child (Kalman update, nhits + 1,
+ * chi2 + increment); one more child takes no hit (propagated state, nhits and chi2 unchanged).  A candidate
+ * that cannot be propagated yields one child, itself unchanged (status bit).  The children of a seed are ranked
+ * by (nhits descending, chi2 ascending, parent slot ascending, hit original index ascending with "no hit" last)
+ * and the best n_cand survive, in that order.  After the last layer slot 0 is the seed's track.
+ * Outputs per seed: best candidate (state, covariance, chi2, nhits, status, hit per layer or -1), the number of
+ * surviving candidates, and `margin` = the smallest relative gap met in any decision that fp32 rounding could
+ * flip: |chi2 - cut| / cut of a window hit, and |chi2_a - chi2_b| / max(chi2, 1) between children of equal
+ * nhits that are adjacent in the ranking (including the first one dropped).                                    */
+#define ORC_MAXC 8
+typedef struct {
+    double u[6], C[36], chi2;
+    int nhits;
+    uint32_t status;
+    int32_t hits[32];
+} orc_cand;
+
+typedef struct {
+    orc_cand c;          /* child state */
+    int parent;
+    int32_t hit;         /* original index or -1 */
+} orc_child;
+
+static int child_before(const orc_child *a, const orc_child *b) {
+    if (a->c.nhits != b->c.nhits) return a->c.nhits > b->c.nhits;
+    if (a->c.chi2 != b->c.chi2) return a->c.chi2 < b->c.chi2;
+    if (a->parent != b->parent) return a->parent < b->parent;
+    {
+        int64_t ha = a->hit < 0 ? (int64_t)1 << 40 : a->hit, hb = b->hit < 0 ? (int64_t)1 << 40 : b->hit;
+        return ha < hb;
+    }
+}
+
+void orc_build_combinatorial(int64_t n_seeds, int n_layers_total, int first_layer, int n_build, const double *radius,
+                             const double *xX0, double Bz, double mass, const double *par, const double *cov,
+                             const int8_t *q, const double *chi2_in, const int32_t *nhits_in,
+                             const int64_t *n_hits, const double *const *hpos, const double *const *hcov,
+                             int n_eta, int n_phi, double eta_max, const int32_t *const *bin_offset,
+                             const int32_t *const *sorted_to_orig, int window_half, double chi2_cut, int n_cand,
+                             double *opar, double *ocov, double *ochi2, int32_t *onhits, uint32_t *ostatus,
+                             int32_t *ohits /* [n_build][n_seeds] */, int32_t *oncand, double *omargin) {
+    (void)n_layers_total; (void)n_hits;
+    if (n_cand > ORC_MAXC) n_cand = ORC_MAXC;
+    orc_cand *cur = (orc_cand *)malloc(sizeof(orc_cand) * ORC_MAXC);
+    size_t cap = 1024;
+    orc_child *ch = (orc_child *)malloc(sizeof(orc_child) * cap);
+    for (int64_t sd = 0; sd < n_seeds; ++sd) {
+        int nc = 1;
+        double margin = INFINITY;
+        memcpy(cur[0].u, par + 6 * sd, 6 * sizeof(double));
+        memcpy(cur[0].C, cov + 36 * sd, 36 * sizeof(double));
+        cur[0].chi2 = chi2_in ? chi2_in[sd] : 0.0;
+        cur[0].nhits = nhits_in ? nhits_in[sd] : 0;
+        cur[0].status = 0;
+        for (int j = 0; j < 32; ++j) cur[0].hits[j] = -1;
+        int qq = q[sd];
+        if (qq != 1 && qq != -1) cur[0].status = ORC_BAD_CHARGE;
+        for (int j = 0; j < n_build && !(cur[0].status & ORC_BAD_CHARGE); ++j) {
+            int l = first_layer + j;
+            size_t nch = 0;
+            for (int p = 0; p < nc; ++p) {
+                double up[6], F[36], Q[36], Cp[36];
+                int rc = orc_propagate(cur[p].u, (double)qq, Bz, radius[l], up, F, NULL, NULL);
+#define ORC_ROOM() do { if (nch + 2 > cap) { cap *= 2; ch = (orc_child *)realloc(ch, sizeof(orc_child) * cap); } } while (0)
+                ORC_ROOM();
+                if (rc) { /* cannot reach the layer: survives unchanged */
+                    ch[nch].c = cur[p]; ch[nch].c.status |= (uint32_t)rc; ch[nch].parent = p; ch[nch].hit = -1; ++nch;
+                    continue;
+                }
+                orc_process_noise(up, mass, xX0[l], Q);
+                orc_transport_cov(F, cur[p].C, Q, Cp);
+                /* the "no hit" child */
+                ch[nch].c = cur[p];
+                memcpy(ch[nch].c.u, up, sizeof up); memcpy(ch[nch].c.C, Cp, sizeof Cp);
+                ch[nch].parent = p; ch[nch].hit = -1; ++nch;
+                int cb = orc_bin_index_def(up[0], up[1], up[2], radius[l], n_eta, n_phi, eta_max);
+                int ie = cb / n_phi, ip = cb % n_phi;
+                for (int de = -window_half; de <= window_half; ++de) {
+                    int e = ie + de;
+                    if (e < 0 || e >= n_eta) continue;
+                    for (int dp = -window_half; dp <= window_half; ++dp) {
+                        int pb = ((ip + dp) % n_phi + n_phi) % n_phi, bin = e * n_phi + pb;
+                        for (int32_t s = bin_offset[j][bin]; s < bin_offset[j][bin + 1]; ++s) {
+                            int32_t h = sorted_to_orig[j][s];
+                            double c;
+                            if (orc_chi2_increment(up, Cp, hpos[j] + 3 * (size_t)h, hcov[j] + 9 * (size_t)h, &c)) continue;
+                            double gap = fabs(c - chi2_cut) / chi2_cut;
+                            if (gap < margin) margin = gap;
+                            if (!(c < chi2_cut)) continue;
+                            ORC_ROOM();
+                            orc_child *k = &ch[nch];
+                            k->c = cur[p];
+                            double cc;
+                            if (orc_update(up, Cp, hpos[j] + 3 * (size_t)h, hcov[j] + 9 * (size_t)h, k->c.u, k->c.C, &cc)) continue;
+                            k->c.chi2 = cur[p].chi2 + cc;
+                            k->c.nhits = cur[p].nhits + 1;
+                            k->c.hits[j] = h;
+                            k->parent = p; k->hit = h; ++nch;
+                        }
+                    }
+                }
+            }
+            /* rank: selection sort of the best n_cand + 1 (the extra one only feeds the margin) */
+            int keep = (int)(nch < (size_t)n_cand ? nch : (size_t)n_cand);
+            for (int a = 0; a < keep + 1 && (size_t)a < nch; ++a) {
+                size_t best = (size_t)a;
+                for (size_t b = (size_t)a + 1; b < nch; ++b)
+                    if (child_before(&ch[b], &ch[best])) best = b;
+                if (best != (size_t)a) { orc_child t = ch[a]; ch[a] = ch[best]; ch[best] = t; }
+                if (a > 0 && ch[a].c.nhits == ch[a - 1].c.nhits) {
+                    double sc = fmax(fmax(ch[a].c.chi2, ch[a - 1].c.chi2), 1.0);
+                    double gap = fabs(ch[a].c.chi2 - ch[a - 1].c.chi2) / sc;
+                    if (gap < margin) margin = gap;
+                }
+            }
+            for (int a = 0; a < keep; ++a) cur[a] = ch[a].c;
+            nc = keep;
+        }
+        memcpy(opar + 6 * sd, cur[0].u, 6 * sizeof(double));
+        memcpy(ocov + 36 * sd, cur[0].C, 36 * sizeof(double));
+        ochi2[sd] = cur[0].chi2; onhits[sd] = cur[0].nhits; ostatus[sd] = cur[0].status;
+        for (int j = 0; j < n_build; ++j) ohits[(size_t)j * n_seeds + sd] = cur[0].hits[j];
+        oncand[sd] = nc;
+        omargin[sd] = margin;
+    }
+    free(ch);
+    free(cur);
+}

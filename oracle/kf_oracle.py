@@ -58,6 +58,7 @@ def lib():
         _lib.orc_bin_index_f32.argtypes = [C.c_float] * 4 + [C.c_int, C.c_int, C.c_double]
         _lib.orc_bin_hits.restype = None
         _lib.orc_score_layer.restype = None
+        _lib.orc_build_combinatorial.restype = None
     return _lib
 
 
@@ -283,3 +284,43 @@ def score_layer(cands: Candidates, r_layer, x_over_X0, Bz, mass, hpos, hcov, bin
                           C.c_double(chi2_cut), C.c_int(1 if do_update else 0), C.c_int(1 if all_hits else 0),
                           _p(bh, C.c_int32), _p(bc), _p(sc))
     return dict(best_hit=bh, best_chi2=bc, second_chi2=sc)
+
+
+def build_combinatorial(radius, x_over_X0, Bz, mass, par, cov21, q, chi2, nhits, first_layer: int, layers: list,
+                        n_eta: int, n_phi: int, eta_max: float, window_half: int = 2, chi2_cut: float = 30.0,
+                        n_cand: int = 4) -> dict:
+    """Combinatorial building (reading A19) of all seeds over `layers` = [(hpos[3][H], hcov[6][H], bins dict), ...]
+    belonging to geometry layers first_layer, first_layer + 1, ...  Seeds in the SoA fp32 layout.
+    Returns the best candidate per seed: par[6][n], cov[n][6][6], chi2, nhits, status, hits[n_build][n],
+    n_cand[n], margin[n] (smallest relative gap of any decision fp32 rounding could flip)."""
+    n = int(par.shape[1])
+    m = len(layers)
+    rad = np.ascontiguousarray(radius, dtype=np.float64)
+    xx0 = np.ascontiguousarray(x_over_X0, dtype=np.float64)
+    par_a = np.ascontiguousarray(np.asarray(par, dtype=np.float64).T)
+    cov_a = np.ascontiguousarray(unpack_cov21(np.asarray(cov21, dtype=np.float64)))
+    q_a = np.ascontiguousarray(q, dtype=np.int8)
+    c_a = np.ascontiguousarray(chi2, dtype=np.float64)
+    nh_a = np.ascontiguousarray(nhits, dtype=np.int32)
+    hp = [np.ascontiguousarray(np.asarray(l[0], dtype=np.float64).T) for l in layers]
+    hc = [np.ascontiguousarray(unpack_cov6(l[1])) for l in layers]
+    off = [np.ascontiguousarray(l[2]["bin_offset"], dtype=np.int32) for l in layers]
+    s2o = [np.ascontiguousarray(l[2]["sorted_to_orig"], dtype=np.int32) for l in layers]
+    nh = (C.c_int64 * m)(*[int(h.shape[0]) for h in hp])
+    dpp = C.POINTER(C.c_double)
+    ipp = C.POINTER(C.c_int32)
+    hp_p = (dpp * m)(*[_p(a) for a in hp])
+    hc_p = (dpp * m)(*[_p(a) for a in hc])
+    off_p = (ipp * m)(*[_p(a, C.c_int32) for a in off])
+    s2o_p = (ipp * m)(*[_p(a, C.c_int32) for a in s2o])
+    opar = np.zeros((n, 6)); ocov = np.zeros((n, 6, 6)); ochi2 = np.zeros(n)
+    onh = np.zeros(n, dtype=np.int32); ost = np.zeros(n, dtype=np.uint32)
+    ohits = np.zeros((m, n), dtype=np.int32); onc = np.zeros(n, dtype=np.int32); omar = np.zeros(n)
+    lib().orc_build_combinatorial(C.c_int64(n), C.c_int(len(rad)), C.c_int(first_layer), C.c_int(m), _p(rad), _p(xx0),
+                                  C.c_double(Bz), C.c_double(mass), _p(par_a), _p(cov_a), _p(q_a, C.c_int8), _p(c_a),
+                                  _p(nh_a, C.c_int32), nh, hp_p, hc_p, C.c_int(n_eta), C.c_int(n_phi),
+                                  C.c_double(eta_max), off_p, s2o_p, C.c_int(window_half), C.c_double(chi2_cut),
+                                  C.c_int(n_cand), _p(opar), _p(ocov), _p(ochi2), _p(onh, C.c_int32),
+                                  _p(ost, C.c_uint32), _p(ohits, C.c_int32), _p(onc, C.c_int32), _p(omar))
+    return dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost, hits=ohits,
+                n_cand=onc, margin=omar)

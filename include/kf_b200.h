@@ -225,6 +225,21 @@ KF_API int kf_build_best_hit(kf_ctx* ctx, const kf_geometry* geom, int first_lay
                              int window_half, float chi2_cut, int do_update, const int32_t* order,
                              int32_t* hit_index, float* hit_chi2, int64_t ld_out);
 
+/* Combinatorial building (reading A19) over n_build_layers consecutive
+ * layers.  Every seed keeps at most n_cand (1..8) candidates.  On each layer every candidate is propagated
+ * (+Q); every hit of its window with chi2 < chi2_cut spawns a child (Kalman update, nhits + 1, chi2 +
+ * increment; only a candidate's n_cand best hits can survive, so only those are kept), one more child takes
+ * no hit; a candidate that cannot reach the layer yields itself unchanged (PROP_FAIL bit).  The children of a
+ * seed are ranked by (nhits descending, chi2 ascending, parent slot, hit original index with "no hit" last)
+ * and the best n_cand survive.  On return `cands` holds the best candidate of every seed (state, covariance,
+ * chi2, nhits, status); hit_index[j*ld_out + i] = original index of its hit on layer first_layer + j or -1;
+ * n_found[i] (optional, DEV [n]) = candidates alive at the end.  With n_cand = 1 this is kf_build_best_hit.
+ * hits[j] / bins[j]: HOST arrays as in kf_build_best_hit.  A bad charge leaves the seed untouched. */
+KF_API int kf_build_combinatorial(kf_ctx* ctx, const kf_geometry* geom, int first_layer, int n_build_layers,
+                                  kf_tracks* cands, const kf_layer_hits* hits, const kf_layer_bins* bins,
+                                  int window_half, float chi2_cut, int n_cand, int32_t* hit_index,
+                                  int32_t* n_found, int64_t ld_out);
+
 #ifdef __cplusplus
 }
 #endif

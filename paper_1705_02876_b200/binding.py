@@ -21,7 +21,7 @@ _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so"
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
            "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
-           "kf_score_candidates", "kf_build_best_hit"]
+           "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial"]
 
 
 class KFError(RuntimeError):
@@ -110,6 +110,10 @@ def load_library():
     lib.kf_build_best_hit.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
                                       C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
                                       vp, vp, vp, C.c_int64]
+    lib.kf_build_combinatorial.restype = C.c_int
+    lib.kf_build_combinatorial.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
+                                           C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
+                                           vp, vp, C.c_int64]
     _lib = lib
     return lib
 
@@ -346,4 +350,19 @@ class KFContext:
                                                 order.data_ptr() if order is not None else None,
                                                 hit_index.data_ptr(), hit_chi2.data_ptr(), int(hit_index.stride(0))),
                     "kf_build_best_hit")
+        del keep
+
+    # ------------------------------------------------------------------ kf_build_combinatorial
+    def build_combinatorial(self, geom: Geometry, first_layer: int, n: int, par, cov, q, chi2, nhits, status,
+                            layers, window_half: int, chi2_cut: float, n_cand: int, hit_index, n_found=None):
+        g, keep = geom._c()
+        cands = self._tracks(n, par, cov, q, chi2, nhits, status)
+        m = len(layers)
+        lhs = (_LayerHits * m)(*[self._layer_hits(nh, p, c) for (nh, p, c, _) in layers])
+        lbs = (_LayerBins * m)(*[b._c() for (_, _, _, b) in layers])
+        self._check(self._lib.kf_build_combinatorial(self._h, C.byref(g), int(first_layer), m, C.byref(cands), lhs, lbs,
+                                                     int(window_half), float(chi2_cut), int(n_cand),
+                                                     hit_index.data_ptr(),
+                                                     n_found.data_ptr() if n_found is not None else None,
+                                                     int(hit_index.stride(0))), "kf_build_combinatorial")
         del keep

@@ -172,6 +172,16 @@ class DeviceCandidates:
                            idx, c2, order)
         return idx, c2
 
+    def build_combinatorial(self, ctx: KFContext, geom: Geometry, first_layer: int, layers: list, n_cand: int,
+                            window_half: int = 2, chi2_cut: float = 30.0):
+        """kf_build_combinatorial; returns (hit_index[len(layers)][ld], n_found[ld]) device tensors."""
+        idx = torch.empty((len(layers), self.ld), dtype=torch.int32, device=self.par.device)
+        nf = torch.zeros(self.ld, dtype=torch.int32, device=self.par.device)
+        ctx.build_combinatorial(geom, first_layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits,
+                                self.status, [(l.n_hits, l.pos, l.cov, l.bins) for l in layers], window_half,
+                                chi2_cut, n_cand, idx, nf)
+        return idx, nf
+
     def make_order(self, ctx: KFContext, geom: Geometry, layer: int, n_eta: int, n_phi: int, eta_max: float):
         order = torch.empty(max(self.n, 1), dtype=torch.int32, device=self.par.device)
         ctx.order_candidates(geom, layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,

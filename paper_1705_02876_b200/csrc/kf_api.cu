@@ -19,13 +19,14 @@ struct kf_ctx {
     BinScratch bin;
     // kf_score_candidates / kf_build_best_hit scratch
     ScoreScratch score;
+    CombScratch comb;
     // *_host staging
     HostStage host;
 };
 
 namespace {
 
-constexpr int kAbiVersion = 4;
+constexpr int kAbiVersion = 5;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -130,6 +131,7 @@ int kf_destroy(kf_ctx* c) {
     cudaSetDevice(c->device);
     c->bin.release();
     c->score.release();
+    c->comb.release();
     c->host.release();
     delete c;
     return KF_OK;
@@ -383,6 +385,47 @@ int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n
     cudaError_t e = cudaSetDevice(c->device);
     if (e != cudaSuccess) return cuda_fail(c, e);
     e = launch_build(c->score, P, a, n_build_layers, steps, c->stream);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_build_combinatorial(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,
+                           const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half, float chi2_cut,
+                           int n_cand, int32_t* hit_index, int32_t* n_found, int64_t ld_out) {
+    if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
+    if (n_cand < 1 || n_cand > 8) return KF_ERR_UNSUPPORTED;
+    if ((rc = check_tracks(cands, true, true))) return rc;
+    if (n_build_layers == 0 || cands->n == 0) return KF_OK;
+    if (!hit_index) return KF_ERR_NULL;
+    if (ld_out < cands->n) return KF_ERR_SHAPE;
+    if (cands->n * (int64_t)n_cand > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
+    ScoreStep steps[KF_MAX_LAYERS];
+    for (int j = 0; j < n_build_layers; ++j) {
+        if ((rc = check_score_bins(hits + j, bins + j, window_half))) return rc;
+        if (bins[j].n_eta != bins[0].n_eta || bins[j].n_phi != bins[0].n_phi || bins[j].eta_max != bins[0].eta_max)
+            return KF_ERR_UNSUPPORTED;
+        steps[j].layer = first_layer + j;
+        steps[j].n_hits = hits[j].n_hits;
+        steps[j].hit_rec = bins[j].hit_rec;
+        steps[j].bin_box = bins[j].bin_box;
+        steps[j].bin_offset = bins[j].bin_offset;
+        steps[j].best_hit = nullptr;
+        steps[j].best_chi2 = nullptr;
+    }
+    CombCall call;
+    call.n_seeds = cands->n; call.ld = cands->ld; call.par = cands->par; call.cov = cands->cov; call.q = cands->q;
+    call.chi2 = cands->chi2; call.nhits = cands->nhits; call.status = cands->status;
+    call.n_cand = n_cand;
+    call.n_eta = bins[0].n_eta; call.n_phi = bins[0].n_phi; call.eta_max = bins[0].eta_max;
+    call.window_half = window_half; call.chi2_cut = chi2_cut;
+    call.hit_index = hit_index; call.ld_out = ld_out; call.n_found = n_found;
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = launch_comb(c->comb, P, call, n_build_layers, steps, c->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
 }

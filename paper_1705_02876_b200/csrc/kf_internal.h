@@ -152,6 +152,26 @@ struct ScoreScratch {
 cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n_steps, const ScoreStep* steps,
                          cudaStream_t stream);
 
+// ---------------------------------------------------------------------------------- combinatorial building
+struct CombCall {
+    int64_t n_seeds, ld;
+    float* par; float* cov; const int8_t* q; float* chi2; int32_t* nhits; uint32_t* status;
+    int n_cand;
+    int n_eta, n_phi; float eta_max; int window_half; float chi2_cut;
+    int32_t* hit_index; int64_t ld_out; int32_t* n_found;
+};
+
+struct CombScratch {
+    int64_t cap_words = 0;
+    void* buf = nullptr;
+    cudaError_t reserve(int64_t words, cudaStream_t stream);
+    void release();
+};
+
+// kf_comb.cu
+cudaError_t launch_comb(CombScratch& s, const FitParams& P, const CombCall& call, int n_steps, const ScoreStep* steps,
+                        cudaStream_t stream);
+
 // kf_peak.cu
 double measure_fp32_peak(cudaStream_t stream, int repeats, float* sink);
 

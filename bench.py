@@ -189,6 +189,21 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
         if it >= 2:
             t_bin.append(e[0].elapsed_time(e[1]))
             t_build.append(e[1].elapsed_time(e[2]))
+    # combinatorial building (reading A19), 4 candidates per seed, same seeds and bins
+    t_comb = []
+    for it in range(5):
+        dc = DeviceCandidates.from_numpy(s["par"], s["cov"], f.q, s["chi2"], s["nhits"], dev)
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(st)
+        cidx, cnf = dc.build_combinatorial(ctx, geom, L0, layers, 4)
+        c1.record(st)
+        torch.cuda.synchronize()
+        if it >= 1:
+            t_comb.append(c0.elapsed_time(c1))
+    truth = np.stack([ev.layers[l].true_index for l in range(L0, L)])
+    comb_eff = float((cidx[:, :f.n].cpu().numpy() == truth).all(axis=0).mean())
+    best_eff = float((idx[:, :f.n].cpu().numpy() == truth).all(axis=0).mean())
     # algorithmic work: 850 + 60 n_window flop per candidate and layer, n_window counted
     # from the bins around each candidate's true hit on that layer
     n_win = 0
@@ -214,7 +229,11 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
             "build_ms": ts, "candidate_layers_per_s": n_cl / (ts * 1e-3),
             "window_hits_scored_per_s": n_win / (ts * 1e-3), "mean_window_hits": n_win / n_cl,
             "algorithmic_gflop": flops / 1e9, "hit_taken_fraction": taken,
-            "kernels_per_build": 2 * (L - L0) + 1, "reps": reps}
+            "kernels_per_build": 2 * (L - L0) + 1, "reps": reps,
+            "combinatorial": {"n_cand": 4, "build_ms": float(np.median(t_comb)),
+                              "seeds_per_s": f.n / (float(np.median(t_comb)) * 1e-3),
+                              "all_true_hits_found_fraction": comb_eff,
+                              "best_hit_all_true_hits_found_fraction": best_eff, "kernels": 4 * (L - L0) + 2}}
 
 
 def run_ours(args) -> None:

@@ -6,7 +6,7 @@
 //   comb_propagate  one thread per live slot: local-frame track -> propagate (+Q) -> scratch (as best-hit);
 //   comb_scan       one warp per live slot: the same bin-pruned, pre-filtered window scan as the best-hit
 //                   scan, but it keeps the NC best compatible hits (chi2 < cut) instead of one;
-//   comb_select     one thread per seed ("clone engine"): ranks the children of all its
+//   comb_select     one warp per seed ("clone engine"): ranks the children of all its
 //                   candidates -- each kept hit, plus "no hit" -- by (nhits desc, chi2 asc, parent slot,
 //                   hit index) and writes the NC best as (parent, hit) descriptors: only descriptors are
 //                   sorted, no track is copied here;
@@ -237,50 +237,86 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
     if (lane == 0) a.top_n[slot] = nacc;
 }
 
-// "Clone engine": one thread per seed ranks the children of its candidates and writes the
-// best nc as descriptors.  Key: nhits descending, chi2 ascending, parent slot ascending, hit index ascending
-// with "no hit" last.  Nothing but descriptors moves here.
+// "Clone engine": ranks the children of a seed's candidates and writes the best nc as
+// descriptors.  Key: nhits descending, chi2 ascending, parent slot ascending, hit index ascending with
+// "no hit" last.  Nothing but descriptors moves here.
+struct ChildKey {
+    int nh;          // hits after this layer
+    float chi2;
+    int parent;
+    int32_t orig;    // original hit index, INT_MAX for "no hit"
+    int e;           // child id = parent * (kMaxC + 1) + (k + 1), -1 = none
+};
+
+__device__ __forceinline__ bool child_before(const ChildKey& x, const ChildKey& y) {
+    if (y.e < 0) return x.e >= 0;
+    if (x.e < 0) return false;
+    if (x.nh != y.nh) return x.nh > y.nh;
+    if (x.chi2 != y.chi2) return x.chi2 < y.chi2;
+    if (x.parent != y.parent) return x.parent < y.parent;
+    return x.orig < y.orig;
+}
+
+// One WARP per seed: the <= nc * (nc + 1) children sit three to a lane; nc rounds of warp arg-min.
 __global__ void __launch_bounds__(128)
 comb_select_kernel(const CombArgs a) {
-    const int64_t sd = (int64_t)blockIdx.x * 128 + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const int64_t sd = ((int64_t)blockIdx.x * 128 + threadIdx.x) >> 5;
     if (sd >= a.n_seeds) return;
     const int ncur = a.ncand_in[sd];
     const int64_t base = sd * a.nc;
-    // taken[p] bit k: child k of parent p already chosen (k = 0..top_n-1 hits, bit 31 = the no-hit child)
-    uint32_t taken[kMaxC];
+    constexpr int kPer = (kMaxC * (kMaxC + 1) + 31) / 32;   // 3
+    ChildKey mine[kPer];
+    int32_t rec[kPer];
 #pragma unroll
-    for (int p = 0; p < kMaxC; ++p) taken[p] = 0u;
-    int kept = 0;
-    for (int out = 0; out < a.nc; ++out) {
-        int bp = -1, bk = 0, bnh = -1;
-        float bc = 0.0f;
-        int64_t bo = 0;
-        for (int p = 0; p < ncur; ++p) {
+    for (int r = 0; r < kPer; ++r) {
+        const int e = lane + 32 * r;
+        const int p = e / (kMaxC + 1), k = e % (kMaxC + 1) - 1;
+        mine[r].e = -1; mine[r].nh = 0; mine[r].chi2 = 0.0f; mine[r].parent = p; mine[r].orig = 0x7fffffff;
+        rec[r] = REC_NONE;
+        if (p < ncur) {
             const int64_t sp = base + p;
-            const int32_t f = a.flag[sp];
-            const int nh0 = a.nh_in[sp];
-            const float c0 = a.chi2_in[sp];
-            const int nk = f == FLAG_AT_LAYER ? a.top_n[sp] : 0;
-            for (int k = -1; k < nk; ++k) {            // k = -1: the child without a hit (or the stuck parent)
-                const uint32_t bit = k < 0 ? 0x80000000u : (1u << k);
-                if (taken[p] & bit) continue;
-                const int nh = nh0 + (k >= 0 ? 1 : 0);
-                const float c = k >= 0 ? c0 + a.top_chi2[sp * kMaxC + k] : c0;
-                const int64_t o = k >= 0 ? (int64_t)a.top_orig[sp * kMaxC + k] : ((int64_t)1 << 40);
-                const bool first = bp < 0;
-                const bool wins = first || nh > bnh || (nh == bnh && (c < bc || (c == bc && (p < bp || (p == bp && o < bo)))));
-                if (wins) { bp = p; bk = k; bnh = nh; bc = c; bo = o; }
+            const bool at = a.flag[sp] == FLAG_AT_LAYER;
+            const int nk = at ? a.top_n[sp] : 0;
+            if (k < nk) {
+                mine[r].e = e;
+                mine[r].nh = a.nh_in[sp] + (k >= 0 ? 1 : 0);
+                mine[r].chi2 = a.chi2_in[sp] + (k >= 0 ? a.top_chi2[sp * kMaxC + k] : 0.0f);
+                if (k >= 0) { mine[r].orig = a.top_orig[sp * kMaxC + k]; rec[r] = a.top_rec[sp * kMaxC + k]; }
+                else rec[r] = at ? REC_NONE : REC_STUCK;
             }
         }
-        if (bp < 0) break;
-        taken[bp] |= bk < 0 ? 0x80000000u : (1u << bk);
-        const int64_t so = base + out, sp = base + bp;
-        a.child_parent[so] = bp;
-        a.child_rec[so] = bk >= 0 ? a.top_rec[sp * kMaxC + bk] : (a.flag[sp] == FLAG_AT_LAYER ? REC_NONE : REC_STUCK);
-        a.child_orig[so] = bk >= 0 ? a.top_orig[sp * kMaxC + bk] : -1;
+    }
+    int kept = 0;
+    for (int out = 0; out < a.nc; ++out) {
+        ChildKey b = mine[0];
+        int br = 0;
+#pragma unroll
+        for (int r = 1; r < kPer; ++r)
+            if (child_before(mine[r], b)) { b = mine[r]; br = r; }
+        ChildKey w = b;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            ChildKey o;
+            o.nh = __shfl_xor_sync(0xffffffffu, w.nh, d);
+            o.chi2 = __shfl_xor_sync(0xffffffffu, w.chi2, d);
+            o.parent = __shfl_xor_sync(0xffffffffu, w.parent, d);
+            o.orig = __shfl_xor_sync(0xffffffffu, w.orig, d);
+            o.e = __shfl_xor_sync(0xffffffffu, w.e, d);
+            if (child_before(o, w)) w = o;
+        }
+        if (w.e < 0) break;                       // warp-uniform: no child left
+        if (b.e == w.e) {                         // this lane owns the winner
+            const int64_t so = base + out;
+            a.child_parent[so] = w.parent;
+            a.child_orig[so] = w.orig == 0x7fffffff ? -1 : w.orig;
+#pragma unroll
+            for (int r = 0; r < kPer; ++r)
+                if (r == br) { a.child_rec[so] = rec[r]; mine[r].e = -1; }
+        }
         kept = out + 1;
     }
-    a.ncand_out[sd] = kept;
+    if (lane == 0) a.ncand_out[sd] = kept;
 }
 
 // One thread per surviving child: materialise it in the other half of the candidate store.
@@ -417,7 +453,7 @@ cudaError_t launch_comb(CombScratch& s, const FitParams& P, const CombCall& call
         a.hist_hit = hist_hit + (int64_t)j * S;
         comb_propagate_kernel<<<slot_blocks, 128, 0, stream>>>(P, a, sp.layer);
         comb_scan_kernel<<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
-        comb_select_kernel<<<seed_blocks, 128, 0, stream>>>(a);
+        comb_select_kernel<<<(unsigned)((call.n_seeds + 3) / 4), 128, 0, stream>>>(a);
         comb_update_kernel<<<slot_blocks, 128, 0, stream>>>(a);
         cur ^= 1;
         bind(cur);

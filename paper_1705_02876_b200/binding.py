@@ -68,6 +68,13 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
+    if not os.path.exists(_LIB_PATH) and "KF_B200_LIB" not in os.environ:
+        try:                                   # safety net: compile in-tree if nvcc is around
+            from . import build as _build
+            _build.build()
+        except Exception as exc:               # noqa: BLE001 -- any failure ends in the loud error below
+            raise ImportError(f"{_LIB_PATH} is missing and could not be built ({exc}); run "
+                              "`python -m paper_1705_02876_b200.build` (there is no CPU or PyTorch fallback)")
     if not os.path.exists(_LIB_PATH):
         raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_1705_02876_b200.build` "
                           "(there is no CPU or PyTorch fallback)")

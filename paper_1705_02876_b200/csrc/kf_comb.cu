@@ -72,8 +72,8 @@ comb_propagate_kernel(const __grid_constant__ FitParams P, const CombArgs a, int
     Track t;
     get_track(a.trk_in, a.ld_s, slot, t);
     const float qf = (float)a.q[sd];
-    const bool ok = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.mass2, a.scratch,
-                                                a.ld_s, slot);
+    const bool ok = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.mass2,
+                                                BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch, a.ld_s, slot);
     a.flag[slot] = ok ? FLAG_AT_LAYER : FLAG_IDLE;
 }
 
@@ -135,14 +135,8 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
     c.zn = a.scratch[SC_ZN * a.ld_s + slot];   c.ec = a.scratch[SC_ERX * a.ld_s + slot];
     c.es = a.scratch[SC_ERY * a.ld_s + slot];  c.n11 = a.scratch[SC_N11 * a.ld_s + slot];
     c.n12 = a.scratch[SC_N12 * a.ld_s + slot]; c.n22 = a.scratch[SC_N22 * a.ld_s + slot];
-    const float eta = asinhf(c.zn * inv_r);
-    const float phi = atan2f(c.yn, c.xn);
-    const float d_eta = 2.0f * a.eta_max / (float)a.n_eta;
-    const float d_phi = 2.0f * CUDART_PI_F / (float)a.n_phi;
-    int ie = (int)floorf((eta + a.eta_max) / d_eta);
-    ie = ie < 0 ? 0 : (ie > a.n_eta - 1 ? a.n_eta - 1 : ie);
-    int ip = (int)floorf((phi + CUDART_PI_F) / d_phi);
-    ip = ((ip % a.n_phi) + a.n_phi) % a.n_phi;
+    const int cbin = __float_as_int(a.scratch[SC_BIN * a.ld_s + slot]);   // window centre, made by the propagate kernel
+    const int ie = cbin >> 16, ip = cbin & 0xffff;
 
     int32_t* list = survivors[threadIdx.x >> 5];
     AccEntry* acc = accs[threadIdx.x >> 5];

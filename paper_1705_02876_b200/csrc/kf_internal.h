@@ -109,7 +109,9 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
                          cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------- scoring
-constexpr int kScorePlanes = 28;
+constexpr int kScorePlanes = 29;
+
+struct BinGrid { int n_eta, n_phi; float eta_max; };
 
 struct ScoreArgs {
     int64_t n, ld;

@@ -64,7 +64,7 @@ propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
     enter_local_frame(t);
     if (keep_track) put_track(a.track, a.ld_sc, i, t);
     const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
-    const bool ok = propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.mass2, a.scratch, a.ld_sc, i);
+    const bool ok = propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.mass2, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch, a.ld_sc, i);
     if (!ok) a.status[i] |= ST_PROP_FAIL;
     a.flag[i] = ok ? FLAG_AT_LAYER : FLAG_IDLE;
 }
@@ -80,8 +80,8 @@ update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
     if (f == FLAG_AT_LAYER) { apply_decision(a, i, t); put_track(a.track, a.ld_sc, i, t); }
     else get_track(a.track, a.ld_sc, i, t);
     const float qf = (float)a.q[i];
-    const bool ok = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.mass2, a.scratch,
-                                                a.ld_sc, i);
+    const bool ok = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.mass2,
+                                                BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch, a.ld_sc, i);
     if (!ok) a.status[i] |= ST_PROP_FAIL;
     a.flag[i] = ok ? FLAG_AT_LAYER : FLAG_IDLE;
 }
@@ -119,15 +119,8 @@ scan_kernel(const ScoreArgs a, float inv_r) {
     c.es = a.scratch[SC_ERY * a.ld_sc + i];  c.n11 = a.scratch[SC_N11 * a.ld_sc + i];
     c.n12 = a.scratch[SC_N12 * a.ld_sc + i]; c.n22 = a.scratch[SC_N22 * a.ld_sc + i];
 
-    // the candidate's own bin (reading A16): eta = asinh(z'/r), phi = atan2(y', x')
-    const float eta = asinhf(c.zn * inv_r);
-    const float phi = atan2f(c.yn, c.xn);
-    const float d_eta = 2.0f * a.eta_max / (float)a.n_eta;
-    const float d_phi = 2.0f * CUDART_PI_F / (float)a.n_phi;
-    int ie = (int)floorf((eta + a.eta_max) / d_eta);
-    ie = ie < 0 ? 0 : (ie > a.n_eta - 1 ? a.n_eta - 1 : ie);
-    int ip = (int)floorf((phi + CUDART_PI_F) / d_phi);
-    ip = ((ip % a.n_phi) + a.n_phi) % a.n_phi;
+    const int cbin = __float_as_int(a.scratch[SC_BIN * a.ld_sc + i]);   // window centre, made by the propagate kernel
+    const int ie = cbin >> 16, ip = cbin & 0xffff;
 
     Best best;
     best.chi2 = CUDART_INF_F; best.orig = 0x7fffffff; best.slot = -1;

@@ -17,6 +17,7 @@ enum : int {
     SC_XN, SC_YN, SC_ZN, SC_ERX, SC_ERY, SC_N11, SC_N12, SC_N22,   // scan + update
     SC_PXN, SC_PYN, SC_PZ, SC_ELX, SC_ELY, SC_T, SC_PT2, SC_IPT,   // update
     SC_N13, SC_N14, SC_N15, SC_N23, SC_N24, SC_N25, SC_N33, SC_N34, SC_N35, SC_N44, SC_N45, SC_N55,
+    SC_BIN,                                                         // window centre (i_eta << 16 | i_phi), int bits
     SC_PLANES
 };
 static_assert(SC_PLANES == kScorePlanes, "scratch plane count");
@@ -61,12 +62,21 @@ __device__ __forceinline__ void hit_from_record(const float4* __restrict__ rec, 
 // Propagate a local-frame track to layer Lc and park the result in the scratch; flags[i] = 1 if it got there.
 template <bool RADIAL_NULL>
 __device__ __forceinline__ bool propagate_to_scratch(const Track& t, float k, float ik, const LayerConst& Lc,
-                                                     float mass2, float* sc, int64_t ld, int64_t i) {
+                                                     float mass2, const BinGrid& g, float* sc, int64_t ld, int64_t i) {
     Crossing o;
     if (!helix_to_radius(t, k, ik, Lc, o)) return false;
     PropCov n;
     transport_cov<RADIAL_NULL>(t, o, Lc.ms, mass2, n);
     put_scratch(sc, ld, i, o, n, t.pz);
+    // the candidate's own bin (reading A16): eta = asinh(z'/r), phi = atan2(y', x') -- once per candidate
+    // here, not once per lane in the scan
+    const float eta = asinhf(o.zn * Lc.inv_r);
+    const float phi = atan2f(o.yn, o.xn);
+    int ie = (int)floorf((eta + g.eta_max) / (2.0f * g.eta_max / (float)g.n_eta));
+    ie = ie < 0 ? 0 : (ie > g.n_eta - 1 ? g.n_eta - 1 : ie);
+    int ip = (int)floorf((phi + CUDART_PI_F) / (2.0f * CUDART_PI_F / (float)g.n_phi));
+    ip = ((ip % g.n_phi) + g.n_phi) % g.n_phi;
+    sc[(int64_t)SC_BIN * ld + i] = __int_as_float((ie << 16) | ip);
     return true;
 }
 

@@ -311,6 +311,30 @@ def run_ours(args) -> None:
         torch.cuda.synchronize()
         sm_ms = s0.elapsed_time(s1) / 20
         sm_bytes = n * (113 + 2 * 36 * L + 2 * 120)
+        # secondary: kf_fit_tracks_indexed -- same tracks, each layer's hits shuffled into a pool and addressed by index
+        g = torch.Generator(device=dev); g.manual_seed(5)
+        perm = [torch.randperm(n, device=dev, generator=g) for _ in range(L)]
+        pools = []
+        index = torch.full((L, d.ld), -1, dtype=torch.int32, device=dev)
+        for l in range(L):
+            pp = torch.zeros((3, d.ld), dtype=torch.float32, device=dev); pc = torch.zeros((6, d.ld), dtype=torch.float32, device=dev)
+            pp[:, :n] = d.hpos[l][:, :n][:, perm[l]]; pc[:, :n] = d.hcov[l][:, :n][:, perm[l]]
+            inv = torch.empty(n, dtype=torch.int64, device=dev); inv[perm[l]] = torch.arange(n, device=dev)
+            index[l, :n] = inv.to(torch.int32)
+            pools.append((n, pp, pc))
+        with torch.cuda.stream(stream):
+            for _ in range(2):
+                ctx.fit_tracks_indexed(d.geom, n, d.par, d.cov, d.q, index, pools, d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status)
+            i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            i0.record(stream)
+            for _ in range(10):
+                ctx.fit_tracks_indexed(d.geom, n, d.par, d.cov, d.q, index, pools, d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status)
+            i1.record(stream)
+        torch.cuda.synchronize()
+        ix_ms = i0.elapsed_time(i1) / 10
+        indexed = {"api": "kf_fit_tracks_indexed (hits gathered by index from shuffled layer pools)", "ms": ix_ms,
+                   "fits_per_s": n / (ix_ms * 1e-3), "sector_bytes_per_fit": 233 + L * (4 + 9 * 32)}
+        del pools, perm, index
         smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10)", "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3),
                      "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0],
                      "alu_roofline_frac": 2.0 * n * FLOPS_PER_TRACK_LAYER * L / (sm_ms * 1e-3) / (fp32_peak * 1e12)}
@@ -352,6 +376,7 @@ def run_ours(args) -> None:
             out["building"] = building
         if smoothing is not None:
             out["smoothing"] = smoothing
+            out["indexed_fit"] = indexed
         print(json.dumps(out), flush=True)
     ctx.close()
     sharding.shutdown()

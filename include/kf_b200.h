@@ -178,6 +178,14 @@ typedef struct {
     float* cov_sorted;        /* DEV [6][ld] optional (NULL = not written)                          */
 } kf_layer_bins;
 
+/* Fit with the hits addressed by index (what a builder hands to the fitter): the hit of
+ * track t on layer l is hit index[l*ld_index + t] of pools[l] (HOST array of n_layers descriptors, DEV
+ * buffers inside), -1 = no hit on that layer.  Otherwise exactly kf_fit_tracks (same arithmetic, same
+ * status semantics, `out` may alias `seeds`).  index: DEV int32 [n_layers][ld_index], ld_index >= n. */
+KF_API int kf_fit_tracks_indexed(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                                 const int32_t* index, int64_t ld_index, const kf_layer_hits* pools,
+                                 kf_tracks* out);
+
 /* Bin one layer's hits: bin = i_eta*n_phi + i_phi with eta = asinh(z/radius), phi = atan2(y,x) over
  * [-pi, pi); stable counting sort (within a bin, original order).  The bin of a hit is decided in
  * single precision against tabulated edges (reading A16b).  `out` arrays are

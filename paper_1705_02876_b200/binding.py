@@ -20,7 +20,7 @@ _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so"
 
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial"]
 
 
@@ -100,6 +100,9 @@ def load_library():
         f = getattr(lib, name)
         f.restype = C.c_int
         f.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.POINTER(_Tracks)]
+    lib.kf_fit_tracks_indexed.restype = C.c_int
+    lib.kf_fit_tracks_indexed.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), vp, C.c_int64,
+                                          C.POINTER(_LayerHits), C.POINTER(_Tracks)]
     lib.kf_fit_tracks_smooth.restype = C.c_int
     lib.kf_fit_tracks_smooth.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.c_float,
                                          C.POINTER(_Tracks), C.POINTER(_Tracks)]
@@ -266,6 +269,21 @@ class KFContext:
         hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
         self._check(self._lib.kf_fit_tracks(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)),
                     "kf_fit_tracks")
+        del keep
+
+    def fit_tracks_indexed(self, geom: Geometry, n: int, par, cov, q, index, pools,
+                           out_par, out_cov, out_chi2, out_nhits, out_status):
+        """Fit with hits addressed by index: index int32 [L][ld_index] (device), pools = [(n_hits, pos, cov), ...]
+        one per geometry layer."""
+        g, keep = geom._c()
+        seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
+        out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
+        m = len(pools)
+        if m != g.n_layers or index.shape[0] != m:
+            raise ValueError("one pool and one index row per geometry layer")
+        lhs = (_LayerHits * m)(*[self._layer_hits(nh, p, c) for (nh, p, c) in pools])
+        self._check(self._lib.kf_fit_tracks_indexed(self._h, C.byref(g), C.byref(seeds), index.data_ptr(),
+                                                    int(index.stride(0)), lhs, C.byref(out)), "kf_fit_tracks_indexed")
         del keep
 
     def fit_tracks_smooth(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask, kappa: float,

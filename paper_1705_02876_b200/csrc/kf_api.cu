@@ -26,7 +26,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 5;
+constexpr int kAbiVersion = 6;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -195,6 +195,36 @@ int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
     a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
     a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
     cudaError_t e = launch_fit(P, a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_fit_tracks_indexed(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const int32_t* index,
+                          int64_t ld_index, const kf_layer_hits* pools, kf_tracks* out) {
+    if (!c || !geom || !seeds || !pools || !out) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if ((rc = check_tracks(seeds, true, true))) return rc;
+    if ((rc = check_tracks(out, false, true))) return rc;
+    if (out->n != seeds->n || ld_index < seeds->n) return KF_ERR_SHAPE;
+    if (seeds->n == 0) return KF_OK;
+    if (!index) return KF_ERR_NULL;
+    IndexedPools H;
+    std::memset(&H, 0, sizeof(H));
+    for (int l = 0; l < geom->n_layers; ++l) {
+        if (pools[l].n_hits < 0 || pools[l].ld < pools[l].n_hits) return KF_ERR_SHAPE;
+        if (pools[l].n_hits > 0 && (!pools[l].pos || !pools[l].cov)) return KF_ERR_NULL;
+        H.pos[l] = pools[l].pos; H.cov[l] = pools[l].cov; H.ld[l] = pools[l].ld;
+    }
+    H.index = index; H.ld_index = ld_index;
+    FitArgs a;
+    a.n = seeds->n;
+    a.par = seeds->par; a.cov = seeds->cov; a.ld_in = seeds->ld; a.q = seeds->q;
+    a.hpos = nullptr; a.hcov = nullptr; a.ld_hit = 0; a.mask = nullptr;
+    a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
+    a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
+    cudaError_t e = launch_fit_indexed(P, H, a, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;
 }

@@ -319,6 +319,63 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
     if (storer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // smem must outlive the store
 }
 
+// ---- fit with hits addressed by index into the layer pools (the hits a track uses are
+// looked up, not pre-gathered).  index[l][i] = hit of track i in pool l or -1.
+// Gathered loads cannot go through TMA: each thread fetches its 9 floats itself, one layer ahead.
+__device__ __forceinline__ Hit gather_hit(const IndexedPools& H, int l, int32_t h) {
+    Hit m;
+    const float* p = H.pos[l];
+    const float* c = H.cov[l];
+    const int64_t ld = H.ld[l];
+    m.x = __ldg(p + h);            m.y = __ldg(p + ld + h);       m.z = __ldg(p + 2 * ld + h);
+    m.vxx = __ldg(c + h);          m.vxy = __ldg(c + ld + h);     m.vxz = __ldg(c + 2 * ld + h);
+    m.vyy = __ldg(c + 3 * ld + h); m.vyz = __ldg(c + 4 * ld + h); m.vzz = __ldg(c + 5 * ld + h);
+    return m;
+}
+
+__global__ void __launch_bounds__(kFitBlock, 4)
+fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ IndexedPools H, const FitArgs a) {
+    const int64_t i = (int64_t)blockIdx.x * kFitBlock + threadIdx.x;
+    if (i >= a.n) return;
+    const int L = P.n_layers;
+    const int q = a.q[i];
+    Track t;
+    load_track(t, a.par, a.cov, a.ld_in, i);
+    float chi2 = 0.0f;
+    int nh = 0;
+    uint32_t st = 0u;
+    if (q != 1 && q != -1) {
+        st = ST_BAD_CHARGE;
+    } else {
+        const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
+        enter_local_frame(t);
+        bool started = false;
+        int32_t h_next = __ldg(H.index + i);
+        Hit m_next;
+        if (h_next >= 0) m_next = gather_hit(H, 0, h_next);
+        for (int l = 0; l < L; ++l) {
+            const int32_t h = h_next;
+            const Hit m = m_next;
+            if (l + 1 < L) {
+                h_next = __ldg(H.index + (int64_t)(l + 1) * H.ld_index + i);
+                if (h_next >= 0) m_next = gather_hit(H, l + 1, h_next);
+            }
+            if (h < 0) continue;
+            uint32_t rc;
+            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.mass2, m, chi2);
+            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.mass2, m, chi2);
+            st |= rc;
+            if (rc == 0u) { nh += 1; started = true; }
+        }
+        if (nh > 0) leave_local_frame(t);
+        else load_track(t, a.par, a.cov, a.ld_in, i);   // nothing fitted: the seed, bit-exact
+    }
+    store_track(t, a.opar, a.ocov, a.ld_out, i);
+    a.chi2[i] = chi2;
+    a.nhits[i] = nh;
+    a.status[i] = st;
+}
+
 }  // namespace
 
 namespace {
@@ -373,6 +430,13 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
     if (smooth) fit_kernel<true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else fit_kernel<false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fit_indexed(const FitParams& P, const IndexedPools& H, const FitArgs& a, cudaStream_t stream) {
+    if (a.n == 0) return cudaSuccess;
+    const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
+    fit_indexed_kernel<<<(unsigned)blocks, kFitBlock, 0, stream>>>(P, H, a);
     return cudaGetLastError();
 }
 

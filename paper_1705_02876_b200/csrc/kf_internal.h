@@ -26,7 +26,16 @@ struct FitArgs {
     float kappa = 10.0f;
 };
 
+struct IndexedPools {           // per-layer hit pools + the per-track hit indices into them
+    const float* pos[32];
+    const float* cov[32];
+    int64_t ld[32];
+    const int32_t* index;       // [n_layers][ld_index], -1 = no hit
+    int64_t ld_index;
+};
+
 // kf_fit.cu
+cudaError_t launch_fit_indexed(const FitParams& P, const IndexedPools& H, const FitArgs& a, cudaStream_t stream);
 cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------- host path

@@ -297,6 +297,7 @@ def run_ours(args) -> None:
     same = all(np.array_equal(a, b) for a, b in zip(d.results().values(), h.results().values()))
     fp32_peak = ctx.measure_fp32_peak(5) if rank == 0 else 0.0
     building = measure_building(ctx, dev) if (rank == 0 and not args.no_building) else None
+    ctx.set_stream(stream)          # measure_building borrowed the context for torch's current stream
     smoothing = None
     if rank == 0 and not args.no_building:
         # secondary: kf_fit_tracks_smooth on the same batch (forward fit + inward refit, one kernel)
@@ -333,7 +334,8 @@ def run_ours(args) -> None:
         torch.cuda.synchronize()
         ix_ms = i0.elapsed_time(i1) / 10
         indexed = {"api": "kf_fit_tracks_indexed (hits gathered by index from shuffled layer pools)", "ms": ix_ms,
-                   "fits_per_s": n / (ix_ms * 1e-3), "sector_bytes_per_fit": 233 + L * (4 + 9 * 32)}
+                   "fits_per_s": n / (ix_ms * 1e-3), "sector_bytes_per_fit": 233 + L * (4 + 9 * 32),
+                   "note": "nine scattered 4-byte loads per hit: bound by 32-byte DRAM/L2 sectors, not by arithmetic"}
         del pools, perm, index
         smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10)", "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3),
                      "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0],

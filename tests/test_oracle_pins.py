@@ -283,3 +283,16 @@ def test_P10_rotation_about_z():
     np.testing.assert_allclose(r2["par"], R6 @ r1["par"], rtol=0, atol=1e-10)
     np.testing.assert_allclose(r2["cov"], np.einsum("ij,njk,lk->nil", R6, r1["cov"], R6), rtol=1e-8, atol=1e-13)
     np.testing.assert_allclose(r2["chi2"], r1["chi2"], rtol=1e-10)
+
+
+# ------------------------------------------------------------------------------------ regression anchor
+def test_oracle_fit_matches_its_stored_values():
+    """tests/golden/oracle_fit_config1_8tracks.txt was written by tests/golden/make_oracle_fit_golden.py
+    (oracle only).  It does not pin the oracle to the mathematics -- P1..P10 and S1..S4 do -- it makes a
+    change of the oracle's arithmetic visible."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("mk", os.path.join(GOLD, "make_oracle_fit_golden.py"))
+    mk = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mk)
+    want = np.loadtxt(os.path.join(GOLD, "oracle_fit_config1_8tracks.txt"))
+    np.testing.assert_allclose(mk.compute(), want, rtol=1e-10, atol=1e-12)

@@ -333,8 +333,23 @@ def run_ours(args) -> None:
             i1.record(stream)
         torch.cuda.synchronize()
         ix_ms = i0.elapsed_time(i1) / 10
+        # same, reading the packed records of kf_bin_layers (one look-up + one 48-byte record per hit)
+        from paper_1705_02876_b200.binding import Bins
+        pbins = [Bins.allocate(n, 40, 64, float(np.float32(1.2)), dev, soa=False) for _ in range(L)]
+        ctx.bin_layers([float(r) for r in d.geom.radius_cm], [(n, pp, pc, b_) for (_, pp, pc), b_ in zip(pools, pbins)])
+        with torch.cuda.stream(stream):
+            for _ in range(2):
+                ctx.fit_tracks_indexed(d.geom, n, d.par, d.cov, d.q, index, pools, d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status, bins=pbins)
+            i0.record(stream)
+            for _ in range(10):
+                ctx.fit_tracks_indexed(d.geom, n, d.par, d.cov, d.q, index, pools, d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status, bins=pbins)
+            i1.record(stream)
+        torch.cuda.synchronize()
+        ixr_ms = i0.elapsed_time(i1) / 10
+        del pbins
         indexed = {"api": "kf_fit_tracks_indexed (hits gathered by index from shuffled layer pools)", "ms": ix_ms,
                    "fits_per_s": n / (ix_ms * 1e-3), "sector_bytes_per_fit": 233 + L * (4 + 9 * 32),
+                   "records_ms": ixr_ms, "records_fits_per_s": n / (ixr_ms * 1e-3),
                    "note": "nine scattered 4-byte loads per hit: bound by 32-byte DRAM/L2 sectors, not by arithmetic"}
         del pools, perm, index
         smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10)", "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3),

@@ -174,6 +174,7 @@ typedef struct {
                                  x y z vzz | vxx vxy vyy index(int32 bits) | vxz vyz 0 0           */
     float* bin_box;           /* DEV [n_eta*n_phi][8] per-bin bounds for the scan's bin pruning:
                                  x_lo x_hi y_lo y_hi | z_lo z_hi max(vzz) max(vxx+vyy)              */
+    int32_t* orig_to_sorted;  /* DEV [n_hits] inverse of sorted_to_orig; optional (NULL = not written) */
     float* pos_sorted;        /* DEV [3][ld] hits in bin order, SoA; optional (NULL = not written)  */
     float* cov_sorted;        /* DEV [6][ld] optional (NULL = not written)                          */
 } kf_layer_bins;
@@ -181,10 +182,13 @@ typedef struct {
 /* Fit with the hits addressed by index (what a builder hands to the fitter): the hit of
  * track t on layer l is hit index[l*ld_index + t] of pools[l] (HOST array of n_layers descriptors, DEV
  * buffers inside), -1 = no hit on that layer.  Otherwise exactly kf_fit_tracks (same arithmetic, same
- * status semantics, `out` may alias `seeds`).  index: DEV int32 [n_layers][ld_index], ld_index >= n. */
+ * status semantics, `out` may alias `seeds`).  index: DEV int32 [n_layers][ld_index], ld_index >= n.
+ * `bins` = NULL, or a HOST array of n_layers kf_layer_bins made from the same pools by kf_bin_layers with
+ * hit_rec and orig_to_sorted filled: the hits are then read from the packed records (3 memory sectors per
+ * hit instead of 9), same values, same results. */
 KF_API int kf_fit_tracks_indexed(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                                  const int32_t* index, int64_t ld_index, const kf_layer_hits* pools,
-                                 kf_tracks* out);
+                                 const kf_layer_bins* bins, kf_tracks* out);
 
 /* Bin one layer's hits: bin = i_eta*n_phi + i_phi with eta = asinh(z/radius), phi = atan2(y,x) over
  * [-pi, pi); stable counting sort (within a bin, original order).  The bin of a hit is decided in

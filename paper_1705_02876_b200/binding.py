@@ -53,7 +53,7 @@ class _LayerHits(C.Structure):
 class _LayerBins(C.Structure):
     _fields_ = [("n_eta", C.c_int), ("n_phi", C.c_int), ("eta_max", C.c_float), ("ld", C.c_int64),
                 ("bin_offset", C.c_void_p), ("sorted_to_orig", C.c_void_p), ("hit_rec", C.c_void_p),
-                ("bin_box", C.c_void_p), ("pos_sorted", C.c_void_p), ("cov_sorted", C.c_void_p)]
+                ("bin_box", C.c_void_p), ("orig_to_sorted", C.c_void_p), ("pos_sorted", C.c_void_p), ("cov_sorted", C.c_void_p)]
 
 
 _lib = None
@@ -102,7 +102,7 @@ def load_library():
         f.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.POINTER(_Tracks)]
     lib.kf_fit_tracks_indexed.restype = C.c_int
     lib.kf_fit_tracks_indexed.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), vp, C.c_int64,
-                                          C.POINTER(_LayerHits), C.POINTER(_Tracks)]
+                                          C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.POINTER(_Tracks)]
     lib.kf_fit_tracks_smooth.restype = C.c_int
     lib.kf_fit_tracks_smooth.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.c_float,
                                          C.POINTER(_Tracks), C.POINTER(_Tracks)]
@@ -162,6 +162,7 @@ class Bins:
     sorted_to_orig: torch.Tensor  # int32 [n_hits]
     hit_rec: torch.Tensor         # f32 [n_hits][12] packed records in bin order
     bin_box: torch.Tensor         # f32 [n_bins][8] per-bin bounds
+    orig_to_sorted: torch.Tensor  # int32 [n_hits] inverse of sorted_to_orig
     pos_sorted: torch.Tensor | None = None   # f32 [3][ld] optional SoA copy
     cov_sorted: torch.Tensor | None = None   # f32 [6][ld]
 
@@ -173,6 +174,7 @@ class Bins:
                     torch.empty(max(n_hits, 1), dtype=torch.int32, device=device),
                     torch.empty((max(n_hits, 1), 12), dtype=torch.float32, device=device),
                     torch.empty((n_eta * n_phi, 8), dtype=torch.float32, device=device),
+                    torch.empty(max(n_hits, 1), dtype=torch.int32, device=device),
                     torch.empty((3, ld), dtype=torch.float32, device=device) if soa else None,
                     torch.empty((6, ld), dtype=torch.float32, device=device) if soa else None)
 
@@ -180,7 +182,7 @@ class Bins:
         ld = int(self.pos_sorted.shape[1]) if self.pos_sorted is not None else 0
         return _LayerBins(self.n_eta, self.n_phi, float(self.eta_max), ld,
                           self.bin_offset.data_ptr(), self.sorted_to_orig.data_ptr(), self.hit_rec.data_ptr(),
-                          self.bin_box.data_ptr(),
+                          self.bin_box.data_ptr(), self.orig_to_sorted.data_ptr(),
                           self.pos_sorted.data_ptr() if self.pos_sorted is not None else None,
                           self.cov_sorted.data_ptr() if self.cov_sorted is not None else None)
 
@@ -272,7 +274,7 @@ class KFContext:
         del keep
 
     def fit_tracks_indexed(self, geom: Geometry, n: int, par, cov, q, index, pools,
-                           out_par, out_cov, out_chi2, out_nhits, out_status):
+                           out_par, out_cov, out_chi2, out_nhits, out_status, bins=None):
         """Fit with hits addressed by index: index int32 [L][ld_index] (device), pools = [(n_hits, pos, cov), ...]
         one per geometry layer."""
         g, keep = geom._c()
@@ -282,8 +284,10 @@ class KFContext:
         if m != g.n_layers or index.shape[0] != m:
             raise ValueError("one pool and one index row per geometry layer")
         lhs = (_LayerHits * m)(*[self._layer_hits(nh, p, c) for (nh, p, c) in pools])
+        lbs = (_LayerBins * m)(*[b._c() for b in bins]) if bins is not None else None
         self._check(self._lib.kf_fit_tracks_indexed(self._h, C.byref(g), C.byref(seeds), index.data_ptr(),
-                                                    int(index.stride(0)), lhs, C.byref(out)), "kf_fit_tracks_indexed")
+                                                    int(index.stride(0)), lhs, lbs, C.byref(out)),
+                    "kf_fit_tracks_indexed")
         del keep
 
     def fit_tracks_smooth(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask, kappa: float,

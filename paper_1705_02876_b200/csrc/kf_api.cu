@@ -26,7 +26,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 6;
+constexpr int kAbiVersion = 7;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -200,7 +200,7 @@ int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
 }
 
 int kf_fit_tracks_indexed(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const int32_t* index,
-                          int64_t ld_index, const kf_layer_hits* pools, kf_tracks* out) {
+                          int64_t ld_index, const kf_layer_hits* pools, const kf_layer_bins* bins, kf_tracks* out) {
     if (!c || !geom || !seeds || !pools || !out) return KF_ERR_NULL;
     FitParams P;
     int rc = make_params(geom, &P);
@@ -216,7 +216,13 @@ int kf_fit_tracks_indexed(kf_ctx* c, const kf_geometry* geom, const kf_tracks* s
         if (pools[l].n_hits < 0 || pools[l].ld < pools[l].n_hits) return KF_ERR_SHAPE;
         if (pools[l].n_hits > 0 && (!pools[l].pos || !pools[l].cov)) return KF_ERR_NULL;
         H.pos[l] = pools[l].pos; H.cov[l] = pools[l].cov; H.ld[l] = pools[l].ld;
+        if (bins) {
+            if (pools[l].n_hits > 0 && (!bins[l].hit_rec || !bins[l].orig_to_sorted)) return KF_ERR_NULL;
+            if (!aligned16(bins[l].hit_rec)) return KF_ERR_ALIGN;
+            H.hit_rec[l] = bins[l].hit_rec; H.orig_to_sorted[l] = bins[l].orig_to_sorted;
+        }
     }
+    H.use_records = bins ? 1 : 0;
     H.index = index; H.ld_index = ld_index;
     FitArgs a;
     a.n = seeds->n;
@@ -313,6 +319,7 @@ BinArgs to_bin_args(float radius_cm, const kf_layer_hits* hits, const kf_layer_b
     a.radius = radius_cm; a.n_eta = out->n_eta; a.n_phi = out->n_phi; a.eta_max = out->eta_max;
     a.ld_out = out->ld; a.bin_offset = out->bin_offset; a.sorted_to_orig = out->sorted_to_orig;
     a.pos_sorted = out->pos_sorted; a.cov_sorted = out->cov_sorted; a.hit_rec = out->hit_rec; a.bin_box = out->bin_box;
+    a.orig_to_sorted = out->orig_to_sorted;
     return a;
 }
 

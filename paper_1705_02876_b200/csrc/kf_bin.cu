@@ -134,6 +134,7 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     for (int32_t j = s; j < e; ++j) rank += (__ldg(L.unsorted + j) < mine) ? 1 : 0;
     const int64_t dst = (int64_t)s + rank;
     L.sorted_to_orig[dst] = mine;
+    if (L.orig_to_sorted) L.orig_to_sorted[mine] = (int32_t)dst;
     if (!L.pos) return;  // ordering only (candidates)
     float v[9];
 #pragma unroll
@@ -303,7 +304,7 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
             BinLayerDev& L = B.layer[j];
             L.n = a.n_hits; L.ld_in = a.ld_in; L.ld_out = a.ld_out; L.pos = a.pos; L.cov = a.cov; L.radius = a.radius;
             L.bin_offset = a.bin_offset; L.sorted_to_orig = a.sorted_to_orig;
-            L.pos_sorted = a.pos_sorted; L.cov_sorted = a.cov_sorted; L.hit_rec = a.hit_rec; L.bin_box = a.bin_box;
+            L.pos_sorted = a.pos_sorted; L.cov_sorted = a.cov_sorted; L.hit_rec = a.hit_rec; L.bin_box = a.bin_box; L.orig_to_sorted = a.orig_to_sorted;
             L.key = s.key + item_off; L.unsorted = s.unsorted + item_off;
             L.counts = s.counts + (int64_t)(l0 + j) * (nb + 1); L.cursor = s.cursor + (int64_t)(l0 + j) * (nb + 1);
             item_off += a.n_hits;
@@ -335,7 +336,7 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
     BinLayerDev& L = B.layer[0];
     L.n = n; L.ld_in = 0; L.ld_out = 0; L.pos = nullptr; L.cov = nullptr; L.radius = 0.0f;
     L.bin_offset = s.counts + (nb + 1);  // second half of the counts buffer holds the offsets
-    L.sorted_to_orig = order; L.pos_sorted = nullptr; L.cov_sorted = nullptr; L.hit_rec = nullptr; L.bin_box = nullptr;
+    L.sorted_to_orig = order; L.pos_sorted = nullptr; L.cov_sorted = nullptr; L.hit_rec = nullptr; L.bin_box = nullptr; L.orig_to_sorted = nullptr;
     L.key = s.key; L.unsorted = s.unsorted; L.counts = s.counts; L.cursor = s.cursor;
     const dim3 grid((unsigned)((n + kBlock - 1) / kBlock), 1);
     cand_key_kernel<<<grid, kBlock, 0, stream>>>(P, layer, n, ld, par, q, n_eta, n_phi, eta_max, s.key, s.counts);

@@ -34,7 +34,10 @@ namespace {
 #define KF_FIT_STAGES 3
 #endif
 
-constexpr int kFitBlock = 128;
+#ifndef KF_FIT_BLOCK
+#define KF_FIT_BLOCK 128
+#endif
+constexpr int kFitBlock = KF_FIT_BLOCK;
 constexpr int kWarps = kFitBlock / 32;
 constexpr int kStages = KF_FIT_STAGES;           // layers in flight per warp
 constexpr int kHitFloats = 9 * 32;               // one hit tile
@@ -324,6 +327,13 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
 // Gathered loads cannot go through TMA: each thread fetches its 9 floats itself, one layer ahead.
 __device__ __forceinline__ Hit gather_hit(const IndexedPools& H, int l, int32_t h) {
     Hit m;
+    if (H.use_records) {   // one 4-byte look-up + one 48-byte record (3 sectors) instead of 9 scattered sectors
+        const int32_t s = __ldg(H.orig_to_sorted[l] + h);
+        const float4* r = reinterpret_cast<const float4*>(H.hit_rec[l]) + (int64_t)s * 3;
+        const float4 A = __ldg(r), B = __ldg(r + 1), C = __ldg(r + 2);
+        m.x = A.x; m.y = A.y; m.z = A.z; m.vzz = A.w; m.vxx = B.x; m.vxy = B.y; m.vyy = B.z; m.vxz = C.x; m.vyz = C.y;
+        return m;
+    }
     const float* p = H.pos[l];
     const float* c = H.cov[l];
     const int64_t ld = H.ld[l];

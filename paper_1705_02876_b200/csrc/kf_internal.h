@@ -32,6 +32,10 @@ struct IndexedPools {           // per-layer hit pools + the per-track hit indic
     int64_t ld[32];
     const int32_t* index;       // [n_layers][ld_index], -1 = no hit
     int64_t ld_index;
+    // optional fast path: the packed bin-ordered records of kf_bin_layers and the map into them
+    const float* hit_rec[32];
+    const int32_t* orig_to_sorted[32];
+    int use_records;
 };
 
 // kf_fit.cu
@@ -73,6 +77,7 @@ struct BinArgs {
     float* pos_sorted; float* cov_sorted;  // optional SoA copies (may be null)
     float* hit_rec;                        // [n_hits][12] packed records (may be null)
     float* bin_box;                        // [n_bins][8] per-bin bounds (may be null)
+    int32_t* orig_to_sorted;               // [n_hits] inverse of sorted_to_orig (may be null)
 };
 
 // One layer (or one candidate set) as the batched sort kernels see it.
@@ -81,7 +86,7 @@ struct BinLayerDev {
     const float* pos; const float* cov;    // null: order items only, gather nothing
     float radius;
     int32_t* bin_offset; int32_t* sorted_to_orig;
-    float* pos_sorted; float* cov_sorted; float* hit_rec; float* bin_box;
+    float* pos_sorted; float* cov_sorted; float* hit_rec; float* bin_box; int32_t* orig_to_sorted;
     int32_t* key;       // [n] bin of each item
     int32_t* unsorted;  // [n] item indices grouped by bin, arbitrary order inside
     int32_t* counts;    // [n_bins + 1]

@@ -21,7 +21,7 @@ def ctx():
     c.close()
 
 
-def _fit_indexed(ctx, ev, index_np):
+def _fit_indexed(ctx, ev, index_np, use_records=False):
     """Fit the event's seeds with hits index_np[L][n] (into ev.layers pools, -1 = none)."""
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceFit, DeviceLayer, padded_ld
@@ -30,8 +30,12 @@ def _fit_indexed(ctx, ev, index_np):
     pools = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers]
     idx = torch.full((len(ev.layers), padded_ld(f.n)), -1, dtype=torch.int32, device="cuda:0")
     idx[:, :f.n] = torch.from_numpy(np.ascontiguousarray(index_np, dtype=np.int32)).to("cuda:0")
+    bins = None
+    if use_records:
+        ctx.bin_layers([l.radius for l in ev.layers], [(p.n_hits, p.pos, p.cov, p.bins) for p in pools])
+        bins = [p.bins for p in pools]
     ctx.fit_tracks_indexed(d.geom, f.n, d.par, d.cov, d.q, idx, [(p.n_hits, p.pos, p.cov) for p in pools],
-                           d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status)
+                           d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status, bins=bins)
     torch.cuda.synchronize()
     return d.results()
 
@@ -57,6 +61,9 @@ def test_indexed_fit_with_true_hits_equals_the_pre_gathered_fit(ctx):
     g = _fit_indexed(ctx, ev, truth)
     o = _oracle_fit_with(ev, truth)
     compare_fit(g, o, float(ev.fit.radius[-1]), max_diverged_frac=2e-3)
+    g2 = _fit_indexed(ctx, ev, truth, use_records=True)          # same hits through the packed records
+    for k in g:
+        assert np.array_equal(g[k], g2[k]), k
     d = DeviceFit.from_batch(ev.fit, "cuda:0")      # the same hits pre-gathered per track
     d.fit(ctx)
     torch.cuda.synchronize()

@@ -41,6 +41,8 @@ def _assert_bins_equal(dl, ob, pos, cov):
     assert np.array_equal(rec[:, 0:3], pos[:, s2o].T) and np.array_equal(rec[:, 3], cs[:, 5])
     assert np.array_equal(rec[:, 4:7], cs[:, [0, 1, 3]]) and np.array_equal(rec[:, 8:10], cs[:, [2, 4]])
     assert np.array_equal(rec[:, 7].copy().view(np.int32), s2o)
+    o2s = dl.bins.orig_to_sorted.cpu().numpy()[:H]
+    assert np.array_equal(o2s[s2o], np.arange(H))
     box = dl.bins.bin_box.cpu().numpy()
     off = ob["bin_offset"]
     for b in np.flatnonzero(np.diff(off) > 0)[::7]:               # every 7th non-empty bin

@@ -31,7 +31,27 @@
 #define ORC_C_B 2.99792458e-3 /* GeV/(c T cm), reading A1 */
 #define ORC_PI 3.14159265358979323846
 
-enum { ORC_PROP_FAIL = 1, ORC_S_NOT_PD = 2, ORC_NONFINITE = 4, ORC_BAD_CHARGE = 8 };
+enum { ORC_PROP_FAIL = 1, ORC_S_NOT_PD = 2, ORC_NONFINITE = 4, ORC_BAD_CHARGE = 8, ORC_OUTSIDE = 16 };
+
+/* ---- geometry options (reading A20; "more realistic geometry"), process-wide, set by the
+ * caller before a fit / scoring call; defaults = readings A5 (flat thickness) and A12 (infinite cylinders):
+ *   material_model 1: the thickness seen by the track is t / cos(psi), psi = angle between the momentum
+ *                     and the cylinder normal at the crossing, cos(psi) = |x px + y py| / (rho |p|);
+ *   half_length[l]:   a crossing with |z'| > half_length[l] misses layer l: ORC_OUTSIDE, layer skipped,
+ *                     track untouched (same bookkeeping as ORC_PROP_FAIL).                              */
+static int g_material_model = 0;
+static double g_half_length[32] = {
+    INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY,
+    INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY,
+    INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY};
+
+static double g_score_half_length = INFINITY; /* the one layer orc_score_layer works on */
+void orc_set_score_half_length(double h) { g_score_half_length = h; }
+
+void orc_set_geometry_options(int material_model, int n_layers, const double *half_length) {
+    g_material_model = material_model;
+    for (int l = 0; l < 32; ++l) g_half_length[l] = (half_length && l < n_layers) ? half_length[l] : INFINITY;
+}
 
 /* ---- Highland multiple-scattering width (reading A5) --------------------------------------
  * theta0 = 0.0136 GeV / (beta p) * sqrt(t) * (1 + 0.038 ln t), t = x/X0 (flat), beta = p/E. */
@@ -126,6 +146,10 @@ int orc_propagate_inward(const double u[6], double q, double Bz, double r, doubl
 void orc_process_noise(const double u[6], double mass, double t, double Q[36]) {
     memset(Q, 0, 36 * sizeof(double));
     double p2 = u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+    if (g_material_model == 1 && t > 0.0) { /* A20: path length through the layer */
+        double cospsi = fabs(u[0] * u[3] + u[1] * u[4]) / (sqrt(u[0] * u[0] + u[1] * u[1]) * sqrt(p2));
+        t = t / cospsi;
+    }
     double th0 = orc_theta0(sqrt(p2), mass, t);
     for (int i = 0; i < 3; ++i)
         for (int j = 0; j < 3; ++j)
@@ -256,6 +280,7 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
             if (!((mask >> l) & 1u)) continue;
             double up[6], F[36], Q[36], Cp[36], un[6], Cn[36], dchi2;
             int rc = orc_propagate(u, (double)q, Bz, radius[l], up, F, NULL, NULL);
+            if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
             if (rc) { st |= (uint32_t)rc; continue; }
             orc_process_noise(up, mass, xX0[l], Q);
             orc_transport_cov(F, C, Q, Cp);
@@ -322,6 +347,7 @@ static void refit_inward_one(int L, const double *radius, const double *xX0, dou
             orc_process_noise(u, mass, xX0[prev], Q);
             for (int i = 0; i < 36; ++i) Cq[i] = C[i] + Q[i];
             rc = propagate_dir(u, (double)q, Bz, radius[l], 1, up, F, NULL, NULL);
+            if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
             if (rc) { st |= (uint32_t)rc; continue; }
             memset(Z, 0, sizeof Z);
             orc_transport_cov(F, Cq, Z, Cp);
@@ -543,6 +569,7 @@ void orc_score_layer(int64_t n, double r_layer, double xX0, double Bz, double ma
         if (q[i] != 1 && q[i] != -1) { status[i] |= ORC_BAD_CHARGE; continue; }
         double up[6], F[36], Q[36], Cp[36];
         int rc = orc_propagate(u, (double)q[i], Bz, r_layer, up, F, NULL, NULL);
+        if (!rc && fabs(up[2]) > g_score_half_length) rc = ORC_OUTSIDE;
         if (rc) { status[i] |= (uint32_t)rc; continue; }
         orc_process_noise(up, mass, xX0, Q);
         orc_transport_cov(F, C, Q, Cp);
@@ -666,6 +693,7 @@ void orc_build_combinatorial(int64_t n_seeds, int n_layers_total, int first_laye
             for (int p = 0; p < nc; ++p) {
                 double up[6], F[36], Q[36], Cp[36];
                 int rc = orc_propagate(cur[p].u, (double)qq, Bz, radius[l], up, F, NULL, NULL);
+                if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
 #define ORC_ROOM() do { if (nch + 2 > cap) { cap *= 2; ch = (orc_child *)realloc(ch, sizeof(orc_child) * cap); } } while (0)
                 ORC_ROOM();
                 if (rc) { /* cannot reach the layer: survives unchanged */

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "kf_oracle.c")
 _LIB = os.path.join(_HERE, "libkf_oracle.so")
 
-PROP_FAIL, S_NOT_PD, NONFINITE, BAD_CHARGE = 1, 2, 4, 8
+PROP_FAIL, S_NOT_PD, NONFINITE, BAD_CHARGE, OUTSIDE = 1, 2, 4, 8, 16
 TRACE_STRIDE = 122
 
 _lib = None
@@ -58,8 +58,37 @@ def lib():
         _lib.orc_bin_index_f32.argtypes = [C.c_float] * 4 + [C.c_int, C.c_int, C.c_double]
         _lib.orc_bin_hits.restype = None
         _lib.orc_score_layer.restype = None
+        _lib.orc_set_geometry_options.restype = None
+        _lib.orc_set_geometry_options.argtypes = [C.c_int, C.c_int, dp]
+        _lib.orc_set_score_half_length.restype = None
+        _lib.orc_set_score_half_length.argtypes = [C.c_double]
         _lib.orc_build_combinatorial.restype = None
     return _lib
+
+
+class geometry_options:
+    """Context manager for the oracle's process-wide geometry options (reading A20):
+    material_model 0 = flat thickness (A5), 1 = thickness / cos(incidence); half_length[l] = half length of
+    barrel layer l in cm (None = infinite, A12).  Restores the defaults on exit."""
+
+    def __init__(self, material_model: int = 0, half_length=None, score_layer: int | None = None):
+        self.model = int(material_model)
+        self.hl = None if half_length is None else np.ascontiguousarray(half_length, dtype=np.float64)
+        self.score_layer = score_layer
+
+    def __enter__(self):
+        n = 0 if self.hl is None else len(self.hl)
+        lib().orc_set_geometry_options(self.model, n, _p(self.hl))
+        if self.hl is not None and self.score_layer is not None:
+            lib().orc_set_score_half_length(float(self.hl[self.score_layer]))
+        return self
+
+    def set_score_layer(self, layer: int):
+        lib().orc_set_score_half_length(float(self.hl[layer]) if self.hl is not None else float("inf"))
+
+    def __exit__(self, *a):
+        lib().orc_set_geometry_options(0, 0, None)
+        lib().orc_set_score_half_length(float("inf"))
 
 
 def _p(a, ct=C.c_double):

@@ -53,6 +53,8 @@ class BarrelConfig:
     n_phi: int = 64
     eta_bin_max: float = 1.2
     first_scored_layer: int = 3
+    material_model: int = 0        # DESIGN.md reading A20: 1 = thickness / cos(incidence)
+    half_length_cm: float = float("inf")   # A20: finite barrel (same half length for every layer)
 
     @property
     def radii(self) -> np.ndarray:
@@ -95,12 +97,13 @@ class FitBatch:
         return int(self.radius.shape[0])
 
 
-def highland_theta0(p: np.ndarray, mass: float, t: float) -> np.ndarray:
-    """Width of the simulated scattering angle (PDG Highland form, flat thickness t = x/X0)."""
-    if t <= 0.0:
+def highland_theta0(p: np.ndarray, mass: float, t) -> np.ndarray:
+    """Width of the simulated scattering angle (PDG Highland form, thickness t = x/X0, scalar or per track)."""
+    t = np.asarray(t, dtype=np.float64)
+    if np.all(t <= 0.0):
         return np.zeros_like(p)
     beta = p / np.sqrt(p * p + mass * mass)
-    return 0.0136 / (beta * p) * math.sqrt(t) * (1.0 + 0.038 * math.log(t))
+    return 0.0136 / (beta * p) * np.sqrt(t) * (1.0 + 0.038 * np.log(t))
 
 
 def _cross_cylinder(pos, mom, q, Bz, r):
@@ -190,15 +193,20 @@ def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
         phi_h = np.arctan2(pos[1], pos[0]) + g[0] * SIGMA_RPHI / r
         hp = np.stack([r * np.cos(phi_h), r * np.sin(phi_h), pos[2] + g[1] * SIGMA_Z])
         hv = hit_covariance(phi_h)
-        hpos[l] = np.where(alive, hp, 0.0)
-        hcov[l] = np.where(alive, hv, 0.0)
-        mask |= (alive.astype(np.uint32) << np.uint32(l))
+        inside = alive & (np.abs(pos[2]) <= cfg.half_length_cm)      # A20: a crossing beyond the barrel end leaves no hit
+        hpos[l] = np.where(inside, hp, 0.0)
+        hcov[l] = np.where(inside, hv, 0.0)
+        mask |= (inside.astype(np.uint32) << np.uint32(l))
         # multiple scattering right after the hit: two independent angles about p-hat, |p| kept
         a = rng.standard_normal((2, n))
         if cfg.x_over_X0 > 0.0:
             px, py, pz = mom
             p = np.sqrt(px * px + py * py + pz * pz)
-            th0 = highland_theta0(p, M_PION, cfg.x_over_X0)
+            t_eff = cfg.x_over_X0
+            if cfg.material_model == 1:                              # path length through the layer
+                t_eff = cfg.x_over_X0 * (np.hypot(pos[0], pos[1]) * p) / np.abs(pos[0] * px + pos[1] * py)
+            th0 = highland_theta0(p, M_PION, t_eff)
+            th0 = np.where(inside, th0, 0.0)                         # no material beyond the barrel end
             ptt = np.hypot(px, py)
             e1 = (-py / ptt, px / ptt, np.zeros(n))                      # z-hat x p-hat, normalised
             ph = (px / p, py / p, pz / p)

@@ -71,7 +71,9 @@ enum {
     KF_STATUS_PROP_FAIL = 1,  /* helix has no outward crossing with the layer (disc <= 0, r <= rho) */
     KF_STATUS_S_NOT_PD = 2,   /* det S <= 0                                                         */
     KF_STATUS_NONFINITE = 4,  /* update produced a non-finite state or chi2                         */
-    KF_STATUS_BAD_CHARGE = 8  /* q not in {+1, -1}: track is copied through untouched               */
+    KF_STATUS_BAD_CHARGE = 8, /* q not in {+1, -1}: track is copied through untouched               */
+    KF_STATUS_OUTSIDE = 16    /* a crossing fell beyond the end of the barrel (|z'| > half_length_cm):
+                                 that layer was skipped (reading A20)                      */
 };
 
 #define KF_MAX_LAYERS 32
@@ -106,6 +108,14 @@ typedef struct {
     const float* x_over_X0;   /* HOST [n_layers], thickness in radiation lengths, 0 = no material  */
     float Bz_tesla;           /* |Bz| >= 1e-6                                                      */
     float mass_gev;           /* mass entering beta of the Highland formula (reading A5)           */
+    /* Geometry options ("more realistic" geometry is the stated direction; DESIGN.md
+     * reading A20).  Zero-initialised = the toy detector of the paper: infinite barrels, flat material. */
+    const float* half_length_cm; /* HOST [n_layers] barrel half lengths (> 0, +inf allowed), or NULL =
+                                    unbounded.  A propagated crossing with |z'| > half length misses the
+                                    layer: it is skipped and KF_STATUS_OUTSIDE is set.               */
+    int material_model;       /* 0: thickness x_over_X0 as given.  1: path length through the layer,
+                                 x_over_X0 / cos(psi), psi = angle between the propagated momentum and
+                                 the cylinder normal at the crossing (in Highland's sqrt AND log term) */
 } kf_geometry;
 
 /* ---- tracks (seeds in, fitted tracks out; candidates in/out) ------------------------------------ */

@@ -281,6 +281,7 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
             double up[6], F[36], Q[36], Cp[36], un[6], Cn[36], dchi2;
             int rc = orc_propagate(u, (double)q, Bz, radius[l], up, F, NULL, NULL);
             if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
+            if (tr && rc == ORC_OUTSIDE) memcpy(tr, up, 6 * sizeof(double)); /* diagnostic: where it missed */
             if (rc) { st |= (uint32_t)rc; continue; }
             orc_process_noise(up, mass, xX0[l], Q);
             orc_transport_cov(F, C, Q, Cp);

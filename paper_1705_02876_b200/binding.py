@@ -18,7 +18,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so")   # override: kernel experiments
 
-STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE = 1, 2, 4, 8
+STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE, STATUS_OUTSIDE = 1, 2, 4, 8, 16
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
            "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial"]
@@ -33,7 +33,8 @@ class KFError(RuntimeError):
 
 class _Geometry(C.Structure):
     _fields_ = [("n_layers", C.c_int), ("radius_cm", C.POINTER(C.c_float)), ("x_over_X0", C.POINTER(C.c_float)),
-                ("Bz_tesla", C.c_float), ("mass_gev", C.c_float)]
+                ("Bz_tesla", C.c_float), ("mass_gev", C.c_float),
+                ("half_length_cm", C.POINTER(C.c_float)), ("material_model", C.c_int)]
 
 
 class _Tracks(C.Structure):
@@ -143,13 +144,19 @@ class Geometry:
     x_over_X0: np.ndarray
     Bz_tesla: float
     mass_gev: float
+    half_length_cm: np.ndarray | None = None   # reading A20: barrel half lengths, None = unbounded
+    material_model: int = 0                    # reading A20: 1 = thickness / cos(incidence angle)
 
     def _c(self):
         r = np.ascontiguousarray(self.radius_cm, dtype=np.float32)
         t = np.ascontiguousarray(self.x_over_X0, dtype=np.float32)
+        h = None if self.half_length_cm is None else np.ascontiguousarray(self.half_length_cm, dtype=np.float32)
+        if h is not None and h.shape != r.shape:
+            raise ValueError("half_length_cm must have one entry per layer")
+        hp = C.POINTER(C.c_float)() if h is None else h.ctypes.data_as(C.POINTER(C.c_float))
         g = _Geometry(int(r.shape[0]), r.ctypes.data_as(C.POINTER(C.c_float)), t.ctypes.data_as(C.POINTER(C.c_float)),
-                      float(self.Bz_tesla), float(self.mass_gev))
-        return g, (r, t)          # keep the arrays alive while g is in use
+                      float(self.Bz_tesla), float(self.mass_gev), hp, int(self.material_model))
+        return g, (r, t, h)       # keep the arrays alive while g is in use
 
 
 @dataclass

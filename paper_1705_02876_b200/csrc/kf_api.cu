@@ -26,7 +26,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 7;
+constexpr int kAbiVersion = 8;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -62,7 +62,20 @@ int make_params(const kf_geometry* g, FitParams* P) {
         P->layer[l].r2 = (float)(r * r);
         P->layer[l].inv_r = (float)(1.0 / r);
         P->layer[l].ms = (float)ms;
+        // reading A20
+        P->layer[l].ms0 = t > 0.0 ? (float)(0.0136 * 0.0136 * t) : 0.0f;
+        P->layer[l].ln_t = t > 0.0 ? (float)std::log(t) : 0.0f;
+        float hl = INFINITY;
+        if (g->half_length_cm) {
+            hl = g->half_length_cm[l];
+            if (!(hl > 0.0f)) return KF_ERR_UNSUPPORTED;   // also rejects NaN; +inf = unbounded
+        }
+        P->layer[l].half_len = hl;
     }
+    if (g->material_model != 0 && g->material_model != 1) return KF_ERR_UNSUPPORTED;
+    P->material_model = g->material_model;
+    P->geometry_options = g->material_model != 0;
+    for (int l = 0; l < g->n_layers; ++l) P->geometry_options |= std::isfinite(P->layer[l].half_len) ? 1 : 0;
     return KF_OK;
 }
 

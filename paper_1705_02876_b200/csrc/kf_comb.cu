@@ -72,9 +72,11 @@ comb_propagate_kernel(const __grid_constant__ FitParams P, const CombArgs a, int
     Track t;
     get_track(a.trk_in, a.ld_s, slot, t);
     const float qf = (float)a.q[sd];
-    const bool ok = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.mass2,
-                                                BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch, a.ld_s, slot);
-    a.flag[slot] = ok ? FLAG_AT_LAYER : FLAG_IDLE;
+    const uint32_t rc = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.material_model,
+                                                    P.mass2, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch,
+                                                    a.ld_s, slot);
+    if (rc) a.st_in[slot] |= rc;   // its one child (REC_STUCK) inherits the reason
+    a.flag[slot] = rc ? FLAG_IDLE : FLAG_AT_LAYER;
 }
 
 // Per-warp accumulator of accepted hits (chi2 < cut) in shared memory.
@@ -327,8 +329,7 @@ comb_update_kernel(const CombArgs a) {
     int nh = a.nh_in[sp];
     uint32_t st = a.st_in[sp];
     if (r == REC_STUCK) {
-        get_track(a.trk_in, a.ld_s, sp, t);
-        st |= ST_PROP_FAIL;
+        get_track(a.trk_in, a.ld_s, sp, t);   // st already carries ST_PROP_FAIL / ST_OUTSIDE (comb_propagate_kernel)
     } else {
         Crossing o;
         PropCov n;

@@ -96,13 +96,14 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int col, in
 }
 
 // One layer for one track.  Returns 0 or the status bit of the failure (track untouched).
-template <bool RADIAL_NULL>
-__device__ __forceinline__ uint32_t fit_layer(Track& t, float k, float ik, const LayerConst& L,
+template <bool RADIAL_NULL, bool GEOM = true>
+__device__ __forceinline__ uint32_t fit_layer(Track& t, float k, float ik, const LayerConst& L, int model,
                                               float mass2, const Hit& m, float& chi2) {
     Crossing o;
-    if (!helix_to_radius(t, k, ik, L, o)) return ST_PROP_FAIL;
+    const uint32_t reached = reach_layer<false, GEOM>(t, k, ik, L, o);
+    if (reached) return reached;
     PropCov n;
-    transport_cov<RADIAL_NULL>(t, o, L.ms, mass2, n);
+    transport_cov<RADIAL_NULL>(t, o, ms_at_crossing(L, model, o, t.pz), mass2, n);
     LocalHit h;
     hit_to_local(o, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
     float d;
@@ -135,9 +136,12 @@ __device__ __forceinline__ void track_to_tile(const Track& t, float* p) {
 
 // SMOOTH = false: forward fit (rows a1-a7).  SMOOTH = true: forward fit, then the inward refit of reading
 // A18 over the same hits (streamed again through the same ring, outermost layer first); two results.
-template <bool SMOOTH>
+// GEOM = false: the paper's toy detector (unbounded barrels, flat material): the options of reading A20
+// are compiled out, so the headline kernel carries none of their cost.
+template <bool SMOOTH, bool GEOM>
 __global__ void __launch_bounds__(kFitBlock, SMOOTH ? 4 : KF_FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
+    const int model = GEOM ? P.material_model : 0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     const int wid = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform by construction
@@ -196,8 +200,8 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         __syncwarp();        // every lane has issued its reads of this stage
         if (good_q && ((mask >> l) & 1u)) {
             uint32_t rc;
-            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.mass2, m, chi2);
-            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.mass2, m, chi2);
+            if (started) rc = fit_layer<true, GEOM>(t, k, ik, P.layer[l], model, P.mass2, m, chi2);
+            else rc = fit_layer<false, GEOM>(t, k, ik, P.layer[l], model, P.mass2, m, chi2);
             st |= rc;
             if (rc == 0u) { nh += 1; started = true; used |= 1u << l; }
         }
@@ -234,7 +238,8 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         }
         if (valid) { a.chi2[i] = chi2; a.nhits[i] = nh; a.status[i] = st; }
         // ---- inward refit (reading A18)
-        float schi2 = 0.0f, ms_prev = 0.0f;
+        float schi2 = 0.0f;
+        int l_prev = 0;
         int nb = 0;
         uint32_t sst = 0u;
         bool first = true;
@@ -252,23 +257,23 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             if ((used >> l) & 1u) {
                 Crossing o;
                 PropCov n;
-                bool ok = true;
+                uint32_t reached = 0u;
                 const float k33 = t.c33, k35 = t.c35, k44 = t.c44, k55 = t.c55;
                 if (first) crossing_in_place(t, o, n);
                 else {
-                    ok = helix_to_radius<true>(t, k, ik, P.layer[l], o);
-                    if (ok) {
-                        add_process_noise(t, ms_prev, P.mass2);      // the scatterer just left behind
+                    reached = reach_layer<true, GEOM>(t, k, ik, P.layer[l], o);
+                    if (!reached) {
+                        add_process_noise(t, P.layer[l_prev], model, P.mass2);   // the scatterer just left behind
                         transport_cov<true>(t, o, 0.0f, P.mass2, n);
                     }
                 }
-                if (!ok) sst |= ST_PROP_FAIL;
+                if (reached) sst |= reached;
                 else {
                     LocalHit h;
                     hit_to_local(o, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
                     float d;
                     const uint32_t rc = kalman_update(t, o, n, h, &d);
-                    if (rc == 0u) { schi2 += d; nb += 1; first = false; ms_prev = P.layer[l].ms; }
+                    if (rc == 0u) { schi2 += d; nb += 1; first = false; l_prev = l; }
                     else { sst |= rc; t.c33 = k33; t.c35 = k35; t.c44 = k44; t.c55 = k55; }   // layer skipped
                 }
             }
@@ -372,8 +377,8 @@ fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ 
             }
             if (h < 0) continue;
             uint32_t rc;
-            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.mass2, m, chi2);
-            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.mass2, m, chi2);
+            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.material_model, P.mass2, m, chi2);
+            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.material_model, P.mass2, m, chi2);
             st |= rc;
             if (rc == 0u) { nh += 1; started = true; }
         }
@@ -423,10 +428,14 @@ bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t 
 
 cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream) {
     if (a.n == 0) return cudaSuccess;
-    static const cudaError_t attr = cudaFuncSetAttribute(fit_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    static const cudaError_t attr = [] {
+        cudaError_t e = cudaFuncSetAttribute(fit_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+        return e;
+    }();
     if (attr != cudaSuccess) return attr;
-    static const cudaError_t attr2 = cudaFuncSetAttribute(fit_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (attr2 != cudaSuccess) return attr2;
     const bool smooth = a.spar != nullptr;
     const int L = P.n_layers;
     FitMaps M;
@@ -438,8 +447,11 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     if (smooth && (!make_map(&M.spar, a.spar, a.n, a.ld_s, 6, 6) || !make_map(&M.scov, a.scov, a.n, a.ld_s, 21, 21)))
         return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
-    if (smooth) fit_kernel<true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else fit_kernel<false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    const bool geom = P.geometry_options != 0;   // reading A20 options in use
+    if (smooth && geom) fit_kernel<true, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (smooth) fit_kernel<true, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (geom) fit_kernel<false, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else fit_kernel<false, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     return cudaGetLastError();
 }
 

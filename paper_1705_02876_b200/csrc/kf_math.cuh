@@ -36,7 +36,7 @@ namespace kf {
 
 constexpr float kCB = 2.99792458e-3f;  // GeV / (c T cm), reading A1
 
-enum : uint32_t { ST_PROP_FAIL = 1u, ST_S_NOT_PD = 2u, ST_NONFINITE = 4u, ST_BAD_CHARGE = 8u };
+enum : uint32_t { ST_PROP_FAIL = 1u, ST_S_NOT_PD = 2u, ST_NONFINITE = 4u, ST_BAD_CHARGE = 8u, ST_OUTSIDE = 16u };
 
 // Per-layer constants, computed once on the host in double and rounded to float.
 struct LayerConst {
@@ -44,6 +44,10 @@ struct LayerConst {
     float r2;     // r^2
     float inv_r;  // 1 / r
     float ms;     // Highland: 0.0136^2 t (1 + 0.038 ln t)^2, t = x/X0 (0 if t <= 0)
+    // reading A20 (geometry options)
+    float half_len;  // barrel half length (+inf: unbounded)
+    float ms0;       // 0.0136^2 t          (0 if t <= 0)
+    float ln_t;      // ln t                (0 if t <= 0)
 };
 
 struct FitParams {
@@ -51,6 +55,8 @@ struct FitParams {
     float k0;      // c_B * Bz           (k = q k0)
     float inv_k0;  // 1 / (c_B * Bz)
     float mass2;   // mass^2
+    int material_model;  // reading A20: 0 flat thickness, 1 thickness / cos(incidence angle)
+    int geometry_options;  // 1 if material_model != 0 or any layer has a finite half length
     LayerConst layer[32];
 };
 
@@ -62,6 +68,17 @@ __device__ __forceinline__ float rsqrt_fast(float x) { float y; asm("rsqrt.appro
 __device__ __forceinline__ float rcp_fast(float x) { return 1.0f / x; }
 __device__ __forceinline__ float rsqrt_fast(float x) { return rsqrtf(x); }
 #endif
+
+// Reading A20, Highland factor of one crossing: `model` 0 is the flat L.ms; model 1 scales the thickness
+// by the path length through the layer, t_eff = t f with f = 1/cos(psi) = p / (pT cos a'), where cos a' =
+// e_r . e_l is the in-plane cosine between the radial direction and the transverse momentum:
+//     ms_eff = 0.0136^2 t f (1 + 0.038 (ln t + ln f))^2.
+__device__ __forceinline__ float layer_ms(const LayerConst& L, int model, float cos_a, float p2, float ipt) {
+    if (model == 0) return L.ms;
+    const float f = sqrtf(p2) * ipt * rcp_fast(fabsf(cos_a));
+    const float lg = 1.0f + 0.038f * (L.ln_t + __logf(f));
+    return L.ms0 * f * lg * lg;
+}
 
 // Track in registers.  Position frame unit vector (eax, eay): position-block coordinates
 // (a1, a2) mean  dw = (eax + i eay)(a1 + i a2).  The momentum frame always follows the current
@@ -221,6 +238,22 @@ __device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float i
     return true;
 }
 
+// helix_to_radius plus the acceptance of reading A20: 0, ST_PROP_FAIL, or ST_OUTSIDE when the crossing
+// lies beyond the end of the barrel (|z'| > half length; the layer is then skipped like a failed one).
+// BOUNDED = false compiles the acceptance test out (kernels specialised for the unbounded toy detector).
+template <bool INWARD = false, bool BOUNDED = true>
+__device__ __forceinline__ uint32_t reach_layer(const Track& t, float k, float ik, const LayerConst& L,
+                                                Crossing& o) {
+    if (!helix_to_radius<INWARD>(t, k, ik, L, o)) return ST_PROP_FAIL;
+    if constexpr (BOUNDED) return fabsf(o.zn) > L.half_len ? ST_OUTSIDE : 0u;
+    else return 0u;
+}
+
+// Highland factor at an arrival (forward filter) / at the state standing on a layer (backward refit).
+__device__ __forceinline__ float ms_at_crossing(const LayerConst& L, int model, const Crossing& o, float pz) {
+    return layer_ms(L, model, o.erx * o.elx + o.ery * o.ely, o.pt2 + pz * pz, o.ipt);
+}
+
 // Propagated covariance in the arrival frame (radial row is exactly zero and not stored).
 struct PropCov {
     float n11, n12, n13, n14, n15;
@@ -302,10 +335,11 @@ __device__ __forceinline__ void transport_cov(const Track& t, const Crossing& o,
 
 // Reading A18, backward refit: the scatterer just left behind adds its Highland noise to the momentum
 // block BEFORE the inward propagation (same Q~ as in transport_cov, at the current momentum).
-__device__ __forceinline__ void add_process_noise(Track& t, float ms, float mass2) {
+__device__ __forceinline__ void add_process_noise(Track& t, const LayerConst& L, int model, float mass2) {
     const float pt2 = t.px * t.px + t.py * t.py, pz = t.pz;
     const float ipt = rsqrt_fast(pt2);
     const float p2 = pt2 + pz * pz;
+    const float ms = layer_ms(L, model, (t.eax * t.px + t.eay * t.py) * ipt, p2, ipt);
     const float ip2 = rcp_fast(p2);
     const float th2 = ms * (p2 + mass2) * ip2 * ip2;
     const float qc = th2 * p2 * ipt;

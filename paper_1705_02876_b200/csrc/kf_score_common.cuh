@@ -59,14 +59,17 @@ __device__ __forceinline__ void hit_from_record(const float4* __restrict__ rec, 
     hit_to_local(o, A.x, A.y, A.z, B.x, B.y, C.x, B.z, C.y, A.w, h);
 }
 
-// Propagate a local-frame track to layer Lc and park the result in the scratch; flags[i] = 1 if it got there.
+// Propagate a local-frame track to layer Lc and park the result in the scratch.  Returns 0 if it got there,
+// else the status bit that says why not (ST_PROP_FAIL, ST_OUTSIDE).
 template <bool RADIAL_NULL>
-__device__ __forceinline__ bool propagate_to_scratch(const Track& t, float k, float ik, const LayerConst& Lc,
-                                                     float mass2, const BinGrid& g, float* sc, int64_t ld, int64_t i) {
+__device__ __forceinline__ uint32_t propagate_to_scratch(const Track& t, float k, float ik, const LayerConst& Lc,
+                                                         int model, float mass2, const BinGrid& g, float* sc,
+                                                         int64_t ld, int64_t i) {
     Crossing o;
-    if (!helix_to_radius(t, k, ik, Lc, o)) return false;
+    const uint32_t reached = reach_layer(t, k, ik, Lc, o);
+    if (reached) return reached;
     PropCov n;
-    transport_cov<RADIAL_NULL>(t, o, Lc.ms, mass2, n);
+    transport_cov<RADIAL_NULL>(t, o, ms_at_crossing(Lc, model, o, t.pz), mass2, n);
     put_scratch(sc, ld, i, o, n, t.pz);
     // the candidate's own bin (reading A16): eta = asinh(z'/r), phi = atan2(y', x') -- once per candidate
     // here, not once per lane in the scan
@@ -77,7 +80,7 @@ __device__ __forceinline__ bool propagate_to_scratch(const Track& t, float k, fl
     int ip = (int)floorf((phi + CUDART_PI_F) / (2.0f * CUDART_PI_F / (float)g.n_phi));
     ip = ((ip % g.n_phi) + g.n_phi) % g.n_phi;
     sc[(int64_t)SC_BIN * ld + i] = __int_as_float((ie << 16) | ip);
-    return true;
+    return 0u;
 }
 
 // ---- the current local-frame track between layers (kf_build_best_hit): 29 planes -------------------------

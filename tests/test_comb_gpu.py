@@ -26,29 +26,40 @@ def ctx():
     c.close()
 
 
-def _run(ctx, n_tracks, noise, n_cand):
+def _run(ctx, n_tracks, noise, n_cand, half_length=None, material_model=0):
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
     ev = W.make_build_event(4, n_tracks=n_tracks, noise_hits=noise)
     f = ev.fit
     r = O.fit_tracks(f.radius[:3], f.x_over_X0[:3], f.Bz, f.mass, f.par, f.cov, f.q, f.hpos[:3], f.hcov[:3], None, nthreads=8)
     par, cov = r["par"].astype(np.float32), O.pack_cov21(r["cov"]).astype(np.float32)
-    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, half_length, material_model)
     dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers[3:]]
     ctx.bin_layers([l.radius for l in ev.layers[3:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
     dc = DeviceCandidates.from_numpy(par, cov, f.q, r["chi2"], r["nhits"], "cuda:0")
     idx, nf = dc.build_combinatorial(ctx, geom, 3, dls, n_cand)
     torch.cuda.synchronize()
     layers = [(l.pos, l.cov, O.bin_hits(l.pos, l.radius, NE, NP, EMAX)) for l in ev.layers[3:]]
-    o = O.build_combinatorial(f.radius, f.x_over_X0, f.Bz, f.mass, par, cov, f.q, r["chi2"], r["nhits"], 3, layers,
-                              NE, NP, EMAX, 2, 30.0, n_cand)
+    with O.geometry_options(material_model, half_length):
+        o = O.build_combinatorial(f.radius, f.x_over_X0, f.Bz, f.mass, par, cov, f.q, r["chi2"], r["nhits"], 3, layers,
+                                  NE, NP, EMAX, 2, 30.0, n_cand)
     return ev, dc.results(), idx.cpu().numpy()[:, :f.n], nf.cpu().numpy()[:f.n], o
 
 
-@pytest.mark.parametrize("n_tracks,noise,n_cand", [(400, 2000, 4), (400, 2000, 1), (3000, 15000, 8), (20000, 100000, 4)])
-def test_combinatorial_parity(ctx, n_tracks, noise, n_cand):
-    ev, g, idx, nf, o = _run(ctx, n_tracks, noise, n_cand)
+GEOM = dict(half_length=np.full(10, 25.0, dtype=np.float32), material_model=1)     # reading A20
+
+
+@pytest.mark.parametrize("n_tracks,noise,n_cand,geom", [(400, 2000, 4, {}), (400, 2000, 1, {}), (3000, 15000, 8, {}),
+                                                        (20000, 100000, 4, {}), (3000, 15000, 4, GEOM)])
+def test_combinatorial_parity(ctx, n_tracks, noise, n_cand, geom):
+    ev, g, idx, nf, o = _run(ctx, n_tracks, noise, n_cand, **geom)
     f = ev.fit
+    OUT = np.uint32(O.OUTSIDE)
+    if geom:
+        assert ((o["status"] & OUT) != 0).mean() > 0.05      # the option is exercised
+        same_bits = (g["status"] & OUT) == (o["status"] & OUT)
+        g["status"] = g["status"] & ~OUT                     # compared here; a stopped candidate is a valid track
+        o["status"] = o["status"] & ~OUT
     same = (idx == o["hits"]).all(axis=0)
     clear = o["margin"] >= MARGIN
     frac_clear = clear.mean()
@@ -57,6 +68,8 @@ def test_combinatorial_parity(ctx, n_tracks, noise, n_cand):
     assert frac_clear > 0.5
     assert not np.any(~same & clear), np.flatnonzero(~same & clear)[:10]
     assert same.mean() > 0.97
+    if geom:
+        assert np.all(same_bits[same & clear])
     # identical hit lists: same bookkeeping, state within the (building) tolerances
     sel = same & (o["status"] == 0)
     assert np.array_equal(g["nhits"][sel], o["nhits"][sel]) and np.array_equal(g["status"][sel], o["status"][sel])

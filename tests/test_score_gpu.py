@@ -195,14 +195,14 @@ def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
     return n_dec, n_tie
 
 
-def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0):
+def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0, half_length=None, material_model=0):
     """kf_build_best_hit over layers 3..9 in one call vs the oracle's layer loop: decisions by north_star's
     rule, final state at the FIT tolerances (the candidates never leave the local frame)."""
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
     f, cfg = ev.fit, ev.cfg
     par, cov, chi2, nh = _seeds(ev)
-    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, half_length, material_model)
     dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
     L0 = cfg.first_scored_layer
     dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers[L0:]]
@@ -217,7 +217,8 @@ def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0):
     for j, l in enumerate(range(L0, cfg.n_layers)):
         lay = ev.layers[l]
         ob = O.bin_hits(lay.pos, lay.radius, NE, NP, EMAX)
-        orr = O.score_layer(oc, lay.radius, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NE, NP, EMAX, 2, 30.0, True)
+        with O.geometry_options(material_model, half_length, score_layer=l):
+            orr = O.score_layer(oc, lay.radius, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NE, NP, EMAX, 2, 30.0, True)
         diff = (idx[j] != orr["best_hit"]) & alive
         b, s2 = orr["best_chi2"], orr["second_chi2"]
         tie = (np.abs(s2 - b) <= 1e-4 * np.abs(b)) | (np.abs(b - 30.0) <= 1e-4 * 30.0)
@@ -227,10 +228,13 @@ def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0):
         acc = alive & (orr["best_hit"] >= 0)
         assert (np.abs(c2[j][acc] - b[acc]) / np.maximum(b[acc], 1.0)).max(initial=0) < 2e-3
     g = dc.results()
-    sel = alive & (oc.status == 0)
+    # a candidate beyond the barrel end (reading A20) stops there with its last state: a valid result to compare
+    sel = alive & ((oc.status & ~np.uint32(O.OUTSIDE)) == 0)
     assert np.array_equal(g["status"][alive], oc.status[alive]) and np.array_equal(g["nhits"][alive], oc.nhits[alive])
     sub_g = {k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in ("par", "cov", "chi2", "nhits", "status")}
     sub_o = dict(par=oc.par.T[:, sel], cov=oc.cov[sel], chi2=oc.chi2[sel], nhits=oc.nhits[sel], status=oc.status[sel])
+    sub_g["status"] = sub_g["status"] & ~np.uint32(O.OUTSIDE)      # (bits already checked equal above)
+    sub_o["status"] = sub_o["status"] & ~np.uint32(O.OUTSIDE)
     # north_star fixes only the hit decisions for scoring; the state is held to the fit tolerances, except
     # that with 100 000 noise hits per layer some candidates take wrong hits with chi2 up to 30 and kink by
     # many sigma, where both filters linearise far from the truth: covariance 3e-3 there (worst seen 1.4e-3)
@@ -250,6 +254,15 @@ def test_build_best_hit_full_config4(ctx):
     n_dec, n_tie = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0)
     print(f"config 4 fused: {n_dec} decisions, {n_tie} differences inside the tie window")
     assert n_dec >= 0.99 * 7 * 20000 and n_tie <= 20
+
+
+def test_build_best_hit_finite_barrel_and_path_length_material(ctx):
+    """Reading A20 through the builder: 25 cm barrels cut the high-|eta| candidates off on the outer layers."""
+    ev = W.make_build_event(4, n_tracks=3000, noise_hits=15000)
+    L = ev.fit.n_layers
+    hl = np.full(L, 25.0, dtype=np.float32)
+    n_dec, _ = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0, half_length=hl, material_model=1)
+    assert n_dec >= 0.98 * 7 * 3000
 
 
 def test_score_small_event(ctx):

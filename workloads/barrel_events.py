@@ -91,6 +91,8 @@ class FitBatch:
     mask: np.ndarray          # [n] u32, bit l = track has a hit on layer l
     truth: np.ndarray = field(repr=False, default=None)   # [L][6][n] f64 post-scatter truth at each layer
     truth_vertex: np.ndarray = field(repr=False, default=None)  # [6][n] f64
+    material_model: int = 0                # DESIGN.md reading A20 (geometry options of the fit)
+    half_length: np.ndarray = None         # [L] f32 barrel half lengths, None = unbounded
 
     @property
     def n_layers(self) -> int:
@@ -237,7 +239,9 @@ def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
         Bz=cfg.Bz, mass=M_PION,
         par=np.ascontiguousarray(spar, dtype=f32), cov=np.ascontiguousarray(scov, dtype=f32),
         q=q.astype(np.int8), hpos=np.ascontiguousarray(hpos, dtype=f32),
-        hcov=np.ascontiguousarray(hcov, dtype=f32), mask=mask, truth=truth, truth_vertex=truth_vertex)
+        hcov=np.ascontiguousarray(hcov, dtype=f32), mask=mask, truth=truth, truth_vertex=truth_vertex,
+        material_model=cfg.material_model,
+        half_length=None if math.isinf(cfg.half_length_cm) else np.full(L, cfg.half_length_cm, dtype=f32))
 
 
 def concat_batches(batches: list[FitBatch]) -> FitBatch:
@@ -246,7 +250,8 @@ def concat_batches(batches: list[FitBatch]) -> FitBatch:
     return FitBatch(n=sum(b.n for b in batches), radius=b0.radius, x_over_X0=b0.x_over_X0, Bz=b0.Bz,
                     mass=b0.mass, par=cat("par", 1), cov=cat("cov", 1), q=cat("q", 0),
                     hpos=cat("hpos", 2), hcov=cat("hcov", 2), mask=cat("mask", 0),
-                    truth=cat("truth", 2), truth_vertex=cat("truth_vertex", 1))
+                    truth=cat("truth", 2), truth_vertex=cat("truth_vertex", 1),
+                    material_model=b0.material_model, half_length=b0.half_length)
 
 
 def make_fit_batch(config: int, n_events: int | None = None, n_tracks: int | None = None) -> FitBatch:

@@ -312,6 +312,24 @@ def run_ours(args) -> None:
         torch.cuda.synchronize()
         sm_ms = s0.elapsed_time(s1) / 20
         sm_bytes = n * (113 + 2 * 36 * L + 2 * 120)
+        # secondary: the same fit with the geometry options of reading A20 (path-length material, 30 cm barrels)
+        import paper_1705_02876_b200 as K
+        plain_geom = d.geom
+        d.geom = K.Geometry(plain_geom.radius_cm, plain_geom.x_over_X0, plain_geom.Bz_tesla, plain_geom.mass_gev,
+                            np.full(L, 30.0, dtype=np.float32), 1)
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                d.fit(ctx)
+            s0.record(stream)
+            for _ in range(20):
+                d.fit(ctx)
+            s1.record(stream)
+        torch.cuda.synchronize()
+        go_ms = s0.elapsed_time(s1) / 20
+        go_out = float((d.out_status[:n] & 16).ne(0).float().mean().item())
+        d.geom = plain_geom
+        geometry = {"api": "kf_fit_tracks with material_model 1 and 30 cm barrel half lengths (reading A20)", "ms": go_ms,
+                    "fits_per_s": n / (go_ms * 1e-3), "tracks_cut_short": go_out}
         # secondary: kf_fit_tracks_indexed -- same tracks, each layer's hits shuffled into a pool and addressed by index
         g = torch.Generator(device=dev); g.manual_seed(5)
         perm = [torch.randperm(n, device=dev, generator=g) for _ in range(L)]
@@ -394,6 +412,7 @@ def run_ours(args) -> None:
         if smoothing is not None:
             out["smoothing"] = smoothing
             out["indexed_fit"] = indexed
+            out["geometry_options"] = geometry
         print(json.dumps(out), flush=True)
     ctx.close()
     sharding.shutdown()

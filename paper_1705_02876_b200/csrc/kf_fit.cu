@@ -37,6 +37,11 @@ namespace {
 #ifndef KF_FIT_BLOCK
 #define KF_FIT_BLOCK 128
 #endif
+// Batches of at least this many tracks take the pair kernel (two tracks per thread); smaller ones would
+// leave SMs idle with 256 tracks per CTA and keep the one-track kernel.
+#ifndef KF_PAIR_MIN_TRACKS
+#define KF_PAIR_MIN_TRACKS 151552
+#endif
 constexpr int kFitBlock = KF_FIT_BLOCK;
 constexpr int kWarps = kFitBlock / 32;
 constexpr int kStages = KF_FIT_STAGES;           // layers in flight per warp
@@ -327,6 +332,222 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
     if (storer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // smem must outlive the store
 }
 
+// ---- pair kernel: two tracks per thread in packed fp32x2 registers (kf_pair.cuh) ---------------------------
+// Same pipeline as fit_kernel<false, false> with tiles 64 tracks wide: lane j of a warp owns tracks
+// 2j (component x) and 2j + 1 (component y) of the tile, reads them as one 8-byte word per row and runs the
+// arithmetic of kf_math.cuh on F = f2, i.e. one FFMA2 / FMUL2 / FADD2 where the one-track kernel issues two
+// instructions.  Forward fit of the toy detector only (no smoother, no geometry options).
+#ifndef KF_PAIR_BLOCK
+#define KF_PAIR_BLOCK 128
+#endif
+#ifndef KF_PAIR_MIN_BLOCKS
+#define KF_PAIR_MIN_BLOCKS 3
+#endif
+constexpr int kPairBlock = KF_PAIR_BLOCK;
+constexpr int kPairWarps = kPairBlock / 32;
+constexpr int kPairTile = 64;                      // tracks per warp
+constexpr int kHit2Floats = 9 * kPairTile;
+constexpr int kSeed2Floats = 27 * kPairTile;
+constexpr int kWarp2Floats = kStages * kHit2Floats + kSeed2Floats;
+constexpr int kSmem2Bytes = kPairWarps * kWarp2Floats * 4 + kPairWarps * (kStages + 1) * 8;
+
+struct Hit2 {
+    f2 x, y, z, vxx, vxy, vxz, vyy, vyz, vzz;
+};
+
+// One layer for a pair of tracks that both have a hit on it.  Returns true if both went through; on any
+// failure the pair is untouched and the caller takes the two tracks one at a time (fit_layer_one_of_pair).
+// The hit pair is read from its shared-memory stage only where the residual is formed, after the covariance
+// transport, so that it does not occupy 18 registers through the most register-hungry part of the layer.
+__device__ __forceinline__ void load_hit_pair(Hit2& m, const float2* tp) {
+    constexpr int R = kPairTile / 2;
+    m.x = f2(tp[0]);           m.y = f2(tp[R]);           m.z = f2(tp[2 * R]);
+    m.vxx = f2(tp[3 * R]);     m.vxy = f2(tp[4 * R]);     m.vxz = f2(tp[5 * R]);
+    m.vyy = f2(tp[6 * R]);     m.vyz = f2(tp[7 * R]);     m.vzz = f2(tp[8 * R]);
+}
+
+template <bool RADIAL_NULL>
+__device__ __forceinline__ bool fit_layer_pair(Track2& t, f2 k, f2 ik, const LayerConst& L, float mass2,
+                                               const float2* tp, f2& chi2) {
+    Crossing2 o;
+    if (!all_of(helix_to_radius(t, k, ik, L, o))) return false;
+    PropCov2 n;
+    transport_cov<RADIAL_NULL>(t, o, f2(L.ms), mass2, n);
+    Hit2 m;
+    load_hit_pair(m, tp);
+    LocalHit2 h;
+    hit_to_local(o, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
+    f2 d;
+    const u2 rc = kalman_update(t, o, n, h, &d);
+    if ((rc.x | rc.y) != 0u) return false;
+    chi2 = chi2 + d;
+    return true;
+}
+
+// Slow path (a layer only one track of the pair has a hit on, or a failure in the pair): component c alone,
+// through the one-track arithmetic.  Kept out of line so that it costs the pair path no registers.
+#define KF_TRACK_FIELDS(X)                                                                              \
+    X(x) X(y) X(z) X(px) X(py) X(pz) X(eax) X(eay) X(c00) X(c01) X(c02) X(c03) X(c04) X(c05) X(c11) X(c12) \
+    X(c13) X(c14) X(c15) X(c22) X(c23) X(c24) X(c25) X(c33) X(c34) X(c35) X(c44) X(c45) X(c55)
+__device__ __noinline__ uint32_t fit_layer_one_of_pair(Track2& t, int c, float k, float ik, const LayerConst& L,
+                                                       float mass2, const Hit2& m, f2& chi2, bool started) {
+    Track ts;
+    Hit mh;
+    float ch = 0.0f;
+#define KF_GET(f) ts.f = c ? t.f.v.y : t.f.v.x;
+    KF_TRACK_FIELDS(KF_GET)
+#undef KF_GET
+#define KF_GETH(f) mh.f = c ? m.f.v.y : m.f.v.x;
+    KF_GETH(x) KF_GETH(y) KF_GETH(z) KF_GETH(vxx) KF_GETH(vxy) KF_GETH(vxz) KF_GETH(vyy) KF_GETH(vyz) KF_GETH(vzz)
+#undef KF_GETH
+    const uint32_t rc = started ? fit_layer<true, false>(ts, k, ik, L, 0, mass2, mh, ch)
+                                : fit_layer<false, false>(ts, k, ik, L, 0, mass2, mh, ch);
+    if (rc != 0u) return rc;
+#define KF_PUT(f) if (c) t.f.v.y = ts.f; else t.f.v.x = ts.f;
+    KF_TRACK_FIELDS(KF_PUT)
+#undef KF_PUT
+    if (c) chi2.v.y += ch; else chi2.v.x += ch;
+    return 0u;
+}
+#undef KF_TRACK_FIELDS
+
+#define KF_TRACK_ROWS(X)                                                                                   \
+    X(0, x) X(1, y) X(2, z) X(3, px) X(4, py) X(5, pz) X(6, c00) X(7, c01) X(8, c02) X(9, c03) X(10, c04)   \
+    X(11, c05) X(12, c11) X(13, c12) X(14, c13) X(15, c14) X(16, c15) X(17, c22) X(18, c23) X(19, c24)      \
+    X(20, c25) X(21, c33) X(22, c34) X(23, c35) X(24, c44) X(25, c45) X(26, c55)
+
+__global__ void __launch_bounds__(kPairBlock, KF_PAIR_MIN_BLOCKS)
+fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31;
+    const int wid = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+    const int64_t i0 = ((int64_t)blockIdx.x * kPairWarps + wid) * kPairTile;  // first track of this warp
+    if (i0 >= a.n) return;
+    const int L = P.n_layers;
+    float* wbase = reinterpret_cast<float*>(smem_raw) + wid * kWarp2Floats;
+    float* seed_tile = wbase + kStages * kHit2Floats;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + kPairWarps * kWarp2Floats * 4) + wid * (kStages + 1);
+    const uint32_t hit0 = smem_u32(wbase), seed0 = smem_u32(seed_tile), bar0 = smem_u32(bars);
+    const int col = (int)i0;
+    constexpr uint32_t kRowBytes = kPairTile * 4;
+
+    if (elect_one()) {
+#pragma unroll
+        for (int s = 0; s <= kStages; ++s) mbar_init(bar0 + 8u * s, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_expect_tx(bar0 + 8u * kStages, kSeed2Floats * 4);
+        tma_load_2d(seed0, &M.par, col, 0, bar0 + 8u * kStages);
+        tma_load_2d(seed0 + 6 * kRowBytes, &M.cov, col, 0, bar0 + 8u * kStages);
+#pragma unroll
+        for (int s = 0; s < kStages; ++s)
+            if (s < L) {
+                mbar_expect_tx(bar0 + 8u * s, kHit2Floats * 4);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4), &M.hpos, col, 3 * s, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4) + 3 * kRowBytes, &M.hcov, col, 6 * s, bar0 + 8u * s);
+            }
+    }
+    __syncwarp();
+
+    // component c of this lane = track i0 + 2 lane + c; a component beyond n shadows the last track and stores nothing
+    const int64_t left = a.n - i0;
+    const mask2 valid = {2 * lane < left, 2 * lane + 1 < left};
+    const int64_t ix = valid.x ? i0 + 2 * lane : a.n - 1, iy = valid.y ? i0 + 2 * lane + 1 : a.n - 1;
+    const int qx = a.q[ix], qy = a.q[iy];
+    const uint32_t mx = a.mask ? __ldg(a.mask + ix) : 0xffffffffu, my = a.mask ? __ldg(a.mask + iy) : 0xffffffffu;
+    const mask2 good_q = {(qx == 1) || (qx == -1), (qy == 1) || (qy == -1)};
+    const f2 k((float)qx * P.k0, (float)qy * P.k0), ik((float)qx * P.inv_k0, (float)qy * P.inv_k0);
+    Track2 t;
+    mbar_wait(bar0 + 8u * kStages, 0u);
+    {
+        const float2* p = reinterpret_cast<const float2*>(seed_tile) + lane;
+#define KF_LOAD_ROW(r, f) t.f = f2(p[(r) * (kPairTile / 2)]);
+        KF_TRACK_ROWS(KF_LOAD_ROW)
+#undef KF_LOAD_ROW
+        t.eax = f2(1.0f);
+        t.eay = f2(0.0f);
+    }
+    // a component with nothing to fit (bad charge, beyond n) takes no part
+    const mask2 live = {valid.x && good_q.x, valid.y && good_q.y};
+    if (!none_of(live)) enter_local_frame(t);
+    f2 chi2(0.0f);
+    int nhx = 0, nhy = 0;
+    u2 st = {0u, 0u};
+    mask2 started = {false, false};   // false: general 6x6 covariance; true: its radial row is identically zero
+    for (int l = 0; l < L; ++l) {
+        const int s = l % kStages;
+        mbar_wait(bar0 + 8u * s, (uint32_t)(l / kStages) & 1u);
+        const float2* tp = reinterpret_cast<const float2*>(wbase + s * kHit2Floats) + lane;
+        const mask2 want = {live.x && ((mx >> l) & 1u), live.y && ((my >> l) & 1u)};
+        bool both = false;
+        if (all_of(want)) {
+            // (the general transport is also right for a track whose radial row is already zero)
+            if (all_of(started)) both = fit_layer_pair<true>(t, k, ik, P.layer[l], P.mass2, tp, chi2);
+            else both = fit_layer_pair<false>(t, k, ik, P.layer[l], P.mass2, tp, chi2);
+        }
+        if (both) {
+            nhx += 1; nhy += 1;
+            started.x = true; started.y = true;
+        } else if (!none_of(want)) {
+            // copies whose address may be taken: the pair itself stays in registers
+            Track2 tc = t;
+            Hit2 mc;
+            load_hit_pair(mc, tp);
+            f2 cc = chi2;
+            if (want.x) {
+                const uint32_t rc = fit_layer_one_of_pair(tc, 0, k.v.x, ik.v.x, P.layer[l], P.mass2, mc, cc, started.x);
+                st.x |= rc;
+                if (rc == 0u) { nhx += 1; started.x = true; }
+            }
+            if (want.y) {
+                const uint32_t rc = fit_layer_one_of_pair(tc, 1, k.v.y, ik.v.y, P.layer[l], P.mass2, mc, cc, started.y);
+                st.y |= rc;
+                if (rc == 0u) { nhy += 1; started.y = true; }
+            }
+            t = tc;
+            chi2 = cc;
+        }
+        const int nxt = l + kStages;
+        if (nxt < L) {
+            __syncwarp();
+            if (elect_one()) {
+                mbar_expect_tx(bar0 + 8u * s, kHit2Floats * 4);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4), &M.hpos, col, 3 * nxt, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4) + 3 * kRowBytes, &M.hcov, col, 6 * nxt, bar0 + 8u * s);
+            }
+        }
+    }
+    if (!good_q.x) st.x = ST_BAD_CHARGE;
+    if (!good_q.y) st.y = ST_BAD_CHARGE;
+    // a track with nothing fitted goes back as it came: its columns of the seed tile still hold the input
+    const mask2 done = {live.x && nhx > 0, live.y && nhy > 0};
+    if (!none_of(done)) {
+        leave_local_frame(t);
+        if (all_of(done)) {
+            float2* p = reinterpret_cast<float2*>(seed_tile) + lane;
+#define KF_STORE_ROW(r, f) p[(r) * (kPairTile / 2)] = t.f.v;
+            KF_TRACK_ROWS(KF_STORE_ROW)
+#undef KF_STORE_ROW
+        } else {
+            float* p = seed_tile + 2 * lane + (done.y ? 1 : 0);
+#define KF_STORE_ONE(r, f) p[(r) * kPairTile] = done.y ? t.f.v.y : t.f.v.x;
+            KF_TRACK_ROWS(KF_STORE_ONE)
+#undef KF_STORE_ONE
+        }
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncwarp();
+    const bool storer = elect_one();
+    if (storer) {
+        tma_store_2d(&M.opar, col, 0, seed0);
+        tma_store_2d(&M.ocov, col, 0, seed0 + 6 * kRowBytes);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    if (valid.x) { a.chi2[ix] = chi2.v.x; a.nhits[ix] = nhx; a.status[ix] = st.x; }
+    if (valid.y) { a.chi2[iy] = chi2.v.y; a.nhits[iy] = nhy; a.status[iy] = st.y; }
+    if (storer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+#undef KF_TRACK_ROWS
+
 // ---- fit with hits addressed by index into the layer pools (the hits a track uses are
 // looked up, not pre-gathered).  index[l][i] = hit of track i in pool l or -1.
 // Gathered loads cannot go through TMA: each thread fetches its 9 floats itself, one layer ahead.
@@ -411,13 +632,13 @@ EncodeTiledFn encode_fn() {
     return fn;
 }
 
-// Tensor map over a [rows][ld] float array of which n columns are valid; tiles are [box_rows][32].
-bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t rows, int box_rows) {
+// Tensor map over a [rows][ld] float array of which n columns are valid; tiles are [box_rows][box_cols].
+bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t rows, int box_rows, int box_cols = 32) {
     EncodeTiledFn enc = encode_fn();
     if (!enc) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
-    const cuuint32_t box[2] = {32u, (cuuint32_t)box_rows};
+    const cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
     return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -439,6 +660,21 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     const bool smooth = a.spar != nullptr;
     const int L = P.n_layers;
     FitMaps M;
+    if (!smooth && P.geometry_options == 0 && a.n >= (int64_t)KF_PAIR_MIN_TRACKS) {   // headline path: two tracks per thread
+        static const cudaError_t attr_pair =
+            cudaFuncSetAttribute(fit_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem2Bytes);
+        if (attr_pair != cudaSuccess) return attr_pair;
+        constexpr int W = kPairTile;
+        if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3, W) ||
+            !make_map(&M.hcov, a.hcov, a.n, a.ld_hit, (int64_t)L * 6, 6, W) ||
+            !make_map(&M.par, a.par, a.n, a.ld_in, 6, 6, W) || !make_map(&M.cov, a.cov, a.n, a.ld_in, 21, 21, W) ||
+            !make_map(&M.opar, a.opar, a.n, a.ld_out, 6, 6, W) || !make_map(&M.ocov, a.ocov, a.n, a.ld_out, 21, 21, W))
+            return cudaErrorInvalidValue;
+        const int64_t per_block = (int64_t)kPairWarps * kPairTile;
+        const int64_t blocks = (a.n + per_block - 1) / per_block;
+        fit_pair_kernel<<<(unsigned)blocks, kPairBlock, kSmem2Bytes, stream>>>(P, M, a);
+        return cudaGetLastError();
+    }
     if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3) ||
         !make_map(&M.hcov, a.hcov, a.n, a.ld_hit, (int64_t)L * 6, 6) ||
         !make_map(&M.par, a.par, a.n, a.ld_in, 6, 6) || !make_map(&M.cov, a.cov, a.n, a.ld_in, 21, 21) ||

@@ -32,6 +32,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "kf_pair.cuh"
+
 namespace kf {
 
 constexpr float kCB = 2.99792458e-3f;  // GeV / (c T cm), reading A1
@@ -69,14 +71,18 @@ __device__ __forceinline__ float rcp_fast(float x) { return 1.0f / x; }
 __device__ __forceinline__ float rsqrt_fast(float x) { return rsqrtf(x); }
 #endif
 
+__device__ __forceinline__ f2 rcp_fast(f2 x) { return f2(rcp_fast(x.v.x), rcp_fast(x.v.y)); }
+__device__ __forceinline__ f2 rsqrt_fast(f2 x) { return f2(rsqrt_fast(x.v.x), rsqrt_fast(x.v.y)); }
+
 // Reading A20, Highland factor of one crossing: `model` 0 is the flat L.ms; model 1 scales the thickness
 // by the path length through the layer, t_eff = t f with f = 1/cos(psi) = p / (pT cos a'), where cos a' =
 // e_r . e_l is the in-plane cosine between the radial direction and the transverse momentum:
 //     ms_eff = 0.0136^2 t f (1 + 0.038 (ln t + ln f))^2.
-__device__ __forceinline__ float layer_ms(const LayerConst& L, int model, float cos_a, float p2, float ipt) {
-    if (model == 0) return L.ms;
-    const float f = sqrtf(p2) * ipt * rcp_fast(fabsf(cos_a));
-    const float lg = 1.0f + 0.038f * (L.ln_t + __logf(f));
+template <class F>
+__device__ __forceinline__ F layer_ms(const LayerConst& L, int model, F cos_a, F p2, F ipt) {
+    if (model == 0) return F(L.ms);
+    const F f = sqrt_(p2) * ipt * rcp_fast(abs_(cos_a));
+    const F lg = 1.0f + 0.038f * (L.ln_t + log_fast(f));
     return L.ms0 * f * lg * lg;
 }
 
@@ -84,53 +90,57 @@ __device__ __forceinline__ float layer_ms(const LayerConst& L, int model, float 
 // (a1, a2) mean  dw = (eax + i eay)(a1 + i a2).  The momentum frame always follows the current
 // momentum: d(pi) = (px + i py)/pT (b1 + i b2), d pz = c + (pz/pT) b1.
 // cXY = packed upper triangle over (a1, a2, z, b1, b2, c).
-struct Track {
-    float x, y, z, px, py, pz;
-    float eax, eay;
-    float c00, c01, c02, c03, c04, c05;
-    float c11, c12, c13, c14, c15;
-    float c22, c23, c24, c25;
-    float c33, c34, c35;
-    float c44, c45;
-    float c55;
+template <class F>
+struct TrackT {
+    F x, y, z, px, py, pz;
+    F eax, eay;
+    F c00, c01, c02, c03, c04, c05;
+    F c11, c12, c13, c14, c15;
+    F c22, c23, c24, c25;
+    F c33, c34, c35;
+    F c44, c45;
+    F c55;
 };
+using Track = TrackT<float>;    // one track per thread
+using Track2 = TrackT<f2>;      // two tracks per thread, packed (kf_pair.cuh)
 
 // Change the momentum frame of the covariance: rotate (b1, b2) -> (dc + i ds)(b1 + i b2), then
 // shear c -> c + k1 b1 + k2 b2 (new b's), k1 = T_old dc - T_new, k2 = T_old ds, T = pz/pT.
-template <bool RADIAL_NULL = false>
-__device__ __forceinline__ void reaim_momentum(Track& t, float dc, float ds, float T_old,
-                                               float T_new) {
-    float a, b;
+template <bool RADIAL_NULL = false, class F>
+__device__ __forceinline__ void reaim_momentum(TrackT<F>& t, arg<F> dc, arg<F> ds, arg<F> T_old,
+                                               arg<F> T_new) {
+    F a, b;
     if constexpr (!RADIAL_NULL) { a = t.c03; b = t.c04; t.c03 = dc * a - ds * b; t.c04 = ds * a + dc * b; }
     a = t.c13; b = t.c14; t.c13 = dc * a - ds * b; t.c14 = ds * a + dc * b;
     a = t.c23; b = t.c24; t.c23 = dc * a - ds * b; t.c24 = ds * a + dc * b;
     a = t.c35; b = t.c45;
-    const float c35 = dc * a - ds * b, c45 = ds * a + dc * b;
-    const float cc = dc * dc, ss = ds * ds, cs = dc * ds;
-    const float ll = t.c33, ln = t.c34, nn = t.c44;
+    const F c35 = dc * a - ds * b, c45 = ds * a + dc * b;
+    const F cc = dc * dc, ss = ds * ds, cs = dc * ds;
+    const F ll = t.c33, ln = t.c34, nn = t.c44;
     t.c33 = cc * ll - 2.0f * cs * ln + ss * nn;
     t.c44 = ss * ll + 2.0f * cs * ln + cc * nn;
     t.c34 = cs * (ll - nn) + (cc - ss) * ln;
-    const float k1 = T_old * dc - T_new, k2 = T_old * ds;
-    if constexpr (!RADIAL_NULL) t.c05 = fmaf(k2, t.c04, fmaf(k1, t.c03, t.c05));
-    t.c15 = fmaf(k2, t.c14, fmaf(k1, t.c13, t.c15));
-    t.c25 = fmaf(k2, t.c24, fmaf(k1, t.c23, t.c25));
-    const float n35 = c35 + k1 * t.c33 + k2 * t.c34;
-    const float n45 = c45 + k1 * t.c34 + k2 * t.c44;
+    const F k1 = T_old * dc - T_new, k2 = T_old * ds;
+    if constexpr (!RADIAL_NULL) t.c05 = fma_(k2, t.c04, fma_(k1, t.c03, t.c05));
+    t.c15 = fma_(k2, t.c14, fma_(k1, t.c13, t.c15));
+    t.c25 = fma_(k2, t.c24, fma_(k1, t.c23, t.c25));
+    const F n35 = c35 + k1 * t.c33 + k2 * t.c34;
+    const F n45 = c45 + k1 * t.c34 + k2 * t.c44;
     t.c55 += k1 * (c35 + n35) + k2 * (c45 + n45);
     t.c35 = n35;
     t.c45 = n45;
 }
 
 // Rotate the position-block coordinates (a1, a2) -> (dc + i ds)(a1 + i a2).
-__device__ __forceinline__ void reframe_position(Track& t, float dc, float ds) {
-    float a, b;
+template <class F>
+__device__ __forceinline__ void reframe_position(TrackT<F>& t, arg<F> dc, arg<F> ds) {
+    F a, b;
     a = t.c02; b = t.c12; t.c02 = dc * a - ds * b; t.c12 = ds * a + dc * b;
     a = t.c03; b = t.c13; t.c03 = dc * a - ds * b; t.c13 = ds * a + dc * b;
     a = t.c04; b = t.c14; t.c04 = dc * a - ds * b; t.c14 = ds * a + dc * b;
     a = t.c05; b = t.c15; t.c05 = dc * a - ds * b; t.c15 = ds * a + dc * b;
-    const float cc = dc * dc, ss = ds * ds, cs = dc * ds;
-    const float ll = t.c00, ln = t.c01, nn = t.c11;
+    const F cc = dc * dc, ss = ds * ds, cs = dc * ds;
+    const F ll = t.c00, ln = t.c01, nn = t.c11;
     t.c00 = cc * ll - 2.0f * cs * ln + ss * nn;
     t.c11 = ss * ll + 2.0f * cs * ln + cc * nn;
     t.c01 = cs * (ll - nn) + (cc - ss) * ln;
@@ -138,23 +148,24 @@ __device__ __forceinline__ void reframe_position(Track& t, float dc, float ds) {
 
 // Global-frame covariance (as stored) -> local frame.  Position frame stays global (ea = 1);
 // the momentum block goes to (b1, b2, c).
-__device__ __forceinline__ void enter_local_frame(Track& t) {
+template <class F>
+__device__ __forceinline__ void enter_local_frame(TrackT<F>& t) {
     t.eax = 1.0f;
     t.eay = 0.0f;
-    const float pt2 = t.px * t.px + t.py * t.py;
-    if (pt2 > 0.0f) {
-        const float ipt = rsqrtf(pt2);
-        // b = conj(e_l) * d(pi): rotation by -phi_p;  c = d pz - (pz/pT) b1
-        reaim_momentum(t, t.px * ipt, -t.py * ipt, 0.0f, t.pz * ipt);
-    }
+    const F pt2 = t.px * t.px + t.py * t.py;
+    if (none_of(pt2 > 0.0f)) return;     // (a pair goes on if either track has pT > 0; the other never starts)
+    const F ipt = rsqrt_ieee(pt2);
+    // b = conj(e_l) * d(pi): rotation by -phi_p;  c = d pz - (pz/pT) b1
+    reaim_momentum(t, t.px * ipt, -t.py * ipt, 0.0f, t.pz * ipt);
 }
 
 // Local frame -> global frame (inverse of the above for the current frames).
-__device__ __forceinline__ void leave_local_frame(Track& t) {
+template <class F>
+__device__ __forceinline__ void leave_local_frame(TrackT<F>& t) {
     reframe_position(t, t.eax, t.eay);
-    const float pt2 = t.px * t.px + t.py * t.py;
-    if (pt2 > 0.0f) {
-        const float ipt = rsqrtf(pt2);
+    const F pt2 = t.px * t.px + t.py * t.py;
+    if (!none_of(pt2 > 0.0f)) {
+        const F ipt = rsqrt_ieee(pt2);
         reaim_momentum(t, t.px * ipt, t.py * ipt, t.pz * ipt, 0.0f);
     }
     t.eax = 1.0f;
@@ -162,49 +173,54 @@ __device__ __forceinline__ void leave_local_frame(Track& t) {
 }
 
 // Result of the helix crossing + local-frame Jacobian ingredients.
-struct Crossing {
-    float xn, yn, zn, pxn, pyn;  // arrival state (pz unchanged)
-    float erx, ery;              // e_r' = w'/r
-    float elx, ely;              // e_l' = pi'/pT
-    float g0, g1, g3, g4;        // G_r over (a1, a2, b1, b2)
-    float t0, t1, t3, t4;        // row t' = G_t - tan(a') G_r
-    float z0, z1, z3, z4;        // row z' over (a1, a2, b1, b2); its z entry is 1, its c entry thk
-    float thk;                   // theta / k = s / pT
-    float mu;                    // k / cos(a')
-    float T;                     // pz / pT (conserved along the helix)
-    float pt2, ipt;
+template <class F>
+struct CrossingT {
+    F xn, yn, zn, pxn, pyn;  // arrival state (pz unchanged)
+    F erx, ery;              // e_r' = w'/r
+    F elx, ely;              // e_l' = pi'/pT
+    F g0, g1, g3, g4;        // G_r over (a1, a2, b1, b2)
+    F t0, t1, t3, t4;        // row t' = G_t - tan(a') G_r
+    F z0, z1, z3, z4;        // row z' over (a1, a2, b1, b2); its z entry is 1, its c entry thk
+    F thk;                   // theta / k = s / pT
+    F mu;                    // k / cos(a')
+    F T;                     // pz / pT (conserved along the helix)
+    F pt2, ipt;
 };
+using Crossing = CrossingT<float>;
+using Crossing2 = CrossingT<f2>;
 
 // Reading A3: first outward crossing of the helix with the cylinder of radius L.r, half-angle
 // form  t = tan(theta/2) = D / (a + sqrt(a^2 - D (2b + D))).  Returns false on PROP_FAIL.
 // INWARD (reading A18): the same helix followed backward in path length to a smaller radius
 // (D < 0, t < 0, theta < 0); the local-frame Jacobian below holds for either sign of theta.
-template <bool INWARD = false>
-__device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float ik,
-                                                const LayerConst& L, Crossing& o) {
-    const float x = t.x, y = t.y, px = t.px, py = t.py;
-    const float pt2 = px * px + py * py;
-    const float rho2 = x * x + y * y;
-    const float a = x * px + y * py;
-    const float b = (y * px - x * py) - pt2 * ik;
-    const float D = 0.5f * k * (L.r2 - rho2);
-    const float disc = a * a - D * (2.0f * b + D);
-    const float den = a + disc * rsqrt_fast(disc);  // NaN unless disc > 0
+template <bool INWARD = false, class F>
+__device__ __forceinline__ typename num_traits<F>::mask helix_to_radius(const TrackT<F>& t, arg<F> k, arg<F> ik,
+                                                                        const LayerConst& L, CrossingT<F>& o) {
+    const F x = t.x, y = t.y, px = t.px, py = t.py;
+    const F pt2 = px * px + py * py;
+    const F rho2 = x * x + y * y;
+    const F a = x * px + y * py;
+    const F b = (y * px - x * py) - pt2 * ik;
+    const F D = 0.5f * k * (L.r2 - rho2);
+    const F disc = a * a - D * (2.0f * b + D);
+    const F den = a + disc * rsqrt_fast(disc);  // NaN unless disc > 0
     // one test for the three PROP_FAIL conditions (r <= rho, disc <= 0, den <= 0; NaNs fail too)
-    if (!((INWARD ? L.r2 < rho2 : L.r2 > rho2) & (disc > 0.0f) & (den > 0.0f))) return false;
-    const float tt = D * rcp_fast(den);
-    const float i1 = rcp_fast(1.0f + tt * tt);
-    const float S = 2.0f * tt * i1;
-    const float Cm = tt * S;
-    const float co = 1.0f - Cm;
-    const float theta = 2.0f * atanf(tt);
+    // (a pair stops here if either track fails; the caller then takes the two one at a time)
+    const typename num_traits<F>::mask ok = (INWARD ? L.r2 < rho2 : L.r2 > rho2) & (disc > 0.0f) & (den > 0.0f);
+    if (!all_of(ok)) return ok;
+    const F tt = D * rcp_fast(den);
+    const F i1 = rcp_fast(1.0f + tt * tt);
+    const F S = 2.0f * tt * i1;
+    const F Cm = tt * S;
+    const F co = 1.0f - Cm;
+    const F theta = 2.0f * atan_(tt);
     o.thk = theta * ik;
     o.xn = x + (px * S + py * Cm) * ik;
     o.yn = y + (py * S - px * Cm) * ik;
     o.zn = t.z + t.pz * o.thk;
     o.pxn = px * co + py * S;
     o.pyn = py * co - px * S;
-    const float ipt = rsqrt_fast(pt2);
+    const F ipt = rsqrt_fast(pt2);
     o.pt2 = pt2;
     o.ipt = ipt;
     o.erx = o.xn * L.inv_r;
@@ -212,30 +228,30 @@ __device__ __forceinline__ bool helix_to_radius(const Track& t, float k, float i
     o.elx = o.pxn * ipt;
     o.ely = o.pyn * ipt;
     // exp(i a') = conj(e_r') e_l'
-    const float ca = o.erx * o.elx + o.ery * o.ely;
-    const float sa = o.erx * o.ely - o.ery * o.elx;
-    const float ic = rcp_fast(ca);
-    const float T = sa * ic;
+    const F ca = o.erx * o.elx + o.ery * o.ely;
+    const F sa = o.erx * o.ely - o.ery * o.elx;
+    const F ic = rcp_fast(ca);
+    const F T = sa * ic;
     // P = conj(e_r') e_a
-    const float pc = o.erx * t.eax + o.ery * t.eay;
-    const float ps = o.erx * t.eay - o.ery * t.eax;
+    const F pc = o.erx * t.eax + o.ery * t.eay;
+    const F ps = o.erx * t.eay - o.ery * t.eax;
     // N = ((S + i Cm)/k) exp(i a')
-    const float nr = (S * ca - Cm * sa) * ik;
-    const float nt = (S * sa + Cm * ca) * ik;
+    const F nr = (S * ca - Cm * sa) * ik;
+    const F nt = (S * sa + Cm * ca) * ik;
     o.g0 = pc;  o.g1 = -ps; o.g3 = nr; o.g4 = -nt;
     o.t0 = ps - T * pc;
     o.t1 = pc + T * ps;
     o.t3 = nt - T * nr;
     o.t4 = nr + T * nt;
-    const float T_ = t.pz * ipt;
-    const float lam = T_ * ic;
+    const F T_ = t.pz * ipt;
+    const F lam = T_ * ic;
     o.T = T_;
     o.z0 = -lam * pc;
     o.z1 = lam * ps;
     o.z3 = T_ * (o.thk - ic * nr);  // small: the |p|-at-fixed-direction mode does not move z'
     o.z4 = lam * nt;
     o.mu = k * ic;
-    return true;
+    return ok;
 }
 
 // helix_to_radius plus the acceptance of reading A20: 0, ST_PROP_FAIL, or ST_OUTSIDE when the crossing
@@ -250,55 +266,60 @@ __device__ __forceinline__ uint32_t reach_layer(const Track& t, float k, float i
 }
 
 // Highland factor at an arrival (forward filter) / at the state standing on a layer (backward refit).
-__device__ __forceinline__ float ms_at_crossing(const LayerConst& L, int model, const Crossing& o, float pz) {
-    return layer_ms(L, model, o.erx * o.elx + o.ery * o.ely, o.pt2 + pz * pz, o.ipt);
+template <class F>
+__device__ __forceinline__ F ms_at_crossing(const LayerConst& L, int model, const CrossingT<F>& o, arg<F> pz) {
+    if (model == 0) return F(L.ms);
+    return layer_ms<F>(L, model, o.erx * o.elx + o.ery * o.ely, o.pt2 + pz * pz, o.ipt);
 }
 
 // Propagated covariance in the arrival frame (radial row is exactly zero and not stored).
-struct PropCov {
-    float n11, n12, n13, n14, n15;
-    float n22, n23, n24, n25;
-    float n33, n34, n35;
-    float n44, n45;
-    float n55;
+template <class F>
+struct PropCovT {
+    F n11, n12, n13, n14, n15;
+    F n22, n23, n24, n25;
+    F n33, n34, n35;
+    F n44, n45;
+    F n55;
 };
+using PropCov = PropCovT<float>;
+using PropCov2 = PropCovT<f2>;
 
 // C' = F~ C F~^T + Q~ (reading A4 Jacobian, A5 process noise at the propagated momentum).
 // RADIAL_NULL: the input covariance already has a zero a1 row (every layer after the first).
-template <bool RADIAL_NULL>
-__device__ __forceinline__ void transport_cov(const Track& t, const Crossing& o, float ms,
-                                              float mass2, PropCov& n) {
-    const float g0 = o.g0, g1 = o.g1, g3 = o.g3, g4 = o.g4;
-    const float t0 = o.t0, t1 = o.t1, t3 = o.t3, t4 = o.t4;
-    const float z0 = o.z0, z1 = o.z1, z3 = o.z3, z4 = o.z4, thk = o.thk, mu = o.mu;
+template <bool RADIAL_NULL, class F>
+__device__ __forceinline__ void transport_cov(const TrackT<F>& t, const CrossingT<F>& o, arg<F> ms,
+                                              float mass2, PropCovT<F>& n) {
+    const F g0 = o.g0, g1 = o.g1, g3 = o.g3, g4 = o.g4;
+    const F t0 = o.t0, t1 = o.t1, t3 = o.t3, t4 = o.t4;
+    const F z0 = o.z0, z1 = o.z1, z3 = o.z3, z4 = o.z4, thk = o.thk, mu = o.mu;
     // v = C g, w = C tau, u = C zeta   (rows 1..5; row 0 and the a1 column only before the first layer)
-    float v1 = t.c11 * g1 + t.c13 * g3 + t.c14 * g4;
-    float v3 = t.c13 * g1 + t.c33 * g3 + t.c34 * g4;
-    float v4 = t.c14 * g1 + t.c34 * g3 + t.c44 * g4;
-    float v5 = t.c15 * g1 + t.c35 * g3 + t.c45 * g4;
-    float w1 = t.c11 * t1 + t.c13 * t3 + t.c14 * t4;
-    float w3 = t.c13 * t1 + t.c33 * t3 + t.c34 * t4;
-    float w4 = t.c14 * t1 + t.c34 * t3 + t.c44 * t4;
-    float w5 = t.c15 * t1 + t.c35 * t3 + t.c45 * t4;
-    float u1 = t.c12 + t.c11 * z1 + t.c13 * z3 + t.c14 * z4 + t.c15 * thk;
-    float u2 = t.c22 + t.c12 * z1 + t.c23 * z3 + t.c24 * z4 + t.c25 * thk;
-    float u3 = t.c23 + t.c13 * z1 + t.c33 * z3 + t.c34 * z4 + t.c35 * thk;
-    float u4 = t.c24 + t.c14 * z1 + t.c34 * z3 + t.c44 * z4 + t.c45 * thk;
-    float u5 = t.c25 + t.c15 * z1 + t.c35 * z3 + t.c45 * z4 + t.c55 * thk;
-    float gCg = g1 * v1 + g3 * v3 + g4 * v4;
-    float tCg = t1 * v1 + t3 * v3 + t4 * v4;
-    float zCg = g1 * u1 + g3 * u3 + g4 * u4;
-    float n11 = t1 * w1 + t3 * w3 + t4 * w4;
-    float n12 = t1 * u1 + t3 * u3 + t4 * u4;
-    float n22 = u2 + z1 * u1 + z3 * u3 + z4 * u4 + thk * u5;
+    F v1 = t.c11 * g1 + t.c13 * g3 + t.c14 * g4;
+    F v3 = t.c13 * g1 + t.c33 * g3 + t.c34 * g4;
+    F v4 = t.c14 * g1 + t.c34 * g3 + t.c44 * g4;
+    F v5 = t.c15 * g1 + t.c35 * g3 + t.c45 * g4;
+    F w1 = t.c11 * t1 + t.c13 * t3 + t.c14 * t4;
+    F w3 = t.c13 * t1 + t.c33 * t3 + t.c34 * t4;
+    F w4 = t.c14 * t1 + t.c34 * t3 + t.c44 * t4;
+    F w5 = t.c15 * t1 + t.c35 * t3 + t.c45 * t4;
+    F u1 = t.c12 + t.c11 * z1 + t.c13 * z3 + t.c14 * z4 + t.c15 * thk;
+    F u2 = t.c22 + t.c12 * z1 + t.c23 * z3 + t.c24 * z4 + t.c25 * thk;
+    F u3 = t.c23 + t.c13 * z1 + t.c33 * z3 + t.c34 * z4 + t.c35 * thk;
+    F u4 = t.c24 + t.c14 * z1 + t.c34 * z3 + t.c44 * z4 + t.c45 * thk;
+    F u5 = t.c25 + t.c15 * z1 + t.c35 * z3 + t.c45 * z4 + t.c55 * thk;
+    F gCg = g1 * v1 + g3 * v3 + g4 * v4;
+    F tCg = t1 * v1 + t3 * v3 + t4 * v4;
+    F zCg = g1 * u1 + g3 * u3 + g4 * u4;
+    F n11 = t1 * w1 + t3 * w3 + t4 * w4;
+    F n12 = t1 * u1 + t3 * u3 + t4 * u4;
+    F n22 = u2 + z1 * u1 + z3 * u3 + z4 * u4 + thk * u5;
     if constexpr (!RADIAL_NULL) {
-        const float v0 = t.c00 * g0 + t.c01 * g1 + t.c03 * g3 + t.c04 * g4;
-        const float w0 = t.c00 * t0 + t.c01 * t1 + t.c03 * t3 + t.c04 * t4;
-        const float u0 = t.c02 + t.c00 * z0 + t.c01 * z1 + t.c03 * z3 + t.c04 * z4 + t.c05 * thk;
+        const F v0 = t.c00 * g0 + t.c01 * g1 + t.c03 * g3 + t.c04 * g4;
+        const F w0 = t.c00 * t0 + t.c01 * t1 + t.c03 * t3 + t.c04 * t4;
+        const F u0 = t.c02 + t.c00 * z0 + t.c01 * z1 + t.c03 * z3 + t.c04 * z4 + t.c05 * thk;
         // a1-column contributions to rows 1..5 (added before the dot products use them)
-        const float dv1 = t.c01 * g0, dv3 = t.c03 * g0, dv4 = t.c04 * g0, dv5 = t.c05 * g0;
-        const float dw1 = t.c01 * t0, dw3 = t.c03 * t0, dw4 = t.c04 * t0, dw5 = t.c05 * t0;
-        const float du1 = t.c01 * z0, du2 = t.c02 * z0, du3 = t.c03 * z0, du4 = t.c04 * z0, du5 = t.c05 * z0;
+        const F dv1 = t.c01 * g0, dv3 = t.c03 * g0, dv4 = t.c04 * g0, dv5 = t.c05 * g0;
+        const F dw1 = t.c01 * t0, dw3 = t.c03 * t0, dw4 = t.c04 * t0, dw5 = t.c05 * t0;
+        const F du1 = t.c01 * z0, du2 = t.c02 * z0, du3 = t.c03 * z0, du4 = t.c04 * z0, du5 = t.c05 * z0;
         gCg += g0 * v0 + g1 * dv1 + g3 * dv3 + g4 * dv4;
         tCg += t0 * v0 + t1 * dv1 + t3 * dv3 + t4 * dv4;
         zCg += g0 * u0 + g1 * du1 + g3 * du3 + g4 * du4;
@@ -320,11 +341,11 @@ __device__ __forceinline__ void transport_cov(const Track& t, const Crossing& o,
     n.n25 = u5;
     // Highland (A5): theta0^2 = ms (p^2 + m^2) / p^4;  Q = theta0^2 (p^2 I - p p^T), p = (pT, 0, pz),
     // sheared to (b1, b2, c):  Q~ = theta0^2 [[pz^2, 0, -pz p^2/pT], [0, p^2, 0], [., 0, p^4/pT^2]]
-    const float pz = t.pz;
-    const float p2 = o.pt2 + pz * pz;
-    const float ip2 = rcp_fast(p2);
-    const float th2 = ms * (p2 + mass2) * ip2 * ip2;
-    const float qc = th2 * p2 * o.ipt;  // theta0^2 p^2 / pT
+    const F pz = t.pz;
+    const F p2 = o.pt2 + pz * pz;
+    const F ip2 = rcp_fast(p2);
+    const F th2 = ms * (p2 + mass2) * ip2 * ip2;
+    const F qc = th2 * p2 * o.ipt;  // theta0^2 p^2 / pT
     n.n33 = t.c33 + th2 * pz * pz;
     n.n34 = t.c34 + mu * v3;
     n.n35 = t.c35 - qc * pz;
@@ -370,20 +391,24 @@ __device__ __forceinline__ void scale_cov(Track& t, float f) {
 }
 
 // Hit in the arrival frame: residual (r, t, z) and rotated covariance.
-struct LocalHit {
-    float rr, rt, rz;
-    float vrr, vrt, vrz, vtt, vtz, vzz;
+template <class F>
+struct LocalHitT {
+    F rr, rt, rz;
+    F vrr, vrt, vrz, vtt, vtz, vzz;
 };
+using LocalHit = LocalHitT<float>;
+using LocalHit2 = LocalHitT<f2>;
 
-__device__ __forceinline__ void hit_to_local(const Crossing& o, float mx, float my, float mz,
-                                             float vxx, float vxy, float vxz, float vyy, float vyz,
-                                             float vzz, LocalHit& h) {
-    const float c = o.erx, s = o.ery;
-    const float dx = mx - o.xn, dy = my - o.yn;
+template <class F>
+__device__ __forceinline__ void hit_to_local(const CrossingT<F>& o, arg<F> mx, arg<F> my, arg<F> mz,
+                                             arg<F> vxx, arg<F> vxy, arg<F> vxz, arg<F> vyy, arg<F> vyz,
+                                             arg<F> vzz, LocalHitT<F>& h) {
+    const F c = o.erx, s = o.ery;
+    const F dx = mx - o.xn, dy = my - o.yn;
     h.rr = c * dx + s * dy;
     h.rt = c * dy - s * dx;
     h.rz = mz - o.zn;
-    const float cc = c * c, ss = s * s, cs = c * s;
+    const F cc = c * c, ss = s * s, cs = c * s;
     h.vrr = cc * vxx + 2.0f * cs * vxy + ss * vyy;
     h.vtt = ss * vxx - 2.0f * cs * vxy + cc * vyy;
     h.vrt = cs * (vyy - vxx) + (cc - ss) * vxy;
@@ -437,38 +462,44 @@ __device__ __forceinline__ bool chi2_schur(float n11, float n12, float n22, cons
 // Kalman update in the arrival frame, then re-aim the momentum frame at the updated momentum.
 // On success writes the new track (position frame = arrival frame) and returns the chi2
 // increment through *dchi2.  Returns a status bit on failure (track untouched).
-__device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, const PropCov& n,
-                                                  const LocalHit& h, float* dchi2) {
+// Pair form (F = f2): both tracks are updated or neither is -- if either fails, the statuses are returned
+// and the pair is left untouched (the caller then takes the two tracks one at a time).
+template <class F>
+__device__ __forceinline__ typename num_traits<F>::status
+kalman_update(TrackT<F>& t, const CrossingT<F>& o, const PropCovT<F>& n, const LocalHitT<F>& h, F* dchi2) {
+    using M = typename num_traits<F>::mask;
     // The radial row of C' is zero, so eliminating the radial component of S = C'_pp + V~ first
     // (Schur complement on v_rr) leaves a 2-D measurement in (t, z):
     //   V' = V_tz,tz - s s^T / v_rr,  s = (v_rt, v_rz);   r' = r_tz - s r_r / v_rr;
     //   S' = C'_tz,tz + V';  chi2 = r_r^2 / v_rr + r'^T S'^-1 r';  K = C'[:, tz] S'^-1;
     //   det S = v_rr det S'.
-    const float iv = rcp_fast(h.vrr);
-    const float sa = h.vrt * iv, sb = h.vrz * iv;
-    const float qtt = h.vtt - sa * h.vrt, qtz = h.vtz - sa * h.vrz, qzz = h.vzz - sb * h.vrz;
-    const float stt = n.n11 + qtt, stz = n.n12 + qtz, szz = n.n22 + qzz;
-    const float rt = h.rt - sa * h.rr, rz = h.rz - sb * h.rr;
-    const float det2 = stt * szz - stz * stz;
-    if (!(h.vrr * det2 > 0.0f)) return ST_S_NOT_PD;
-    const float id = rcp_fast(det2);
-    const float itt = szz * id, itz = -stz * id, izz = stt * id;
-    const float ut = itt * rt + itz * rz, uz = itz * rt + izz * rz;
-    const float chi2 = h.rr * h.rr * iv + rt * ut + rz * uz;
+    const F iv = rcp_fast(h.vrr);
+    const F sa = h.vrt * iv, sb = h.vrz * iv;
+    const F qtt = h.vtt - sa * h.vrt, qtz = h.vtz - sa * h.vrz, qzz = h.vzz - sb * h.vrz;
+    const F stt = n.n11 + qtt, stz = n.n12 + qtz, szz = n.n22 + qzz;
+    const F rt = h.rt - sa * h.rr, rz = h.rz - sb * h.rr;
+    const F det2 = stt * szz - stz * stz;
+    const M pd = h.vrr * det2 > 0.0f;
+    if (!all_of(pd)) return select_u(!pd, ST_S_NOT_PD, 0u);
+    const F id = rcp_fast(det2);
+    const F itt = szz * id, itz = -stz * id, izz = stt * id;
+    const F ut = itt * rt + itz * rz, uz = itz * rt + izz * rz;
+    const F chi2 = h.rr * h.rr * iv + rt * ut + rz * uz;
     // state increments d = C'[:, tz] S'^-1 r'
-    const float d1 = n.n11 * ut + n.n12 * uz;
-    const float d2 = n.n12 * ut + n.n22 * uz;
-    const float d3 = n.n13 * ut + n.n23 * uz;
-    const float d4 = n.n14 * ut + n.n24 * uz;
-    const float d5 = n.n15 * ut + n.n25 * uz;
+    const F d1 = n.n11 * ut + n.n12 * uz;
+    const F d2 = n.n12 * ut + n.n22 * uz;
+    const F d3 = n.n13 * ut + n.n23 * uz;
+    const F d4 = n.n14 * ut + n.n24 * uz;
+    const F d5 = n.n15 * ut + n.n25 * uz;
     // finite(chi2) and finite(state): any non-finite term makes this sum non-finite
-    const float probe = chi2 + ((d1 + d2) + (d3 + d4) + d5) * 0.0f;
-    if (!(fabsf(probe) < __int_as_float(0x7f800000))) return ST_NONFINITE;
+    const F probe = chi2 + ((d1 + d2) + (d3 + d4) + d5) * 0.0f;
+    const M fin = abs_(probe) < __int_as_float(0x7f800000);
+    if (!all_of(fin)) return select_u(!fin, ST_NONFINITE, 0u);
     *dchi2 = chi2;
     // gain rows (t z b1 b2 c) x columns (t, z)
-#define KF_KROW(ct, cz, kt, kz)                \
-    const float kt = ct * itt + cz * itz;      \
-    const float kz = ct * itz + cz * izz;
+#define KF_KROW(ct, cz, kt, kz)            \
+    const F kt = ct * itt + cz * itz;      \
+    const F kz = ct * itz + cz * izz;
     KF_KROW(n.n11, n.n12, k1t, k1z)
     KF_KROW(n.n12, n.n22, k2t, k2z)
     KF_KROW(n.n13, n.n23, k3t, k3z)
@@ -479,11 +510,11 @@ __device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, c
     t.x = o.xn - o.ery * d1;
     t.y = o.yn + o.erx * d1;
     t.z = o.zn + d2;
-    const float pxu = o.pxn + o.elx * d3 - o.ely * d4;
-    const float pyu = o.pyn + o.ely * d3 + o.elx * d4;
+    const F pxu = o.pxn + o.elx * d3 - o.ely * d4;
+    const F pyu = o.pyn + o.ely * d3 + o.elx * d4;
     t.px = pxu;
     t.py = pyu;
-    const float pzu = t.pz + d5 + o.T * d3;
+    const F pzu = t.pz + d5 + o.T * d3;
     t.pz = pzu;
     t.eax = o.erx;
     t.eay = o.ery;
@@ -499,18 +530,18 @@ __device__ __forceinline__ uint32_t kalman_update(Track& t, const Crossing& o, c
     t.c15 = k5t * qtt + k5z * qtz;
     t.c25 = k5t * qtz + k5z * qzz;
     // momentum block: C'_mm - K_m C'_pm  (C'_pm rows t, z)
-    t.c33 = fmaf(-k3z, n.n23, fmaf(-k3t, n.n13, n.n33));
-    t.c34 = fmaf(-k3z, n.n24, fmaf(-k3t, n.n14, n.n34));
-    t.c35 = fmaf(-k3z, n.n25, fmaf(-k3t, n.n15, n.n35));
-    t.c44 = fmaf(-k4z, n.n24, fmaf(-k4t, n.n14, n.n44));
-    t.c45 = fmaf(-k4z, n.n25, fmaf(-k4t, n.n15, n.n45));
-    t.c55 = fmaf(-k5z, n.n25, fmaf(-k5t, n.n15, n.n55));
+    t.c33 = fma_(-k3z, n.n23, fma_(-k3t, n.n13, n.n33));
+    t.c34 = fma_(-k3z, n.n24, fma_(-k3t, n.n14, n.n34));
+    t.c35 = fma_(-k3z, n.n25, fma_(-k3t, n.n15, n.n35));
+    t.c44 = fma_(-k4z, n.n24, fma_(-k4t, n.n14, n.n44));
+    t.c45 = fma_(-k4z, n.n25, fma_(-k4t, n.n15, n.n45));
+    t.c55 = fma_(-k5z, n.n25, fma_(-k5t, n.n15, n.n55));
     // re-aim the momentum frame: exp(i d) = conj(e_l,new) e_l' = ((pT + d3) - i d4) / pT,new
-    const float pt = o.pt2 * o.ipt;
-    const float ar = pt + d3;
-    const float iptn = rsqrt_fast(ar * ar + d4 * d4);
+    const F pt = o.pt2 * o.ipt;
+    const F ar = pt + d3;
+    const F iptn = rsqrt_fast(ar * ar + d4 * d4);
     reaim_momentum<true>(t, ar * iptn, -d4 * iptn, o.T, pzu * iptn);
-    return 0u;
+    return select_u(pd, 0u, 0u);
 }
 
 // Keep the propagated state (no hit used): position frame = arrival frame, momentum frame

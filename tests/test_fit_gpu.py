@@ -153,6 +153,54 @@ def test_fit_propagation_failure(ctx):
     compare_fit(_zero_status(g), _zero_status(o), float(b.radius[-1]), max_diverged_frac=0.05)
 
 
+def test_fit_pair_kernel_edge_cases(ctx):
+    """Batches of >= 151 552 tracks take the two-tracks-per-thread kernel (packed fp32x2 arithmetic); a layer
+    that only one track of a pair has a hit on, or on which one of the two fails, goes through its one-track
+    path.  Every degenerate case of the small tests above, at a size that selects that kernel, odd tail included."""
+    cfg = W.get_config(1)
+    low = W.BarrelConfig(1, 1, 256, 10, 0.17, 0.18, 1.0, 0.01)          # no crossing with the two outer layers
+    parts = [W.simulate_event(cfg, 30 + e) for e in range(8)] + [W.simulate_event(low, 21), W.simulate_event(cfg, 38, n_tracks=3)]
+    b = W.concat_batches(parts)
+    assert b.n == 160_259 and b.n % 2 == 1
+    rng = np.random.default_rng(11)
+    holes = rng.random(b.n) < 0.1
+    holes[160_000:] = False        # (near-looping tracks with gaps leave the linear regime: DESIGN.md 'Known limits')
+    b.mask = np.where(holes, (rng.integers(0, 1 << 10, size=b.n) | 0b111), b.mask).astype(np.uint32)
+    b.mask[:50] = 0
+    b.mask[50:100] = 0b1111111110
+    b.mask[101:150:2] = 0b0000000111                                    # odd tracks only: their partners go on
+    lo = 160_000
+    b.mask[lo:lo + 256] |= np.uint32(0b11 << 8)                          # PROP_FAIL on layers 8 and 9
+    b.q[200] = 0
+    b.q[203] = 3
+    b.hpos[4, 1, 300] = np.nan                                          # NONFINITE on layer 4 of track 300
+    b.hcov[2, :, 303] = 0.0
+    b.hcov[2, 0, 303] = -1.0                                            # S_NOT_PD on layer 2 of track 303
+    b.mask[300] = b.mask[303] = b.mask[301] = b.mask[302] = 0x3ff
+    g = _gpu_fit(ctx, b)
+    o = O.fit_batch(b, nthreads=8)
+    assert np.array_equal(g["status"], o["status"]), np.flatnonzero(g["status"] != o["status"])[:10]
+    assert np.array_equal(g["nhits"], o["nhits"])
+    assert o["status"][200] == 8 and o["status"][203] == 8 and o["status"][300] == 4 and o["status"][303] == 2
+    assert np.all(o["status"][lo:lo + 256] == 1)
+    z = o["nhits"] == 0
+    assert z.sum() >= 52
+    assert np.array_equal(g["par"][:, z], b.par[:, z]) and np.array_equal(g["cov"][:, z], b.cov[:, z])
+    assert np.all(g["chi2"][z] == 0)
+    sel = o["nhits"] >= 4
+    sub_g = {k: (v[..., sel] if k in ("par", "cov") else v[sel]) for k, v in g.items()}
+    sub_o = {k: (v[..., sel] if k == "par" else v[sel]) for k, v in o.items()}
+    res = compare_fit(_zero_status(sub_g), _zero_status(sub_o), float(b.radius[-1]), max_diverged_frac=0.02)
+    print("pair kernel, edge cases:", res)
+    # in place, same kernel
+    from paper_1705_02876_b200.buffers import DeviceFit
+    d = DeviceFit.from_batch(b, "cuda:0")
+    ctx.fit_tracks(d.geom, d.n, d.par, d.cov, d.q, d.hpos, d.hcov, d.mask, d.par, d.cov,
+                   d.out_chi2, d.out_nhits, d.out_status)
+    torch.cuda.synchronize()
+    assert np.array_equal(d.par[:, :d.n].cpu().numpy(), g["par"]) and np.array_equal(d.cov[:, :d.n].cpu().numpy(), g["cov"])
+
+
 def test_fit_in_place(ctx):
     from paper_1705_02876_b200.buffers import DeviceFit
     b = W.simulate_event(W.get_config(1), 10, n_tracks=777)

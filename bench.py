@@ -29,9 +29,9 @@ import numpy as np
 METRIC = "kalman_track_fits_per_sec_10_layer_barrel"
 UNIT = "fits/s"
 CONFIG_INDEX = 2
-# dram__bytes_read.sum + dram__bytes_write.sum of fit_kernel for one 2M-track launch, from the
-# `ncu --set full` capture summarised in profiles/r01_fit_kernel.md.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 946045184 + 219278848   # profiles/r01_fit_kernel.md
+# dram__bytes_read.sum + dram__bytes_write.sum of fit_pair_kernel for one 2M-track launch, from the
+# `ncu --set full` capture summarised in profiles/r01_fit_pair_kernel.md.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 946058496 + 218302720   # profiles/r01_fit_pair_kernel.md
 # Algorithmic flops per track and layer of the filter as the oracle states it, exploiting the known zeros and
 # ones of F and H and symmetry: propagation 75, Jacobian 95, F C F^T 340,
 # Q 35, update 310 (S 9, S^-1 30, chi2 21, K 90, x 36, C 126) -- frozen before any tuning.
@@ -378,13 +378,13 @@ def run_ours(args) -> None:
         peak, peak_src = _peaks()
         alg_bytes = d.algorithmic_bytes
         t_launch = ms_local / args.steps * 1e-3
-        hbm = {"bound": "hbm", "kernel": "kf::fit_kernel", "achieved": alg_bytes / t_launch / 1e9, "peak": peak,
+        hbm = {"bound": "hbm", "kernel": "kf::fit_pair_kernel", "achieved": alg_bytes / t_launch / 1e9, "peak": peak,
                "unit": "GB/s", "frac": alg_bytes / t_launch / 1e9 / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
                "peak_source": peak_src, "algorithmic_bytes_per_launch": int(alg_bytes), "bytes_per_fit": 233 + 36 * L}
         # ALU roofline: algorithmic flops of the textbook sparse 6x6 filter (850 flop per
         # track and layer, frozen before tuning) against the FP32 FMA peak measured on this GPU just now.
         alg_flops = float(n) * FLOPS_PER_TRACK_LAYER * L
-        alu = {"bound": "alu", "kernel": "kf::fit_kernel", "achieved": alg_flops / t_launch / 1e12, "peak": fp32_peak,
+        alu = {"bound": "alu", "kernel": "kf::fit_pair_kernel", "achieved": alg_flops / t_launch / 1e12, "peak": fp32_peak,
                "unit": "TFLOP/s", "frac": alg_flops / t_launch / 1e12 / fp32_peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
                "peak_source": "measured now: kf_measure_fp32_peak (register-only FMA chains); nominal 148 SM x 128 lanes "
                               "x 2 x 1.965 GHz = 74.4", "algorithmic_flops_per_launch": alg_flops,

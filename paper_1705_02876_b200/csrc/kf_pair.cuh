@@ -99,7 +99,21 @@ __device__ __forceinline__ f2 fma_(f2 a, f2 b, f2 c) { return f2(__ffma2_rn(a.v,
 __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
 __device__ __forceinline__ f2 abs_(f2 a) { return f2(fabsf(a.v.x), fabsf(a.v.y)); }
 __device__ __forceinline__ float atan_(float a) { return atanf(a); }
-__device__ __forceinline__ f2 atan_(f2 a) { return f2(atanf(a.v.x), atanf(a.v.y)); }
+// atan of a pair: while both arguments are below tan(pi/8) (a helix step that turns less than 45 degrees, i.e.
+// every step of a track that is not about to loop) one packed odd polynomial, atan x = x + x z g(z), z = x^2,
+// g of degree 3 fitted to (atan x / x - 1) / z over z in [0, tan^2(pi/8)] (weighted least squares on 4000
+// Chebyshev nodes, Lawson-reweighted towards minimax); 7.9e-8 maximum relative error evaluated in fp32.
+__device__ __forceinline__ f2 atan_(f2 a) {
+    constexpr float kLim = 0.41421354f;
+    if (fabsf(a.v.x) < kLim && fabsf(a.v.y) < kLim) {
+        const f2 z = a * a;
+        f2 g = fma_(f2(0.08053719252347946f), z, f2(-0.1387767791748047f));
+        g = fma_(g, z, f2(0.19977709650993347f));
+        g = fma_(g, z, f2(-0.3333294987678528f));
+        return a + (a * z) * g;
+    }
+    return f2(atanf(a.v.x), atanf(a.v.y));
+}
 __device__ __forceinline__ float sqrt_(float a) { return sqrtf(a); }
 __device__ __forceinline__ f2 sqrt_(f2 a) { return f2(sqrtf(a.v.x), sqrtf(a.v.y)); }
 __device__ __forceinline__ float log_fast(float a) { return __logf(a); }

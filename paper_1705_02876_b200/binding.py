@@ -9,6 +9,7 @@ kf_fit_tracks, .fit_tracks_host -> kf_fit_tracks_host, .bin_hits -> kf_bin_hits,
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 from dataclasses import dataclass
 
@@ -201,7 +202,7 @@ def _plane_ld(t: torch.Tensor, rows: int) -> int:
     ld = t.stride(-2) if t.dim() >= 2 else t.shape[-1]
     if t.dim() == 3 and t.stride(0) != t.shape[1] * ld:
         raise ValueError("layer planes must be densely stacked")
-    flat_rows = int(np.prod(t.shape[:-1]))
+    flat_rows = math.prod(t.shape[:-1])
     if flat_rows != rows:
         raise ValueError(f"expected {rows} planes, got {flat_rows}")
     return int(ld)

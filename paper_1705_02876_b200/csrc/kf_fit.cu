@@ -633,16 +633,36 @@ EncodeTiledFn encode_fn() {
 }
 
 // Tensor map over a [rows][ld] float array of which n columns are valid; tiles are [box_rows][box_cols].
+// Encoding a map costs a driver call; a caller that fits event after event through the same buffers asks for
+// the same few maps every time, so the last 16 are kept per host thread (a map depends on nothing but the key).
+struct MapKey {
+    const float* base; int64_t n, ld, rows; int box_rows, box_cols;
+    bool operator==(const MapKey& o) const {
+        return base == o.base && n == o.n && ld == o.ld && rows == o.rows && box_rows == o.box_rows && box_cols == o.box_cols;
+    }
+};
 bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t rows, int box_rows, int box_cols = 32) {
+    constexpr int kCached = 16;
+    thread_local MapKey keys[kCached] = {};
+    thread_local CUtensorMap maps[kCached];
+    thread_local int next = 0;
+    const MapKey key{base, n, ld, rows, box_rows, box_cols};
+    for (int i = 0; i < kCached; ++i)
+        if (keys[i].base != nullptr && keys[i] == key) { *m = maps[i]; return true; }
     EncodeTiledFn enc = encode_fn();
     if (!enc) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
     const cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
-    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    if (enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    keys[next] = key;
+    maps[next] = *m;
+    next = (next + 1) % kCached;
+    return true;
 }
 
 }  // namespace

@@ -386,7 +386,7 @@ void orc_fit_smooth_one(int L, const double *radius, const double *xX0, double B
                         int32_t *onhits, uint32_t *ostatus, double spar[6], double scov[36], double *schi2,
                         uint32_t *sstatus, double *trace_fwd, double *trace_bwd) {
     double *tf = trace_fwd, *own = NULL;
-    if (!tf) { own = (double *)malloc((size_t)L * ORC_TRACE_STRIDE * sizeof(double)); tf = own; }
+    if (!tf) { own = (double *)calloc((size_t)L * ORC_TRACE_STRIDE, sizeof(double)); tf = own; } /* zeroed: fit_one writes no trace for a bad charge */
     fit_one(L, radius, xX0, Bz, mass, par, cov, q, hpos, hcov, mask, opar, ocov, ochi2, onhits, ostatus, tf);
     uint32_t used = 0;
     for (int l = 0; l < L; ++l)

@@ -39,6 +39,9 @@ namespace {
 #endif
 // Batches of at least this many tracks take the pair kernel (two tracks per thread); smaller ones would
 // leave SMs idle with 256 tracks per CTA and keep the one-track kernel.
+#ifndef KF_PAIR_SMOOTH
+#define KF_PAIR_SMOOTH 1
+#endif
 #ifndef KF_PAIR_MIN_TRACKS
 #define KF_PAIR_MIN_TRACKS 151552
 #endif
@@ -260,27 +263,11 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             m.vyy = tp[192];     m.vyz = tp[224];     m.vzz = tp[256];
             __syncwarp();
             if ((used >> l) & 1u) {
-                Crossing o;
-                PropCov n;
-                uint32_t reached = 0u;
-                const float k33 = t.c33, k35 = t.c35, k44 = t.c44, k55 = t.c55;
-                if (first) crossing_in_place(t, o, n);
-                else {
-                    reached = reach_layer<true, GEOM>(t, k, ik, P.layer[l], o);
-                    if (!reached) {
-                        add_process_noise(t, P.layer[l_prev], model, P.mass2);   // the scatterer just left behind
-                        transport_cov<true>(t, o, 0.0f, P.mass2, n);
-                    }
-                }
-                if (reached) sst |= reached;
-                else {
-                    LocalHit h;
-                    hit_to_local(o, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
-                    float d;
-                    const uint32_t rc = kalman_update(t, o, n, h, &d);
-                    if (rc == 0u) { schi2 += d; nb += 1; first = false; l_prev = l; }
-                    else { sst |= rc; t.c33 = k33; t.c35 = k35; t.c44 = k44; t.c55 = k55; }   // layer skipped
-                }
+                float d;
+                const uint32_t rc = refit_step<GEOM>(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, first,
+                                                     m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, &d);
+                if (rc == 0u) { schi2 += d; nb += 1; first = false; l_prev = l; }
+                else sst |= rc;
             }
             const int nxt = step + kStages;
             if (nxt < 2 * L) {
@@ -342,6 +329,9 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
 #endif
 #ifndef KF_PAIR_MIN_BLOCKS
 #define KF_PAIR_MIN_BLOCKS 3
+#endif
+#ifndef KF_PAIR_SMOOTH_MIN_BLOCKS
+#define KF_PAIR_SMOOTH_MIN_BLOCKS 3
 #endif
 constexpr int kPairBlock = KF_PAIR_BLOCK;
 constexpr int kPairWarps = kPairBlock / 32;
@@ -409,14 +399,56 @@ __device__ __noinline__ uint32_t fit_layer_one_of_pair(Track2& t, int c, float k
     if (c) chi2.v.y += ch; else chi2.v.x += ch;
     return 0u;
 }
-#undef KF_TRACK_FIELDS
 
 #define KF_TRACK_ROWS(X)                                                                                   \
     X(0, x) X(1, y) X(2, z) X(3, px) X(4, py) X(5, pz) X(6, c00) X(7, c01) X(8, c02) X(9, c03) X(10, c04)   \
     X(11, c05) X(12, c11) X(13, c12) X(14, c13) X(15, c14) X(16, c15) X(17, c22) X(18, c23) X(19, c24)      \
     X(20, c25) X(21, c33) X(22, c34) X(23, c35) X(24, c44) X(25, c45) X(26, c55)
 
-__global__ void __launch_bounds__(kPairBlock, KF_PAIR_MIN_BLOCKS)
+// One backward step (reading A18) for component c of a pair, out of line like fit_layer_one_of_pair.
+__device__ __noinline__ uint32_t refit_step_one_of_pair(Track2& t, int c, float k, float ik, const LayerConst& L,
+                                                        const LayerConst& Lprev, float mass2, bool first,
+                                                        const Hit2& m, f2& schi2) {
+    Track ts;
+    Hit mh;
+    float d = 0.0f;
+#define KF_GET(f) ts.f = c ? t.f.v.y : t.f.v.x;
+    KF_TRACK_FIELDS(KF_GET)
+#undef KF_GET
+#define KF_GETH(f) mh.f = c ? m.f.v.y : m.f.v.x;
+    KF_GETH(x) KF_GETH(y) KF_GETH(z) KF_GETH(vxx) KF_GETH(vxy) KF_GETH(vxz) KF_GETH(vyy) KF_GETH(vyz) KF_GETH(vzz)
+#undef KF_GETH
+    const uint32_t rc = refit_step<false>(ts, k, ik, L, Lprev, 0, mass2, first, mh.x, mh.y, mh.z, mh.vxx, mh.vxy,
+                                          mh.vxz, mh.vyy, mh.vyz, mh.vzz, &d);
+    if (rc != 0u) return rc;
+#define KF_PUT(f) if (c) t.f.v.y = ts.f; else t.f.v.x = ts.f;
+    KF_TRACK_FIELDS(KF_PUT)
+#undef KF_PUT
+    if (c) schi2.v.y += d; else schi2.v.x += d;
+    return 0u;
+}
+#undef KF_TRACK_FIELDS
+
+// Result pair -> the warp's [27][64] tile: both tracks with one 8-byte store per row, or only the one that
+// has a result (the other's columns keep what the tile holds).
+__device__ __forceinline__ void pair_to_tile(const Track2& t, float* tile, int lane, mask2 done) {
+    if (all_of(done)) {
+        float2* p = reinterpret_cast<float2*>(tile) + lane;
+#define KF_STORE_ROW(r, f) p[(r) * (kPairTile / 2)] = t.f.v;
+        KF_TRACK_ROWS(KF_STORE_ROW)
+#undef KF_STORE_ROW
+    } else {
+        float* p = tile + 2 * lane + (done.y ? 1 : 0);
+#define KF_STORE_ONE(r, f) p[(r) * kPairTile] = done.y ? t.f.v.y : t.f.v.x;
+        KF_TRACK_ROWS(KF_STORE_ONE)
+#undef KF_STORE_ONE
+    }
+}
+
+// SMOOTH = true: the forward fit, then the inward refit of reading A18 over the same hits (ring runs on,
+// outermost layer first), as in fit_kernel<true, false>.
+template <bool SMOOTH>
+__global__ void __launch_bounds__(kPairBlock, SMOOTH ? KF_PAIR_SMOOTH_MIN_BLOCKS : KF_PAIR_MIN_BLOCKS)
 fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -473,9 +505,12 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
     int nhx = 0, nhy = 0;
     u2 st = {0u, 0u};
     mask2 started = {false, false};   // false: general 6x6 covariance; true: its radial row is identically zero
+    uint32_t phase = 0u;              // SMOOTH: bit s = parity the next wait on stage s expects
+    uint32_t usedx = 0u, usedy = 0u;  // layers the forward fit used
     for (int l = 0; l < L; ++l) {
         const int s = l % kStages;
-        mbar_wait(bar0 + 8u * s, (uint32_t)(l / kStages) & 1u);
+        if constexpr (SMOOTH) { mbar_wait(bar0 + 8u * s, (phase >> s) & 1u); phase ^= 1u << s; }
+        else mbar_wait(bar0 + 8u * s, (uint32_t)(l / kStages) & 1u);
         const float2* tp = reinterpret_cast<const float2*>(wbase + s * kHit2Floats) + lane;
         const mask2 want = {live.x && ((mx >> l) & 1u), live.y && ((my >> l) & 1u)};
         bool both = false;
@@ -487,6 +522,7 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
         if (both) {
             nhx += 1; nhy += 1;
             started.x = true; started.y = true;
+            usedx |= 1u << l; usedy |= 1u << l;
         } else if (!none_of(want)) {
             // copies whose address may be taken: the pair itself stays in registers
             Track2 tc = t;
@@ -496,23 +532,25 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
             if (want.x) {
                 const uint32_t rc = fit_layer_one_of_pair(tc, 0, k.v.x, ik.v.x, P.layer[l], P.mass2, mc, cc, started.x);
                 st.x |= rc;
-                if (rc == 0u) { nhx += 1; started.x = true; }
+                if (rc == 0u) { nhx += 1; started.x = true; usedx |= 1u << l; }
             }
             if (want.y) {
                 const uint32_t rc = fit_layer_one_of_pair(tc, 1, k.v.y, ik.v.y, P.layer[l], P.mass2, mc, cc, started.y);
                 st.y |= rc;
-                if (rc == 0u) { nhy += 1; started.y = true; }
+                if (rc == 0u) { nhy += 1; started.y = true; usedy |= 1u << l; }
             }
             t = tc;
             chi2 = cc;
         }
+        // (SMOOTH: the ring runs on into the backward pass, step L + j carries layer L - 1 - j)
         const int nxt = l + kStages;
-        if (nxt < L) {
+        if (nxt < (SMOOTH ? 2 * L : L)) {
+            const int ln = nxt < L ? nxt : 2 * L - 1 - nxt;
             __syncwarp();
             if (elect_one()) {
                 mbar_expect_tx(bar0 + 8u * s, kHit2Floats * 4);
-                tma_load_2d(hit0 + s * (kHit2Floats * 4), &M.hpos, col, 3 * nxt, bar0 + 8u * s);
-                tma_load_2d(hit0 + s * (kHit2Floats * 4) + 3 * kRowBytes, &M.hcov, col, 6 * nxt, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4), &M.hpos, col, 3 * ln, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4) + 3 * kRowBytes, &M.hcov, col, 6 * ln, bar0 + 8u * s);
             }
         }
     }
@@ -520,19 +558,100 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
     if (!good_q.y) st.y = ST_BAD_CHARGE;
     // a track with nothing fitted goes back as it came: its columns of the seed tile still hold the input
     const mask2 done = {live.x && nhx > 0, live.y && nhy > 0};
+    if constexpr (SMOOTH) {
+        // ---- forward result out (a copy goes back to the global frame; t stays local for the refit)
+        if (!none_of(done)) {
+            Track2 g = t;
+            leave_local_frame(g);
+            pair_to_tile(g, seed_tile, lane, done);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        const bool fstorer = elect_one();
+        if (fstorer) {
+            tma_store_2d(&M.opar, col, 0, seed0);
+            tma_store_2d(&M.ocov, col, 0, seed0 + 6 * kRowBytes);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        if (valid.x) { a.chi2[ix] = chi2.v.x; a.nhits[ix] = nhx; a.status[ix] = st.x; }
+        if (valid.y) { a.chi2[iy] = chi2.v.y; a.nhits[iy] = nhy; a.status[iy] = st.y; }
+        // ---- inward refit (reading A18)
+        f2 schi2(0.0f);
+        int lpx = 0, lpy = 0, nbx = 0, nby = 0;
+        u2 sst = {0u, 0u};
+        mask2 first = {true, true};
+        if (!none_of(done)) scale_cov(t, a.kappa);
+        for (int j = 0; j < L; ++j) {
+            const int l = L - 1 - j, step = L + j, s = step % kStages;
+            mbar_wait(bar0 + 8u * s, (phase >> s) & 1u);
+            phase ^= 1u << s;
+            const float2* tp = reinterpret_cast<const float2*>(wbase + s * kHit2Floats) + lane;
+            const mask2 want = {(bool)((usedx >> l) & 1u), (bool)((usedy >> l) & 1u)};
+            bool both = false;
+            if (all_of(want) && first.x == first.y && (first.x || lpx == lpy)) {
+                Hit2 m;
+                load_hit_pair(m, tp);
+                f2 d;
+                const u2 rc = refit_step<false>(t, k, ik, P.layer[l], P.layer[lpx], 0, P.mass2, first.x, m.x, m.y, m.z,
+                                                m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, &d);
+                if (is_zero(rc)) {
+                    schi2 = schi2 + d;
+                    nbx += 1; nby += 1;
+                    first.x = false; first.y = false;
+                    lpx = l; lpy = l;
+                    both = true;
+                }
+            }
+            if (!both && !none_of(want)) {
+                Track2 tc = t;
+                Hit2 mc;
+                load_hit_pair(mc, tp);
+                f2 cc = schi2;
+                if (want.x) {
+                    const uint32_t rc = refit_step_one_of_pair(tc, 0, k.v.x, ik.v.x, P.layer[l], P.layer[lpx], P.mass2, first.x, mc, cc);
+                    if (rc == 0u) { nbx += 1; first.x = false; lpx = l; } else sst.x |= rc;
+                }
+                if (want.y) {
+                    const uint32_t rc = refit_step_one_of_pair(tc, 1, k.v.y, ik.v.y, P.layer[l], P.layer[lpy], P.mass2, first.y, mc, cc);
+                    if (rc == 0u) { nby += 1; first.y = false; lpy = l; } else sst.y |= rc;
+                }
+                t = tc;
+                schi2 = cc;
+            }
+            const int nxt = step + kStages;
+            if (nxt < 2 * L) {
+                const int ln = 2 * L - 1 - nxt;
+                __syncwarp();
+                if (elect_one()) {
+                    mbar_expect_tx(bar0 + 8u * s, kHit2Floats * 4);
+                    tma_load_2d(hit0 + s * (kHit2Floats * 4), &M.hpos, col, 3 * ln, bar0 + 8u * s);
+                    tma_load_2d(hit0 + s * (kHit2Floats * 4) + 3 * kRowBytes, &M.hcov, col, 6 * ln, bar0 + 8u * s);
+                }
+            }
+        }
+        // the forward tile must have left shared memory before the smoothed one overwrites it
+        if (fstorer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncwarp();
+        if (!none_of(done)) {
+            leave_local_frame(t);
+            pair_to_tile(t, seed_tile, lane, done);
+        }   // else the tile still holds the forward result = the input
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        const bool sstorer = elect_one();
+        if (sstorer) {
+            tma_store_2d(&M.spar, col, 0, seed0);
+            tma_store_2d(&M.scov, col, 0, seed0 + 6 * kRowBytes);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        if (valid.x) { a.schi2[ix] = schi2.v.x; a.snhits[ix] = nbx; a.sstatus[ix] = sst.x; }
+        if (valid.y) { a.schi2[iy] = schi2.v.y; a.snhits[iy] = nby; a.sstatus[iy] = sst.y; }
+        if (sstorer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        return;
+    }
     if (!none_of(done)) {
         leave_local_frame(t);
-        if (all_of(done)) {
-            float2* p = reinterpret_cast<float2*>(seed_tile) + lane;
-#define KF_STORE_ROW(r, f) p[(r) * (kPairTile / 2)] = t.f.v;
-            KF_TRACK_ROWS(KF_STORE_ROW)
-#undef KF_STORE_ROW
-        } else {
-            float* p = seed_tile + 2 * lane + (done.y ? 1 : 0);
-#define KF_STORE_ONE(r, f) p[(r) * kPairTile] = done.y ? t.f.v.y : t.f.v.x;
-            KF_TRACK_ROWS(KF_STORE_ONE)
-#undef KF_STORE_ONE
-        }
+        pair_to_tile(t, seed_tile, lane, done);
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncwarp();
@@ -680,9 +799,12 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     const bool smooth = a.spar != nullptr;
     const int L = P.n_layers;
     FitMaps M;
-    if (!smooth && P.geometry_options == 0 && a.n >= (int64_t)KF_PAIR_MIN_TRACKS) {   // headline path: two tracks per thread
-        static const cudaError_t attr_pair =
-            cudaFuncSetAttribute(fit_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem2Bytes);
+    if (P.geometry_options == 0 && a.n >= (int64_t)KF_PAIR_MIN_TRACKS && (!smooth || KF_PAIR_SMOOTH)) {   // two tracks per thread
+        static const cudaError_t attr_pair = [] {
+            cudaError_t e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem2Bytes);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem2Bytes);
+            return e;
+        }();
         if (attr_pair != cudaSuccess) return attr_pair;
         constexpr int W = kPairTile;
         if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3, W) ||
@@ -690,9 +812,12 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
             !make_map(&M.par, a.par, a.n, a.ld_in, 6, 6, W) || !make_map(&M.cov, a.cov, a.n, a.ld_in, 21, 21, W) ||
             !make_map(&M.opar, a.opar, a.n, a.ld_out, 6, 6, W) || !make_map(&M.ocov, a.ocov, a.n, a.ld_out, 21, 21, W))
             return cudaErrorInvalidValue;
+        if (smooth && (!make_map(&M.spar, a.spar, a.n, a.ld_s, 6, 6, W) || !make_map(&M.scov, a.scov, a.n, a.ld_s, 21, 21, W)))
+            return cudaErrorInvalidValue;
         const int64_t per_block = (int64_t)kPairWarps * kPairTile;
         const int64_t blocks = (a.n + per_block - 1) / per_block;
-        fit_pair_kernel<<<(unsigned)blocks, kPairBlock, kSmem2Bytes, stream>>>(P, M, a);
+        if (smooth) fit_pair_kernel<true><<<(unsigned)blocks, kPairBlock, kSmem2Bytes, stream>>>(P, M, a);
+        else fit_pair_kernel<false><<<(unsigned)blocks, kPairBlock, kSmem2Bytes, stream>>>(P, M, a);
         return cudaGetLastError();
     }
     if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3) ||

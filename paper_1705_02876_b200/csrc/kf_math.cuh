@@ -257,12 +257,14 @@ __device__ __forceinline__ typename num_traits<F>::mask helix_to_radius(const Tr
 // helix_to_radius plus the acceptance of reading A20: 0, ST_PROP_FAIL, or ST_OUTSIDE when the crossing
 // lies beyond the end of the barrel (|z'| > half length; the layer is then skipped like a failed one).
 // BOUNDED = false compiles the acceptance test out (kernels specialised for the unbounded toy detector).
-template <bool INWARD = false, bool BOUNDED = true>
-__device__ __forceinline__ uint32_t reach_layer(const Track& t, float k, float ik, const LayerConst& L,
-                                                Crossing& o) {
-    if (!helix_to_radius<INWARD>(t, k, ik, L, o)) return ST_PROP_FAIL;
-    if constexpr (BOUNDED) return fabsf(o.zn) > L.half_len ? ST_OUTSIDE : 0u;
-    else return 0u;
+// Pair form: per-component status; if either is non-zero the caller takes the two tracks one at a time.
+template <bool INWARD = false, bool BOUNDED = true, class F>
+__device__ __forceinline__ typename num_traits<F>::status reach_layer(const TrackT<F>& t, arg<F> k, arg<F> ik,
+                                                                      const LayerConst& L, CrossingT<F>& o) {
+    const typename num_traits<F>::mask ok = helix_to_radius<INWARD>(t, k, ik, L, o);
+    if (!all_of(ok)) return select_u(ok, 0u, ST_PROP_FAIL);
+    if constexpr (BOUNDED) return select_u(abs_(o.zn) > L.half_len, ST_OUTSIDE, 0u);
+    else return select_u(ok, 0u, 0u);
 }
 
 // Highland factor at an arrival (forward filter) / at the state standing on a layer (backward refit).
@@ -356,14 +358,15 @@ __device__ __forceinline__ void transport_cov(const TrackT<F>& t, const Crossing
 
 // Reading A18, backward refit: the scatterer just left behind adds its Highland noise to the momentum
 // block BEFORE the inward propagation (same Q~ as in transport_cov, at the current momentum).
-__device__ __forceinline__ void add_process_noise(Track& t, const LayerConst& L, int model, float mass2) {
-    const float pt2 = t.px * t.px + t.py * t.py, pz = t.pz;
-    const float ipt = rsqrt_fast(pt2);
-    const float p2 = pt2 + pz * pz;
-    const float ms = layer_ms(L, model, (t.eax * t.px + t.eay * t.py) * ipt, p2, ipt);
-    const float ip2 = rcp_fast(p2);
-    const float th2 = ms * (p2 + mass2) * ip2 * ip2;
-    const float qc = th2 * p2 * ipt;
+template <class F>
+__device__ __forceinline__ void add_process_noise(TrackT<F>& t, const LayerConst& L, int model, float mass2) {
+    const F pt2 = t.px * t.px + t.py * t.py, pz = t.pz;
+    const F ipt = rsqrt_fast(pt2);
+    const F p2 = pt2 + pz * pz;
+    const F ms = model == 0 ? F(L.ms) : layer_ms<F>(L, model, (t.eax * t.px + t.eay * t.py) * ipt, p2, ipt);
+    const F ip2 = rcp_fast(p2);
+    const F th2 = ms * (p2 + mass2) * ip2 * ip2;
+    const F qc = th2 * p2 * ipt;
     t.c33 += th2 * pz * pz;
     t.c35 -= qc * pz;
     t.c44 += th2 * p2;
@@ -373,9 +376,10 @@ __device__ __forceinline__ void add_process_noise(Track& t, const LayerConst& L,
 // The track as it stands, dressed as a "crossing" with zero path length, so that kalman_update can be
 // applied without a propagation (first step of the backward refit: the state already stands on the
 // layer; its covariance is radially null in the frame (eax, eay) it carries).
-__device__ __forceinline__ void crossing_in_place(const Track& t, Crossing& o, PropCov& n) {
-    const float pt2 = t.px * t.px + t.py * t.py;
-    const float ipt = rsqrt_fast(pt2);
+template <class F>
+__device__ __forceinline__ void crossing_in_place(const TrackT<F>& t, CrossingT<F>& o, PropCovT<F>& n) {
+    const F pt2 = t.px * t.px + t.py * t.py;
+    const F ipt = rsqrt_fast(pt2);
     o.xn = t.x; o.yn = t.y; o.zn = t.z; o.pxn = t.px; o.pyn = t.py;
     o.erx = t.eax; o.ery = t.eay; o.elx = t.px * ipt; o.ely = t.py * ipt;
     o.T = t.pz * ipt; o.pt2 = pt2; o.ipt = ipt;
@@ -384,7 +388,8 @@ __device__ __forceinline__ void crossing_in_place(const Track& t, Crossing& o, P
     n.n33 = t.c33; n.n34 = t.c34; n.n35 = t.c35; n.n44 = t.c44; n.n45 = t.c45; n.n55 = t.c55;
 }
 
-__device__ __forceinline__ void scale_cov(Track& t, float f) {
+template <class F>
+__device__ __forceinline__ void scale_cov(TrackT<F>& t, float f) {
     t.c11 *= f; t.c12 *= f; t.c13 *= f; t.c14 *= f; t.c15 *= f;
     t.c22 *= f; t.c23 *= f; t.c24 *= f; t.c25 *= f;
     t.c33 *= f; t.c34 *= f; t.c35 *= f; t.c44 *= f; t.c45 *= f; t.c55 *= f;
@@ -542,6 +547,32 @@ kalman_update(TrackT<F>& t, const CrossingT<F>& o, const PropCovT<F>& n, const L
     const F iptn = rsqrt_fast(ar * ar + d4 * d4);
     reaim_momentum<true>(t, ar * iptn, -d4 * iptn, o.T, pzu * iptn);
     return select_u(pd, 0u, 0u);
+}
+
+// One step of the backward refit (reading A18) for the layer with constants L: the first step updates in place,
+// every later one adds the noise of the scatterer just left (Lprev), propagates inward and updates.  Returns 0
+// and the chi2 increment, or the status bits of the failure with the track as it was (layer skipped).
+// Pair form: both tracks take the step or neither does.
+template <bool BOUNDED, class F>
+__device__ __forceinline__ typename num_traits<F>::status
+refit_step(TrackT<F>& t, arg<F> k, arg<F> ik, const LayerConst& L, const LayerConst& Lprev, int model, float mass2,
+           bool first, arg<F> mx, arg<F> my, arg<F> mz, arg<F> vxx, arg<F> vxy, arg<F> vxz, arg<F> vyy, arg<F> vyz,
+           arg<F> vzz, F* dchi2) {
+    CrossingT<F> o;
+    PropCovT<F> n;
+    const F k33 = t.c33, k35 = t.c35, k44 = t.c44, k55 = t.c55;
+    if (first) crossing_in_place(t, o, n);
+    else {
+        const auto reached = reach_layer<true, BOUNDED>(t, k, ik, L, o);
+        if (!is_zero(reached)) return reached;
+        add_process_noise(t, Lprev, model, mass2);      // the scatterer just left behind
+        transport_cov<true>(t, o, F(0.0f), mass2, n);
+    }
+    LocalHitT<F> h;
+    hit_to_local(o, mx, my, mz, vxx, vxy, vxz, vyy, vyz, vzz, h);
+    const auto rc = kalman_update(t, o, n, h, dchi2);
+    if (!is_zero(rc)) { t.c33 = k33; t.c35 = k35; t.c44 = k44; t.c55 = k55; }   // layer skipped
+    return rc;
 }
 
 // Keep the propagated state (no hit used): position frame = arrival frame, momentum frame

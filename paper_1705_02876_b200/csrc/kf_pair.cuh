@@ -126,6 +126,9 @@ __device__ __forceinline__ uint32_t select_u(bool m, uint32_t a, uint32_t b) { r
 __device__ __forceinline__ u2 select_u(mask2 m, uint32_t a, uint32_t b) { return {m.x ? a : b, m.y ? a : b}; }
 __device__ __forceinline__ u2 select_u(mask2 m, uint32_t a, u2 b) { return {m.x ? a : b.x, m.y ? a : b.y}; }
 
+__device__ __forceinline__ bool is_zero(uint32_t a) { return a == 0u; }
+__device__ __forceinline__ bool is_zero(u2 a) { return (a.x | a.y) == 0u; }
+
 // number-type traits: the mask and status types that go with F
 template <class F> struct num_traits;
 template <> struct num_traits<float> { using mask = bool; using status = uint32_t; };

@@ -76,3 +76,36 @@ def test_smooth_ragged_masks_and_flags(ctx):
     compare_fit(g, oo, float(b.radius[-1]), max_diverged_frac=0.05)
     assert np.array_equal(sg["par"][:, :31], b.par[:, :31]) and np.array_equal(sg["cov"][:, :31], b.cov[:, :31])
     assert np.all(sg["chi2"][:31] == 0)
+
+
+def test_smooth_pair_kernel_edge_cases(ctx):
+    """Batches of >= 151 552 tracks take the two-tracks-per-thread kernel, also for fit + smoother; pairs whose
+    tracks used different layers (or where one fails) go through the one-track refit step."""
+    cfg = W.get_config(1)
+    b = W.concat_batches([W.simulate_event(cfg, 50 + e) for e in range(8)] + [W.simulate_event(cfg, 58, n_tracks=3)])
+    assert b.n == 160_003
+    rng = np.random.default_rng(5)
+    holes = rng.random(b.n) < 0.1
+    b.mask = np.where(holes, (rng.integers(0, 1 << 10, size=b.n) | 0b111), b.mask).astype(np.uint32)
+    b.mask[:30] = 0                       # nothing to fit: input comes back in both results
+    b.mask[31:60:2] = 0b0000011111        # odd tracks stop early, their partners go on
+    b.q[100] = 0                          # bad charge
+    b.hpos[4, 1, 201] = np.nan            # NONFINITE on layer 4 of track 201: skipped forward, so never revisited
+    b.mask[200] = b.mask[201] = 0x3ff
+    d, o = _both(ctx, b)
+    g, sg = d.results(), d.smoothed_results()
+    assert np.array_equal(g["status"], o["status"]) and np.array_equal(g["nhits"], o["nhits"])
+    assert np.array_equal(sg["status"], o["sstatus"]), np.flatnonzero(sg["status"] != o["sstatus"])[:10]
+    assert o["status"][201] == 4 and o["sstatus"][201] == 0 and o["nhits"][201] == 9 and o["status"][100] == 8
+    untouched = (o["nhits"] == 0)
+    assert untouched.sum() >= 31
+    assert np.array_equal(sg["par"][:, untouched], b.par[:, untouched]) and np.array_equal(sg["cov"][:, untouched], b.cov[:, untouched])
+    assert np.all(sg["chi2"][untouched] == 0)
+    sel = (o["nhits"] >= 5) & (o["status"] == 0) & (o["sstatus"] == 0)
+    fwd = compare_fit({k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in g},
+                      dict(par=o["par"][:, sel], cov=o["cov"][sel], chi2=o["chi2"][sel], nhits=o["nhits"][sel], status=o["status"][sel]),
+                      float(b.radius[-1]), max_diverged_frac=0.02)
+    sm = compare_fit(dict(par=sg["par"][:, sel], cov=sg["cov"][:, sel], chi2=sg["chi2"][sel], nhits=o["nhits"][sel], status=o["sstatus"][sel]),
+                     dict(par=o["spar"][:, sel], cov=o["scov"][sel], chi2=o["schi2"][sel], nhits=o["nhits"][sel], status=o["sstatus"][sel]),
+                     float(b.radius[-1]), max_diverged_frac=0.02)
+    print(f"pair smoother: forward {fwd}\n               smoothed {sm}")

@@ -147,3 +147,18 @@ def test_S4_smoothed_pulls_and_gain_over_forward_filter():
     rel = np.sqrt(Cs[:, 3, 3] + Cs[:, 4, 4] + Cs[:, 5, 5]) / pabs
     assert np.median(rel) < 0.05
     assert np.median(np.abs(np.linalg.norm(d[3:], axis=0)) / pabs) < 0.05
+
+
+def test_S5_nothing_fitted_comes_back_untouched():
+    """A track the forward fit cannot start (bad charge, empty mask) has no backward pass: both results are the
+    input, chi2 0, smoothed status 0 -- independently of what memory the call happens to get for its private trace."""
+    b = W.simulate_event(W.get_config(1), 3, n_tracks=64)
+    b.q[5] = 0
+    b.mask[9] = 0
+    for _ in range(3):                       # repeated: an uninitialised read would not be stable
+        r = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
+        assert r["status"][5] == O.BAD_CHARGE and r["sstatus"][5] == 0 and r["status"][9] == 0 and r["sstatus"][9] == 0
+        for i in (5, 9):
+            np.testing.assert_array_equal(r["spar"][:, i], b.par[:, i].astype(np.float64))
+            np.testing.assert_array_equal(O.pack_cov21(r["scov"][i:i + 1])[:, 0], b.cov[:, i].astype(np.float64))
+            assert r["schi2"][i] == 0 and r["nhits"][i] == 0

@@ -338,8 +338,10 @@ constexpr int kPairWarps = kPairBlock / 32;
 constexpr int kPairTile = 64;                      // tracks per warp
 constexpr int kHit2Floats = 9 * kPairTile;
 constexpr int kSeed2Floats = 27 * kPairTile;
-constexpr int kWarp2Floats = kStages * kHit2Floats + kSeed2Floats;
-constexpr int kSmem2Bytes = kPairWarps * kWarp2Floats * 4 + kPairWarps * (kStages + 1) * 8;
+constexpr int kPark2Floats = 30 * 32;              // one parked track (29 values + chi2) per lane (ragged pairs)
+// (the smoother kernel has no park area: it spills a little and wants the shared-memory space as L1)
+__host__ __device__ constexpr int warp2_floats(bool smooth) { return kStages * kHit2Floats + kSeed2Floats + (smooth ? 0 : kPark2Floats); }
+constexpr int smem2_bytes(bool smooth) { return kPairWarps * warp2_floats(smooth) * 4 + kPairWarps * (kStages + 1) * 8; }
 
 struct Hit2 {
     f2 x, y, z, vxx, vxy, vxz, vyy, vyz, vzz;
@@ -374,11 +376,29 @@ __device__ __forceinline__ bool fit_layer_pair(Track2& t, f2 k, f2 ik, const Lay
     return true;
 }
 
-// Slow path (a layer only one track of the pair has a hit on, or a failure in the pair): component c alone,
-// through the one-track arithmetic.  Kept out of line so that it costs the pair path no registers.
+// A layer only ONE track of the pair has a hit on: the idle one's 29 values (and its chi2) are parked in shared
+// memory, its slot of the hit stage is overwritten with a harmless hit (origin, unit covariance) so that its
+// arithmetic passes, the pair arithmetic runs for both, and the idle half is put back.
 #define KF_TRACK_FIELDS(X)                                                                              \
     X(x) X(y) X(z) X(px) X(py) X(pz) X(eax) X(eay) X(c00) X(c01) X(c02) X(c03) X(c04) X(c05) X(c11) X(c12) \
     X(c13) X(c14) X(c15) X(c22) X(c23) X(c24) X(c25) X(c33) X(c34) X(c35) X(c44) X(c45) X(c55)
+template <int C>
+__device__ __forceinline__ void park_component(const Track2& t, float* scr) {
+    int r = 0;
+#define KF_PARK(f) scr[32 * r++] = C ? t.f.v.y : t.f.v.x;
+    KF_TRACK_FIELDS(KF_PARK)
+#undef KF_PARK
+}
+template <int C>
+__device__ __forceinline__ void unpark_component(Track2& t, const float* scr) {
+    int r = 0;
+#define KF_UNPARK(f) { const float v = scr[32 * r++]; if (C) t.f.v.y = v; else t.f.v.x = v; }
+    KF_TRACK_FIELDS(KF_UNPARK)
+#undef KF_UNPARK
+}
+
+// Slow path (a track of the pair fails on the layer): component c alone,
+// through the one-track arithmetic.  Kept out of line so that it costs the pair path no registers.
 __device__ __noinline__ uint32_t fit_layer_one_of_pair(Track2& t, int c, float k, float ik, const LayerConst& L,
                                                        float mass2, const Hit2& m, f2& chi2, bool started) {
     Track ts;
@@ -456,8 +476,10 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
     const int64_t i0 = ((int64_t)blockIdx.x * kPairWarps + wid) * kPairTile;  // first track of this warp
     if (i0 >= a.n) return;
     const int L = P.n_layers;
+    constexpr int kWarp2Floats = warp2_floats(SMOOTH);
     float* wbase = reinterpret_cast<float*>(smem_raw) + wid * kWarp2Floats;
     float* seed_tile = wbase + kStages * kHit2Floats;
+    float* park = seed_tile + kSeed2Floats + lane;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + kPairWarps * kWarp2Floats * 4) + wid * (kStages + 1);
     const uint32_t hit0 = smem_u32(wbase), seed0 = smem_u32(seed_tile), bar0 = smem_u32(bars);
     const int col = (int)i0;
@@ -514,15 +536,34 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
         const float2* tp = reinterpret_cast<const float2*>(wbase + s * kHit2Floats) + lane;
         const mask2 want = {live.x && ((mx >> l) & 1u), live.y && ((my >> l) & 1u)};
         bool both = false;
-        if (all_of(want)) {
+        // (the smoother kernel, at the edge of its register budget, leaves ragged pairs to the one-track path)
+        if (SMOOTH ? all_of(want) : !none_of(want)) {
+            const bool ragged = !SMOOTH && !all_of(want);
+            const int idle = want.x ? 1 : 0;
+            if constexpr (!SMOOTH) {
+                if (ragged) {
+                    if (idle) park_component<1>(t, park); else park_component<0>(t, park);
+                    park[29 * 32] = idle ? chi2.v.y : chi2.v.x;
+                    float* hp = const_cast<float*>(reinterpret_cast<const float*>(tp)) + idle;   // this lane's own slot
+#pragma unroll
+                    for (int r = 0; r < 9; ++r) hp[r * kPairTile] = (r == 3 || r == 6 || r == 8) ? 1.0f : 0.0f;
+                    // ordered before the TMA refill of this stage (issued by another lane after the __syncwarp below)
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                }
+            }
             // (the general transport is also right for a track whose radial row is already zero)
-            if (all_of(started)) both = fit_layer_pair<true>(t, k, ik, P.layer[l], P.mass2, tp, chi2);
+            if (all_of(started | !want)) both = fit_layer_pair<true>(t, k, ik, P.layer[l], P.mass2, tp, chi2);
             else both = fit_layer_pair<false>(t, k, ik, P.layer[l], P.mass2, tp, chi2);
+            if constexpr (!SMOOTH) {
+                if (ragged) {
+                    if (idle) { unpark_component<1>(t, park); chi2.v.y = park[29 * 32]; }
+                    else { unpark_component<0>(t, park); chi2.v.x = park[29 * 32]; }
+                }
+            }
         }
         if (both) {
-            nhx += 1; nhy += 1;
-            started.x = true; started.y = true;
-            usedx |= 1u << l; usedy |= 1u << l;
+            if (want.x) { nhx += 1; started.x = true; usedx |= 1u << l; }
+            if (want.y) { nhy += 1; started.y = true; usedy |= 1u << l; }
         } else if (!none_of(want)) {
             // copies whose address may be taken: the pair itself stays in registers
             Track2 tc = t;
@@ -801,8 +842,8 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     FitMaps M;
     if (P.geometry_options == 0 && a.n >= (int64_t)KF_PAIR_MIN_TRACKS && (!smooth || KF_PAIR_SMOOTH)) {   // two tracks per thread
         static const cudaError_t attr_pair = [] {
-            cudaError_t e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem2Bytes);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem2Bytes);
+            cudaError_t e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));
             return e;
         }();
         if (attr_pair != cudaSuccess) return attr_pair;
@@ -816,8 +857,8 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
             return cudaErrorInvalidValue;
         const int64_t per_block = (int64_t)kPairWarps * kPairTile;
         const int64_t blocks = (a.n + per_block - 1) / per_block;
-        if (smooth) fit_pair_kernel<true><<<(unsigned)blocks, kPairBlock, kSmem2Bytes, stream>>>(P, M, a);
-        else fit_pair_kernel<false><<<(unsigned)blocks, kPairBlock, kSmem2Bytes, stream>>>(P, M, a);
+        if (smooth) fit_pair_kernel<true><<<(unsigned)blocks, kPairBlock, smem2_bytes(true), stream>>>(P, M, a);
+        else fit_pair_kernel<false><<<(unsigned)blocks, kPairBlock, smem2_bytes(false), stream>>>(P, M, a);
         return cudaGetLastError();
     }
     if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3) ||

@@ -294,7 +294,15 @@ def run_ours(args) -> None:
     d2h = n * (27 * 4 + 12)
     e2e = {"value": n_all * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
            "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "kf_fit_tracks_host, pinned host SoA buffers"}
-    same = all(np.array_equal(a, b) for a, b in zip(d.results().values(), h.results().values()))
+    # the host path fits chunks with the one-track kernel, the resident path uses the pair kernel: same arithmetic,
+    # different instruction selection, so the two agree to rounding, not bit for bit
+    host_vs_dev, h_res = {}, h.results()
+    for key, a in d.results().items():
+        b = h_res[key]
+        if np.issubdtype(a.dtype, np.floating):
+            host_vs_dev[key + "_max_abs_diff_over_max_abs"] = float(np.max(np.abs(a.astype(np.float64) - b)) / max(np.max(np.abs(a)), 1e-30))
+        else:
+            host_vs_dev[key + "_equal"] = bool(np.array_equal(a, b))
     fp32_peak = ctx.measure_fp32_peak(5) if rank == 0 else 0.0
     building = measure_building(ctx, dev) if (rank == 0 and not args.no_building) else None
     ctx.set_stream(stream)          # measure_building borrowed the context for torch's current stream
@@ -405,7 +413,7 @@ def run_ours(args) -> None:
                           "tracks_per_gpu": n, "n_layers": L, "parallelism": f"events sharded over {ws} GPU(s), no collective",
                           "l2": "inputs+outputs (%.2f GB) larger than the 126 MB L2, no flush" % (alg_bytes / 1e9)},
                "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "roofline_other": other,
-               "cpu_baseline": cpu, "host_path_equals_device_path": bool(same)}
+               "cpu_baseline": cpu, "host_path_vs_device_path": host_vs_dev}
         if building is not None:
             building["alu_roofline_frac"] = building["algorithmic_gflop"] * 1e9 / (building["build_ms"] * 1e-3) / (fp32_peak * 1e12)
             out["building"] = building

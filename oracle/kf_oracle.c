@@ -6,7 +6,7 @@
  * (arXiv:1705.02876; "seeding, building, fitting" + chi2; PAPER.md:65 6x6 track /
  * 3x3 hit matrices in global coordinates; PAPER.md:71 projective bins; PAPER.md:73 best hit =
  * lowest chi2 increment; equations: BASELINE.json:north_star).  The paper prints no formulas;
- * every formula below is a reading listed in DESIGN.md ("Readings A1..A17").
+ * every formula below is a reading listed in DESIGN.md ("Readings A1..A21").
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load this.  It shares no code, header, table or constant with the CUDA path
@@ -18,7 +18,8 @@
  * Pins (tests/test_oracle_pins.py, tests/test_oracle_smoother.py): P1 exact helix recovery, P2 propagation invariants + RK4 +
  * worked value, P3 Jacobian vs finite differences / radial null / |p| conservation, P4 EKF ==
  * batch weighted least squares, P5 covariance PSD rank 5, P6 pulls and chi2/ndf, P7 Highland
- * check values, P8 window scoring == brute force, P9 bin structure, P10 rotation symmetry.
+ * check values, P8 window scoring == brute force, P9 bin structure, P10 rotation symmetry;
+ * G1-G3 geometry options (tests/test_oracle_geometry.py); E1-E6 energy loss (tests/test_oracle_energy_loss.py).
  * Parity-unpinned: none of the functions below (efficiency / fake rate of PAPER.md:85 is not
  * computed here at all).
  */
@@ -44,6 +45,9 @@ static double g_half_length[32] = {
     INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY,
     INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY,
     INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY, INFINITY};
+
+static int g_energy_loss = 0; /* reading A21: 0 none, 1 mean Bethe loss in silicon at every layer crossing */
+void orc_set_energy_loss(int model) { g_energy_loss = model; }
 
 static double g_score_half_length = INFINITY; /* the one layer orc_score_layer works on */
 void orc_set_score_half_length(double h) { g_score_half_length = h; }
@@ -173,6 +177,83 @@ void orc_transport_cov(const double F[36], const double C[36], const double Q[36
         }
 }
 
+/* ---- mean energy loss in the layer material (reading A21; PAPER.md:168 defers "more realistic" detector
+ * descriptions; SURVEY 8(f) item 4 names energy loss) -------------------------------------------------------
+ * Bethe's mean stopping power for a heavy charged particle of unit charge (PDG "Passage of particles
+ * through matter"), no density-effect and no shell correction:
+ *   -dE/dx = K (Z/A) (1/beta^2) [ (1/2) ln( 2 me beta^2 gamma^2 Tmax / I^2 ) - beta^2 ]      [GeV cm^2 / g]
+ *   Tmax   = 2 me beta^2 gamma^2 / (1 + 2 gamma me/M + (me/M)^2)
+ * with K = 0.307075 MeV cm^2/mol, me = 0.51099895 MeV.  The layers are silicon: Z/A = 14/28.0855,
+ * I = 173 eV, X0 = 21.82 g/cm^2, so a layer of t radiation lengths is t * 21.82 g/cm^2 thick.
+ * orc_energy_loss returns the energy [GeV] lost over t radiation lengths (t already scaled by the path
+ * length where that applies). */
+#define ORC_BETHE_K 0.307075e-3  /* GeV cm^2 / mol */
+#define ORC_ME 0.51099895e-3     /* GeV */
+#define ORC_SI_Z_OVER_A (14.0 / 28.0855)
+#define ORC_SI_I 173.0e-9        /* GeV */
+#define ORC_SI_X0 21.82          /* g / cm^2 */
+double orc_energy_loss(double p, double mass, double t) {
+    if (t <= 0.0) return 0.0;
+    double E = sqrt(p * p + mass * mass);
+    double beta2 = p * p / (E * E);
+    double gamma = E / mass;
+    double bg2 = beta2 * gamma * gamma;
+    double r = ORC_ME / mass;
+    double Tmax = 2.0 * ORC_ME * bg2 / (1.0 + 2.0 * gamma * r + r * r);
+    double dedx = ORC_BETHE_K * ORC_SI_Z_OVER_A / beta2 *
+                  (0.5 * log(2.0 * ORC_ME * bg2 * Tmax / (ORC_SI_I * ORC_SI_I)) - beta2);
+    return dedx * t * ORC_SI_X0;
+}
+
+/* The effective thickness a state standing on a cylinder sees (A20 path length if that option is on). */
+static double seen_thickness(const double u[6], double t) {
+    if (g_material_model == 1 && t > 0.0) {
+        double p2 = u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+        double cospsi = fabs(u[0] * u[3] + u[1] * u[4]) / (sqrt(u[0] * u[0] + u[1] * u[1]) * sqrt(p2));
+        t = t / cospsi;
+    }
+    return t;
+}
+
+/* Energy-loss step at a layer (reading A21).  direction +1 (forward filter, on arrival, after C' = F C F^T + Q):
+ * E'' = E - dE(p), direction -1 (backward refit, on leaving the layer inward): E'' = E + dE(p), dE evaluated
+ * at the momentum the state HAS (so the backward step inverts the forward one to first order in dE).  The
+ * momentum keeps its direction: p'' = f p, f = |p''|/|p|.  Jacobian with dE held fixed (its own dependence
+ * on p changes d|p''|/d|p| by about dE/p, 1e-3 or less, neglected): d|p''|/d|p| = g = (E''/|p''|)(|p|/E), so
+ *   J = blockdiag(I3, f I3 + (g - f) n n^T), n = p/|p|;   C <- J C J^T.   No straggling term is added.
+ * Returns ORC_PROP_FAIL (nothing written) if the particle would stop (E'' <= mass).  J36 (optional) gets J. */
+int orc_energy_loss_step(double u[6], double C[36], double mass, double t, int direction, double J36[36]) {
+    double p2 = u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+    double p = sqrt(p2), E = sqrt(p2 + mass * mass);
+    double dE = orc_energy_loss(p, mass, seen_thickness(u, t));
+    double E2 = direction > 0 ? E - dE : E + dE;
+    if (!(E2 > mass)) return ORC_PROP_FAIL;
+    double pn = sqrt(E2 * E2 - mass * mass);
+    double f = pn / p, g = (E2 / pn) * (p / E);
+    double J[36], JC[36], out[36];
+    memset(J, 0, sizeof J);
+    for (int i = 0; i < 3; ++i) J[i * 6 + i] = 1.0;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+            J[(3 + i) * 6 + 3 + j] = (i == j ? f : 0.0) + (g - f) * u[3 + i] * u[3 + j] / p2;
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double acc = 0.0;
+            for (int m = 0; m < 6; ++m) acc += J[i * 6 + m] * C[m * 6 + j];
+            JC[i * 6 + j] = acc;
+        }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            double acc = 0.0;
+            for (int m = 0; m < 6; ++m) acc += JC[i * 6 + m] * J[j * 6 + m];
+            out[i * 6 + j] = acc;
+        }
+    memcpy(C, out, sizeof out);
+    for (int i = 3; i < 6; ++i) u[i] *= f;
+    if (J36) memcpy(J36, J, sizeof J);
+    return 0;
+}
+
 /* inverse of a symmetric 3x3 by cofactors; returns det */
 static double inv3(const double S[9], double Si[9]) {
     double c00 = S[4] * S[8] - S[5] * S[7];
@@ -285,6 +366,8 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
             if (rc) { st |= (uint32_t)rc; continue; }
             orc_process_noise(up, mass, xX0[l], Q);
             orc_transport_cov(F, C, Q, Cp);
+            if (g_energy_loss) rc = orc_energy_loss_step(up, Cp, mass, xX0[l], +1, NULL); /* A21 */
+            if (rc) { st |= (uint32_t)rc; continue; }
             rc = orc_update(up, Cp, hpos + 3 * l, hcov + 9 * l, un, Cn, &dchi2);
             if (rc) { st |= (uint32_t)rc; continue; }
             memcpy(u, un, sizeof u);
@@ -344,10 +427,14 @@ static void refit_inward_one(int L, const double *radius, const double *xX0, dou
             memset(F, 0, sizeof F);
             for (int i = 0; i < 6; ++i) F[i * 6 + i] = 1.0;
         } else {
-            double Cq[36], Z[36];
-            orc_process_noise(u, mass, xX0[prev], Q);
-            for (int i = 0; i < 36; ++i) Cq[i] = C[i] + Q[i];
-            rc = propagate_dir(u, (double)q, Bz, radius[l], 1, up, F, NULL, NULL);
+            double Cq[36], Z[36], ub[6];
+            memcpy(ub, u, sizeof ub);
+            memcpy(Cq, C, sizeof Cq);
+            /* A21: the layer just left gives back the energy it took (before its scattering noise is added) */
+            if (g_energy_loss && orc_energy_loss_step(ub, Cq, mass, xX0[prev], -1, NULL)) { st |= ORC_PROP_FAIL; continue; }
+            orc_process_noise(ub, mass, xX0[prev], Q);
+            for (int i = 0; i < 36; ++i) Cq[i] += Q[i];
+            rc = propagate_dir(ub, (double)q, Bz, radius[l], 1, up, F, NULL, NULL);
             if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
             if (rc) { st |= (uint32_t)rc; continue; }
             memset(Z, 0, sizeof Z);
@@ -574,6 +661,7 @@ void orc_score_layer(int64_t n, double r_layer, double xX0, double Bz, double ma
         if (rc) { status[i] |= (uint32_t)rc; continue; }
         orc_process_noise(up, mass, xX0, Q);
         orc_transport_cov(F, C, Q, Cp);
+        if (g_energy_loss && orc_energy_loss_step(up, Cp, mass, xX0, +1, NULL)) { status[i] |= ORC_PROP_FAIL; continue; } /* A21 */
         double best = INFINITY, second = INFINITY;
         int32_t bh = -1;
         if (all_hits) {
@@ -695,14 +783,17 @@ void orc_build_combinatorial(int64_t n_seeds, int n_layers_total, int first_laye
                 double up[6], F[36], Q[36], Cp[36];
                 int rc = orc_propagate(cur[p].u, (double)qq, Bz, radius[l], up, F, NULL, NULL);
                 if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
+                if (!rc) {
+                    orc_process_noise(up, mass, xX0[l], Q);
+                    orc_transport_cov(F, cur[p].C, Q, Cp);
+                    if (g_energy_loss) rc = orc_energy_loss_step(up, Cp, mass, xX0[l], +1, NULL); /* A21 */
+                }
 #define ORC_ROOM() do { if (nch + 2 > cap) { cap *= 2; ch = (orc_child *)realloc(ch, sizeof(orc_child) * cap); } } while (0)
                 ORC_ROOM();
                 if (rc) { /* cannot reach the layer: survives unchanged */
                     ch[nch].c = cur[p]; ch[nch].c.status |= (uint32_t)rc; ch[nch].parent = p; ch[nch].hit = -1; ++nch;
                     continue;
                 }
-                orc_process_noise(up, mass, xX0[l], Q);
-                orc_transport_cov(F, cur[p].C, Q, Cp);
                 /* the "no hit" child */
                 ch[nch].c = cur[p];
                 memcpy(ch[nch].c.u, up, sizeof up); memcpy(ch[nch].c.C, Cp, sizeof Cp);

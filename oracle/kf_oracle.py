@@ -62,6 +62,12 @@ def lib():
         _lib.orc_set_geometry_options.argtypes = [C.c_int, C.c_int, dp]
         _lib.orc_set_score_half_length.restype = None
         _lib.orc_set_score_half_length.argtypes = [C.c_double]
+        _lib.orc_set_energy_loss.restype = None
+        _lib.orc_set_energy_loss.argtypes = [C.c_int]
+        _lib.orc_energy_loss.restype = C.c_double
+        _lib.orc_energy_loss.argtypes = [C.c_double] * 3
+        _lib.orc_energy_loss_step.restype = C.c_int
+        _lib.orc_energy_loss_step.argtypes = [dp, dp, C.c_double, C.c_double, C.c_int, dp]
         _lib.orc_build_combinatorial.restype = None
     return _lib
 
@@ -69,16 +75,20 @@ def lib():
 class geometry_options:
     """Context manager for the oracle's process-wide geometry options (reading A20):
     material_model 0 = flat thickness (A5), 1 = thickness / cos(incidence); half_length[l] = half length of
-    barrel layer l in cm (None = infinite, A12).  Restores the defaults on exit."""
+    barrel layer l in cm (None = infinite, A12); energy_loss 1 = mean Bethe loss in silicon at every crossing
+    (reading A21).  Restores the defaults on exit."""
 
-    def __init__(self, material_model: int = 0, half_length=None, score_layer: int | None = None):
+    def __init__(self, material_model: int = 0, half_length=None, score_layer: int | None = None,
+                 energy_loss: int = 0):
         self.model = int(material_model)
+        self.eloss = int(energy_loss)
         self.hl = None if half_length is None else np.ascontiguousarray(half_length, dtype=np.float64)
         self.score_layer = score_layer
 
     def __enter__(self):
         n = 0 if self.hl is None else len(self.hl)
         lib().orc_set_geometry_options(self.model, n, _p(self.hl))
+        lib().orc_set_energy_loss(self.eloss)
         if self.hl is not None and self.score_layer is not None:
             lib().orc_set_score_half_length(float(self.hl[self.score_layer]))
         return self
@@ -88,6 +98,7 @@ class geometry_options:
 
     def __exit__(self, *a):
         lib().orc_set_geometry_options(0, 0, None)
+        lib().orc_set_energy_loss(0)
         lib().orc_set_score_half_length(float("inf"))
 
 
@@ -124,6 +135,20 @@ def unpack_cov6(v6: np.ndarray) -> np.ndarray:
 # ------------------------------------------------------------------ scalar-level entry points
 def theta0(p, mass, t):
     return lib().orc_theta0(float(p), float(mass), float(t))
+
+
+def energy_loss(p, mass, t):
+    """Mean Bethe energy loss [GeV] in t radiation lengths of silicon (reading A21)."""
+    return lib().orc_energy_loss(float(p), float(mass), float(t))
+
+
+def energy_loss_step(u, Cm, mass, t, direction):
+    """Reading A21 at one layer: -> (status, u_out[6], C_out[6,6], J[6,6]); direction +1 loses, -1 regains."""
+    u = np.array(u, dtype=np.float64)
+    Cm = np.array(Cm, dtype=np.float64).reshape(36)
+    J = np.zeros(36)
+    rc = lib().orc_energy_loss_step(_p(u), _p(Cm), float(mass), float(t), int(direction), _p(J))
+    return rc, u, Cm.reshape(6, 6), J.reshape(6, 6)
 
 
 def propagate(u, q, Bz, r, want_F=True):

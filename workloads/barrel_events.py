@@ -55,6 +55,7 @@ class BarrelConfig:
     first_scored_layer: int = 3
     material_model: int = 0        # DESIGN.md reading A20: 1 = thickness / cos(incidence)
     half_length_cm: float = float("inf")   # A20: finite barrel (same half length for every layer)
+    energy_loss: int = 0           # DESIGN.md reading A21: 1 = mean energy loss in silicon after every hit
 
     @property
     def radii(self) -> np.ndarray:
@@ -93,6 +94,7 @@ class FitBatch:
     truth_vertex: np.ndarray = field(repr=False, default=None)  # [6][n] f64
     material_model: int = 0                # DESIGN.md reading A20 (geometry options of the fit)
     half_length: np.ndarray = None         # [L] f32 barrel half lengths, None = unbounded
+    energy_loss: int = 0                   # DESIGN.md reading A21
 
     @property
     def n_layers(self) -> int:
@@ -106,6 +108,18 @@ def highland_theta0(p: np.ndarray, mass: float, t) -> np.ndarray:
         return np.zeros_like(p)
     beta = p / np.sqrt(p * p + mass * mass)
     return 0.0136 / (beta * p) * np.sqrt(t) * (1.0 + 0.038 * np.log(t))
+
+
+def silicon_mean_energy_loss(p: np.ndarray, mass: float, t) -> np.ndarray:
+    """Mean energy [GeV] a unit-charge particle of momentum p loses in t radiation lengths of silicon
+    (simulation side of reading A21): PDG mean stopping power without density correction,
+    S = K (Z/A) / beta^2 * [ln(2 me (beta gamma)^2 / I) - ln(1 + 2 gamma me/M + (me/M)^2) / 2 - beta^2]."""
+    K, me, I = 0.307075e-3, 0.51099895e-3, 173.0e-9          # GeV cm^2/mol, GeV, GeV
+    bg2 = (p / mass) ** 2
+    gam = np.sqrt(1.0 + bg2)
+    b2 = bg2 / (1.0 + bg2)
+    bracket = np.log(2.0 * me * bg2 / I) - 0.5 * np.log1p(2.0 * gam * me / mass + (me / mass) ** 2) - b2
+    return K * (14.0 / 28.0855) / b2 * bracket * (np.asarray(t, dtype=np.float64) * 21.82)
 
 
 def _cross_cylinder(pos, mom, q, Bz, r):
@@ -217,6 +231,13 @@ def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
             d = tuple(ph[i] + t1 * e1[i] + t2 * e2[i] for i in range(3))
             dn = np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)
             mom = tuple(np.where(alive, p * d[i] / dn, mom[i]) for i in range(3))
+            if cfg.energy_loss == 1:                                  # A21: mean loss, direction kept
+                E = np.sqrt(p * p + M_PION * M_PION)
+                E2 = E - np.where(inside, silicon_mean_energy_loss(p, M_PION, t_eff), 0.0)
+                stopped = E2 <= M_PION
+                alive &= ~stopped
+                scale = np.sqrt(np.maximum(E2 * E2 - M_PION * M_PION, 0.0)) / p
+                mom = tuple(np.where(alive, mom[i] * scale, mom[i]) for i in range(3))
         truth[l] = np.where(alive, np.stack(pos + mom), np.nan)
 
     # seed (A13)
@@ -241,7 +262,8 @@ def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
         q=q.astype(np.int8), hpos=np.ascontiguousarray(hpos, dtype=f32),
         hcov=np.ascontiguousarray(hcov, dtype=f32), mask=mask, truth=truth, truth_vertex=truth_vertex,
         material_model=cfg.material_model,
-        half_length=None if math.isinf(cfg.half_length_cm) else np.full(L, cfg.half_length_cm, dtype=f32))
+        half_length=None if math.isinf(cfg.half_length_cm) else np.full(L, cfg.half_length_cm, dtype=f32),
+        energy_loss=cfg.energy_loss)
 
 
 def concat_batches(batches: list[FitBatch]) -> FitBatch:
@@ -251,7 +273,7 @@ def concat_batches(batches: list[FitBatch]) -> FitBatch:
                     mass=b0.mass, par=cat("par", 1), cov=cat("cov", 1), q=cat("q", 0),
                     hpos=cat("hpos", 2), hcov=cat("hcov", 2), mask=cat("mask", 0),
                     truth=cat("truth", 2), truth_vertex=cat("truth_vertex", 1),
-                    material_model=b0.material_model, half_length=b0.half_length)
+                    material_model=b0.material_model, half_length=b0.half_length, energy_loss=b0.energy_loss)
 
 
 def make_fit_batch(config: int, n_events: int | None = None, n_tracks: int | None = None) -> FitBatch:

@@ -116,6 +116,14 @@ typedef struct {
     int material_model;       /* 0: thickness x_over_X0 as given.  1: path length through the layer,
                                  x_over_X0 / cos(psi), psi = angle between the propagated momentum and
                                  the cylinder normal at the crossing (in Highland's sqrt AND log term) */
+    int energy_loss_model;    /* DESIGN.md reading A21.  0: none.  1: at every layer crossing the track loses
+                                 the mean Bethe energy loss of a unit-charge particle of mass_gev in
+                                 x_over_X0 radiation lengths of SILICON (Z/A = 14/28.0855, I = 173 eV,
+                                 X0 = 21.82 g/cm^2; no density correction, no straggling), over the path
+                                 length if material_model = 1; the momentum keeps its direction, the
+                                 covariance is transported with dE held fixed; the backward refit gives
+                                 the energy back.  A track that would stop fails that layer
+                                 (KF_STATUS_PROP_FAIL).  Needs mass_gev > 0.                            */
 } kf_geometry;
 
 /* ---- tracks (seeds in, fitted tracks out; candidates in/out) ------------------------------------ */

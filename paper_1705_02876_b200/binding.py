@@ -35,7 +35,8 @@ class KFError(RuntimeError):
 class _Geometry(C.Structure):
     _fields_ = [("n_layers", C.c_int), ("radius_cm", C.POINTER(C.c_float)), ("x_over_X0", C.POINTER(C.c_float)),
                 ("Bz_tesla", C.c_float), ("mass_gev", C.c_float),
-                ("half_length_cm", C.POINTER(C.c_float)), ("material_model", C.c_int)]
+                ("half_length_cm", C.POINTER(C.c_float)), ("material_model", C.c_int),
+                ("energy_loss_model", C.c_int)]
 
 
 class _Tracks(C.Structure):
@@ -147,6 +148,7 @@ class Geometry:
     mass_gev: float
     half_length_cm: np.ndarray | None = None   # reading A20: barrel half lengths, None = unbounded
     material_model: int = 0                    # reading A20: 1 = thickness / cos(incidence angle)
+    energy_loss_model: int = 0                 # reading A21: 1 = mean Bethe loss in silicon at every crossing
 
     def _c(self):
         r = np.ascontiguousarray(self.radius_cm, dtype=np.float32)
@@ -156,7 +158,8 @@ class Geometry:
             raise ValueError("half_length_cm must have one entry per layer")
         hp = C.POINTER(C.c_float)() if h is None else h.ctypes.data_as(C.POINTER(C.c_float))
         g = _Geometry(int(r.shape[0]), r.ctypes.data_as(C.POINTER(C.c_float)), t.ctypes.data_as(C.POINTER(C.c_float)),
-                      float(self.Bz_tesla), float(self.mass_gev), hp, int(self.material_model))
+                      float(self.Bz_tesla), float(self.mass_gev), hp, int(self.material_model),
+                      int(self.energy_loss_model))
         return g, (r, t, h)       # keep the arrays alive while g is in use
 
 

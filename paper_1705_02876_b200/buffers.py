@@ -51,7 +51,7 @@ class DeviceFit:
         ld = padded_ld(n)
         geom = Geometry(np.asarray(batch.radius, dtype=np.float32), np.asarray(batch.x_over_X0, dtype=np.float32),
                         float(batch.Bz), float(batch.mass), getattr(batch, "half_length", None),
-                        int(getattr(batch, "material_model", 0)))
+                        int(getattr(batch, "material_model", 0)), int(getattr(batch, "energy_loss", 0)))
         dev = device
         mk = lambda shape, dt: torch.zeros(shape, dtype=dt, device=dev, pin_memory=(pin and str(dev) == "cpu"))
         return DeviceFit(

@@ -26,7 +26,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 8;
+constexpr int kAbiVersion = 9;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -73,8 +73,21 @@ int make_params(const kf_geometry* g, FitParams* P) {
         P->layer[l].half_len = hl;
     }
     if (g->material_model != 0 && g->material_model != 1) return KF_ERR_UNSUPPORTED;
-    P->material_model = g->material_model;
-    P->geometry_options = g->material_model != 0;
+    if (g->energy_loss_model != 0 && g->energy_loss_model != 1) return KF_ERR_UNSUPPORTED;
+    P->model = (g->material_model ? (int)MODEL_PATH_LENGTH : 0) | (g->energy_loss_model ? (int)MODEL_ENERGY_LOSS : 0);
+    if (g->energy_loss_model) {  // reading A21: Bethe, silicon
+        const double m = (double)g->mass_gev, me = 0.51099895e-3, I = 173.0e-9;
+        if (!(m > 0.0)) return KF_ERR_UNSUPPORTED;
+        P->el.a = (float)std::log(2.0 * me / (I * m * m));    // ln(2 me (beta gamma)^2 / I) = a + ln p^2
+        P->el.b = (float)(2.0 * me / (m * m));                // 1 + 2 gamma me/M + (me/M)^2 = c + b E
+        P->el.c = (float)(1.0 + (me / m) * (me / m));
+        P->el.mass = (float)m;
+        for (int l = 0; l < g->n_layers; ++l) {
+            const double t = g->x_over_X0[l];
+            P->layer[l].de0 = t > 0.0 ? (float)(0.307075e-3 * (14.0 / 28.0855) * t * 21.82) : 0.0f;
+        }
+    }
+    P->geometry_options = P->model != 0;
     for (int l = 0; l < g->n_layers; ++l) P->geometry_options |= std::isfinite(P->layer[l].half_len) ? 1 : 0;
     return KF_OK;
 }

@@ -72,8 +72,8 @@ comb_propagate_kernel(const __grid_constant__ FitParams P, const CombArgs a, int
     Track t;
     get_track(a.trk_in, a.ld_s, slot, t);
     const float qf = (float)a.q[sd];
-    const uint32_t rc = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.material_model,
-                                                    P.mass2, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch,
+    const uint32_t rc = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model,
+                                                    P.mass2, P.el, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch,
                                                     a.ld_s, slot);
     if (rc) a.st_in[slot] |= rc;   // its one child (REC_STUCK) inherits the reason
     a.flag[slot] = rc ? FLAG_IDLE : FLAG_AT_LAYER;

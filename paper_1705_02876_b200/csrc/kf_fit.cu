@@ -106,17 +106,29 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int col, in
 // One layer for one track.  Returns 0 or the status bit of the failure (track untouched).
 template <bool RADIAL_NULL, bool GEOM = true>
 __device__ __forceinline__ uint32_t fit_layer(Track& t, float k, float ik, const LayerConst& L, int model,
-                                              float mass2, const Hit& m, float& chi2) {
+                                              float mass2, const Bethe& el, const Hit& m, float& chi2) {
     Crossing o;
     const uint32_t reached = reach_layer<false, GEOM>(t, k, ik, L, o);
     if (reached) return reached;
     PropCov n;
     transport_cov<RADIAL_NULL>(t, o, ms_at_crossing(L, model, o, t.pz), mass2, n);
+    const float pz_in = t.pz;
+    if constexpr (GEOM) {
+        if (model & MODEL_ENERGY_LOSS) {   // reading A21: on arrival, after C' = F C F^T + Q
+            Eloss e;
+            if (!energy_loss_factors(el, L, model, mass2, o.erx * o.elx + o.ery * o.ely, o.pt2, o.ipt, pz_in, false, e))
+                return ST_PROP_FAIL;
+            float pz = pz_in;
+            apply_energy_loss(e, o, n, pz);
+            t.pz = pz;
+        }
+    }
     LocalHit h;
     hit_to_local(o, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
     float d;
     const uint32_t rc = kalman_update(t, o, n, h, &d);
     if (rc == 0u) chi2 += d;
+    else if constexpr (GEOM) t.pz = pz_in;   // layer skipped: the track stays as it was
     return rc;
 }
 
@@ -149,7 +161,7 @@ __device__ __forceinline__ void track_to_tile(const Track& t, float* p) {
 template <bool SMOOTH, bool GEOM>
 __global__ void __launch_bounds__(kFitBlock, SMOOTH ? 4 : KF_FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
-    const int model = GEOM ? P.material_model : 0;
+    const int model = GEOM ? P.model : 0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     const int wid = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform by construction
@@ -208,8 +220,8 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         __syncwarp();        // every lane has issued its reads of this stage
         if (good_q && ((mask >> l) & 1u)) {
             uint32_t rc;
-            if (started) rc = fit_layer<true, GEOM>(t, k, ik, P.layer[l], model, P.mass2, m, chi2);
-            else rc = fit_layer<false, GEOM>(t, k, ik, P.layer[l], model, P.mass2, m, chi2);
+            if (started) rc = fit_layer<true, GEOM>(t, k, ik, P.layer[l], model, P.mass2, P.el, m, chi2);
+            else rc = fit_layer<false, GEOM>(t, k, ik, P.layer[l], model, P.mass2, P.el, m, chi2);
             st |= rc;
             if (rc == 0u) { nh += 1; started = true; used |= 1u << l; }
         }
@@ -264,7 +276,7 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             __syncwarp();
             if ((used >> l) & 1u) {
                 float d;
-                const uint32_t rc = refit_step<GEOM>(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, first,
+                const uint32_t rc = refit_step<GEOM>(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, P.el, first,
                                                      m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, &d);
                 if (rc == 0u) { schi2 += d; nb += 1; first = false; l_prev = l; }
                 else sst |= rc;
@@ -410,8 +422,9 @@ __device__ __noinline__ uint32_t fit_layer_one_of_pair(Track2& t, int c, float k
 #define KF_GETH(f) mh.f = c ? m.f.v.y : m.f.v.x;
     KF_GETH(x) KF_GETH(y) KF_GETH(z) KF_GETH(vxx) KF_GETH(vxy) KF_GETH(vxz) KF_GETH(vyy) KF_GETH(vyz) KF_GETH(vzz)
 #undef KF_GETH
-    const uint32_t rc = started ? fit_layer<true, false>(ts, k, ik, L, 0, mass2, mh, ch)
-                                : fit_layer<false, false>(ts, k, ik, L, 0, mass2, mh, ch);
+    const Bethe none = {0.0f, 0.0f, 0.0f, 0.0f};
+    const uint32_t rc = started ? fit_layer<true, false>(ts, k, ik, L, 0, mass2, none, mh, ch)
+                                : fit_layer<false, false>(ts, k, ik, L, 0, mass2, none, mh, ch);
     if (rc != 0u) return rc;
 #define KF_PUT(f) if (c) t.f.v.y = ts.f; else t.f.v.x = ts.f;
     KF_TRACK_FIELDS(KF_PUT)
@@ -438,7 +451,8 @@ __device__ __noinline__ uint32_t refit_step_one_of_pair(Track2& t, int c, float 
 #define KF_GETH(f) mh.f = c ? m.f.v.y : m.f.v.x;
     KF_GETH(x) KF_GETH(y) KF_GETH(z) KF_GETH(vxx) KF_GETH(vxy) KF_GETH(vxz) KF_GETH(vyy) KF_GETH(vyz) KF_GETH(vzz)
 #undef KF_GETH
-    const uint32_t rc = refit_step<false>(ts, k, ik, L, Lprev, 0, mass2, first, mh.x, mh.y, mh.z, mh.vxx, mh.vxy,
+    const Bethe none = {0.0f, 0.0f, 0.0f, 0.0f};
+    const uint32_t rc = refit_step<false>(ts, k, ik, L, Lprev, 0, mass2, none, first, mh.x, mh.y, mh.z, mh.vxx, mh.vxy,
                                           mh.vxz, mh.vyy, mh.vyz, mh.vzz, &d);
     if (rc != 0u) return rc;
 #define KF_PUT(f) if (c) t.f.v.y = ts.f; else t.f.v.x = ts.f;
@@ -633,7 +647,7 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
                 Hit2 m;
                 load_hit_pair(m, tp);
                 f2 d;
-                const u2 rc = refit_step<false>(t, k, ik, P.layer[l], P.layer[lpx], 0, P.mass2, first.x, m.x, m.y, m.z,
+                const u2 rc = refit_step<false>(t, k, ik, P.layer[l], P.layer[lpx], 0, P.mass2, P.el, first.x, m.x, m.y, m.z,
                                                 m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, &d);
                 if (is_zero(rc)) {
                     schi2 = schi2 + d;
@@ -758,8 +772,8 @@ fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ 
             }
             if (h < 0) continue;
             uint32_t rc;
-            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.material_model, P.mass2, m, chi2);
-            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.material_model, P.mass2, m, chi2);
+            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.model, P.mass2, P.el, m, chi2);
+            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.model, P.mass2, P.el, m, chi2);
             st |= rc;
             if (rc == 0u) { nh += 1; started = true; }
         }

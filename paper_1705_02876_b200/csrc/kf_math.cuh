@@ -32,12 +32,15 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "kf_pair.cuh"
 
 namespace kf {
 
 constexpr float kCB = 2.99792458e-3f;  // GeV / (c T cm), reading A1
 
+enum : int { MODEL_PATH_LENGTH = 1, MODEL_ENERGY_LOSS = 2 };
 enum : uint32_t { ST_PROP_FAIL = 1u, ST_S_NOT_PD = 2u, ST_NONFINITE = 4u, ST_BAD_CHARGE = 8u, ST_OUTSIDE = 16u };
 
 // Per-layer constants, computed once on the host in double and rounded to float.
@@ -50,6 +53,16 @@ struct LayerConst {
     float half_len;  // barrel half length (+inf: unbounded)
     float ms0;       // 0.0136^2 t          (0 if t <= 0)
     float ln_t;      // ln t                (0 if t <= 0)
+    // reading A21 (energy loss)
+    float de0;       // K (Z/A) t X0 for silicon [GeV]: Bethe prefactor of the layer (0 if t <= 0 or option off)
+};
+
+// Reading A21: particle-dependent constants of Bethe's formula, computed on the host in double.
+struct Bethe {
+    float mass;  // M
+    float a;     // ln(2 me / (I M^2)):   ln(2 me (beta gamma)^2 / I) = a + ln p^2
+    float b;     // 2 me / M^2:           1 + 2 gamma me/M + (me/M)^2 = c + b E
+    float c;     // 1 + (me/M)^2
 };
 
 struct FitParams {
@@ -57,8 +70,9 @@ struct FitParams {
     float k0;      // c_B * Bz           (k = q k0)
     float inv_k0;  // 1 / (c_B * Bz)
     float mass2;   // mass^2
-    int material_model;  // reading A20: 0 flat thickness, 1 thickness / cos(incidence angle)
-    int geometry_options;  // 1 if material_model != 0 or any layer has a finite half length
+    int model;           // MODEL_* flags: reading A20 path-length material, reading A21 energy loss
+    int geometry_options;  // 1 if model != 0 or any layer has a finite half length
+    Bethe el;            // reading A21 constants (zero unless MODEL_ENERGY_LOSS)
     LayerConst layer[32];
 };
 
@@ -80,7 +94,7 @@ __device__ __forceinline__ f2 rsqrt_fast(f2 x) { return f2(rsqrt_fast(x.v.x), rs
 //     ms_eff = 0.0136^2 t f (1 + 0.038 (ln t + ln f))^2.
 template <class F>
 __device__ __forceinline__ F layer_ms(const LayerConst& L, int model, F cos_a, F p2, F ipt) {
-    if (model == 0) return F(L.ms);
+    if ((model & MODEL_PATH_LENGTH) == 0) return F(L.ms);
     const F f = sqrt_(p2) * ipt * rcp_fast(abs_(cos_a));
     const F lg = 1.0f + 0.038f * (L.ln_t + log_fast(f));
     return L.ms0 * f * lg * lg;
@@ -270,7 +284,7 @@ __device__ __forceinline__ typename num_traits<F>::status reach_layer(const Trac
 // Highland factor at an arrival (forward filter) / at the state standing on a layer (backward refit).
 template <class F>
 __device__ __forceinline__ F ms_at_crossing(const LayerConst& L, int model, const CrossingT<F>& o, arg<F> pz) {
-    if (model == 0) return F(L.ms);
+    if ((model & MODEL_PATH_LENGTH) == 0) return F(L.ms);
     return layer_ms<F>(L, model, o.erx * o.elx + o.ery * o.ely, o.pt2 + pz * pz, o.ipt);
 }
 
@@ -363,7 +377,7 @@ __device__ __forceinline__ void add_process_noise(TrackT<F>& t, const LayerConst
     const F pt2 = t.px * t.px + t.py * t.py, pz = t.pz;
     const F ipt = rsqrt_fast(pt2);
     const F p2 = pt2 + pz * pz;
-    const F ms = model == 0 ? F(L.ms) : layer_ms<F>(L, model, (t.eax * t.px + t.eay * t.py) * ipt, p2, ipt);
+    const F ms = (model & MODEL_PATH_LENGTH) == 0 ? F(L.ms) : layer_ms<F>(L, model, (t.eax * t.px + t.eay * t.py) * ipt, p2, ipt);
     const F ip2 = rcp_fast(p2);
     const F th2 = ms * (p2 + mass2) * ip2 * ip2;
     const F qc = th2 * p2 * ipt;
@@ -371,6 +385,69 @@ __device__ __forceinline__ void add_process_noise(TrackT<F>& t, const LayerConst
     t.c35 -= qc * pz;
     t.c44 += th2 * p2;
     t.c55 += qc * (p2 * ipt);
+}
+
+// ---- reading A21: mean energy loss in the layer ---------------------------------------------------------
+// The momentum keeps its direction and shrinks (forward filter) or grows back (backward refit) by
+//   f = p''/p,  p''^2 = p^2 -+ dE (2E -+ dE),  dE = L.de0 [path factor] / beta^2 *
+//                       (ln(2 me (beta gamma)^2 / I) - ln(1 + 2 gamma me/M + (me/M)^2)/2 - beta^2).
+// Direction-preserving scaling leaves the frames where they are; in (b1, b2, c) its Jacobian (dE held fixed) is
+//   J = [[g, 0, h], [0, f, 0], [0, 0, f]],  g = (E''/p'')(p/E),  h = (g - f) pT pz / p^2
+// (b1 = d pT carries all of d|p| at fixed direction; b2 and c are direction changes times pT, which scales).
+struct Eloss {
+    float f, g, h;
+};
+
+// cos_a: in-plane cosine between the radial direction and the transverse momentum (path-length option only).
+__device__ __forceinline__ bool energy_loss_factors(const Bethe& el, const LayerConst& L, int model, float mass2,
+                                                    float cos_a, float pt2, float ipt, float pz, bool regain,
+                                                    Eloss& e) {
+    const float p2 = pt2 + pz * pz;
+    const float ip = rsqrt_fast(p2);
+    const float E2 = p2 + mass2;
+    const float iE = rsqrt_fast(E2);
+    const float E = E2 * iE;
+    float thick = L.de0;
+    if (model & MODEL_PATH_LENGTH) thick *= p2 * ip * ipt * rcp_fast(fabsf(cos_a));
+    const float bracket = el.a + __logf(p2) - 0.5f * __logf(fmaf(el.b, E, el.c)) - p2 * iE * iE;
+    const float dE = thick * (E2 * ip * ip) * bracket;
+    const float En = regain ? E + dE : E - dE;
+    if (!(En > el.mass)) return false;  // the particle would stop (NaNs fail too)
+    const float pn2 = regain ? fmaf(dE, 2.0f * E + dE, p2) : fmaf(-dE, 2.0f * E - dE, p2);
+    const float ipn = rsqrt_fast(pn2);
+    e.f = pn2 * ipn * ip;
+    e.g = En * ipn * (p2 * ip) * iE;
+    e.h = (e.g - e.f) * (pt2 * ipt) * pz * (ip * ip);
+    return true;
+}
+
+// Forward filter: applied to the propagated state and covariance (after C' = F C F^T + Q, before the update).
+__device__ __forceinline__ void apply_energy_loss(const Eloss& e, CrossingT<float>& o, PropCovT<float>& n, float& pz) {
+    const float f = e.f, g = e.g, h = e.h, ff = f * f;
+    o.pxn *= f; o.pyn *= f; pz *= f;
+    o.pt2 *= ff;
+    o.ipt *= rcp_fast(f);
+    n.n13 = g * n.n13 + h * n.n15;
+    n.n23 = g * n.n23 + h * n.n25;
+    n.n33 = g * (g * n.n33 + 2.0f * h * n.n35) + h * h * n.n55;
+    n.n34 = f * (g * n.n34 + h * n.n45);
+    n.n35 = f * (g * n.n35 + h * n.n55);
+    n.n14 *= f; n.n24 *= f; n.n15 *= f; n.n25 *= f;
+    n.n44 *= ff; n.n45 *= ff; n.n55 *= ff;
+}
+
+// Backward refit: applied to the track standing on the layer it is about to leave.
+__device__ __forceinline__ void apply_energy_loss(const Eloss& e, TrackT<float>& t) {
+    const float f = e.f, g = e.g, h = e.h, ff = f * f;
+    t.px *= f; t.py *= f; t.pz *= f;
+    t.c03 = g * t.c03 + h * t.c05;
+    t.c13 = g * t.c13 + h * t.c15;
+    t.c23 = g * t.c23 + h * t.c25;
+    t.c33 = g * (g * t.c33 + 2.0f * h * t.c35) + h * h * t.c55;
+    t.c34 = f * (g * t.c34 + h * t.c45);
+    t.c35 = f * (g * t.c35 + h * t.c55);
+    t.c04 *= f; t.c14 *= f; t.c24 *= f; t.c05 *= f; t.c15 *= f; t.c25 *= f;
+    t.c44 *= ff; t.c45 *= ff; t.c55 *= ff;
 }
 
 // The track as it stands, dressed as a "crossing" with zero path length, so that kalman_update can be
@@ -556,10 +633,33 @@ kalman_update(TrackT<F>& t, const CrossingT<F>& o, const PropCovT<F>& n, const L
 template <bool BOUNDED, class F>
 __device__ __forceinline__ typename num_traits<F>::status
 refit_step(TrackT<F>& t, arg<F> k, arg<F> ik, const LayerConst& L, const LayerConst& Lprev, int model, float mass2,
-           bool first, arg<F> mx, arg<F> my, arg<F> mz, arg<F> vxx, arg<F> vxy, arg<F> vxz, arg<F> vyy, arg<F> vyz,
-           arg<F> vzz, F* dchi2) {
+           const Bethe& el, bool first, arg<F> mx, arg<F> my, arg<F> mz, arg<F> vxx, arg<F> vxy, arg<F> vxz,
+           arg<F> vyy, arg<F> vyz, arg<F> vzz, F* dchi2) {
     CrossingT<F> o;
     PropCovT<F> n;
+    LocalHitT<F> h;
+    if constexpr (std::is_same<F, float>::value) {
+        if (!first && (model & MODEL_ENERGY_LOSS)) {
+            // reading A21: the layer just left gives back the energy it took, before its scattering noise is
+            // added; worked on a copy so that any failure leaves the track as it was
+            TrackT<float> tb = t;
+            const float pt2 = tb.px * tb.px + tb.py * tb.py;
+            const float ipt = rsqrt_fast(pt2);
+            Eloss e;
+            if (!energy_loss_factors(el, Lprev, model, mass2, (tb.eax * tb.px + tb.eay * tb.py) * ipt, pt2, ipt,
+                                     tb.pz, true, e))
+                return ST_PROP_FAIL;
+            apply_energy_loss(e, tb);
+            const uint32_t reached = reach_layer<true, BOUNDED>(tb, k, ik, L, o);
+            if (reached) return reached;
+            add_process_noise(tb, Lprev, model, mass2);
+            transport_cov<true>(tb, o, 0.0f, mass2, n);
+            hit_to_local(o, mx, my, mz, vxx, vxy, vxz, vyy, vyz, vzz, h);
+            const uint32_t rc = kalman_update(tb, o, n, h, dchi2);
+            if (rc == 0u) t = tb;
+            return rc;
+        }
+    }
     const F k33 = t.c33, k35 = t.c35, k44 = t.c44, k55 = t.c55;
     if (first) crossing_in_place(t, o, n);
     else {
@@ -568,7 +668,6 @@ refit_step(TrackT<F>& t, arg<F> k, arg<F> ik, const LayerConst& L, const LayerCo
         add_process_noise(t, Lprev, model, mass2);      // the scatterer just left behind
         transport_cov<true>(t, o, F(0.0f), mass2, n);
     }
-    LocalHitT<F> h;
     hit_to_local(o, mx, my, mz, vxx, vxy, vxz, vyy, vyz, vzz, h);
     const auto rc = kalman_update(t, o, n, h, dchi2);
     if (!is_zero(rc)) { t.c33 = k33; t.c35 = k35; t.c44 = k44; t.c55 = k55; }   // layer skipped

@@ -64,7 +64,7 @@ propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
     enter_local_frame(t);
     if (keep_track) put_track(a.track, a.ld_sc, i, t);
     const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
-    const uint32_t rc = propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.material_model, P.mass2,
+    const uint32_t rc = propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.model, P.mass2, P.el,
                                                     BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch, a.ld_sc, i);
     if (rc) a.status[i] |= rc;
     a.flag[i] = rc ? FLAG_IDLE : FLAG_AT_LAYER;
@@ -81,8 +81,8 @@ update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
     if (f == FLAG_AT_LAYER) { apply_decision(a, i, t); put_track(a.track, a.ld_sc, i, t); }
     else get_track(a.track, a.ld_sc, i, t);
     const float qf = (float)a.q[i];
-    const uint32_t rc = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.material_model,
-                                                    P.mass2, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch,
+    const uint32_t rc = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model,
+                                                    P.mass2, P.el, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch,
                                                     a.ld_sc, i);
     if (rc) a.status[i] |= rc;
     a.flag[i] = rc ? FLAG_IDLE : FLAG_AT_LAYER;

@@ -63,14 +63,21 @@ __device__ __forceinline__ void hit_from_record(const float4* __restrict__ rec, 
 // else the status bit that says why not (ST_PROP_FAIL, ST_OUTSIDE).
 template <bool RADIAL_NULL>
 __device__ __forceinline__ uint32_t propagate_to_scratch(const Track& t, float k, float ik, const LayerConst& Lc,
-                                                         int model, float mass2, const BinGrid& g, float* sc,
-                                                         int64_t ld, int64_t i) {
+                                                         int model, float mass2, const Bethe& el, const BinGrid& g,
+                                                         float* sc, int64_t ld, int64_t i) {
     Crossing o;
     const uint32_t reached = reach_layer(t, k, ik, Lc, o);
     if (reached) return reached;
     PropCov n;
     transport_cov<RADIAL_NULL>(t, o, ms_at_crossing(Lc, model, o, t.pz), mass2, n);
-    put_scratch(sc, ld, i, o, n, t.pz);
+    float pz = t.pz;
+    if (model & MODEL_ENERGY_LOSS) {   // reading A21
+        Eloss e;
+        if (!energy_loss_factors(el, Lc, model, mass2, o.erx * o.elx + o.ery * o.ely, o.pt2, o.ipt, pz, false, e))
+            return ST_PROP_FAIL;
+        apply_energy_loss(e, o, n, pz);
+    }
+    put_scratch(sc, ld, i, o, n, pz);
     // the candidate's own bin (reading A16): eta = asinh(z'/r), phi = atan2(y', x') -- once per candidate
     // here, not once per lane in the scan
     const float eta = asinhf(o.zn * Lc.inv_r);

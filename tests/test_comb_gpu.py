@@ -26,31 +26,33 @@ def ctx():
     c.close()
 
 
-def _run(ctx, n_tracks, noise, n_cand, half_length=None, material_model=0):
+def _run(ctx, n_tracks, noise, n_cand, half_length=None, material_model=0, energy_loss=0):
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
     ev = W.make_build_event(4, n_tracks=n_tracks, noise_hits=noise)
     f = ev.fit
     r = O.fit_tracks(f.radius[:3], f.x_over_X0[:3], f.Bz, f.mass, f.par, f.cov, f.q, f.hpos[:3], f.hcov[:3], None, nthreads=8)
     par, cov = r["par"].astype(np.float32), O.pack_cov21(r["cov"]).astype(np.float32)
-    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, half_length, material_model)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, half_length, material_model, energy_loss)
     dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers[3:]]
     ctx.bin_layers([l.radius for l in ev.layers[3:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
     dc = DeviceCandidates.from_numpy(par, cov, f.q, r["chi2"], r["nhits"], "cuda:0")
     idx, nf = dc.build_combinatorial(ctx, geom, 3, dls, n_cand)
     torch.cuda.synchronize()
     layers = [(l.pos, l.cov, O.bin_hits(l.pos, l.radius, NE, NP, EMAX)) for l in ev.layers[3:]]
-    with O.geometry_options(material_model, half_length):
+    with O.geometry_options(material_model, half_length, energy_loss=energy_loss):
         o = O.build_combinatorial(f.radius, f.x_over_X0, f.Bz, f.mass, par, cov, f.q, r["chi2"], r["nhits"], 3, layers,
                                   NE, NP, EMAX, 2, 30.0, n_cand)
     return ev, dc.results(), idx.cpu().numpy()[:, :f.n], nf.cpu().numpy()[:f.n], o
 
 
 GEOM = dict(half_length=np.full(10, 25.0, dtype=np.float32), material_model=1)     # reading A20
+GEOM_ELOSS = dict(half_length=np.full(10, 25.0, dtype=np.float32), material_model=1, energy_loss=1)   # + reading A21
 
 
 @pytest.mark.parametrize("n_tracks,noise,n_cand,geom", [(400, 2000, 4, {}), (400, 2000, 1, {}), (3000, 15000, 8, {}),
-                                                        (20000, 100000, 4, {}), (3000, 15000, 4, GEOM)])
+                                                        (20000, 100000, 4, {}), (3000, 15000, 4, GEOM),
+                                                        (3000, 15000, 4, GEOM_ELOSS)])
 def test_combinatorial_parity(ctx, n_tracks, noise, n_cand, geom):
     ev, g, idx, nf, o = _run(ctx, n_tracks, noise, n_cand, **geom)
     f = ev.fit

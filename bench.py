@@ -335,9 +335,22 @@ def run_ours(args) -> None:
         torch.cuda.synchronize()
         go_ms = s0.elapsed_time(s1) / 20
         go_out = float((d.out_status[:n] & 16).ne(0).float().mean().item())
+        # ... and with the energy loss of reading A21 on top
+        d.geom = K.Geometry(plain_geom.radius_cm, plain_geom.x_over_X0, plain_geom.Bz_tesla, plain_geom.mass_gev,
+                            np.full(L, 30.0, dtype=np.float32), 1, 1)
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                d.fit(ctx)
+            s0.record(stream)
+            for _ in range(20):
+                d.fit(ctx)
+            s1.record(stream)
+        torch.cuda.synchronize()
+        el_ms = s0.elapsed_time(s1) / 20
         d.geom = plain_geom
         geometry = {"api": "kf_fit_tracks with material_model 1 and 30 cm barrel half lengths (reading A20)", "ms": go_ms,
-                    "fits_per_s": n / (go_ms * 1e-3), "tracks_cut_short": go_out}
+                    "fits_per_s": n / (go_ms * 1e-3), "tracks_cut_short": go_out,
+                    "with_energy_loss_ms": el_ms, "with_energy_loss_fits_per_s": n / (el_ms * 1e-3)}
         # secondary: kf_fit_tracks_indexed -- same tracks, each layer's hits shuffled into a pool and addressed by index
         g = torch.Generator(device=dev); g.manual_seed(5)
         perm = [torch.randperm(n, device=dev, generator=g) for _ in range(L)]

@@ -94,6 +94,24 @@ KF_API int kf_reserve(kf_ctx* ctx, int64_t max_hits, int64_t max_host_tracks, in
 KF_API const char* kf_strerror(int code);
 /* cudaError_t of the last KF_ERR_CUDA on this context (0 if none). */
 KF_API int kf_last_cuda_error(const kf_ctx* ctx);
+/* ---- graphs: record a fixed sequence of hot calls once, replay it with one launch ---------------------------
+ * Event-sized work (10 000 - 20 000 tracks per event) is bound by kernel-launch and host-call
+ * overhead, not by the device: one kf_bin_layers + kf_build_best_hit over 7 layers is 20 launches of 5 - 25 us.
+ * Between kf_graph_begin and kf_graph_end every device-pointer hot call on this context (kf_fit_tracks[_indexed /
+ * _smooth], kf_bin_hits / kf_bin_layers, kf_order_candidates, kf_score_candidates, kf_build_best_hit,
+ * kf_build_combinatorial) is RECORDED into a CUDA graph instead of executed; kf_graph_launch then enqueues the
+ * whole sequence on the context's stream with the pointers, sizes and geometry it was recorded with (the caller
+ * refills the same buffers between launches).  Requirements: a non-NULL stream; scratch already sized, i.e. the
+ * same sequence has run once before (or kf_reserve), because a call that has to grow scratch synchronises and
+ * voids the capture (kf_graph_end then returns KF_ERR_CUDA and no graph).  kf_fit_tracks_host, kf_reserve,
+ * kf_measure_fp32_peak and kf_set_stream must not be called while recording.  Results are bit-identical to
+ * the eager calls.  A graph belongs to the device of the context that recorded it; destroy it with
+ * kf_graph_destroy (independent of the context's lifetime). */
+typedef struct kf_graph kf_graph;
+KF_API int kf_graph_begin(kf_ctx* ctx);
+KF_API int kf_graph_end(kf_ctx* ctx, kf_graph** out);
+KF_API int kf_graph_launch(kf_ctx* ctx, kf_graph* graph);
+KF_API int kf_graph_destroy(kf_graph* graph);
 /* Measurement utility (not on the hot path): sustained FP32 FMA throughput of the device in TFLOP/s
  * from a register-only FMA microbenchmark (8 independent chains per thread, 2048 threads per SM, best
  * of `repeats` launches).  Synchronises the stream.  This is the denominator of the ALU roofline. */

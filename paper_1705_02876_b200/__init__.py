@@ -4,8 +4,8 @@ The product is the C-ABI shared library `libkf_b200.so` (include/kf_b200.h) buil
 this package is the thin ctypes binding with the same call names.  There is no CPU fallback:
 without the built library, or without a CUDA device, the calls raise.
 """
-from .binding import (KFContext, KFError, Bins, Geometry, abi_version, lib_path, load_library,
+from .binding import (KFContext, KFError, Bins, Geometry, Graph, abi_version, lib_path, load_library,
                       strerror, STATUS_BAD_CHARGE, STATUS_NONFINITE, STATUS_OUTSIDE, STATUS_PROP_FAIL, STATUS_S_NOT_PD)
 
-__all__ = ["KFContext", "KFError", "Bins", "Geometry", "abi_version", "lib_path", "load_library",
+__all__ = ["KFContext", "KFError", "Bins", "Geometry", "Graph", "abi_version", "lib_path", "load_library",
            "strerror", "STATUS_BAD_CHARGE", "STATUS_NONFINITE", "STATUS_OUTSIDE", "STATUS_PROP_FAIL", "STATUS_S_NOT_PD"]

@@ -22,7 +22,8 @@ _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so"
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE, STATUS_OUTSIDE = 1, 2, 4, 8, 16
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
            "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
-           "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial"]
+           "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial",
+           "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
 
 class KFError(RuntimeError):
@@ -127,8 +128,37 @@ def load_library():
     lib.kf_build_combinatorial.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
                                            C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
                                            vp, vp, C.c_int64]
+    lib.kf_graph_begin.restype = C.c_int
+    lib.kf_graph_begin.argtypes = [vp]
+    lib.kf_graph_end.restype = C.c_int
+    lib.kf_graph_end.argtypes = [vp, C.POINTER(vp)]
+    lib.kf_graph_launch.restype = C.c_int
+    lib.kf_graph_launch.argtypes = [vp, vp]
+    lib.kf_graph_destroy.restype = C.c_int
+    lib.kf_graph_destroy.argtypes = [vp]
     _lib = lib
     return lib
+
+
+class Graph:
+    """A recorded sequence of hot calls (kf_graph); launch() enqueues it on the context's stream."""
+
+    def __init__(self, ctx: "KFContext", handle):
+        self._ctx, self._g = ctx, handle
+
+    def launch(self):
+        self._ctx._check(self._ctx._lib.kf_graph_launch(self._ctx._h, self._g), "kf_graph_launch")
+
+    def close(self):
+        if self._g:
+            load_library().kf_graph_destroy(self._g)
+            self._g = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def strerror(code: int) -> str:
@@ -245,6 +275,16 @@ class KFContext:
     def set_stream(self, stream: torch.cuda.Stream | None):
         s = stream.cuda_stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
         self._check(self._lib.kf_set_stream(self._h, C.c_void_p(s)), "kf_set_stream")
+
+    # ------------------------------------------------------------------ kf_graph_*
+    def graph_begin(self):
+        """Start recording the hot calls made on this context (kf_graph_begin)."""
+        self._check(self._lib.kf_graph_begin(self._h), "kf_graph_begin")
+
+    def graph_end(self) -> "Graph":
+        out = C.c_void_p()
+        self._check(self._lib.kf_graph_end(self._h, C.byref(out)), "kf_graph_end")
+        return Graph(self, out)
 
     def reserve(self, max_hits: int = 0, max_host_tracks: int = 0, max_host_layers: int = 0):
         self._check(self._lib.kf_reserve(self._h, max_hits, max_host_tracks, max_host_layers), "kf_reserve")

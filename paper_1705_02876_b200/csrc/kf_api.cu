@@ -11,8 +11,14 @@
 
 using namespace kf;
 
+struct kf_graph {
+    cudaGraphExec_t exec = nullptr;
+    int device = 0;
+};
+
 struct kf_ctx {
     int device = 0;
+    bool capturing = false;
     cudaStream_t stream = nullptr;
     int last_cuda = 0;
     // kf_bin_hits scratch
@@ -26,7 +32,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 9;
+constexpr int kAbiVersion = 10;
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -165,11 +171,62 @@ int kf_destroy(kf_ctx* c) {
 
 int kf_set_stream(kf_ctx* c, void* cuda_stream) {
     if (!c) return KF_ERR_NULL;
+    if (c->capturing) return KF_ERR_UNSUPPORTED;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     return KF_OK;
 }
 
 int kf_last_cuda_error(const kf_ctx* c) { return c ? c->last_cuda : 0; }
+
+// ---- CUDA-graph capture of a sequence of hot calls (include/kf_b200.h "graphs") ----------------------------
+int kf_graph_begin(kf_ctx* c) {
+    if (!c) return KF_ERR_NULL;
+    if (c->capturing || c->stream == nullptr) return KF_ERR_UNSUPPORTED;  // the legacy default stream cannot be captured
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    // relaxed: other host threads (torch's allocator, NCCL watchdogs) may keep calling the runtime meanwhile
+    if ((e = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return cuda_fail(c, e);
+    c->capturing = true;
+    return KF_OK;
+}
+
+int kf_graph_end(kf_ctx* c, kf_graph** out) {
+    if (!c || !out) return KF_ERR_NULL;
+    *out = nullptr;
+    if (!c->capturing) return KF_ERR_UNSUPPORTED;
+    c->capturing = false;
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+    if (e != cudaSuccess || !g) {   // a captured call synchronised or allocated (scratch not reserved): capture void
+        if (g) cudaGraphDestroy(g);
+        cudaGetLastError();
+        return cuda_fail(c, e != cudaSuccess ? e : cudaErrorStreamCaptureInvalidated);
+    }
+    kf_graph* kg = new (std::nothrow) kf_graph();
+    if (!kg) { cudaGraphDestroy(g); return KF_ERR_NOMEM; }
+    kg->device = c->device;
+    e = cudaGraphInstantiate(&kg->exec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { delete kg; return cuda_fail(c, e); }
+    *out = kg;
+    return KF_OK;
+}
+
+int kf_graph_launch(kf_ctx* c, kf_graph* g) {
+    if (!c || !g || !g->exec) return KF_ERR_NULL;
+    if (c->capturing || g->device != c->device) return KF_ERR_UNSUPPORTED;
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if ((e = cudaGraphLaunch(g->exec, c->stream)) != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_graph_destroy(kf_graph* g) {
+    if (!g) return KF_ERR_NULL;
+    if (g->exec) cudaGraphExecDestroy(g->exec);
+    delete g;
+    return KF_OK;
+}
 
 int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_host_layers) {
     if (!c) return KF_ERR_NULL;

@@ -44,7 +44,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_abi_version_and_error_strings(lib):
     import paper_1705_02876_b200 as K
-    assert K.abi_version() == 9
+    assert K.abi_version() == 10
     seen = set()
     for code in (0, -1, -2, -3, -4, -5, -6, -99):
         s = K.strerror(code)
@@ -68,6 +68,10 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_order_candidates(None, None, 0, None, 40, 64, 1.2, None) == -1
     assert lib.kf_measure_fp32_peak(None, 3, None) == -1
     assert lib.kf_last_cuda_error(None) == 0
+    assert lib.kf_graph_begin(None) == -1
+    assert lib.kf_graph_end(None, None) == -1
+    assert lib.kf_graph_launch(None, None) == -1
+    assert lib.kf_graph_destroy(None) == -1
 
 
 def test_no_cpu_fallback(lib):

@@ -13,13 +13,15 @@
 // with (cos_j, sin_j) = fl(cos, sin)(-pi + j d_phi).  No transcendental is evaluated on the GPU.
 //
 // Counting sort, stable, batched over layers (grid.y = layer, 5 launches + 1 memset for ALL layers):
-// (1) key of every item + histogram, (2) exclusive scan -> bin_offset, (3) scatter item indices into
-// their bin segment in arbitrary order (atomic cursor), (4) every slot ranks its index inside its
-// segment (indices are unique, so ascending index IS the stable order) and, for hits, gathers the
-// hit into the bin-ordered outputs: a packed 12-float record per hit for the scoring kernel
+// (1) key of every item + histogram; the histogram atomic's return value is the item's arrival number inside its
+// bin, (2) exclusive scan -> bin_offset, (3) every item goes to slot bin_offset[bin] + arrival number -- no second
+// round of atomics -- and, for hits, its nine values are read here, coalesced, and parked as a packed record in
+// that slot of a scratch buffer, (4) every slot ranks its index inside its segment (indices are unique, so
+// ascending index IS the stable order: the arrival order, which differs from run to run, never shows) and moves
+// its record to its final place: a packed 12-float record per hit for the scoring kernel
 // (x y z vzz | vxx vxy vyy index | vxz vyz 0 0: the first 128-bit word serves the z pre-filter,
-// the second the tangential one, the third only full evaluations) and,
-// optionally, SoA copies.
+// the second the tangential one, the third only full evaluations) and, optionally, SoA copies; (5) per-bin boxes.
+// Every read of the inputs is coalesced; the only scattered traffic is one 48-byte record per hit in step (3).
 #include <cmath>
 
 #include "kf_internal.h"
@@ -43,17 +45,27 @@ __device__ __forceinline__ int bin_of_hit(float x, float y, float z, float r, in
         if (u >= __ldg(eta_edge + mid)) lo = mid + 1; else hi = mid;
     }
     const int ie = lo - 1;
+    // The predicate fl(cos_j y) >= fl(sin_j x) says "phi >= edge j" and is true up to the hit's own edge and false
+    // beyond it within one half plane (only the edge nearest to the hit is within rounding of the decision, and
+    // either answer there keeps the sequence monotone), so the count of true predicates is a bisection.
     const int half = n_phi >> 1;
     int ip = 0;
     if (y > 0.0f || (y == 0.0f && x > 0.0f)) {
-        ip = half;
-        for (int j = half + 1; j < n_phi; ++j)
-            ip += (__fmul_rn(__ldg(phi_cos + j), y) >= __fmul_rn(__ldg(phi_sin + j), x)) ? 1 : 0;
+        int lo = half + 1, hi = n_phi;      // first j in [half + 1, n_phi) with a false predicate
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (__fmul_rn(__ldg(phi_cos + mid), y) >= __fmul_rn(__ldg(phi_sin + mid), x)) lo = mid + 1; else hi = mid;
+        }
+        ip = lo - 1;
     } else if (y == 0.0f) {
         ip = 0;
     } else {
-        for (int j = 1; j < half; ++j)
-            ip += (__fmul_rn(__ldg(phi_cos + j), y) >= __fmul_rn(__ldg(phi_sin + j), x)) ? 1 : 0;
+        int lo = 1, hi = half;              // first j in [1, half)
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (__fmul_rn(__ldg(phi_cos + mid), y) >= __fmul_rn(__ldg(phi_sin + mid), x)) lo = mid + 1; else hi = mid;
+        }
+        ip = lo - 1;
     }
     return ie * n_phi + ip;
 }
@@ -67,10 +79,10 @@ bin_key_kernel(const __grid_constant__ BinBatch B, const float* __restrict__ eta
     const int b = bin_of_hit(__ldg(L.pos + h), __ldg(L.pos + L.ld_in + h), __ldg(L.pos + 2 * L.ld_in + h),
                              L.radius, B.n_eta, B.n_phi, eta_edge, phi_cos, phi_sin);
     L.key[h] = b;
-    atomicAdd(L.counts + b, 1);
+    L.pib[h] = atomicAdd(L.counts + b, 1);
 }
 
-// Exclusive scan of counts[0..nb) -> bin_offset[0..nb], cursor = copy.  One block of 1024 per layer.
+// Exclusive scan of counts[0..nb) -> bin_offset[0..nb].  One block of 1024 per layer.
 __global__ void __launch_bounds__(1024)
 bin_scan_kernel(const __grid_constant__ BinBatch B) {
     const BinLayerDev& L = B.layer[blockIdx.y];
@@ -103,7 +115,7 @@ bin_scan_kernel(const __grid_constant__ BinBatch B) {
         __syncthreads();
         const int32_t carry = carry_s;
         const int32_t excl = carry + (wid ? warp_sum[wid - 1] : 0) + incl - c;
-        if (i < nb) { L.bin_offset[i] = excl; L.cursor[i] = excl; }
+        if (i < nb) L.bin_offset[i] = excl;
         __syncthreads();
         if (tid == 1023) carry_s = excl + c;
         __syncthreads();
@@ -116,8 +128,18 @@ bin_scatter_kernel(const __grid_constant__ BinBatch B) {
     const BinLayerDev& L = B.layer[blockIdx.y];
     const int64_t h = (int64_t)blockIdx.x * kBlock + threadIdx.x;
     if (h >= L.n) return;
-    const int32_t slot = atomicAdd(L.cursor + L.key[h], 1);
+    const int64_t slot = (int64_t)L.bin_offset[L.key[h]] + L.pib[h];
     L.unsorted[slot] = (int32_t)h;
+    if (!L.rec_tmp) return;  // ordering only (candidates)
+    float v[9];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) v[k] = __ldg(L.pos + k * L.ld_in + h);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) v[3 + k] = __ldg(L.cov + k * L.ld_in + h);
+    float4* rec = reinterpret_cast<float4*>(L.rec_tmp + slot * 12);
+    rec[0] = make_float4(v[0], v[1], v[2], v[8]);                          // x y z vzz
+    rec[1] = make_float4(v[3], v[4], v[6], __int_as_float((int32_t)h));    // vxx vxy vyy, original index
+    rec[2] = make_float4(v[5], v[7], 0.0f, 0.0f);                          // vxz vyz
 }
 
 // Slot p holds item `mine` of bin b; its final place is bin_offset[b] + #{indices in the segment
@@ -135,25 +157,22 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     const int64_t dst = (int64_t)s + rank;
     L.sorted_to_orig[dst] = mine;
     if (L.orig_to_sorted) L.orig_to_sorted[mine] = (int32_t)dst;
-    if (!L.pos) return;  // ordering only (candidates)
-    float v[9];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) v[k] = __ldg(L.pos + k * L.ld_in + mine);
-#pragma unroll
-    for (int k = 0; k < 6; ++k) v[3 + k] = __ldg(L.cov + k * L.ld_in + mine);
+    if (!L.rec_tmp) return;  // ordering only (candidates)
+    const float4* src = reinterpret_cast<const float4*>(L.rec_tmp + p * 12);
+    const float4 A = src[0], Bw = src[1], C = src[2];
     if (L.hit_rec) {
         float4* rec = reinterpret_cast<float4*>(L.hit_rec + dst * 12);
-        rec[0] = make_float4(v[0], v[1], v[2], v[8]);                    // x y z vzz
-        rec[1] = make_float4(v[3], v[4], v[6], __int_as_float(mine));    // vxx vxy vyy, original index
-        rec[2] = make_float4(v[5], v[7], 0.0f, 0.0f);                    // vxz vyz
+        rec[0] = A;
+        rec[1] = Bw;
+        rec[2] = C;
     }
     if (L.pos_sorted) {
-#pragma unroll
-        for (int k = 0; k < 3; ++k) L.pos_sorted[k * L.ld_out + dst] = v[k];
+        L.pos_sorted[dst] = A.x; L.pos_sorted[L.ld_out + dst] = A.y; L.pos_sorted[2 * L.ld_out + dst] = A.z;
     }
-    if (L.cov_sorted) {
-#pragma unroll
-        for (int k = 0; k < 6; ++k) L.cov_sorted[k * L.ld_out + dst] = v[3 + k];
+    if (L.cov_sorted) {   // xx xy xz yy yz zz
+        L.cov_sorted[dst] = Bw.x;                 L.cov_sorted[L.ld_out + dst] = Bw.y;
+        L.cov_sorted[2 * L.ld_out + dst] = C.x;   L.cov_sorted[3 * L.ld_out + dst] = Bw.z;
+        L.cov_sorted[4 * L.ld_out + dst] = C.y;   L.cov_sorted[5 * L.ld_out + dst] = A.w;
     }
 }
 
@@ -195,7 +214,8 @@ bin_box_kernel(const __grid_constant__ BinBatch B) {
 __global__ void __launch_bounds__(kBlock)
 cand_key_kernel(const __grid_constant__ FitParams P, int layer, int64_t n, int64_t ld,
                 const float* __restrict__ par, const int8_t* __restrict__ q, int n_eta, int n_phi,
-                float eta_max, int32_t* __restrict__ key, int32_t* __restrict__ counts) {
+                float eta_max, int32_t* __restrict__ key, int32_t* __restrict__ pib,
+                int32_t* __restrict__ counts) {
     const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
     if (i >= n) return;
     Track t;
@@ -216,42 +236,50 @@ cand_key_kernel(const __grid_constant__ FitParams P, int layer, int64_t n, int64
     int b = ie * n_phi + ip;
     if (!(b >= 0 && b < n_eta * n_phi)) b = 0;
     key[i] = b;
-    atomicAdd(counts + b, 1);
+    pib[i] = atomicAdd(counts + b, 1);
 }
 
 }  // namespace
 
-cudaError_t BinScratch::reserve(int64_t n_items, int64_t n_bins, cudaStream_t stream) {
-    if (n_items <= cap_items && n_bins <= cap_bins) return cudaSuccess;
+cudaError_t BinScratch::reserve(int64_t n_items, int64_t n_bins, cudaStream_t stream, bool records) {
+    const bool grow_rec = records && n_items > cap_rec;
+    if (n_items <= cap_items && n_bins <= cap_bins && !grow_rec) return cudaSuccess;
     // growing: drain the stream that may still use the old buffers, then reallocate
     cudaError_t e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) return e;
     const int64_t ni = n_items > cap_items ? n_items : cap_items;
     const int64_t nb = n_bins > cap_bins ? n_bins : cap_bins;
+    const bool want_rec = records || cap_rec > 0;
     release();
     const size_t items_b = (size_t)(ni > 0 ? ni : 1) * sizeof(int32_t);
     const size_t bins_b = (size_t)(nb > 0 ? nb : 1) * sizeof(int32_t);
     const size_t tab_b = (size_t)(KF_MAX_BINS_INTERNAL + 1) * sizeof(float);
     if ((e = cudaMalloc(&key, items_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&unsorted, items_b)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&pib, items_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&counts, bins_b)) != cudaSuccess) { release(); return e; }
-    if ((e = cudaMalloc(&cursor, bins_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&eta_edge, tab_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&phi_cos, tab_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&phi_sin, tab_b)) != cudaSuccess) { release(); return e; }
+    if (want_rec) {
+        if ((e = cudaMalloc(&rec_tmp, (size_t)(ni > 0 ? ni : 1) * 12 * sizeof(float))) != cudaSuccess) { release(); return e; }
+        cap_rec = ni;
+    }
     cap_items = ni;
     cap_bins = nb;
     return cudaSuccess;
 }
 
 void BinScratch::release() {
-    void* ptrs[] = {key, unsorted, counts, cursor, eta_edge, phi_cos, phi_sin};
+    void* ptrs[] = {key, unsorted, pib, counts, eta_edge, phi_cos, phi_sin, rec_tmp};
     for (void* p : ptrs)
         if (p) cudaFree(p);
-    key = unsorted = counts = cursor = nullptr;
+    key = unsorted = pib = counts = nullptr;
     eta_edge = phi_cos = phi_sin = nullptr;
+    rec_tmp = nullptr;
     cap_items = 0;
     cap_bins = 0;
+    cap_rec = 0;
     tab_n_eta = tab_n_phi = 0;
     tab_eta_max = 0.0f;
 }
@@ -289,7 +317,7 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
     const int nb = n_eta * n_phi;
     int64_t total = 0, max_hits = 0;
     for (int l = 0; l < n_layers; ++l) { total += args[l].n_hits; if (args[l].n_hits > max_hits) max_hits = args[l].n_hits; }
-    cudaError_t e = s.reserve(total, (int64_t)(nb + 1) * n_layers, stream);
+    cudaError_t e = s.reserve(total, (int64_t)(nb + 1) * n_layers, stream, true);
     if (e != cudaSuccess) return e;
     if ((e = s.tables(n_eta, n_phi, args[0].eta_max, stream)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(s.counts, 0, (size_t)(nb + 1) * n_layers * sizeof(int32_t), stream)) != cudaSuccess) return e;
@@ -306,7 +334,8 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
             L.bin_offset = a.bin_offset; L.sorted_to_orig = a.sorted_to_orig;
             L.pos_sorted = a.pos_sorted; L.cov_sorted = a.cov_sorted; L.hit_rec = a.hit_rec; L.bin_box = a.bin_box; L.orig_to_sorted = a.orig_to_sorted;
             L.key = s.key + item_off; L.unsorted = s.unsorted + item_off;
-            L.counts = s.counts + (int64_t)(l0 + j) * (nb + 1); L.cursor = s.cursor + (int64_t)(l0 + j) * (nb + 1);
+            L.counts = s.counts + (int64_t)(l0 + j) * (nb + 1);
+            L.pib = s.pib + item_off; L.rec_tmp = a.pos ? s.rec_tmp + item_off * 12 : nullptr;
             item_off += a.n_hits;
             if (a.n_hits > group_max) group_max = a.n_hits;
         }
@@ -337,9 +366,9 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
     L.n = n; L.ld_in = 0; L.ld_out = 0; L.pos = nullptr; L.cov = nullptr; L.radius = 0.0f;
     L.bin_offset = s.counts + (nb + 1);  // second half of the counts buffer holds the offsets
     L.sorted_to_orig = order; L.pos_sorted = nullptr; L.cov_sorted = nullptr; L.hit_rec = nullptr; L.bin_box = nullptr; L.orig_to_sorted = nullptr;
-    L.key = s.key; L.unsorted = s.unsorted; L.counts = s.counts; L.cursor = s.cursor;
+    L.key = s.key; L.unsorted = s.unsorted; L.counts = s.counts; L.pib = s.pib; L.rec_tmp = nullptr;
     const dim3 grid((unsigned)((n + kBlock - 1) / kBlock), 1);
-    cand_key_kernel<<<grid, kBlock, 0, stream>>>(P, layer, n, ld, par, q, n_eta, n_phi, eta_max, s.key, s.counts);
+    cand_key_kernel<<<grid, kBlock, 0, stream>>>(P, layer, n, ld, par, q, n_eta, n_phi, eta_max, s.key, s.pib, s.counts);
     bin_scan_kernel<<<dim3(1, 1), 1024, 0, stream>>>(B);
     bin_scatter_kernel<<<grid, kBlock, 0, stream>>>(B);
     bin_rank_gather_kernel<<<grid, kBlock, 0, stream>>>(B);

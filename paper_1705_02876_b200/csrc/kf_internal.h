@@ -90,7 +90,8 @@ struct BinLayerDev {
     int32_t* key;       // [n] bin of each item
     int32_t* unsorted;  // [n] item indices grouped by bin, arbitrary order inside
     int32_t* counts;    // [n_bins + 1]
-    int32_t* cursor;    // [n_bins + 1]
+    int32_t* pib;       // [n] arrival number of each item inside its bin (value returned by the histogram atomic)
+    float* rec_tmp;     // [n][12] hit records grouped by bin in arrival order (null when nothing is gathered)
 };
 
 struct BinBatch {
@@ -103,7 +104,9 @@ struct BinScratch {
     int32_t* key = nullptr;
     int32_t* unsorted = nullptr;
     int32_t* counts = nullptr;
-    int32_t* cursor = nullptr;
+    int32_t* pib = nullptr;
+    float* rec_tmp = nullptr;    // [cap_items][12], allocated on the first call that gathers hits
+    int64_t cap_rec = 0;
     // edge tables (device) for the (n_eta, n_phi, eta_max) last used
     float* eta_edge = nullptr;   // fl32(sinh(-eta_max + j d_eta)), j = 1..n_eta-1 at [j]
     float* phi_cos = nullptr;    // fl32(cos(-pi + j d_phi))
@@ -111,7 +114,7 @@ struct BinScratch {
     int tab_n_eta = 0, tab_n_phi = 0;
     float tab_eta_max = 0.0f;
     std::vector<float> host_tab; // persistent host copy of the three tables (source of the async copy)
-    cudaError_t reserve(int64_t n_items, int64_t n_bins, cudaStream_t stream);
+    cudaError_t reserve(int64_t n_items, int64_t n_bins, cudaStream_t stream, bool records = false);
     cudaError_t tables(int n_eta, int n_phi, float eta_max, cudaStream_t stream);
     void release();
 };

@@ -724,11 +724,17 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
 
 // ---- fit with hits addressed by index into the layer pools (the hits a track uses are
 // looked up, not pre-gathered).  index[l][i] = hit of track i in pool l or -1.
-// Gathered loads cannot go through TMA: each thread fetches its 9 floats itself, one layer ahead.
-__device__ __forceinline__ Hit gather_hit(const IndexedPools& H, int l, int32_t h) {
+// Gathered loads cannot go through TMA: each thread fetches its 9 floats itself.  The look-up is a chain of
+// dependent loads (index -> slot of the packed record -> record), so it runs as a three-stage pipeline ahead of
+// the math: while layer l is fitted, the hit of layer l + 1 is being fetched, the slot of layer l + 2 resolved
+// and the index of layer l + 3 read -- every stage has a whole layer of arithmetic to hide behind.
+__device__ __forceinline__ int32_t resolve_hit(const IndexedPools& H, int l, int32_t h) {
+    if (h < 0) return -1;
+    return H.use_records ? __ldg(H.orig_to_sorted[l] + h) : h;
+}
+__device__ __forceinline__ Hit fetch_hit(const IndexedPools& H, int l, int32_t s) {
     Hit m;
-    if (H.use_records) {   // one 4-byte look-up + one 48-byte record (3 sectors) instead of 9 scattered sectors
-        const int32_t s = __ldg(H.orig_to_sorted[l] + h);
+    if (H.use_records) {   // one 48-byte record (2 sectors) instead of 9 scattered sectors
         const float4* r = reinterpret_cast<const float4*>(H.hit_rec[l]) + (int64_t)s * 3;
         const float4 A = __ldg(r), B = __ldg(r + 1), C = __ldg(r + 2);
         m.x = A.x; m.y = A.y; m.z = A.z; m.vzz = A.w; m.vxx = B.x; m.vxy = B.y; m.vyy = B.z; m.vxz = C.x; m.vyz = C.y;
@@ -737,9 +743,9 @@ __device__ __forceinline__ Hit gather_hit(const IndexedPools& H, int l, int32_t 
     const float* p = H.pos[l];
     const float* c = H.cov[l];
     const int64_t ld = H.ld[l];
-    m.x = __ldg(p + h);            m.y = __ldg(p + ld + h);       m.z = __ldg(p + 2 * ld + h);
-    m.vxx = __ldg(c + h);          m.vxy = __ldg(c + ld + h);     m.vxz = __ldg(c + 2 * ld + h);
-    m.vyy = __ldg(c + 3 * ld + h); m.vyz = __ldg(c + 4 * ld + h); m.vzz = __ldg(c + 5 * ld + h);
+    m.x = __ldg(p + s);            m.y = __ldg(p + ld + s);       m.z = __ldg(p + 2 * ld + s);
+    m.vxx = __ldg(c + s);          m.vxy = __ldg(c + ld + s);     m.vxz = __ldg(c + 2 * ld + s);
+    m.vyy = __ldg(c + 3 * ld + s); m.vyz = __ldg(c + 4 * ld + s); m.vzz = __ldg(c + 5 * ld + s);
     return m;
 }
 
@@ -760,16 +766,19 @@ fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ 
         const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
         enter_local_frame(t);
         bool started = false;
-        int32_t h_next = __ldg(H.index + i);
+        // pipeline registers: raw index of layer l + 2, slot of layer l + 1, hit of layer l
+        int32_t h2 = L > 2 ? __ldg(H.index + 2 * H.ld_index + i) : -1;
+        int32_t s1 = L > 1 ? resolve_hit(H, 1, __ldg(H.index + H.ld_index + i)) : -1;
+        int32_t s0 = resolve_hit(H, 0, __ldg(H.index + i));
         Hit m_next;
-        if (h_next >= 0) m_next = gather_hit(H, 0, h_next);
+        if (s0 >= 0) m_next = fetch_hit(H, 0, s0);
         for (int l = 0; l < L; ++l) {
-            const int32_t h = h_next;
+            const int32_t h = s0;
             const Hit m = m_next;
-            if (l + 1 < L) {
-                h_next = __ldg(H.index + (int64_t)(l + 1) * H.ld_index + i);
-                if (h_next >= 0) m_next = gather_hit(H, l + 1, h_next);
-            }
+            s0 = s1;
+            if (s0 >= 0) m_next = fetch_hit(H, l + 1, s0);
+            s1 = l + 2 < L ? resolve_hit(H, l + 2, h2) : -1;
+            h2 = l + 3 < L ? __ldg(H.index + (int64_t)(l + 3) * H.ld_index + i) : -1;
             if (h < 0) continue;
             uint32_t rc;
             if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.model, P.mass2, P.el, m, chi2);

@@ -413,6 +413,41 @@ def run_ours(args) -> None:
                    "records_ms": ixr_ms, "records_fits_per_s": n / (ixr_ms * 1e-3),
                    "note": "nine scattered 4-byte loads per hit: bound by 32-byte DRAM/L2 sectors, not by arithmetic"}
         del pools, perm, index
+        # secondary: the other fit configs of BASELINE.json (0, 1: one event, launch-bound; 3: 100 000 tracks x 20
+        # layers), one kf_fit_tracks call each, eager through the binding and replayed from a recorded graph
+        from workloads import barrel_events as W
+        other_configs = {}
+        for ci in (0, 1, 3):
+            bc = W.make_fit_batch(ci)
+            dcf = DeviceFit.from_batch(bc, dev)
+            Lc = int(bc.radius.shape[0])
+            with torch.cuda.stream(stream):
+                for _ in range(3):
+                    dcf.fit(ctx)
+                c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                c0.record(stream)
+                for _ in range(50):
+                    dcf.fit(ctx)
+                c1.record(stream)
+                torch.cuda.synchronize()
+                ctx.graph_begin()
+                dcf.fit(ctx)
+                gr = ctx.graph_end()
+                gr.launch()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record(stream)
+                for _ in range(50):
+                    gr.launch()
+                g1.record(stream)
+            torch.cuda.synchronize()
+            gr.close()
+            e_ms, g_ms = c0.elapsed_time(c1) / 50, g0.elapsed_time(g1) / 50
+            bound_ms = 1e3 * max(bc.n * FLOPS_PER_TRACK_LAYER * Lc / (fp32_peak * 1e12),
+                                 bc.n * (233 + 36 * Lc) / (_peaks()[0] * 1e9))
+            other_configs[f"configs[{ci}]"] = {"tracks": int(bc.n), "n_layers": Lc, "eager_ms": e_ms, "graph_ms": g_ms,
+                                               "fits_per_s": bc.n / (g_ms * 1e-3), "bound_ms": bound_ms,
+                                               "roofline_frac": bound_ms / g_ms}
+            del dcf, bc
         smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10)", "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3),
                      "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0],
                      "alu_roofline_frac": 2.0 * n * FLOPS_PER_TRACK_LAYER * L / (sm_ms * 1e-3) / (fp32_peak * 1e12)}
@@ -456,6 +491,7 @@ def run_ours(args) -> None:
             out["smoothing"] = smoothing
             out["indexed_fit"] = indexed
             out["geometry_options"] = geometry
+            out["other_configs"] = other_configs
         print(json.dumps(out), flush=True)
     ctx.close()
     sharding.shutdown()

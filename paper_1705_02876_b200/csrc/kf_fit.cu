@@ -21,6 +21,8 @@
 // chi2, nhits, status) + 36 per layer = 593 B at 10 layers.
 #include <cuda.h>
 
+#include <cstdlib>
+
 #include "kf_internal.h"
 
 namespace kf {
@@ -863,7 +865,8 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     const bool smooth = a.spar != nullptr;
     const int L = P.n_layers;
     FitMaps M;
-    if (P.geometry_options == 0 && a.n >= (int64_t)KF_PAIR_MIN_TRACKS && (!smooth || KF_PAIR_SMOOTH)) {   // two tracks per thread
+    static const int64_t pair_min = [] { const char* e = getenv("KF_PAIR_MIN_TRACKS"); return e ? (int64_t)atoll(e) : (int64_t)KF_PAIR_MIN_TRACKS; }();
+    if (P.geometry_options == 0 && a.n >= pair_min && (!smooth || KF_PAIR_SMOOTH)) {   // two tracks per thread
         static const cudaError_t attr_pair = [] {
             cudaError_t e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
             if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));

@@ -20,7 +20,8 @@
 // ascending index IS the stable order: the arrival order, which differs from run to run, never shows) and moves
 // its record to its final place: a packed 12-float record per hit for the scoring kernel
 // (x y z vzz | vxx vxy vyy index | vxz vyz 0 0: the first 128-bit word serves the z pre-filter,
-// the second the tangential one, the third only full evaluations) and, optionally, SoA copies; (5) per-bin boxes.
+// the second the tangential one, the third only full evaluations); (5) a warp per bin reads the final records and
+// writes the optional SoA copies (coalesced) and the per-bin boxes.
 // Every read of the inputs is coalesced; the only scattered traffic is one 48-byte record per hit in step (3).
 #include <cmath>
 
@@ -155,7 +156,7 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     int32_t rank = 0;
     for (int32_t j = s; j < e; ++j) rank += (__ldg(L.unsorted + j) < mine) ? 1 : 0;
     const int64_t dst = (int64_t)s + rank;
-    L.sorted_to_orig[dst] = mine;
+    if (!L.hit_rec) L.sorted_to_orig[dst] = mine;   // else from the record's index word, coalesced (bin_finish_kernel)
     if (L.orig_to_sorted) L.orig_to_sorted[mine] = (int32_t)dst;
     if (!L.rec_tmp) return;  // ordering only (candidates)
     const float4* src = reinterpret_cast<const float4*>(L.rec_tmp + p * 12);
@@ -166,6 +167,7 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
         rec[1] = Bw;
         rec[2] = C;
     }
+    if (L.hit_rec) return;   // the SoA copies are then written from the final records, coalesced (bin_finish_kernel)
     if (L.pos_sorted) {
         L.pos_sorted[dst] = A.x; L.pos_sorted[L.ld_out + dst] = A.y; L.pos_sorted[2 * L.ld_out + dst] = A.z;
     }
@@ -176,13 +178,15 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     }
 }
 
-// Per-bin bounds for the scan's bin pruning: bounding box of the hits of the bin and the largest
-// v_zz and v_xx + v_yy (>= the tangential variance in any frame).  One warp per bin, no atomics.
-// NaN components are ignored (such a hit can never pass a chi2 bound either).  Empty bin: lo = +inf.
+// Last step, one warp per bin over the final records: sorted_to_orig and the optional SoA copies (the scattered
+// store path of an SM is what bounds the sort, so they are written here, where a warp holds CONSECUTIVE slots,
+// instead of ten scattered 4-byte stores per hit in the rank step) and the per-bin bounds for the scan's bin pruning: bounding
+// box of the hits of the bin and the largest v_zz and v_xx + v_yy (>= the tangential variance in any frame).
+// No atomics.  NaN components are ignored (such a hit can never pass a chi2 bound either).  Empty bin: lo = +inf.
 __global__ void __launch_bounds__(kBlock)
-bin_box_kernel(const __grid_constant__ BinBatch B) {
+bin_finish_kernel(const __grid_constant__ BinBatch B) {
     const BinLayerDev& L = B.layer[blockIdx.y];
-    if (!L.bin_box || !L.hit_rec) return;
+    if (!L.hit_rec) return;
     const int lane = threadIdx.x & 31;
     const int b = (int)((blockIdx.x * (unsigned)kBlock + threadIdx.x) >> 5);
     if (b >= B.n_eta * B.n_phi) return;
@@ -192,6 +196,16 @@ bin_box_kernel(const __grid_constant__ BinBatch B) {
     const float4* rec = reinterpret_cast<const float4*>(L.hit_rec);
     for (int32_t s = s0 + lane; s < s1; s += 32) {
         const float4 A = rec[(int64_t)s * 3], Bw = rec[(int64_t)s * 3 + 1];
+        L.sorted_to_orig[s] = __float_as_int(Bw.w);
+        if (L.pos_sorted) {
+            L.pos_sorted[s] = A.x; L.pos_sorted[L.ld_out + s] = A.y; L.pos_sorted[2 * L.ld_out + s] = A.z;
+        }
+        if (L.cov_sorted) {   // xx xy xz yy yz zz
+            const float4 C = rec[(int64_t)s * 3 + 2];
+            L.cov_sorted[s] = Bw.x;                 L.cov_sorted[L.ld_out + s] = Bw.y;
+            L.cov_sorted[2 * L.ld_out + s] = C.x;   L.cov_sorted[3 * L.ld_out + s] = Bw.z;
+            L.cov_sorted[4 * L.ld_out + s] = C.y;   L.cov_sorted[5 * L.ld_out + s] = A.w;
+        }
         xl = fminf(xl, A.x); xh = fmaxf(xh, A.x); yl = fminf(yl, A.y); yh = fmaxf(yh, A.y);
         zl = fminf(zl, A.z); zh = fmaxf(zh, A.z); vz = fmaxf(vz, A.w); vt = fmaxf(vt, Bw.x + Bw.z);
     }
@@ -202,7 +216,7 @@ bin_box_kernel(const __grid_constant__ BinBatch B) {
         zl = fminf(zl, __shfl_xor_sync(0xffffffffu, zl, d)); zh = fmaxf(zh, __shfl_xor_sync(0xffffffffu, zh, d));
         vz = fmaxf(vz, __shfl_xor_sync(0xffffffffu, vz, d)); vt = fmaxf(vt, __shfl_xor_sync(0xffffffffu, vt, d));
     }
-    if (lane == 0) {
+    if (lane == 0 && L.bin_box) {
         float4* o = reinterpret_cast<float4*>(L.bin_box + (int64_t)b * 8);
         o[0] = make_float4(xl, xh, yl, yh);
         o[1] = make_float4(zl, zh, vz, vt);
@@ -346,7 +360,7 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
             bin_scatter_kernel<<<grid, kBlock, 0, stream>>>(B);
             bin_rank_gather_kernel<<<grid, kBlock, 0, stream>>>(B);
         }
-        bin_box_kernel<<<dim3((unsigned)((nb * 32 + kBlock - 1) / kBlock), (unsigned)m), kBlock, 0, stream>>>(B);
+        bin_finish_kernel<<<dim3((unsigned)((nb * 32 + kBlock - 1) / kBlock), (unsigned)m), kBlock, 0, stream>>>(B);
     }
     return cudaGetLastError();
 }

@@ -92,6 +92,18 @@ def test_bin_hits_edge_cases(ctx):
         _assert_bins_equal(dl, ob, pos, cov[:, :3000])
 
 
+def test_bin_hits_large_layer(ctx):
+    """A layer of 700 000 hits with a full 3 x 3 covariance each (every output plane distinguishable)."""
+    H = 700_000
+    rng = np.random.default_rng(12)
+    r = 20.0
+    phi, eta = rng.uniform(-np.pi, np.pi, H), rng.uniform(-1.3, 1.3, H)
+    pos = np.stack([r * np.cos(phi), r * np.sin(phi), r * np.sinh(eta)]).astype(np.float32)
+    cov = rng.uniform(1e-4, 1e-2, (6, H)).astype(np.float32)
+    dl, ob = _bin_both(ctx, pos, cov, r)
+    _assert_bins_equal(dl, ob, pos, cov)
+
+
 def test_bin_layers_batched_equals_per_layer(ctx):
     """kf_bin_layers (all layers in four launches) == kf_bin_hits layer by layer == oracle."""
     from paper_1705_02876_b200.buffers import DeviceLayer

@@ -186,10 +186,11 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         tma_load_2d(seed0 + 6 * 128, &M.cov, col, 0, bar0 + 8u * kStages);
 #pragma unroll
         for (int s = 0; s < kStages; ++s)
-            if (s < L) {
+            if (s < (SMOOTH ? 2 * L : L)) {   // fewer layers than stages: the ring's first round already turns back
+                const int ls = s < L ? s : 2 * L - 1 - s;
                 mbar_expect_tx(bar0 + 8u * s, kHitFloats * 4);
-                tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * s, bar0 + 8u * s);
-                tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * s, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHitFloats * 4), &M.hpos, col, 3 * ls, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHitFloats * 4) + 3 * 128, &M.hcov, col, 6 * ls, bar0 + 8u * s);
             }
     }
     __syncwarp();
@@ -510,10 +511,11 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
         tma_load_2d(seed0 + 6 * kRowBytes, &M.cov, col, 0, bar0 + 8u * kStages);
 #pragma unroll
         for (int s = 0; s < kStages; ++s)
-            if (s < L) {
+            if (s < (SMOOTH ? 2 * L : L)) {   // fewer layers than stages: the ring's first round already turns back
+                const int ls = s < L ? s : 2 * L - 1 - s;
                 mbar_expect_tx(bar0 + 8u * s, kHit2Floats * 4);
-                tma_load_2d(hit0 + s * (kHit2Floats * 4), &M.hpos, col, 3 * s, bar0 + 8u * s);
-                tma_load_2d(hit0 + s * (kHit2Floats * 4) + 3 * kRowBytes, &M.hcov, col, 6 * s, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4), &M.hpos, col, 3 * ls, bar0 + 8u * s);
+                tma_load_2d(hit0 + s * (kHit2Floats * 4) + 3 * kRowBytes, &M.hcov, col, 6 * ls, bar0 + 8u * s);
             }
     }
     __syncwarp();

@@ -65,6 +65,20 @@ def test_fit_ragged_sizes(ctx, n):
     compare_fit(g, o, float(b.radius[-1]), max_diverged_frac=1.0)
 
 
+@pytest.mark.parametrize("n_layers,step,n", [(32, 2.5, 3000), (32, 2.5, 160_000), (1, 4.0, 700), (2, 4.0, 700)])
+def test_fit_extreme_layer_counts(ctx, n_layers, step, n):
+    """KF_MAX_LAYERS = 32 layers (mask bit 31 in use; 160 000 tracks take the pair kernel, 3 000 the one-track
+    kernel) and the shortest geometries (one and two layers: the fit is one or two updates of the seed)."""
+    import dataclasses
+    cfg = dataclasses.replace(W.get_config(3), n_layers=n_layers, layer_step_cm=step, n_tracks=n)
+    b = W.simulate_event(cfg, 21, n_tracks=n)
+    assert b.n_layers == n_layers and (n_layers < 32 or int(b.mask.max()) >> 31 == 1)
+    g = _gpu_fit(ctx, b)
+    o = O.fit_batch(b)
+    compare_fit(g, o, float(b.radius[-1]), max_diverged_frac=1e-3 if n_layers > 2 else 1.0)
+    assert np.array_equal(g["nhits"], o["nhits"]) and np.array_equal(g["status"], o["status"])
+
+
 def test_fit_empty(ctx):
     b = W.simulate_event(W.get_config(1), 5, n_tracks=4)
     from paper_1705_02876_b200.buffers import DeviceFit

@@ -27,8 +27,8 @@ def _both(ctx, b, kappa=O.SMOOTH_KAPPA):
     return d, o
 
 
-def _compare(d, o, r_last, max_div=1e-3):
-    fwd = compare_fit(d.results(), {k: o[k] for k in ("par", "cov", "chi2", "nhits", "status")}, r_last, max_div)
+def _compare(d, o, r_last, max_div=1e-3, loosen=None):
+    fwd = compare_fit(d.results(), {k: o[k] for k in ("par", "cov", "chi2", "nhits", "status")}, r_last, max_div, loosen)
     sg = d.smoothed_results()
     assert np.array_equal(sg["status"], o["sstatus"])
     # Smoothed result, same metric.  Excluded (A14): tracks the FORWARD fit flagged or that diverged there, and
@@ -37,7 +37,7 @@ def _compare(d, o, r_last, max_div=1e-3):
     fwd_div = o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)
     excl = o["status"] | o["sstatus"] | (fwd_div.astype(np.uint32) << 4)
     so = dict(par=o["spar"], cov=o["scov"], chi2=o["schi2"], nhits=o["nhits"], status=excl)
-    sm = compare_fit(dict(sg, status=excl, nhits=o["nhits"]), so, r_last, max_diverged_frac=max(max_div, 2e-3))
+    sm = compare_fit(dict(sg, status=excl, nhits=o["nhits"]), so, r_last, max_diverged_frac=max(max_div, 2e-3), loosen=loosen)
     return fwd, sm
 
 
@@ -47,6 +47,25 @@ def test_smooth_parity_full_config(ctx, config):
     d, o = _both(ctx, b)
     fwd, sm = _compare(d, o, float(b.radius[-1]))
     print(f"config {config}: forward {fwd}\n          smoothed {sm}")
+
+
+@pytest.mark.parametrize("n_layers,step,n", [(32, 2.5, 3000), (32, 2.5, 160_000), (1, 4.0, 700), (2, 4.0, 700), (3, 4.0, 700),
+                                             (3, 4.0, 160_000)])
+def test_smooth_extreme_layer_counts(ctx, n_layers, step, n):
+    """KF_MAX_LAYERS layers (64 steps of the hit ring; pair and one-track kernels) and geometries with fewer layers
+    than the hit ring has stages, where the ring's first round already holds steps of the backward pass (one
+    layer: the refit is a single update of the inflated forward result)."""
+    import dataclasses
+    # short geometries with config-1 kinematics: three hits barely constrain a 0.3 GeV track at |eta| = 1.5
+    cfg = dataclasses.replace(W.get_config(3 if n_layers > 3 else 1), n_layers=n_layers, layer_step_cm=step, n_tracks=n)
+    b = W.simulate_event(cfg, 22, n_tracks=n)
+    d, o = _both(ctx, b)
+    # Three hits barely constrain |p| (5 parameters from 6 good coordinates): the fit is ill-conditioned and the
+    # worst of 160 000 such tracks reaches 2.2e-4 relative on the momentum in fp32 (99 % stay below 0.2e-4), so the
+    # short geometries are held to 4 x the momentum tolerance (DESIGN.md, known limits).
+    fwd, sm = _compare(d, o, float(b.radius[-1]), max_div=1e-3 if n_layers > 3 else 1.0,
+                       loosen={"mom": 4.0} if n_layers <= 3 else None)
+    assert n_layers > 3 or (fwd["mom_p99"] <= 0.5 and sm["mom_p99"] <= 0.5)
 
 
 def test_smooth_forward_part_equals_plain_fit(ctx):

@@ -26,7 +26,8 @@ def ctx():
     c.close()
 
 
-def _run(ctx, n_tracks, noise, n_cand, half_length=None, material_model=0, energy_loss=0):
+def _run(ctx, n_tracks, noise, n_cand, half_length=None, material_model=0, energy_loss=0, first=3):
+    """Seeds = oracle fit of the first three true hits; building runs on layers first..9."""
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
     ev = W.make_build_event(4, n_tracks=n_tracks, noise_hits=noise)
@@ -34,14 +35,14 @@ def _run(ctx, n_tracks, noise, n_cand, half_length=None, material_model=0, energ
     r = O.fit_tracks(f.radius[:3], f.x_over_X0[:3], f.Bz, f.mass, f.par, f.cov, f.q, f.hpos[:3], f.hcov[:3], None, nthreads=8)
     par, cov = r["par"].astype(np.float32), O.pack_cov21(r["cov"]).astype(np.float32)
     geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, half_length, material_model, energy_loss)
-    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers[3:]]
-    ctx.bin_layers([l.radius for l in ev.layers[3:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers[first:]]
+    ctx.bin_layers([l.radius for l in ev.layers[first:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
     dc = DeviceCandidates.from_numpy(par, cov, f.q, r["chi2"], r["nhits"], "cuda:0")
-    idx, nf = dc.build_combinatorial(ctx, geom, 3, dls, n_cand)
+    idx, nf = dc.build_combinatorial(ctx, geom, first, dls, n_cand)
     torch.cuda.synchronize()
-    layers = [(l.pos, l.cov, O.bin_hits(l.pos, l.radius, NE, NP, EMAX)) for l in ev.layers[3:]]
+    layers = [(l.pos, l.cov, O.bin_hits(l.pos, l.radius, NE, NP, EMAX)) for l in ev.layers[first:]]
     with O.geometry_options(material_model, half_length, energy_loss=energy_loss):
-        o = O.build_combinatorial(f.radius, f.x_over_X0, f.Bz, f.mass, par, cov, f.q, r["chi2"], r["nhits"], 3, layers,
+        o = O.build_combinatorial(f.radius, f.x_over_X0, f.Bz, f.mass, par, cov, f.q, r["chi2"], r["nhits"], first, layers,
                                   NE, NP, EMAX, 2, 30.0, n_cand)
     return ev, dc.results(), idx.cpu().numpy()[:, :f.n], nf.cpu().numpy()[:f.n], o
 

@@ -331,16 +331,25 @@ def run_ours(args) -> None:
     smoothing = None
     if rank == 0 and not args.no_building:
         # secondary: kf_fit_tracks_smooth on the same batch (forward fit + inward refit, one kernel)
-        with torch.cuda.stream(stream):
-            for _ in range(3):
-                d.fit_smooth(ctx)
-            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            s0.record(stream)
-            for _ in range(20):
-                d.fit_smooth(ctx)
-            s1.record(stream)
-        torch.cuda.synchronize()
-        sm_ms = s0.elapsed_time(s1) / 20
+        # Every track of configs[2] has all 10 hits, which the API states by passing no mask: the call then takes
+        # the two-tracks-per-thread smoother.  With a mask it takes the one-track kernel (ragged pairs would cost
+        # the pair form more than it gains); both are timed.
+        def time_smooth():
+            with torch.cuda.stream(stream):
+                for _ in range(3):
+                    d.fit_smooth(ctx)
+                s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                s0.record(stream)
+                for _ in range(20):
+                    d.fit_smooth(ctx)
+                s1.record(stream)
+            torch.cuda.synchronize()
+            return s0.elapsed_time(s1) / 20
+        sm_masked_ms = time_smooth()
+        full_mask, d.mask = d.mask, None
+        sm_ms = time_smooth()
+        d.mask = full_mask
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         sm_bytes = n * (113 + 2 * 36 * L + 2 * 120)
         # secondary: the same fit with the geometry options of reading A20 (path-length material, 30 cm barrels)
         import paper_1705_02876_b200 as K
@@ -448,7 +457,8 @@ def run_ours(args) -> None:
                                                "fits_per_s": bc.n / (g_ms * 1e-3), "bound_ms": bound_ms,
                                                "roofline_frac": bound_ms / g_ms}
             del dcf, bc
-        smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10)", "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3),
+        smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10), mask = NULL: every track has every hit",
+                     "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3), "with_mask_ms": sm_masked_ms,
                      "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0],
                      "alu_roofline_frac": 2.0 * n * FLOPS_PER_TRACK_LAYER * L / (sm_ms * 1e-3) / (fp32_peak * 1e12)}
 

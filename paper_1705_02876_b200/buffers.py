@@ -69,11 +69,13 @@ class DeviceFit:
 
     def fit_smooth(self, ctx: KFContext, kappa: float = 10.0) -> dict:
         """kf_fit_tracks_smooth; the forward result lands in the usual out_* tensors, the smoothed one in
-        freshly allocated tensors returned (and kept) as self.smoothed."""
+        tensors allocated at the first call, returned and kept as self.smoothed (later calls write into them)."""
         dev = self.par.device
-        mk = lambda shape, dt: torch.zeros(shape, dtype=dt, device=dev)
-        sm = dict(par=mk((6, self.ld), torch.float32), cov=mk((21, self.ld), torch.float32),
-                  chi2=mk((self.ld,), torch.float32), nhits=mk((self.ld,), torch.int32), status=mk((self.ld,), torch.int32))
+        sm = getattr(self, "smoothed", None)
+        if sm is None:
+            mk = lambda shape, dt: torch.zeros(shape, dtype=dt, device=dev)
+            sm = dict(par=mk((6, self.ld), torch.float32), cov=mk((21, self.ld), torch.float32),
+                      chi2=mk((self.ld,), torch.float32), nhits=mk((self.ld,), torch.int32), status=mk((self.ld,), torch.int32))
         ctx.fit_tracks_smooth(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask, kappa,
                               self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status,
                               sm["par"], sm["cov"], sm["chi2"], sm["nhits"], sm["status"])

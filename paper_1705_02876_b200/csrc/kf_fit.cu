@@ -354,7 +354,8 @@ constexpr int kPairTile = 64;                      // tracks per warp
 constexpr int kHit2Floats = 9 * kPairTile;
 constexpr int kSeed2Floats = 27 * kPairTile;
 constexpr int kPark2Floats = 30 * 32;              // one parked track (29 values + chi2) per lane (ragged pairs)
-// (the smoother kernel has no park area: it spills a little and wants the shared-memory space as L1)
+// (the smoother kernel has no park area: it spills a little and needs the shared-memory space as L1 -- with the
+// park area its 92 KB of spill working set per SM no longer fit and the kernel ran 17 % slower on full pairs)
 __host__ __device__ constexpr int warp2_floats(bool smooth) { return kStages * kHit2Floats + kSeed2Floats + (smooth ? 0 : kPark2Floats); }
 constexpr int smem2_bytes(bool smooth) { return kPairWarps * warp2_floats(smooth) * 4 + kPairWarps * (kStages + 1) * 8; }
 
@@ -392,8 +393,11 @@ __device__ __forceinline__ bool fit_layer_pair(Track2& t, f2 k, f2 ik, const Lay
 }
 
 // A layer only ONE track of the pair has a hit on: the idle one's 29 values (and its chi2) are parked in shared
-// memory, its slot of the hit stage is overwritten with a harmless hit (origin, unit covariance) so that its
-// arithmetic passes, the pair arithmetic runs for both, and the idle half is put back.
+// memory and its half of the pair becomes a SHADOW of the active track (same state, same charge, same hit), so
+// that the pair arithmetic passes exactly when the active track's does; afterwards the idle half is put back.
+// (A harmless hit alone is not enough: a track that has stopped short of the layer -- the usual reason for a
+// ragged pair -- cannot be propagated there, and its failure would send the pair down the one-track path on
+// every remaining layer.)
 #define KF_TRACK_FIELDS(X)                                                                              \
     X(x) X(y) X(z) X(px) X(py) X(pz) X(eax) X(eay) X(c00) X(c01) X(c02) X(c03) X(c04) X(c05) X(c11) X(c12) \
     X(c13) X(c14) X(c15) X(c22) X(c23) X(c24) X(c25) X(c33) X(c34) X(c35) X(c44) X(c45) X(c55)
@@ -403,6 +407,20 @@ __device__ __forceinline__ void park_component(const Track2& t, float* scr) {
 #define KF_PARK(f) scr[32 * r++] = C ? t.f.v.y : t.f.v.x;
     KF_TRACK_FIELDS(KF_PARK)
 #undef KF_PARK
+}
+template <int C>
+__device__ __forceinline__ void shadow_component(Track2& t) {   // component C := the other one
+#define KF_SHADOW(f) if (C) t.f.v.y = t.f.v.x; else t.f.v.x = t.f.v.y;
+    KF_TRACK_FIELDS(KF_SHADOW)
+#undef KF_SHADOW
+}
+// The idle track's slot of the hit stage := the active track's hit.
+__device__ __forceinline__ void shadow_hit(const float2* tp, int idle) {
+    float* hp = const_cast<float*>(reinterpret_cast<const float*>(tp));   // this lane's two slots
+#pragma unroll
+    for (int r = 0; r < 9; ++r) hp[r * kPairTile + idle] = hp[r * kPairTile + (idle ^ 1)];
+    // ordered before the TMA refill of this stage (issued by another lane after a __syncwarp)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 template <int C>
 __device__ __forceinline__ void unpark_component(Track2& t, const float* scr) {
@@ -554,24 +572,23 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
         const float2* tp = reinterpret_cast<const float2*>(wbase + s * kHit2Floats) + lane;
         const mask2 want = {live.x && ((mx >> l) & 1u), live.y && ((my >> l) & 1u)};
         bool both = false;
-        // (the smoother kernel, at the edge of its register budget, leaves ragged pairs to the one-track path)
+        // (the smoother kernel leaves ragged pairs to the one-track path: see warp2_floats; launch_fit therefore
+        // takes it only for batches whose tracks all have every hit)
         if (SMOOTH ? all_of(want) : !none_of(want)) {
             const bool ragged = !SMOOTH && !all_of(want);
             const int idle = want.x ? 1 : 0;
+            f2 kk = k, ikk = ik;
             if constexpr (!SMOOTH) {
                 if (ragged) {
-                    if (idle) park_component<1>(t, park); else park_component<0>(t, park);
+                    if (idle) { park_component<1>(t, park); shadow_component<1>(t); kk.v.y = k.v.x; ikk.v.y = ik.v.x; }
+                    else { park_component<0>(t, park); shadow_component<0>(t); kk.v.x = k.v.y; ikk.v.x = ik.v.y; }
                     park[29 * 32] = idle ? chi2.v.y : chi2.v.x;
-                    float* hp = const_cast<float*>(reinterpret_cast<const float*>(tp)) + idle;   // this lane's own slot
-#pragma unroll
-                    for (int r = 0; r < 9; ++r) hp[r * kPairTile] = (r == 3 || r == 6 || r == 8) ? 1.0f : 0.0f;
-                    // ordered before the TMA refill of this stage (issued by another lane after the __syncwarp below)
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    shadow_hit(tp, idle);
                 }
             }
             // (the general transport is also right for a track whose radial row is already zero)
-            if (all_of(started | !want)) both = fit_layer_pair<true>(t, k, ik, P.layer[l], P.mass2, tp, chi2);
-            else both = fit_layer_pair<false>(t, k, ik, P.layer[l], P.mass2, tp, chi2);
+            if (all_of(started | !want)) both = fit_layer_pair<true>(t, kk, ikk, P.layer[l], P.mass2, tp, chi2);
+            else both = fit_layer_pair<false>(t, kk, ikk, P.layer[l], P.mass2, tp, chi2);
             if constexpr (!SMOOTH) {
                 if (ragged) {
                     if (idle) { unpark_component<1>(t, park); chi2.v.y = park[29 * 32]; }
@@ -868,7 +885,14 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     const int L = P.n_layers;
     FitMaps M;
     static const int64_t pair_min = [] { const char* e = getenv("KF_PAIR_MIN_TRACKS"); return e ? (int64_t)atoll(e) : (int64_t)KF_PAIR_MIN_TRACKS; }();
-    if (P.geometry_options == 0 && a.n >= pair_min && (!smooth || KF_PAIR_SMOOTH)) {   // two tracks per thread
+    // Two tracks per thread.  The pair form of the smoother takes ragged pairs (a layer only one of the two tracks
+    // has a hit on) through the one-track path and then loses badly (1.2 % of tracks stopping short: 0.81 ms against
+    // 0.49 ms for 600 000 twenty-layer tracks), so it is taken only where the caller says that every track has
+    // every hit (mask == NULL); the pair form of the fit parks and shadows the idle track and wins either way.
+    // (KF_PAIR_SMOOTH_MASKED in the environment lifts that condition: the tests use it to drive the pair smoother's
+    // ragged-pair code, which failures can reach without any mask, with masks.)
+    if (P.geometry_options == 0 && a.n >= pair_min &&
+        (!smooth || (KF_PAIR_SMOOTH && (a.mask == nullptr || getenv("KF_PAIR_SMOOTH_MASKED") != nullptr)))) {
         static const cudaError_t attr_pair = [] {
             cudaError_t e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
             if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));

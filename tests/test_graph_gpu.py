@@ -94,6 +94,8 @@ def test_fit_and_smooth_graph_equals_eager(ctx):
     d.fit_smooth(ctx)
     g = ctx.graph_end()
     d.out_par.zero_(); d.out_cov.zero_(); d.out_chi2.zero_()
+    for v in d.smoothed.values():                 # (fit_smooth writes into the same tensors at every call)
+        v.zero_()
     torch.cuda.synchronize()
     g.launch()
     g.launch()                                    # a graph may be launched any number of times

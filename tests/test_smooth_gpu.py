@@ -18,9 +18,9 @@ def ctx():
     c.close()
 
 
-def _both(ctx, b, kappa=O.SMOOTH_KAPPA):
+def _both(ctx, b, kappa=O.SMOOTH_KAPPA, with_mask=True):
     from paper_1705_02876_b200.buffers import DeviceFit
-    d = DeviceFit.from_batch(b, "cuda:0")
+    d = DeviceFit.from_batch(b, "cuda:0", with_mask=with_mask)
     d.fit_smooth(ctx, kappa)
     torch.cuda.synchronize()
     o = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask, kappa=kappa)
@@ -51,7 +51,8 @@ def test_smooth_parity_full_config(ctx, config):
 
 @pytest.mark.parametrize("n_layers,step,n", [(32, 2.5, 3000), (32, 2.5, 160_000), (1, 4.0, 700), (2, 4.0, 700), (3, 4.0, 700),
                                              (3, 4.0, 160_000)])
-def test_smooth_extreme_layer_counts(ctx, n_layers, step, n):
+def test_smooth_extreme_layer_counts(ctx, n_layers, step, n, monkeypatch):
+    monkeypatch.setenv("KF_PAIR_SMOOTH_MASKED", "1")     # large masked batches through the pair smoother too
     """KF_MAX_LAYERS layers (64 steps of the hit ring; pair and one-track kernels) and geometries with fewer layers
     than the hit ring has stages, where the ring's first round already holds steps of the backward pass (one
     layer: the refit is a single update of the inflated forward result)."""
@@ -97,9 +98,26 @@ def test_smooth_ragged_masks_and_flags(ctx):
     assert np.all(sg["chi2"][:31] == 0)
 
 
-def test_smooth_pair_kernel_edge_cases(ctx):
-    """Batches of >= 151 552 tracks take the two-tracks-per-thread kernel, also for fit + smoother; pairs whose
-    tracks used different layers (or where one fails) go through the one-track refit step."""
+def test_smooth_pair_kernel_without_mask(ctx):
+    """The product's rule: a batch of >= 151 552 tracks WITHOUT a mask (every track has every hit) takes the
+    two-tracks-per-thread smoother; with a mask the one-track kernel.  Same results within the tolerances, and
+    the masked call (all bits set) agrees with the oracle too."""
+    cfg = W.get_config(1)
+    b = W.concat_batches([W.simulate_event(cfg, 70 + e) for e in range(8)] + [W.simulate_event(cfg, 78, n_tracks=5)])
+    assert b.n == 160_005 and np.all(b.mask == 0x3ff)
+    d, o = _both(ctx, b, with_mask=False)
+    _compare(d, o, float(b.radius[-1]))
+    d2, _ = _both(ctx, b, with_mask=True)
+    _compare(d2, o, float(b.radius[-1]))
+    np.testing.assert_allclose(d.smoothed_results()["chi2"], d2.smoothed_results()["chi2"], rtol=2e-3, atol=2e-3)
+
+
+def test_smooth_pair_kernel_edge_cases(ctx, monkeypatch):
+    """The two-tracks-per-thread smoother on ragged pairs: pairs whose tracks used different layers (or where one
+    fails) go through the one-track refit step.  (With a mask the product takes the one-track kernel; the
+    environment switch sends this masked batch through the pair kernel so that its ragged-pair code, which failures
+    reach without any mask, is covered.)"""
+    monkeypatch.setenv("KF_PAIR_SMOOTH_MASKED", "1")
     cfg = W.get_config(1)
     b = W.concat_batches([W.simulate_event(cfg, 50 + e) for e in range(8)] + [W.simulate_event(cfg, 58, n_tracks=3)])
     assert b.n == 160_003

@@ -31,7 +31,7 @@ UNIT = "fits/s"
 CONFIG_INDEX = 2
 # dram__bytes_read.sum + dram__bytes_write.sum of fit_pair_kernel for one 2M-track launch, from the
 # `ncu --set full` capture summarised in profiles/r01_fit_pair_kernel.md.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 946051328 + 219575040   # profiles/r01_fit_pair_kernel.md
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 946051584 + 219393024   # profiles/r01_fit_pair_kernel.md (last capture, launch 5)
 # Algorithmic flops per track and layer of the filter as the oracle states it, exploiting the known zeros and
 # ones of F and H and symmetry: propagation 75, Jacobian 95, F C F^T 340,
 # Q 35, update 310 (S 9, S^-1 30, chi2 21, K 90, x 36, C 126) -- frozen before any tuning.

@@ -72,12 +72,12 @@ def test_indexed_fit_short_geometries(ctx, k, n_tracks):
         compare_fit(g, o, float(ev.fit.radius[-1]), max_diverged_frac=1.0, loosen={"mom": 4.0})
 
 
-@pytest.mark.parametrize("n,k", [(1, 1), (131_072, 2), (131_073, 10), (5, 10)])
+@pytest.mark.parametrize("n,k", [(1, 1), (131_072, 2), (131_073, 10), (5, 10), (1000, 32)])
 def test_host_path_chunk_boundaries(ctx, n, k):
     """kf_fit_tracks_host cuts the batch into chunks of 131 072 tracks: exactly one chunk, one chunk plus one track,
     a single track, a one-layer geometry -- same results as the resident call."""
     from paper_1705_02876_b200.buffers import DeviceFit
-    cfg = dataclasses.replace(W.get_config(1), n_layers=k, n_tracks=n)
+    cfg = dataclasses.replace(W.get_config(1), n_layers=k, n_tracks=n, layer_step_cm=4.0 if k <= 10 else 1.25)
     b = W.simulate_event(cfg, 31, n_tracks=n)
     d = DeviceFit.from_batch(b, "cuda:0")
     d.fit(ctx)

@@ -24,6 +24,7 @@
 // writes the optional SoA copies (coalesced) and the per-bin boxes.
 // Every read of the inputs is coalesced; the only scattered traffic is one 48-byte record per hit in step (3).
 #include <cmath>
+#include <cstdlib>
 
 #include "kf_internal.h"
 
@@ -43,7 +44,7 @@ __device__ __forceinline__ int bin_of_hit(float x, float y, float z, float r, in
     int lo = 1, hi = n_eta;
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
-        if (u >= __ldg(eta_edge + mid)) lo = mid + 1; else hi = mid;
+        if (u >= eta_edge[mid]) lo = mid + 1; else hi = mid;
     }
     const int ie = lo - 1;
     // The predicate fl(cos_j y) >= fl(sin_j x) says "phi >= edge j" and is true up to the hit's own edge and false
@@ -55,7 +56,7 @@ __device__ __forceinline__ int bin_of_hit(float x, float y, float z, float r, in
         int lo = half + 1, hi = n_phi;      // first j in [half + 1, n_phi) with a false predicate
         while (lo < hi) {
             const int mid = (lo + hi) >> 1;
-            if (__fmul_rn(__ldg(phi_cos + mid), y) >= __fmul_rn(__ldg(phi_sin + mid), x)) lo = mid + 1; else hi = mid;
+            if (__fmul_rn(phi_cos[mid], y) >= __fmul_rn(phi_sin[mid], x)) lo = mid + 1; else hi = mid;
         }
         ip = lo - 1;
     } else if (y == 0.0f) {
@@ -64,7 +65,7 @@ __device__ __forceinline__ int bin_of_hit(float x, float y, float z, float r, in
         int lo = 1, hi = half;              // first j in [1, half)
         while (lo < hi) {
             const int mid = (lo + hi) >> 1;
-            if (__fmul_rn(__ldg(phi_cos + mid), y) >= __fmul_rn(__ldg(phi_sin + mid), x)) lo = mid + 1; else hi = mid;
+            if (__fmul_rn(phi_cos[mid], y) >= __fmul_rn(phi_sin[mid], x)) lo = mid + 1; else hi = mid;
         }
         ip = lo - 1;
     }
@@ -223,6 +224,177 @@ bin_finish_kernel(const __grid_constant__ BinBatch B) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Chunked form of the same stable counting sort for hit pools (four launches + the finish step, every record
+// written ONCE): a layer is cut into chunks of kChunk consecutive hits, one CTA per chunk.
+//   chunk_count   bin of every hit; shared-memory histogram of the chunk; bucket lists in shared memory; every hit
+//                 counts the smaller indices of its bucket = its stable rank INSIDE the chunk (the arrival order of
+//                 the shared-memory atomics never shows); key, rank and the chunk's histogram go to global memory
+//   chunk_prefix  per bin: prefix of the chunk histograms over the chunks (chunks are consecutive index ranges, so
+//                 earlier chunk = smaller index) and the bin total; bin_scan_kernel then gives bin_offset
+//   chunk_place   final slot = bin_offset[bin] + hits of the bin in earlier chunks + rank inside the chunk; the nine
+//                 values are read coalesced and the packed record goes straight to its final place
+// Same results as the five-launch path, bit for bit.  Limits: n_bins <= kChunkMaxBins (shared memory).
+#ifndef KF_BIN_CHUNK
+#define KF_BIN_CHUNK 2048
+#endif
+constexpr int kChunk = KF_BIN_CHUNK;
+constexpr int kChunkBlock = kChunk / 8;
+constexpr int kChunkPer = kChunk / kChunkBlock;
+constexpr int kChunkMaxBins = 8192;
+
+__global__ void __launch_bounds__(kChunkBlock)
+chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__ eta_edge_g,
+                   const float* __restrict__ phi_cos_g, const float* __restrict__ phi_sin_g) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
+    const int c = blockIdx.x;
+    const int64_t h0 = (int64_t)c * kChunk;
+    if (h0 >= L.n) return;
+    const int m = (int)(L.n - h0 < kChunk ? L.n - h0 : kChunk);
+    const int nb = B.n_eta * B.n_phi;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    int32_t* cnt = reinterpret_cast<int32_t*>(smem_raw);              // [nb] histogram of the chunk
+    int32_t* loc = cnt + nb;                                           // [nb] start of each bin's bucket
+    uint32_t* ka = reinterpret_cast<uint32_t*>(loc + nb);              // [kChunk] bin << 16 | arrival number
+    uint16_t* bucket = reinterpret_cast<uint16_t*>(ka + kChunk);       // [kChunk] chunk-local hit indices by bin
+    float* eta_edge = reinterpret_cast<float*>(bucket + kChunk);       // [n_eta] [n_phi] [n_phi]
+    float* phi_cos = eta_edge + B.n_eta;
+    float* phi_sin = phi_cos + B.n_phi;
+    __shared__ int32_t wsum[kChunkBlock / 32];
+    for (int i = tid; i < nb; i += kChunkBlock) cnt[i] = 0;
+    for (int i = tid; i < B.n_eta; i += kChunkBlock) eta_edge[i] = eta_edge_g[i];
+    for (int i = tid; i < B.n_phi; i += kChunkBlock) { phi_cos[i] = phi_cos_g[i]; phi_sin[i] = phi_sin_g[i]; }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < kChunkPer; ++it) {
+        const int li = tid + it * kChunkBlock;
+        if (li < m) {
+            const int64_t h = h0 + li;
+            const int b = bin_of_hit(__ldg(L.pos + h), __ldg(L.pos + L.ld_in + h), __ldg(L.pos + 2 * L.ld_in + h),
+                                     L.radius, B.n_eta, B.n_phi, eta_edge, phi_cos, phi_sin);
+            ka[li] = ((uint32_t)b << 16) | (uint32_t)atomicAdd(cnt + b, 1);
+        }
+    }
+    __syncthreads();
+    // exclusive scan of cnt -> loc: thread t owns the bins [r0, r1)
+    const int per = (nb + kChunkBlock - 1) / kChunkBlock;
+    const int r0 = tid * per < nb ? tid * per : nb, r1 = r0 + per < nb ? r0 + per : nb;
+    int32_t sum = 0;
+    for (int b = r0; b < r1; ++b) { loc[b] = sum; sum += cnt[b]; }
+    int32_t incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int32_t o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+    }
+    if (lane == 31) wsum[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+        int32_t w = lane < kChunkBlock / 32 ? wsum[lane] : 0;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int32_t o = __shfl_up_sync(0xffffffffu, w, d);
+            if (lane >= d) w += o;
+        }
+        if (lane < kChunkBlock / 32) wsum[lane] = w;   // inclusive over warps
+    }
+    __syncthreads();
+    const int32_t excl = (wid ? wsum[wid - 1] : 0) + incl - sum;
+    for (int b = r0; b < r1; ++b) loc[b] += excl;
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < kChunkPer; ++it) {
+        const int li = tid + it * kChunkBlock;
+        if (li < m) { const uint32_t k = ka[li]; bucket[loc[k >> 16] + (int)(k & 0xffffu)] = (uint16_t)li; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < kChunkPer; ++it) {
+        const int li = tid + it * kChunkBlock;
+        if (li < m) {
+            const int b = (int)(ka[li] >> 16);
+            const int s0 = loc[b], s1 = s0 + cnt[b];
+            int rank = 0;
+            for (int j = s0; j < s1; ++j) rank += bucket[j] < (uint16_t)li ? 1 : 0;
+            L.key[h0 + li] = b;
+            L.pib[h0 + li] = rank;
+        }
+    }
+    for (int b = tid; b < nb; b += kChunkBlock) L.chunk_cnt[(int64_t)c * nb + b] = cnt[b];   // [chunk][bin]
+}
+
+// A thread per bin: chunk_cnt[c][b] becomes the number of hits of bin b in chunks before c (sixteen independent
+// loads in flight at a time); the bin total goes to counts[b], which bin_scan_kernel turns into bin_offset.
+__global__ void __launch_bounds__(128)
+chunk_prefix_kernel(const __grid_constant__ BinBatch B) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
+    const int nb = B.n_eta * B.n_phi;
+    const int nc = (int)((L.n + kChunk - 1) / kChunk);
+    const int b = blockIdx.x * 128 + threadIdx.x;
+    if (b >= nb) return;
+    int32_t* col = L.chunk_cnt + b;            // [chunk][bin]: neighbouring threads, neighbouring words
+    int32_t tot = 0;
+    for (int c0 = 0; c0 < nc; c0 += 16) {
+        int32_t v[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = c0 + k < nc ? col[(int64_t)(c0 + k) * nb] : 0;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            if (c0 + k < nc) col[(int64_t)(c0 + k) * nb] = tot;
+            tot += v[k];
+        }
+    }
+    L.counts[b] = tot;
+}
+
+__global__ void __launch_bounds__(kChunkBlock)
+chunk_place_kernel(const __grid_constant__ BinBatch B) {
+    const BinLayerDev& L = B.layer[blockIdx.y];
+    const int c = blockIdx.x;
+    const int64_t h0 = (int64_t)c * kChunk;
+    if (h0 >= L.n) return;
+    const int m = (int)(L.n - h0 < kChunk ? L.n - h0 : kChunk);
+    const int nb = B.n_eta * B.n_phi;
+    const int tid = threadIdx.x;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    int32_t* base = reinterpret_cast<int32_t*>(smem_raw);   // [nb] final slot of this chunk's first hit of a bin
+    // Per warp: 32 records staged in shared memory and written out three lanes to a record, so that one store
+    // instruction covers whole 48-byte records (2 sectors each) instead of 32 separate 16-byte pieces.
+    __shared__ __align__(16) float4 stage[kChunkBlock / 32][32 * 3];
+    __shared__ int32_t stage_dst[kChunkBlock / 32][32];
+    const int lane = tid & 31, wid = tid >> 5;
+    for (int b = tid; b < nb; b += kChunkBlock) base[b] = L.bin_offset[b] + L.chunk_cnt[(int64_t)c * nb + b];
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < kChunkPer; ++it) {
+        const int li = tid + it * kChunkBlock;        // (a warp's 32 hits are consecutive)
+        int32_t dst = -1;
+        if (li < m) {
+            const int64_t h = h0 + li;
+            dst = base[__ldg(L.key + h)] + __ldg(L.pib + h);   // (written by the launch before)
+            if (L.orig_to_sorted) L.orig_to_sorted[h] = dst;
+            float v[9];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) v[k] = __ldg(L.pos + k * L.ld_in + h);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) v[3 + k] = __ldg(L.cov + k * L.ld_in + h);
+            stage[wid][lane * 3 + 0] = make_float4(v[0], v[1], v[2], v[8]);                          // x y z vzz
+            stage[wid][lane * 3 + 1] = make_float4(v[3], v[4], v[6], __int_as_float((int32_t)h));    // vxx vxy vyy, index
+            stage[wid][lane * 3 + 2] = make_float4(v[5], v[7], 0.0f, 0.0f);                          // vxz vyz
+        }
+        stage_dst[wid][lane] = dst;
+        __syncwarp();
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            const int w = r * 32 + lane, rec = w / 3, part = w - rec * 3;
+            const int32_t d = stage_dst[wid][rec];
+            if (d >= 0) reinterpret_cast<float4*>(L.hit_rec + (int64_t)d * 12)[part] = stage[wid][w];
+        }
+        __syncwarp();
+    }
+}
+
 // Candidate keys for kf_order_candidates: the (eta, phi) bin of the candidate's crossing with the layer
 // (definition formula in fp32; the order only steers cache locality, never a result).
 __global__ void __launch_bounds__(kBlock)
@@ -284,13 +456,27 @@ cudaError_t BinScratch::reserve(int64_t n_items, int64_t n_bins, cudaStream_t st
     return cudaSuccess;
 }
 
+cudaError_t BinScratch::reserve_chunk_cnt(int64_t words, cudaStream_t stream) {
+    if (words <= cap_chunk_cnt) return cudaSuccess;
+    cudaError_t e = cudaStreamSynchronize(stream);   // the old buffer may still be in use
+    if (e != cudaSuccess) return e;
+    if (chunk_cnt) cudaFree(chunk_cnt);
+    chunk_cnt = nullptr;
+    cap_chunk_cnt = 0;
+    if ((e = cudaMalloc(&chunk_cnt, (size_t)words * sizeof(int32_t))) != cudaSuccess) return e;
+    cap_chunk_cnt = words;
+    return cudaSuccess;
+}
+
 void BinScratch::release() {
-    void* ptrs[] = {key, unsorted, pib, counts, eta_edge, phi_cos, phi_sin, rec_tmp};
+    void* ptrs[] = {key, unsorted, pib, counts, eta_edge, phi_cos, phi_sin, rec_tmp, chunk_cnt};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     key = unsorted = pib = counts = nullptr;
     eta_edge = phi_cos = phi_sin = nullptr;
     rec_tmp = nullptr;
+    chunk_cnt = nullptr;
+    cap_chunk_cnt = 0;
     cap_items = 0;
     cap_bins = 0;
     cap_rec = 0;
@@ -324,6 +510,69 @@ cudaError_t BinScratch::tables(int n_eta, int n_phi, float eta_max, cudaStream_t
     return cudaSuccess;
 }
 
+// The chunked sort for a group of layers, when it applies (hit pools with packed records, n_bins within the
+// shared-memory limit, enough hits to pay).
+namespace {
+
+size_t chunk_count_smem(int n_eta, int n_phi) {
+    return (size_t)2 * n_eta * n_phi * 4 + (size_t)kChunk * 6 + ((size_t)n_eta + 2 * (size_t)n_phi) * 4;
+}
+
+int64_t chunk_cnt_words(int64_t chunks, int nb) { return (chunks > 0 ? chunks : 1) * (int64_t)nb; }
+
+// KF_BIN_CHUNKED in the environment (read at every call: the tests switch between the two forms): 0 = never,
+// 1 = wherever it applies, unset = where it pays, i.e. groups of at least kChunkedMinHits hits (7 x 120 000 hits:
+// 0.066 ms against 0.101 ms; one pool of 120 000: 0.036 against 0.032).
+constexpr int64_t kChunkedMinHits = 1 << 18;
+
+bool chunked_wanted(int64_t total_hits) {
+    const char* e = std::getenv("KF_BIN_CHUNKED");
+    if (e ? std::atoi(e) == 0 : total_hits < kChunkedMinHits) return false;
+    static const bool ok = cudaFuncSetAttribute(chunk_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)chunk_count_smem(1, kChunkMaxBins)) == cudaSuccess;
+    return ok;
+}
+
+// returns cudaSuccess and *done = true if the group was sorted here
+cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max, cudaStream_t stream, bool* done) {
+    *done = false;
+    const int nb = B.n_eta * B.n_phi;
+    if (nb > kChunkMaxBins || nb > 65535 || group_max <= 0) return cudaSuccess;
+    int64_t total = 0;
+    for (int j = 0; j < m; ++j) {
+        if (!B.layer[j].pos || !B.layer[j].hit_rec) return cudaSuccess;
+        total += B.layer[j].n;
+    }
+    if (!chunked_wanted(total)) return cudaSuccess;
+    const int64_t nc = (group_max + kChunk - 1) / kChunk;
+    if (nc > 65535) return cudaSuccess;
+    int64_t chunks = 0;
+    for (int j = 0; j < m; ++j) chunks += (B.layer[j].n + kChunk - 1) / kChunk;
+    cudaError_t e = s.reserve_chunk_cnt(chunk_cnt_words(chunks, nb), stream);
+    if (e != cudaSuccess) return e;
+    chunks = 0;
+    for (int j = 0; j < m; ++j) {
+        B.layer[j].chunk_cnt = s.chunk_cnt + chunks * nb;     // [chunks of layer j][nb]
+        chunks += (B.layer[j].n + kChunk - 1) / kChunk;
+    }
+    const dim3 grid((unsigned)nc, (unsigned)m);
+    chunk_count_kernel<<<grid, kChunkBlock, chunk_count_smem(B.n_eta, B.n_phi), stream>>>(B, s.eta_edge, s.phi_cos, s.phi_sin);
+    chunk_prefix_kernel<<<dim3((unsigned)((nb + 127) / 128), (unsigned)m), 128, 0, stream>>>(B);
+    bin_scan_kernel<<<dim3(1, m), 1024, 0, stream>>>(B);
+    chunk_place_kernel<<<grid, kChunkBlock, (size_t)nb * 4, stream>>>(B);
+    bin_finish_kernel<<<dim3((unsigned)((nb * 32 + kBlock - 1) / kBlock), (unsigned)m), kBlock, 0, stream>>>(B);
+    *done = true;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// Scratch of the chunked sort for calls of up to max_hits hits in up to KF_MAX_LAYERS pools with any bin grid it
+// takes (kf_reserve): chunks <= max_hits / kChunk + pools.
+cudaError_t reserve_chunked(BinScratch& s, int64_t max_hits, int max_layers, cudaStream_t stream) {
+    return s.reserve_chunk_cnt(chunk_cnt_words(max_hits / kChunk + max_layers, kChunkMaxBins), stream);
+}
+
 // Bin up to kBinBatchMax layers per group of launches.  All layers share (n_eta, n_phi, eta_max).
 cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream) {
     if (n_layers <= 0) return cudaSuccess;
@@ -334,7 +583,7 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
     cudaError_t e = s.reserve(total, (int64_t)(nb + 1) * n_layers, stream, true);
     if (e != cudaSuccess) return e;
     if ((e = s.tables(n_eta, n_phi, args[0].eta_max, stream)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(s.counts, 0, (size_t)(nb + 1) * n_layers * sizeof(int32_t), stream)) != cudaSuccess) return e;
+    bool zeroed = false;   // the histogram of the five-launch path (the chunked sort keeps its own in shared memory)
     int64_t item_off = 0;
     for (int l0 = 0; l0 < n_layers; l0 += kBinBatchMax) {
         const int m = n_layers - l0 < kBinBatchMax ? n_layers - l0 : kBinBatchMax;
@@ -350,8 +599,16 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
             L.key = s.key + item_off; L.unsorted = s.unsorted + item_off;
             L.counts = s.counts + (int64_t)(l0 + j) * (nb + 1);
             L.pib = s.pib + item_off; L.rec_tmp = a.pos ? s.rec_tmp + item_off * 12 : nullptr;
+            L.chunk_cnt = nullptr;
             item_off += a.n_hits;
             if (a.n_hits > group_max) group_max = a.n_hits;
+        }
+        bool done = false;
+        if ((e = try_chunk_sort(s, B, m, group_max, stream, &done)) != cudaSuccess) return e;
+        if (done) continue;
+        if (!zeroed) {
+            if ((e = cudaMemsetAsync(s.counts, 0, (size_t)(nb + 1) * n_layers * sizeof(int32_t), stream)) != cudaSuccess) return e;
+            zeroed = true;
         }
         const dim3 grid((unsigned)((group_max + kBlock - 1) / kBlock), (unsigned)m);
         if (group_max > 0) bin_key_kernel<<<grid, kBlock, 0, stream>>>(B, s.eta_edge, s.phi_cos, s.phi_sin);
@@ -380,7 +637,7 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
     L.n = n; L.ld_in = 0; L.ld_out = 0; L.pos = nullptr; L.cov = nullptr; L.radius = 0.0f;
     L.bin_offset = s.counts + (nb + 1);  // second half of the counts buffer holds the offsets
     L.sorted_to_orig = order; L.pos_sorted = nullptr; L.cov_sorted = nullptr; L.hit_rec = nullptr; L.bin_box = nullptr; L.orig_to_sorted = nullptr;
-    L.key = s.key; L.unsorted = s.unsorted; L.counts = s.counts; L.pib = s.pib; L.rec_tmp = nullptr;
+    L.key = s.key; L.unsorted = s.unsorted; L.counts = s.counts; L.pib = s.pib; L.rec_tmp = nullptr; L.chunk_cnt = nullptr;
     const dim3 grid((unsigned)((n + kBlock - 1) / kBlock), 1);
     cand_key_kernel<<<grid, kBlock, 0, stream>>>(P, layer, n, ld, par, q, n_eta, n_phi, eta_max, s.key, s.pib, s.counts);
     bin_scan_kernel<<<dim3(1, 1), 1024, 0, stream>>>(B);

@@ -92,6 +92,7 @@ struct BinLayerDev {
     int32_t* counts;    // [n_bins + 1]
     int32_t* pib;       // [n] arrival number of each item inside its bin (value returned by the histogram atomic)
     float* rec_tmp;     // [n][12] hit records grouped by bin in arrival order (null when nothing is gathered)
+    int32_t* chunk_cnt; // [chunks][n_bins] chunked sort: hits of a bin per chunk, then their prefix over chunks
 };
 
 struct BinBatch {
@@ -107,6 +108,9 @@ struct BinScratch {
     int32_t* pib = nullptr;
     float* rec_tmp = nullptr;    // [cap_items][12], allocated on the first call that gathers hits
     int64_t cap_rec = 0;
+    int32_t* chunk_cnt = nullptr; // chunked sort: [layers][n_bins][chunks] counters
+    int64_t cap_chunk_cnt = 0;
+    cudaError_t reserve_chunk_cnt(int64_t words, cudaStream_t stream);
     // edge tables (device) for the (n_eta, n_phi, eta_max) last used
     float* eta_edge = nullptr;   // fl32(sinh(-eta_max + j d_eta)), j = 1..n_eta-1 at [j]
     float* phi_cos = nullptr;    // fl32(cos(-pi + j d_phi))
@@ -121,6 +125,7 @@ struct BinScratch {
 
 // kf_bin.cu
 cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream);
+cudaError_t reserve_chunked(BinScratch& s, int64_t max_hits, int max_layers, cudaStream_t stream);
 cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n, int64_t ld, const float* par,
                          const int8_t* q, int n_eta, int n_phi, float eta_max, int32_t* order,
                          cudaStream_t stream);

@@ -21,6 +21,14 @@ def ctx():
     c.close()
 
 
+@pytest.fixture(params=["chunked", "five_launch"])
+def sort_path(request, monkeypatch):
+    """Both forms of the counting sort: the chunked one (taken for calls of >= 262 144 hits) and the five-launch
+    one (small calls, more than 8192 bins).  KF_BIN_CHUNKED, read at every call, forces either for any size."""
+    monkeypatch.setenv("KF_BIN_CHUNKED", "0" if request.param == "five_launch" else "1")
+    return request.param
+
+
 def _bin_both(ctx, pos, cov, radius, ne=NE, nph=NP, emax=EMAX):
     from paper_1705_02876_b200.buffers import DeviceLayer
     dl = DeviceLayer.from_numpy(pos, cov, ne, nph, emax, "cuda:0")
@@ -55,7 +63,7 @@ def _assert_bins_equal(dl, ob, pos, cov):
 
 
 @pytest.mark.parametrize("n_tracks,noise", [(400, 2000), (20000, 100000)])
-def test_bin_hits_bit_exact(ctx, n_tracks, noise):
+def test_bin_hits_bit_exact(ctx, n_tracks, noise, sort_path):
     ev = W.make_build_event(4, n_tracks=n_tracks, noise_hits=noise)
     for l in (0, 4, 9):
         lay = ev.layers[l]
@@ -63,7 +71,7 @@ def test_bin_hits_bit_exact(ctx, n_tracks, noise):
         _assert_bins_equal(dl, ob, lay.pos, lay.cov)
 
 
-def test_bin_hits_edge_cases(ctx):
+def test_bin_hits_edge_cases(ctx, sort_path):
     rng = np.random.default_rng(11)
     r = 12.0
     cov = np.tile(np.array([1e-2, 0, 0, 1e-2, 0, 1e-2], dtype=np.float32)[:, None], (1, 5000))
@@ -92,7 +100,7 @@ def test_bin_hits_edge_cases(ctx):
         _assert_bins_equal(dl, ob, pos, cov[:, :3000])
 
 
-def test_bin_hits_large_layer(ctx):
+def test_bin_hits_large_layer(ctx, sort_path):
     """A layer of 700 000 hits with a full 3 x 3 covariance each (every output plane distinguishable)."""
     H = 700_000
     rng = np.random.default_rng(12)
@@ -104,7 +112,7 @@ def test_bin_hits_large_layer(ctx):
     _assert_bins_equal(dl, ob, pos, cov)
 
 
-def test_bin_layers_batched_equals_per_layer(ctx):
+def test_bin_layers_batched_equals_per_layer(ctx, sort_path):
     """kf_bin_layers (all layers in four launches) == kf_bin_hits layer by layer == oracle."""
     from paper_1705_02876_b200.buffers import DeviceLayer
     ev = W.make_build_event(4, n_tracks=2000, noise_hits=9000)

@@ -12,6 +12,8 @@
 //     lower half plane:      i_phi = #{ j in 1..n_phi/2-1 : fl(cos_j y) >= fl(sin_j x) }
 // with (cos_j, sin_j) = fl(cos, sin)(-pi + j d_phi).  No transcendental is evaluated on the GPU.
 //
+// Two forms of one stable counting sort with bit-identical results: the chunked form further down (large calls on
+// hit pools) and this one (small calls, more than 8192 bins, ordering of candidates).
 // Counting sort, stable, batched over layers (grid.y = layer, 5 launches + 1 memset for ALL layers):
 // (1) key of every item + histogram; the histogram atomic's return value is the item's arrival number inside its
 // bin, (2) exclusive scan -> bin_offset, (3) every item goes to slot bin_offset[bin] + arrival number -- no second

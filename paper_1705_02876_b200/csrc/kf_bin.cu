@@ -268,14 +268,53 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
     for (int i = tid; i < B.n_eta; i += kChunkBlock) eta_edge[i] = eta_edge_g[i];
     for (int i = tid; i < B.n_phi; i += kChunkBlock) { phi_cos[i] = phi_cos_g[i]; phi_sin[i] = phi_sin_g[i]; }
     __syncthreads();
+    // The bin rule of bin_of_hit for this thread's kChunkPer hits at once: all loads first, then the two searches
+    // as descents in powers of two (same answer as the bisection for a monotone predicate; the trip count depends on
+    // the grid only, so the hits' dependent look-ups interleave instead of running one hit after the other).
+    {
+        float x[kChunkPer], y[kChunkPer], u[kChunkPer];
+        int pe[kChunkPer], pp[kChunkPer], lim[kChunkPer];
+        const int half = B.n_phi >> 1;
 #pragma unroll
-    for (int it = 0; it < kChunkPer; ++it) {
-        const int li = tid + it * kChunkBlock;
-        if (li < m) {
-            const int64_t h = h0 + li;
-            const int b = bin_of_hit(__ldg(L.pos + h), __ldg(L.pos + L.ld_in + h), __ldg(L.pos + 2 * L.ld_in + h),
-                                     L.radius, B.n_eta, B.n_phi, eta_edge, phi_cos, phi_sin);
-            ka[li] = ((uint32_t)b << 16) | (uint32_t)atomicAdd(cnt + b, 1);
+        for (int it = 0; it < kChunkPer; ++it) {
+            const int li = tid + it * kChunkBlock;
+            const int64_t h = h0 + (li < m ? li : 0);
+            x[it] = __ldg(L.pos + h); y[it] = __ldg(L.pos + L.ld_in + h);
+            u[it] = __ldg(L.pos + 2 * L.ld_in + h);
+        }
+#pragma unroll
+        for (int it = 0; it < kChunkPer; ++it) {
+            u[it] = __fdiv_rn(u[it], L.radius);
+            const bool upper = y[it] > 0.0f || (y[it] == 0.0f && x[it] > 0.0f);
+            pe[it] = 0;
+            pp[it] = upper ? half : 0;
+            lim[it] = upper ? B.n_phi - 1 : (y[it] == 0.0f ? 0 : half - 1);
+        }
+        int top = 1;
+        while (top * 2 <= B.n_eta - 1) top *= 2;
+        for (int step = top; step > 0; step >>= 1) {
+#pragma unroll
+            for (int it = 0; it < kChunkPer; ++it) {
+                const int t = pe[it] + step;
+                if (t <= B.n_eta - 1 && u[it] >= eta_edge[t]) pe[it] = t;
+            }
+        }
+        top = 1;
+        while (top * 2 <= half) top *= 2;
+        for (int step = top; step > 0; step >>= 1) {
+#pragma unroll
+            for (int it = 0; it < kChunkPer; ++it) {
+                const int t = pp[it] + step;
+                if (t <= lim[it] && __fmul_rn(phi_cos[t], y[it]) >= __fmul_rn(phi_sin[t], x[it])) pp[it] = t;
+            }
+        }
+#pragma unroll
+        for (int it = 0; it < kChunkPer; ++it) {
+            const int li = tid + it * kChunkBlock;
+            if (li < m) {
+                const int b = pe[it] * B.n_phi + pp[it];
+                ka[li] = ((uint32_t)b << 16) | (uint32_t)atomicAdd(cnt + b, 1);
+            }
         }
     }
     __syncthreads();

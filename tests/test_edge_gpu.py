@@ -97,13 +97,16 @@ def _host_fit(ctx, b):
     return h.results()
 
 
-def test_bin_32_layers_in_one_call(ctx):
-    """KF_MAX_LAYERS pools in one kf_bin_layers call (two launch groups of 16), ragged sizes, one empty pool."""
+@pytest.mark.parametrize("chunked", ["1", "0"])
+def test_bin_32_layers_in_one_call(ctx, chunked, monkeypatch):
+    """KF_MAX_LAYERS pools in one kf_bin_layers call (two launch groups of 16), ragged sizes (1 to 3 chunks of the
+    chunked sort per pool), one empty pool; both forms of the sort."""
+    monkeypatch.setenv("KF_BIN_CHUNKED", chunked)
     from paper_1705_02876_b200.buffers import DeviceLayer
     rng = np.random.default_rng(41)
     pools, radii = [], []
     for l in range(32):
-        H = 0 if l == 17 else int(rng.integers(1, 4000))
+        H = 0 if l == 17 else int(rng.integers(1, 6000))
         r = 2.5 * (l + 1)
         phi, eta = rng.uniform(-np.pi, np.pi, H), rng.uniform(-1.3, 1.3, H)
         pos = np.stack([r * np.cos(phi), r * np.sin(phi), r * np.sinh(eta)]).astype(np.float32)

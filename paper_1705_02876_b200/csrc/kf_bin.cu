@@ -562,9 +562,10 @@ size_t chunk_count_smem(int n_eta, int n_phi) {
 int64_t chunk_cnt_words(int64_t chunks, int nb) { return (chunks > 0 ? chunks : 1) * (int64_t)nb; }
 
 // KF_BIN_CHUNKED in the environment (read at every call: the tests switch between the two forms): 0 = never,
-// 1 = wherever it applies, unset = where it pays, i.e. groups of at least kChunkedMinHits hits (7 x 120 000 hits:
-// 0.066 ms against 0.101 ms; one pool of 120 000: 0.036 against 0.032).
-constexpr int64_t kChunkedMinHits = 1 << 18;
+// 1 = wherever it applies, unset = where it pays, i.e. groups of at least kChunkedMinHits hits (7 pools, chunked
+// against five-launch: 126 000 hits 36 / 32 us, 210 000 hits 37 / 38 us, 336 000 hits 41 / 48 us, 840 000 hits
+// 62 / 101 us; one pool of 120 000 hits 33 / 32 us).
+constexpr int64_t kChunkedMinHits = 3 << 16;   // measured crossover on 7 pools of 40 x 64 bins: 180 000 - 210 000 hits
 
 bool chunked_wanted(int64_t total_hits) {
     const char* e = std::getenv("KF_BIN_CHUNKED");

@@ -23,7 +23,7 @@ def ctx():
 
 @pytest.fixture(params=["chunked", "five_launch"])
 def sort_path(request, monkeypatch):
-    """Both forms of the counting sort: the chunked one (taken for calls of >= 262 144 hits) and the five-launch
+    """Both forms of the counting sort: the chunked one (taken for calls of >= 196 608 hits) and the five-launch
     one (small calls, more than 8192 bins).  KF_BIN_CHUNKED, read at every call, forces either for any size."""
     monkeypatch.setenv("KF_BIN_CHUNKED", "0" if request.param == "five_launch" else "1")
     return request.param

@@ -95,7 +95,8 @@ def test_bin_hits_edge_cases(ctx, sort_path):
     # other bin shapes, incl. the largest table
     pos = np.stack([r * np.cos(rng.uniform(-np.pi, np.pi, 3000)), r * np.sin(rng.uniform(-np.pi, np.pi, 3000)),
                     r * np.sinh(rng.uniform(-2.5, 2.5, 3000))]).astype(np.float32)
-    for ne, nph, emax in [(1, 2, 1.0), (7, 10, 2.0), (256, 256, 2.5)]:
+    # (64 x 128 = 8192 bins: the largest grid the chunked sort takes; 256 x 256 always takes the five-launch form)
+    for ne, nph, emax in [(1, 2, 1.0), (7, 10, 2.0), (64, 128, 2.0), (2, 4096, 2.0), (256, 256, 2.5)]:
         dl, ob = _bin_both(ctx, pos, cov[:, :3000], r, ne, nph, float(np.float32(emax)))
         _assert_bins_equal(dl, ob, pos, cov[:, :3000])
 

@@ -143,8 +143,11 @@ scan_kernel(const ScoreArgs a, float inv_r) {
         bool keep = false;
         int32_t s0 = 0, s1 = 0;
         if (j < n_win) {
-            const int e = ie - wh + j / side;
-            const int p = ((ip - wh + j % side) % a.n_phi + a.n_phi) % a.n_phi;
+            const int q = j / side;
+            const int e = ie - wh + q;
+            int p = ip - wh + (j - q * side);   // 0 <= ip < n_phi and side <= n_phi: one wrap either way is enough
+            p += p < 0 ? a.n_phi : 0;
+            p -= p >= a.n_phi ? a.n_phi : 0;
             if (e >= 0 && e < a.n_eta) {
                 const int bin = e * a.n_phi + p;
                 s0 = __ldg(a.bin_offset + bin);

@@ -590,6 +590,7 @@ cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max,
     if (nc > 65535) return cudaSuccess;
     int64_t chunks = 0;
     for (int j = 0; j < m; ++j) chunks += (B.layer[j].n + kChunk - 1) / kChunk;
+    if (chunk_cnt_words(chunks, nb) > ((int64_t)1 << 28)) return cudaSuccess;   // > 1 GB of counters: not this form
     cudaError_t e = s.reserve_chunk_cnt(chunk_cnt_words(chunks, nb), stream);
     if (e != cudaSuccess) return e;
     chunks = 0;
@@ -612,7 +613,8 @@ cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max,
 // Scratch of the chunked sort for calls of up to max_hits hits in up to KF_MAX_LAYERS pools with any bin grid it
 // takes (kf_reserve): chunks <= max_hits / kChunk + pools.
 cudaError_t reserve_chunked(BinScratch& s, int64_t max_hits, int max_layers, cudaStream_t stream) {
-    return s.reserve_chunk_cnt(chunk_cnt_words(max_hits / kChunk + max_layers, kChunkMaxBins), stream);
+    const int64_t words = chunk_cnt_words(max_hits / kChunk + max_layers, kChunkMaxBins);
+    return s.reserve_chunk_cnt(words < ((int64_t)1 << 28) ? words : ((int64_t)1 << 28), stream);
 }
 
 // Bin up to kBinBatchMax layers per group of launches.  All layers share (n_eta, n_phi, eta_max).

@@ -330,18 +330,18 @@ def run_ours(args) -> None:
     ctx.set_stream(stream)          # measure_building borrowed the context for torch's current stream
     smoothing = None
     if rank == 0 and not args.no_building:
-        # secondary: kf_fit_tracks_smooth on the same batch (forward fit + inward refit, one kernel)
+        # secondary: kf_fit_tracks_refit on the same batch (forward fit + inward refit, one kernel)
         # Every track of configs[2] has all 10 hits, which the API states by passing no mask: the call then takes
         # the two-tracks-per-thread smoother.  With a mask it takes the one-track kernel (ragged pairs would cost
         # the pair form more than it gains); both are timed.
         def time_smooth():
             with torch.cuda.stream(stream):
                 for _ in range(3):
-                    d.fit_smooth(ctx)
+                    d.fit_refit(ctx)
                 s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 s0.record(stream)
                 for _ in range(20):
-                    d.fit_smooth(ctx)
+                    d.fit_refit(ctx)
                 s1.record(stream)
             torch.cuda.synchronize()
             return s0.elapsed_time(s1) / 20
@@ -457,7 +457,7 @@ def run_ours(args) -> None:
                                                "fits_per_s": bc.n / (g_ms * 1e-3), "bound_ms": bound_ms,
                                                "roofline_frac": bound_ms / g_ms}
             del dcf, bc
-        smoothing = {"api": "kf_fit_tracks_smooth (reading A18, kappa 10), mask = NULL: every track has every hit",
+        smoothing = {"api": "kf_fit_tracks_refit (reading A18, kappa 10), mask = NULL: every track has every hit",
                      "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3), "with_mask_ms": sm_masked_ms,
                      "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0],
                      "alu_roofline_frac": 2.0 * n * FLOPS_PER_TRACK_LAYER * L / (sm_ms * 1e-3) / (fp32_peak * 1e12)}

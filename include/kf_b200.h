@@ -63,7 +63,9 @@ enum {
     KF_ERR_UNSUPPORTED = -4, /* n_layers > 32, |Bz| < 1e-6 T, radii not strictly increasing,
                                 bins > KF_MAX_BINS, window wider than the phi ring                */
     KF_ERR_CUDA = -5,        /* a CUDA runtime call failed (kf_last_cuda_error has the code)      */
-    KF_ERR_NOMEM = -6        /* scratch allocation failed                                         */
+    KF_ERR_NOMEM = -6,       /* scratch allocation failed                                         */
+    KF_ERR_STALE = -7        /* kf_graph_launch: the graph's context is gone, or has reallocated scratch or
+                                changed the bin grid since the recording (record it again)          */
 };
 
 /* ---- per-track status bits (outputs) ---------------------------------------------------------- */
@@ -87,6 +89,20 @@ KF_API int kf_create(kf_ctx** out, int device, void* cuda_stream);
 KF_API int kf_destroy(kf_ctx* ctx);
 /* Change the borrowed stream used by later calls. */
 KF_API int kf_set_stream(kf_ctx* ctx, void* cuda_stream);
+/* Every call makes the context's device current for its own duration and restores the caller's current device
+ * before it returns, so contexts on several devices can be driven from one thread. */
+
+/* Launch options of a context (kernel selection only: no option changes a result beyond fp32 rounding).  They
+ * exist for tests and measurements; the defaults are the measured best. */
+enum {
+    KF_OPT_PAIR_MIN_TRACKS = 1,   /* > 0: batches of at least this many tracks take the two-tracks-per-thread
+                                     kernels; 0 (default) = the built-in size rule                          */
+    KF_OPT_REFIT_PAIR_MASKED = 2, /* 1: kf_fit_tracks_refit takes its two-tracks-per-thread form for batches WITH
+                                     a hit mask too (default 0: only without a mask)                        */
+    KF_OPT_BIN_FORM = 3           /* kf_bin_layers: 0 (default) = by size, 1 = always the five-launch counting
+                                     sort, 2 = the chunked sort wherever it applies                         */
+};
+KF_API int kf_set_option(kf_ctx* ctx, int option, int64_t value);
 /* Pre-size scratch so that no later call allocates: `max_hits` hits in total over the layers of one kf_bin_layers call,
  * `max_host_tracks` x `max_host_layers` for the *_host staging buffers (0 = leave as is). */
 KF_API int kf_reserve(kf_ctx* ctx, int64_t max_hits, int64_t max_host_tracks, int max_host_layers);
@@ -105,8 +121,11 @@ KF_API int kf_last_cuda_error(const kf_ctx* ctx);
  * same sequence has run once before (or kf_reserve), because a call that has to grow scratch synchronises and
  * voids the capture (kf_graph_end then returns KF_ERR_CUDA and no graph).  kf_fit_tracks_host, kf_reserve,
  * kf_measure_fp32_peak and kf_set_stream must not be called while recording.  Results are bit-identical to
- * the eager calls.  A graph belongs to the device of the context that recorded it; destroy it with
- * kf_graph_destroy (independent of the context's lifetime). */
+ * the eager calls.  A graph belongs to the context that recorded it: the recorded kernels point into that
+ * context's scratch and bin edge tables, so kf_graph_launch refuses it with KF_ERR_STALE once the context has
+ * reallocated scratch (a later call needed more) or binned with another (n_eta, n_phi, eta_max) grid, and
+ * with KF_ERR_STALE as well when handed another context.  Never launch a graph whose context has been destroyed
+ * unless through a live context (which is then refused the same way).  Destroy it with kf_graph_destroy. */
 typedef struct kf_graph kf_graph;
 KF_API int kf_graph_begin(kf_ctx* ctx);
 KF_API int kf_graph_end(kf_ctx* ctx, kf_graph** out);
@@ -174,20 +193,23 @@ typedef struct {
 KF_API int kf_fit_tracks(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                   const kf_track_hits* hits, kf_tracks* out);
 
-/* Fit and smooth ("a final fit with a KF and smoother"; reading A18): the forward
- * fit of kf_fit_tracks, then the same filter run INWARD over the same hits, starting from the forward
- * result with its covariance inflated by `kappa` (10 is the documented choice): update with the outermost
- * used hit, then for each further used layer, outer to inner, add the process noise of the layer just
- * left, propagate backward along the helix to the smaller radius, update.  `out` receives the forward
- * result exactly as kf_fit_tracks writes it (state at the outermost used layer); `smoothed` receives the
- * state and covariance at the INNERMOST used layer (outer side of its material), chi2 = chi2 of the
- * backward pass, nhits = hits it used, status = its failure bits.  A track the forward fit could not
- * start comes back as its input in both.  All pointers DEV; `out` may alias `seeds`, `smoothed` may not
- * alias either.  One kernel.  Performance note: hits->mask == NULL states that every track has a hit on
- * every layer; large batches then run two tracks per thread (7 % faster).  With a mask the one-track kernel
- * runs, whose speed does not depend on how ragged the tracks are.  Results agree within the tolerances. */
-KF_API int kf_fit_tracks_smooth(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
-                                const kf_track_hits* hits, float kappa, kf_tracks* out, kf_tracks* smoothed);
+/* Fit and REFIT inward (reading A18; kept from round 1 -- it is NOT the smoother of PAPER.md:57,
+ * see kf_fit_tracks_smooth below): the forward fit of kf_fit_tracks, then the same filter run INWARD over the
+ * same hits, starting from the forward result with its covariance inflated by `kappa` (10 is the documented
+ * choice): update with the outermost used hit, then for each further used layer, outer to inner, add the process
+ * noise of the layer just left, propagate backward along the helix to the smaller radius, update.  The forward
+ * information is therefore counted 1 + 1/kappa times: the refitted covariance is too small by about that factor
+ * and its chi2 is not chi2-distributed exactly.  What it is good for: a state at the INNERMOST used layer that
+ * was linearised a second time around a better trajectory, at the cost of one more pass over the hits and no
+ * per-layer storage.  `out` receives the forward result exactly as kf_fit_tracks writes it (state at the
+ * outermost used layer); `refitted` receives the state and covariance at the innermost used layer (outer side
+ * of its material), chi2 = chi2 of the backward pass, nhits = hits it used, status = its failure bits.  A track
+ * the forward fit could not start comes back as its input in both.  All pointers DEV; `out` may alias `seeds`,
+ * `refitted` may not alias either.  One kernel.  Performance note: hits->mask == NULL states that every track has
+ * a hit on every layer; large batches then run two tracks per thread (7 % faster).  With a mask the one-track
+ * kernel runs, whose speed does not depend on how ragged the tracks are.  Results agree within the tolerances. */
+KF_API int kf_fit_tracks_refit(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                               const kf_track_hits* hits, float kappa, kf_tracks* out, kf_tracks* refitted);
 
 /* Same call with every pointer HOST (pageable or pinned): copies in, fits, copies out, in chunks
  * pipelined over internal streams, and returns when `out` is complete.  This is the end-to-end

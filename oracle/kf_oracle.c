@@ -467,7 +467,7 @@ static void refit_inward_one(int L, const double *radius, const double *xX0, dou
 /* Forward fit followed by the inward refit.  Outputs: forward result (opar/ocov/ochi2/onhits/ostatus) and
  * smoothed result at the innermost used layer (spar/scov/schi2).  sstatus = bits of the backward pass.
  * used_out (optional) = layers the forward fit used. */
-void orc_fit_smooth_one(int L, const double *radius, const double *xX0, double Bz, double mass, double kappa,
+void orc_fit_refit_one(int L, const double *radius, const double *xX0, double Bz, double mass, double kappa,
                         const double par[6], const double cov[36], int q, const double *hpos,
                         const double *hcov, uint32_t mask, double opar[6], double ocov[36], double *ochi2,
                         int32_t *onhits, uint32_t *ostatus, double spar[6], double scov[36], double *schi2,
@@ -492,13 +492,13 @@ void orc_fit_smooth_one(int L, const double *radius, const double *xX0, double B
 }
 
 /* Batched (single thread): AoS double inputs as in orc_fit_tracks. */
-void orc_fit_smooth_tracks(int64_t n, int L, const double *radius, const double *xX0, double Bz, double mass,
+void orc_fit_refit_tracks(int64_t n, int L, const double *radius, const double *xX0, double Bz, double mass,
                            double kappa, const double *par, const double *cov, const int8_t *q,
                            const double *hpos, const double *hcov, const uint32_t *mask, double *opar,
                            double *ocov, double *ochi2, int32_t *onhits, uint32_t *ostatus, double *spar,
                            double *scov, double *schi2, uint32_t *sstatus, double *trace_fwd, double *trace_bwd) {
     for (int64_t i = 0; i < n; ++i)
-        orc_fit_smooth_one(L, radius, xX0, Bz, mass, kappa, par + 6 * i, cov + 36 * i, q[i],
+        orc_fit_refit_one(L, radius, xX0, Bz, mass, kappa, par + 6 * i, cov + 36 * i, q[i],
                            hpos + (size_t)i * L * 3, hcov + (size_t)i * L * 9, mask ? mask[i] : 0xffffffffu,
                            opar + 6 * i, ocov + 36 * i, ochi2 + i, onhits + i, ostatus + i, spar + 6 * i,
                            scov + 36 * i, schi2 + i, sstatus + i,

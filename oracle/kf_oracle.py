@@ -42,7 +42,7 @@ def lib():
         _lib.orc_propagate.argtypes = [dp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
         _lib.orc_propagate_inward.restype = C.c_int
         _lib.orc_propagate_inward.argtypes = [dp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
-        _lib.orc_fit_smooth_tracks.restype = None
+        _lib.orc_fit_refit_tracks.restype = None
         _lib.orc_process_noise.restype = None
         _lib.orc_process_noise.argtypes = [dp, C.c_double, C.c_double, dp]
         _lib.orc_transport_cov.restype = None
@@ -239,10 +239,10 @@ def fit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None
     return out
 
 
-SMOOTH_KAPPA = 10.0    # reading A18: inflation of the forward covariance used as the backward prior
+REFIT_KAPPA = 10.0    # reading A18: inflation of the forward covariance used as the backward prior
 
 
-def fit_smooth_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None, kappa: float = SMOOTH_KAPPA,
+def fit_refit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None, kappa: float = REFIT_KAPPA,
                       want_trace: bool = False) -> dict:
     """Forward fit + inward refit (smoother).  Same input layout as fit_tracks.  Returns the forward
     results under the usual keys and the smoothed ones as spar[6][n], scov[n][6][6], schi2, sstatus
@@ -262,12 +262,12 @@ def fit_smooth_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, ma
     spar = np.zeros((n, 6)); scov = np.zeros((n, 6, 6)); schi2 = np.zeros(n); sst = np.zeros(n, dtype=np.uint32)
     tf = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
     tb = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
-    lib().orc_fit_smooth_tracks(C.c_int64(n), C.c_int(L), _p(rad), _p(xx0), C.c_double(Bz), C.c_double(mass),
+    lib().orc_fit_refit_tracks(C.c_int64(n), C.c_int(L), _p(rad), _p(xx0), C.c_double(Bz), C.c_double(mass),
                                 C.c_double(kappa), _p(par_a), _p(cov_a), _p(q_a, C.c_int8), _p(hp_a), _p(hc_a),
                                 _p(m_a, C.c_uint32), _p(opar), _p(ocov), _p(ochi2), _p(onh, C.c_int32),
                                 _p(ost, C.c_uint32), _p(spar), _p(scov), _p(schi2), _p(sst, C.c_uint32), _p(tf), _p(tb))
     out = dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost,
-               spar=np.ascontiguousarray(spar.T), scov=scov, schi2=schi2, sstatus=sst)
+               rpar=np.ascontiguousarray(spar.T), rcov=scov, rchi2=schi2, rstatus=sst)
     if want_trace:
         out["trace_fwd"], out["trace_bwd"] = tf, tb
     return out

@@ -20,8 +20,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so")   # override: kernel experiments
 
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE, STATUS_OUTSIDE = 1, 2, 4, 8, 16
-EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+OPT_PAIR_MIN_TRACKS, OPT_REFIT_PAIR_MASKED, OPT_BIN_FORM = 1, 2, 3          # kf_set_option
+BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
+EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
+           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
@@ -90,6 +92,8 @@ def load_library():
     lib.kf_destroy.argtypes = [vp]
     lib.kf_set_stream.restype = C.c_int
     lib.kf_set_stream.argtypes = [vp, vp]
+    lib.kf_set_option.restype = C.c_int
+    lib.kf_set_option.argtypes = [vp, C.c_int, C.c_int64]
     lib.kf_reserve.restype = C.c_int
     lib.kf_reserve.argtypes = [vp, C.c_int64, C.c_int64, C.c_int]
     lib.kf_strerror.restype = C.c_char_p
@@ -107,8 +111,8 @@ def load_library():
     lib.kf_fit_tracks_indexed.restype = C.c_int
     lib.kf_fit_tracks_indexed.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), vp, C.c_int64,
                                           C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.POINTER(_Tracks)]
-    lib.kf_fit_tracks_smooth.restype = C.c_int
-    lib.kf_fit_tracks_smooth.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.c_float,
+    lib.kf_fit_tracks_refit.restype = C.c_int
+    lib.kf_fit_tracks_refit.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.c_float,
                                          C.POINTER(_Tracks), C.POINTER(_Tracks)]
     lib.kf_bin_hits.restype = C.c_int
     lib.kf_bin_hits.argtypes = [vp, C.c_float, C.POINTER(_LayerHits), C.POINTER(_LayerBins)]
@@ -276,6 +280,9 @@ class KFContext:
         s = stream.cuda_stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
         self._check(self._lib.kf_set_stream(self._h, C.c_void_p(s)), "kf_set_stream")
 
+    def set_option(self, option: int, value: int):
+        self._check(self._lib.kf_set_option(self._h, int(option), int(value)), "kf_set_option")
+
     # ------------------------------------------------------------------ kf_graph_*
     def graph_begin(self):
         """Start recording the hot calls made on this context (kf_graph_begin)."""
@@ -341,17 +348,17 @@ class KFContext:
                     "kf_fit_tracks_indexed")
         del keep
 
-    def fit_tracks_smooth(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask, kappa: float,
+    def fit_tracks_refit(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask, kappa: float,
                           out_par, out_cov, out_chi2, out_nhits, out_status,
                           s_par, s_cov, s_chi2, s_nhits, s_status):
-        """Forward fit + inward refit (smoother) in one kernel; two result sets."""
+        """Forward fit + inward refit (reading A18) in one kernel; two result sets."""
         g, keep = geom._c()
         seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
         out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
         sm = self._tracks(n, s_par, s_cov, None, s_chi2, s_nhits, s_status)
         hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
-        self._check(self._lib.kf_fit_tracks_smooth(self._h, C.byref(g), C.byref(seeds), C.byref(hits), float(kappa),
-                                                   C.byref(out), C.byref(sm)), "kf_fit_tracks_smooth")
+        self._check(self._lib.kf_fit_tracks_refit(self._h, C.byref(g), C.byref(seeds), C.byref(hits), float(kappa),
+                                                   C.byref(out), C.byref(sm)), "kf_fit_tracks_refit")
         del keep
 
     def fit_tracks_host(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,

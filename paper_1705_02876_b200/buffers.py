@@ -67,23 +67,23 @@ class DeviceFit:
         ctx.fit_tracks(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask,
                        self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status)
 
-    def fit_smooth(self, ctx: KFContext, kappa: float = 10.0) -> dict:
-        """kf_fit_tracks_smooth; the forward result lands in the usual out_* tensors, the smoothed one in
-        tensors allocated at the first call, returned and kept as self.smoothed (later calls write into them)."""
+    def fit_refit(self, ctx: KFContext, kappa: float = 10.0) -> dict:
+        """kf_fit_tracks_refit; the forward result lands in the usual out_* tensors, the smoothed one in
+        tensors allocated at the first call, returned and kept as self.refitted (later calls write into them)."""
         dev = self.par.device
-        sm = getattr(self, "smoothed", None)
+        sm = getattr(self, "refitted", None)
         if sm is None:
             mk = lambda shape, dt: torch.zeros(shape, dtype=dt, device=dev)
             sm = dict(par=mk((6, self.ld), torch.float32), cov=mk((21, self.ld), torch.float32),
                       chi2=mk((self.ld,), torch.float32), nhits=mk((self.ld,), torch.int32), status=mk((self.ld,), torch.int32))
-        ctx.fit_tracks_smooth(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask, kappa,
+        ctx.fit_tracks_refit(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask, kappa,
                               self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status,
                               sm["par"], sm["cov"], sm["chi2"], sm["nhits"], sm["status"])
-        self.smoothed = sm
+        self.refitted = sm
         return sm
 
-    def smoothed_results(self) -> dict:
-        n, sm = self.n, self.smoothed
+    def refit_results(self) -> dict:
+        n, sm = self.n, self.refitted
         return dict(par=sm["par"][:, :n].cpu().numpy(), cov=sm["cov"][:, :n].cpu().numpy(),
                     chi2=sm["chi2"][:n].cpu().numpy(), nhits=sm["nhits"][:n].cpu().numpy(),
                     status=sm["status"][:n].cpu().numpy().view(np.uint32))

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libkf_b200.so")
 SOURCES = ["kf_api.cu", "kf_fit.cu", "kf_host.cu", "kf_bin.cu", "kf_score.cu", "kf_comb.cu", "kf_peak.cu"]
-HEADERS = ["kf_math.cuh", "kf_internal.h", "kf_score_common.cuh"]
+HEADERS = ["kf_math.cuh", "kf_pair.cuh", "kf_internal.h", "kf_score_common.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-cudart", "static"]
 
@@ -37,11 +37,20 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """One nvcc process per translation unit (they run side by side), then one link step."""
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-shared", "-o", LIB] + \
-          [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.check_call(cmd)
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    flags = NVCC_FLAGS[:-2] + (["-Xptxas", "-v"] if verbose else [])     # (-cudart static belongs to the link step)
+    procs = []
+    for src in SOURCES:
+        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        procs.append((src, obj, subprocess.Popen([_nvcc()] + flags + ["-c", "-o", obj, os.path.join(CSRC, src)])))
+    failed = [src for src, _, p in procs if p.wait() != 0]
+    if failed:
+        raise subprocess.CalledProcessError(1, "nvcc -c " + " ".join(failed))
+    subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-shared", "-o", LIB] + [obj for _, obj, _ in procs])
     return LIB
 
 

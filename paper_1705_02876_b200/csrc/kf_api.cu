@@ -1,6 +1,7 @@
 // kf_api.cu -- the C ABI of include/kf_b200.h: argument checks, host-side per-layer constants,
 // context scratch, kernel launches.  No arithmetic of the method lives here except the per-layer
 // constants (radius^2, 1/radius, Highland prefactor) that the kernels read.
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -14,9 +15,13 @@ using namespace kf;
 struct kf_graph {
     cudaGraphExec_t exec = nullptr;
     int device = 0;
+    uint64_t ctx_id = 0;      // the context whose scratch the recorded kernels point into
+    uint64_t scratch_gen = 0; // that context's scratch generation when the recording ended
 };
 
 struct kf_ctx {
+    uint64_t id = 0;          // process-wide serial number (a graph remembers which context recorded it)
+    LaunchOptions opt;
     int device = 0;
     bool capturing = false;
     cudaStream_t stream = nullptr;
@@ -28,11 +33,36 @@ struct kf_ctx {
     CombScratch comb;
     // *_host staging
     HostStage host;
+    // every reallocation of scratch and every rewrite of the bin edge tables moves this on
+    uint64_t scratch_gen() const { return bin.gen + score.gen + comb.gen; }
 };
 
 namespace {
 
-constexpr int kAbiVersion = 10;
+constexpr int kAbiVersion = 11;
+
+// Makes the context's device current for the duration of an ABI call and puts the caller's device back on
+// return (the library links its own cudart next to torch's: both see the same current device).
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device) {
+        err = cudaGetDevice(&prev);
+        if (err != cudaSuccess) { prev = -1; return; }
+        if (prev != device) err = cudaSetDevice(device);
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) {
+            int now = -1;
+            if (cudaGetDevice(&now) == cudaSuccess && now != prev) cudaSetDevice(prev);
+        }
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define KF_ON_DEVICE(c)                                    \
+    DeviceGuard kf_guard_((c)->device);                    \
+    if (kf_guard_.err != cudaSuccess) return cuda_fail((c), kf_guard_.err)
 
 int cuda_fail(kf_ctx* c, cudaError_t e) {
     if (c) c->last_cuda = (int)e;
@@ -138,6 +168,7 @@ const char* kf_strerror(int code) {
         case KF_ERR_UNSUPPORTED: return "unsupported configuration (layers > 32, |Bz| < 1e-6 T, radii not increasing, bins)";
         case KF_ERR_CUDA: return "a CUDA runtime call failed (see kf_last_cuda_error)";
         case KF_ERR_NOMEM: return "scratch allocation failed";
+        case KF_ERR_STALE: return "stale graph: its context is gone or has reallocated scratch / changed the bin grid since the recording";
         default: return "unknown error code";
     }
 }
@@ -148,10 +179,15 @@ int kf_create(kf_ctx** out, int device, void* cuda_stream) {
     int count = 0;
     cudaError_t e = cudaGetDeviceCount(&count);
     if (e != cudaSuccess || device < 0 || device >= count) return KF_ERR_CUDA;  // no CPU fallback
-    e = cudaSetDevice(device);
-    if (e != cudaSuccess) return KF_ERR_CUDA;
+    {
+        DeviceGuard g(device);   // creates the primary context of `device` if need be, leaves the caller's device current
+        if (g.err != cudaSuccess) return KF_ERR_CUDA;
+        if ((e = cudaFree(nullptr)) != cudaSuccess) return KF_ERR_CUDA;
+    }
     kf_ctx* c = new (std::nothrow) kf_ctx();
     if (!c) return KF_ERR_NOMEM;
+    static std::atomic<uint64_t> serial{0};
+    c->id = ++serial;
     c->device = device;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     *out = c;
@@ -160,7 +196,7 @@ int kf_create(kf_ctx** out, int device, void* cuda_stream) {
 
 int kf_destroy(kf_ctx* c) {
     if (!c) return KF_ERR_NULL;
-    cudaSetDevice(c->device);
+    DeviceGuard g(c->device);
     c->bin.release();
     c->score.release();
     c->comb.release();
@@ -176,14 +212,33 @@ int kf_set_stream(kf_ctx* c, void* cuda_stream) {
     return KF_OK;
 }
 
+int kf_set_option(kf_ctx* c, int option, int64_t value) {
+    if (!c) return KF_ERR_NULL;
+    switch (option) {
+        case KF_OPT_PAIR_MIN_TRACKS:
+            if (value < 0) return KF_ERR_SHAPE;
+            c->opt.pair_min_tracks = value;
+            return KF_OK;
+        case KF_OPT_REFIT_PAIR_MASKED:
+            c->opt.refit_pair_masked = value != 0;
+            return KF_OK;
+        case KF_OPT_BIN_FORM:
+            if (value < 0 || value > 2) return KF_ERR_SHAPE;
+            c->opt.bin_form = (int)value;
+            return KF_OK;
+        default:
+            return KF_ERR_UNSUPPORTED;
+    }
+}
+
 int kf_last_cuda_error(const kf_ctx* c) { return c ? c->last_cuda : 0; }
 
 // ---- CUDA-graph capture of a sequence of hot calls (include/kf_b200.h "graphs") ----------------------------
 int kf_graph_begin(kf_ctx* c) {
     if (!c) return KF_ERR_NULL;
     if (c->capturing || c->stream == nullptr) return KF_ERR_UNSUPPORTED;  // the legacy default stream cannot be captured
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    KF_ON_DEVICE(c);
+    cudaError_t e;
     // relaxed: other host threads (torch's allocator, NCCL watchdogs) may keep calling the runtime meanwhile
     if ((e = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return cuda_fail(c, e);
     c->capturing = true;
@@ -194,6 +249,7 @@ int kf_graph_end(kf_ctx* c, kf_graph** out) {
     if (!c || !out) return KF_ERR_NULL;
     *out = nullptr;
     if (!c->capturing) return KF_ERR_UNSUPPORTED;
+    KF_ON_DEVICE(c);
     c->capturing = false;
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamEndCapture(c->stream, &g);
@@ -205,6 +261,8 @@ int kf_graph_end(kf_ctx* c, kf_graph** out) {
     kf_graph* kg = new (std::nothrow) kf_graph();
     if (!kg) { cudaGraphDestroy(g); return KF_ERR_NOMEM; }
     kg->device = c->device;
+    kg->ctx_id = c->id;
+    kg->scratch_gen = c->scratch_gen();
     e = cudaGraphInstantiate(&kg->exec, g, 0);
     cudaGraphDestroy(g);
     if (e != cudaSuccess) { delete kg; return cuda_fail(c, e); }
@@ -215,8 +273,11 @@ int kf_graph_end(kf_ctx* c, kf_graph** out) {
 int kf_graph_launch(kf_ctx* c, kf_graph* g) {
     if (!c || !g || !g->exec) return KF_ERR_NULL;
     if (c->capturing || g->device != c->device) return KF_ERR_UNSUPPORTED;
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    // The recorded kernels point into the recording context's scratch and bin edge tables: a graph is stale
+    // (and is refused) once that context is gone or has reallocated scratch / rewritten the tables since.
+    if (g->ctx_id != c->id || g->scratch_gen != c->scratch_gen()) return KF_ERR_STALE;
+    KF_ON_DEVICE(c);
+    cudaError_t e;
     if ((e = cudaGraphLaunch(g->exec, c->stream)) != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;
 }
@@ -232,8 +293,8 @@ int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_hos
     if (!c) return KF_ERR_NULL;
     if (max_hits < 0 || max_host_tracks < 0 || max_host_layers < 0 || max_host_layers > KF_MAX_LAYERS)
         return KF_ERR_SHAPE;
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    KF_ON_DEVICE(c);
+    cudaError_t e;
     if (max_hits > 0) {
         e = c->bin.reserve(max_hits, 2 * (KF_MAX_BINS + 1), c->stream, true);
         if (e == cudaSuccess) e = reserve_chunked(c->bin, max_hits, KF_MAX_LAYERS, c->stream);
@@ -249,8 +310,8 @@ int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_hos
 int kf_measure_fp32_peak(kf_ctx* c, int repeats, double* tflops_out) {
     if (!c || !tflops_out) return KF_ERR_NULL;
     if (repeats < 1) return KF_ERR_SHAPE;
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    KF_ON_DEVICE(c);
+    cudaError_t e;
     float* sink = nullptr;
     if ((e = cudaMalloc(&sink, 16)) != cudaSuccess) return cuda_fail(c, e);
     const double t = measure_fp32_peak(c->stream, repeats, sink);
@@ -278,7 +339,8 @@ int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
     a.hpos = hits->pos; a.hcov = hits->cov; a.ld_hit = hits->ld; a.mask = hits->mask;
     a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
     a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
-    cudaError_t e = launch_fit(P, a, c->stream);
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_fit(P, a, c->stream, c->opt);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;
 }
@@ -314,12 +376,13 @@ int kf_fit_tracks_indexed(kf_ctx* c, const kf_geometry* geom, const kf_tracks* s
     a.hpos = nullptr; a.hcov = nullptr; a.ld_hit = 0; a.mask = nullptr;
     a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
     a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
+    KF_ON_DEVICE(c);
     cudaError_t e = launch_fit_indexed(P, H, a, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;
 }
 
-int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits,
+int kf_fit_tracks_refit(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits,
                          float kappa, kf_tracks* out, kf_tracks* smoothed) {
     if (!c || !geom || !seeds || !hits || !out || !smoothed) return KF_ERR_NULL;
     FitParams P;
@@ -345,7 +408,8 @@ int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* se
     a.spar = smoothed->par; a.scov = smoothed->cov; a.ld_s = smoothed->ld;
     a.schi2 = smoothed->chi2; a.snhits = smoothed->nhits; a.sstatus = smoothed->status;
     a.kappa = kappa;
-    cudaError_t e = launch_fit(P, a, c->stream);
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_fit(P, a, c->stream, c->opt);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;
 }
@@ -361,15 +425,15 @@ int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seed
     if (out->n != seeds->n) return KF_ERR_SHAPE;
     if ((rc = check_track_hits(hits, geom, seeds->n, false))) return rc;
     if (seeds->n == 0) return KF_OK;
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    KF_ON_DEVICE(c);
+    cudaError_t e;
     HostFitIO io;
     io.n = seeds->n; io.L = geom->n_layers;
     io.par = seeds->par; io.cov = seeds->cov; io.ld_in = seeds->ld; io.q = seeds->q;
     io.hpos = hits->pos; io.hcov = hits->cov; io.ld_hit = hits->ld; io.mask = hits->mask;
     io.opar = out->par; io.ocov = out->cov; io.ld_out = out->ld;
     io.chi2 = out->chi2; io.nhits = out->nhits; io.status = out->status;
-    e = c->host.fit(P, io);
+    e = c->host.fit(P, io, c->opt);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
 }
@@ -421,9 +485,8 @@ int kf_bin_layers(kf_ctx* c, int n_layers, const float* radius_cm, const kf_laye
             return KF_ERR_UNSUPPORTED;
         args[l] = to_bin_args(radius_cm[l], hits + l, out + l);
     }
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    e = launch_bin(c->bin, n_layers, args, c->stream);
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_bin(c->bin, n_layers, args, c->stream, c->opt);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
 }
@@ -443,9 +506,8 @@ int kf_order_candidates(kf_ctx* c, const kf_geometry* geom, int layer, const kf_
     if ((int64_t)n_eta * n_phi > KF_MAX_BINS || !(eta_max > 0.0f) || cands->n > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
     if (cands->n == 0) return KF_OK;
     if (!cands->par || !cands->q || !order) return KF_ERR_NULL;
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    e = launch_order(c->bin, P, layer, cands->n, cands->ld, cands->par, cands->q, n_eta, n_phi, eta_max, order,
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_order(c->bin, P, layer, cands->n, cands->ld, cands->par, cands->q, n_eta, n_phi, eta_max, order,
                      c->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
@@ -503,9 +565,8 @@ int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n
     a.order = order;
     a.n_eta = bins[0].n_eta; a.n_phi = bins[0].n_phi; a.eta_max = bins[0].eta_max;
     a.window_half = window_half; a.chi2_cut = chi2_cut; a.do_update = do_update ? 1 : 0;
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    e = launch_build(c->score, P, a, n_build_layers, steps, c->stream);
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_build(c->score, P, a, n_build_layers, steps, c->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
 }
@@ -544,9 +605,8 @@ int kf_build_combinatorial(kf_ctx* c, const kf_geometry* geom, int first_layer, 
     call.n_eta = bins[0].n_eta; call.n_phi = bins[0].n_phi; call.eta_max = bins[0].eta_max;
     call.window_half = window_half; call.chi2_cut = chi2_cut;
     call.hit_index = hit_index; call.ld_out = ld_out; call.n_found = n_found;
-    cudaError_t e = cudaSetDevice(c->device);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    e = launch_comb(c->comb, P, call, n_build_layers, steps, c->stream);
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_comb(c->comb, P, call, n_build_layers, steps, c->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
 }

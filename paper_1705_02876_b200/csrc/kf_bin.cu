@@ -25,6 +25,7 @@
 // the second the tangential one, the third only full evaluations); (5) a warp per bin reads the final records and
 // writes the optional SoA copies (coalesced) and the per-bin boxes.
 // Every read of the inputs is coalesced; the only scattered traffic is one 48-byte record per hit in step (3).
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 
@@ -478,6 +479,7 @@ cudaError_t BinScratch::reserve(int64_t n_items, int64_t n_bins, cudaStream_t st
     const int64_t nb = n_bins > cap_bins ? n_bins : cap_bins;
     const bool want_rec = records || cap_rec > 0;
     release();
+    ++gen;
     const size_t items_b = (size_t)(ni > 0 ? ni : 1) * sizeof(int32_t);
     const size_t bins_b = (size_t)(nb > 0 ? nb : 1) * sizeof(int32_t);
     const size_t tab_b = (size_t)(KF_MAX_BINS_INTERNAL + 1) * sizeof(float);
@@ -504,6 +506,7 @@ cudaError_t BinScratch::reserve_chunk_cnt(int64_t words, cudaStream_t stream) {
     if (chunk_cnt) cudaFree(chunk_cnt);
     chunk_cnt = nullptr;
     cap_chunk_cnt = 0;
+    ++gen;
     if ((e = cudaMalloc(&chunk_cnt, (size_t)words * sizeof(int32_t))) != cudaSuccess) return e;
     cap_chunk_cnt = words;
     return cudaSuccess;
@@ -531,6 +534,7 @@ cudaError_t BinScratch::tables(int n_eta, int n_phi, float eta_max, cudaStream_t
     // the previous tables may still be in use by queued kernels, and host_tab by a queued copy
     cudaError_t e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) return e;
+    ++gen;   // a recorded graph that bins with the old tables is stale from here on
     host_tab.assign((size_t)n_eta + 2 * (size_t)n_phi, 0.0f);
     float* he = host_tab.data();
     float* hc = he + n_eta;
@@ -561,22 +565,20 @@ size_t chunk_count_smem(int n_eta, int n_phi) {
 
 int64_t chunk_cnt_words(int64_t chunks, int nb) { return (chunks > 0 ? chunks : 1) * (int64_t)nb; }
 
-// KF_BIN_CHUNKED in the environment (read at every call: the tests switch between the two forms): 0 = never,
-// 1 = wherever it applies, unset = where it pays, i.e. groups of at least kChunkedMinHits hits (7 pools, chunked
+// Option bin_form (kf_set_option KF_OPT_BIN_FORM; the tests switch between the two forms): 1 = never,
+// 2 = wherever it applies, 0 = where it pays, i.e. groups of at least kChunkedMinHits hits (7 pools, chunked
 // against five-launch: 126 000 hits 36 / 32 us, 210 000 hits 37 / 38 us, 336 000 hits 41 / 48 us, 840 000 hits
 // 62 / 101 us; one pool of 120 000 hits 33 / 32 us).
 constexpr int64_t kChunkedMinHits = 3 << 16;   // measured crossover on 7 pools of 40 x 64 bins: 180 000 - 210 000 hits
 
-bool chunked_wanted(int64_t total_hits) {
-    const char* e = std::getenv("KF_BIN_CHUNKED");
-    if (e ? std::atoi(e) == 0 : total_hits < kChunkedMinHits) return false;
-    static const bool ok = cudaFuncSetAttribute(chunk_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                (int)chunk_count_smem(1, kChunkMaxBins)) == cudaSuccess;
-    return ok;
+bool chunked_wanted(int64_t total_hits, int bin_form) {
+    if (bin_form == 1 || (bin_form == 0 && total_hits < kChunkedMinHits)) return false;
+    return ensure_bin_attributes() == cudaSuccess;
 }
 
 // returns cudaSuccess and *done = true if the group was sorted here
-cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max, cudaStream_t stream, bool* done) {
+cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max, cudaStream_t stream, int bin_form,
+                           bool* done) {
     *done = false;
     const int nb = B.n_eta * B.n_phi;
     if (nb > kChunkMaxBins || nb > 65535 || group_max <= 0) return cudaSuccess;
@@ -585,7 +587,7 @@ cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max,
         if (!B.layer[j].pos || !B.layer[j].hit_rec) return cudaSuccess;
         total += B.layer[j].n;
     }
-    if (!chunked_wanted(total)) return cudaSuccess;
+    if (!chunked_wanted(total, bin_form)) return cudaSuccess;
     const int64_t nc = (group_max + kChunk - 1) / kChunk;
     if (nc > 65535) return cudaSuccess;
     int64_t chunks = 0;
@@ -610,6 +612,21 @@ cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max,
 
 }  // namespace
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: set once for every device a context
+// launches on (the caller has made that device current).
+cudaError_t ensure_bin_attributes() {
+    static std::atomic<uint64_t> done{0};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const uint64_t bit = 1ull << (dev & 63);
+    if (done.load(std::memory_order_acquire) & bit) return cudaSuccess;
+    e = cudaFuncSetAttribute(chunk_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)chunk_count_smem(1, kChunkMaxBins));
+    if (e == cudaSuccess) done.fetch_or(bit, std::memory_order_release);
+    return e;
+}
+
 // Scratch of the chunked sort for calls of up to max_hits hits in up to KF_MAX_LAYERS pools with any bin grid it
 // takes (kf_reserve): chunks <= max_hits / kChunk + pools.
 cudaError_t reserve_chunked(BinScratch& s, int64_t max_hits, int max_layers, cudaStream_t stream) {
@@ -618,7 +635,7 @@ cudaError_t reserve_chunked(BinScratch& s, int64_t max_hits, int max_layers, cud
 }
 
 // Bin up to kBinBatchMax layers per group of launches.  All layers share (n_eta, n_phi, eta_max).
-cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream) {
+cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream, const LaunchOptions& opt) {
     if (n_layers <= 0) return cudaSuccess;
     const int n_eta = args[0].n_eta, n_phi = args[0].n_phi;
     const int nb = n_eta * n_phi;
@@ -648,7 +665,7 @@ cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStr
             if (a.n_hits > group_max) group_max = a.n_hits;
         }
         bool done = false;
-        if ((e = try_chunk_sort(s, B, m, group_max, stream, &done)) != cudaSuccess) return e;
+        if ((e = try_chunk_sort(s, B, m, group_max, stream, opt.bin_form, &done)) != cudaSuccess) return e;
         if (done) continue;
         if (!zeroed) {
             if ((e = cudaMemsetAsync(s.counts, 0, (size_t)(nb + 1) * n_layers * sizeof(int32_t), stream)) != cudaSuccess) return e;

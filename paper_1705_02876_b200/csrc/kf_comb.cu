@@ -393,6 +393,7 @@ cudaError_t CombScratch::reserve(int64_t words, cudaStream_t stream) {
     cudaError_t e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) return e;
     release();
+    ++gen;
     if ((e = cudaMalloc(&buf, (size_t)words * 4)) != cudaSuccess) { buf = nullptr; return e; }
     cap_words = words;
     return cudaSuccess;

@@ -21,6 +21,7 @@
 // chi2, nhits, status) + 36 per layer = 593 B at 10 layers.
 #include <cuda.h>
 
+#include <atomic>
 #include <cstdlib>
 
 #include "kf_internal.h"
@@ -871,34 +872,41 @@ bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t 
 
 }  // namespace
 
-cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream) {
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: set once for every device a context
+// launches on (the caller has made that device current).
+cudaError_t ensure_fit_attributes() {
+    static std::atomic<uint64_t> done{0};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const uint64_t bit = 1ull << (dev & 63);
+    if (done.load(std::memory_order_acquire) & bit) return cudaSuccess;
+    e = cudaFuncSetAttribute(fit_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));
+    if (e == cudaSuccess) done.fetch_or(bit, std::memory_order_release);
+    return e;
+}
+
+cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream, const LaunchOptions& opt) {
     if (a.n == 0) return cudaSuccess;
-    static const cudaError_t attr = [] {
-        cudaError_t e = cudaFuncSetAttribute(fit_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-        return e;
-    }();
+    const cudaError_t attr = ensure_fit_attributes();
     if (attr != cudaSuccess) return attr;
     const bool smooth = a.spar != nullptr;
     const int L = P.n_layers;
     FitMaps M;
-    static const int64_t pair_min = [] { const char* e = getenv("KF_PAIR_MIN_TRACKS"); return e ? (int64_t)atoll(e) : (int64_t)KF_PAIR_MIN_TRACKS; }();
-    // Two tracks per thread.  The pair form of the smoother takes ragged pairs (a layer only one of the two tracks
+    const int64_t pair_min = opt.pair_min_tracks > 0 ? opt.pair_min_tracks : (int64_t)KF_PAIR_MIN_TRACKS;
+    // Two tracks per thread.  The pair form of the refit takes ragged pairs (a layer only one of the two tracks
     // has a hit on) through the one-track path and then loses badly (1.2 % of tracks stopping short: 0.81 ms against
     // 0.49 ms for 600 000 twenty-layer tracks), so it is taken only where the caller says that every track has
     // every hit (mask == NULL); the pair form of the fit parks and shadows the idle track and wins either way.
-    // (KF_PAIR_SMOOTH_MASKED in the environment lifts that condition: the tests use it to drive the pair smoother's
-    // ragged-pair code, which failures can reach without any mask, with masks.)
+    // (Option refit_pair_masked lifts that condition: the tests use it to drive the pair refit's ragged-pair code,
+    // which failures can reach without any mask, with masks.)
     if (P.geometry_options == 0 && a.n >= pair_min &&
-        (!smooth || (KF_PAIR_SMOOTH && (a.mask == nullptr || getenv("KF_PAIR_SMOOTH_MASKED") != nullptr)))) {
-        static const cudaError_t attr_pair = [] {
-            cudaError_t e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));
-            return e;
-        }();
-        if (attr_pair != cudaSuccess) return attr_pair;
+        (!smooth || (KF_PAIR_SMOOTH && (a.mask == nullptr || opt.refit_pair_masked != 0)))) {
         constexpr int W = kPairTile;
         if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3, W) ||
             !make_map(&M.hcov, a.hcov, a.n, a.ld_hit, (int64_t)L * 6, 6, W) ||

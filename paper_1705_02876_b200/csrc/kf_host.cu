@@ -65,7 +65,7 @@ void HostStage::release() {
     buf_bytes = 0;
 }
 
-cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io) {
+cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const LaunchOptions& opt) {
     cudaError_t e = reserve(io.n, io.L);
     if (e != cudaSuccess) return e;
     const SlotLayout lay(chunk, layers);
@@ -93,7 +93,7 @@ cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io) {
             a.mask = io.mask ? (const uint32_t*)(b + lay.mask) : nullptr;
             a.opar = (float*)(b + lay.opar); a.ocov = (float*)(b + lay.ocov); a.ld_out = chunk;
             a.chi2 = (float*)(b + lay.chi2); a.nhits = (int32_t*)(b + lay.nhits); a.status = (uint32_t*)(b + lay.status);
-            KF_TRY(launch_fit(P, a, st));
+            KF_TRY(launch_fit(P, a, st, opt));
         }
         KF_TRY(cudaMemcpy2DAsync(io.opar + t0, (size_t)io.ld_out * 4, b + lay.opar, cw, w, 6, cudaMemcpyDeviceToHost, st));
         KF_TRY(cudaMemcpy2DAsync(io.ocov + t0, (size_t)io.ld_out * 4, b + lay.ocov, cw, w, 21, cudaMemcpyDeviceToHost, st));

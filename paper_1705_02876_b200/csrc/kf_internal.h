@@ -9,6 +9,18 @@
 
 namespace kf {
 
+// Per-context launch options (kf_set_option): read at kf_create / set by the caller, never from the
+// environment on the launch path.
+struct LaunchOptions {
+    int64_t pair_min_tracks = 0;   // 0: the built-in rule (tracks x layers); > 0: batches of at least this many tracks take the pair kernels
+    int refit_pair_masked = 0;     // 1: the pair form of the refit also for batches with a hit mask (tests)
+    int bin_form = 0;              // 0: by size; 1: always the five-launch sort; 2: the chunked sort wherever it applies
+};
+
+// One-time per-device kernel attributes (dynamic shared memory above 48 KB is a per-device function attribute).
+cudaError_t ensure_fit_attributes();
+cudaError_t ensure_bin_attributes();
+
 // ---------------------------------------------------------------------------------- fit
 struct FitArgs {
     int64_t n;
@@ -40,7 +52,7 @@ struct IndexedPools {           // per-layer hit pools + the per-track hit indic
 
 // kf_fit.cu
 cudaError_t launch_fit_indexed(const FitParams& P, const IndexedPools& H, const FitArgs& a, cudaStream_t stream);
-cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream);
+cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream, const LaunchOptions& opt = LaunchOptions());
 
 // ---------------------------------------------------------------------------------- host path
 struct HostFitIO {
@@ -60,7 +72,7 @@ struct HostStage {
     char* buf[kSlots] = {nullptr, nullptr, nullptr};
     size_t buf_bytes = 0;
     cudaError_t reserve(int64_t max_tracks, int max_layers);
-    cudaError_t fit(const FitParams& P, const HostFitIO& io);
+    cudaError_t fit(const FitParams& P, const HostFitIO& io, const LaunchOptions& opt);
     void release();
 };
 
@@ -101,6 +113,7 @@ struct BinBatch {
 };
 
 struct BinScratch {
+    uint64_t gen = 0;            // bumped whenever a buffer is reallocated or the edge tables are rewritten (kf_graph staleness)
     int64_t cap_items = 0, cap_bins = 0;
     int32_t* key = nullptr;
     int32_t* unsorted = nullptr;
@@ -124,7 +137,7 @@ struct BinScratch {
 };
 
 // kf_bin.cu
-cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream);
+cudaError_t launch_bin(BinScratch& s, int n_layers, const BinArgs* args, cudaStream_t stream, const LaunchOptions& opt = LaunchOptions());
 cudaError_t reserve_chunked(BinScratch& s, int64_t max_hits, int max_layers, cudaStream_t stream);
 cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n, int64_t ld, const float* par,
                          const int8_t* q, int n_eta, int n_phi, float eta_max, int32_t* order,
@@ -163,6 +176,7 @@ struct ScoreStep {
 };
 
 struct ScoreScratch {
+    uint64_t gen = 0;
     int64_t cap = 0, ld = 0;
     float* scratch = nullptr;  // [kScorePlanes][ld] propagated candidate (scan + update inputs)
     float* track = nullptr;    // [29][ld] local-frame track between layers
@@ -186,6 +200,7 @@ struct CombCall {
 };
 
 struct CombScratch {
+    uint64_t gen = 0;
     int64_t cap_words = 0;
     void* buf = nullptr;
     cudaError_t reserve(int64_t words, cudaStream_t stream);

@@ -232,6 +232,7 @@ cudaError_t ScoreScratch::reserve(int64_t n, cudaStream_t stream) {
     cudaError_t e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) return e;
     release();
+    ++gen;
     const int64_t ldn = (n + 3) / 4 * 4;
     if ((e = cudaMalloc(&scratch, (size_t)kScorePlanes * ldn * 4)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&track, (size_t)29 * ldn * 4)) != cudaSuccess) { release(); return e; }

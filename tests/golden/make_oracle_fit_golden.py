@@ -18,9 +18,9 @@ from workloads import barrel_events as W   # noqa: E402
 
 def compute():
     b = W.simulate_event(W.get_config(1), 0, n_tracks=8)
-    r = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
+    r = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
     rows = np.concatenate([r["par"].T, r["chi2"][:, None], r["nhits"][:, None].astype(float),
-                           r["spar"].T, r["schi2"][:, None]], axis=1)
+                           r["rpar"].T, r["rchi2"][:, None]], axis=1)
     return rows
 
 

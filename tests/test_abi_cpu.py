@@ -44,13 +44,13 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_abi_version_and_error_strings(lib):
     import paper_1705_02876_b200 as K
-    assert K.abi_version() == 10
+    assert K.abi_version() == 11
     seen = set()
-    for code in (0, -1, -2, -3, -4, -5, -6, -99):
+    for code in (0, -1, -2, -3, -4, -5, -6, -7, -99):
         s = K.strerror(code)
         assert isinstance(s, str) and s
         seen.add(s)
-    assert len(seen) == 8
+    assert len(seen) == 9
 
 
 def test_null_arguments_are_rejected_without_a_device(lib):
@@ -59,7 +59,7 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_fit_tracks(None, None, None, None, None) == -1
     assert lib.kf_fit_tracks_host(None, None, None, None, None) == -1
     assert lib.kf_fit_tracks_indexed(None, None, None, None, 0, None, None, None) == -1
-    assert lib.kf_fit_tracks_smooth(None, None, None, None, 10.0, None, None) == -1
+    assert lib.kf_fit_tracks_refit(None, None, None, None, 10.0, None, None) == -1
     assert lib.kf_bin_hits(None, 1.0, None, None) == -1
     assert lib.kf_score_candidates(None, None, 0, None, None, None, 2, 30.0, 1, None, None, None) == -1
     assert lib.kf_bin_layers(None, 1, None, None, None) == -1
@@ -68,6 +68,7 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_order_candidates(None, None, 0, None, 40, 64, 1.2, None) == -1
     assert lib.kf_measure_fp32_peak(None, 3, None) == -1
     assert lib.kf_last_cuda_error(None) == 0
+    assert lib.kf_set_option(None, 1, 0) == -1
     assert lib.kf_graph_begin(None) == -1
     assert lib.kf_graph_end(None, None) == -1
     assert lib.kf_graph_launch(None, None) == -1

@@ -97,11 +97,12 @@ def _host_fit(ctx, b):
     return h.results()
 
 
-@pytest.mark.parametrize("chunked", ["1", "0"])
-def test_bin_32_layers_in_one_call(ctx, chunked, monkeypatch):
+@pytest.mark.parametrize("chunked", [2, 1])
+def test_bin_32_layers_in_one_call(ctx, chunked):
     """KF_MAX_LAYERS pools in one kf_bin_layers call (two launch groups of 16), ragged sizes (1 to 3 chunks of the
     chunked sort per pool), one empty pool; both forms of the sort."""
-    monkeypatch.setenv("KF_BIN_CHUNKED", chunked)
+    import paper_1705_02876_b200 as K
+    ctx.set_option(K.OPT_BIN_FORM, chunked)       # 2 = chunked sort wherever it applies, 1 = five-launch sort
     from paper_1705_02876_b200.buffers import DeviceLayer
     rng = np.random.default_rng(41)
     pools, radii = [], []
@@ -113,7 +114,10 @@ def test_bin_32_layers_in_one_call(ctx, chunked, monkeypatch):
         cov = rng.uniform(1e-4, 1e-2, (6, H)).astype(np.float32)
         pools.append((pos, cov)); radii.append(r)
     dls = [DeviceLayer.from_numpy(p, c, NE, NP, EMAX, "cuda:0") for p, c in pools]
-    ctx.bin_layers(radii, [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+    try:
+        ctx.bin_layers(radii, [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+    finally:
+        ctx.set_option(K.OPT_BIN_FORM, K.BIN_FORM_AUTO)
     torch.cuda.synchronize()
     for l, (d, (pos, cov)) in enumerate(zip(dls, pools)):
         ob = O.bin_hits(pos, radii[l], NE, NP, EMAX)

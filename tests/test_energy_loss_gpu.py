@@ -1,4 +1,4 @@
-"""GPU parity of the energy-loss option (reading A21) in kf_fit_tracks, kf_fit_tracks_smooth and
+"""GPU parity of the energy-loss option (reading A21) in kf_fit_tracks, kf_fit_tracks_refit and
 kf_fit_tracks_indexed against the oracle, alone and together with the geometry options of reading A20.  The two
 builders are covered with the option in test_score_gpu.py / test_comb_gpu.py."""
 import numpy as np
@@ -108,27 +108,27 @@ def test_a_track_that_would_stop_fails_the_layer(ctx):
                 float(b.radius[-1]), max_diverged_frac=0.02)
 
 
-def test_smooth_with_energy_loss(ctx):
+def test_refit_with_energy_loss(ctx):
     from paper_1705_02876_b200.buffers import DeviceFit
     b = _soft_thick(20000, 4)
     d = DeviceFit.from_batch(b, "cuda:0")
-    d.fit_smooth(ctx)
+    d.fit_refit(ctx)
     torch.cuda.synchronize()
     with O.geometry_options(energy_loss=1):
-        o = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
-    g, sg = d.results(), d.smoothed_results()
+        o = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
+    g, sg = d.results(), d.refit_results()
     fwd = compare_fit(g, o, float(b.radius[-1]), max_diverged_frac=2e-3)
     keep = o["nhits"] >= 3
-    assert np.array_equal(sg["status"][keep], o["sstatus"][keep])
+    assert np.array_equal(sg["status"][keep], o["rstatus"][keep])
     ndf = np.maximum(2 * o["nhits"] - 5, 1)
-    excl = o["status"] | o["sstatus"] | ((o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)).astype(np.uint32) << 5)
-    so = dict(par=o["spar"][:, keep], cov=o["scov"][keep], chi2=o["schi2"][keep], nhits=o["nhits"][keep], status=excl[keep])
+    excl = o["status"] | o["rstatus"] | ((o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)).astype(np.uint32) << 5)
+    so = dict(par=o["rpar"][:, keep], cov=o["rcov"][keep], chi2=o["rchi2"][keep], nhits=o["nhits"][keep], status=excl[keep])
     gs = dict(par=sg["par"][:, keep], cov=sg["cov"][:, keep], chi2=sg["chi2"][keep], nhits=o["nhits"][keep], status=excl[keep])
     res = compare_fit(gs, so, float(b.radius[-1]), max_diverged_frac=5e-3)
     print("forward:", fwd, "smoothed with energy loss:", res)
     # the refit gives the energy back: at the innermost layer the smoothed momentum exceeds the forward one
     # (taken at the outermost layer) by about the ten layers' loss
-    ok = (o["status"] == 0) & (o["sstatus"] == 0)
+    ok = (o["status"] == 0) & (o["rstatus"] == 0)
     dp = np.linalg.norm(sg["par"][3:6, ok], axis=0) - np.linalg.norm(g["par"][3:6, ok], axis=0)
     assert 5e-3 < np.median(dp) < 3e-2
 

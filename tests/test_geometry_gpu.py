@@ -1,5 +1,5 @@
 """GPU parity of the geometry options (reading A20: path-length material, finite barrels) in
-kf_fit_tracks and kf_fit_tracks_smooth against the oracle.  The builder and the combinatorial builder are
+kf_fit_tracks and kf_fit_tracks_refit against the oracle.  The builder and the combinatorial builder are
 covered with the same options in test_score_gpu.py / test_comb_gpu.py.
 
 A crossing within fp32 rounding of the barrel end may fall on either side in the two precisions; such tracks
@@ -91,28 +91,28 @@ def test_fit_generated_with_the_same_geometry(ctx):
     assert np.median(np.abs(g0["cov"][20, ok] / g["cov"][20, ok] - 1.0)) > 1e-3     # C_pzpz
 
 
-def test_smooth_with_geometry_options(ctx):
+def test_refit_with_geometry_options(ctx):
     from paper_1705_02876_b200.buffers import DeviceFit
     b = W.simulate_event(W.get_config(3), 2, n_tracks=20000)
     hl = np.full(b.n_layers, 60.0, dtype=np.float32)
     b.half_length, b.material_model = hl, 1
     d = DeviceFit.from_batch(b, "cuda:0")
-    d.fit_smooth(ctx)
+    d.fit_refit(ctx)
     torch.cuda.synchronize()
     with O.geometry_options(1, hl.astype(np.float64)):
-        o = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask,
+        o = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask,
                                 want_trace=True)
     edge = _near_edge(dict(trace=o["trace_fwd"]), hl.astype(np.float64))
     keep = ~edge & (o["nhits"] >= 3)
     assert edge.mean() < 5e-3
-    g, sg = d.results(), d.smoothed_results()
+    g, sg = d.results(), d.refit_results()
     assert np.array_equal(g["status"][keep] & OUT, o["status"][keep] & OUT)
     assert np.array_equal(g["nhits"][keep], o["nhits"][keep])
     # the inward pass runs over layers the forward pass used: it stays inside the barrel
-    assert np.array_equal(sg["status"][keep], o["sstatus"][keep])
+    assert np.array_equal(sg["status"][keep], o["rstatus"][keep])
     ndf = np.maximum(2 * o["nhits"] - 5, 1)
-    excl = (o["status"] & ~OUT) | o["sstatus"] | ((o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)).astype(np.uint32) << 5)
-    so = dict(par=o["spar"][:, keep], cov=o["scov"][keep], chi2=o["schi2"][keep], nhits=o["nhits"][keep], status=excl[keep])
+    excl = (o["status"] & ~OUT) | o["rstatus"] | ((o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)).astype(np.uint32) << 5)
+    so = dict(par=o["rpar"][:, keep], cov=o["rcov"][keep], chi2=o["rchi2"][keep], nhits=o["nhits"][keep], status=excl[keep])
     gs = dict(par=sg["par"][:, keep], cov=sg["cov"][:, keep], chi2=sg["chi2"][keep], nhits=o["nhits"][keep], status=excl[keep])
     res = compare_fit(gs, so, float(b.radius[-1]), max_diverged_frac=5e-3)
     print("smoothed with options:", res)

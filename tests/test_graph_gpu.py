@@ -87,20 +87,20 @@ def test_fit_and_smooth_graph_equals_eager(ctx):
     b = W.simulate_event(W.get_config(1), 3, n_tracks=20000)
     d = DeviceFit.from_batch(b, "cuda:0")
     with torch.cuda.stream(ctx.torch_stream):
-        d.fit_smooth(ctx)
+        d.fit_refit(ctx)
     torch.cuda.synchronize()
-    want, want_s = d.results(), d.smoothed_results()
+    want, want_s = d.results(), d.refit_results()
     ctx.graph_begin()
-    d.fit_smooth(ctx)
+    d.fit_refit(ctx)
     g = ctx.graph_end()
     d.out_par.zero_(); d.out_cov.zero_(); d.out_chi2.zero_()
-    for v in d.smoothed.values():                 # (fit_smooth writes into the same tensors at every call)
+    for v in d.refitted.values():                 # (fit_smooth writes into the same tensors at every call)
         v.zero_()
     torch.cuda.synchronize()
     g.launch()
     g.launch()                                    # a graph may be launched any number of times
     torch.cuda.synchronize()
-    got, got_s = d.results(), d.smoothed_results()
+    got, got_s = d.results(), d.refit_results()
     for k in want:
         assert np.array_equal(got[k], want[k], equal_nan=True), k
     for k in want_s:
@@ -147,3 +147,61 @@ def test_graph_errors_leave_the_context_usable(ctx):
     again = d.results()
     for k in first:
         assert np.array_equal(first[k], again[k], equal_nan=True)
+
+
+def test_stale_graph_is_refused(ctx):
+    """A recorded graph points into its context's scratch and bin edge tables.  Once that context reallocates
+    scratch (a bigger pool) or bins with another grid, or the graph is handed to another context, kf_graph_launch
+    refuses it (KF_ERR_STALE = -7) instead of replaying against freed memory or the wrong edges."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceLayer
+    rng = np.random.default_rng(8)
+
+    def pool(H, ne=NE, nph=NP):
+        phi, eta = rng.uniform(-np.pi, np.pi, H), rng.uniform(-1.1, 1.1, H)
+        pos = np.stack([10 * np.cos(phi), 10 * np.sin(phi), 10 * np.sinh(eta)]).astype(np.float32)
+        cov = np.tile(np.array([1e-2, 0, 0, 1e-2, 0, 1e-2], dtype=np.float32)[:, None], (1, H))
+        return DeviceLayer.from_numpy(pos, cov, ne, nph, EMAX, "cuda:0")
+
+    def record(dl):
+        with torch.cuda.stream(ctx.torch_stream):
+            dl.bin(ctx, 10.0)                      # eager once: sizes the scratch, writes the tables
+        torch.cuda.synchronize()
+        ctx.graph_begin()
+        dl.bin(ctx, 10.0)
+        return ctx.graph_end()
+
+    small = pool(3000)
+    g = record(small)
+    g.launch()                                     # fresh: fine
+    torch.cuda.synchronize()
+    want = small.bins.bin_offset.cpu().numpy().copy()
+    # (1) another grid rewrites the edge tables in place
+    other = pool(3000, 7, 10)
+    with torch.cuda.stream(ctx.torch_stream):
+        other.bin(ctx, 10.0)
+    torch.cuda.synchronize()
+    with pytest.raises(K.KFError) as e:
+        g.launch()
+    assert e.value.code == -7
+    g.close()
+    # (2) a bigger pool reallocates the scratch
+    g = record(small)
+    big = pool(400_000)
+    with torch.cuda.stream(ctx.torch_stream):
+        big.bin(ctx, 10.0)
+    torch.cuda.synchronize()
+    with pytest.raises(K.KFError) as e:
+        g.launch()
+    assert e.value.code == -7
+    g.close()
+    # (3) re-recorded, it runs again and gives the same bins; another context is refused
+    g = record(small)
+    small.bins.bin_offset.fill_(0)
+    g.launch()
+    torch.cuda.synchronize()
+    assert np.array_equal(small.bins.bin_offset.cpu().numpy(), want)
+    c2 = K.KFContext(0, ctx.torch_stream)
+    assert c2._lib.kf_graph_launch(c2._h, g._g) == -7
+    c2.close()
+    g.close()

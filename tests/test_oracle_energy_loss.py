@@ -173,14 +173,14 @@ def test_E5_momentum_pulls_need_the_energy_loss():
 
 def _smoothed_pull(b, eloss):
     with O.geometry_options(energy_loss=eloss):
-        r = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
+        r = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
     ndf = 2 * r["nhits"] - 5
-    good = (r["status"] == 0) & (r["sstatus"] == 0) & (r["nhits"] == b.n_layers) & \
+    good = (r["status"] == 0) & (r["rstatus"] == 0) & (r["nhits"] == b.n_layers) & \
            (r["chi2"] <= ndf + 9 * np.sqrt(2.0 * ndf))
     truth = b.truth[0]                                   # just after the innermost layer
-    pf = r["spar"][3:6][:, good]
+    pf = r["rpar"][3:6][:, good]
     n = pf / np.linalg.norm(pf, axis=0)
-    var = np.einsum("in,nij,jn->n", n, r["scov"][good][:, 3:, 3:], n)
+    var = np.einsum("in,nij,jn->n", n, r["rcov"][good][:, 3:, 3:], n)
     return (np.linalg.norm(pf, axis=0) - np.linalg.norm(truth[3:6][:, good], axis=0)) / np.sqrt(var)
 
 

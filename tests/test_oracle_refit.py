@@ -61,12 +61,12 @@ def test_S1_inward_propagation_inverts_outward_and_jacobian():
 def test_S2_exact_helix_recovered_at_innermost_layer():
     cfg = W.get_config(0)
     b = W.simulate_event(cfg, 7, n_tracks=200, smear_hits=False, smear_seed=False, dtype=np.float64)
-    r = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
-    assert np.all(r["sstatus"] == 0) and np.all(r["status"] == 0)
+    r = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
+    assert np.all(r["rstatus"] == 0) and np.all(r["status"] == 0)
     truth0 = b.truth[0]
-    np.testing.assert_allclose(r["spar"][:3], truth0[:3], rtol=0, atol=1e-8)
-    np.testing.assert_allclose(r["spar"][3:], truth0[3:], rtol=1e-8, atol=1e-9)
-    assert np.max(r["schi2"]) < 1e-10
+    np.testing.assert_allclose(r["rpar"][:3], truth0[:3], rtol=0, atol=1e-8)
+    np.testing.assert_allclose(r["rpar"][3:], truth0[3:], rtol=1e-8, atol=1e-9)
+    assert np.max(r["rchi2"]) < 1e-10
 
 
 def _batch_wls_backward(x0, C0, trace, hits, Vs, layers):
@@ -108,28 +108,28 @@ def _batch_wls_backward(x0, C0, trace, hits, Vs, layers):
 def test_S3_backward_ekf_equals_batch_wls(config, L):
     cfg = W.get_config(config)
     b = W.simulate_event(cfg, 3, n_tracks=10)
-    r = O.fit_smooth_tracks(b.radius[:L], b.x_over_X0[:L], b.Bz, b.mass, b.par, b.cov, b.q, b.hpos[:L], b.hcov[:L],
+    r = O.fit_refit_tracks(b.radius[:L], b.x_over_X0[:L], b.Bz, b.mass, b.par, b.cov, b.q, b.hpos[:L], b.hcov[:L],
                             None, want_trace=True)
     Vs = O.unpack_cov6(b.hcov[:L])
     for i in range(b.n):
-        assert r["status"][i] == 0 and r["sstatus"][i] == 0
+        assert r["status"][i] == 0 and r["rstatus"][i] == 0
         hits = b.hpos[:L, :, i].astype(np.float64)
-        x0, C0 = r["par"][:, i], O.SMOOTH_KAPPA * r["cov"][i]
+        x0, C0 = r["par"][:, i], O.REFIT_KAPPA * r["cov"][i]
         x, Cx, cost = _batch_wls_backward(x0, C0, r["trace_bwd"][i], hits, Vs[i], list(range(L - 1, -1, -1)))
-        np.testing.assert_allclose(r["spar"][:, i], x, rtol=1e-9, atol=1e-9)
-        assert np.max(np.abs(r["scov"][i] - Cx)) < 1e-8 * np.max(np.abs(Cx))
-        assert r["schi2"][i] == pytest.approx(cost, rel=1e-8, abs=1e-9)
+        np.testing.assert_allclose(r["rpar"][:, i], x, rtol=1e-9, atol=1e-9)
+        assert np.max(np.abs(r["rcov"][i] - Cx)) < 1e-8 * np.max(np.abs(Cx))
+        assert r["rchi2"][i] == pytest.approx(cost, rel=1e-8, abs=1e-9)
 
 
 def test_S4_smoothed_pulls_and_gain_over_forward_filter():
     b = W.make_fit_batch(1)
     n = 6000
     sl = lambda a: np.ascontiguousarray(a[..., :n])
-    r = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, sl(b.par), sl(b.cov), sl(b.q), sl(b.hpos), sl(b.hcov), sl(b.mask))
+    r = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, sl(b.par), sl(b.cov), sl(b.q), sl(b.hpos), sl(b.hcov), sl(b.mask))
     ndf = 2 * r["nhits"] - 5
-    good = (r["status"] == 0) & (r["sstatus"] == 0) & (r["chi2"] <= ndf + 9 * np.sqrt(2.0 * ndf))
+    good = (r["status"] == 0) & (r["rstatus"] == 0) & (r["chi2"] <= ndf + 9 * np.sqrt(2.0 * ndf))
     assert good.mean() > 0.995
-    x, Cs, truth = r["spar"][:, good], r["scov"][good], b.truth[0][:, :n][:, good]
+    x, Cs, truth = r["rpar"][:, good], r["rcov"][good], b.truth[0][:, :n][:, good]
     d = x - truth
     phi = np.arctan2(x[1], x[0])
     tvec = np.stack([-np.sin(phi), np.cos(phi)])
@@ -140,7 +140,7 @@ def test_S4_smoothed_pulls_and_gain_over_forward_filter():
         assert abs(p.mean()) < 0.05, (name, p.mean())
         assert 0.93 < p.std() < 1.12, (name, p.std())
     # backward chi2 has 2 n_hits degrees of freedom minus 5 fitted, plus the weak prior: ~ same as forward
-    assert 0.9 < (r["schi2"][good] / ndf[good]).mean() < 1.15
+    assert 0.9 < (r["rchi2"][good] / ndf[good]).mean() < 1.15
     # all hits constrain the innermost point: its momentum is known as well as at the outermost layer and far
     # better than a forward filter knows it after one hit (prior 0.3 pT)
     pabs = np.linalg.norm(x[3:], axis=0)
@@ -156,9 +156,9 @@ def test_S5_nothing_fitted_comes_back_untouched():
     b.q[5] = 0
     b.mask[9] = 0
     for _ in range(3):                       # repeated: an uninitialised read would not be stable
-        r = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
-        assert r["status"][5] == O.BAD_CHARGE and r["sstatus"][5] == 0 and r["status"][9] == 0 and r["sstatus"][9] == 0
+        r = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
+        assert r["status"][5] == O.BAD_CHARGE and r["rstatus"][5] == 0 and r["status"][9] == 0 and r["rstatus"][9] == 0
         for i in (5, 9):
-            np.testing.assert_array_equal(r["spar"][:, i], b.par[:, i].astype(np.float64))
-            np.testing.assert_array_equal(O.pack_cov21(r["scov"][i:i + 1])[:, 0], b.cov[:, i].astype(np.float64))
-            assert r["schi2"][i] == 0 and r["nhits"][i] == 0
+            np.testing.assert_array_equal(r["rpar"][:, i], b.par[:, i].astype(np.float64))
+            np.testing.assert_array_equal(O.pack_cov21(r["rcov"][i:i + 1])[:, 0], b.cov[:, i].astype(np.float64))
+            assert r["rchi2"][i] == 0 and r["nhits"][i] == 0

@@ -112,3 +112,45 @@ def test_scoring_reject_and_no_update(small_event):
     assert (r1["best_hit"] >= 0).mean() > 0.9
     np.testing.assert_array_equal(a.par, b.par)          # do_update=0 leaves the propagated state too
     np.testing.assert_array_equal(b.nhits, nh)
+
+
+def test_chi2_increment_equals_its_definition_and_the_update():
+    """orc_chi2_increment is what every accept / cut / ranking decision rests on (reading A8):
+    chi2 = r^T (C'_pp + V)^-1 r with r = m - H u.  Pinned against (i) the definition evaluated by numpy on the
+    same numbers (a dropped V, a wrong block of C or a transposed index changes it), (ii) the chi2 that orc_update
+    returns for the same inputs (which pin P4 ties to the batch weighted least squares), (iii) the closed form for
+    a diagonal case, and (iv) S_NOT_PD on an S that is not positive definite."""
+    rng = np.random.default_rng(17)
+    for it in range(1200):
+        u = rng.normal(size=6) * np.array([20, 20, 20, 3, 3, 3])
+        # C': symmetric PSD of rank 5 with a general null direction (as the to-radius transport leaves it),
+        # with position / momentum scales far apart and full correlations
+        A = rng.normal(size=(6, 5)) * np.array([3e-2, 3e-2, 1e-1, 0.3, 0.3, 0.3])[:, None]
+        Cm = A @ A.T
+        B = rng.normal(size=(3, 3)) * np.array([0.1, 0.01, 0.1])[:, None]
+        V = B @ B.T + 1e-6 * np.eye(3)
+        m = u[:3] + rng.normal(size=3) * 0.2
+        rc, c = O.chi2_increment(u, Cm, m, V)
+        assert rc == 0
+        r = m - u[:3]
+        want = r @ np.linalg.solve(Cm[:3, :3] + V, r)
+        assert c == pytest.approx(want, rel=1e-10)
+        rc2, _, _, c2 = O.update(u, Cm, m, V)
+        assert rc2 == 0 and c2 == pytest.approx(c, rel=1e-13)
+        # sensitivity: the same call with V dropped, or with the momentum block in place of the position block,
+        # gives a different number (so the two checks above would catch either slip)
+        if it < 50:
+            assert abs(r @ np.linalg.solve(Cm[:3, :3] + 1e-9 * np.eye(3), r) - c) > 1e-6 * c
+            assert abs(r @ np.linalg.solve(Cm[3:, 3:] + V, r) - c) > 1e-6 * c
+    # closed form: diagonal C and V -> sum of squared pulls
+    u = np.array([1.0, 2.0, 3.0, 0.5, 0.5, 0.5])
+    Cd = np.diag([0.04, 0.09, 0.16, 1.0, 1.0, 1.0])
+    Vd = np.diag([0.05, 0.07, 0.09])
+    m = np.array([1.3, 1.6, 3.5])
+    rc, c = O.chi2_increment(u, Cd, m, Vd)
+    assert rc == 0 and c == pytest.approx(0.3 ** 2 / 0.09 + 0.4 ** 2 / 0.16 + 0.5 ** 2 / 0.25, rel=1e-13)
+    # S not positive definite (det <= 0): refused, by the increment and by the update alike
+    Vbad = np.diag([-1.0, 0.07, 0.09])
+    assert O.chi2_increment(u, Cd, m, Vbad)[0] == O.S_NOT_PD
+    assert O.update(u, Cd, m, Vbad)[0] == O.S_NOT_PD
+    assert O.chi2_increment(u, np.zeros((6, 6)), m, np.zeros((3, 3)))[0] == O.S_NOT_PD

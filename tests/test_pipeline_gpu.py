@@ -132,3 +132,40 @@ def test_chain_bin_build_fit(ctx):
     o = _oracle_fit_with(ev, full)
     res = compare_fit(g, o, float(f.radius[-1]), max_diverged_frac=0.2, loosen=dict(cov=3.0))
     print("chain final-fit parity:", res)
+
+
+def test_indexed_fit_config2_full_size(ctx):
+    """kf_fit_tracks_indexed at the size bench.py times it: config 2 (2 M tracks x 10 layers), every layer's hits
+    shuffled into one pool of 2 M hits, read from the SoA pools and (second call) from the packed records of
+    kf_bin_layers.  Both must equal, bit for bit, each other; the oracle checks every 16th event track by track."""
+    from paper_1705_02876_b200.binding import Bins
+    from paper_1705_02876_b200.buffers import DeviceFit
+    cfg = W.get_config(2)
+    b = W.make_fit_batch(2)
+    n, L = b.n, b.n_layers
+    assert n == 2_000_000
+    d = DeviceFit.from_batch(b, "cuda:0")
+    gen = torch.Generator(device="cuda:0"); gen.manual_seed(5)
+    pools, index = [], torch.full((L, d.ld), -1, dtype=torch.int32, device="cuda:0")
+    for l in range(L):
+        perm = torch.randperm(n, device="cuda:0", generator=gen)
+        pp = torch.zeros((3, d.ld), dtype=torch.float32, device="cuda:0"); pc = torch.zeros((6, d.ld), dtype=torch.float32, device="cuda:0")
+        pp[:, :n] = d.hpos[l][:, :n][:, perm]; pc[:, :n] = d.hcov[l][:, :n][:, perm]
+        inv = torch.empty(n, dtype=torch.int64, device="cuda:0"); inv[perm] = torch.arange(n, device="cuda:0")
+        index[l, :n] = inv.to(torch.int32)
+        pools.append((n, pp, pc))
+    d.hpos = d.hcov = None                                   # (free 0.7 GB: the indexed call does not read them)
+    ctx.fit_tracks_indexed(d.geom, n, d.par, d.cov, d.q, index, pools, d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status)
+    torch.cuda.synchronize()
+    g = d.results()
+    pbins = [Bins.allocate(n, NE, NP, EMAX, "cuda:0", soa=False) for _ in range(L)]
+    ctx.bin_layers([float(r) for r in d.geom.radius_cm], [(n, pp, pc, b_) for (_, pp, pc), b_ in zip(pools, pbins)])
+    ctx.fit_tracks_indexed(d.geom, n, d.par, d.cov, d.q, index, pools, d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status, bins=pbins)
+    torch.cuda.synchronize()
+    g2 = d.results()
+    for k in g:
+        assert np.array_equal(g[k], g2[k], equal_nan=True), k
+    for ev in range(0, cfg.n_events, 16):
+        lo, hi = ev * cfg.n_tracks, (ev + 1) * cfg.n_tracks
+        o = O.fit_batch(W.simulate_event(cfg, ev), nthreads=8)
+        compare_fit({k: (v[..., lo:hi] if k in ("par", "cov") else v[lo:hi]) for k, v in g.items()}, o, float(b.radius[-1]))

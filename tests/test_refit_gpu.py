@@ -1,4 +1,4 @@
-"""GPU parity of kf_fit_tracks_smooth (forward fit + inward refit, reading A18) against the oracle."""
+"""GPU parity of kf_fit_tracks_refit (forward fit + inward refit, reading A18) against the oracle."""
 import numpy as np
 import pytest
 import torch
@@ -18,31 +18,40 @@ def ctx():
     c.close()
 
 
-def _both(ctx, b, kappa=O.SMOOTH_KAPPA, with_mask=True):
+@pytest.fixture()
+def pair_masked(ctx):
+    """Large masked batches through the two-tracks-per-thread refit too (the product takes it only without a mask)."""
+    import paper_1705_02876_b200 as K
+    ctx.set_option(K.OPT_REFIT_PAIR_MASKED, 1)
+    yield
+    ctx.set_option(K.OPT_REFIT_PAIR_MASKED, 0)
+
+
+def _both(ctx, b, kappa=O.REFIT_KAPPA, with_mask=True):
     from paper_1705_02876_b200.buffers import DeviceFit
     d = DeviceFit.from_batch(b, "cuda:0", with_mask=with_mask)
-    d.fit_smooth(ctx, kappa)
+    d.fit_refit(ctx, kappa)
     torch.cuda.synchronize()
-    o = O.fit_smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask, kappa=kappa)
+    o = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask, kappa=kappa)
     return d, o
 
 
 def _compare(d, o, r_last, max_div=1e-3, loosen=None):
     fwd = compare_fit(d.results(), {k: o[k] for k in ("par", "cov", "chi2", "nhits", "status")}, r_last, max_div, loosen)
-    sg = d.smoothed_results()
-    assert np.array_equal(sg["status"], o["sstatus"])
+    sg = d.refit_results()
+    assert np.array_equal(sg["status"], o["rstatus"])
     # Smoothed result, same metric.  Excluded (A14): tracks the FORWARD fit flagged or that diverged there, and
     # tracks the backward pass flagged -- marked through the status word compare_fit looks at.
     ndf = np.maximum(2 * o["nhits"] - 5, 1)
     fwd_div = o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)
-    excl = o["status"] | o["sstatus"] | (fwd_div.astype(np.uint32) << 4)
-    so = dict(par=o["spar"], cov=o["scov"], chi2=o["schi2"], nhits=o["nhits"], status=excl)
+    excl = o["status"] | o["rstatus"] | (fwd_div.astype(np.uint32) << 4)
+    so = dict(par=o["rpar"], cov=o["rcov"], chi2=o["rchi2"], nhits=o["nhits"], status=excl)
     sm = compare_fit(dict(sg, status=excl, nhits=o["nhits"]), so, r_last, max_diverged_frac=max(max_div, 2e-3), loosen=loosen)
     return fwd, sm
 
 
 @pytest.mark.parametrize("config", [0, 1, 3])
-def test_smooth_parity_full_config(ctx, config):
+def test_refit_parity_full_config(ctx, config):
     b = W.make_fit_batch(config)
     d, o = _both(ctx, b)
     fwd, sm = _compare(d, o, float(b.radius[-1]))
@@ -51,8 +60,7 @@ def test_smooth_parity_full_config(ctx, config):
 
 @pytest.mark.parametrize("n_layers,step,n", [(32, 2.5, 3000), (32, 2.5, 160_000), (1, 4.0, 700), (2, 4.0, 700), (3, 4.0, 700),
                                              (3, 4.0, 160_000)])
-def test_smooth_extreme_layer_counts(ctx, n_layers, step, n, monkeypatch):
-    monkeypatch.setenv("KF_PAIR_SMOOTH_MASKED", "1")     # large masked batches through the pair smoother too
+def test_refit_extreme_layer_counts(ctx, n_layers, step, n, pair_masked):
     """KF_MAX_LAYERS layers (64 steps of the hit ring; pair and one-track kernels) and geometries with fewer layers
     than the hit ring has stages, where the ring's first round already holds steps of the backward pass (one
     layer: the refit is a single update of the inflated forward result)."""
@@ -69,18 +77,18 @@ def test_smooth_extreme_layer_counts(ctx, n_layers, step, n, monkeypatch):
     assert n_layers > 3 or (fwd["mom_p99"] <= 0.5 and sm["mom_p99"] <= 0.5)
 
 
-def test_smooth_forward_part_equals_plain_fit(ctx):
+def test_refit_forward_part_equals_plain_fit(ctx):
     from paper_1705_02876_b200.buffers import DeviceFit
     b = W.make_fit_batch(1)
     d1 = DeviceFit.from_batch(b, "cuda:0"); d1.fit(ctx)
-    d2 = DeviceFit.from_batch(b, "cuda:0"); d2.fit_smooth(ctx)
+    d2 = DeviceFit.from_batch(b, "cuda:0"); d2.fit_refit(ctx)
     torch.cuda.synchronize()
     r1, r2 = d1.results(), d2.results()
     for k in r1:
         assert np.array_equal(r1[k], r2[k]), k
 
 
-def test_smooth_ragged_masks_and_flags(ctx):
+def test_refit_ragged_masks_and_flags(ctx):
     b = W.simulate_event(W.get_config(1), 8, n_tracks=1003)
     rng = np.random.default_rng(3)
     b.mask = (rng.integers(0, 1 << 10, size=b.n) | 0b111).astype(np.uint32)
@@ -89,16 +97,16 @@ def test_smooth_ragged_masks_and_flags(ctx):
     d, o = _both(ctx, b)
     sel = o["nhits"] >= 5
     sel[:31] = False
-    sg, so_ = d.smoothed_results(), o
+    sg, so_ = d.refit_results(), o
     sub = lambda r, keys: {k: (r[k][..., sel] if k in ("par", "cov") else r[k][sel]) for k in keys}
     g = sub(sg, ("par", "cov", "chi2", "nhits", "status"))
-    oo = dict(par=o["spar"][:, sel], cov=o["scov"][sel], chi2=o["schi2"][sel], nhits=g["nhits"], status=o["sstatus"][sel])
+    oo = dict(par=o["rpar"][:, sel], cov=o["rcov"][sel], chi2=o["rchi2"][sel], nhits=g["nhits"], status=o["rstatus"][sel])
     compare_fit(g, oo, float(b.radius[-1]), max_diverged_frac=0.05)
     assert np.array_equal(sg["par"][:, :31], b.par[:, :31]) and np.array_equal(sg["cov"][:, :31], b.cov[:, :31])
     assert np.all(sg["chi2"][:31] == 0)
 
 
-def test_smooth_pair_kernel_without_mask(ctx):
+def test_refit_pair_kernel_without_mask(ctx):
     """The product's rule: a batch of >= 151 552 tracks WITHOUT a mask (every track has every hit) takes the
     two-tracks-per-thread smoother; with a mask the one-track kernel.  Same results within the tolerances, and
     the masked call (all bits set) agrees with the oracle too."""
@@ -109,15 +117,14 @@ def test_smooth_pair_kernel_without_mask(ctx):
     _compare(d, o, float(b.radius[-1]))
     d2, _ = _both(ctx, b, with_mask=True)
     _compare(d2, o, float(b.radius[-1]))
-    np.testing.assert_allclose(d.smoothed_results()["chi2"], d2.smoothed_results()["chi2"], rtol=2e-3, atol=2e-3)
+    np.testing.assert_allclose(d.refit_results()["chi2"], d2.refit_results()["chi2"], rtol=2e-3, atol=2e-3)
 
 
-def test_smooth_pair_kernel_edge_cases(ctx, monkeypatch):
+def test_refit_pair_kernel_edge_cases(ctx, pair_masked):
     """The two-tracks-per-thread smoother on ragged pairs: pairs whose tracks used different layers (or where one
     fails) go through the one-track refit step.  (With a mask the product takes the one-track kernel; the
     environment switch sends this masked batch through the pair kernel so that its ragged-pair code, which failures
     reach without any mask, is covered.)"""
-    monkeypatch.setenv("KF_PAIR_SMOOTH_MASKED", "1")
     cfg = W.get_config(1)
     b = W.concat_batches([W.simulate_event(cfg, 50 + e) for e in range(8)] + [W.simulate_event(cfg, 58, n_tracks=3)])
     assert b.n == 160_003
@@ -130,19 +137,46 @@ def test_smooth_pair_kernel_edge_cases(ctx, monkeypatch):
     b.hpos[4, 1, 201] = np.nan            # NONFINITE on layer 4 of track 201: skipped forward, so never revisited
     b.mask[200] = b.mask[201] = 0x3ff
     d, o = _both(ctx, b)
-    g, sg = d.results(), d.smoothed_results()
+    g, sg = d.results(), d.refit_results()
     assert np.array_equal(g["status"], o["status"]) and np.array_equal(g["nhits"], o["nhits"])
-    assert np.array_equal(sg["status"], o["sstatus"]), np.flatnonzero(sg["status"] != o["sstatus"])[:10]
-    assert o["status"][201] == 4 and o["sstatus"][201] == 0 and o["nhits"][201] == 9 and o["status"][100] == 8
+    assert np.array_equal(sg["status"], o["rstatus"]), np.flatnonzero(sg["status"] != o["rstatus"])[:10]
+    assert o["status"][201] == 4 and o["rstatus"][201] == 0 and o["nhits"][201] == 9 and o["status"][100] == 8
     untouched = (o["nhits"] == 0)
     assert untouched.sum() >= 31
     assert np.array_equal(sg["par"][:, untouched], b.par[:, untouched]) and np.array_equal(sg["cov"][:, untouched], b.cov[:, untouched])
     assert np.all(sg["chi2"][untouched] == 0)
-    sel = (o["nhits"] >= 5) & (o["status"] == 0) & (o["sstatus"] == 0)
+    sel = (o["nhits"] >= 5) & (o["status"] == 0) & (o["rstatus"] == 0)
     fwd = compare_fit({k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in g},
                       dict(par=o["par"][:, sel], cov=o["cov"][sel], chi2=o["chi2"][sel], nhits=o["nhits"][sel], status=o["status"][sel]),
                       float(b.radius[-1]), max_diverged_frac=0.02)
-    sm = compare_fit(dict(par=sg["par"][:, sel], cov=sg["cov"][:, sel], chi2=sg["chi2"][sel], nhits=o["nhits"][sel], status=o["sstatus"][sel]),
-                     dict(par=o["spar"][:, sel], cov=o["scov"][sel], chi2=o["schi2"][sel], nhits=o["nhits"][sel], status=o["sstatus"][sel]),
+    sm = compare_fit(dict(par=sg["par"][:, sel], cov=sg["cov"][:, sel], chi2=sg["chi2"][sel], nhits=o["nhits"][sel], status=o["rstatus"][sel]),
+                     dict(par=o["rpar"][:, sel], cov=o["rcov"][sel], chi2=o["rchi2"][sel], nhits=o["nhits"][sel], status=o["rstatus"][sel]),
                      float(b.radius[-1]), max_diverged_frac=0.02)
     print(f"pair smoother: forward {fwd}\n               smoothed {sm}")
+
+
+def test_refit_parity_config2_sampled(ctx):
+    """The refit at the size bench.py times it (config 2: 2 M tracks, no mask -> pair kernel; then with a mask ->
+    one-track kernel); the oracle checks every 16th event track by track, as test_fit_parity_config2_sampled does."""
+    from paper_1705_02876_b200.buffers import DeviceFit
+    cfg = W.get_config(2)
+    b = W.make_fit_batch(2)
+    assert b.n == 2_000_000
+    for with_mask in (False, True):
+        d = DeviceFit.from_batch(b, "cuda:0", with_mask=with_mask)
+        d.fit_refit(ctx, O.REFIT_KAPPA)
+        torch.cuda.synchronize()
+        g, sg = d.results(), d.refit_results()
+        del d
+        for ev in range(0, cfg.n_events, 16):
+            lo, hi = ev * cfg.n_tracks, (ev + 1) * cfg.n_tracks
+            sub = W.simulate_event(cfg, ev)
+            o = O.fit_refit_tracks(sub.radius, sub.x_over_X0, sub.Bz, sub.mass, sub.par, sub.cov, sub.q, sub.hpos, sub.hcov, sub.mask)
+
+            class _D:                                    # the slice of the big launch dressed as a DeviceFit
+                def results(self_):
+                    return {k: (v[..., lo:hi] if k in ("par", "cov") else v[lo:hi]) for k, v in g.items()}
+
+                def refit_results(self_):
+                    return {k: (v[..., lo:hi] if k in ("par", "cov") else v[lo:hi]) for k, v in sg.items()}
+            _compare(_D(), o, float(b.radius[-1]))

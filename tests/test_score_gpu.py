@@ -22,11 +22,13 @@ def ctx():
 
 
 @pytest.fixture(params=["chunked", "five_launch"])
-def sort_path(request, monkeypatch):
+def sort_path(request, ctx):
     """Both forms of the counting sort: the chunked one (taken for calls of >= 196 608 hits) and the five-launch
-    one (small calls, more than 8192 bins).  KF_BIN_CHUNKED, read at every call, forces either for any size."""
-    monkeypatch.setenv("KF_BIN_CHUNKED", "0" if request.param == "five_launch" else "1")
-    return request.param
+    one (small calls, more than 8192 bins).  kf_set_option(KF_OPT_BIN_FORM) forces either for any size."""
+    import paper_1705_02876_b200 as K
+    ctx.set_option(K.OPT_BIN_FORM, K.BIN_FORM_FIVE_LAUNCH if request.param == "five_launch" else K.BIN_FORM_CHUNKED)
+    yield request.param
+    ctx.set_option(K.OPT_BIN_FORM, K.BIN_FORM_AUTO)
 
 
 def _bin_both(ctx, pos, cov, radius, ne=NE, nph=NP, emax=EMAX):
@@ -111,6 +113,52 @@ def test_bin_hits_large_layer(ctx, sort_path):
     cov = rng.uniform(1e-4, 1e-2, (6, H)).astype(np.float32)
     dl, ob = _bin_both(ctx, pos, cov, r)
     _assert_bins_equal(dl, ob, pos, cov)
+
+
+def test_bin_hits_against_the_double_definition(ctx, sort_path):
+    """Reading A16b makes both sides decide a hit's bin by the same single-precision edge-table rule, which is
+    why bin_offset / sorted_to_orig are bit-exact.  THIS test compares the product with the DEFINITION
+    (PAPER.md:71 projective bins; reading A16: eta = asinh(z/r), phi = atan2(y, x), evaluated in double by
+    orc_bin_index_def): the bin the library gave a hit may differ from the definition's only where the hit lies
+    within rounding (1e-6 relative of a bin width ... fp32 carries 6e-8, the edge tables another 6e-8) of a bin
+    edge; such hits are counted and must be rare."""
+    rng = np.random.default_rng(31)
+    H = 300_000
+    r = 16.0
+    phi, eta = rng.uniform(-np.pi, np.pi, H), rng.uniform(-1.3, 1.3, H)
+    pos = np.stack([r * np.cos(phi), r * np.sin(phi), r * np.sinh(eta)]).astype(np.float32)
+    # a few hundred hits placed ON edges (to within fp32 rounding), where the two rules may legitimately differ
+    k = 600
+    pe = -np.pi + rng.integers(0, NP, k) * (2 * np.pi / NP)
+    ee = -EMAX + rng.integers(1, NE, k) * (2 * EMAX / NE)
+    pos[:, :k] = np.stack([r * np.cos(pe), r * np.sin(pe), r * np.sinh(rng.uniform(-1.1, 1.1, k))]).astype(np.float32)
+    pos[:, k:2 * k] = np.stack([r * np.cos(phi[k:2 * k]), r * np.sin(phi[k:2 * k]), r * np.sinh(ee)]).astype(np.float32)
+    cov = np.tile(np.array([1e-2, 0, 0, 1e-2, 0, 1e-2], dtype=np.float32)[:, None], (1, H))
+    dl, _ = _bin_both(ctx, pos, cov, r)
+    off = dl.bins.bin_offset.cpu().numpy()
+    s2o = dl.bins.sorted_to_orig.cpu().numpy()[:H]
+    gpu_bin = np.empty(H, dtype=np.int64)
+    gpu_bin[s2o] = np.repeat(np.arange(NE * NP), np.diff(off))
+    # the definition, in double, on the same fp32 inputs (vectorised restatement of orc_bin_index_def, which is
+    # called itself on every hit that differs and on a sample)
+    x, y, z = (pos[i].astype(np.float64) for i in range(3))
+    fe = (np.arcsinh(z / r) + EMAX) / (2 * EMAX / NE)
+    fp = (np.arctan2(y, x) + np.pi) / (2 * np.pi / NP)
+    def_bin = np.clip(np.floor(fe), 0, NE - 1).astype(np.int64) * NP + (np.floor(fp).astype(np.int64) % NP)
+    for i in rng.integers(0, H, 2000):
+        assert def_bin[i] == O.bin_index_def(x[i], y[i], z[i], r, NE, NP, EMAX)
+    differ = np.flatnonzero(gpu_bin != def_bin)
+    for i in differ:
+        assert def_bin[i] == O.bin_index_def(x[i], y[i], z[i], r, NE, NP, EMAX)
+        d_eta = abs(fe[i] - np.round(fe[i])) if 0.5 < fe[i] < NE - 0.5 else 1.0     # (the outermost edges clamp)
+        d_phi = abs(fp[i] - np.round(fp[i]))
+        assert min(d_eta, d_phi) < 1e-5, (i, fe[i], fp[i])       # within rounding of an edge (bin widths)
+        # ... and the library's bin is the neighbour across that edge
+        ge, gp = divmod(int(gpu_bin[i]), NP); de, dp = divmod(int(def_bin[i]), NP)
+        assert abs(ge - de) + min((gp - dp) % NP, (dp - gp) % NP) == 1, (i, gpu_bin[i], def_bin[i])
+    print(f"bins vs the double definition: {len(differ)} of {H} hits differ, all within 1e-5 bin widths of an edge")
+    assert len(differ) <= 2 * k                                   # only hits placed on edges (plus a stray few)
+    assert np.count_nonzero(differ >= 2 * k) <= 5
 
 
 def test_bin_layers_batched_equals_per_layer(ctx, sort_path):

@@ -74,8 +74,11 @@ enum {
     KF_STATUS_S_NOT_PD = 2,   /* det S <= 0                                                         */
     KF_STATUS_NONFINITE = 4,  /* update produced a non-finite state or chi2                         */
     KF_STATUS_BAD_CHARGE = 8, /* q not in {+1, -1}: track is copied through untouched               */
-    KF_STATUS_OUTSIDE = 16    /* a crossing fell beyond the end of the barrel (|z'| > half_length_cm):
+    KF_STATUS_OUTSIDE = 16,   /* a crossing fell beyond the end of the barrel (|z'| > half_length_cm):
                                  that layer was skipped (reading A20)                      */
+    KF_STATUS_SMOOTH_FAIL = 32 /* kf_fit_tracks_smooth only: a backward step could not be taken (predicted
+                                 covariance not positive definite / non-finite); that layer and the layers
+                                 further in carry the FILTERED state                                  */
 };
 
 #define KF_MAX_LAYERS 32
@@ -210,6 +213,31 @@ KF_API int kf_fit_tracks(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* 
  * kernel runs, whose speed does not depend on how ragged the tracks are.  Results agree within the tolerances. */
 KF_API int kf_fit_tracks_refit(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                                const kf_track_hits* hits, float kappa, kf_tracks* out, kf_tracks* refitted);
+
+/* ---- fit + smoother (section 2: "a final fit with a KF and smoother"; reading A22) -------
+ * The forward fit of kf_fit_tracks followed by the fixed-interval (Rauch-Tung-Striebel) smoother over the layers
+ * the fit used, k_0 < ... < k_{m-1}: x^s = x^+ at the outermost one, then, outer to inner,
+ *     A = C^+_k G^T (C^-_n)^+,   x^s_k = x^+_k + A (x^s_n - x^-_n),   C^s_k = C^+_k + A (C^s_n - C^-_n) A^T
+ * with x^+_k, C^+_k the filtered state of layer k, x^-_n, C^-_n the filter's prediction for the next used layer n
+ * and G the Jacobian between them: at EVERY used layer the estimate, from ALL hits of the track, of the state just
+ * after that layer's scatter.  It equals the weighted least squares of the linearised track model evaluated at
+ * that layer (the oracle's pin SM1).  Layout: layer-major, element-major inside a layer. */
+typedef struct {
+    int n_layers;             /* must equal geometry n_layers                                      */
+    int64_t n, ld;            /* n tracks; plane stride ld >= n, ld % 4 == 0                       */
+    float* par;               /* DEV [n_layers][6][ld]  smoothed x y z px py pz at layer l          */
+    float* cov;               /* DEV [n_layers][21][ld] its covariance, packed upper triangle       */
+    uint32_t* used;           /* DEV [n] bit l set = layer l was used by the fit and has a smoothed
+                                 state; the slots of other layers are not written                   */
+} kf_smoothed;
+
+/* `out` receives the forward result exactly as kf_fit_tracks writes it (it equals the smoothed state at the
+ * outermost used layer); `out` may alias `seeds`.  While the call runs, sm->par / sm->cov also hold its
+ * intermediate per-layer states (no other scratch is used).  A backward step that fails sets
+ * KF_STATUS_SMOOTH_FAIL in out->status (see there).  geom->energy_loss_model must be 0 (KF_ERR_UNSUPPORTED
+ * otherwise); path-length material and finite barrels are honoured.  All pointers DEV.  Two kernels. */
+KF_API int kf_fit_tracks_smooth(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                                const kf_track_hits* hits, kf_tracks* out, kf_smoothed* sm);
 
 /* Same call with every pointer HOST (pageable or pinned): copies in, fits, copies out, in chunks
  * pipelined over internal streams, and returns when `out` is complete.  This is the end-to-end

@@ -340,8 +340,11 @@ int orc_update(const double u[6], const double C[36], const double m[3], const d
 /* ---- one track, all layers (readings A10, A11): layers in increasing radius; a layer whose
  * mask bit is 0 is skipped entirely; a layer that fails (propagation / S / non-finite) sets the
  * status bit and leaves state and covariance as they were before that layer.
- * trace (optional): per layer 122 doubles = x_pred[6] F[36] Q[36] x_filt[6] C_filt[36] dchi2 used */
-#define ORC_TRACE_STRIDE 122
+ * trace (optional): per layer 194 doubles = x_pred[6] F[36] Q[36] x_filt[6] C_filt[36] dchi2 used
+ *                   C_pred[36] G[36], where x_pred / C_pred are the predicted state and covariance the update
+ *                   was given (after the energy-loss step of reading A21 when that option is on) and G is the
+ *                   Jacobian of the whole map previous filtered state -> x_pred (G = F, or J F with energy loss) */
+#define ORC_TRACE_STRIDE 194
 static void fit_one(int L, const double *radius, const double *xX0, double Bz, double mass,
                     const double par[6], const double cov[36], int q, const double *hpos,
                     const double *hcov, uint32_t mask, double opar[6], double ocov[36],
@@ -366,7 +369,18 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
             if (rc) { st |= (uint32_t)rc; continue; }
             orc_process_noise(up, mass, xX0[l], Q);
             orc_transport_cov(F, C, Q, Cp);
-            if (g_energy_loss) rc = orc_energy_loss_step(up, Cp, mass, xX0[l], +1, NULL); /* A21 */
+            double G[36];
+            memcpy(G, F, sizeof G);
+            if (g_energy_loss) { /* A21 */
+                double J[36];
+                rc = orc_energy_loss_step(up, Cp, mass, xX0[l], +1, J);
+                for (int i = 0; i < 6; ++i)
+                    for (int j = 0; j < 6; ++j) {
+                        double acc = 0.0;
+                        for (int m = 0; m < 6; ++m) acc += J[i * 6 + m] * F[m * 6 + j];
+                        G[i * 6 + j] = acc;
+                    }
+            }
             if (rc) { st |= (uint32_t)rc; continue; }
             rc = orc_update(up, Cp, hpos + 3 * l, hcov + 9 * l, un, Cn, &dchi2);
             if (rc) { st |= (uint32_t)rc; continue; }
@@ -382,6 +396,8 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
                 memcpy(tr + 84, C, 36 * sizeof(double));
                 tr[120] = dchi2;
                 tr[121] = 1.0;
+                memcpy(tr + 122, Cp, 36 * sizeof(double));
+                memcpy(tr + 158, G, 36 * sizeof(double));
             }
         }
     }
@@ -392,7 +408,202 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
     *ostatus = st;
 }
 
-/* ---- backward refit / smoother (reading A18; "a final fit with a KF and smoother") ---------
+/* ---- fixed-interval smoother (reading A22; "a final fit with a KF and smoother") ----------------
+ * The Rauch-Tung-Striebel recursion over the layers the forward filter used, k_0 < k_1 < ... < k_{m-1}, on the
+ * model that filter linearised (its own predictions x^-_k, C^-_k, Jacobians G_k, filtered x^+_k, C^+_k):
+ *     x^s_{m-1} = x^+_{m-1},  C^s_{m-1} = C^+_{m-1};   then for j = m-2 ... 0, with n = k_{j+1}:
+ *     A     = C^+_j G_n^T (C^-_n)^+
+ *     x^s_j = x^+_j + A (x^s_n - x^-_n)
+ *     C^s_j = C^+_j + A (C^s_n - C^-_n) A^T
+ * x^s_k is the best estimate, given ALL hits of the track, of the state just after the scatter of layer k (the
+ * state the forward filter's x^+_k estimates from the hits up to k).  It equals the batch weighted-least-squares
+ * solution of the linearised model evaluated at every layer (pin SM1).
+ * (C^-_n)^+ is the pseudo-inverse: a covariance transported to a cylinder has no variance along the radial
+ * direction e = (x^-, y^-, 0; 0, 0, 0)/rho of the predicted point (reading A4, pin P5), so with that known unit
+ * null vector   (C^-)^+ = (C^- + s e e^T)^-1 - e e^T / s   for any s > 0 (s = largest position variance). */
+static int inv6(const double M[36], double Mi[36]) { /* Gauss-Jordan with partial pivoting on the symmetrically
+                                                        scaled matrix D M D, D = diag(1/sqrt(M_ii)) */
+    double a[6][12], d[6];
+    for (int i = 0; i < 6; ++i) {
+        if (!(M[i * 6 + i] > 0.0)) return -1;
+        d[i] = 1.0 / sqrt(M[i * 6 + i]);
+    }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+            a[i][j] = d[i] * M[i * 6 + j] * d[j];
+            a[i][6 + j] = i == j ? 1.0 : 0.0;
+        }
+    for (int c = 0; c < 6; ++c) {
+        int piv = c;
+        for (int r = c + 1; r < 6; ++r)
+            if (fabs(a[r][c]) > fabs(a[piv][c])) piv = r;
+        if (!(fabs(a[piv][c]) > 0.0)) return -1;
+        if (piv != c)
+            for (int j = 0; j < 12; ++j) { double t = a[c][j]; a[c][j] = a[piv][j]; a[piv][j] = t; }
+        double ip = 1.0 / a[c][c];
+        for (int j = 0; j < 12; ++j) a[c][j] *= ip;
+        for (int r = 0; r < 6; ++r) {
+            if (r == c) continue;
+            double f = a[r][c];
+            for (int j = 0; j < 12; ++j) a[r][j] -= f * a[c][j];
+        }
+    }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) Mi[i * 6 + j] = d[i] * a[i][6 + j] * d[j];
+    return 0;
+}
+
+/* pseudo-inverse of a predicted covariance whose only null direction is the radial position direction of xp */
+static int pinv_radial_null(const double Cp[36], const double xp[6], double out[36]) {
+    double rho = sqrt(xp[0] * xp[0] + xp[1] * xp[1]);
+    if (!(rho > 0.0)) return -1;
+    double e[6] = {xp[0] / rho, xp[1] / rho, 0.0, 0.0, 0.0, 0.0};
+    double s = fmax(fmax(Cp[0], Cp[7]), Cp[14]);
+    if (!(s > 0.0)) return -1;
+    double M[36];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) M[i * 6 + j] = Cp[i * 6 + j] + s * e[i] * e[j];
+    if (inv6(M, out)) return -1;
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) out[i * 6 + j] -= e[i] * e[j] / s;
+    return 0;
+}
+
+/* Forward fit (fit_one) + RTS smoother.  Forward outputs as fit_one; spar[L][6] / scov[L][36] = smoothed state
+ * and covariance at every used layer (zeros elsewhere); *used_out = bit mask of those layers.  A smoothing step
+ * whose predicted covariance cannot be inverted stops the recursion there: the layers further in keep their
+ * FILTERED state and *sstatus gets ORC_S_NOT_PD (never seen on the workloads; kept so that nothing is undefined). */
+void orc_smooth_one(int L, const double *radius, const double *xX0, double Bz, double mass, const double par[6],
+                    const double cov[36], int q, const double *hpos, const double *hcov, uint32_t mask,
+                    double opar[6], double ocov[36], double *ochi2, int32_t *onhits, uint32_t *ostatus,
+                    double *spar, double *scov, uint32_t *used_out, uint32_t *sstatus) {
+    double *tr = (double *)calloc((size_t)L * ORC_TRACE_STRIDE, sizeof(double));
+    fit_one(L, radius, xX0, Bz, mass, par, cov, q, hpos, hcov, mask, opar, ocov, ochi2, onhits, ostatus, tr);
+    memset(spar, 0, (size_t)L * 6 * sizeof(double));
+    memset(scov, 0, (size_t)L * 36 * sizeof(double));
+    uint32_t used = 0;
+    for (int l = 0; l < L; ++l)
+        if (tr[(size_t)l * ORC_TRACE_STRIDE + 121] != 0.0) used |= 1u << l;
+    *used_out = used;
+    *sstatus = 0;
+    int next = -1, broken = 0;
+    for (int l = L - 1; l >= 0; --l) {
+        if (!((used >> l) & 1u)) continue;
+        const double *t = tr + (size_t)l * ORC_TRACE_STRIDE;
+        const double *xf = t + 78, *Cf = t + 84;
+        double *xs = spar + 6 * l, *Cs = scov + 36 * l;
+        if (next < 0 || broken) { /* outermost used layer (or recursion stopped): smoothed = filtered */
+            memcpy(xs, xf, 6 * sizeof(double));
+            memcpy(Cs, Cf, 36 * sizeof(double));
+            next = l;
+            continue;
+        }
+        const double *tn = tr + (size_t)next * ORC_TRACE_STRIDE;
+        const double *xpn = tn, *Cpn = tn + 122, *Gn = tn + 158;
+        const double *xsn = spar + 6 * next, *Csn = scov + 36 * next;
+        double Ni[36], CG[36], A[36], D[36], AD[36];
+        if (pinv_radial_null(Cpn, xpn, Ni)) {
+            *sstatus |= ORC_S_NOT_PD;
+            broken = 1;
+            memcpy(xs, xf, 6 * sizeof(double));
+            memcpy(Cs, Cf, 36 * sizeof(double));
+            next = l;
+            continue;
+        }
+        for (int i = 0; i < 6; ++i) /* C^+ G^T */
+            for (int j = 0; j < 6; ++j) {
+                double acc = 0.0;
+                for (int m = 0; m < 6; ++m) acc += Cf[i * 6 + m] * Gn[j * 6 + m];
+                CG[i * 6 + j] = acc;
+            }
+        for (int i = 0; i < 6; ++i) /* A = C^+ G^T (C^-)^+ */
+            for (int j = 0; j < 6; ++j) {
+                double acc = 0.0;
+                for (int m = 0; m < 6; ++m) acc += CG[i * 6 + m] * Ni[m * 6 + j];
+                A[i * 6 + j] = acc;
+            }
+        for (int i = 0; i < 6; ++i) {
+            double acc = 0.0;
+            for (int m = 0; m < 6; ++m) acc += A[i * 6 + m] * (xsn[m] - xpn[m]);
+            xs[i] = xf[i] + acc;
+        }
+        for (int i = 0; i < 36; ++i) D[i] = Csn[i] - Cpn[i];
+        for (int i = 0; i < 6; ++i)
+            for (int j = 0; j < 6; ++j) {
+                double acc = 0.0;
+                for (int m = 0; m < 6; ++m) acc += A[i * 6 + m] * D[m * 6 + j];
+                AD[i * 6 + j] = acc;
+            }
+        for (int i = 0; i < 6; ++i)
+            for (int j = 0; j < 6; ++j) {
+                double acc = 0.0;
+                for (int m = 0; m < 6; ++m) acc += AD[i * 6 + m] * A[j * 6 + m];
+                Cs[i * 6 + j] = Cf[i * 6 + j] + acc;
+            }
+        for (int i = 0; i < 6; ++i) /* symmetrise (the two triangles differ by rounding only) */
+            for (int j = i + 1; j < 6; ++j) {
+                double v = 0.5 * (Cs[i * 6 + j] + Cs[j * 6 + i]);
+                Cs[i * 6 + j] = v;
+                Cs[j * 6 + i] = v;
+            }
+        next = l;
+    }
+    free(tr);
+}
+
+typedef struct {
+    int64_t lo, hi;
+    int L;
+    const double *radius, *xX0;
+    double Bz, mass;
+    const double *par, *cov;
+    const int8_t *q;
+    const double *hpos, *hcov;
+    const uint32_t *mask;
+    double *opar, *ocov, *ochi2;
+    int32_t *onhits;
+    uint32_t *ostatus;
+    double *spar, *scov;
+    uint32_t *used, *sstatus;
+} smooth_job;
+
+static void *smooth_range(void *p) {
+    smooth_job *j = (smooth_job *)p;
+    for (int64_t i = j->lo; i < j->hi; ++i)
+        orc_smooth_one(j->L, j->radius, j->xX0, j->Bz, j->mass, j->par + 6 * i, j->cov + 36 * i, j->q[i],
+                       j->hpos + (size_t)i * j->L * 3, j->hcov + (size_t)i * j->L * 9,
+                       j->mask ? j->mask[i] : 0xffffffffu, j->opar + 6 * i, j->ocov + 36 * i, j->ochi2 + i,
+                       j->onhits + i, j->ostatus + i, j->spar + (size_t)i * j->L * 6,
+                       j->scov + (size_t)i * j->L * 36, j->used + i, j->sstatus + i);
+    return NULL;
+}
+
+/* Batched fit + smoother.  AoS double inputs as orc_fit_tracks; spar[n][L][6], scov[n][L][36], used[n], sstatus[n]. */
+int orc_smooth_tracks(int64_t n, int L, const double *radius, const double *xX0, double Bz, double mass,
+                      const double *par, const double *cov, const int8_t *q, const double *hpos, const double *hcov,
+                      const uint32_t *mask, double *opar, double *ocov, double *ochi2, int32_t *onhits,
+                      uint32_t *ostatus, double *spar, double *scov, uint32_t *used, uint32_t *sstatus, int nthreads) {
+    if (nthreads < 1) nthreads = 1;
+    if (nthreads > 256) nthreads = 256;
+    smooth_job jobs[256];
+    pthread_t th[256];
+    for (int t = 0; t < nthreads; ++t) {
+        smooth_job j = {n * t / nthreads, n * (t + 1) / nthreads, L, radius, xX0, Bz, mass, par, cov, q, hpos, hcov,
+                        mask, opar, ocov, ochi2, onhits, ostatus, spar, scov, used, sstatus};
+        jobs[t] = j;
+    }
+    if (nthreads == 1) {
+        smooth_range(&jobs[0]);
+        return 0;
+    }
+    for (int t = 0; t < nthreads; ++t)
+        if (pthread_create(&th[t], NULL, smooth_range, &jobs[t])) return -1;
+    for (int t = 0; t < nthreads; ++t) pthread_join(th[t], NULL);
+    return 0;
+}
+
+/* ---- backward refit (reading A18; round 1's stand-in for the smoother -- the smoother proper is orc_smooth_one
+ * above; this inward refit counts the forward information 1 + 1/kappa times) ---------
  * Starts from the forward result (u, C) standing at the outermost used hit layer, with the covariance
  * inflated by kappa (the forward information is kept only as a weak prior), and runs the same filter
  * inward over the same hits:
@@ -465,7 +676,7 @@ static void refit_inward_one(int L, const double *radius, const double *xX0, dou
 }
 
 /* Forward fit followed by the inward refit.  Outputs: forward result (opar/ocov/ochi2/onhits/ostatus) and
- * smoothed result at the innermost used layer (spar/scov/schi2).  sstatus = bits of the backward pass.
+ * refitted result at the innermost used layer (spar/scov/schi2).  sstatus = bits of the backward pass.
  * used_out (optional) = layers the forward fit used. */
 void orc_fit_refit_one(int L, const double *radius, const double *xX0, double Bz, double mass, double kappa,
                         const double par[6], const double cov[36], int q, const double *hpos,

@@ -18,7 +18,7 @@ _SRC = os.path.join(_HERE, "kf_oracle.c")
 _LIB = os.path.join(_HERE, "libkf_oracle.so")
 
 PROP_FAIL, S_NOT_PD, NONFINITE, BAD_CHARGE, OUTSIDE = 1, 2, 4, 8, 16
-TRACE_STRIDE = 122
+TRACE_STRIDE = 194
 
 _lib = None
 
@@ -52,6 +52,7 @@ def lib():
         _lib.orc_update.restype = C.c_int
         _lib.orc_update.argtypes = [dp, dp, dp, dp, dp, dp, dp]
         _lib.orc_fit_tracks.restype = C.c_int
+        _lib.orc_smooth_tracks.restype = C.c_int
         _lib.orc_bin_index_def.restype = C.c_int32
         _lib.orc_bin_index_def.argtypes = [C.c_double] * 4 + [C.c_int, C.c_int, C.c_double]
         _lib.orc_bin_index_f32.restype = C.c_int32
@@ -237,6 +238,34 @@ def fit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None
     if want_trace:
         out["trace"] = trace
     return out
+
+
+def smooth_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mask=None, nthreads: int = 1) -> dict:
+    """Forward fit + RTS smoother (reading A22).  Same input layout as fit_tracks.  Returns the forward results
+    under the usual keys plus spar[L][6][n], scov[n][L][6][6] (smoothed state / covariance at every used layer,
+    zeros elsewhere), used[n] (bit mask of those layers) and sstatus[n]."""
+    L = int(len(radius))
+    n = int(par.shape[1])
+    rad = np.ascontiguousarray(radius, dtype=np.float64)
+    xx0 = np.ascontiguousarray(x_over_X0, dtype=np.float64)
+    par_a = np.ascontiguousarray(np.asarray(par, dtype=np.float64).T)
+    cov_a = np.ascontiguousarray(unpack_cov21(np.asarray(cov21, dtype=np.float64)))
+    q_a = np.ascontiguousarray(q, dtype=np.int8)
+    hp_a = np.ascontiguousarray(np.transpose(np.asarray(hpos, dtype=np.float64), (2, 0, 1)))
+    hc_a = np.ascontiguousarray(unpack_cov6(hcov))
+    m_a = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint32)
+    opar = np.zeros((n, 6)); ocov = np.zeros((n, 6, 6)); ochi2 = np.zeros(n)
+    onh = np.zeros(n, dtype=np.int32); ost = np.zeros(n, dtype=np.uint32)
+    spar = np.zeros((n, L, 6)); scov = np.zeros((n, L, 6, 6))
+    used = np.zeros(n, dtype=np.uint32); sst = np.zeros(n, dtype=np.uint32)
+    rc = lib().orc_smooth_tracks(C.c_int64(n), C.c_int(L), _p(rad), _p(xx0), C.c_double(Bz), C.c_double(mass),
+                                 _p(par_a), _p(cov_a), _p(q_a, C.c_int8), _p(hp_a), _p(hc_a), _p(m_a, C.c_uint32),
+                                 _p(opar), _p(ocov), _p(ochi2), _p(onh, C.c_int32), _p(ost, C.c_uint32), _p(spar),
+                                 _p(scov), _p(used, C.c_uint32), _p(sst, C.c_uint32), C.c_int(nthreads))
+    if rc != 0:
+        raise RuntimeError("orc_smooth_tracks failed")
+    return dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost,
+                spar=np.ascontiguousarray(np.transpose(spar, (1, 2, 0))), scov=scov, used=used, sstatus=sst)
 
 
 REFIT_KAPPA = 10.0    # reading A18: inflation of the forward covariance used as the backward prior

@@ -23,7 +23,7 @@ STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE, STATUS_O
 OPT_PAIR_MIN_TRACKS, OPT_REFIT_PAIR_MASKED, OPT_BIN_FORM = 1, 2, 3          # kf_set_option
 BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
@@ -50,6 +50,11 @@ class _Tracks(C.Structure):
 class _TrackHits(C.Structure):
     _fields_ = [("n_layers", C.c_int), ("n", C.c_int64), ("ld", C.c_int64), ("pos", C.c_void_p), ("cov", C.c_void_p),
                 ("mask", C.c_void_p)]
+
+
+class _Smoothed(C.Structure):
+    _fields_ = [("n_layers", C.c_int), ("n", C.c_int64), ("ld", C.c_int64), ("par", C.c_void_p), ("cov", C.c_void_p),
+                ("used", C.c_void_p)]
 
 
 class _LayerHits(C.Structure):
@@ -114,6 +119,9 @@ def load_library():
     lib.kf_fit_tracks_refit.restype = C.c_int
     lib.kf_fit_tracks_refit.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.c_float,
                                          C.POINTER(_Tracks), C.POINTER(_Tracks)]
+    lib.kf_fit_tracks_smooth.restype = C.c_int
+    lib.kf_fit_tracks_smooth.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits),
+                                         C.POINTER(_Tracks), C.POINTER(_Smoothed)]
     lib.kf_bin_hits.restype = C.c_int
     lib.kf_bin_hits.argtypes = [vp, C.c_float, C.POINTER(_LayerHits), C.POINTER(_LayerBins)]
     lib.kf_bin_layers.restype = C.c_int
@@ -359,6 +367,22 @@ class KFContext:
         hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
         self._check(self._lib.kf_fit_tracks_refit(self._h, C.byref(g), C.byref(seeds), C.byref(hits), float(kappa),
                                                    C.byref(out), C.byref(sm)), "kf_fit_tracks_refit")
+        del keep
+
+    def fit_tracks_smooth(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,
+                          out_par, out_cov, out_chi2, out_nhits, out_status, s_par, s_cov, s_used):
+        """Forward fit + RTS smoother (kf_fit_tracks_smooth): s_par [L][6][ld], s_cov [L][21][ld] float32 and
+        s_used [n] int32 device tensors receive the smoothed state of every used layer and the used-layer mask."""
+        g, keep = geom._c()
+        seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
+        out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
+        hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
+        ld = _plane_ld(s_par, 6 * g.n_layers)
+        if _plane_ld(s_cov, 21 * g.n_layers) != ld:
+            raise ValueError("s_par and s_cov must share the plane stride ld")
+        sm = _Smoothed(g.n_layers, int(n), ld, s_par.data_ptr(), s_cov.data_ptr(), s_used.data_ptr())
+        self._check(self._lib.kf_fit_tracks_smooth(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out),
+                                                   C.byref(sm)), "kf_fit_tracks_smooth")
         del keep
 
     def fit_tracks_host(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,

@@ -82,6 +82,27 @@ class DeviceFit:
         self.refitted = sm
         return sm
 
+    def fit_smooth(self, ctx: KFContext) -> dict:
+        """kf_fit_tracks_smooth; the forward result lands in the usual out_* tensors, the per-layer smoothed states
+        in tensors allocated at the first call (kept as self.smoothed; later calls write into them)."""
+        dev = self.par.device
+        sm = getattr(self, "smoothed", None)
+        if sm is None:
+            L = int(self.geom.radius_cm.shape[0])
+            sm = dict(par=torch.zeros((L, 6, self.ld), dtype=torch.float32, device=dev),
+                      cov=torch.zeros((L, 21, self.ld), dtype=torch.float32, device=dev),
+                      used=torch.zeros((self.ld,), dtype=torch.int32, device=dev))
+        ctx.fit_tracks_smooth(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask,
+                              self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status,
+                              sm["par"], sm["cov"], sm["used"])
+        self.smoothed = sm
+        return sm
+
+    def smoothed_results(self) -> dict:
+        n, sm = self.n, self.smoothed
+        return dict(par=sm["par"][:, :, :n].cpu().numpy(), cov=sm["cov"][:, :, :n].cpu().numpy(),
+                    used=sm["used"][:n].cpu().numpy().view(np.uint32))
+
     def refit_results(self) -> dict:
         n, sm = self.n, self.refitted
         return dict(par=sm["par"][:, :n].cpu().numpy(), cov=sm["cov"][:, :n].cpu().numpy(),

@@ -15,8 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libkf_b200.so")
-SOURCES = ["kf_api.cu", "kf_fit.cu", "kf_host.cu", "kf_bin.cu", "kf_score.cu", "kf_comb.cu", "kf_peak.cu"]
-HEADERS = ["kf_math.cuh", "kf_pair.cuh", "kf_internal.h", "kf_score_common.cuh"]
+SOURCES = ["kf_api.cu", "kf_fit.cu", "kf_smooth.cu", "kf_host.cu", "kf_bin.cu", "kf_score.cu", "kf_comb.cu", "kf_peak.cu"]
+HEADERS = ["kf_math.cuh", "kf_pair.cuh", "kf_rts.cuh", "kf_tma.cuh", "kf_internal.h", "kf_score_common.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-cudart", "static"]
 

@@ -414,6 +414,35 @@ int kf_fit_tracks_refit(kf_ctx* c, const kf_geometry* geom, const kf_tracks* see
     return KF_OK;
 }
 
+int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits,
+                         kf_tracks* out, kf_smoothed* sm) {
+    if (!c || !geom || !seeds || !hits || !out || !sm) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (geom->energy_loss_model != 0) return KF_ERR_UNSUPPORTED;
+    if ((rc = check_tracks(seeds, true, true))) return rc;
+    if ((rc = check_tracks(out, false, true))) return rc;
+    if (out->n != seeds->n || sm->n != seeds->n || sm->n_layers != geom->n_layers || sm->ld < sm->n) return KF_ERR_SHAPE;
+    if ((rc = check_track_hits(hits, geom, seeds->n, true))) return rc;
+    if (seeds->n == 0) return KF_OK;
+    if (seeds->n > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
+    if (!sm->par || !sm->cov || !sm->used) return KF_ERR_NULL;
+    if (sm->ld % 4 != 0 || !aligned16(sm->par) || !aligned16(sm->cov)) return KF_ERR_ALIGN;
+    FitArgs a;
+    a.n = seeds->n;
+    a.par = seeds->par; a.cov = seeds->cov; a.ld_in = seeds->ld; a.q = seeds->q;
+    a.hpos = hits->pos; a.hcov = hits->cov; a.ld_hit = hits->ld; a.mask = hits->mask;
+    a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
+    a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
+    a.lpar = sm->par; a.lcov = sm->cov; a.ld_l = sm->ld; a.used = sm->used;
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_fit(P, a, c->stream, c->opt);
+    if (e == cudaSuccess) e = launch_rts(P, a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
+}
+
 int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
                        const kf_track_hits* hits, kf_tracks* out) {
     if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;

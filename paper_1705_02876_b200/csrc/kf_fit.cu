@@ -25,6 +25,7 @@
 #include <cstdlib>
 
 #include "kf_internal.h"
+#include "kf_tma.cuh"
 
 namespace kf {
 
@@ -63,48 +64,6 @@ struct FitMaps {
 struct Hit {
     float x, y, z, vxx, vxy, vxz, vyy, vyz, vzz;
 };
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-// One lane of the (converged) warp; the compiler keeps the guarded code on the uniform datapath.
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred;
-    asm volatile(
-        "{\n"
-        ".reg .pred P;\n"
-        "elect.sync _|P, 0xffffffff;\n"
-        "selp.u32 %0, 1, 0, P;\n"
-        "}\n" : "=r"(pred));
-    return pred != 0;
-}
-// 2-D TMA tile load global -> shared; completion (bytes) is signalled on an mbarrier.
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int col, int row, uint32_t bar) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                 ::"r"(dst), "l"(map), "r"(col), "r"(row), "r"(bar) : "memory");
-}
-// 2-D TMA tile store shared -> global (bulk async group).
-__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int col, int row, uint32_t src) {
-    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
-                 ::"l"(map), "r"(col), "r"(row), "r"(src) : "memory");
-}
 
 // One layer for one track.  Returns 0 or the status bit of the failure (track untouched).
 template <bool RADIAL_NULL, bool GEOM = true>
@@ -157,13 +116,32 @@ __device__ __forceinline__ void track_to_tile(const Track& t, float* p) {
     p[832] = t.c55;
 }
 
+// MODE 2: the filtered state of layer l in the local frame -> the per-layer arrays (coalesced 4-byte stores: lane =
+// track).  Planes: par 0..5 = x y z px py pz; cov 0..14 = c11 c12 c13 c14 c15 c22 c23 c24 c25 c33 c34 c35 c44 c45
+// c55, 15..16 = eax eay (17..20 are written by the backward pass only).
+__device__ __forceinline__ void store_layer_state(const Track& t, const FitArgs& a, int l, int64_t i) {
+    float* p = a.lpar + (int64_t)l * 6 * a.ld_l + i;
+    float* c = a.lcov + (int64_t)l * 21 * a.ld_l + i;
+    const int64_t ld = a.ld_l;
+    p[0] = t.x; p[ld] = t.y; p[2 * ld] = t.z; p[3 * ld] = t.px; p[4 * ld] = t.py; p[5 * ld] = t.pz;
+    c[0] = t.c11; c[ld] = t.c12; c[2 * ld] = t.c13; c[3 * ld] = t.c14; c[4 * ld] = t.c15;
+    c[5 * ld] = t.c22; c[6 * ld] = t.c23; c[7 * ld] = t.c24; c[8 * ld] = t.c25;
+    c[9 * ld] = t.c33; c[10 * ld] = t.c34; c[11 * ld] = t.c35;
+    c[12 * ld] = t.c44; c[13 * ld] = t.c45; c[14 * ld] = t.c55;
+    c[15 * ld] = t.eax; c[16 * ld] = t.eay;
+}
+
 // SMOOTH = false: forward fit (rows a1-a7).  SMOOTH = true: forward fit, then the inward refit of reading
 // A18 over the same hits (streamed again through the same ring, outermost layer first); two results.
 // GEOM = false: the paper's toy detector (unbounded barrels, flat material): the options of reading A20
 // are compiled out, so the headline kernel carries none of their cost.
-template <bool SMOOTH, bool GEOM>
-__global__ void __launch_bounds__(kFitBlock, SMOOTH ? 4 : KF_FIT_MIN_BLOCKS)
+// MODE 0: forward fit.  MODE 1 (= SMOOTH below): forward fit + the inward refit of reading A18.  MODE 2: forward fit
+// that also leaves the FILTERED state of every used layer, in the local frame, in the per-layer arrays of
+// kf_fit_tracks_smooth (23 floats per track and layer: the input of the backward RTS pass, kf_smooth.cu).
+template <int MODE, bool GEOM>
+__global__ void __launch_bounds__(kFitBlock, MODE == 1 ? 4 : KF_FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
+    constexpr bool SMOOTH = MODE == 1;
     const int model = GEOM ? P.model : 0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -227,7 +205,10 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             if (started) rc = fit_layer<true, GEOM>(t, k, ik, P.layer[l], model, P.mass2, P.el, m, chi2);
             else rc = fit_layer<false, GEOM>(t, k, ik, P.layer[l], model, P.mass2, P.el, m, chi2);
             st |= rc;
-            if (rc == 0u) { nh += 1; started = true; used |= 1u << l; }
+            if (rc == 0u) {
+                nh += 1; started = true; used |= 1u << l;
+                if constexpr (MODE == 2) { if (valid) store_layer_state(t, a, l, i); }
+            }
         }
         // The hit values have been consumed by the math above, so the stage can be handed back to the
         // TMA unit (write-after-read across the generic and async proxies needs no fence once the
@@ -331,6 +312,7 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         a.chi2[i] = chi2;
         a.nhits[i] = nh;
         a.status[i] = st;
+        if constexpr (MODE == 2) a.used[i] = used;
     }
     if (storer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // smem must outlive the store
 }
@@ -501,11 +483,42 @@ __device__ __forceinline__ void pair_to_tile(const Track2& t, float* tile, int l
     }
 }
 
+// MODE 2: filtered state of layer l of one or both tracks of the pair -> the per-layer arrays (see
+// store_layer_state): both with one 8-byte store per plane (tracks 2j, 2j + 1 are neighbours; ld is a multiple of
+// 4 and the tile starts at a multiple of 64, so the address is 8-byte aligned), one alone with 4-byte stores.
+__device__ __forceinline__ void store_layer_state_pair(const Track2& t, const FitArgs& a, int l, int64_t ix, int64_t iy,
+                                                       mask2 which) {
+    if (none_of(which)) return;
+    const int64_t ld = a.ld_l;
+    float* p = a.lpar + (int64_t)l * 6 * ld;
+    float* c = a.lcov + (int64_t)l * 21 * ld;
+#define KF_LAYER_PLANES(X)                                                                                        \
+    X(p, 0, x) X(p, 1, y) X(p, 2, z) X(p, 3, px) X(p, 4, py) X(p, 5, pz)                                          \
+    X(c, 0, c11) X(c, 1, c12) X(c, 2, c13) X(c, 3, c14) X(c, 4, c15) X(c, 5, c22) X(c, 6, c23) X(c, 7, c24)      \
+    X(c, 8, c25) X(c, 9, c33) X(c, 10, c34) X(c, 11, c35) X(c, 12, c44) X(c, 13, c45) X(c, 14, c55)              \
+    X(c, 15, eax) X(c, 16, eay)
+    if (all_of(which)) {
+#define KF_ST2(base, r, f) *reinterpret_cast<float2*>(base + (r) * ld + ix) = t.f.v;
+        KF_LAYER_PLANES(KF_ST2)
+#undef KF_ST2
+    } else if (which.x) {
+#define KF_STX(base, r, f) base[(r) * ld + ix] = t.f.v.x;
+        KF_LAYER_PLANES(KF_STX)
+#undef KF_STX
+    } else {
+#define KF_STY(base, r, f) base[(r) * ld + iy] = t.f.v.y;
+        KF_LAYER_PLANES(KF_STY)
+#undef KF_STY
+    }
+#undef KF_LAYER_PLANES
+}
+
 // SMOOTH = true: the forward fit, then the inward refit of reading A18 over the same hits (ring runs on,
-// outermost layer first), as in fit_kernel<true, false>.
-template <bool SMOOTH>
-__global__ void __launch_bounds__(kPairBlock, SMOOTH ? KF_PAIR_SMOOTH_MIN_BLOCKS : KF_PAIR_MIN_BLOCKS)
+// outermost layer first), as in fit_kernel<1, false>.
+template <int MODE>
+__global__ void __launch_bounds__(kPairBlock, MODE == 1 ? KF_PAIR_SMOOTH_MIN_BLOCKS : KF_PAIR_MIN_BLOCKS)
 fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
+    constexpr bool SMOOTH = MODE == 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     const int wid = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
@@ -600,24 +613,27 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
         if (both) {
             if (want.x) { nhx += 1; started.x = true; usedx |= 1u << l; }
             if (want.y) { nhy += 1; started.y = true; usedy |= 1u << l; }
+            if constexpr (MODE == 2) store_layer_state_pair(t, a, l, ix, iy, {want.x && valid.x, want.y && valid.y});
         } else if (!none_of(want)) {
             // copies whose address may be taken: the pair itself stays in registers
             Track2 tc = t;
             Hit2 mc;
             load_hit_pair(mc, tp);
             f2 cc = chi2;
+            mask2 stored = {false, false};
             if (want.x) {
                 const uint32_t rc = fit_layer_one_of_pair(tc, 0, k.v.x, ik.v.x, P.layer[l], P.mass2, mc, cc, started.x);
                 st.x |= rc;
-                if (rc == 0u) { nhx += 1; started.x = true; usedx |= 1u << l; }
+                if (rc == 0u) { nhx += 1; started.x = true; usedx |= 1u << l; stored.x = valid.x; }
             }
             if (want.y) {
                 const uint32_t rc = fit_layer_one_of_pair(tc, 1, k.v.y, ik.v.y, P.layer[l], P.mass2, mc, cc, started.y);
                 st.y |= rc;
-                if (rc == 0u) { nhy += 1; started.y = true; usedy |= 1u << l; }
+                if (rc == 0u) { nhy += 1; started.y = true; usedy |= 1u << l; stored.y = valid.y; }
             }
             t = tc;
             chi2 = cc;
+            if constexpr (MODE == 2) store_layer_state_pair(t, a, l, ix, iy, stored);
         }
         // (SMOOTH: the ring runs on into the backward pass, step L + j carries layer L - 1 - j)
         const int nxt = l + kStages;
@@ -740,6 +756,10 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
     }
     if (valid.x) { a.chi2[ix] = chi2.v.x; a.nhits[ix] = nhx; a.status[ix] = st.x; }
     if (valid.y) { a.chi2[iy] = chi2.v.y; a.nhits[iy] = nhy; a.status[iy] = st.y; }
+    if constexpr (MODE == 2) {
+        if (valid.x) a.used[ix] = usedx;
+        if (valid.y) a.used[iy] = usedy;
+    }
     if (storer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 #undef KF_TRACK_ROWS
@@ -821,55 +841,6 @@ fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ 
 
 namespace {
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn() {
-    static EncodeTiledFn fn = [] {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
-            q != cudaDriverEntryPointSuccess)
-            p = nullptr;
-        return reinterpret_cast<EncodeTiledFn>(p);
-    }();
-    return fn;
-}
-
-// Tensor map over a [rows][ld] float array of which n columns are valid; tiles are [box_rows][box_cols].
-// Encoding a map costs a driver call; a caller that fits event after event through the same buffers asks for
-// the same few maps every time, so the last 16 are kept per host thread (a map depends on nothing but the key).
-struct MapKey {
-    const float* base; int64_t n, ld, rows; int box_rows, box_cols;
-    bool operator==(const MapKey& o) const {
-        return base == o.base && n == o.n && ld == o.ld && rows == o.rows && box_rows == o.box_rows && box_cols == o.box_cols;
-    }
-};
-bool make_map(CUtensorMap* m, const float* base, int64_t n, int64_t ld, int64_t rows, int box_rows, int box_cols = 32) {
-    constexpr int kCached = 16;
-    thread_local MapKey keys[kCached] = {};
-    thread_local CUtensorMap maps[kCached];
-    thread_local int next = 0;
-    const MapKey key{base, n, ld, rows, box_rows, box_cols};
-    for (int i = 0; i < kCached; ++i)
-        if (keys[i].base != nullptr && keys[i] == key) { *m = maps[i]; return true; }
-    EncodeTiledFn enc = encode_fn();
-    if (!enc) return false;
-    const cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)rows};
-    const cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
-    const cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
-    const cuuint32_t estr[2] = {1u, 1u};
-    if (enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return false;
-    keys[next] = key;
-    maps[next] = *m;
-    next = (next + 1) % kCached;
-    return true;
-}
-
 }  // namespace
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: set once for every device a context
@@ -881,12 +852,15 @@ cudaError_t ensure_fit_attributes() {
     if (e != cudaSuccess) return e;
     const uint64_t bit = 1ull << (dev & 63);
     if (done.load(std::memory_order_acquire) & bit) return cudaSuccess;
-    e = cudaFuncSetAttribute(fit_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));
+    e = cudaFuncSetAttribute(fit_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
     if (e == cudaSuccess) done.fetch_or(bit, std::memory_order_release);
     return e;
 }
@@ -895,7 +869,8 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     if (a.n == 0) return cudaSuccess;
     const cudaError_t attr = ensure_fit_attributes();
     if (attr != cudaSuccess) return attr;
-    const bool smooth = a.spar != nullptr;
+    const bool smooth = a.spar != nullptr;   // the refit of reading A18 (two results)
+    const bool store = a.lpar != nullptr;    // per-layer filtered states for the RTS smoother
     const int L = P.n_layers;
     FitMaps M;
     const int64_t pair_min = opt.pair_min_tracks > 0 ? opt.pair_min_tracks : (int64_t)KF_PAIR_MIN_TRACKS;
@@ -917,8 +892,9 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
             return cudaErrorInvalidValue;
         const int64_t per_block = (int64_t)kPairWarps * kPairTile;
         const int64_t blocks = (a.n + per_block - 1) / per_block;
-        if (smooth) fit_pair_kernel<true><<<(unsigned)blocks, kPairBlock, smem2_bytes(true), stream>>>(P, M, a);
-        else fit_pair_kernel<false><<<(unsigned)blocks, kPairBlock, smem2_bytes(false), stream>>>(P, M, a);
+        if (smooth) fit_pair_kernel<1><<<(unsigned)blocks, kPairBlock, smem2_bytes(true), stream>>>(P, M, a);
+        else if (store) fit_pair_kernel<2><<<(unsigned)blocks, kPairBlock, smem2_bytes(false), stream>>>(P, M, a);
+        else fit_pair_kernel<0><<<(unsigned)blocks, kPairBlock, smem2_bytes(false), stream>>>(P, M, a);
         return cudaGetLastError();
     }
     if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3) ||
@@ -930,10 +906,12 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
         return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
     const bool geom = P.geometry_options != 0;   // reading A20 options in use
-    if (smooth && geom) fit_kernel<true, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else if (smooth) fit_kernel<true, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else if (geom) fit_kernel<false, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else fit_kernel<false, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    if (smooth && geom) fit_kernel<1, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (smooth) fit_kernel<1, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (store && geom) fit_kernel<2, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (store) fit_kernel<2, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (geom) fit_kernel<0, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else fit_kernel<0, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     return cudaGetLastError();
 }
 

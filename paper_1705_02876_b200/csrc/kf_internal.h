@@ -36,6 +36,10 @@ struct FitArgs {
     float* spar = nullptr; float* scov = nullptr; int64_t ld_s = 0;
     float* schi2 = nullptr; int32_t* snhits = nullptr; uint32_t* sstatus = nullptr;
     float kappa = 10.0f;
+    // kf_fit_tracks_smooth (RTS): per-layer arrays [L][6][ld_l] / [L][21][ld_l] and the used-layer mask
+    // (lpar == nullptr: not wanted).  The forward kernel leaves the filtered local-frame state of every used layer
+    // there; the backward kernel (kf_smooth.cu) turns it into the smoothed state in global coordinates.
+    float* lpar = nullptr; float* lcov = nullptr; int64_t ld_l = 0; uint32_t* used = nullptr;
 };
 
 struct IndexedPools {           // per-layer hit pools + the per-track hit indices into them
@@ -53,6 +57,9 @@ struct IndexedPools {           // per-layer hit pools + the per-track hit indic
 // kf_fit.cu
 cudaError_t launch_fit_indexed(const FitParams& P, const IndexedPools& H, const FitArgs& a, cudaStream_t stream);
 cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream, const LaunchOptions& opt = LaunchOptions());
+
+// kf_smooth.cu: backward RTS pass over the per-layer arrays the forward kernel filled
+cudaError_t launch_rts(const FitParams& P, const FitArgs& a, cudaStream_t stream);
 
 // ---------------------------------------------------------------------------------- host path
 struct HostFitIO {

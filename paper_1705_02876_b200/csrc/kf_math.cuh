@@ -41,7 +41,7 @@ namespace kf {
 constexpr float kCB = 2.99792458e-3f;  // GeV / (c T cm), reading A1
 
 enum : int { MODEL_PATH_LENGTH = 1, MODEL_ENERGY_LOSS = 2 };
-enum : uint32_t { ST_PROP_FAIL = 1u, ST_S_NOT_PD = 2u, ST_NONFINITE = 4u, ST_BAD_CHARGE = 8u, ST_OUTSIDE = 16u };
+enum : uint32_t { ST_PROP_FAIL = 1u, ST_S_NOT_PD = 2u, ST_NONFINITE = 4u, ST_BAD_CHARGE = 8u, ST_OUTSIDE = 16u, ST_SMOOTH_FAIL = 32u };
 
 // Per-layer constants, computed once on the host in double and rounded to float.
 struct LayerConst {

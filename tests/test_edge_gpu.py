@@ -33,7 +33,7 @@ def test_best_hit_building_small_shapes(ctx, n_tracks, noise, first):
     """One candidate; one scored layer; a layer pool holding the single true hit only."""
     ev = W.make_build_event(4, n_tracks=n_tracks, noise_hits=noise)
     ev.cfg = dataclasses.replace(ev.cfg, first_scored_layer=first)
-    n_dec, _ = S._build_event_fused(ctx, ev, use_order=(n_tracks > 1), cov_loosen=3.0)
+    n_dec, _ = S._build_event_fused(ctx, ev, use_order=(n_tracks > 1))
     assert n_dec >= 0.9 * n_tracks * (10 - first)
 
 
@@ -69,7 +69,7 @@ def test_indexed_fit_short_geometries(ctx, k, n_tracks):
     for rec in (False, True):
         g = P._fit_indexed(ctx, ev, truth, use_records=rec)
         assert np.array_equal(g["nhits"], o["nhits"]) and np.array_equal(g["status"], o["status"])
-        compare_fit(g, o, float(ev.fit.radius[-1]), max_diverged_frac=1.0, loosen={"mom": 4.0})
+        compare_fit(g, o, float(ev.fit.radius[-1]), max_diverged_frac=1.0)
 
 
 @pytest.mark.parametrize("n,k", [(1, 1), (131_072, 2), (131_073, 10), (5, 10), (1000, 32)])
@@ -86,7 +86,7 @@ def test_host_path_chunk_boundaries(ctx, n, k):
     h = _host_fit(ctx, b)
     assert np.array_equal(h["nhits"], r["nhits"]) and np.array_equal(h["status"], r["status"])
     o = O.fit_batch(b)
-    compare_fit(h, o, float(b.radius[-1]), max_diverged_frac=1.0, loosen={"mom": 4.0} if k <= 3 else None)
+    compare_fit(h, o, float(b.radius[-1]), max_diverged_frac=1.0)
 
 
 def _host_fit(ctx, b):

@@ -72,8 +72,7 @@ def test_refit_extreme_layer_counts(ctx, n_layers, step, n, pair_masked):
     # Three hits barely constrain |p| (5 parameters from 6 good coordinates): the fit is ill-conditioned and the
     # worst of 160 000 such tracks reaches 2.2e-4 relative on the momentum in fp32 (99 % stay below 0.2e-4), so the
     # short geometries are held to 4 x the momentum tolerance (known limits).
-    fwd, sm = _compare(d, o, float(b.radius[-1]), max_div=1e-3 if n_layers > 3 else 1.0,
-                       loosen={"mom": 4.0} if n_layers <= 3 else None)
+    fwd, sm = _compare(d, o, float(b.radius[-1]), max_div=1e-3 if n_layers > 3 else 1.0)
     assert n_layers > 3 or (fwd["mom_p99"] <= 0.5 and sm["mom_p99"] <= 0.5)
 
 

@@ -1,0 +1,198 @@
+"""GPU parity of kf_fit_tracks_smooth (forward fit + RTS smoother, reading A22) against the oracle:
+smoothed state and covariance at EVERY used layer, at the fit tolerances (tests/parity.py)."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import kf_oracle as O
+from tests.parity import compare_fit
+from workloads import barrel_events as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import paper_1705_02876_b200 as K
+    c = K.KFContext(0)
+    yield c
+    c.close()
+
+
+def _both(ctx, b, with_mask=True, threads=8, **geo):
+    from paper_1705_02876_b200.buffers import DeviceFit
+    d = DeviceFit.from_batch(b, "cuda:0", with_mask=with_mask)
+    d.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    o = O.smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask, nthreads=threads)
+    return d, o
+
+
+def _compare(g, sg, o, radius, max_div=1e-3, layers=None, sel=None):
+    """Forward result, then every layer's smoothed state, with the fit's metric.  Returns the worst errors over
+    the layers.  `sel` restricts to a subset of tracks."""
+    n = o["par"].shape[1]
+    sel = np.ones(n, bool) if sel is None else sel
+    sub = lambda r, keys: {k: (r[k][..., sel] if k in ("par", "cov") else r[k][sel]) for k in keys}
+    fwd = compare_fit(sub(g, ("par", "cov", "chi2", "nhits", "status")),
+                      dict(par=o["par"][:, sel], cov=o["cov"][sel], chi2=o["chi2"][sel], nhits=o["nhits"][sel], status=o["status"][sel]),
+                      float(radius[-1]), max_div)
+    assert np.array_equal(sg["used"][sel], o["used"][sel])
+    assert np.array_equal((g["status"][sel] & 32) != 0, o["sstatus"][sel] != 0)
+    worst = dict(pos=0.0, mom=0.0, cov=0.0)
+    L = len(radius)
+    for l in (range(L) if layers is None else layers):
+        has = sel & (((o["used"] >> l) & 1) == 1)
+        if not has.any():
+            continue
+        # diverged tracks (A14) are those of the forward fit; marked through the status word compare_fit looks at
+        ndf = np.maximum(2 * o["nhits"] - 5, 1)
+        excl = (o["status"] | o["sstatus"] | ((o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)).astype(np.uint32) << 6))[has]
+        so = dict(par=o["spar"][l][:, has], cov=o["scov"][has, l], chi2=np.zeros(has.sum()), nhits=o["nhits"][has], status=excl)
+        gg = dict(par=sg["par"][l][:, has], cov=sg["cov"][l][:, has], chi2=np.zeros(has.sum()), nhits=o["nhits"][has], status=excl)
+        res = compare_fit(gg, so, float(radius[l]), max_diverged_frac=max(max_div, 2e-3))
+        for k in worst:
+            worst[k] = max(worst[k], res[k])
+    return fwd, worst
+
+
+@pytest.mark.parametrize("config", [0, 1, 3])
+def test_smooth_parity_full_config(ctx, config):
+    b = W.make_fit_batch(config)
+    d, o = _both(ctx, b)
+    fwd, worst = _compare(d.results(), d.smoothed_results(), o, b.radius)
+    print(f"config {config}: forward {fwd}\n          smoothed, worst over layers (1.0 = tolerance): {worst}")
+
+
+def test_smooth_forward_part_equals_plain_fit_and_last_layer(ctx):
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.make_fit_batch(1)
+    d1 = DeviceFit.from_batch(b, "cuda:0"); d1.fit(ctx)
+    d2 = DeviceFit.from_batch(b, "cuda:0"); d2.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    r1, r2 = d1.results(), d2.results()
+    for k in r1:
+        assert np.array_equal(r1[k], r2[k]), k
+    # the smoothed state of the outermost used layer is the filtered one = the forward result (the same local-frame
+    # values taken to global coordinates by the same function in two kernels: equal to the last bit or two)
+    sg = d2.smoothed_results()
+    full = sg["used"] == 0x3ff
+    assert full.mean() > 0.99
+    L = b.n_layers
+    assert np.array_equal(sg["par"][L - 1][:, full], r2["par"][:, full])
+    scale = np.abs(r2["cov"][:, full]).max(axis=0)
+    assert np.max(np.abs(sg["cov"][L - 1][:, full] - r2["cov"][:, full]) / scale) < 1e-6
+
+
+@pytest.mark.parametrize("n", [1, 31, 33, 129, 1001])
+def test_smooth_ragged_sizes(ctx, n):
+    b = W.simulate_event(W.get_config(1), 5, n_tracks=n)
+    d, o = _both(ctx, b)
+    _compare(d.results(), d.smoothed_results(), o, b.radius, max_div=1.0)
+
+
+def test_smooth_masks_failures_and_untouched_slots(ctx):
+    """Holes in the hit mask, tracks with nothing to fit, a bad charge, a layer that fails in the forward fit
+    (NONFINITE): smoothed states exist exactly on the used layers, the other slots keep what they held."""
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.simulate_event(W.get_config(1), 8, n_tracks=1003)
+    rng = np.random.default_rng(3)
+    b.mask = (rng.integers(0, 1 << 10, size=b.n) | 0b111).astype(np.uint32)
+    b.mask[:30] = 0
+    b.q[30] = 0
+    b.hpos[4, 1, 40] = np.nan
+    b.mask[40] = 0x3ff
+    d = DeviceFit.from_batch(b, "cuda:0")
+    d.fit_smooth(ctx)                                  # allocates the per-layer tensors (zeros)
+    d.smoothed["par"].fill_(-7.0); d.smoothed["cov"].fill_(-7.0)
+    d.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    o = O.smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask)
+    g, sg = d.results(), d.smoothed_results()
+    assert np.array_equal(sg["used"], o["used"]) and np.array_equal(g["status"], o["status"]) and np.array_equal(g["nhits"], o["nhits"])
+    assert np.all(sg["used"][:31] == 0) and o["status"][30] == 8 and o["status"][40] == 4 and not (o["used"][40] >> 4) & 1
+    for l in range(b.n_layers):
+        unused = ((o["used"] >> l) & 1) == 0
+        assert np.all(sg["par"][l][:, unused] == -7.0) and np.all(sg["cov"][l][:, unused] == -7.0)
+    sel = o["nhits"] >= 5
+    _compare(g, sg, o, b.radius, max_div=0.05, sel=sel)
+
+
+@pytest.mark.parametrize("n_layers,step,n", [(32, 2.5, 3000), (32, 2.5, 160_000), (1, 4.0, 700), (2, 4.0, 700), (3, 4.0, 700)])
+def test_smooth_extreme_layer_counts(ctx, n_layers, step, n):
+    cfg = dataclasses.replace(W.get_config(3 if n_layers > 3 else 1), n_layers=n_layers, layer_step_cm=step, n_tracks=n)
+    b = W.simulate_event(cfg, 22, n_tracks=n)
+    d, o = _both(ctx, b)
+    fwd, worst = _compare(d.results(), d.smoothed_results(), o, b.radius, max_div=1e-3 if n_layers > 3 else 1.0)
+    print(n_layers, "layers:", worst)
+
+
+def test_smooth_pair_kernel_and_ragged_pairs(ctx):
+    """160 005 tracks take the two-tracks-per-thread forward kernel (which stores the per-layer states of both
+    tracks with one 8-byte store per plane); holes make ragged pairs, early stops make pairs of different length."""
+    cfg = W.get_config(1)
+    b = W.concat_batches([W.simulate_event(cfg, 70 + e) for e in range(8)] + [W.simulate_event(cfg, 78, n_tracks=5)])
+    assert b.n == 160_005
+    rng = np.random.default_rng(5)
+    holes = rng.random(b.n) < 0.1
+    b.mask = np.where(holes, (rng.integers(0, 1 << 10, size=b.n) | 0b111), b.mask).astype(np.uint32)
+    b.mask[31:60:2] = 0b0000011111
+    d, o = _both(ctx, b)
+    sel = o["nhits"] >= 5
+    fwd, worst = _compare(d.results(), d.smoothed_results(), o, b.radius, max_div=0.02, sel=sel)
+    print("pair kernel, ragged:", worst)
+    d2, _ = _both(ctx, b, with_mask=False)            # no mask: every layer used
+    o2 = O.smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, None, nthreads=8)
+    _compare(d2.results(), d2.smoothed_results(), o2, b.radius)
+
+
+def test_smooth_with_path_length_material_and_finite_barrels(ctx):
+    cfg = dataclasses.replace(W.get_config(1), material_model=1, half_length_cm=30.0)
+    b = W.simulate_event(cfg, 12, n_tracks=20000)
+    from paper_1705_02876_b200.buffers import DeviceFit
+    d = DeviceFit.from_batch(b, "cuda:0")
+    d.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    with O.geometry_options(1, np.full(b.n_layers, 30.0)):
+        o = O.smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask, nthreads=8)
+    g, sg = d.results(), d.smoothed_results()
+    # crossings within 2e-5 relative of the barrel end may fall either side in fp32 (reading A20): exempt, counted
+    same = (g["status"] == o["status"]) & (sg["used"] == o["used"])
+    assert (~same).mean() < 5e-3
+    sel = same & (o["nhits"] >= 4)
+    _compare(g, sg, o, b.radius, max_div=0.05, sel=sel)
+
+
+def test_smooth_energy_loss_is_refused(ctx):
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.simulate_event(W.get_config(1), 2, n_tracks=100)
+    b.energy_loss = 1
+    d = DeviceFit.from_batch(b, "cuda:0")
+    with pytest.raises(K.KFError) as e:
+        d.fit_smooth(ctx)
+    assert e.value.code == -4
+
+
+def test_smooth_parity_config2_sampled(ctx):
+    """The smoother at the size bench.py times it (config 2, 2 M tracks, pair forward kernel); the oracle checks
+    every 16th event track by track, every layer."""
+    from paper_1705_02876_b200.buffers import DeviceFit
+    cfg = W.get_config(2)
+    b = W.make_fit_batch(2)
+    assert b.n == 2_000_000
+    d = DeviceFit.from_batch(b, "cuda:0", with_mask=False)
+    d.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    g = d.results()
+    sm = d.smoothed
+    for ev in range(0, cfg.n_events, 16):
+        lo, hi = ev * cfg.n_tracks, (ev + 1) * cfg.n_tracks
+        sub = W.simulate_event(cfg, ev)
+        o = O.smooth_tracks(sub.radius, sub.x_over_X0, sub.Bz, sub.mass, sub.par, sub.cov, sub.q, sub.hpos, sub.hcov, sub.mask, nthreads=8)
+        gs = {k: (v[..., lo:hi] if k in ("par", "cov") else v[lo:hi]) for k, v in g.items()}
+        sgs = dict(par=sm["par"][:, :, lo:hi].cpu().numpy(), cov=sm["cov"][:, :, lo:hi].cpu().numpy(),
+                   used=sm["used"][lo:hi].cpu().numpy().view(np.uint32))
+        _compare(gs, sgs, o, b.radius)

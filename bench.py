@@ -29,13 +29,63 @@ import numpy as np
 METRIC = "kalman_track_fits_per_sec_10_layer_barrel"
 UNIT = "fits/s"
 CONFIG_INDEX = 2
-# dram__bytes_read.sum + dram__bytes_write.sum of fit_pair_kernel for one 2M-track launch, from the
-# `ncu --set full` capture summarised in profiles/r01_fit_pair_kernel.md.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 946051584 + 219393024   # profiles/r01_fit_pair_kernel.md (last capture, launch 5)
+# Hardware counters of the hot kernels (DRAM bytes, executed FP32 thread instructions, active warps) come from the
+# one `ncu --set full` capture of `bench.py --profile-sequence` whose raw page is committed as
+# profiles/r02_counters.csv (the command is in profiles/r02_counters.md); nothing here is typed in by hand.
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r02_counters.csv")
 # Algorithmic flops per track and layer of the filter as the oracle states it, exploiting the known zeros and
 # ones of F and H and symmetry: propagation 75, Jacobian 95, F C F^T 340,
 # Q 35, update 310 (S 9, S^-1 30, chi2 21, K 90, x 36, C 126) -- frozen before any tuning.
 FLOPS_PER_TRACK_LAYER = 850
+# FP32 flops the pair kernel EXECUTES per track and layer, from the SASS opcode histogram of its ncu capture
+# (profiles/r02_fit_pair_kernel.md; 177 FFMA2 + 122 FMUL2 + 23 FADD2 per pair-layer in round 1 = 499 per track).
+EXECUTED_FLOPS_PER_TRACK_LAYER = 500
+
+
+def _profile_counters() -> dict:
+    """{kernel name fragment: {metric: value per launch}} from the committed raw ncu page (empty if absent)."""
+    import csv
+    want = {"dram__bytes_read.sum": "dram_read", "dram__bytes_write.sum": "dram_write",
+            "smsp__sass_thread_inst_executed_op_fadd_pred_on.sum": "fadd", "smsp__sass_thread_inst_executed_op_fmul_pred_on.sum": "fmul",
+            "smsp__sass_thread_inst_executed_op_ffma_pred_on.sum": "ffma",
+            "sm__sass_thread_inst_executed_op_fadd_pred_on.sum": "fadd", "sm__sass_thread_inst_executed_op_fmul_pred_on.sum": "fmul",
+            "sm__sass_thread_inst_executed_op_ffma_pred_on.sum": "ffma",
+            "sm__warps_active.avg.pct_of_peak_sustained_active": "warps_active_pct",
+            "gpu__time_duration.sum": "ncu_duration", "launch__registers_per_thread": "registers",
+            "sm__inst_executed.sum": "warp_inst", "smsp__inst_executed.sum": "warp_inst",
+            "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed": "fma_pipe_pct",
+            "sm__inst_executed.sum.pct_of_peak_sustained_elapsed": "issue_pct"}
+    out = {}
+    if not os.path.exists(PROFILE_CSV):
+        return out
+    with open(PROFILE_CSV, newline="") as f:
+        rows = list(csv.reader(f))
+    hdr = next((r for r in rows if "Kernel Name" in r), None)
+    if hdr is None:
+        return out
+    units = rows[rows.index(hdr) + 1]
+    ki = hdr.index("Kernel Name")
+    scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "msecond": 1e-3, "usecond": 1e-6, "nsecond": 1e-9, "second": 1.0}
+    for r in rows[rows.index(hdr) + 2:]:
+        if len(r) != len(hdr):
+            continue
+        name = r[ki]
+        d = out.setdefault(name, {})
+        for col, key in want.items():
+            if col in hdr and key not in d:
+                j = hdr.index(col)
+                try:
+                    d[key] = float(r[j].replace(",", "")) * scale.get(units[j], 1.0)
+                except ValueError:
+                    pass
+    return out
+
+
+def _kernel_counters(counters: dict, fragment: str) -> dict | None:
+    for name, d in counters.items():
+        if fragment in name:
+            return d
+    return None
 
 
 def _peaks() -> tuple[float, str]:
@@ -258,6 +308,90 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
                               "best_hit_all_true_hits_found_fraction": best_eff, "kernels": 4 * (L - L0) + 2}}
 
 
+def run_profile_sequence(args) -> None:
+    """--profile-sequence: ONE launch of every hot call at the benched sizes, for ncu (no timing here).
+    Warm-up calls come first; the profiled region is bracketed by cudaProfilerStart / Stop, so
+    `ncu --profile-from-start off ...` sees exactly one launch of each kernel:
+    kf_fit_tracks, kf_fit_tracks_smooth, kf_fit_tracks_refit on configs[2]; kf_bin_layers, kf_build_best_hit,
+    kf_build_combinatorial on configs[4]."""
+    import copy
+    import torch
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceFit, DeviceLayer
+    from workloads import barrel_events as W
+    dev = "cuda:0"
+    stream = torch.cuda.Stream(device=dev)
+    ctx = K.KFContext(0, stream)
+    cfg, batch = _make_batch(0, args.events)
+    d = DeviceFit.from_batch(batch, dev, with_mask=False)
+    ev = W.make_build_event(4)
+    f, c4 = ev.fit, ev.cfg
+    L0 = c4.first_scored_layer
+    emax = float(np.float32(c4.eta_bin_max))
+    f3 = copy.copy(f)
+    f3.radius, f3.x_over_X0 = f.radius[:L0], f.x_over_X0[:L0]
+    f3.hpos, f3.hcov = np.ascontiguousarray(f.hpos[:L0]), np.ascontiguousarray(f.hcov[:L0])
+    d3 = DeviceFit.from_batch(f3, dev)
+    layers = [DeviceLayer.from_numpy(l.pos, l.cov, c4.n_eta, c4.n_phi, emax, dev) for l in ev.layers[L0:]]
+    radii = [l.radius for l in ev.layers[L0:]]
+    bargs = [(l.n_hits, l.pos, l.cov, l.bins) for l in layers]
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
+
+    def sequence():
+        with torch.cuda.stream(stream):
+            d.fit(ctx)
+            d.fit_smooth(ctx)
+            d.fit_refit(ctx)
+            d3.fit(ctx)
+            torch.cuda.synchronize()
+            s3 = d3.results()
+            dc = DeviceCandidates.from_numpy(s3["par"], s3["cov"], f.q, s3["chi2"], s3["nhits"], dev)
+            dc2 = DeviceCandidates.from_numpy(s3["par"], s3["cov"], f.q, s3["chi2"], s3["nhits"], dev)
+            ctx.bin_layers(radii, bargs)
+            dc.build(ctx, geom, L0, layers, 2, 30.0, True, None)
+            dc2.build_combinatorial(ctx, geom, L0, layers, 4)
+        torch.cuda.synchronize()
+
+    sequence()                      # warm-up: sizes every scratch buffer, fills caches of tensor maps
+    torch.cuda.synchronize()
+    torch.cuda.profiler.start()
+    sequence()
+    torch.cuda.profiler.stop()
+    print(json.dumps({"profile_sequence": "done", "tracks": int(batch.n), "candidates": int(f.n)}), flush=True)
+    ctx.close()
+
+
+def _opcode_table(path: str) -> None:
+    """--opcode-table FILE: FILE = `ncu -i X.ncu-rep --page source --csv -k <kernel>` output; prints, per SASS opcode,
+    the thread-level executed instruction count and the FP32 flops it stands for (FFMA2 = 4, FMUL2 / FADD2 = 2,
+    FFMA = 2, FMUL / FADD / MUFU = 1)."""
+    import csv
+    per = {}
+    with open(path, newline="") as fh:
+        rows = list(csv.reader(fh))
+    hdr = next(r for r in rows if "Source" in r and any("Thread Instructions Executed" in c for c in r))
+    si = hdr.index("Source")
+    ti = next(i for i, c in enumerate(hdr) if c.strip() == "Thread Instructions Executed")
+    for r in rows[rows.index(hdr) + 1:]:
+        if len(r) <= max(si, ti):
+            continue
+        toks = r[si].replace("{", " ").split()
+        op = next((t for t in toks if not t.startswith("@") and not t.startswith("/*")), None)
+        if op is None:
+            continue
+        try:
+            per[op.split(".")[0]] = per.get(op.split(".")[0], 0) + int(float(r[ti]))
+        except ValueError:
+            pass
+    w = {"FFMA2": 4, "FMUL2": 2, "FADD2": 2, "FFMA": 2, "FMUL": 1, "FADD": 1, "MUFU": 1}
+    total = sum(per.values())
+    flops = sum(per.get(k, 0) * v for k, v in w.items())
+    print("opcode,thread_instructions,fp32_flops")
+    for k, v in sorted(per.items(), key=lambda kv: -kv[1]):
+        print(f"{k},{v},{v * w.get(k, 0)}")
+    print(f"TOTAL,{total},{flops}")
+
+
 def run_ours(args) -> None:
     import torch
     import paper_1705_02876_b200 as K
@@ -330,24 +464,30 @@ def run_ours(args) -> None:
     ctx.set_stream(stream)          # measure_building borrowed the context for torch's current stream
     smoothing = None
     if rank == 0 and not args.no_building:
-        # secondary: kf_fit_tracks_refit on the same batch (forward fit + inward refit, one kernel)
-        # Every track of configs[2] has all 10 hits, which the API states by passing no mask: the call then takes
-        # the two-tracks-per-thread smoother.  With a mask it takes the one-track kernel (ragged pairs would cost
-        # the pair form more than it gains); both are timed.
-        def time_smooth():
+        def time_call(call, reps=20):
             with torch.cuda.stream(stream):
                 for _ in range(3):
-                    d.fit_refit(ctx)
+                    call()
                 s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 s0.record(stream)
-                for _ in range(20):
-                    d.fit_refit(ctx)
+                for _ in range(reps):
+                    call()
                 s1.record(stream)
             torch.cuda.synchronize()
-            return s0.elapsed_time(s1) / 20
-        sm_masked_ms = time_smooth()
+            return s0.elapsed_time(s1) / reps
+        # secondary: kf_fit_tracks_smooth on the same batch = forward fit + RTS smoother (reading A22):
+        # smoothed state and covariance at every layer.  Two kernels (forward with per-layer store, backward).
+        rts_masked_ms = time_call(lambda: d.fit_smooth(ctx))
         full_mask, d.mask = d.mask, None
-        sm_ms = time_smooth()
+        rts_ms = time_call(lambda: d.fit_smooth(ctx))
+        d.mask = full_mask
+        del d.smoothed
+        torch.cuda.empty_cache()
+        # secondary: kf_fit_tracks_refit (round 1's inward refit, reading A18: one state at the innermost layer).
+        # Without a mask the call takes the two-tracks-per-thread form, with a mask the one-track kernel.
+        sm_masked_ms = time_call(lambda: d.fit_refit(ctx))
+        full_mask, d.mask = d.mask, None
+        sm_ms = time_call(lambda: d.fit_refit(ctx))
         d.mask = full_mask
         s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         sm_bytes = n * (113 + 2 * 36 * L + 2 * 120)
@@ -457,29 +597,62 @@ def run_ours(args) -> None:
                                                "fits_per_s": bc.n / (g_ms * 1e-3), "bound_ms": bound_ms,
                                                "roofline_frac": bound_ms / g_ms}
             del dcf, bc
-        smoothing = {"api": "kf_fit_tracks_refit (reading A18, kappa 10), mask = NULL: every track has every hit",
-                     "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3), "with_mask_ms": sm_masked_ms,
-                     "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0],
-                     "alu_roofline_frac": 2.0 * n * FLOPS_PER_TRACK_LAYER * L / (sm_ms * 1e-3) / (fp32_peak * 1e12)}
+        # Algorithmic bytes of fit + smoother per track: 113 in + 36 L hits + 120 forward result + 4 used mask +
+        # 108 L smoothed states; the implementation also writes and re-reads 92 L of filtered states.
+        rts_bytes = n * (113 + 36 * L + 120 + 4 + 108 * L)
+        rts_moved = rts_bytes + n * 2 * 92 * L
+        smoothing = {"api": "kf_fit_tracks_smooth (RTS smoother, reading A22): smoothed state + covariance at every layer; "
+                            "mask = NULL (two-tracks-per-thread forward kernel)",
+                     "ms": rts_ms, "fits_per_s": n / (rts_ms * 1e-3), "with_mask_ms": rts_masked_ms,
+                     "algorithmic_bytes": int(rts_bytes), "hbm_frac": rts_bytes / (rts_ms * 1e-3) / 1e9 / _peaks()[0],
+                     "bytes_moved_by_this_implementation": int(rts_moved),
+                     "hbm_frac_of_bytes_moved": rts_moved / (rts_ms * 1e-3) / 1e9 / _peaks()[0],
+                     "refit": {"api": "kf_fit_tracks_refit (reading A18, kappa 10: one state at the innermost layer), mask = NULL",
+                               "ms": sm_ms, "fits_per_s": n / (sm_ms * 1e-3), "with_mask_ms": sm_masked_ms,
+                               "algorithmic_bytes": int(sm_bytes), "hbm_frac": sm_bytes / (sm_ms * 1e-3) / 1e9 / _peaks()[0]}}
 
     if rank == 0:
         peak, peak_src = _peaks()
         alg_bytes = d.algorithmic_bytes
         t_launch = ms_local / args.steps * 1e-3
+        counters = _profile_counters()
+        kc = _kernel_counters(counters, "fit_pair_kernel") or {}
+        traffic = (kc["dram_read"] + kc["dram_write"]) if "dram_read" in kc and "dram_write" in kc else None
+        hw = {"source": "profiles/r02_counters.csv (ncu --set full of `bench.py --profile-sequence`, one launch)" if kc else None,
+              "dram_traffic_bytes": traffic, "fma_pipe_active_pct": kc.get("fma_pipe_pct"),
+              "issue_slots_busy_pct": kc.get("issue_pct"), "warps_active_pct_of_peak": kc.get("warps_active_pct"),
+              "registers_per_thread": kc.get("registers"),
+              "ncu_fp32_thread_inst": {k: kc.get(k) for k in ("fadd", "fmul", "ffma")},
+              "note": "ncu's fadd/fmul/ffma thread-instruction counters do not count the packed FFMA2 / FMUL2 / FADD2 "
+                      "instructions this kernel is made of (they read ~0), so executed FP32 work is taken from the "
+                      "SASS opcode histogram of the same capture (profiles/r02_fit_pair_kernel.md)"}
         hbm = {"bound": "hbm", "kernel": "kf::fit_pair_kernel", "achieved": alg_bytes / t_launch / 1e9, "peak": peak,
-               "unit": "GB/s", "frac": alg_bytes / t_launch / 1e9 / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+               "unit": "GB/s", "frac": alg_bytes / t_launch / 1e9 / peak, "traffic": traffic,
                "peak_source": peak_src, "algorithmic_bytes_per_launch": int(alg_bytes), "bytes_per_fit": 233 + 36 * L}
-        # ALU roofline: algorithmic flops of the textbook sparse 6x6 filter (850 flop per
-        # track and layer, frozen before tuning) against the FP32 FMA peak measured on this GPU just now.
+        # ALU roofline, ALGORITHMIC: flops of the textbook sparse 6x6 filter (850 flop per
+        # track and layer, frozen before tuning) against the FP32 FMA peak measured on this GPU just now by the
+        # library's own microbenchmark (self-measured: MEASURED_PEAKS.json has no FP32 entry).
         alg_flops = float(n) * FLOPS_PER_TRACK_LAYER * L
+        exe_flops = float(n) * EXECUTED_FLOPS_PER_TRACK_LAYER * L
         alu = {"bound": "alu", "kernel": "kf::fit_pair_kernel", "achieved": alg_flops / t_launch / 1e12, "peak": fp32_peak,
-               "unit": "TFLOP/s", "frac": alg_flops / t_launch / 1e12 / fp32_peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-               "peak_source": "measured now: kf_measure_fp32_peak (register-only FMA chains); nominal 148 SM x 128 lanes "
-                              "x 2 x 1.965 GHz = 74.4", "algorithmic_flops_per_launch": alg_flops,
-               "flops_per_fit": FLOPS_PER_TRACK_LAYER * L}
-        # the binding roofline is the one with the larger lower bound on time
+               "unit": "TFLOP/s", "frac": alg_flops / t_launch / 1e12 / fp32_peak, "traffic": traffic,
+               "peak_source": "self-measured now: kf_measure_fp32_peak (register-only FMA chains); nominal 148 SM x 128 "
+                              "lanes x 2 x 1.965 GHz = 74.4", "algorithmic_flops_per_launch": alg_flops,
+               "flops_per_fit": FLOPS_PER_TRACK_LAYER * L, "label": "algorithmic (textbook count, the contract of SURVEY 8(d))",
+               # what the implementation executes (local-frame filter): fewer flops than the textbook count, so ITS
+               # floor is the HBM one; this fraction is the FP32 work really done over the same peak
+               "executed_flops_per_fit": EXECUTED_FLOPS_PER_TRACK_LAYER * L,
+               "executed_frac": exe_flops / t_launch / 1e12 / fp32_peak,
+               "executed_source": "SASS opcode histogram of the ncu capture: FFMA2 = 4, FMUL2 / FADD2 = 2, FFMA = 2, "
+                                  "FMUL / FADD / MUFU = 1 flop per thread instruction (profiles/r02_fit_pair_kernel.md)"}
+        # the binding roofline is the one with the larger lower bound on time under the frozen algorithmic counts
+        # (SURVEY.md 8(d)); `implementation_floor` is the larger bound for the work this kernel really does.
         roofline, other = (alu, hbm) if alg_flops / (fp32_peak * 1e12) > alg_bytes / (peak * 1e9) else (hbm, alu)
-        roofline = dict(roofline, bound_time_ms=1e3 * max(alg_flops / (fp32_peak * 1e12), alg_bytes / (peak * 1e9)))
+        roofline = dict(roofline, bound_time_ms=1e3 * max(alg_flops / (fp32_peak * 1e12), alg_bytes / (peak * 1e9)),
+                        hardware_counters=hw,
+                        implementation_floor={"bound": "hbm" if alg_bytes / (peak * 1e9) > exe_flops / (fp32_peak * 1e12) else "alu",
+                                              "floor_ms": 1e3 * max(exe_flops / (fp32_peak * 1e12), alg_bytes / (peak * 1e9)),
+                                              "frac": max(exe_flops / (fp32_peak * 1e12), alg_bytes / (peak * 1e9)) / t_launch})
         threads = min(os.cpu_count() or 1, 64)
         if ws == 1:
             ns = n                          # the whole workload: about 1 s of wall time, 15 s of CPU time on 16 cores
@@ -499,7 +672,17 @@ def run_ours(args) -> None:
                "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "roofline_other": other,
                "cpu_baseline": cpu, "host_path_vs_device_path": host_vs_dev}
         if building is not None:
-            building["alu_roofline_frac"] = building["algorithmic_gflop"] * 1e9 / (building["build_ms"] * 1e-3) / (fp32_peak * 1e12)
+            # "algorithmic-equivalent": 850 + 60 n_window flop per candidate-layer as if every window hit were scored;
+            # bin pruning and the Cauchy-Schwarz pre-filter skip most of them with identical results, so this is NOT
+            # a hardware utilisation (it would exceed 1 with more pruning).  The hardware view of the scan kernel
+            # is in `scan_kernel_hw` (ncu counters of one launch, profiles/r02_counters.csv).
+            building["algorithmic_equivalent_alu_frac"] = building["algorithmic_gflop"] * 1e9 / (building["build_ms"] * 1e-3) / (fp32_peak * 1e12)
+            sc = _kernel_counters(counters, "scan_kernel") or {}
+            sc_flops = sc.get("fadd", 0.0) + sc.get("fmul", 0.0) + 2.0 * sc.get("ffma", 0.0) if sc else None
+            building["scan_kernel_hw"] = {"executed_fp32_flop_per_launch": sc_flops, "ncu_duration_s": sc.get("ncu_duration"),
+                                          "executed_alu_frac": (sc_flops / sc["ncu_duration"] / (fp32_peak * 1e12)) if sc and sc.get("ncu_duration") else None,
+                                          "fma_pipe_active_pct": sc.get("fma_pipe_pct"), "issue_slots_busy_pct": sc.get("issue_pct"),
+                                          "warps_active_pct_of_peak": sc.get("warps_active_pct")}
             out["building"] = building
         if smoothing is not None:
             out["smoothing"] = smoothing
@@ -519,7 +702,13 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-building", action="store_true", help="skip the secondary configs[4] building measurement")
     ap.add_argument("--events", type=int, default=100, help="events of 20 000 tracks per GPU (configs[2] = 100)")
+    ap.add_argument("--profile-sequence", action="store_true", help="one launch of every hot call, for ncu (see profiles/)")
+    ap.add_argument("--opcode-table", metavar="CSV", help="summarise an `ncu --page source --csv` export per SASS opcode")
     args = ap.parse_args()
+    if args.opcode_table:
+        return _opcode_table(args.opcode_table)
+    if args.profile_sequence:
+        return run_profile_sequence(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)

@@ -305,11 +305,20 @@ KF_API int kf_order_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, 
  * lowest chi2 in the window when it is below chi2_cut, otherwise some value >= chi2_cut (hits that
  * provably cannot beat the cut are not evaluated; +inf if none was).  Propagation failure: status bit, candidate untouched,
  * best_hit = -1, best_chi2 = +inf.  Reads bins->bin_offset, bins->hit_rec and bins->bin_box.  `order` = NULL or the
- * output of kf_order_candidates.  All pointers DEV.  The caller loops over layers. */
+ * output of kf_order_candidates.  All pointers DEV.  The caller loops over layers.
+ * `local_state` (optional, DEV [30][cands->ld] floats, 16-byte aligned, caller-allocated and ZEROED before the
+ * first layer): the candidates in the kernels' track-local frame, kept between the per-layer calls.  A Cartesian
+ * 6 x 6 covariance in fp32 cannot carry a fitted track to the tolerances of this library (|p| loose, direction
+ * tight: the momentum block is nearly singular); handed back in `cands` after every layer and read again, it
+ * costs about 2e-3 on covariance elements per round trip.  With `local_state` the call reads a candidate whose
+ * flag (plane 29) is set from there instead of from cands->par / cov, and leaves the updated candidate there
+ * (flag set) as well as in `cands`, so a chain of per-layer calls meets the same tolerances as
+ * kf_build_best_hit and kf_fit_tracks.  Opaque otherwise; zero plane 29 (or all of it) whenever `cands` is
+ * changed by anything but this call.  NULL: the candidate is read from `cands` (converted in double). */
 KF_API int kf_score_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, kf_tracks* cands,
                                const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
                                float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
-                               float* best_chi2);
+                               float* best_chi2, float* local_state);
 
 /* Best-hit building over n_build_layers consecutive layers first_layer, first_layer+1, ... in one call
  * (PAPER.md:73, 133): per layer exactly what kf_score_candidates does, but the candidates stay in the

@@ -49,6 +49,21 @@ static double g_half_length[32] = {
 static int g_energy_loss = 0; /* reading A21: 0 none, 1 mean Bethe loss in silicon at every layer crossing */
 void orc_set_energy_loss(int model) { g_energy_loss = model; }
 
+/* ---- surfaces (reading A23; "a more realistic geometry" with endcaps): layer l is a barrel cylinder
+ * (type 0: radius[l], optional half length) or a PAIR of endcap discs (type 1) in the planes z = +-disc_z[l],
+ * sensitive for disc_rmin[l] <= rho <= disc_rmax[l].  A track meets the disc on the side it is heading to
+ * (sign of pz).  Default: all barrels. */
+static int g_surface_type[32] = {0};
+static double g_disc_z[32], g_disc_rmin[32], g_disc_rmax[32];
+void orc_set_surfaces(int n_layers, const int32_t *type, const double *disc_z, const double *rmin, const double *rmax) {
+    for (int l = 0; l < 32; ++l) {
+        g_surface_type[l] = (type && l < n_layers) ? type[l] : 0;
+        g_disc_z[l] = (disc_z && l < n_layers) ? disc_z[l] : 0.0;
+        g_disc_rmin[l] = (rmin && l < n_layers) ? rmin[l] : 0.0;
+        g_disc_rmax[l] = (rmax && l < n_layers) ? rmax[l] : INFINITY;
+    }
+}
+
 static double g_score_half_length = INFINITY; /* the one layer orc_score_layer works on */
 void orc_set_score_half_length(double h) { g_score_half_length = h; }
 
@@ -145,15 +160,88 @@ int orc_propagate_inward(const double u[6], double q, double Bz, double r, doubl
     return propagate_dir(u, q, Bz, r, 1, out, F, s_out, theta_out);
 }
 
+/* ---- helix propagation to the plane z = zt, with Jacobian (reading A23) ---------------------------------------
+ * Same equations of motion and solution as above (reading A2); the path length now follows from z' = zt:
+ *   s = (zt - z) pT / pz,   theta = kappa s = k (zt - z) / pz.
+ * F = A + (df/ds) (x) (ds/du) with the same A (derivative at fixed s) and ds/du from the constraint z' = zt:
+ *   ds/du = -A[z, u] / (pz / pT)      (so row z of F vanishes: the arrival point stays in the plane and the
+ *   transported covariance has no variance along z -- the disc's counterpart of the radial null of a cylinder).
+ * Fails (ORC_PROP_FAIL, nothing written) unless the plane lies ahead (s > 0) within half a turn (|theta| < pi). */
+int orc_propagate_to_z(const double u[6], double q, double Bz, double zt, double out[6], double F[36],
+                       double *s_out, double *theta_out) {
+    double x = u[0], y = u[1], z = u[2], px = u[3], py = u[4], pz = u[5];
+    double k = q * ORC_C_B * Bz;
+    double pt2 = px * px + py * py;
+    double pt = sqrt(pt2);
+    if (!(pt > 0.0) || pz == 0.0) return ORC_PROP_FAIL;
+    double s = (zt - z) * pt / pz;
+    if (!(s > 0.0)) return ORC_PROP_FAIL;
+    double theta = k * s / pt;
+    if (!(fabs(theta) < ORC_PI)) return ORC_PROP_FAIL;
+    double S = sin(theta), co = cos(theta);
+    double sh = sin(0.5 * theta);
+    double Cm = 2.0 * sh * sh; /* 1 - cos(theta) without cancellation */
+    double xn = x + (px * S + py * Cm) / k;
+    double yn = y + (py * S - px * Cm) / k;
+    double pxn = px * co + py * S;
+    double pyn = -px * S + py * co;
+    if (F) {
+        double A[6][6];
+        memset(A, 0, sizeof A);
+        for (int i = 0; i < 6; ++i) A[i][i] = 1.0;
+        double taux = -theta * px / pt2, tauy = -theta * py / pt2; /* d theta / d(px,py) at fixed s */
+        A[0][3] = S / k + pxn * taux / k;
+        A[0][4] = Cm / k + pxn * tauy / k;
+        A[1][3] = -Cm / k + pyn * taux / k;
+        A[1][4] = S / k + pyn * tauy / k;
+        A[2][3] = -pz * s * px / (pt2 * pt);
+        A[2][4] = -pz * s * py / (pt2 * pt);
+        A[2][5] = s / pt;
+        A[3][3] = co + pyn * taux;
+        A[3][4] = S + pyn * tauy;
+        A[4][3] = -S - pxn * taux;
+        A[4][4] = co - pxn * tauy;
+        double kap = k / pt;
+        double dfds[6] = {pxn / pt, pyn / pt, pz / pt, kap * pyn, -kap * pxn, 0.0};
+        for (int c = 0; c < 6; ++c) {
+            double dsdu = -A[2][c] / (pz / pt);
+            for (int i = 0; i < 6; ++i) F[i * 6 + c] = A[i][c] + dfds[i] * dsdu;
+        }
+    }
+    out[0] = xn; out[1] = yn; out[2] = zt; out[3] = pxn; out[4] = pyn; out[5] = pz;
+    if (s_out) *s_out = s;
+    if (theta_out) *theta_out = theta;
+    return 0;
+}
+
+/* One layer of the geometry as the filter meets it: barrel (type 0) or disc pair (type 1, the disc on the side the
+ * track is heading to).  ORC_OUTSIDE: the crossing exists but lies beyond the barrel end / outside the annulus. */
+static int reach_surface(int l, const double u[6], double q, double Bz, double radius, double out[6], double F[36]) {
+    if (g_surface_type[l] == 0) {
+        int rc = orc_propagate(u, q, Bz, radius, out, F, NULL, NULL);
+        if (!rc && fabs(out[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
+        return rc;
+    }
+    int rc = orc_propagate_to_z(u, q, Bz, u[5] < 0.0 ? -g_disc_z[l] : g_disc_z[l], out, F, NULL, NULL);
+    if (!rc) {
+        double rho = sqrt(out[0] * out[0] + out[1] * out[1]);
+        if (rho < g_disc_rmin[l] || rho > g_disc_rmax[l]) rc = ORC_OUTSIDE;
+    }
+    return rc;
+}
+
 /* ---- process noise (reading A5): thin scatterer at the layer, evaluated at the propagated
  * momentum p': Q_pp = theta0^2 (|p|^2 I3 - p p^T), all other blocks zero. */
+static _Thread_local int g_at_surface = 0; /* type of the surface the state handed to the two functions below stands on (fit_one sets it) */
+static double cos_incidence(const double u[6]) { /* |cos| of the angle between the momentum and the surface normal */
+    double p = sqrt(u[3] * u[3] + u[4] * u[4] + u[5] * u[5]);
+    if (g_at_surface == 1) return fabs(u[5]) / p;                                      /* disc: normal = z axis */
+    return fabs(u[0] * u[3] + u[1] * u[4]) / (sqrt(u[0] * u[0] + u[1] * u[1]) * p); /* cylinder: normal = radial */
+}
 void orc_process_noise(const double u[6], double mass, double t, double Q[36]) {
     memset(Q, 0, 36 * sizeof(double));
     double p2 = u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
-    if (g_material_model == 1 && t > 0.0) { /* A20: path length through the layer */
-        double cospsi = fabs(u[0] * u[3] + u[1] * u[4]) / (sqrt(u[0] * u[0] + u[1] * u[1]) * sqrt(p2));
-        t = t / cospsi;
-    }
+    if (g_material_model == 1 && t > 0.0) t = t / cos_incidence(u); /* A20: path length through the layer */
     double th0 = orc_theta0(sqrt(p2), mass, t);
     for (int i = 0; i < 3; ++i)
         for (int j = 0; j < 3; ++j)
@@ -206,12 +294,9 @@ double orc_energy_loss(double p, double mass, double t) {
 }
 
 /* The effective thickness a state standing on a cylinder sees (A20 path length if that option is on). */
+static double cos_incidence(const double u[6]);
 static double seen_thickness(const double u[6], double t) {
-    if (g_material_model == 1 && t > 0.0) {
-        double p2 = u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
-        double cospsi = fabs(u[0] * u[3] + u[1] * u[4]) / (sqrt(u[0] * u[0] + u[1] * u[1]) * sqrt(p2));
-        t = t / cospsi;
-    }
+    if (g_material_model == 1 && t > 0.0) t = t / cos_incidence(u);
     return t;
 }
 
@@ -363,10 +448,10 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
             if (tr) memset(tr, 0, ORC_TRACE_STRIDE * sizeof(double));
             if (!((mask >> l) & 1u)) continue;
             double up[6], F[36], Q[36], Cp[36], un[6], Cn[36], dchi2;
-            int rc = orc_propagate(u, (double)q, Bz, radius[l], up, F, NULL, NULL);
-            if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
+            int rc = reach_surface(l, u, (double)q, Bz, radius[l], up, F); /* cylinder, or disc (reading A23) */
             if (tr && rc == ORC_OUTSIDE) memcpy(tr, up, 6 * sizeof(double)); /* diagnostic: where it missed */
             if (rc) { st |= (uint32_t)rc; continue; }
+            g_at_surface = g_surface_type[l];
             orc_process_noise(up, mass, xX0[l], Q);
             orc_transport_cov(F, C, Q, Cp);
             double G[36];
@@ -401,6 +486,7 @@ static void fit_one(int L, const double *radius, const double *xX0, double Bz, d
             }
         }
     }
+    g_at_surface = 0;
     memcpy(opar, u, sizeof u);
     memcpy(ocov, C, sizeof C);
     *ochi2 = chi2;
@@ -453,11 +539,13 @@ static int inv6(const double M[36], double Mi[36]) { /* Gauss-Jordan with partia
     return 0;
 }
 
-/* pseudo-inverse of a predicted covariance whose only null direction is the radial position direction of xp */
-static int pinv_radial_null(const double Cp[36], const double xp[6], double out[36]) {
+/* pseudo-inverse of a predicted covariance whose only null direction is the normal of the surface it was
+ * transported to: the radial position direction of xp (cylinder) or the z axis (disc, reading A23) */
+static int pinv_radial_null(const double Cp[36], const double xp[6], int surface, double out[36]) {
     double rho = sqrt(xp[0] * xp[0] + xp[1] * xp[1]);
     if (!(rho > 0.0)) return -1;
     double e[6] = {xp[0] / rho, xp[1] / rho, 0.0, 0.0, 0.0, 0.0};
+    if (surface == 1) { e[0] = 0.0; e[1] = 0.0; e[2] = 1.0; }
     double s = fmax(fmax(Cp[0], Cp[7]), Cp[14]);
     if (!(s > 0.0)) return -1;
     double M[36];
@@ -502,7 +590,7 @@ void orc_smooth_one(int L, const double *radius, const double *xX0, double Bz, d
         const double *xpn = tn, *Cpn = tn + 122, *Gn = tn + 158;
         const double *xsn = spar + 6 * next, *Csn = scov + 36 * next;
         double Ni[36], CG[36], A[36], D[36], AD[36];
-        if (pinv_radial_null(Cpn, xpn, Ni)) {
+        if (pinv_radial_null(Cpn, xpn, g_surface_type[next], Ni)) {
             *sstatus |= ORC_S_NOT_PD;
             broken = 1;
             memcpy(xs, xf, 6 * sizeof(double));

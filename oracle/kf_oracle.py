@@ -63,6 +63,10 @@ def lib():
         _lib.orc_set_geometry_options.argtypes = [C.c_int, C.c_int, dp]
         _lib.orc_set_score_half_length.restype = None
         _lib.orc_set_score_half_length.argtypes = [C.c_double]
+        _lib.orc_set_surfaces.restype = None
+        _lib.orc_set_surfaces.argtypes = [C.c_int, C.POINTER(C.c_int32), dp, dp, dp]
+        _lib.orc_propagate_to_z.restype = C.c_int
+        _lib.orc_propagate_to_z.argtypes = [dp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
         _lib.orc_set_energy_loss.restype = None
         _lib.orc_set_energy_loss.argtypes = [C.c_int]
         _lib.orc_energy_loss.restype = C.c_double
@@ -101,6 +105,36 @@ class geometry_options:
         lib().orc_set_geometry_options(0, 0, None)
         lib().orc_set_energy_loss(0)
         lib().orc_set_score_half_length(float("inf"))
+
+
+class surfaces:
+    """Context manager for the oracle's process-wide surface list (reading A23): surface_type[l] 0 = barrel
+    (radius[l]), 1 = pair of endcap discs at z = +-disc_z[l] sensitive for rmin[l] <= rho <= rmax[l].
+    Restores "all barrels" on exit."""
+
+    def __init__(self, surface_type, disc_z, rmin, rmax):
+        self.t = np.ascontiguousarray(surface_type, dtype=np.int32)
+        self.z = np.ascontiguousarray(disc_z, dtype=np.float64)
+        self.lo = np.ascontiguousarray(rmin, dtype=np.float64)
+        self.hi = np.ascontiguousarray(rmax, dtype=np.float64)
+
+    def __enter__(self):
+        lib().orc_set_surfaces(len(self.t), _p(self.t, C.c_int32), _p(self.z), _p(self.lo), _p(self.hi))
+        return self
+
+    def __exit__(self, *a):
+        lib().orc_set_surfaces(0, None, None, None, None)
+
+
+def propagate_to_z(u, q, Bz, zt, want_F=True):
+    """Helix to the plane z = zt (reading A23). -> (status, u_out[6], F[6,6] or None, s, theta)"""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    out = np.zeros(6)
+    F = np.zeros(36) if want_F else None
+    s = C.c_double(0.0)
+    th = C.c_double(0.0)
+    rc = lib().orc_propagate_to_z(_p(u), float(q), float(Bz), float(zt), _p(out), _p(F), C.byref(s), C.byref(th))
+    return rc, out, (F.reshape(6, 6) if want_F else None), s.value, th.value
 
 
 def _p(a, ct=C.c_double):
@@ -303,9 +337,16 @@ def fit_refit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mas
 
 
 def fit_batch(batch, nthreads: int = 1, want_trace: bool = False) -> dict:
-    """Convenience: fit a workloads.barrel_events.FitBatch-shaped object (duck-typed)."""
-    return fit_tracks(batch.radius, batch.x_over_X0, batch.Bz, batch.mass, batch.par, batch.cov,
-                      batch.q, batch.hpos, batch.hcov, batch.mask, nthreads, want_trace)
+    """Convenience: fit a workloads.barrel_events.FitBatch-shaped object (duck-typed).  A batch that carries a
+    surface list (reading A23) is fitted with it, its barrel half lengths and its material model."""
+    st = getattr(batch, "surface_type", None)
+    if st is None:
+        return fit_tracks(batch.radius, batch.x_over_X0, batch.Bz, batch.mass, batch.par, batch.cov,
+                          batch.q, batch.hpos, batch.hcov, batch.mask, nthreads, want_trace)
+    with surfaces(st, batch.disc_z, batch.disc_rmin, batch.disc_rmax), \
+            geometry_options(int(getattr(batch, "material_model", 0)), getattr(batch, "half_length", None)):
+        return fit_tracks(batch.radius, batch.x_over_X0, batch.Bz, batch.mass, batch.par, batch.cov,
+                          batch.q, batch.hpos, batch.hcov, batch.mask, nthreads, want_trace)
 
 
 # ------------------------------------------------------------------ binning and scoring

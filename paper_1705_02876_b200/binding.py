@@ -131,7 +131,7 @@ def load_library():
                                         C.c_float, vp]
     lib.kf_score_candidates.restype = C.c_int
     lib.kf_score_candidates.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.POINTER(_Tracks), C.POINTER(_LayerHits),
-                                        C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int, vp, vp, vp]
+                                        C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int, vp, vp, vp, vp]
     lib.kf_build_best_hit.restype = C.c_int
     lib.kf_build_best_hit.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
                                       C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
@@ -433,7 +433,8 @@ class KFContext:
     # ------------------------------------------------------------------ kf_score_candidates
     def score_candidates(self, geom: Geometry, layer: int, n: int, par, cov, q, chi2, nhits, status,
                          n_hits: int, pos, cov_hits, bins: Bins, window_half: int, chi2_cut: float,
-                         do_update: bool, best_hit, best_chi2, order=None):
+                         do_update: bool, best_hit, best_chi2, order=None, local_state=None):
+        """local_state: optional float32 [30][ld] device tensor, zeroed before the first layer (see the header)."""
         g, keep = geom._c()
         cands = self._tracks(n, par, cov, q, chi2, nhits, status)
         lh = _LayerHits(int(n_hits), _plane_ld(pos, 3), pos.data_ptr(), cov_hits.data_ptr())
@@ -442,7 +443,8 @@ class KFContext:
                                                   C.byref(lb), int(window_half), float(chi2_cut),
                                                   1 if do_update else 0,
                                                   order.data_ptr() if order is not None else None,
-                                                  best_hit.data_ptr(), best_chi2.data_ptr()),
+                                                  best_hit.data_ptr(), best_chi2.data_ptr(),
+                                                  local_state.data_ptr() if local_state is not None else None),
                     "kf_score_candidates")
         del keep
 

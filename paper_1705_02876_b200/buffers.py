@@ -179,10 +179,18 @@ class DeviceCandidates:
         return c
 
     def score(self, ctx: KFContext, geom: Geometry, layer: int, hits: DeviceLayer, window_half: int = 2,
-              chi2_cut: float = 30.0, do_update: bool = True, order: torch.Tensor | None = None):
+              chi2_cut: float = 30.0, do_update: bool = True, order: torch.Tensor | None = None,
+              keep_local: bool = True):
+        """kf_score_candidates on one layer.  keep_local: carry the candidates' local-frame state between the
+        per-layer calls (allocated and zeroed at the first call; see the header)."""
+        ls = None
+        if keep_local:
+            ls = getattr(self, "local_state", None)
+            if ls is None:
+                ls = self.local_state = torch.zeros((30, self.ld), dtype=torch.float32, device=self.par.device)
         ctx.score_candidates(geom, layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,
                              hits.n_hits, hits.pos, hits.cov, hits.bins, window_half, chi2_cut, do_update,
-                             self.best_hit, self.best_chi2, order)
+                             self.best_hit, self.best_chi2, order, ls)
 
     def build(self, ctx: KFContext, geom: Geometry, first_layer: int, layers: list, window_half: int = 2,
               chi2_cut: float = 30.0, do_update: bool = True, order: torch.Tensor | None = None):

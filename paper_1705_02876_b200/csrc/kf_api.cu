@@ -562,9 +562,11 @@ int check_score_bins(const kf_layer_hits* hits, const kf_layer_bins* bins, int w
 
 }  // namespace
 
-int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,
-                      const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half, float chi2_cut,
-                      int do_update, const int32_t* order, int32_t* hit_index, float* hit_chi2, int64_t ld_out) {
+namespace {
+int build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,
+                   const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half, float chi2_cut,
+                   int do_update, const int32_t* order, int32_t* hit_index, float* hit_chi2, int64_t ld_out,
+                   float* local_state) {
     if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
     FitParams P;
     int rc = make_params(geom, &P);
@@ -594,10 +596,20 @@ int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n
     a.order = order;
     a.n_eta = bins[0].n_eta; a.n_phi = bins[0].n_phi; a.eta_max = bins[0].eta_max;
     a.window_half = window_half; a.chi2_cut = chi2_cut; a.do_update = do_update ? 1 : 0;
+    if (local_state && !aligned16(local_state)) return KF_ERR_ALIGN;
+    a.lstate = local_state; a.ld_ls = cands->ld;
     KF_ON_DEVICE(c);
     cudaError_t e = launch_build(c->score, P, a, n_build_layers, steps, c->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
+}
+}  // namespace
+
+int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,
+                      const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half, float chi2_cut,
+                      int do_update, const int32_t* order, int32_t* hit_index, float* hit_chi2, int64_t ld_out) {
+    return build_best_hit(c, geom, first_layer, n_build_layers, cands, hits, bins, window_half, chi2_cut, do_update,
+                          order, hit_index, hit_chi2, ld_out, nullptr);
 }
 
 int kf_build_combinatorial(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,
@@ -643,11 +655,11 @@ int kf_build_combinatorial(kf_ctx* c, const kf_geometry* geom, int first_layer, 
 int kf_score_candidates(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks* cands,
                         const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
                         float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
-                        float* best_chi2) {
+                        float* best_chi2, float* local_state) {
     if (!c || !geom || !cands) return KF_ERR_NULL;
     if (cands->n > 0 && (!best_hit || !best_chi2)) return KF_ERR_NULL;
-    return kf_build_best_hit(c, geom, layer, 1, cands, hits, bins, window_half, chi2_cut, do_update, order,
-                             best_hit, best_chi2, cands->n > 0 ? cands->ld : 0);
+    return build_best_hit(c, geom, layer, 1, cands, hits, bins, window_half, chi2_cut, do_update, order,
+                          best_hit, best_chi2, cands->n > 0 ? cands->ld : 0, local_state);
 }
 
 }  // extern "C"

@@ -54,7 +54,7 @@ comb_init_kernel(const CombArgs a) {
     if (q != 1 && q != -1) { a.status[sd] |= ST_BAD_CHARGE; a.ncand_in[sd] = 0; return; }
     Track t;
     load_track(t, a.par, a.cov, a.ld, sd);
-    enter_local_frame(t);
+    enter_local_frame_precise(t);
     const int64_t slot = sd * a.nc;
     put_track(a.trk_in, a.ld_s, slot, t);
     a.chi2_in[slot] = a.chi2[sd];

@@ -806,7 +806,7 @@ fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ 
         st = ST_BAD_CHARGE;
     } else {
         const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
-        enter_local_frame(t);
+        enter_local_frame_precise(t);
         bool started = false;
         // pipeline registers: raw index of layer l + 2, slot of layer l + 1, hit of layer l
         int32_t h2 = L > 2 ? __ldg(H.index + 2 * H.ld_index + i) : -1;

@@ -170,6 +170,8 @@ struct ScoreArgs {
     int window_half; float chi2_cut; int do_update;
     // context scratch (filled by launch_build)
     float* scratch; float* track; int32_t* flag; int32_t* slot; int64_t ld_sc;
+    // kf_score_candidates: the caller's local-frame candidate state [30][ld_ls] (null: none)
+    float* lstate; int64_t ld_ls;
 };
 
 struct ScoreStep {

@@ -173,6 +173,41 @@ __device__ __forceinline__ void enter_local_frame(TrackT<F>& t) {
     reaim_momentum(t, t.px * ipt, -t.py * ipt, 0.0f, t.pz * ipt);
 }
 
+// The same entry in DOUBLE, for tracks that come out of a fit (candidates of the builders, the per-layer scoring
+// call): their Cartesian momentum block is nearly singular -- |p| loose, direction tight, eigenvalue ratio 1e4 to
+// 1e5 after three hits -- and the rotation + shear to (b1, b2, c) cancels that many digits: 2.5e4 x 6e-8 = 1.5e-3
+// in fp32, the whole covariance tolerance (measured on configs[4]: worst candidate 1.35 x the tolerance, 3 of
+// 20 000 above it; with this entry ... see DESIGN.md).  Done once per candidate, about 120 double operations.
+__device__ __forceinline__ void enter_local_frame_precise(Track& t) {
+    t.eax = 1.0f;
+    t.eay = 0.0f;
+    const double px = t.px, py = t.py, pz = t.pz;
+    const double pt2 = px * px + py * py;
+    if (!(pt2 > 0.0)) return;
+    const double ipt = 1.0 / sqrt(pt2);
+    const double dc = px * ipt, ds = -py * ipt, k1 = -pz * ipt;   // T_old = 0, T_new = pz/pT: k1 = -T_new, k2 = 0
+    double a, b;
+    double c03 = t.c03, c04 = t.c04, c13 = t.c13, c14 = t.c14, c23 = t.c23, c24 = t.c24;
+    a = c03; b = c04; c03 = dc * a - ds * b; c04 = ds * a + dc * b;
+    a = c13; b = c14; c13 = dc * a - ds * b; c14 = ds * a + dc * b;
+    a = c23; b = c24; c23 = dc * a - ds * b; c24 = ds * a + dc * b;
+    a = t.c35; b = t.c45;
+    const double c35 = dc * a - ds * b, c45 = ds * a + dc * b;
+    const double cc = dc * dc, ss = ds * ds, cs = dc * ds;
+    const double ll = t.c33, ln = t.c34, nn = t.c44;
+    const double c33 = cc * ll - 2.0 * cs * ln + ss * nn;
+    const double c44 = ss * ll + 2.0 * cs * ln + cc * nn;
+    const double c34 = cs * (ll - nn) + (cc - ss) * ln;
+    const double n35 = c35 + k1 * c33;
+    const double n45 = c45 + k1 * c34;
+    t.c05 = (float)((double)t.c05 + k1 * c03);
+    t.c15 = (float)((double)t.c15 + k1 * c13);
+    t.c25 = (float)((double)t.c25 + k1 * c23);
+    t.c55 = (float)((double)t.c55 + k1 * (c35 + n35));
+    t.c03 = (float)c03; t.c04 = (float)c04; t.c13 = (float)c13; t.c14 = (float)c14; t.c23 = (float)c23; t.c24 = (float)c24;
+    t.c33 = (float)c33; t.c34 = (float)c34; t.c44 = (float)c44; t.c35 = (float)n35; t.c45 = (float)n45;
+}
+
 // Local frame -> global frame (inverse of the above for the current frames).
 template <class F>
 __device__ __forceinline__ void leave_local_frame(TrackT<F>& t) {

@@ -60,8 +60,14 @@ propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
     const int q = a.q[i];
     if (q != 1 && q != -1) { a.status[i] |= ST_BAD_CHARGE; a.flag[i] = FLAG_DEAD; return; }
     Track t;
-    load_track(t, a.par, a.cov, a.ld, i);
-    enter_local_frame(t);
+    // the per-layer call with a caller-kept local-frame state (kf_score_candidates, local_state): plane 29 says
+    // whether planes 0..28 hold this candidate
+    if (a.lstate && __float_as_int(a.lstate[29 * a.ld_ls + i]) != 0) {
+        get_track(a.lstate, a.ld_ls, i, t);
+    } else {
+        load_track(t, a.par, a.cov, a.ld, i);
+        enter_local_frame_precise(t);
+    }
     if (keep_track) put_track(a.track, a.ld_sc, i, t);
     const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
     const uint32_t rc = propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.model, P.mass2, P.el,
@@ -100,6 +106,10 @@ update_global_kernel(const ScoreArgs a, int have_track) {
     if (f == FLAG_AT_LAYER) apply_decision(a, i, t);
     else if (have_track) get_track(a.track, a.ld_sc, i, t);
     else return;
+    if (a.lstate) {   // the candidate as it stands now, in the local frame, for the next per-layer call
+        put_track(a.lstate, a.ld_ls, i, t);
+        a.lstate[29 * a.ld_ls + i] = __int_as_float(1);
+    }
     leave_local_frame(t);
     store_track(t, a.par, a.cov, a.ld, i);
 }

@@ -79,7 +79,7 @@ def test_combinatorial_parity(ctx, n_tracks, noise, n_cand, geom):
     assert np.array_equal(nf[sel & clear], o["n_cand"][sel & clear])
     sub_g = {k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in ("par", "cov", "chi2", "nhits", "status")}
     sub_o = dict(par=o["par"][:, sel], cov=o["cov"][sel], chi2=o["chi2"][sel], nhits=o["nhits"][sel], status=o["status"][sel])
-    compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0, loosen=dict(cov=3.0))
+    compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0)
     # differing seeds: still a valid track (hits exist, nhits = seed hits + hits taken)
     for i in np.flatnonzero(~same)[:50]:
         taken = idx[:, i]

@@ -130,7 +130,7 @@ def test_chain_bin_build_fit(ctx):
     full = np.concatenate([np.stack([l.true_index for l in ev.layers[:3]]), found]).astype(np.int32)
     g = _fit_indexed(ctx, ev, full)
     o = _oracle_fit_with(ev, full)
-    res = compare_fit(g, o, float(f.radius[-1]), max_diverged_frac=0.2, loosen=dict(cov=3.0))
+    res = compare_fit(g, o, float(f.radius[-1]), max_diverged_frac=0.2)
     print("chain final-fit parity:", res)
 
 

@@ -36,8 +36,8 @@ def _both(ctx, b, kappa=O.REFIT_KAPPA, with_mask=True):
     return d, o
 
 
-def _compare(d, o, r_last, max_div=1e-3, loosen=None):
-    fwd = compare_fit(d.results(), {k: o[k] for k in ("par", "cov", "chi2", "nhits", "status")}, r_last, max_div, loosen)
+def _compare(d, o, r_last, max_div=1e-3, loosen=None, ill=None, max_ill_frac=0.0):
+    fwd = compare_fit(d.results(), {k: o[k] for k in ("par", "cov", "chi2", "nhits", "status")}, r_last, max_div)
     sg = d.refit_results()
     assert np.array_equal(sg["status"], o["rstatus"])
     # Smoothed result, same metric.  Excluded (A14): tracks the FORWARD fit flagged or that diverged there, and
@@ -46,7 +46,8 @@ def _compare(d, o, r_last, max_div=1e-3, loosen=None):
     fwd_div = o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)
     excl = o["status"] | o["rstatus"] | (fwd_div.astype(np.uint32) << 4)
     so = dict(par=o["rpar"], cov=o["rcov"], chi2=o["rchi2"], nhits=o["nhits"], status=excl)
-    sm = compare_fit(dict(sg, status=excl, nhits=o["nhits"]), so, r_last, max_diverged_frac=max(max_div, 2e-3), loosen=loosen)
+    sm = compare_fit(dict(sg, status=excl, nhits=o["nhits"]), so, r_last, max_diverged_frac=max(max_div, 2e-3), loosen=loosen,
+                     ill=ill, max_ill_frac=max_ill_frac)
     return fwd, sm
 
 
@@ -69,10 +70,18 @@ def test_refit_extreme_layer_counts(ctx, n_layers, step, n, pair_masked):
     cfg = dataclasses.replace(W.get_config(3 if n_layers > 3 else 1), n_layers=n_layers, layer_step_cm=step, n_tracks=n)
     b = W.simulate_event(cfg, 22, n_tracks=n)
     d, o = _both(ctx, b)
-    # Three hits barely constrain |p| (5 parameters from 6 good coordinates): the fit is ill-conditioned and the
-    # worst of 160 000 such tracks reaches 2.2e-4 relative on the momentum in fp32 (99 % stay below 0.2e-4), so the
-    # short geometries are held to 4 x the momentum tolerance (known limits).
-    fwd, sm = _compare(d, o, float(b.radius[-1]), max_div=1e-3 if n_layers > 3 else 1.0)
+    # Three hits barely constrain |p| (5 parameters from 6 good coordinates).  The forward fit meets the tolerances
+    # all the same; the REFIT, which starts from that fit inflated by kappa, moves the momentum of a few such
+    # tracks by 80 - 440 % of itself -- far outside the range where its linearisation means anything, and where
+    # fp32 and fp64 follow different branches.  Oracle-side rule: a refit that moved |p| by more than half of
+    # itself is ill-conditioned (measured: 10 of 160 000 three-hit tracks exceed the tolerance, every one of them
+    # has a shift > 0.79; the rule marks about 2 %); those are held to 4 x the momentum tolerance, all others to 1 x.
+    ill = None
+    if n_layers <= 3:
+        pabs = np.linalg.norm(o["rpar"][3:], axis=0)
+        ill = np.linalg.norm(o["rpar"][3:] - o["par"][3:], axis=0) > 0.5 * pabs
+    fwd, sm = _compare(d, o, float(b.radius[-1]), max_div=1e-3 if n_layers > 3 else 1.0,
+                       loosen={"mom": 4.0} if n_layers <= 3 else None, ill=ill, max_ill_frac=0.05)
     assert n_layers > 3 or (fwd["mom_p99"] <= 0.5 and sm["mom_p99"] <= 0.5)
 
 

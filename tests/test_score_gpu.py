@@ -216,8 +216,10 @@ def _seeds(ev):
     return r["par"].astype(np.float32), O.pack_cov21(r["cov"]).astype(np.float32), r["chi2"], r["nhits"]
 
 
-def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
-    """Layers 3..9 on both sides; returns (decisions, differing decisions inside the tie window)."""
+def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True, keep_local=True):
+    """Layers 3..9 on both sides; returns (decisions, differing decisions inside the tie window).
+    keep_local: the per-layer calls carry the candidates' local-frame state (kf_score_candidates, local_state);
+    the final state is then held to the FIT tolerances."""
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
     f, cfg = ev.fit, ev.cfg
@@ -227,11 +229,12 @@ def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
     oc = O.Candidates(par, cov, f.q, chi2, nh)
     alive = np.ones(f.n, dtype=bool)         # candidates whose decisions agreed so far
     n_dec = n_tie = 0
+    worst_chi2 = 0.0
     for l in range(cfg.first_scored_layer, cfg.n_layers):
         lay = ev.layers[l]
         dl = DeviceLayer.from_numpy(lay.pos, lay.cov, NE, NP, EMAX, "cuda:0")
         dl.bin(ctx, lay.radius)
-        dc.score(ctx, geom, l, dl, 2, chi2_cut, do_update)
+        dc.score(ctx, geom, l, dl, 2, chi2_cut, do_update, keep_local=keep_local)
         torch.cuda.synchronize()
         ob = O.bin_hits(lay.pos, lay.radius, NE, NP, EMAX)
         orr = O.score_layer(oc, lay.radius, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NE, NP, EMAX,
@@ -246,8 +249,12 @@ def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
         n_tie += int(diff.sum())
         alive &= ~diff                       # such a candidate is not compared further
         acc = alive & (orr["best_hit"] >= 0)
+        # chi2 of ONE hit: fp32 positions carry one or two ulp of r = 40 cm (4e-6 .. 8e-6 cm = up to 8e-4 sigma_rphi),
+        # so d(chi2) ~ 2 sqrt(chi2) * 8e-4: 1.6e-3 at chi2 = 1 (SURVEY hard part 3).  Bound: 2e-3 max(chi2, 1); the
+        # total chi2 of a track is held to north_star's 1e-3 below.
         rel = np.abs(g["best_chi2"][acc] - b[acc]) / np.maximum(b[acc], 1.0)
-        assert rel.max(initial=0) < 1e-2, rel.max()      # informational bound; the index rule above is the contract
+        worst_chi2 = max(worst_chi2, rel.max(initial=0))
+        assert rel.max(initial=0) < 2e-3, rel.max()
         assert np.array_equal(g["status"][alive], oc.status[alive])
         assert np.array_equal(g["nhits"][alive], oc.nhits[alive])
     if check_state:
@@ -255,16 +262,20 @@ def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True):
         sel = alive & (oc.status == 0)
         sub_g = {k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in ("par", "cov", "chi2", "nhits", "status")}
         sub_o = dict(par=oc.par.T[:, sel], cov=oc.cov[sel], chi2=oc.chi2[sel], nhits=oc.nhits[sel], status=oc.status[sel])
-        # per-layer calls hand the covariance back in the GLOBAL frame in fp32 after every layer; that
-        # storage alone costs ~2e-3 on covariance elements (SURVEY.md hard part 1), so the state is held
-        # to 10x the fit's covariance tolerance and 3x its momentum tolerance here; the decisions above
-        # are held to north_star's rule unchanged.
-        res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0, loosen=dict(cov=10.0, mom=3.0))
-        print("scoring state parity:", res)
+        if keep_local:
+            # the candidates stayed in the local frame between the calls: the fit tolerances, unloosened
+            res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0)
+        else:
+            # Without local_state every layer hands the covariance back in the GLOBAL frame in fp32 and reads it
+            # again: about 2e-3 on covariance elements per round trip (SURVEY.md hard part 1; the header says so).
+            # That mode promises the decisions (checked above, unchanged) -- its state is only reported.
+            res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0,
+                              loosen=dict(cov=1e9, mom=1e9, pos=1e9, chi2=1e9))
+        print(f"scoring state parity (keep_local={keep_local}):", res, " worst per-layer chi2 error:", worst_chi2)
     return n_dec, n_tie
 
 
-def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0, half_length=None, material_model=0, energy_loss=0):
+def _build_event_fused(ctx, ev, use_order, half_length=None, material_model=0, energy_loss=0):
     """kf_build_best_hit over layers 3..9 in one call vs the oracle's layer loop: decisions by north_star's
     rule, final state at the FIT tolerances (the candidates never leave the local frame)."""
     import paper_1705_02876_b200 as K
@@ -304,10 +315,9 @@ def _build_event_fused(ctx, ev, use_order, cov_loosen=1.0, half_length=None, mat
     sub_o = dict(par=oc.par.T[:, sel], cov=oc.cov[sel], chi2=oc.chi2[sel], nhits=oc.nhits[sel], status=oc.status[sel])
     sub_g["status"] = sub_g["status"] & ~np.uint32(O.OUTSIDE)      # (bits already checked equal above)
     sub_o["status"] = sub_o["status"] & ~np.uint32(O.OUTSIDE)
-    # north_star fixes only the hit decisions for scoring; the state is held to the fit tolerances, except
-    # that with 100 000 noise hits per layer some candidates take wrong hits with chi2 up to 30 and kink by
-    # many sigma, where both filters linearise far from the truth: covariance 3e-3 there (worst seen 1.4e-3)
-    res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0, loosen=dict(cov=cov_loosen))
+    # north_star fixes only the hit decisions for scoring; the state is held to the fit tolerances all the same
+    # (the candidates enter the local frame in double: DESIGN.md 5.3)
+    res = compare_fit(sub_g, sub_o, float(f.radius[-1]), max_diverged_frac=1.0)
     print("fused building state parity:", res)
     return n_dec, n_tie
 
@@ -320,7 +330,7 @@ def test_build_best_hit_small_event(ctx):
 
 def test_build_best_hit_full_config4(ctx):
     ev = W.make_build_event(4)
-    n_dec, n_tie = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0)
+    n_dec, n_tie = _build_event_fused(ctx, ev, use_order=True)
     print(f"config 4 fused: {n_dec} decisions, {n_tie} differences inside the tie window")
     assert n_dec >= 0.99 * 7 * 20000 and n_tie <= 20
 
@@ -330,7 +340,7 @@ def test_build_best_hit_finite_barrel_and_path_length_material(ctx):
     ev = W.make_build_event(4, n_tracks=3000, noise_hits=15000)
     L = ev.fit.n_layers
     hl = np.full(L, 25.0, dtype=np.float32)
-    n_dec, _ = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0, half_length=hl, material_model=1)
+    n_dec, _ = _build_event_fused(ctx, ev, use_order=True, half_length=hl, material_model=1)
     assert n_dec >= 0.98 * 7 * 3000
 
 
@@ -338,13 +348,15 @@ def test_build_best_hit_with_energy_loss(ctx):
     """Reading A21 through the builder (with path-length material): same decisions as the oracle with the option,
     and the option is felt (the candidates end with less momentum than without it)."""
     ev = W.make_build_event(4, n_tracks=3000, noise_hits=15000)
-    n_dec, _ = _build_event_fused(ctx, ev, use_order=True, cov_loosen=3.0, material_model=1, energy_loss=1)
+    n_dec, _ = _build_event_fused(ctx, ev, use_order=True, material_model=1, energy_loss=1)
     assert n_dec >= 0.98 * 7 * 3000
 
 
 def test_score_small_event(ctx):
     ev = W.make_build_event(4, n_tracks=400, noise_hits=2000)
     n_dec, n_tie = _score_event(ctx, ev)
+    assert n_dec >= 0.99 * 7 * 400
+    n_dec, n_tie = _score_event(ctx, ev, keep_local=False)      # decisions do not need the local state
     assert n_dec >= 0.99 * 7 * 400
 
 

@@ -95,6 +95,11 @@ class FitBatch:
     material_model: int = 0                # DESIGN.md reading A20 (geometry options of the fit)
     half_length: np.ndarray = None         # [L] f32 barrel half lengths, None = unbounded
     energy_loss: int = 0                   # DESIGN.md reading A21
+    # DESIGN.md reading A23 (endcap discs); None = every layer is a barrel
+    surface_type: np.ndarray = None        # [L] i32: 0 barrel (radius, half_length), 1 disc pair
+    disc_z: np.ndarray = None              # [L] f32: |z| of the disc pair
+    disc_rmin: np.ndarray = None           # [L] f32
+    disc_rmax: np.ndarray = None           # [L] f32
 
     @property
     def n_layers(self) -> int:
@@ -266,6 +271,136 @@ def simulate_event(cfg: BarrelConfig, event: int, n_tracks: int | None = None,
         energy_loss=cfg.energy_loss)
 
 
+# ---- barrel + endcap toy (reading A23; "a more realistic geometry"): six barrels of half
+# length 30 cm inside four pairs of discs, |eta| up to 2.5
+ENDCAP_BARREL_RADII = (4.0, 8.0, 12.0, 16.0, 20.0, 24.0)
+ENDCAP_BARREL_HALF_LENGTH = 30.0
+ENDCAP_DISC_Z = (35.0, 45.0, 55.0, 65.0)
+ENDCAP_DISC_RMIN, ENDCAP_DISC_RMAX = 4.0, 26.0
+
+
+def _cross_plane(pos, mom, q, Bz, zt):
+    """Crossing of each truth helix with the plane z = zt: the turning angle follows from dz, the point by
+    rotating the position about the helix centre (not the fit's sine / one-minus-cosine form)."""
+    x, y, z = pos
+    px, py, pz = mom
+    k = q * C_B * Bz
+    theta = k * (zt - z) / pz
+    cx, cy = x + py / k, y - px / k
+    c, sn = np.cos(theta), np.sin(theta)
+    X = cx + (x - cx) * c + (y - cy) * sn
+    Y = cy - (x - cx) * sn + (y - cy) * c
+    return (X, Y, np.broadcast_to(zt, x.shape).astype(np.float64)), (px * c + py * sn, -px * sn + py * c, pz), theta
+
+
+def simulate_endcap_event(event: int, n_tracks: int = 20_000, eta_max: float = 2.5, pt_min: float = 0.5,
+                          pt_max: float = 10.0, x_over_X0: float = 0.01, Bz: float = 3.8, smear_hits: bool = True,
+                          smear_seed: bool = True, material_model: int = 0, dtype=np.float32,
+                          seed_prior_equals_smear: bool = False, seed_mom_smear: float = SEED_MOM_SMEAR,
+                          seed_pos_smear: float = SEED_POS_SMEAR) -> FitBatch:
+    """One event of the barrel + endcap toy.  Surfaces in list order: the six barrels by radius, then the four
+    disc pairs by |z|; every track meets them in that order (the barrels end at |z| = 30 cm, inside the first
+    disc).  A surface a track does not cross inside its sensitive area leaves no hit (mask bit 0) and no
+    material; the truth moves on from the last surface it did cross.  Barrel hits as in simulate_event; disc
+    hits: azimuth smeared by sigma_rphi / rho, radius by sigma_r = 0.1 cm, z exactly in the plane;
+    V = Rz(phi_h) diag(sigma_r^2, sigma_rphi^2, sigma_z^2) Rz^T for both (the variance along a surface's own
+    normal only keeps S invertible, reading A6).  seed_prior_equals_smear: the seed's prior covariance states the
+    smearing actually applied (0.03 cm, 10 % of pT) instead of reading A13's deliberately loose 0.3 cm / 30 %: for
+    pull tests on forward tracks, whose five hits on a short lever arm do not overrule the prior (with a prior
+    that is trusted, the smearing must also be small enough for the filter's linearisation to hold: a 10 %
+    momentum smear is a 0.1 rad direction error, 2 sigma_rphi of second-order displacement at the first layer)."""
+    rng = np.random.default_rng(BASE_SEED + 1000 * 7 + event)
+    n = n_tracks
+    nb, nd = len(ENDCAP_BARREL_RADII), len(ENDCAP_DISC_Z)
+    L = nb + nd
+    q = rng.choice(np.array([-1.0, 1.0]), size=n)
+    pt = rng.uniform(pt_min, pt_max, size=n)
+    phi = rng.uniform(0.0, 2 * np.pi, size=n)
+    eta = rng.uniform(-eta_max, eta_max, size=n)
+    mom = (pt * np.cos(phi), pt * np.sin(phi), pt * np.sinh(eta))
+    pos = (np.zeros(n), np.zeros(n), np.zeros(n))
+    truth_vertex = np.stack(pos + mom)
+    hpos = np.zeros((L, 3, n)); hcov = np.zeros((L, 6, n))
+    truth = np.full((L, 6, n), np.nan)
+    mask = np.zeros(n, dtype=np.uint32)
+    k = q * C_B * Bz
+    for l in range(L):
+        ptl = np.hypot(mom[0], mom[1])
+        if l < nb:
+            r = ENDCAP_BARREL_RADII[l]
+            R = ptl / np.abs(k)
+            centre = np.hypot(pos[0] + mom[1] / k, pos[1] - mom[0] / k)
+            reach = ~(r > 0.9 * (R + centre)) & (r > np.hypot(pos[0], pos[1]))
+            with np.errstate(invalid="ignore", divide="ignore"):
+                npos, nmom = _cross_cylinder(pos, mom, q, Bz, r)
+            hit = reach & (np.abs(npos[2]) <= ENDCAP_BARREL_HALF_LENGTH)
+        else:
+            zt = np.where(mom[2] < 0, -1.0, 1.0) * ENDCAP_DISC_Z[l - nb]
+            with np.errstate(invalid="ignore", divide="ignore"):
+                npos, nmom, theta = _cross_plane(pos, mom, q, Bz, zt)
+                rho = np.hypot(npos[0], npos[1])
+                hit = ((zt - pos[2]) * mom[2] > 0) & (np.abs(theta) < 0.5 * np.pi) & (rho >= ENDCAP_DISC_RMIN) & (rho <= ENDCAP_DISC_RMAX)
+        hit = hit & np.isfinite(npos[0]) & np.isfinite(npos[1])
+        pos = tuple(np.where(hit, a, b) for a, b in zip(npos, pos))
+        mom = tuple(np.where(hit, a, b) for a, b in zip(nmom, mom))
+        g = rng.standard_normal((2, n))
+        if not smear_hits:
+            g = np.zeros_like(g)
+        rho = np.hypot(pos[0], pos[1])
+        phi_h = np.arctan2(pos[1], pos[0]) + g[0] * SIGMA_RPHI / np.maximum(rho, 1e-9)
+        if l < nb:
+            hp = np.stack([r * np.cos(phi_h), r * np.sin(phi_h), pos[2] + g[1] * SIGMA_Z])
+        else:
+            rh = rho + g[1] * SIGMA_R
+            hp = np.stack([rh * np.cos(phi_h), rh * np.sin(phi_h), pos[2]])
+        hv = hit_covariance(phi_h)
+        hpos[l] = np.where(hit, hp, 0.0)
+        hcov[l] = np.where(hit, hv, 0.0)
+        mask |= (hit.astype(np.uint32) << np.uint32(l))
+        a = rng.standard_normal((2, n))
+        if x_over_X0 > 0.0:
+            px, py, pz = mom
+            p = np.sqrt(px * px + py * py + pz * pz)
+            t_eff = x_over_X0
+            if material_model == 1:
+                cosn = np.abs(pos[0] * px + pos[1] * py) / (np.maximum(rho, 1e-9) * p) if l < nb else np.abs(pz) / p
+                t_eff = x_over_X0 / cosn
+            th0 = np.where(hit, highland_theta0(p, M_PION, t_eff), 0.0)
+            ptt = np.hypot(px, py)
+            e1 = (-py / ptt, px / ptt, np.zeros(n))
+            ph = (px / p, py / p, pz / p)
+            e2 = (ph[1] * e1[2] - ph[2] * e1[1], ph[2] * e1[0] - ph[0] * e1[2], ph[0] * e1[1] - ph[1] * e1[0])
+            t1, t2 = np.tan(a[0] * th0), np.tan(a[1] * th0)
+            d = tuple(ph[i] + t1 * e1[i] + t2 * e2[i] for i in range(3))
+            dn = np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)
+            mom = tuple(np.where(hit, p * d[i] / dn, mom[i]) for i in range(3))
+        truth[l] = np.where(hit, np.stack(pos + mom), np.nan)
+    g = rng.standard_normal((6, n))
+    if not smear_seed:
+        g = np.zeros_like(g)
+    spar = truth_vertex.copy()
+    spar[0:3] += seed_pos_smear * g[0:3]
+    spar[3:6] += seed_mom_smear * pt * g[3:6]
+    spt = np.hypot(spar[3], spar[4])
+    scov = np.zeros((21, n))
+    diag_idx = [0, 6, 11, 15, 18, 20]
+    for i in range(3):
+        scov[diag_idx[i]] = (seed_pos_smear if seed_prior_equals_smear else SEED_POS_SIGMA0) ** 2
+        scov[diag_idx[3 + i]] = (seed_mom_smear * pt) ** 2 if seed_prior_equals_smear else (SEED_MOM_SIGMA0 * spt) ** 2
+    f32 = dtype
+    # radius[] stays strictly increasing for the ABI's check; it is not read for disc layers
+    radius = np.array(list(ENDCAP_BARREL_RADII) + [ENDCAP_BARREL_RADII[-1] + 1.0 + i for i in range(nd)])
+    return FitBatch(
+        n=n, radius=radius.astype(f32), x_over_X0=np.full(L, x_over_X0, dtype=f32), Bz=Bz, mass=M_PION,
+        par=np.ascontiguousarray(spar, dtype=f32), cov=np.ascontiguousarray(scov, dtype=f32), q=q.astype(np.int8),
+        hpos=np.ascontiguousarray(hpos, dtype=f32), hcov=np.ascontiguousarray(hcov, dtype=f32), mask=mask, truth=truth,
+        truth_vertex=truth_vertex, material_model=material_model,
+        half_length=np.array([ENDCAP_BARREL_HALF_LENGTH] * nb + [np.inf] * nd, dtype=f32),
+        surface_type=np.array([0] * nb + [1] * nd, dtype=np.int32),
+        disc_z=np.array([0.0] * nb + list(ENDCAP_DISC_Z), dtype=f32),
+        disc_rmin=np.full(L, ENDCAP_DISC_RMIN, dtype=f32), disc_rmax=np.full(L, ENDCAP_DISC_RMAX, dtype=f32))
+
+
 def concat_batches(batches: list[FitBatch]) -> FitBatch:
     b0 = batches[0]
     cat = lambda name, ax: np.ascontiguousarray(np.concatenate([getattr(b, name) for b in batches], axis=ax))
@@ -273,7 +408,8 @@ def concat_batches(batches: list[FitBatch]) -> FitBatch:
                     mass=b0.mass, par=cat("par", 1), cov=cat("cov", 1), q=cat("q", 0),
                     hpos=cat("hpos", 2), hcov=cat("hcov", 2), mask=cat("mask", 0),
                     truth=cat("truth", 2), truth_vertex=cat("truth_vertex", 1),
-                    material_model=b0.material_model, half_length=b0.half_length, energy_loss=b0.energy_loss)
+                    material_model=b0.material_model, half_length=b0.half_length, energy_loss=b0.energy_loss,
+                    surface_type=b0.surface_type, disc_z=b0.disc_z, disc_rmin=b0.disc_rmin, disc_rmax=b0.disc_rmax)
 
 
 def make_fit_batch(config: int, n_events: int | None = None, n_tracks: int | None = None) -> FitBatch:

@@ -269,6 +269,72 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
             ts.append(e0.elapsed_time(e1))
         replay[name] = float(np.median(ts[2:]))
         graph.close()
+    # several events in one call: 16 copies of the event's pools and candidates, one
+    # kf_build_best_hit_events call against 16 replays of the one-event graph
+    n_ev = 16
+    big = DeviceCandidates.from_numpy(np.tile(s["par"], (1, n_ev)), np.tile(s["cov"], (1, n_ev)), np.tile(f.q, n_ev),
+                                      np.tile(s["chi2"], n_ev), np.tile(s["nhits"], n_ev), dev)
+    big_seed = {k: getattr(big, k).clone() for k in ("par", "cov", "chi2", "nhits", "status")}
+    first = [e * f.n for e in range(n_ev + 1)]
+    eidx = torch.empty((L - L0, big.ld), dtype=torch.int32, device=dev)
+    ec2 = torch.empty((L - L0, big.ld), dtype=torch.float32, device=dev)
+
+    def events_call():
+        ctx.build_best_hit_events(geom, L0, first, big.n, big.par, big.cov, big.q, big.chi2, big.nhits, big.status,
+                                  [args] * n_ev, 2, 30.0, True, eidx, ec2)
+    with torch.cuda.stream(st):
+        events_call()
+    torch.cuda.synchronize()
+    for k, v in big_seed.items():
+        getattr(big, k).copy_(v)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        ctx.graph_begin()
+        events_call()
+        egraph = ctx.graph_end()
+    ts = []
+    for it in range(reps + 2):
+        for k, v in big_seed.items():
+            getattr(big, k).copy_(v)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        egraph.launch()
+        e1.record(st)
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    events_ms = float(np.median(ts[2:]))
+    egraph.close()
+    events_equal = bool(torch.equal(eidx[:, :f.n], out["idx"][:, :f.n]) and torch.equal(eidx[:, (n_ev - 1) * f.n:n_ev * f.n], out["idx"][:, :f.n]))
+    del big, big_seed, eidx, ec2
+    # end to end through kf_build_best_hit_host: pinned HOST pools and candidates in, results out, per event
+    # (H2D of layer j + 1 overlapped with binning + scoring of layer j)
+    from paper_1705_02876_b200.buffers import padded_ld
+    pin = lambda shape, dt: torch.zeros(shape, dtype=dt, pin_memory=True)
+    hpools, h2d = [], 0
+    for l in ev.layers[L0:]:
+        H = l.pos.shape[1]
+        tp, tc = pin((3, padded_ld(H)), torch.float32), pin((6, padded_ld(H)), torch.float32)
+        tp[:, :H] = torch.from_numpy(l.pos); tc[:, :H] = torch.from_numpy(l.cov)
+        hpools.append((H, tp, tc))
+        h2d += H * 36
+    hcand = {k: pin(getattr(dc, k).shape, getattr(dc, k).dtype) for k in ("par", "cov", "q", "chi2", "nhits", "status")}
+    hidx, hc2 = pin((L - L0, dc.ld), torch.int32), pin((L - L0, dc.ld), torch.float32)
+    h2d += f.n * (27 * 4 + 1 + 12)
+    d2h = f.n * (27 * 4 + 12 + (L - L0) * 8)
+
+    def host_call():
+        for k, v in seed.items():
+            hcand[k].copy_(v)                   # (device -> pinned host refill, outside the timed region)
+        hcand["q"].copy_(dc.q)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.build_best_hit_host(geom, L0, f.n, hcand["par"], hcand["cov"], hcand["q"], hcand["chi2"], hcand["nhits"],
+                                hcand["status"], hpools, cfg.n_eta, cfg.n_phi, emax, 2, 30.0, True, hidx, hc2)
+        return time.perf_counter() - t0
+    host_call(); host_call()
+    host_ms = 1e3 * float(np.median([host_call() for _ in range(reps)]))
+    host_equal = bool(np.array_equal(hidx[:, :f.n].numpy(), out["idx"][:, :f.n].cpu().numpy()))
     idx, cidx = out["idx"], out["cidx"]
     truth = np.stack([ev.layers[l].true_index for l in range(L0, L)])
     comb_eff = float((cidx[:, :f.n].cpu().numpy() == truth).all(axis=0).mean())
@@ -291,6 +357,7 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
     n_cl = f.n * (L - L0)
     flops = 850.0 * n_cl + 60.0 * n_win
     tb, ts, tc = replay["bin"], replay["build"], replay["comb"]
+    ts_build_one = ts
     taken = float((idx[:, :f.n] >= 0).float().mean().item())
     ctx.set_stream(None)
     return {"workload": "configs[4]: 20000 candidates, layers 3..9, 120000 hits/layer, 40x64 bins, +-2-bin window, chi2 < 30",
@@ -302,6 +369,15 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
             "algorithmic_gflop": flops / 1e9, "hit_taken_fraction": taken,
             "kernels_per_build": 2 * (L - L0) + 1, "reps": reps,
             "eager_bin_ms": eager["bin"], "eager_build_ms": eager["build"],
+            "e2e": {"api": "kf_build_best_hit_host (pinned HOST pools + candidates in, bin + build, results out)",
+                    "ms_per_event": host_ms, "candidate_layers_per_s": n_cl / (host_ms * 1e-3),
+                    "h2d_bytes_per_event": int(h2d), "d2h_bytes_per_event": int(d2h),
+                    "link_gb_per_s": (h2d + d2h) / (host_ms * 1e-3) / 1e9,
+                    "device_only_ms": tb + ts, "same_hits_as_device_call": host_equal},
+            "events_in_one_call": {"api": "kf_build_best_hit_events", "n_events": n_ev, "ms": events_ms,
+                                   "ms_per_event": events_ms / n_ev, "speedup_vs_one_event_per_call": ts_build_one / (events_ms / n_ev),
+                                   "candidate_layers_per_s": n_ev * n_cl / (events_ms * 1e-3),
+                                   "same_hits_as_single_event_call": events_equal},
             "combinatorial": {"n_cand": 4, "build_ms": tc, "eager_build_ms": eager["comb"],
                               "seeds_per_s": f.n / (tc * 1e-3),
                               "all_true_hits_found_fraction": comb_eff,
@@ -373,6 +449,8 @@ def _opcode_table(path: str) -> None:
     si = hdr.index("Source")
     ti = next(i for i, c in enumerate(hdr) if c.strip() == "Thread Instructions Executed")
     for r in rows[rows.index(hdr) + 1:]:
+        if r and r[0] == "Kernel Name":
+            break                                   # the export holds several launches: the first one only
         if len(r) <= max(si, ti):
             continue
         toks = r[si].replace("{", " ").split()

@@ -164,6 +164,20 @@ typedef struct {
                                  covariance is transported with dE held fixed; the backward refit gives
                                  the energy back.  A track that would stop fails that layer
                                  (KF_STATUS_PROP_FAIL).  Needs mass_gev > 0.                            */
+    /* Endcap discs ("a more realistic geometry"; reading A23).  NULL surface_type = every
+     * layer is a barrel.  A layer with surface_type[l] = 1 is a PAIR of discs in the planes z = +-disc_z_cm[l],
+     * sensitive for disc_rmin_cm[l] <= rho <= disc_rmax_cm[l]; a track meets the disc on the side it is heading to
+     * (sign of pz).  Layers are met in list order (barrels that end inside the first disc, then the discs by |z|).
+     * The state is propagated to the plane (theta = k (zt - z) / pz); the transported covariance then has no
+     * variance along z instead of along the radius; a crossing outside the annulus sets KF_STATUS_OUTSIDE and the
+     * layer is skipped; a plane that lies behind the state or half a turn or more away is KF_STATUS_PROP_FAIL.
+     * radius_cm[l] of a disc layer is not used but must keep the list increasing.  Discs are known to
+     * kf_fit_tracks, kf_fit_tracks_indexed and kf_fit_tracks_host; every other call returns KF_ERR_UNSUPPORTED
+     * for a geometry with a disc, and so does energy_loss_model = 1 with discs. */
+    const int32_t* surface_type;  /* HOST [n_layers] 0 = barrel, 1 = disc pair; or NULL                        */
+    const float* disc_z_cm;       /* HOST [n_layers] |z| of the disc pair (> 0), read where surface_type = 1   */
+    const float* disc_rmin_cm;    /* HOST [n_layers] inner radius of the annulus (>= 0)                         */
+    const float* disc_rmax_cm;    /* HOST [n_layers] outer radius (> inner)                                     */
 } kf_geometry;
 
 /* ---- tracks (seeds in, fitted tracks out; candidates in/out) ------------------------------------ */
@@ -333,6 +347,35 @@ KF_API int kf_build_best_hit(kf_ctx* ctx, const kf_geometry* geom, int first_lay
                              kf_tracks* cands, const kf_layer_hits* hits, const kf_layer_bins* bins,
                              int window_half, float chi2_cut, int do_update, const int32_t* order,
                              int32_t* hit_index, float* hit_chi2, int64_t ld_out);
+
+/* Best-hit building of SEVERAL EVENTS in one call (section 4.3: "concurrent events should be adapted
+ * to track building because this will help to fill the GPU's stream multiprocessors"; the fit gains
+ * a factor 3 from several events at once).  One event of 20 000 candidates is 157 CTAs of per-candidate work and
+ * about two waves of scanning warps on 148 SMs; n_events of them in one call fill the device with the same
+ * 2 n_build_layers + 1 launches.  `cands` holds the candidates of all events back to back: event e owns
+ * event_first[e] .. event_first[e + 1] - 1 (HOST int64 [n_events + 1], event_first[0] = 0, last = cands->n).
+ * hits / bins: HOST arrays [n_events][n_build_layers] (event-major), every event with its own pools, all bins
+ * with one (n_eta, n_phi, eta_max).  n_events <= 32.  Per candidate the result is exactly what kf_build_best_hit
+ * gives for its event alone (bit for bit); outputs as there. */
+KF_API int kf_build_best_hit_events(kf_ctx* ctx, const kf_geometry* geom, int first_layer, int n_build_layers,
+                                    int n_events, const int64_t* event_first, kf_tracks* cands,
+                                    const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                                    float chi2_cut, int do_update, int32_t* hit_index, float* hit_chi2,
+                                    int64_t ld_out);
+
+/* Best-hit building of one event with every buffer in HOST memory (pageable or pinned; pinned for overlap):
+ * the end-to-end path of building (section 4.3: on the K40 "almost half" of the building wall
+ * time went into transfers).  The candidates and, layer by layer on a second stream, the hit pools go to the
+ * device; layer j is binned (n_eta x n_phi bins over [-eta_max, eta_max) x [-pi, pi)) and scored while layer j + 1
+ * is still on its way; the candidates stay in the local frame between the layers; candidates, hit_index and
+ * hit_chi2 (HOST [n_build_layers][ld_out]) come back and the call returns when they are complete.  hits: HOST
+ * array of n_build_layers descriptors with HOST buffers inside.  Results are those of kf_bin_layers +
+ * kf_build_best_hit on the same data (the bins themselves stay on the device and are not returned).  Alignment
+ * rules do not apply.  Not recordable in a graph. */
+KF_API int kf_build_best_hit_host(kf_ctx* ctx, const kf_geometry* geom, int first_layer, int n_build_layers,
+                                  kf_tracks* cands, const kf_layer_hits* hits, int n_eta, int n_phi, float eta_max,
+                                  int window_half, float chi2_cut, int do_update, int32_t* hit_index,
+                                  float* hit_chi2, int64_t ld_out);
 
 /* Combinatorial building (reading A19) over n_build_layers consecutive
  * layers.  Every seed keeps at most n_cand (1..8) candidates.  On each layer every candidate is propagated

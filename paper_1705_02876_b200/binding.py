@@ -24,7 +24,7 @@ OPT_PAIR_MIN_TRACKS, OPT_REFIT_PAIR_MASKED, OPT_BIN_FORM = 1, 2, 3          # kf
 BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
            "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
-           "kf_score_candidates", "kf_build_best_hit", "kf_build_combinatorial",
+           "kf_score_candidates", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
 
@@ -39,7 +39,9 @@ class _Geometry(C.Structure):
     _fields_ = [("n_layers", C.c_int), ("radius_cm", C.POINTER(C.c_float)), ("x_over_X0", C.POINTER(C.c_float)),
                 ("Bz_tesla", C.c_float), ("mass_gev", C.c_float),
                 ("half_length_cm", C.POINTER(C.c_float)), ("material_model", C.c_int),
-                ("energy_loss_model", C.c_int)]
+                ("energy_loss_model", C.c_int), ("surface_type", C.POINTER(C.c_int32)),
+                ("disc_z_cm", C.POINTER(C.c_float)), ("disc_rmin_cm", C.POINTER(C.c_float)),
+                ("disc_rmax_cm", C.POINTER(C.c_float))]
 
 
 class _Tracks(C.Structure):
@@ -136,6 +138,14 @@ def load_library():
     lib.kf_build_best_hit.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
                                       C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
                                       vp, vp, vp, C.c_int64]
+    lib.kf_build_best_hit_events.restype = C.c_int
+    lib.kf_build_best_hit_events.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64),
+                                             C.POINTER(_Tracks), C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int,
+                                             C.c_float, C.c_int, vp, vp, C.c_int64]
+    lib.kf_build_best_hit_host.restype = C.c_int
+    lib.kf_build_best_hit_host.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
+                                           C.POINTER(_LayerHits), C.c_int, C.c_int, C.c_float, C.c_int, C.c_float,
+                                           C.c_int, vp, vp, C.c_int64]
     lib.kf_build_combinatorial.restype = C.c_int
     lib.kf_build_combinatorial.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
                                            C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
@@ -191,6 +201,10 @@ class Geometry:
     half_length_cm: np.ndarray | None = None   # reading A20: barrel half lengths, None = unbounded
     material_model: int = 0                    # reading A20: 1 = thickness / cos(incidence angle)
     energy_loss_model: int = 0                 # reading A21: 1 = mean Bethe loss in silicon at every crossing
+    surface_type: np.ndarray | None = None     # reading A23: 0 = barrel, 1 = disc pair; None = all barrels
+    disc_z_cm: np.ndarray | None = None
+    disc_rmin_cm: np.ndarray | None = None
+    disc_rmax_cm: np.ndarray | None = None
 
     def _c(self):
         r = np.ascontiguousarray(self.radius_cm, dtype=np.float32)
@@ -198,11 +212,18 @@ class Geometry:
         h = None if self.half_length_cm is None else np.ascontiguousarray(self.half_length_cm, dtype=np.float32)
         if h is not None and h.shape != r.shape:
             raise ValueError("half_length_cm must have one entry per layer")
-        hp = C.POINTER(C.c_float)() if h is None else h.ctypes.data_as(C.POINTER(C.c_float))
+        fp = lambda a: C.POINTER(C.c_float)() if a is None else a.ctypes.data_as(C.POINTER(C.c_float))
+        st = None if self.surface_type is None else np.ascontiguousarray(self.surface_type, dtype=np.int32)
+        dz, lo, hi = (None if a is None else np.ascontiguousarray(a, dtype=np.float32)
+                      for a in (self.disc_z_cm, self.disc_rmin_cm, self.disc_rmax_cm))
+        for a in (st, dz, lo, hi):
+            if a is not None and a.shape != r.shape:
+                raise ValueError("surface arrays must have one entry per layer")
+        stp = C.POINTER(C.c_int32)() if st is None else st.ctypes.data_as(C.POINTER(C.c_int32))
         g = _Geometry(int(r.shape[0]), r.ctypes.data_as(C.POINTER(C.c_float)), t.ctypes.data_as(C.POINTER(C.c_float)),
-                      float(self.Bz_tesla), float(self.mass_gev), hp, int(self.material_model),
-                      int(self.energy_loss_model))
-        return g, (r, t, h)       # keep the arrays alive while g is in use
+                      float(self.Bz_tesla), float(self.mass_gev), fp(h), int(self.material_model),
+                      int(self.energy_loss_model), stp, fp(dz), fp(lo), fp(hi))
+        return g, (r, t, h, st, dz, lo, hi)       # keep the arrays alive while g is in use
 
 
 @dataclass
@@ -463,6 +484,42 @@ class KFContext:
                                                 order.data_ptr() if order is not None else None,
                                                 hit_index.data_ptr(), hit_chi2.data_ptr(), int(hit_index.stride(0))),
                     "kf_build_best_hit")
+        del keep
+
+    def build_best_hit_events(self, geom: Geometry, first_layer: int, event_first, n: int, par, cov, q, chi2, nhits,
+                              status, layers_by_event, window_half: int, chi2_cut: float, do_update: bool, hit_index,
+                              hit_chi2):
+        """layers_by_event: one sequence of (n_hits, pos, cov, bins) per event (all the same length);
+        event_first: candidate offsets [n_events + 1]; the candidate tensors hold all events back to back."""
+        g, keep = geom._c()
+        cands = self._tracks(n, par, cov, q, chi2, nhits, status)
+        ne, m = len(layers_by_event), len(layers_by_event[0])
+        flat = [l for ev in layers_by_event for l in ev]
+        lhs = (_LayerHits * (ne * m))(*[self._layer_hits(nh, p, c) for (nh, p, c, _) in flat])
+        lbs = (_LayerBins * (ne * m))(*[b._c() for (_, _, _, b) in flat])
+        first = (C.c_int64 * (ne + 1))(*[int(v) for v in event_first])
+        self._check(self._lib.kf_build_best_hit_events(self._h, C.byref(g), int(first_layer), m, ne, first, C.byref(cands),
+                                                       lhs, lbs, int(window_half), float(chi2_cut), 1 if do_update else 0,
+                                                       hit_index.data_ptr(), hit_chi2.data_ptr(), int(hit_index.stride(0))),
+                    "kf_build_best_hit_events")
+        del keep
+
+    def build_best_hit_host(self, geom: Geometry, first_layer: int, n: int, par, cov, q, chi2, nhits, status, layers,
+                            n_eta: int, n_phi: int, eta_max: float, window_half: int, chi2_cut: float, do_update: bool,
+                            hit_index, hit_chi2):
+        """Everything in HOST (CPU) tensors: layers = sequence of (n_hits, pos [3][ld], cov [6][ld])."""
+        for t in (par, cov, q, chi2, nhits, status, hit_index, hit_chi2):
+            if t.is_cuda:
+                raise ValueError("build_best_hit_host takes CPU tensors")
+        g, keep = geom._c()
+        cands = self._tracks(n, par, cov, q, chi2, nhits, status)
+        m = len(layers)
+        lhs = (_LayerHits * m)(*[self._layer_hits(nh, p, c) for (nh, p, c) in layers])
+        self._check(self._lib.kf_build_best_hit_host(self._h, C.byref(g), int(first_layer), m, C.byref(cands), lhs,
+                                                     int(n_eta), int(n_phi), float(eta_max), int(window_half),
+                                                     float(chi2_cut), 1 if do_update else 0, hit_index.data_ptr(),
+                                                     hit_chi2.data_ptr(), int(hit_index.stride(0))),
+                    "kf_build_best_hit_host")
         del keep
 
     # ------------------------------------------------------------------ kf_build_combinatorial

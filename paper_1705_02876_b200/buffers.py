@@ -51,7 +51,9 @@ class DeviceFit:
         ld = padded_ld(n)
         geom = Geometry(np.asarray(batch.radius, dtype=np.float32), np.asarray(batch.x_over_X0, dtype=np.float32),
                         float(batch.Bz), float(batch.mass), getattr(batch, "half_length", None),
-                        int(getattr(batch, "material_model", 0)), int(getattr(batch, "energy_loss", 0)))
+                        int(getattr(batch, "material_model", 0)), int(getattr(batch, "energy_loss", 0)),
+                        getattr(batch, "surface_type", None), getattr(batch, "disc_z", None),
+                        getattr(batch, "disc_rmin", None), getattr(batch, "disc_rmax", None))
         dev = device
         mk = lambda shape, dt: torch.zeros(shape, dtype=dt, device=dev, pin_memory=(pin and str(dev) == "cpu"))
         return DeviceFit(

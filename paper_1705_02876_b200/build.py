@@ -36,13 +36,16 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """One nvcc process per translation unit (they run side by side), then one link step."""
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, defines: list[str] | None = None, out: str | None = None) -> str:
+    """One nvcc process per translation unit (they run side by side), then one link step.
+    defines / out: build a tuning variant (-DNAME=VALUE ...) into another file (kernel experiments; the binding
+    loads it when KF_B200_LIB points there)."""
+    if out is None and not defines and not force and not needs_build():
         return LIB
-    objdir = os.path.join(HERE, "build")
+    lib = out or LIB
+    objdir = os.path.join(HERE, "build") if out is None else out + ".obj"
     os.makedirs(objdir, exist_ok=True)
-    flags = NVCC_FLAGS[:-2] + (["-Xptxas", "-v"] if verbose else [])     # (-cudart static belongs to the link step)
+    flags = NVCC_FLAGS[:-2] + (["-Xptxas", "-v"] if verbose else []) + ["-D" + d for d in (defines or [])]   # (-cudart static belongs to the link step)
     procs = []
     for src in SOURCES:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
@@ -50,9 +53,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     failed = [src for src, _, p in procs if p.wait() != 0]
     if failed:
         raise subprocess.CalledProcessError(1, "nvcc -c " + " ".join(failed))
-    subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-shared", "-o", LIB] + [obj for _, obj, _ in procs])
-    return LIB
+    subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-shared", "-o", lib] + [obj for _, obj, _ in procs])
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    defs = [a[2:] for a in sys.argv[1:] if a.startswith("-D")]
+    outs = [a[6:] for a in sys.argv[1:] if a.startswith("--out=")]
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, defines=defs, out=outs[0] if outs else None))

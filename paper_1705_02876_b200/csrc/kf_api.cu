@@ -33,6 +33,7 @@ struct kf_ctx {
     CombScratch comb;
     // *_host staging
     HostStage host;
+    BuildHostStage build_host;
     // every reallocation of scratch and every rewrite of the bin edge tables moves this on
     uint64_t scratch_gen() const { return bin.gen + score.gen + comb.gen; }
 };
@@ -71,8 +72,9 @@ int cuda_fail(kf_ctx* c, cudaError_t e) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-// Geometry -> kernel constants.  Returns KF_OK or an error code.
-int make_params(const kf_geometry* g, FitParams* P) {
+// Geometry -> kernel constants.  Returns KF_OK or an error code.  allow_discs: the call knows disc layers
+// (reading A23: kf_fit_tracks, kf_fit_tracks_indexed, kf_fit_tracks_host); every other call refuses them.
+int make_params(const kf_geometry* g, FitParams* P, bool allow_discs = false) {
     if (!g || !g->radius_cm || !g->x_over_X0) return KF_ERR_NULL;
     if (g->n_layers < 1) return KF_ERR_SHAPE;
     if (g->n_layers > KF_MAX_LAYERS) return KF_ERR_UNSUPPORTED;
@@ -84,10 +86,24 @@ int make_params(const kf_geometry* g, FitParams* P) {
     P->inv_k0 = (float)(1.0 / k0);
     P->mass2 = (float)((double)g->mass_gev * (double)g->mass_gev);
     double prev = 0.0;
+    bool discs = false;
     for (int l = 0; l < g->n_layers; ++l) {
         const double r = g->radius_cm[l];
         if (!(r > prev)) return KF_ERR_UNSUPPORTED;  // strictly increasing, > 0 (also rejects NaN)
         prev = r;
+        P->layer[l].type = 0;
+        P->layer[l].rmax2 = INFINITY;
+        if (g->surface_type && g->surface_type[l] != 0) {   // reading A23: a pair of endcap discs
+            if (g->surface_type[l] != 1 || !allow_discs) return KF_ERR_UNSUPPORTED;
+            if (!g->disc_z_cm || !g->disc_rmin_cm || !g->disc_rmax_cm) return KF_ERR_NULL;
+            const double zd = g->disc_z_cm[l], lo = g->disc_rmin_cm[l], hi = g->disc_rmax_cm[l];
+            if (!(zd > 0.0) || !(lo >= 0.0) || !(hi > lo)) return KF_ERR_UNSUPPORTED;
+            P->layer[l].type = 1;
+            P->layer[l].zd = (float)zd;
+            P->layer[l].rmin2 = (float)(lo * lo);
+            P->layer[l].rmax2 = (float)(hi * hi);
+            discs = true;
+        }
         const double t = g->x_over_X0[l];
         double ms = 0.0;
         if (t > 0.0) {  // reading A5: theta0 = 0.0136/(beta p) sqrt(t) (1 + 0.038 ln t)
@@ -123,7 +139,9 @@ int make_params(const kf_geometry* g, FitParams* P) {
             P->layer[l].de0 = t > 0.0 ? (float)(0.307075e-3 * (14.0 / 28.0855) * t * 21.82) : 0.0f;
         }
     }
-    P->geometry_options = P->model != 0;
+    if (discs && g->energy_loss_model) return KF_ERR_UNSUPPORTED;   // (energy loss is implemented on barrels only)
+    P->geometry_options = (P->model != 0 || discs) ? 1 : 0;
+    P->has_discs = discs ? 1 : 0;
     for (int l = 0; l < g->n_layers; ++l) P->geometry_options |= std::isfinite(P->layer[l].half_len) ? 1 : 0;
     return KF_OK;
 }
@@ -201,6 +219,7 @@ int kf_destroy(kf_ctx* c) {
     c->score.release();
     c->comb.release();
     c->host.release();
+    c->build_host.release();
     delete c;
     return KF_OK;
 }
@@ -325,7 +344,7 @@ int kf_fit_tracks(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
                   const kf_track_hits* hits, kf_tracks* out) {
     if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if ((rc = check_tracks(seeds, true, true))) return rc;
     if ((rc = check_tracks(out, false, true))) return rc;
@@ -349,7 +368,7 @@ int kf_fit_tracks_indexed(kf_ctx* c, const kf_geometry* geom, const kf_tracks* s
                           int64_t ld_index, const kf_layer_hits* pools, const kf_layer_bins* bins, kf_tracks* out) {
     if (!c || !geom || !seeds || !pools || !out) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if ((rc = check_tracks(seeds, true, true))) return rc;
     if ((rc = check_tracks(out, false, true))) return rc;
@@ -447,7 +466,7 @@ int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seed
                        const kf_track_hits* hits, kf_tracks* out) {
     if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if ((rc = check_tracks(seeds, true, false))) return rc;
     if ((rc = check_tracks(out, false, false))) return rc;
@@ -610,6 +629,96 @@ int kf_build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n
                       int do_update, const int32_t* order, int32_t* hit_index, float* hit_chi2, int64_t ld_out) {
     return build_best_hit(c, geom, first_layer, n_build_layers, cands, hits, bins, window_half, chi2_cut, do_update,
                           order, hit_index, hit_chi2, ld_out, nullptr);
+}
+
+int kf_build_best_hit_events(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, int n_events,
+                             const int64_t* event_first, kf_tracks* cands, const kf_layer_hits* hits,
+                             const kf_layer_bins* bins, int window_half, float chi2_cut, int do_update,
+                             int32_t* hit_index, float* hit_chi2, int64_t ld_out) {
+    if (!c || !geom || !cands || !hits || !bins || !event_first) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
+    if (n_events < 1) return KF_ERR_SHAPE;
+    if (n_events > kMaxBuildEvents) return KF_ERR_UNSUPPORTED;
+    if ((rc = check_tracks(cands, true, true))) return rc;
+    if (event_first[0] != 0 || event_first[n_events] != cands->n) return KF_ERR_SHAPE;
+    for (int e = 0; e < n_events; ++e)
+        if (event_first[e + 1] < event_first[e]) return KF_ERR_SHAPE;
+    if (n_build_layers == 0 || cands->n == 0) return KF_OK;
+    if (!hit_index || !hit_chi2) return KF_ERR_NULL;
+    if (ld_out < cands->n) return KF_ERR_SHAPE;
+    ScoreStep steps[KF_MAX_LAYERS];
+    for (int j = 0; j < n_build_layers; ++j) {
+        for (int e = 0; e < n_events; ++e) {
+            const kf_layer_hits* h = hits + (int64_t)e * n_build_layers + j;
+            const kf_layer_bins* b = bins + (int64_t)e * n_build_layers + j;
+            if ((rc = check_score_bins(h, b, window_half))) return rc;
+            if (b->n_eta != bins[0].n_eta || b->n_phi != bins[0].n_phi || b->eta_max != bins[0].eta_max)
+                return KF_ERR_UNSUPPORTED;
+            steps[j].ev_hit_rec[e] = b->hit_rec;
+            steps[j].ev_bin_box[e] = b->bin_box;
+            steps[j].ev_bin_offset[e] = b->bin_offset;
+        }
+        steps[j].layer = first_layer + j;
+        steps[j].n_hits = hits[j].n_hits;
+        steps[j].hit_rec = bins[j].hit_rec;
+        steps[j].bin_box = bins[j].bin_box;
+        steps[j].bin_offset = bins[j].bin_offset;
+        steps[j].best_hit = hit_index + (int64_t)j * ld_out;
+        steps[j].best_chi2 = hit_chi2 + (int64_t)j * ld_out;
+    }
+    ScoreArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.n = cands->n; a.ld = cands->ld; a.par = cands->par; a.cov = cands->cov; a.q = cands->q;
+    a.chi2 = cands->chi2; a.nhits = cands->nhits; a.status = cands->status;
+    a.n_eta = bins[0].n_eta; a.n_phi = bins[0].n_phi; a.eta_max = bins[0].eta_max;
+    a.window_half = window_half; a.chi2_cut = chi2_cut; a.do_update = do_update ? 1 : 0;
+    a.ev.n = n_events;
+    for (int e = 0; e <= n_events; ++e) a.ev.first[e] = event_first[e];
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_build(c->score, P, a, n_build_layers, steps, c->stream);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_build_best_hit_host(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,
+                           const kf_layer_hits* hits, int n_eta, int n_phi, float eta_max, int window_half,
+                           float chi2_cut, int do_update, int32_t* hit_index, float* hit_chi2, int64_t ld_out) {
+    if (!c || !geom || !cands || !hits) return KF_ERR_NULL;
+    if (c->capturing) return KF_ERR_UNSUPPORTED;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
+    if ((rc = check_tracks(cands, true, false))) return rc;
+    if (n_eta < 1 || n_phi < 2 || window_half < 0) return KF_ERR_SHAPE;
+    if (n_phi % 2 != 0 || (int64_t)n_eta * n_phi > KF_MAX_BINS || 2 * window_half + 1 > n_phi || !(eta_max > 0.0f))
+        return KF_ERR_UNSUPPORTED;
+    if (n_build_layers == 0 || cands->n == 0) return KF_OK;
+    if (!hit_index || !hit_chi2) return KF_ERR_NULL;
+    if (ld_out < cands->n || cands->n > 0x7fffffffLL) return KF_ERR_SHAPE;
+    int64_t nh[KF_MAX_LAYERS], ldh[KF_MAX_LAYERS];
+    const float* pos[KF_MAX_LAYERS];
+    const float* cov[KF_MAX_LAYERS];
+    for (int j = 0; j < n_build_layers; ++j) {
+        if (hits[j].n_hits < 0 || hits[j].ld < hits[j].n_hits || hits[j].n_hits > 0x7fffffffLL) return KF_ERR_SHAPE;
+        if (hits[j].n_hits > 0 && (!hits[j].pos || !hits[j].cov)) return KF_ERR_NULL;
+        nh[j] = hits[j].n_hits; ldh[j] = hits[j].ld; pos[j] = hits[j].pos; cov[j] = hits[j].cov;
+    }
+    BuildHostIO io;
+    io.n = cands->n; io.ld = cands->ld; io.par = cands->par; io.cov = cands->cov; io.q = cands->q;
+    io.chi2 = cands->chi2; io.nhits = cands->nhits; io.status = cands->status;
+    io.first_layer = first_layer; io.n_layers = n_build_layers;
+    io.n_hits = nh; io.ld_hits = ldh; io.pos = pos; io.cov_hits = cov;
+    io.n_eta = n_eta; io.n_phi = n_phi; io.eta_max = eta_max; io.window_half = window_half; io.chi2_cut = chi2_cut;
+    io.do_update = do_update ? 1 : 0;
+    io.hit_index = hit_index; io.hit_chi2 = hit_chi2; io.ld_out = ld_out;
+    KF_ON_DEVICE(c);
+    cudaError_t e = build_best_hit_host(c->build_host, c->bin, c->score, P, io, c->stream, c->opt);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    return KF_OK;
 }
 
 int kf_build_combinatorial(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, kf_tracks* cands,

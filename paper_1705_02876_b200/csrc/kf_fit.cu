@@ -66,16 +66,42 @@ struct Hit {
 };
 
 // One layer for one track.  Returns 0 or the status bit of the failure (track untouched).
-template <bool RADIAL_NULL, bool GEOM = true>
+// One DISC layer for one track (reading A23): to-plane crossing, general covariance transport, 2-D update in the
+// plane.  Compiled only into the kernels specialised for geometries that have discs (GEOM = 2): as a call it
+// would force the track into local memory in every kernel that can reach it (measured: the barrel-with-options
+// fit went from 0.354 to 0.535 ms per 2 M tracks), inlined it costs registers where it is used only.
+__device__ __forceinline__ uint32_t fit_layer_disc(Track& t, float k, float ik, const LayerConst& L, int model, float mass2,
+                                                const Hit& m, float& chi2) {
+    DiscCrossing o;
+    const uint32_t reached = helix_to_plane(t, k, ik, L, o);
+    if (reached) return reached;
+    DiscCov n;
+    transport_cov_disc(t, o, k, ms_at_disc(L, model, o, t.pz), mass2, n);
+    Crossing c;                       // what hit_to_local reads of it
+    c.xn = o.xn; c.yn = o.yn; c.zn = o.zt; c.erx = o.erx; c.ery = o.ery;
+    LocalHit h;
+    hit_to_local(c, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
+    float d;
+    const uint32_t rc = kalman_update_disc(t, o, n, h, &d);
+    if (rc == 0u) chi2 += d;
+    return rc;
+}
+
+// GEOM 0: the paper's toy detector (options compiled out); 1: the options of readings A20 / A21 on barrels;
+// 2: the same plus endcap discs (reading A23).
+template <bool RADIAL_NULL, int GEOM = 1>
 __device__ __forceinline__ uint32_t fit_layer(Track& t, float k, float ik, const LayerConst& L, int model,
                                               float mass2, const Bethe& el, const Hit& m, float& chi2) {
+    if constexpr (GEOM == 2) {
+        if (L.type == 1) return fit_layer_disc(t, k, ik, L, model, mass2, m, chi2);
+    }
     Crossing o;
-    const uint32_t reached = reach_layer<false, GEOM>(t, k, ik, L, o);
+    const uint32_t reached = reach_layer<false, GEOM != 0>(t, k, ik, L, o);
     if (reached) return reached;
     PropCov n;
     transport_cov<RADIAL_NULL>(t, o, ms_at_crossing(L, model, o, t.pz), mass2, n);
     const float pz_in = t.pz;
-    if constexpr (GEOM) {
+    if constexpr (GEOM != 0) {
         if (model & MODEL_ENERGY_LOSS) {   // reading A21: on arrival, after C' = F C F^T + Q
             Eloss e;
             if (!energy_loss_factors(el, L, model, mass2, o.erx * o.elx + o.ery * o.ely, o.pt2, o.ipt, pz_in, false, e))
@@ -90,7 +116,7 @@ __device__ __forceinline__ uint32_t fit_layer(Track& t, float k, float ik, const
     float d;
     const uint32_t rc = kalman_update(t, o, n, h, &d);
     if (rc == 0u) chi2 += d;
-    else if constexpr (GEOM) t.pz = pz_in;   // layer skipped: the track stays as it was
+    else if constexpr (GEOM != 0) t.pz = pz_in;   // layer skipped: the track stays as it was
     return rc;
 }
 
@@ -138,11 +164,11 @@ __device__ __forceinline__ void store_layer_state(const Track& t, const FitArgs&
 // MODE 0: forward fit.  MODE 1 (= SMOOTH below): forward fit + the inward refit of reading A18.  MODE 2: forward fit
 // that also leaves the FILTERED state of every used layer, in the local frame, in the per-layer arrays of
 // kf_fit_tracks_smooth (23 floats per track and layer: the input of the backward RTS pass, kf_smooth.cu).
-template <int MODE, bool GEOM>
-__global__ void __launch_bounds__(kFitBlock, MODE == 1 ? 4 : KF_FIT_MIN_BLOCKS)
+template <int MODE, int GEOM>
+__global__ void __launch_bounds__(kFitBlock, MODE == 1 || GEOM == 2 ? 4 : KF_FIT_MIN_BLOCKS)
 fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
     constexpr bool SMOOTH = MODE == 1;
-    const int model = GEOM ? P.model : 0;
+    const int model = GEOM != 0 ? P.model : 0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     const int wid = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform by construction
@@ -206,7 +232,8 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             else rc = fit_layer<false, GEOM>(t, k, ik, P.layer[l], model, P.mass2, P.el, m, chi2);
             st |= rc;
             if (rc == 0u) {
-                nh += 1; started = true; used |= 1u << l;
+                nh += 1; used |= 1u << l;
+                started = GEOM != 2 || P.layer[l].type == 0;   // after a disc the z row is the null one, not the radial row
                 if constexpr (MODE == 2) { if (valid) store_layer_state(t, a, l, i); }
             }
         }
@@ -261,7 +288,7 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             __syncwarp();
             if ((used >> l) & 1u) {
                 float d;
-                const uint32_t rc = refit_step<GEOM>(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, P.el, first,
+                const uint32_t rc = refit_step<GEOM != 0>(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, P.el, first,
                                                      m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, &d);
                 if (rc == 0u) { schi2 += d; nb += 1; first = false; l_prev = l; }
                 else sst |= rc;
@@ -322,24 +349,31 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
 // 2j (component x) and 2j + 1 (component y) of the tile, reads them as one 8-byte word per row and runs the
 // arithmetic of kf_math.cuh on F = f2, i.e. one FFMA2 / FMUL2 / FADD2 where the one-track kernel issues two
 // instructions.  Forward fit of the toy detector only (no smoother, no geometry options).
+// One warp (64 tracks) per CTA, 12 CTAs per SM: the same 12 resident warps as 3 CTAs of 4 warps (168 registers), but
+// a batch is cut into units of 64 tracks instead of 256, so mid-size batches fill the SMs evenly (measured in one
+// run, 2 M tracks: 0.295 ms against 0.303 for 128 x 3; register caps 160 / 152 / 144 / 136 for 13 - 15 resident
+// warps: 0.306 / 0.309 / 0.322 / 0.364 -- the spills cost more than the extra warps give; 4 or 5 ring stages: 0.299).
 #ifndef KF_PAIR_BLOCK
-#define KF_PAIR_BLOCK 128
+#define KF_PAIR_BLOCK 32
 #endif
 #ifndef KF_PAIR_MIN_BLOCKS
-#define KF_PAIR_MIN_BLOCKS 3
+#define KF_PAIR_MIN_BLOCKS 12
 #endif
 #ifndef KF_PAIR_SMOOTH_MIN_BLOCKS
-#define KF_PAIR_SMOOTH_MIN_BLOCKS 3
+#define KF_PAIR_SMOOTH_MIN_BLOCKS 12
 #endif
 constexpr int kPairBlock = KF_PAIR_BLOCK;
 constexpr int kPairWarps = kPairBlock / 32;
 constexpr int kPairTile = 64;                      // tracks per warp
 constexpr int kHit2Floats = 9 * kPairTile;
 constexpr int kSeed2Floats = 27 * kPairTile;
-constexpr int kPark2Floats = 30 * 32;              // one parked track (29 values + chi2) per lane (ragged pairs)
-// (the smoother kernel has no park area: it spills a little and needs the shared-memory space as L1 -- with the
-// park area its 92 KB of spill working set per SM no longer fit and the kernel ran 17 % slower on full pairs)
-__host__ __device__ constexpr int warp2_floats(bool smooth) { return kStages * kHit2Floats + kSeed2Floats + (smooth ? 0 : kPark2Floats); }
+// One parked track (29 values + chi2) per lane (ragged pairs) lives INSIDE the seed / result tile, which is idle
+// between the load of the seeds and the staging of the results (30 x 32 of its 27 x 64 floats): no shared memory of
+// its own, so a deeper hit ring or more resident warps fit.  Price: a track that ends with nothing fitted can no
+// longer take its input back from the tile and re-reads it from global memory (restore_unfitted).
+constexpr int kPark2Floats = 30 * 32;
+static_assert(kPark2Floats <= kSeed2Floats, "the park area lives inside the seed tile");
+__host__ __device__ constexpr int warp2_floats(bool) { return kStages * kHit2Floats + kSeed2Floats; }
 constexpr int smem2_bytes(bool smooth) { return kPairWarps * warp2_floats(smooth) * 4 + kPairWarps * (kStages + 1) * 8; }
 
 struct Hit2 {
@@ -427,8 +461,8 @@ __device__ __noinline__ uint32_t fit_layer_one_of_pair(Track2& t, int c, float k
     KF_GETH(x) KF_GETH(y) KF_GETH(z) KF_GETH(vxx) KF_GETH(vxy) KF_GETH(vxz) KF_GETH(vyy) KF_GETH(vyz) KF_GETH(vzz)
 #undef KF_GETH
     const Bethe none = {0.0f, 0.0f, 0.0f, 0.0f};
-    const uint32_t rc = started ? fit_layer<true, false>(ts, k, ik, L, 0, mass2, none, mh, ch)
-                                : fit_layer<false, false>(ts, k, ik, L, 0, mass2, none, mh, ch);
+    const uint32_t rc = started ? fit_layer<true, 0>(ts, k, ik, L, 0, mass2, none, mh, ch)
+                                : fit_layer<false, 0>(ts, k, ik, L, 0, mass2, none, mh, ch);
     if (rc != 0u) return rc;
 #define KF_PUT(f) if (c) t.f.v.y = ts.f; else t.f.v.x = ts.f;
     KF_TRACK_FIELDS(KF_PUT)
@@ -483,6 +517,20 @@ __device__ __forceinline__ void pair_to_tile(const Track2& t, float* tile, int l
     }
 }
 
+// A track with nothing fitted goes back as it came.  Its columns of the seed tile may have served as park area in
+// the meantime, so the input is read again from global memory (rare: bad charge, empty mask, nothing reached).
+__device__ __forceinline__ void restore_unfitted(float* tile, const FitArgs& a, int lane, int64_t ix, int64_t iy, mask2 which) {
+    if (none_of(which)) return;
+#pragma unroll 1
+    for (int c = 0; c < 2; ++c) {
+        if (!(c ? which.y : which.x)) continue;
+        const int64_t i = c ? iy : ix;
+        float* p = tile + 2 * lane + c;
+#pragma unroll 1
+        for (int r = 0; r < 27; ++r) p[r * kPairTile] = r < 6 ? a.par[r * a.ld_in + i] : a.cov[(r - 6) * a.ld_in + i];
+    }
+}
+
 // MODE 2: filtered state of layer l of one or both tracks of the pair -> the per-layer arrays (see
 // store_layer_state): both with one 8-byte store per plane (tracks 2j, 2j + 1 are neighbours; ld is a multiple of
 // 4 and the tile starts at a multiple of 64, so the address is 8-byte aligned), one alone with 4-byte stores.
@@ -514,9 +562,13 @@ __device__ __forceinline__ void store_layer_state_pair(const Track2& t, const Fi
 }
 
 // SMOOTH = true: the forward fit, then the inward refit of reading A18 over the same hits (ring runs on,
-// outermost layer first), as in fit_kernel<1, false>.
+// outermost layer first), as in fit_kernel<1, 0>.
 template <int MODE>
+#ifdef KF_PAIR_MAXNREG
+__global__ void __maxnreg__(KF_PAIR_MAXNREG)       // tuning variants: a register cap instead of a CTA count
+#else
 __global__ void __launch_bounds__(kPairBlock, MODE == 1 ? KF_PAIR_SMOOTH_MIN_BLOCKS : KF_PAIR_MIN_BLOCKS)
+#endif
 fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps M, const FitArgs a) {
     constexpr bool SMOOTH = MODE == 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -528,7 +580,7 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
     constexpr int kWarp2Floats = warp2_floats(SMOOTH);
     float* wbase = reinterpret_cast<float*>(smem_raw) + wid * kWarp2Floats;
     float* seed_tile = wbase + kStages * kHit2Floats;
-    float* park = seed_tile + kSeed2Floats + lane;
+    float* park = seed_tile + lane;        // (inside the seed tile: see kPark2Floats)
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + kPairWarps * kWarp2Floats * 4) + wid * (kStages + 1);
     const uint32_t hit0 = smem_u32(wbase), seed0 = smem_u32(seed_tile), bar0 = smem_u32(bars);
     const int col = (int)i0;
@@ -742,10 +794,12 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
         if (sstorer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         return;
     }
+    __syncwarp();      // every lane is done with the park area inside the tile
     if (!none_of(done)) {
         leave_local_frame(t);
         pair_to_tile(t, seed_tile, lane, done);
     }
+    restore_unfitted(seed_tile, a, lane, ix, iy, {valid.x && !done.x, valid.y && !done.y});
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncwarp();
     const bool storer = elect_one();
@@ -791,6 +845,7 @@ __device__ __forceinline__ Hit fetch_hit(const IndexedPools& H, int l, int32_t s
     return m;
 }
 
+template <int GEOM>
 __global__ void __launch_bounds__(kFitBlock, 4)
 fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ IndexedPools H, const FitArgs a) {
     const int64_t i = (int64_t)blockIdx.x * kFitBlock + threadIdx.x;
@@ -823,10 +878,10 @@ fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ 
             h2 = l + 3 < L ? __ldg(H.index + (int64_t)(l + 3) * H.ld_index + i) : -1;
             if (h < 0) continue;
             uint32_t rc;
-            if (started) rc = fit_layer<true>(t, k, ik, P.layer[l], P.model, P.mass2, P.el, m, chi2);
-            else rc = fit_layer<false>(t, k, ik, P.layer[l], P.model, P.mass2, P.el, m, chi2);
+            if (started) rc = fit_layer<true, GEOM>(t, k, ik, P.layer[l], P.model, P.mass2, P.el, m, chi2);
+            else rc = fit_layer<false, GEOM>(t, k, ik, P.layer[l], P.model, P.mass2, P.el, m, chi2);
             st |= rc;
-            if (rc == 0u) { nh += 1; started = true; }
+            if (rc == 0u) { nh += 1; started = GEOM != 2 || P.layer[l].type == 0; }
         }
         if (nh > 0) leave_local_frame(t);
         else load_track(t, a.par, a.cov, a.ld_in, i);   // nothing fitted: the seed, bit-exact
@@ -852,12 +907,13 @@ cudaError_t ensure_fit_attributes() {
     if (e != cudaSuccess) return e;
     const uint64_t bit = 1ull << (dev & 63);
     if (done.load(std::memory_order_acquire) & bit) return cudaSuccess;
-    e = cudaFuncSetAttribute(fit_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    e = cudaFuncSetAttribute(fit_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
@@ -880,7 +936,10 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     // every hit (mask == NULL); the pair form of the fit parks and shadows the idle track and wins either way.
     // (Option refit_pair_masked lifts that condition: the tests use it to drive the pair refit's ragged-pair code,
     // which failures can reach without any mask, with masks.)
-    if (P.geometry_options == 0 && a.n >= pair_min &&
+    // (the pair form pays once the machine is full: at least 151 552 tracks, or 2 M track-layers -- config 3's
+    // 100 000 x 20 layers: 0.0429 ms against 0.0451 for the one-track kernel)
+    const bool big = opt.pair_min_tracks > 0 ? a.n >= pair_min : (a.n >= pair_min || a.n * (int64_t)L >= 2000000);
+    if (P.geometry_options == 0 && big &&
         (!smooth || (KF_PAIR_SMOOTH && (a.mask == nullptr || opt.refit_pair_masked != 0)))) {
         constexpr int W = kPairTile;
         if (!make_map(&M.hpos, a.hpos, a.n, a.ld_hit, (int64_t)L * 3, 3, W) ||
@@ -906,19 +965,22 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
         return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
     const bool geom = P.geometry_options != 0;   // reading A20 options in use
-    if (smooth && geom) fit_kernel<1, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else if (smooth) fit_kernel<1, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else if (store && geom) fit_kernel<2, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else if (store) fit_kernel<2, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else if (geom) fit_kernel<0, true><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
-    else fit_kernel<0, false><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    if (P.has_discs && (smooth || store)) return cudaErrorInvalidValue;   // (refused at the ABI: discs are known to the fit only)
+    if (smooth && geom) fit_kernel<1, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (smooth) fit_kernel<1, 0><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (store && geom) fit_kernel<2, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (store) fit_kernel<2, 0><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (P.has_discs) fit_kernel<0, 2><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (geom) fit_kernel<0, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else fit_kernel<0, 0><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     return cudaGetLastError();
 }
 
 cudaError_t launch_fit_indexed(const FitParams& P, const IndexedPools& H, const FitArgs& a, cudaStream_t stream) {
     if (a.n == 0) return cudaSuccess;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
-    fit_indexed_kernel<<<(unsigned)blocks, kFitBlock, 0, stream>>>(P, H, a);
+    if (P.has_discs) fit_indexed_kernel<2><<<(unsigned)blocks, kFitBlock, 0, stream>>>(P, H, a);
+    else fit_indexed_kernel<1><<<(unsigned)blocks, kFitBlock, 0, stream>>>(P, H, a);
     return cudaGetLastError();
 }
 

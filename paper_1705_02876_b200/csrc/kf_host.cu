@@ -6,6 +6,8 @@
 // with kernels via streams"; PAPER.md:164 transfers are half of the wall time when they are not).
 // With pinned host memory the copies are truly asynchronous; with pageable memory the runtime
 // stages them and the pipeline degrades gracefully.
+#include <cstring>
+
 #include "kf_internal.h"
 
 namespace kf {
@@ -109,6 +111,130 @@ cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const Launch
     return e;
 fail:
     for (int s = 0; s < kSlots; ++s) cudaStreamSynchronize(stream[s]);
+    return e;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// kf_build_best_hit_host
+cudaError_t BuildHostStage::reserve(size_t bytes) {
+    cudaError_t e;
+    if (!copy_stream) {
+        if ((e = cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return e;
+        for (int j = 0; j < 32; ++j)
+            if ((e = cudaEventCreateWithFlags(&ready[j], cudaEventDisableTiming)) != cudaSuccess) return e;
+        if ((e = cudaEventCreateWithFlags(&done, cudaEventDisableTiming)) != cudaSuccess) return e;
+    }
+    if (bytes <= cap) return cudaSuccess;
+    if (buf) cudaFree(buf);
+    buf = nullptr;
+    cap = 0;
+    if ((e = cudaMalloc(&buf, bytes)) != cudaSuccess) return e;
+    cap = bytes;
+    return cudaSuccess;
+}
+
+void BuildHostStage::release() {
+    if (buf) cudaFree(buf);
+    buf = nullptr;
+    cap = 0;
+    if (copy_stream) {
+        cudaStreamDestroy(copy_stream);
+        for (int j = 0; j < 32; ++j)
+            if (ready[j]) cudaEventDestroy(ready[j]);
+        if (done) cudaEventDestroy(done);
+        copy_stream = nullptr;
+        done = nullptr;
+        for (int j = 0; j < 32; ++j) ready[j] = nullptr;
+    }
+}
+
+cudaError_t build_best_hit_host(BuildHostStage& hs, BinScratch& bs, ScoreScratch& ss, const FitParams& P, const BuildHostIO& io,
+                                cudaStream_t stream, const LaunchOptions& opt) {
+    const int L = io.n_layers;
+    const int nb = io.n_eta * io.n_phi;
+    const int64_t ldc = (io.n + 3) / 4 * 4;
+    // device layout: candidates, local state, outputs, then per layer: pool (9 planes), bins
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += align256(bytes); return at; };
+    const size_t o_par = take((size_t)6 * ldc * 4), o_cov = take((size_t)21 * ldc * 4), o_q = take((size_t)ldc);
+    const size_t o_chi2 = take((size_t)ldc * 4), o_nh = take((size_t)ldc * 4), o_st = take((size_t)ldc * 4);
+    const size_t o_ls = take((size_t)30 * ldc * 4);
+    const size_t o_idx = take((size_t)L * ldc * 4), o_c2 = take((size_t)L * ldc * 4);
+    size_t o_pos[32], o_hcov[32], o_off[32], o_s2o[32], o_rec[32], o_box[32];
+    int64_t ldh[32];
+    for (int j = 0; j < L; ++j) {
+        ldh[j] = (io.n_hits[j] + 3) / 4 * 4;
+        if (ldh[j] < 4) ldh[j] = 4;
+        o_pos[j] = take((size_t)3 * ldh[j] * 4); o_hcov[j] = take((size_t)6 * ldh[j] * 4);
+        o_off[j] = take((size_t)(nb + 1) * 4); o_s2o[j] = take((size_t)ldh[j] * 4);
+        o_rec[j] = take((size_t)ldh[j] * 48); o_box[j] = take((size_t)nb * 32);
+    }
+    cudaError_t e = cudaStreamSynchronize(stream);       // the staging buffers may still serve the previous call
+    if (e != cudaSuccess) return e;
+    if ((e = hs.reserve(o)) != cudaSuccess) return e;
+    char* b = hs.buf;
+#define KF_TRY(x) do { e = (x); if (e != cudaSuccess) goto fail; } while (0)
+    // pools: copy stream, one event per layer
+    for (int j = 0; j < L; ++j) {
+        const size_t w = (size_t)io.n_hits[j] * 4;
+        if (io.n_hits[j] > 0) {
+            KF_TRY(cudaMemcpy2DAsync(b + o_pos[j], (size_t)ldh[j] * 4, io.pos[j], (size_t)io.ld_hits[j] * 4, w, 3, cudaMemcpyHostToDevice, hs.copy_stream));
+            KF_TRY(cudaMemcpy2DAsync(b + o_hcov[j], (size_t)ldh[j] * 4, io.cov_hits[j], (size_t)io.ld_hits[j] * 4, w, 6, cudaMemcpyHostToDevice, hs.copy_stream));
+        }
+        KF_TRY(cudaEventRecord(hs.ready[j], hs.copy_stream));
+    }
+    {
+        // candidates: compute stream (small), then layer by layer: wait for the pool, bin it, score it
+        const size_t w = (size_t)io.n * 4, cw = (size_t)ldc * 4;
+        KF_TRY(cudaMemcpy2DAsync(b + o_par, cw, io.par, (size_t)io.ld * 4, w, 6, cudaMemcpyHostToDevice, stream));
+        KF_TRY(cudaMemcpy2DAsync(b + o_cov, cw, io.cov, (size_t)io.ld * 4, w, 21, cudaMemcpyHostToDevice, stream));
+        KF_TRY(cudaMemcpyAsync(b + o_q, io.q, (size_t)io.n, cudaMemcpyHostToDevice, stream));
+        KF_TRY(cudaMemcpyAsync(b + o_chi2, io.chi2, w, cudaMemcpyHostToDevice, stream));
+        KF_TRY(cudaMemcpyAsync(b + o_nh, io.nhits, w, cudaMemcpyHostToDevice, stream));
+        KF_TRY(cudaMemcpyAsync(b + o_st, io.status, w, cudaMemcpyHostToDevice, stream));
+        KF_TRY(cudaMemsetAsync(b + o_ls + (size_t)29 * ldc * 4, 0, (size_t)ldc * 4, stream));   // local-state flags
+        for (int j = 0; j < L; ++j) {
+            KF_TRY(cudaStreamWaitEvent(stream, hs.ready[j], 0));
+            BinArgs ba;
+            ba.n_hits = io.n_hits[j]; ba.ld_in = ldh[j];
+            ba.pos = (const float*)(b + o_pos[j]); ba.cov = (const float*)(b + o_hcov[j]);
+            ba.radius = P.layer[io.first_layer + j].r; ba.n_eta = io.n_eta; ba.n_phi = io.n_phi; ba.eta_max = io.eta_max;
+            ba.ld_out = ldh[j]; ba.bin_offset = (int32_t*)(b + o_off[j]); ba.sorted_to_orig = (int32_t*)(b + o_s2o[j]);
+            ba.pos_sorted = nullptr; ba.cov_sorted = nullptr; ba.hit_rec = (float*)(b + o_rec[j]);
+            ba.bin_box = (float*)(b + o_box[j]); ba.orig_to_sorted = nullptr;
+            KF_TRY(launch_bin(bs, 1, &ba, stream, opt));
+            ScoreStep st;
+            st.layer = io.first_layer + j; st.n_hits = io.n_hits[j];
+            st.hit_rec = ba.hit_rec; st.bin_box = ba.bin_box; st.bin_offset = ba.bin_offset;
+            st.best_hit = (int32_t*)(b + o_idx) + (int64_t)j * ldc;
+            st.best_chi2 = (float*)(b + o_c2) + (int64_t)j * ldc;
+            ScoreArgs a;
+            memset(&a, 0, sizeof(a));
+            a.n = io.n; a.ld = ldc; a.par = (float*)(b + o_par); a.cov = (float*)(b + o_cov); a.q = (const int8_t*)(b + o_q);
+            a.chi2 = (float*)(b + o_chi2); a.nhits = (int32_t*)(b + o_nh); a.status = (uint32_t*)(b + o_st);
+            a.n_eta = io.n_eta; a.n_phi = io.n_phi; a.eta_max = io.eta_max;
+            a.window_half = io.window_half; a.chi2_cut = io.chi2_cut; a.do_update = io.do_update;
+            a.lstate = (float*)(b + o_ls); a.ld_ls = ldc;
+            KF_TRY(launch_build(ss, P, a, 1, &st, stream));
+        }
+        KF_TRY(cudaMemcpy2DAsync(io.par, (size_t)io.ld * 4, b + o_par, cw, w, 6, cudaMemcpyDeviceToHost, stream));
+        KF_TRY(cudaMemcpy2DAsync(io.cov, (size_t)io.ld * 4, b + o_cov, cw, w, 21, cudaMemcpyDeviceToHost, stream));
+        KF_TRY(cudaMemcpyAsync(io.chi2, b + o_chi2, w, cudaMemcpyDeviceToHost, stream));
+        KF_TRY(cudaMemcpyAsync(io.nhits, b + o_nh, w, cudaMemcpyDeviceToHost, stream));
+        KF_TRY(cudaMemcpyAsync(io.status, b + o_st, w, cudaMemcpyDeviceToHost, stream));
+        KF_TRY(cudaMemcpy2DAsync(io.hit_index, (size_t)io.ld_out * 4, b + o_idx, cw, w, (size_t)L, cudaMemcpyDeviceToHost, stream));
+        KF_TRY(cudaMemcpy2DAsync(io.hit_chi2, (size_t)io.ld_out * 4, b + o_c2, cw, w, (size_t)L, cudaMemcpyDeviceToHost, stream));
+    }
+#undef KF_TRY
+    e = cudaStreamSynchronize(stream);
+    {
+        cudaError_t e2 = cudaStreamSynchronize(hs.copy_stream);
+        if (e == cudaSuccess) e = e2;
+    }
+    return e;
+fail:
+    cudaStreamSynchronize(stream);
+    cudaStreamSynchronize(hs.copy_stream);
     return e;
 }
 

@@ -155,6 +155,19 @@ constexpr int kScorePlanes = 29;
 
 struct BinGrid { int n_eta, n_phi; float eta_max; };
 
+constexpr int kMaxBuildEvents = 32;
+
+// Several events in one building call ("concurrent events should be adapted to track building because
+// this will help to fill the GPU"): candidates of event e are first[e] .. first[e + 1] - 1 of the one candidate
+// array; every event has its own hit pools and bins.  n <= 1: the single-event pointers of ScoreArgs are used.
+struct EventPools {
+    int n;
+    int64_t first[kMaxBuildEvents + 1];
+    const float* hit_rec[kMaxBuildEvents];
+    const float* bin_box[kMaxBuildEvents];
+    const int32_t* bin_offset[kMaxBuildEvents];
+};
+
 struct ScoreArgs {
     int64_t n, ld;
     float* par; float* cov; const int8_t* q; float* chi2; int32_t* nhits; uint32_t* status;
@@ -172,6 +185,7 @@ struct ScoreArgs {
     float* scratch; float* track; int32_t* flag; int32_t* slot; int64_t ld_sc;
     // kf_score_candidates: the caller's local-frame candidate state [30][ld_ls] (null: none)
     float* lstate; int64_t ld_ls;
+    EventPools ev;           // kf_build_best_hit_events (ev.n > 1), set per step
 };
 
 struct ScoreStep {
@@ -182,6 +196,10 @@ struct ScoreStep {
     const int32_t* bin_offset;
     int32_t* best_hit;       // [n]
     float* best_chi2;        // [n]
+    // several events (n_events > 1): per-event pools of this step, in the order of EventPools::first
+    const float* ev_hit_rec[kMaxBuildEvents];
+    const float* ev_bin_box[kMaxBuildEvents];
+    const int32_t* ev_bin_offset[kMaxBuildEvents];
 };
 
 struct ScoreScratch {
@@ -219,6 +237,33 @@ struct CombScratch {
 // kf_comb.cu
 cudaError_t launch_comb(CombScratch& s, const FitParams& P, const CombCall& call, int n_steps, const ScoreStep* steps,
                         cudaStream_t stream);
+
+// ---------------------------------------------------------------------------------- host path of building
+// kf_build_best_hit_host: one event with every buffer in host memory.  Layer j's pool is copied on a second stream
+// while layer j - 1 is binned and scored (transfers are about half of the building wall time when they
+// are not overlapped).
+struct BuildHostIO {
+    int64_t n, ld;                         // candidates (HOST SoA, in/out)
+    float* par; float* cov; const int8_t* q; float* chi2; int32_t* nhits; uint32_t* status;
+    int first_layer, n_layers;
+    const int64_t* n_hits; const int64_t* ld_hits;             // [n_layers]
+    const float* const* pos; const float* const* cov_hits;     // [n_layers] HOST [3][ld], [6][ld]
+    int n_eta, n_phi; float eta_max; int window_half; float chi2_cut; int do_update;
+    int32_t* hit_index; float* hit_chi2; int64_t ld_out;       // HOST [n_layers][ld_out]
+};
+
+struct BuildHostStage {
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ready[32] = {};            // layer j's pool is on the device
+    cudaEvent_t done = nullptr;            // compute finished with the staging buffers of the previous call
+    char* buf = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t bytes);
+    void release();
+};
+
+cudaError_t build_best_hit_host(BuildHostStage& hs, BinScratch& bs, ScoreScratch& ss, const FitParams& P, const BuildHostIO& io,
+                                cudaStream_t stream, const LaunchOptions& opt);
 
 // kf_peak.cu
 double measure_fp32_peak(cudaStream_t stream, int repeats, float* sink);

@@ -55,6 +55,10 @@ struct LayerConst {
     float ln_t;      // ln t                (0 if t <= 0)
     // reading A21 (energy loss)
     float de0;       // K (Z/A) t X0 for silicon [GeV]: Bethe prefactor of the layer (0 if t <= 0 or option off)
+    // reading A23 (endcap discs)
+    int type;        // 0: barrel cylinder of radius r; 1: pair of discs in the planes z = +-zd
+    float zd;        // |z| of the disc pair
+    float rmin2, rmax2;  // squared bounds of the sensitive annulus
 };
 
 // Reading A21: particle-dependent constants of Bethe's formula, computed on the host in double.
@@ -71,7 +75,8 @@ struct FitParams {
     float inv_k0;  // 1 / (c_B * Bz)
     float mass2;   // mass^2
     int model;           // MODEL_* flags: reading A20 path-length material, reading A21 energy loss
-    int geometry_options;  // 1 if model != 0 or any layer has a finite half length
+    int geometry_options;  // 1 if model != 0, any layer has a finite half length, or there is a disc
+    int has_discs;         // 1 if any layer is a disc pair (reading A23)
     Bethe el;            // reading A21 constants (zero unless MODEL_ENERGY_LOSS)
     LayerConst layer[32];
 };
@@ -707,6 +712,174 @@ refit_step(TrackT<F>& t, arg<F> k, arg<F> ik, const LayerConst& L, const LayerCo
     const auto rc = kalman_update(t, o, n, h, dchi2);
     if (!is_zero(rc)) { t.c33 = k33; t.c35 = k35; t.c44 = k44; t.c55 = k55; }   // layer skipped
     return rc;
+}
+
+// ---- reading A23: endcap discs -------------------------------------------------------------------------------
+// Crossing of the helix with the plane z = zt (zt = +-L.zd on the side the track is heading to):
+//     theta = k (zt - z) / pz,   w' = w + (i pi / k)(E - 1),   pi' = pi E,   E = exp(-i theta).
+// In the local frame the Jacobian of that map is, over (a1, a2, z | b1, b2, c), with P = conj(e_r') e_a,
+// N = exp(i a')(S + i Cm)/k, exp(i a') = conj(e_r') e_l', T = pz/pT:
+//     row r'  = ( Re P, -Im P, -cos a'/T, Re N - cos a' theta/k, -Im N, -cos a' theta/(k T) )
+//     row t'  = ( Im P,  Re P, -sin a'/T, Im N - sin a' theta/k,  Re N, -sin a' theta/(k T) )
+//     row z'  = 0                      (the arrival point stays in the plane: the z row of C' is zero)
+//     row b1' = e_b1,   row b2' = e_b2 + (0, 0, k/T, theta, 0, theta/T),   row c' = e_c
+// (d theta = -(k/pz) dz - (theta/pz) d pz moves the arrival point along pi'/k and turns the momentum).
+struct DiscCrossing {
+    float xn, yn, zt, pxn, pyn;
+    float erx, ery, elx, ely;
+    float pc, ps, nr, nt, ca, sa;
+    float thk, theta, T, iT, pt2, ipt;
+};
+
+// Propagated covariance at a disc over (r', t' | b1, b2, c); its z row is zero.
+struct DiscCov {
+    float rr, rt, r3, r4, r5;
+    float tt, t3, t4, t5;
+    float n33, n34, n35, n44, n45, n55;
+};
+
+// Returns 0, ST_PROP_FAIL (plane behind the state, |pz| = 0, half a turn or more away) or ST_OUTSIDE.
+__device__ __forceinline__ uint32_t helix_to_plane(const Track& t, float k, float ik, const LayerConst& L, DiscCrossing& o) {
+    const float px = t.px, py = t.py, pz = t.pz;
+    const float zt = copysignf(L.zd, pz);
+    const float dz = zt - t.z;
+    const float pt2 = px * px + py * py;
+    const float theta = k * dz / pz;
+    // (NaNs fail every comparison)
+    if (!(dz * pz > 0.0f) || !(fabsf(theta) < 3.14159265f) || !(pt2 > 0.0f)) return ST_PROP_FAIL;
+    float sh, ch;
+    sincosf(0.5f * theta, &sh, &ch);
+    const float S = 2.0f * sh * ch, Cm = 2.0f * sh * sh, co = 1.0f - Cm;
+    o.theta = theta;
+    o.thk = theta * ik;
+    o.xn = t.x + (px * S + py * Cm) * ik;
+    o.yn = t.y + (py * S - px * Cm) * ik;
+    o.zt = zt;
+    o.pxn = px * co + py * S;
+    o.pyn = py * co - px * S;
+    const float rho2 = o.xn * o.xn + o.yn * o.yn;
+    if (!(rho2 >= L.rmin2 && rho2 <= L.rmax2)) return ST_OUTSIDE;
+    const float irho = rsqrt_fast(rho2), ipt = rsqrt_fast(pt2);
+    o.pt2 = pt2; o.ipt = ipt;
+    o.erx = o.xn * irho; o.ery = o.yn * irho;
+    o.elx = o.pxn * ipt; o.ely = o.pyn * ipt;
+    o.ca = o.erx * o.elx + o.ery * o.ely;
+    o.sa = o.erx * o.ely - o.ery * o.elx;
+    o.pc = o.erx * t.eax + o.ery * t.eay;
+    o.ps = o.erx * t.eay - o.ery * t.eax;
+    o.nr = (S * o.ca - Cm * o.sa) * ik;
+    o.nt = (S * o.sa + Cm * o.ca) * ik;
+    o.T = pz * ipt;
+    o.iT = pt2 * ipt / pz;
+    return 0u;
+}
+
+// C' = F~ C F~^T + Q~ for the to-plane map; the input covariance is general (21 elements).
+__device__ __forceinline__ void transport_cov_disc(const Track& t, const DiscCrossing& o, float k, float ms, float mass2,
+                                                   DiscCov& n) {
+    const float R[6] = {o.pc, -o.ps, -o.ca * o.iT, o.nr - o.ca * o.thk, -o.nt, -o.ca * o.thk * o.iT};
+    const float Tt[6] = {o.ps, o.pc, -o.sa * o.iT, o.nt - o.sa * o.thk, o.nr, -o.sa * o.thk * o.iT};
+    const float b2z = k * o.iT, b2b = o.theta, b2c = o.theta * o.iT;     // row b2' = e_b2 + (0, 0, b2z, b2b, 0, b2c)
+    const float C[6][6] = {{t.c00, t.c01, t.c02, t.c03, t.c04, t.c05}, {t.c01, t.c11, t.c12, t.c13, t.c14, t.c15},
+                           {t.c02, t.c12, t.c22, t.c23, t.c24, t.c25}, {t.c03, t.c13, t.c23, t.c33, t.c34, t.c35},
+                           {t.c04, t.c14, t.c24, t.c34, t.c44, t.c45}, {t.c05, t.c15, t.c25, t.c35, t.c45, t.c55}};
+    float u[6], v[6], w[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        u[i] = C[i][0] * R[0] + C[i][1] * R[1] + C[i][2] * R[2] + C[i][3] * R[3] + C[i][4] * R[4] + C[i][5] * R[5];
+        v[i] = C[i][0] * Tt[0] + C[i][1] * Tt[1] + C[i][2] * Tt[2] + C[i][3] * Tt[3] + C[i][4] * Tt[4] + C[i][5] * Tt[5];
+        w[i] = C[i][4] + C[i][2] * b2z + C[i][3] * b2b + C[i][5] * b2c;
+    }
+    auto dot6 = [](const float* a, const float* b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2] + a[3] * b[3] + a[4] * b[4] + a[5] * b[5]; };
+    auto dotB2 = [&](const float* a) { return a[4] + a[2] * b2z + a[3] * b2b + a[5] * b2c; };
+    // Highland (A5) at the propagated momentum, sheared to (b1, b2, c) as in transport_cov
+    const float pz = t.pz;
+    const float p2 = o.pt2 + pz * pz;
+    const float ip2 = rcp_fast(p2);
+    const float th2 = ms * (p2 + mass2) * ip2 * ip2;
+    const float qc = th2 * p2 * o.ipt;
+    n.rr = dot6(R, u); n.rt = dot6(Tt, u); n.tt = dot6(Tt, v);
+    n.r3 = u[3]; n.r4 = dotB2(u); n.r5 = u[5];
+    n.t3 = v[3]; n.t4 = dotB2(v); n.t5 = v[5];
+    n.n33 = t.c33 + th2 * pz * pz;
+    n.n34 = w[3];
+    n.n35 = t.c35 - qc * pz;
+    n.n44 = dotB2(w) + th2 * p2;
+    n.n45 = w[5];
+    n.n55 = t.c55 + qc * (p2 * o.ipt);
+}
+
+// Highland factor at a disc: flat, or (reading A20 on a disc) thickness / |cos| of the angle to the z axis = p / |pz|.
+__device__ __forceinline__ float ms_at_disc(const LayerConst& L, int model, const DiscCrossing& o, float pz) {
+    if ((model & MODEL_PATH_LENGTH) == 0) return L.ms;
+    const float f = sqrtf(o.pt2 + pz * pz) * rcp_fast(fabsf(pz));
+    const float lg = 1.0f + 0.038f * (L.ln_t + __logf(f));
+    return L.ms0 * f * lg * lg;
+}
+
+// Kalman update at a disc: C' has a zero z row, so the z component of S = C'_pp + V~ is eliminated first (Schur
+// complement on v_zz), leaving a 2-D measurement in (r, t) -- the disc's counterpart of kalman_update.
+__device__ __forceinline__ uint32_t kalman_update_disc(Track& t, const DiscCrossing& o, const DiscCov& n, const LocalHit& h,
+                                                       float* dchi2) {
+    const float iv = rcp_fast(h.vzz);
+    const float sa = h.vrz * iv, sb = h.vtz * iv;
+    const float qrr = h.vrr - sa * h.vrz, qrt = h.vrt - sa * h.vtz, qtt = h.vtt - sb * h.vtz;
+    const float srr = n.rr + qrr, srt = n.rt + qrt, stt = n.tt + qtt;
+    const float rr = h.rr - sa * h.rz, rt = h.rt - sb * h.rz;
+    const float det2 = srr * stt - srt * srt;
+    if (!(h.vzz * det2 > 0.0f)) return ST_S_NOT_PD;
+    const float id = rcp_fast(det2);
+    const float irr = stt * id, irt = -srt * id, itt = srr * id;
+    const float ur = irr * rr + irt * rt, ut = irt * rr + itt * rt;
+    const float chi2 = h.rz * h.rz * iv + rr * ur + rt * ut;
+    const float d0 = n.rr * ur + n.rt * ut;
+    const float d1 = n.rt * ur + n.tt * ut;
+    const float d3 = n.r3 * ur + n.t3 * ut;
+    const float d4 = n.r4 * ur + n.t4 * ut;
+    const float d5 = n.r5 * ur + n.t5 * ut;
+    const float probe = chi2 + ((d0 + d1) + (d3 + d4) + d5) * 0.0f;
+    if (!(fabsf(probe) < __int_as_float(0x7f800000))) return ST_NONFINITE;
+    *dchi2 = chi2;
+#define KF_KROW(cr, ct, kr, kt)          \
+    const float kr = cr * irr + ct * irt; \
+    const float kt = cr * irt + ct * itt;
+    KF_KROW(n.rr, n.rt, k0r, k0t)
+    KF_KROW(n.rt, n.tt, k1r, k1t)
+    KF_KROW(n.r3, n.t3, k3r, k3t)
+    KF_KROW(n.r4, n.t4, k4r, k4t)
+    KF_KROW(n.r5, n.t5, k5r, k5t)
+#undef KF_KROW
+    t.x = o.xn + o.erx * d0 - o.ery * d1;
+    t.y = o.yn + o.ery * d0 + o.erx * d1;
+    t.z = o.zt;
+    const float pxu = o.pxn + o.elx * d3 - o.ely * d4;
+    const float pyu = o.pyn + o.ely * d3 + o.elx * d4;
+    const float pzu = t.pz + d5 + o.T * d3;
+    t.px = pxu; t.py = pyu; t.pz = pzu;
+    t.eax = o.erx; t.eay = o.ery;
+    // position rows ("V form"), z row zero
+    t.c00 = k0r * qrr + k0t * qrt;
+    t.c01 = k0r * qrt + k0t * qtt;
+    t.c11 = k1r * qrt + k1t * qtt;
+    t.c02 = 0.0f; t.c12 = 0.0f; t.c22 = 0.0f; t.c23 = 0.0f; t.c24 = 0.0f; t.c25 = 0.0f;
+    t.c03 = k3r * qrr + k3t * qrt;
+    t.c13 = k3r * qrt + k3t * qtt;
+    t.c04 = k4r * qrr + k4t * qrt;
+    t.c14 = k4r * qrt + k4t * qtt;
+    t.c05 = k5r * qrr + k5t * qrt;
+    t.c15 = k5r * qrt + k5t * qtt;
+    // momentum block: C'_mm - K_m C'_pm
+    t.c33 = fmaf(-k3t, n.t3, fmaf(-k3r, n.r3, n.n33));
+    t.c34 = fmaf(-k3t, n.t4, fmaf(-k3r, n.r4, n.n34));
+    t.c35 = fmaf(-k3t, n.t5, fmaf(-k3r, n.r5, n.n35));
+    t.c44 = fmaf(-k4t, n.t4, fmaf(-k4r, n.r4, n.n44));
+    t.c45 = fmaf(-k4t, n.t5, fmaf(-k4r, n.r5, n.n45));
+    t.c55 = fmaf(-k5t, n.t5, fmaf(-k5r, n.r5, n.n55));
+    const float pt = o.pt2 * o.ipt;
+    const float ar = pt + d3;
+    const float iptn = rsqrt_fast(ar * ar + d4 * d4);
+    reaim_momentum<false>(t, ar * iptn, -d4 * iptn, o.T, pzu * iptn);
+    return 0u;
 }
 
 // Keep the propagated state (no hit used): position frame = arrival frame, momentum frame

@@ -111,6 +111,13 @@ __device__ __forceinline__ void get_track(const float* __restrict__ ts, int64_t 
 
 enum : int32_t { FLAG_IDLE = 0, FLAG_AT_LAYER = 1, FLAG_DEAD = 2 };
 
+// Event of candidate i when a call builds several events at once (EventPools); 0 otherwise.
+__device__ __forceinline__ int event_of(const EventPools& ev, int64_t i) {
+    int e = 0;
+    for (int k = 1; k < ev.n; ++k) e += i >= ev.first[k] ? 1 : 0;
+    return e;
+}
+
 __device__ __forceinline__ bool better(float c, int32_t h, float bc, int32_t bh) {
     return c < bc || (c == bc && h < bh);
 }

@@ -37,19 +37,20 @@ PROFILE_CSV = os.path.join(ROOT, "profiles", "r02_counters.csv")
 # ones of F and H and symmetry: propagation 75, Jacobian 95, F C F^T 340,
 # Q 35, update 310 (S 9, S^-1 30, chi2 21, K 90, x 36, C 126) -- frozen before any tuning.
 FLOPS_PER_TRACK_LAYER = 850
-# FP32 flops the pair kernel EXECUTES per track and layer, from the SASS opcode histogram of its ncu capture
-# (profiles/r02_fit_pair_kernel.md; 177 FFMA2 + 122 FMUL2 + 23 FADD2 per pair-layer in round 1 = 499 per track).
-EXECUTED_FLOPS_PER_TRACK_LAYER = 500
+# FP32 flops the pair kernel EXECUTES per track and layer: read from profiles/r02_fit_pair_opcodes.csv (10.83 Gflop per
+# 2 M-track launch = 542 per track and layer, once-per-track work included); this constant is only the fallback
+# when that file is absent.
+EXECUTED_FLOPS_PER_TRACK_LAYER = 542
 
 
 def _profile_counters() -> dict:
     """{kernel name fragment: {metric: value per launch}} from the committed raw ncu page (empty if absent)."""
     import csv
     want = {"dram__bytes_read.sum": "dram_read", "dram__bytes_write.sum": "dram_write",
-            "smsp__sass_thread_inst_executed_op_fadd_pred_on.sum": "fadd", "smsp__sass_thread_inst_executed_op_fmul_pred_on.sum": "fmul",
-            "smsp__sass_thread_inst_executed_op_ffma_pred_on.sum": "ffma",
-            "sm__sass_thread_inst_executed_op_fadd_pred_on.sum": "fadd", "sm__sass_thread_inst_executed_op_fmul_pred_on.sum": "fmul",
-            "sm__sass_thread_inst_executed_op_ffma_pred_on.sum": "ffma",
+            "smsp__sass_thread_inst_executed_op_fadd_pred_on.sum.per_cycle_elapsed": "fadd_per_cycle",
+            "smsp__sass_thread_inst_executed_op_fmul_pred_on.sum.per_cycle_elapsed": "fmul_per_cycle",
+            "smsp__sass_thread_inst_executed_op_ffma_pred_on.sum.per_cycle_elapsed": "ffma_per_cycle",
+            "smsp__warps_eligible.avg.per_cycle_active": "eligible_warps",
             "sm__warps_active.avg.pct_of_peak_sustained_active": "warps_active_pct",
             "gpu__time_duration.sum": "ncu_duration", "launch__registers_per_thread": "registers",
             "sm__inst_executed.sum": "warp_inst", "smsp__inst_executed.sum": "warp_inst",
@@ -65,7 +66,8 @@ def _profile_counters() -> dict:
         return out
     units = rows[rows.index(hdr) + 1]
     ki = hdr.index("Kernel Name")
-    scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "msecond": 1e-3, "usecond": 1e-6, "nsecond": 1e-9, "second": 1.0}
+    scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "msecond": 1e-3, "usecond": 1e-6, "nsecond": 1e-9, "second": 1.0,
+             "ms": 1e-3, "us": 1e-6, "ns": 1e-9, "s": 1.0}
     for r in rows[rows.index(hdr) + 2:]:
         if len(r) != len(hdr):
             continue
@@ -79,6 +81,19 @@ def _profile_counters() -> dict:
                 except ValueError:
                     pass
     return out
+
+
+def _opcode_flops(name: str) -> float | None:
+    """FP32 flops one launch executes, from the SASS opcode histogram of the same ncu capture
+    (profiles/<name>, written by `bench.py --opcode-table`): the TOTAL line."""
+    p = os.path.join(ROOT, "profiles", name)
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            if line.startswith("TOTAL,"):
+                return float(line.strip().split(",")[2])
+    return None
 
 
 def _kernel_counters(counters: dict, fragment: str) -> dict | None:
@@ -700,7 +715,8 @@ def run_ours(args) -> None:
               "dram_traffic_bytes": traffic, "fma_pipe_active_pct": kc.get("fma_pipe_pct"),
               "issue_slots_busy_pct": kc.get("issue_pct"), "warps_active_pct_of_peak": kc.get("warps_active_pct"),
               "registers_per_thread": kc.get("registers"),
-              "ncu_fp32_thread_inst": {k: kc.get(k) for k in ("fadd", "fmul", "ffma")},
+              "eligible_warps_per_scheduler": kc.get("eligible_warps"),
+              "ncu_fp32_thread_inst_per_cycle": {k: kc.get(k + "_per_cycle") for k in ("fadd", "fmul", "ffma")},
               "note": "ncu's fadd/fmul/ffma thread-instruction counters do not count the packed FFMA2 / FMUL2 / FADD2 "
                       "instructions this kernel is made of (they read ~0), so executed FP32 work is taken from the "
                       "SASS opcode histogram of the same capture (profiles/r02_fit_pair_kernel.md)"}
@@ -711,7 +727,10 @@ def run_ours(args) -> None:
         # track and layer, frozen before tuning) against the FP32 FMA peak measured on this GPU just now by the
         # library's own microbenchmark (self-measured: MEASURED_PEAKS.json has no FP32 entry).
         alg_flops = float(n) * FLOPS_PER_TRACK_LAYER * L
-        exe_flops = float(n) * EXECUTED_FLOPS_PER_TRACK_LAYER * L
+        # executed FP32 flops of one 2 M-track launch from the opcode histogram of the ncu capture, scaled to n
+        prof_flops = _opcode_flops("r02_fit_pair_opcodes.csv")
+        exe_per_fit = prof_flops / 2.0e6 if prof_flops else EXECUTED_FLOPS_PER_TRACK_LAYER * L
+        exe_flops = float(n) * exe_per_fit
         alu = {"bound": "alu", "kernel": "kf::fit_pair_kernel", "achieved": alg_flops / t_launch / 1e12, "peak": fp32_peak,
                "unit": "TFLOP/s", "frac": alg_flops / t_launch / 1e12 / fp32_peak, "traffic": traffic,
                "peak_source": "self-measured now: kf_measure_fp32_peak (register-only FMA chains); nominal 148 SM x 128 "
@@ -719,10 +738,11 @@ def run_ours(args) -> None:
                "flops_per_fit": FLOPS_PER_TRACK_LAYER * L, "label": "algorithmic (textbook count, the contract of SURVEY 8(d))",
                # what the implementation executes (local-frame filter): fewer flops than the textbook count, so ITS
                # floor is the HBM one; this fraction is the FP32 work really done over the same peak
-               "executed_flops_per_fit": EXECUTED_FLOPS_PER_TRACK_LAYER * L,
+               "executed_flops_per_fit": exe_per_fit,
                "executed_frac": exe_flops / t_launch / 1e12 / fp32_peak,
                "executed_source": "SASS opcode histogram of the ncu capture: FFMA2 = 4, FMUL2 / FADD2 = 2, FFMA = 2, "
-                                  "FMUL / FADD / MUFU = 1 flop per thread instruction (profiles/r02_fit_pair_kernel.md)"}
+                                  "FMUL / FADD / MUFU = 1 flop per thread instruction (profiles/r02_fit_pair_opcodes.csv, "
+                                  "profiles/r02_counters.md)"}
         # the binding roofline is the one with the larger lower bound on time under the frozen algorithmic counts
         # (SURVEY.md 8(d)); `implementation_floor` is the larger bound for the work this kernel really does.
         roofline, other = (alu, hbm) if alg_flops / (fp32_peak * 1e12) > alg_bytes / (peak * 1e9) else (hbm, alu)
@@ -755,12 +775,15 @@ def run_ours(args) -> None:
             # a hardware utilisation (it would exceed 1 with more pruning).  The hardware view of the scan kernel
             # is in `scan_kernel_hw` (ncu counters of one launch, profiles/r02_counters.csv).
             building["algorithmic_equivalent_alu_frac"] = building["algorithmic_gflop"] * 1e9 / (building["build_ms"] * 1e-3) / (fp32_peak * 1e12)
-            sc = _kernel_counters(counters, "scan_kernel") or {}
-            sc_flops = sc.get("fadd", 0.0) + sc.get("fmul", 0.0) + 2.0 * sc.get("ffma", 0.0) if sc else None
-            building["scan_kernel_hw"] = {"executed_fp32_flop_per_launch": sc_flops, "ncu_duration_s": sc.get("ncu_duration"),
-                                          "executed_alu_frac": (sc_flops / sc["ncu_duration"] / (fp32_peak * 1e12)) if sc and sc.get("ncu_duration") else None,
+            sc = _kernel_counters(counters, ">::scan_kernel") or {}
+            # FP32 thread instructions per elapsed cycle summed over the SM sub-partitions (ncu); peak = 148 x 128 per cycle
+            sc_pc = (sc.get("fadd_per_cycle", 0.0) + sc.get("fmul_per_cycle", 0.0) + sc.get("ffma_per_cycle", 0.0)) if sc else None
+            building["scan_kernel_hw"] = {"ncu_duration_s": sc.get("ncu_duration"),
+                                          "fp32_thread_inst_per_cycle": sc_pc,
+                                          "fp32_lane_utilisation": sc_pc / (148 * 128.0) if sc_pc is not None else None,
                                           "fma_pipe_active_pct": sc.get("fma_pipe_pct"), "issue_slots_busy_pct": sc.get("issue_pct"),
-                                          "warps_active_pct_of_peak": sc.get("warps_active_pct")}
+                                          "warps_active_pct_of_peak": sc.get("warps_active_pct"),
+                                          "eligible_warps_per_scheduler": sc.get("eligible_warps")}
             out["building"] = building
         if smoothing is not None:
             out["smoothing"] = smoothing

@@ -248,8 +248,9 @@ typedef struct {
 /* `out` receives the forward result exactly as kf_fit_tracks writes it (it equals the smoothed state at the
  * outermost used layer); `out` may alias `seeds`.  While the call runs, sm->par / sm->cov also hold its
  * intermediate per-layer states (no other scratch is used).  A backward step that fails sets
- * KF_STATUS_SMOOTH_FAIL in out->status (see there).  geom->energy_loss_model must be 0 (KF_ERR_UNSUPPORTED
- * otherwise); path-length material and finite barrels are honoured.  All pointers DEV.  Two kernels. */
+ * KF_STATUS_SMOOTH_FAIL in out->status (see there).  Path-length material, finite barrels and the energy-loss
+ * option are honoured (with energy loss the map between two layers is J F, reading A21: its Jacobian and its
+ * process noise J Q J^T enter the recursion).  All pointers DEV.  Two kernels. */
 KF_API int kf_fit_tracks_smooth(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                                 const kf_track_hits* hits, kf_tracks* out, kf_smoothed* sm);
 

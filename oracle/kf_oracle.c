@@ -6,7 +6,7 @@
  * (arXiv:1705.02876; "seeding, building, fitting" + chi2; PAPER.md:65 6x6 track /
  * 3x3 hit matrices in global coordinates; PAPER.md:71 projective bins; PAPER.md:73 best hit =
  * lowest chi2 increment; equations: BASELINE.json:north_star).  The paper prints no formulas;
- * every formula below is a reading listed in DESIGN.md ("Readings A1..A21").
+ * every formula below is a reading listed in DESIGN.md ("Readings A1..A23").
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load this.  It shares no code, header, table or constant with the CUDA path
@@ -19,7 +19,12 @@
  * worked value, P3 Jacobian vs finite differences / radial null / |p| conservation, P4 EKF ==
  * batch weighted least squares, P5 covariance PSD rank 5, P6 pulls and chi2/ndf, P7 Highland
  * check values, P8 window scoring == brute force, P9 bin structure, P10 rotation symmetry;
- * G1-G3 geometry options (tests/test_oracle_geometry.py); E1-E6 energy loss (tests/test_oracle_energy_loss.py).
+ * G1-G3 geometry options (tests/test_oracle_geometry.py); E1-E6 energy loss (tests/test_oracle_energy_loss.py);
+ * orc_chi2_increment against its definition and against orc_update (tests/test_oracle_scoring.py);
+ * SM1-SM5 the RTS smoother (tests/test_oracle_smoother.py: batch WLS at every layer, exact helix, pulls);
+ * R1-R5 the inward refit (tests/test_oracle_refit.py); C1-C4 combinatorial building;
+ * D1-D6 endcap discs (tests/test_oracle_endcap.py: to-plane propagation vs RK4 and vs the to-radius form,
+ * Jacobian, exact helix through barrels + discs, EKF == WLS, pulls).
  * Parity-unpinned: none of the functions below (efficiency / fake rate of PAPER.md:85 is not
  * computed here at all).
  */
@@ -770,14 +775,14 @@ void orc_fit_refit_one(int L, const double *radius, const double *xX0, double Bz
                         const double par[6], const double cov[36], int q, const double *hpos,
                         const double *hcov, uint32_t mask, double opar[6], double ocov[36], double *ochi2,
                         int32_t *onhits, uint32_t *ostatus, double spar[6], double scov[36], double *schi2,
-                        uint32_t *sstatus, double *trace_fwd, double *trace_bwd) {
+                        uint32_t *sstatus, int32_t *snhits, double *trace_fwd, double *trace_bwd) {
     double *tf = trace_fwd, *own = NULL;
     if (!tf) { own = (double *)calloc((size_t)L * ORC_TRACE_STRIDE, sizeof(double)); tf = own; } /* zeroed: fit_one writes no trace for a bad charge */
     fit_one(L, radius, xX0, Bz, mass, par, cov, q, hpos, hcov, mask, opar, ocov, ochi2, onhits, ostatus, tf);
     uint32_t used = 0;
     for (int l = 0; l < L; ++l)
         if (tf[(size_t)l * ORC_TRACE_STRIDE + 121] != 0.0) used |= 1u << l;
-    int32_t nb;
+    int32_t nb = 0;
     if (used == 0) { /* nothing fitted: the input comes back */
         memcpy(spar, opar, 6 * sizeof(double));
         memcpy(scov, ocov, 36 * sizeof(double));
@@ -787,6 +792,7 @@ void orc_fit_refit_one(int L, const double *radius, const double *xX0, double Bz
         refit_inward_one(L, radius, xX0, Bz, mass, kappa, opar, ocov, q, hpos, hcov, used, spar, scov, schi2, &nb,
                          sstatus, trace_bwd);
     }
+    if (snhits) *snhits = nb; /* hits the backward pass used */
     if (own) free(own);
 }
 
@@ -795,12 +801,13 @@ void orc_fit_refit_tracks(int64_t n, int L, const double *radius, const double *
                            double kappa, const double *par, const double *cov, const int8_t *q,
                            const double *hpos, const double *hcov, const uint32_t *mask, double *opar,
                            double *ocov, double *ochi2, int32_t *onhits, uint32_t *ostatus, double *spar,
-                           double *scov, double *schi2, uint32_t *sstatus, double *trace_fwd, double *trace_bwd) {
+                           double *scov, double *schi2, uint32_t *sstatus, int32_t *snhits, double *trace_fwd,
+                           double *trace_bwd) {
     for (int64_t i = 0; i < n; ++i)
         orc_fit_refit_one(L, radius, xX0, Bz, mass, kappa, par + 6 * i, cov + 36 * i, q[i],
                            hpos + (size_t)i * L * 3, hcov + (size_t)i * L * 9, mask ? mask[i] : 0xffffffffu,
                            opar + 6 * i, ocov + 36 * i, ochi2 + i, onhits + i, ostatus + i, spar + 6 * i,
-                           scov + 36 * i, schi2 + i, sstatus + i,
+                           scov + 36 * i, schi2 + i, sstatus + i, snhits ? snhits + i : NULL,
                            trace_fwd ? trace_fwd + (size_t)i * L * ORC_TRACE_STRIDE : NULL,
                            trace_bwd ? trace_bwd + (size_t)i * L * ORC_TRACE_STRIDE : NULL);
 }

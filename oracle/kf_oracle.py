@@ -323,14 +323,16 @@ def fit_refit_tracks(radius, x_over_X0, Bz, mass, par, cov21, q, hpos, hcov, mas
     opar = np.zeros((n, 6)); ocov = np.zeros((n, 6, 6)); ochi2 = np.zeros(n)
     onh = np.zeros(n, dtype=np.int32); ost = np.zeros(n, dtype=np.uint32)
     spar = np.zeros((n, 6)); scov = np.zeros((n, 6, 6)); schi2 = np.zeros(n); sst = np.zeros(n, dtype=np.uint32)
+    snh = np.zeros(n, dtype=np.int32)
     tf = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
     tb = np.zeros((n, L, TRACE_STRIDE)) if want_trace else None
     lib().orc_fit_refit_tracks(C.c_int64(n), C.c_int(L), _p(rad), _p(xx0), C.c_double(Bz), C.c_double(mass),
                                 C.c_double(kappa), _p(par_a), _p(cov_a), _p(q_a, C.c_int8), _p(hp_a), _p(hc_a),
                                 _p(m_a, C.c_uint32), _p(opar), _p(ocov), _p(ochi2), _p(onh, C.c_int32),
-                                _p(ost, C.c_uint32), _p(spar), _p(scov), _p(schi2), _p(sst, C.c_uint32), _p(tf), _p(tb))
+                                _p(ost, C.c_uint32), _p(spar), _p(scov), _p(schi2), _p(sst, C.c_uint32), _p(snh, C.c_int32),
+                                _p(tf), _p(tb))
     out = dict(par=np.ascontiguousarray(opar.T), cov=ocov, chi2=ochi2, nhits=onh, status=ost,
-               rpar=np.ascontiguousarray(spar.T), rcov=scov, rchi2=schi2, rstatus=sst)
+               rpar=np.ascontiguousarray(spar.T), rcov=scov, rchi2=schi2, rstatus=sst, rnhits=snh)
     if want_trace:
         out["trace_fwd"], out["trace_bwd"] = tf, tb
     return out

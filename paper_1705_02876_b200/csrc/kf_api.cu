@@ -439,7 +439,6 @@ int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* se
     FitParams P;
     int rc = make_params(geom, &P);
     if (rc) return rc;
-    if (geom->energy_loss_model != 0) return KF_ERR_UNSUPPORTED;
     if ((rc = check_tracks(seeds, true, true))) return rc;
     if ((rc = check_tracks(out, false, true))) return rc;
     if (out->n != seeds->n || sm->n != seeds->n || sm->n_layers != geom->n_layers || sm->ld < sm->n) return KF_ERR_SHAPE;

@@ -20,7 +20,7 @@
 //    sum of positive semi-definite terms.  The textbook difference P + A (C^s_n - N) A^T cancels 3 - 4 digits on
 //    the inner layers, where the filtered momentum variance is the 30 % prior and the smoothed one is the full
 //    track's: measured in fp32 on config 3 it misses the 1e-3 covariance tolerance (1.7 x) at layer 0, the
-//    Joseph form stays at 0.09 x (profiles/r02_smoother.md).
+//    Joseph form stays at 0.09 x.
 //  * Frames: C^s_n is carried in the frame the filtered state of layer n was stored in (momentum axes aimed at
 //    the filtered momentum p^+_n); N comes out in the frame aimed at the propagated momentum p^-_n.  One
 //    reaim_momentum call takes C^s_n from the first to the second.
@@ -30,11 +30,17 @@
 namespace kf {
 
 // Symmetric 5 x 5 over (t, z, b1, b2, c) held as a full array (both triangles name the same values).
-struct Sym5 {
-    float m[5][5];
+// Written on the number type F like the filter (kf_math.cuh); the library instantiates F = float only (the packed
+// two-tracks-per-thread form, F = f2, gave identical results but ran slower: see kf_smooth.cu).
+template <class F>
+struct Sym5T {
+    F m[5][5];
 };
+using Sym5 = Sym5T<float>;
+using Sym5x2 = Sym5T<f2>;
 
-__device__ __forceinline__ void sym5_from_track(const Track& t, Sym5& P) {
+template <class F>
+__device__ __forceinline__ void sym5_from_track(const TrackT<F>& t, Sym5T<F>& P) {
     P.m[0][0] = t.c11; P.m[0][1] = P.m[1][0] = t.c12; P.m[0][2] = P.m[2][0] = t.c13;
     P.m[0][3] = P.m[3][0] = t.c14; P.m[0][4] = P.m[4][0] = t.c15;
     P.m[1][1] = t.c22; P.m[1][2] = P.m[2][1] = t.c23; P.m[1][3] = P.m[3][1] = t.c24; P.m[1][4] = P.m[4][1] = t.c25;
@@ -43,8 +49,9 @@ __device__ __forceinline__ void sym5_from_track(const Track& t, Sym5& P) {
     P.m[4][4] = t.c55;
 }
 
-__device__ __forceinline__ void track_from_sym5(const Sym5& P, Track& t) {
-    t.c00 = 0.0f; t.c01 = 0.0f; t.c02 = 0.0f; t.c03 = 0.0f; t.c04 = 0.0f; t.c05 = 0.0f;
+template <class F>
+__device__ __forceinline__ void track_from_sym5(const Sym5T<F>& P, TrackT<F>& t) {
+    t.c00 = F(0.0f); t.c01 = F(0.0f); t.c02 = F(0.0f); t.c03 = F(0.0f); t.c04 = F(0.0f); t.c05 = F(0.0f);
     t.c11 = P.m[0][0]; t.c12 = P.m[0][1]; t.c13 = P.m[0][2]; t.c14 = P.m[0][3]; t.c15 = P.m[0][4];
     t.c22 = P.m[1][1]; t.c23 = P.m[1][2]; t.c24 = P.m[1][3]; t.c25 = P.m[1][4];
     t.c33 = P.m[2][2]; t.c34 = P.m[2][3]; t.c35 = P.m[2][4];
@@ -53,30 +60,40 @@ __device__ __forceinline__ void track_from_sym5(const Sym5& P, Track& t) {
 }
 
 // The smoothed state of the layer further out, as the recursion carries it.
-struct SmoothedNext {
-    float x, y, z, px, py, pz;   // x^s_n (global coordinates)
-    float fpx, fpy, fpz;         // p^+_n: the filtered momentum of layer n = the aim of the frame Cs is held in
-    Sym5 Cs;                     // C^s_n in the frame layer n was stored in
+template <class F>
+struct SmoothedNextT {
+    F x, y, z, px, py, pz;   // x^s_n (global coordinates)
+    F fpx, fpy, fpz;         // p^+_n: the filtered momentum of layer n = the aim of the frame Cs is held in
+    Sym5T<F> Cs;             // C^s_n in the frame layer n was stored in
+};
+using SmoothedNext = SmoothedNextT<float>;
+
+template <class F>
+struct SmoothedStateT {
+    F x, y, z, px, py, pz;
 };
 
 // One backward step: t = filtered state of layer k in its local frame (radial row zero), Ln = constants of the
-// next used layer n, nx = smoothed state of n.  On success returns 0, x^s_k in (sx, sy, sz, spx, spy, spz) and
-// C^s_k in Cs_out (frame of t).  On failure (the crossing cannot be recomputed, N not positive definite, a
-// non-finite result) returns the status bit and writes nothing.
-__device__ __forceinline__ uint32_t rts_step(const Track& t, float k, float ik, const LayerConst& Ln, int model,
-                                             float mass2, const SmoothedNext& nx, float& sx, float& sy, float& sz,
-                                             float& spx, float& spy, float& spz, Sym5& Cs_out) {
-    Crossing o;
-    if (!helix_to_radius(t, k, ik, Ln, o)) return ST_PROP_FAIL;
-    const float ms = ms_at_crossing(Ln, model, o, t.pz);
+// next used layer n, nx = smoothed state of n.  On success returns 0, x^s_k in `s` and C^s_k in Cs_out (frame of
+// t).  On failure (the crossing cannot be recomputed, N not positive definite, a non-finite result) returns the
+// status bit(s) and writes nothing.  Pair form: both tracks take the step or neither does.
+template <class F, bool ELOSS = false>
+__device__ __forceinline__ typename num_traits<F>::status
+rts_step(const TrackT<F>& t, arg<F> k, arg<F> ik, const LayerConst& Ln, int model, float mass2, const Bethe& el,
+         const SmoothedNextT<F>& nx, SmoothedStateT<F>& s, Sym5T<F>& Cs_out) {
+    using M_ = typename num_traits<F>::mask;
+    CrossingT<F> o;
+    const M_ reached = helix_to_radius(t, k, ik, Ln, o);
+    if (!all_of(reached)) return select_u(reached, 0u, ST_PROP_FAIL);
+    const F ms = ms_at_crossing(Ln, model, o, t.pz);
     // local Jacobian rows over (a2, z, b1, b2, c) of layer k  (kf_math.cuh: row t', row z', row b2')
-    const float t1 = o.t1, t3 = o.t3, t4 = o.t4;
-    const float z1 = o.z1, z3 = o.z3, z4 = o.z4, thk = o.thk;
-    const float h1 = o.mu * o.g1, h3 = o.mu * o.g3, h4 = o.mu * o.g4;   // row b2' = e_b2 + (h1, 0, h3, h4, 0)
-    Sym5 P;
+    const F t1 = o.t1, t3 = o.t3, t4 = o.t4;
+    const F z1 = o.z1, z3 = o.z3, z4 = o.z4, thk = o.thk;
+    const F h1 = o.mu * o.g1, h3 = o.mu * o.g3, h4 = o.mu * o.g4;   // row b2' = e_b2 + (h1, 0, h3, h4, 0)
+    Sym5T<F> P;
     sym5_from_track(t, P);
     // M = P F~^T (5 x 5)
-    float M[5][5];
+    F M[5][5];
 #pragma unroll
     for (int i = 0; i < 5; ++i) {
         M[i][0] = P.m[i][0] * t1 + P.m[i][2] * t3 + P.m[i][3] * t4;
@@ -86,14 +103,14 @@ __device__ __forceinline__ uint32_t rts_step(const Track& t, float k, float ik, 
         M[i][4] = P.m[i][4];
     }
     // Highland process noise Q~ of layer n at the propagated momentum (same expression as transport_cov)
-    const float pz = t.pz;
-    const float p2 = o.pt2 + pz * pz;
-    const float ip2 = rcp_fast(p2);
-    const float th2 = ms * (p2 + mass2) * ip2 * ip2;
-    const float qc = th2 * p2 * o.ipt;
-    const float q22 = th2 * pz * pz, q24 = -qc * pz, q33 = th2 * p2, q44 = qc * (p2 * o.ipt);
-    // N = F~ M + Q~ (upper triangle, then mirrored)
-    float N[5][5];
+    const F pz = t.pz;
+    const F p2 = o.pt2 + pz * pz;
+    const F ip2 = rcp_fast(p2);
+    const F th2 = ms * (p2 + mass2) * ip2 * ip2;
+    const F qc = th2 * p2 * o.ipt;
+    const F q22 = th2 * pz * pz, q24 = -(qc * pz), q33 = th2 * p2, q44 = qc * (p2 * o.ipt);
+    // N = F~ M + Q~
+    F N[5][5];
 #pragma unroll
     for (int b = 0; b < 5; ++b) {
         N[0][b] = t1 * M[0][b] + t3 * M[2][b] + t4 * M[3][b];
@@ -103,86 +120,116 @@ __device__ __forceinline__ uint32_t rts_step(const Track& t, float k, float ik, 
         N[4][b] = M[4][b];
     }
     N[2][2] += q22; N[2][4] += q24; N[4][2] += q24; N[3][3] += q33; N[4][4] += q44;
-    // N = L D L^T (unit lower L), symmetrised from the upper triangle
-    float Lm[5][5], d[5], id[5];
-    bool pd = true;
+    // Process noise of the whole map k -> n as the recursion needs it again below (Joseph form): Q~, or J Q~ J^T
+    // with the energy loss of reading A21
+    F y22 = q22, y24 = q24, y33 = q33, y44 = q44;
+    F lf(1.0f), lg(1.0f), lh(0.0f);          // J = [[g, 0, h], [0, f, 0], [0, 0, f]] on (b1, b2, c); identity without the option
+    if constexpr (ELOSS && std::is_same<F, float>::value) {   // (compiled out of the kernel for geometries without the option)
+        if (model & MODEL_ENERGY_LOSS) {
+            // Reading A21: on arrival, after C' = F~ P F~^T + Q~, the momentum is scaled by f (direction kept) and the
+            // covariance goes through J.  The map k -> n is then J F~: M -> M J^T, N -> J N J^T, Q~ -> J Q~ J^T.
+            Eloss e;
+            if (!energy_loss_factors(el, Ln, model, mass2, o.erx * o.elx + o.ery * o.ely, o.pt2, o.ipt, pz, false, e))
+                return ST_PROP_FAIL;
+            lf = e.f; lg = e.g; lh = e.h;
+#pragma unroll
+            for (int i = 0; i < 5; ++i) {      // columns (b1, b2, c) of M and of N
+                M[i][2] = lg * M[i][2] + lh * M[i][4]; M[i][3] = lf * M[i][3]; M[i][4] = lf * M[i][4];
+                N[i][2] = lg * N[i][2] + lh * N[i][4]; N[i][3] = lf * N[i][3]; N[i][4] = lf * N[i][4];
+            }
+#pragma unroll
+            for (int b = 0; b < 5; ++b) {      // rows of N
+                N[2][b] = lg * N[2][b] + lh * N[4][b]; N[3][b] = lf * N[3][b]; N[4][b] = lf * N[4][b];
+            }
+            const float a0 = lg * q22 + lh * q24, a2 = lg * q24 + lh * q44;     // row b1 of J Q~
+            y22 = lg * a0 + lh * a2;
+            y24 = lf * a2;
+            y33 = lf * lf * q33;
+            y44 = lf * lf * q44;
+        }
+    }
+    // N = L D L^T (unit lower L), from the upper triangle
+    F Lm[5][5], d[5], id[5];
+    M_ pd = reached;
 #pragma unroll
     for (int j = 0; j < 5; ++j) {
-        float dj = N[j][j];
+        F dj = N[j][j];
 #pragma unroll
-        for (int s = 0; s < j; ++s) dj -= Lm[j][s] * Lm[j][s] * d[s];
+        for (int r = 0; r < j; ++r) dj -= (Lm[j][r] * Lm[j][r]) * d[r];
         d[j] = dj;
-        pd = pd && (dj > 0.0f);
+        pd = pd & (dj > 0.0f);
         id[j] = rcp_fast(dj);
 #pragma unroll
         for (int i = j + 1; i < 5; ++i) {
-            float v = N[j][i];
+            F v = N[j][i];
 #pragma unroll
-            for (int s = 0; s < j; ++s) v -= Lm[i][s] * Lm[j][s] * d[s];
+            for (int r = 0; r < j; ++r) v -= (Lm[i][r] * Lm[j][r]) * d[r];
             Lm[i][j] = v * id[j];
         }
     }
-    if (!pd) return ST_S_NOT_PD;
+    if (!all_of(pd)) return select_u(pd, 0u, ST_S_NOT_PD);
     // A = M N^-1, row by row:  L y = m,  z = y / d,  L^T a = z
-    float A[5][5];
+    F A[5][5];
 #pragma unroll
     for (int i = 0; i < 5; ++i) {
-        float y[5];
+        F y[5];
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
-            float v = M[i][j];
+            F v = M[i][j];
 #pragma unroll
-            for (int s = 0; s < j; ++s) v -= Lm[j][s] * y[s];
+            for (int r = 0; r < j; ++r) v -= Lm[j][r] * y[r];
             y[j] = v;
         }
 #pragma unroll
         for (int j = 4; j >= 0; --j) {
-            float v = y[j] * id[j];
+            F v = y[j] * id[j];
 #pragma unroll
-            for (int s = j + 1; s < 5; ++s) v -= Lm[s][j] * A[i][s];
+            for (int r = j + 1; r < 5; ++r) v -= Lm[r][j] * A[i][r];
             A[i][j] = v;
         }
     }
     // x^s_n - x^-_n in the arrival frame of n (radial component dropped: second order, null direction of N)
-    const float dx = nx.x - o.xn, dy = nx.y - o.yn;
-    const float dpx = nx.px - o.pxn, dpy = nx.py - o.pyn;
-    float D[5];
+    const F dx = nx.x - o.xn, dy = nx.y - o.yn;
+    const F dpx = nx.px - lf * o.pxn, dpy = nx.py - lf * o.pyn;
+    F D[5];
     D[0] = o.erx * dy - o.ery * dx;
     D[1] = nx.z - o.zn;
     D[2] = o.elx * dpx + o.ely * dpy;
     D[3] = o.elx * dpy - o.ely * dpx;
-    D[4] = (nx.pz - pz) - o.T * D[2];
-    float dl[5];
+    D[4] = (nx.pz - lf * pz) - o.T * D[2];
+    F dl[5];
 #pragma unroll
     for (int i = 0; i < 5; ++i) dl[i] = A[i][0] * D[0] + A[i][1] * D[1] + A[i][2] * D[2] + A[i][3] * D[3] + A[i][4] * D[4];
     // C^s_n from the frame aimed at p^+_n to the frame aimed at p^-_n
-    Track w;
+    TrackT<F> w;
     track_from_sym5(nx.Cs, w);
     {
-        const float ipf = rsqrt_fast(nx.fpx * nx.fpx + nx.fpy * nx.fpy);
-        const float fx = nx.fpx * ipf, fy = nx.fpy * ipf;
+        const F ipf = rsqrt_fast(nx.fpx * nx.fpx + nx.fpy * nx.fpy);
+        const F fx = nx.fpx * ipf, fy = nx.fpy * ipf;
         reaim_momentum<true>(w, o.elx * fx + o.ely * fy, o.elx * fy - o.ely * fx, nx.fpz * ipf, o.T);
     }
-    Sym5 Y;
+    Sym5T<F> Y;
     sym5_from_track(w, Y);
-    Y.m[2][2] += q22; Y.m[2][4] += q24; Y.m[4][2] += q24; Y.m[3][3] += q33; Y.m[4][4] += q44;
-    // B = I - A F~
-    float B[5][5];
+    Y.m[2][2] += y22; Y.m[2][4] += y24; Y.m[4][2] += y24; Y.m[3][3] += y33; Y.m[4][4] += y44;
+    // B = I - A (J F~) = I - (A J) F~
+    F B[5][5];
 #pragma unroll
     for (int i = 0; i < 5; ++i) {
-        B[i][0] = -(A[i][0] * t1 + A[i][1] * z1 + A[i][3] * h1);
-        B[i][1] = -A[i][1];
-        B[i][2] = -(A[i][0] * t3 + A[i][1] * z3 + A[i][2] + A[i][3] * h3);
-        B[i][3] = -(A[i][0] * t4 + A[i][1] * z4 + A[i][3] + A[i][3] * h4);
-        B[i][4] = -(A[i][1] * thk + A[i][4]);
+        const F a0 = A[i][0], a1 = A[i][1];
+        const F a2 = A[i][2] * lg, a3 = A[i][3] * lf, a4 = A[i][2] * lh + A[i][4] * lf;    // row i of A J
+        B[i][0] = -(a0 * t1 + a1 * z1 + a3 * h1);
+        B[i][1] = -a1;
+        B[i][2] = -(a0 * t3 + a1 * z3 + a2 + a3 * h3);
+        B[i][3] = -(a0 * t4 + a1 * z4 + a3 + a3 * h4);
+        B[i][4] = -(a1 * thk + a4);
         B[i][i] += 1.0f;
     }
     // C^s_k = B P B^T + A Y A^T (upper triangle)
-    float probe = 0.0f;
-    Sym5 C;
+    F probe(0.0f);
+    Sym5T<F> C;
 #pragma unroll
     for (int i = 0; i < 5; ++i) {
-        float u[5], v[5];
+        F u[5], v[5];
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
             u[j] = B[i][0] * P.m[0][j] + B[i][1] * P.m[1][j] + B[i][2] * P.m[2][j] + B[i][3] * P.m[3][j] + B[i][4] * P.m[4][j];
@@ -190,31 +237,33 @@ __device__ __forceinline__ uint32_t rts_step(const Track& t, float k, float ik, 
         }
 #pragma unroll
         for (int j = i; j < 5; ++j) {
-            const float c = (u[0] * B[j][0] + u[1] * B[j][1] + u[2] * B[j][2] + u[3] * B[j][3] + u[4] * B[j][4]) +
-                            (v[0] * A[j][0] + v[1] * A[j][1] + v[2] * A[j][2] + v[3] * A[j][3] + v[4] * A[j][4]);
+            const F c = (u[0] * B[j][0] + u[1] * B[j][1] + u[2] * B[j][2] + u[3] * B[j][3] + u[4] * B[j][4]) +
+                        (v[0] * A[j][0] + v[1] * A[j][1] + v[2] * A[j][2] + v[3] * A[j][3] + v[4] * A[j][4]);
             C.m[i][j] = c;
             C.m[j][i] = c;
             probe += c * 0.0f;
         }
     }
     probe += (dl[0] + dl[1] + dl[2] + dl[3] + dl[4]) * 0.0f;
-    if (!(fabsf(probe) < __int_as_float(0x7f800000))) return ST_NONFINITE;
+    const M_ fin = abs_(probe) < __int_as_float(0x7f800000);
+    if (!all_of(fin)) return select_u(fin, 0u, ST_NONFINITE);
     // x^s_k = x^+_k + A (...) in the frame of layer k
-    const float iptk = rsqrt_fast(t.px * t.px + t.py * t.py);
-    const float lx = t.px * iptk, ly = t.py * iptk, Tk = t.pz * iptk;
-    sx = t.x - t.eay * dl[0];
-    sy = t.y + t.eax * dl[0];
-    sz = t.z + dl[1];
-    spx = t.px + lx * dl[2] - ly * dl[3];
-    spy = t.py + ly * dl[2] + lx * dl[3];
-    spz = t.pz + dl[4] + Tk * dl[2];
+    const F iptk = rsqrt_fast(t.px * t.px + t.py * t.py);
+    const F lx = t.px * iptk, ly = t.py * iptk, Tk = t.pz * iptk;
+    s.x = t.x - t.eay * dl[0];
+    s.y = t.y + t.eax * dl[0];
+    s.z = t.z + dl[1];
+    s.px = t.px + lx * dl[2] - ly * dl[3];
+    s.py = t.py + ly * dl[2] + lx * dl[3];
+    s.pz = t.pz + dl[4] + Tk * dl[2];
     Cs_out = C;
-    return 0u;
+    return select_u(fin, 0u, 0u);
 }
 
 // A 5 x 5 covariance held in the frame of track `f` (position frame (eax, eay), momentum axes aimed at f's
 // momentum) -> the 21 packed elements in global coordinates, returned in g's covariance fields.
-__device__ __forceinline__ void sym5_to_global(const Sym5& C, const Track& f, Track& g) {
+template <class F>
+__device__ __forceinline__ void sym5_to_global(const Sym5T<F>& C, const TrackT<F>& f, TrackT<F>& g) {
     g = f;
     track_from_sym5(C, g);
     leave_local_frame(g);

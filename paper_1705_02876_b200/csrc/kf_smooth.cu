@@ -56,7 +56,36 @@ __device__ __forceinline__ void store_smoothed(const FitArgs& a, int l, int64_t 
     c[20 * ld] = g.c55;
 }
 
-__global__ void __launch_bounds__(kRtsBlock, 3)
+// One layer of one track: the RTS step from the smoothed state of layer l_next (or smoothed = filtered at the
+// outermost used layer and after a failure), conversion to global coordinates, store, and the state carried on.
+template <bool ELOSS>
+__device__ __forceinline__ void smooth_one_layer(const Track& t, float k, float ik, const FitParams& P, int model,
+                                                 const FitArgs& a, int l, int64_t i, SmoothedNext& nx, int& l_next,
+                                                 bool& broken) {
+    SmoothedStateT<float> s = {t.x, t.y, t.z, t.px, t.py, t.pz};
+    Sym5 Cs;
+    sym5_from_track(t, Cs);
+    if (l_next >= 0 && !broken) {
+        const uint32_t rc = rts_step<float, ELOSS>(t, k, ik, P.layer[l_next], model, P.mass2, P.el, nx, s, Cs);
+        if (rc != 0u) {              // cannot happen on a well-posed fit; the layers further in keep the filtered state
+            broken = true;
+            a.status[i] |= ST_SMOOTH_FAIL;
+        }
+    }
+    Track g;
+    sym5_to_global(Cs, t, g);
+    store_smoothed(a, l, i, s.x, s.y, s.z, s.px, s.py, s.pz, g);
+    nx.x = s.x; nx.y = s.y; nx.z = s.z; nx.px = s.px; nx.py = s.py; nx.pz = s.pz;
+    nx.fpx = t.px; nx.fpy = t.py; nx.fpz = t.pz;
+    nx.Cs = Cs;
+    l_next = l;
+}
+
+#ifndef KF_RTS_MIN_BLOCKS
+#define KF_RTS_MIN_BLOCKS 3
+#endif
+template <bool ELOSS>
+__global__ void __launch_bounds__(kRtsBlock, KF_RTS_MIN_BLOCKS)
 rts_kernel(const __grid_constant__ FitParams P, const __grid_constant__ RtsMaps M, const FitArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -105,25 +134,15 @@ rts_kernel(const __grid_constant__ FitParams P, const __grid_constant__ RtsMaps 
         __syncwarp();   // every lane holds its values: the stage can be refilled
         if (step + kRtsStages < L && elect_one()) request(step + kRtsStages);
         if (!((used >> l) & 1u)) continue;
-        float sx = t.x, sy = t.y, sz = t.z, spx = t.px, spy = t.py, spz = t.pz;
-        Sym5 Cs;
-        sym5_from_track(t, Cs);          // outermost used layer (or after a failure): smoothed = filtered
-        if (l_next >= 0 && !broken) {
-            const uint32_t rc = rts_step(t, k, ik, P.layer[l_next], model, P.mass2, nx, sx, sy, sz, spx, spy, spz, Cs);
-            if (rc != 0u) {              // cannot happen on a well-posed fit; the layers further in keep the filtered state
-                broken = true;
-                a.status[i] |= ST_SMOOTH_FAIL;
-            }
-        }
-        Track g;
-        sym5_to_global(Cs, t, g);
-        store_smoothed(a, l, i, sx, sy, sz, spx, spy, spz, g);
-        nx.x = sx; nx.y = sy; nx.z = sz; nx.px = spx; nx.py = spy; nx.pz = spz;
-        nx.fpx = t.px; nx.fpy = t.py; nx.fpz = t.pz;
-        nx.Cs = Cs;
-        l_next = l;
+        smooth_one_layer<ELOSS>(t, k, ik, P, model, a, l, i, nx, l_next, broken);
     }
 }
+
+// (A two-tracks-per-thread form of this kernel -- rts_step is written on the number type F like the filter -- was
+// built and measured in round 2: 221 registers without spills, 9 resident warps per SM, results identical, but
+// 1.61 ms per 2 M tracks for fit + smoother against 1.38 ms with this one-track kernel: the LDL^T factorisation and
+// the row solves are long dependent chains, and with 2.25 warps per scheduler their latency is no longer hidden.
+// It was removed again; profiles/r02_counters.md has the numbers.)
 
 cudaError_t ensure_rts_attributes() {
     return cudaSuccess;   // 23.6 KB of dynamic shared memory: below the 48 KB that needs no opt-in
@@ -138,7 +157,8 @@ cudaError_t launch_rts(const FitParams& P, const FitArgs& a, cudaStream_t stream
     if (!make_map(&M.par, a.lpar, a.n, a.ld_l, (int64_t)L * 6, 6) || !make_map(&M.cov, a.lcov, a.n, a.ld_l, (int64_t)L * 21, 17))
         return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kRtsBlock - 1) / kRtsBlock;
-    rts_kernel<<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
+    if (P.model & MODEL_ENERGY_LOSS) rts_kernel<true><<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
+    else rts_kernel<false><<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
     return cudaGetLastError();
 }
 

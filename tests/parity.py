@@ -33,7 +33,7 @@ def diverged_mask(oracle: dict) -> np.ndarray:
 
 def compare_fit(gpu: dict, oracle: dict, r_last: float | np.ndarray, max_diverged_frac: float = 1e-3,
                 loosen: dict | None = None, ill: np.ndarray | None = None, max_ill_frac: float = 0.0,
-                per_track: bool = False) -> dict:
+                per_track: bool = False, max_strict_fail_frac: float = 1e-2) -> dict:
     """gpu: par[6][n] f32, cov[21][n] f32, chi2[n], nhits[n], status[n]; oracle: O.fit_tracks dict.
     Returns the worst normalised errors (each must be <= 1 to pass) and raises AssertionError on failure.
     `ill` (optional, bool[n]): tracks an ORACLE-SIDE rule identifies as ill-conditioned (stated by the caller,
@@ -59,8 +59,14 @@ def compare_fit(gpu: dict, oracle: dict, r_last: float | np.ndarray, max_diverge
                                 np.repeat(d[:, 3:].max(axis=1, keepdims=True), 3, 1)], axis=1))
     scale = s[:, :, None] * s[:, None, :]
     e_cov = (np.abs(gc - oc) / (TOL_COV * scale)).reshape(n, -1).max(axis=1)
-    dd = np.sqrt(np.clip(d, 1e-300, None))
-    e_cov_strict = (np.abs(gc - oc) / (TOL_COV * dd[:, :, None] * dd[:, None, :])).reshape(n, -1).max(axis=1)
+    # stricter, element-wise: |dC_ij| <= 1e-3 sqrt(C_ii C_jj) -- on the elements where that scale means something:
+    # a covariance transported to a surface has NO variance along the surface normal, so for axis-aligned tracks
+    # (and for every track that ends on a disc: C_zz = 0) some C_ii are zero up to rounding and the ratio is
+    # undefined; elements whose scale is below 1e-2 of their blocks' scale are left to the block metric above
+    dd = np.sqrt(np.clip(d, 0.0, None))
+    sc_strict = dd[:, :, None] * dd[:, None, :]
+    defined = sc_strict >= 1e-2 * scale
+    e_cov_strict = np.where(defined, np.abs(gc - oc) / (TOL_COV * np.where(defined, sc_strict, 1.0)), 0.0).reshape(n, -1).max(axis=1)
     gchi = np.asarray(gpu["chi2"], dtype=np.float64)[:n]
     e_chi = np.abs(gchi - oracle["chi2"]) / (TOL_CHI2 * np.maximum(oracle["chi2"], 1.0))
     res = dict(n=n, n_diverged=int(bad.sum()),
@@ -72,6 +78,10 @@ def compare_fit(gpu: dict, oracle: dict, r_last: float | np.ndarray, max_diverge
                chi2_p99=float(np.percentile(e_chi[ok], 99)) if ok.any() else 0.0)
     assert np.array_equal(np.asarray(gpu["nhits"])[:n][ok], oracle["nhits"][ok]), "nhits differ"
     assert np.array_equal(np.asarray(gpu["status"])[:n][ok], oracle["status"][ok]), "status differ"
+    # the stricter element-wise metric |dC_ij| <= 1e-3 sqrt(C_ii C_jj) is ill-posed on the structurally null
+    # direction of axis-aligned tracks (A15), so it is not THE bound -- but the fraction of tracks missing it is held
+    assert res["cov_strict_fail_frac"] <= max_strict_fail_frac or loosen.get("cov", 1.0) > 1e6, \
+        f"{res['cov_strict_fail_frac']:.2e} of the tracks miss the element-wise covariance metric: {res}"
     errs = dict(pos=e_pos, mom=e_mom, cov=e_cov, chi2=e_chi)
     if per_track:
         res["per_track"] = dict(errs, ok=ok)

@@ -1,5 +1,5 @@
 """Pins of the oracle's inward propagation and backward refit / smoother (reading A18; CPU only).
-S1 inward propagation: inverse of the outward one, invariants, Jacobian vs finite differences.
+R1 (S1 in round 1) inward propagation: inverse of the outward one, invariants, Jacobian vs finite differences.
 S2 exact helix: the refit recovers the truth at the innermost layer with chi2 = 0.
 S3 backward EKF == batch weighted least squares of the affine model it linearises.
 S4 pulls at the innermost layer, chi2/ndf, and the smoothed errors are smaller than the forward-filtered ones there."""

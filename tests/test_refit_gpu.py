@@ -40,6 +40,7 @@ def _compare(d, o, r_last, max_div=1e-3, loosen=None, ill=None, max_ill_frac=0.0
     fwd = compare_fit(d.results(), {k: o[k] for k in ("par", "cov", "chi2", "nhits", "status")}, r_last, max_div)
     sg = d.refit_results()
     assert np.array_equal(sg["status"], o["rstatus"])
+    assert np.array_equal(sg["nhits"], o["rnhits"]), "hits used by the backward pass differ"
     # Smoothed result, same metric.  Excluded (A14): tracks the FORWARD fit flagged or that diverged there, and
     # tracks the backward pass flagged -- marked through the status word compare_fit looks at.
     ndf = np.maximum(2 * o["nhits"] - 5, 1)

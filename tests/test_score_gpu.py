@@ -249,12 +249,12 @@ def _score_event(ctx, ev, do_update=True, chi2_cut=30.0, check_state=True, keep_
         n_tie += int(diff.sum())
         alive &= ~diff                       # such a candidate is not compared further
         acc = alive & (orr["best_hit"] >= 0)
-        # chi2 of ONE hit: fp32 positions carry one or two ulp of r = 40 cm (4e-6 .. 8e-6 cm = up to 8e-4 sigma_rphi),
-        # so d(chi2) ~ 2 sqrt(chi2) * 8e-4: 1.6e-3 at chi2 = 1 (SURVEY hard part 3).  Bound: 2e-3 max(chi2, 1); the
-        # total chi2 of a track is held to north_star's 1e-3 below.
+        # chi2 of ONE hit, held to north_star's 1e-3 max(chi2, 1) like the total (fp32 positions carry one or two ulp
+        # of r = 40 cm = up to 8e-4 sigma_rphi, SURVEY hard part 3; worst seen over the 140 000 decisions of
+        # configs[4]: 5.5e-4)
         rel = np.abs(g["best_chi2"][acc] - b[acc]) / np.maximum(b[acc], 1.0)
         worst_chi2 = max(worst_chi2, rel.max(initial=0))
-        assert rel.max(initial=0) < 2e-3, rel.max()
+        assert rel.max(initial=0) < 1e-3, rel.max()
         assert np.array_equal(g["status"][alive], oc.status[alive])
         assert np.array_equal(g["nhits"][alive], oc.nhits[alive])
     if check_state:
@@ -306,7 +306,7 @@ def _build_event_fused(ctx, ev, use_order, half_length=None, material_model=0, e
         n_dec += int(alive.sum()); n_tie += int(diff.sum())
         alive &= ~diff
         acc = alive & (orr["best_hit"] >= 0)
-        assert (np.abs(c2[j][acc] - b[acc]) / np.maximum(b[acc], 1.0)).max(initial=0) < 2e-3
+        assert (np.abs(c2[j][acc] - b[acc]) / np.maximum(b[acc], 1.0)).max(initial=0) < 1e-3
     g = dc.results()
     # a candidate beyond the barrel end (reading A20) stops there with its last state: a valid result to compare
     sel = alive & ((oc.status & ~np.uint32(O.OUTSIDE)) == 0)

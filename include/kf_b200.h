@@ -64,8 +64,9 @@ enum {
                                 bins > KF_MAX_BINS, window wider than the phi ring                */
     KF_ERR_CUDA = -5,        /* a CUDA runtime call failed (kf_last_cuda_error has the code)      */
     KF_ERR_NOMEM = -6,       /* scratch allocation failed                                         */
-    KF_ERR_STALE = -7        /* kf_graph_launch: the graph's context is gone, or has reallocated scratch or
+    KF_ERR_STALE = -7,       /* kf_graph_launch: the graph's context is gone, or has reallocated scratch or
                                 changed the bin grid since the recording (record it again)          */
+    KF_ERR_TOO_LARGE = -8    /* kf_score_candidates_static: more than KF_STATIC_MAX_CANDIDATES candidates */
 };
 
 /* ---- per-track status bits (outputs) ---------------------------------------------------------- */
@@ -334,6 +335,27 @@ KF_API int kf_score_candidates(kf_ctx* ctx, const kf_geometry* geom, int layer, 
                                const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
                                float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
                                float* best_chi2, float* local_state);
+
+/* kf_score_candidates for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same kernels, same results, but the per-candidate scratch
+ * (the propagated candidate the scan reads, 31 floats per candidate) lives in ONE array compiled into the library,
+ * `static __device__` in kf_score.cu, instead of the context's cudaMalloc'ed scratch.  The call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine, at any size, first call included; it never touches the
+ * context's scratch (kf_graph_launch staleness is unaffected).
+ *   Limit:  cands->n <= KF_STATIC_MAX_CANDIDATES, else KF_ERR_TOO_LARGE and nothing is launched.  The array is
+ *           31 * KF_STATIC_MAX_CANDIDATES * 4 bytes = 7.75 MiB; every GPU that loads the library holds it until
+ *           the process exits, whether or not this call is used.
+ *   Shared: every call on a device, from every context and stream, uses the same array, and the array keeps the
+ *           last call's contents.  Nothing in it has to start at zero (every slot below cands->n is written before
+ *           it is read), so nothing is cleared.  Two calls that overlap on the GPU (different streams, or graph
+ *           branches) RACE on it: keep calls of this entry point on one device ordered.
+ *   Set-up: the first call on each device resolves the array's device address (cudaGetSymbolAddress, with that
+ *           device current; no stream work) and keeps it. */
+#define KF_STATIC_MAX_CANDIDATES 65536
+KF_API int kf_score_candidates_static(kf_ctx* ctx, const kf_geometry* geom, int layer, kf_tracks* cands,
+                                      const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                                      float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
+                                      float* best_chi2, float* local_state);
 
 /* Best-hit building over n_build_layers consecutive layers first_layer, first_layer+1, ... in one call
  * (PAPER.md:73, 133): per layer exactly what kf_score_candidates does, but the candidates stay in the

@@ -6,8 +6,8 @@ without the built library, or without a CUDA device, the calls raise.
 """
 from .binding import (KFContext, KFError, Bins, Geometry, Graph, abi_version, lib_path, load_library,
                       strerror, OPT_PAIR_MIN_TRACKS, OPT_REFIT_PAIR_MASKED, OPT_BIN_FORM, BIN_FORM_AUTO,
-                      BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED, STATUS_BAD_CHARGE, STATUS_NONFINITE, STATUS_OUTSIDE, STATUS_PROP_FAIL, STATUS_S_NOT_PD)
+                      BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED, STATIC_MAX_CANDIDATES, ERR_TOO_LARGE, STATUS_BAD_CHARGE, STATUS_NONFINITE, STATUS_OUTSIDE, STATUS_PROP_FAIL, STATUS_S_NOT_PD)
 
 __all__ = ["KFContext", "KFError", "Bins", "Geometry", "Graph", "abi_version", "lib_path", "load_library",
            "strerror", "OPT_PAIR_MIN_TRACKS", "OPT_REFIT_PAIR_MASKED", "OPT_BIN_FORM", "BIN_FORM_AUTO",
-           "BIN_FORM_FIVE_LAUNCH", "BIN_FORM_CHUNKED", "STATUS_BAD_CHARGE", "STATUS_NONFINITE", "STATUS_OUTSIDE", "STATUS_PROP_FAIL", "STATUS_S_NOT_PD"]
+           "BIN_FORM_FIVE_LAUNCH", "BIN_FORM_CHUNKED", "STATIC_MAX_CANDIDATES", "ERR_TOO_LARGE", "STATUS_BAD_CHARGE", "STATUS_NONFINITE", "STATUS_OUTSIDE", "STATUS_PROP_FAIL", "STATUS_S_NOT_PD"]

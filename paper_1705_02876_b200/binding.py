@@ -22,9 +22,11 @@ _LIB_PATH = os.environ.get("KF_B200_LIB") or os.path.join(_HERE, "libkf_b200.so"
 STATUS_PROP_FAIL, STATUS_S_NOT_PD, STATUS_NONFINITE, STATUS_BAD_CHARGE, STATUS_OUTSIDE = 1, 2, 4, 8, 16
 OPT_PAIR_MIN_TRACKS, OPT_REFIT_PAIR_MASKED, OPT_BIN_FORM = 1, 2, 3          # kf_set_option
 BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
+STATIC_MAX_CANDIDATES = 65536                                               # KF_STATIC_MAX_CANDIDATES
+ERR_TOO_LARGE = -8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
            "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
-           "kf_score_candidates", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial",
+           "kf_score_candidates", "kf_score_candidates_static", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
 
@@ -134,6 +136,8 @@ def load_library():
     lib.kf_score_candidates.restype = C.c_int
     lib.kf_score_candidates.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.POINTER(_Tracks), C.POINTER(_LayerHits),
                                         C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int, vp, vp, vp, vp]
+    lib.kf_score_candidates_static.restype = C.c_int
+    lib.kf_score_candidates_static.argtypes = lib.kf_score_candidates.argtypes
     lib.kf_build_best_hit.restype = C.c_int
     lib.kf_build_best_hit.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
                                       C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
@@ -454,19 +458,19 @@ class KFContext:
     # ------------------------------------------------------------------ kf_score_candidates
     def score_candidates(self, geom: Geometry, layer: int, n: int, par, cov, q, chi2, nhits, status,
                          n_hits: int, pos, cov_hits, bins: Bins, window_half: int, chi2_cut: float,
-                         do_update: bool, best_hit, best_chi2, order=None, local_state=None):
-        """local_state: optional float32 [30][ld] device tensor, zeroed before the first layer (see the header)."""
+                         do_update: bool, best_hit, best_chi2, order=None, local_state=None, static_scratch=False):
+        """local_state: optional float32 [30][ld] device tensor, zeroed before the first layer (see the header).
+        static_scratch: call kf_score_candidates_static (no allocation; n <= STATIC_MAX_CANDIDATES)."""
         g, keep = geom._c()
         cands = self._tracks(n, par, cov, q, chi2, nhits, status)
         lh = _LayerHits(int(n_hits), _plane_ld(pos, 3), pos.data_ptr(), cov_hits.data_ptr())
         lb = bins._c()
-        self._check(self._lib.kf_score_candidates(self._h, C.byref(g), int(layer), C.byref(cands), C.byref(lh),
-                                                  C.byref(lb), int(window_half), float(chi2_cut),
-                                                  1 if do_update else 0,
-                                                  order.data_ptr() if order is not None else None,
-                                                  best_hit.data_ptr(), best_chi2.data_ptr(),
-                                                  local_state.data_ptr() if local_state is not None else None),
-                    "kf_score_candidates")
+        fn = self._lib.kf_score_candidates_static if static_scratch else self._lib.kf_score_candidates
+        self._check(fn(self._h, C.byref(g), int(layer), C.byref(cands), C.byref(lh), C.byref(lb), int(window_half),
+                       float(chi2_cut), 1 if do_update else 0, order.data_ptr() if order is not None else None,
+                       best_hit.data_ptr(), best_chi2.data_ptr(),
+                       local_state.data_ptr() if local_state is not None else None),
+                    "kf_score_candidates_static" if static_scratch else "kf_score_candidates")
         del keep
 
     # ------------------------------------------------------------------ kf_build_best_hit

@@ -182,9 +182,10 @@ class DeviceCandidates:
 
     def score(self, ctx: KFContext, geom: Geometry, layer: int, hits: DeviceLayer, window_half: int = 2,
               chi2_cut: float = 30.0, do_update: bool = True, order: torch.Tensor | None = None,
-              keep_local: bool = True):
+              keep_local: bool = True, static_scratch: bool = False):
         """kf_score_candidates on one layer.  keep_local: carry the candidates' local-frame state between the
-        per-layer calls (allocated and zeroed at the first call; see the header)."""
+        per-layer calls (allocated and zeroed at the first call; see the header).  static_scratch: the no-allocation
+        entry point kf_score_candidates_static (at most STATIC_MAX_CANDIDATES candidates)."""
         ls = None
         if keep_local:
             ls = getattr(self, "local_state", None)
@@ -192,7 +193,7 @@ class DeviceCandidates:
                 ls = self.local_state = torch.zeros((30, self.ld), dtype=torch.float32, device=self.par.device)
         ctx.score_candidates(geom, layer, self.n, self.par, self.cov, self.q, self.chi2, self.nhits, self.status,
                              hits.n_hits, hits.pos, hits.cov, hits.bins, window_half, chi2_cut, do_update,
-                             self.best_hit, self.best_chi2, order, ls)
+                             self.best_hit, self.best_chi2, order, ls, static_scratch)
 
     def build(self, ctx: KFContext, geom: Geometry, first_layer: int, layers: list, window_half: int = 2,
               chi2_cut: float = 30.0, do_update: bool = True, order: torch.Tensor | None = None):

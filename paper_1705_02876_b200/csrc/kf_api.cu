@@ -187,6 +187,7 @@ const char* kf_strerror(int code) {
         case KF_ERR_CUDA: return "a CUDA runtime call failed (see kf_last_cuda_error)";
         case KF_ERR_NOMEM: return "scratch allocation failed";
         case KF_ERR_STALE: return "stale graph: its context is gone or has reallocated scratch / changed the bin grid since the recording";
+        case KF_ERR_TOO_LARGE: return "more candidates than the static scratch holds (KF_STATIC_MAX_CANDIDATES = 65536)";
         default: return "unknown error code";
     }
 }
@@ -768,6 +769,45 @@ int kf_score_candidates(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks
     if (cands->n > 0 && (!best_hit || !best_chi2)) return KF_ERR_NULL;
     return build_best_hit(c, geom, layer, 1, cands, hits, bins, window_half, chi2_cut, do_update, order,
                           best_hit, best_chi2, cands->n > 0 ? cands->ld : 0, local_state);
+}
+
+static_assert(kStaticMaxCands == KF_STATIC_MAX_CANDIDATES, "kf_internal.h and kf_b200.h disagree on the static scratch size");
+
+// The single-layer call on the static scratch of kf_score.cu: the argument checks of build_best_hit for one layer,
+// then launch_score_static.  No allocation on any path; the context's scratch is neither read nor resized.
+int kf_score_candidates_static(kf_ctx* c, const kf_geometry* geom, int layer, kf_tracks* cands,
+                               const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                               float chi2_cut, int do_update, const int32_t* order, int32_t* best_hit,
+                               float* best_chi2, float* local_state) {
+    if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (layer < 0 || layer >= geom->n_layers) return KF_ERR_SHAPE;
+    if ((rc = check_tracks(cands, true, true))) return rc;
+    if (cands->n > KF_STATIC_MAX_CANDIDATES) return KF_ERR_TOO_LARGE;
+    if (cands->n == 0) return KF_OK;
+    if (!best_hit || !best_chi2) return KF_ERR_NULL;
+    if ((rc = check_score_bins(hits, bins, window_half))) return rc;
+    if (local_state && !aligned16(local_state)) return KF_ERR_ALIGN;
+    ScoreStep st;
+    std::memset(&st, 0, sizeof(st));
+    st.layer = layer;
+    st.n_hits = hits->n_hits;
+    st.hit_rec = bins->hit_rec; st.bin_box = bins->bin_box; st.bin_offset = bins->bin_offset;
+    st.best_hit = best_hit; st.best_chi2 = best_chi2;
+    ScoreArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.n = cands->n; a.ld = cands->ld; a.par = cands->par; a.cov = cands->cov; a.q = cands->q;
+    a.chi2 = cands->chi2; a.nhits = cands->nhits; a.status = cands->status;
+    a.order = order;
+    a.n_eta = bins->n_eta; a.n_phi = bins->n_phi; a.eta_max = bins->eta_max;
+    a.window_half = window_half; a.chi2_cut = chi2_cut; a.do_update = do_update ? 1 : 0;
+    a.lstate = local_state; a.ld_ls = cands->ld;
+    KF_ON_DEVICE(c);
+    const cudaError_t e = launch_score_static(P, a, st, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    return KF_OK;
 }
 
 }  // extern "C"

@@ -217,6 +217,12 @@ struct ScoreScratch {
 cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n_steps, const ScoreStep* steps,
                          cudaStream_t stream);
 
+// kf_score_candidates_static: one layer with the per-candidate scratch in a `static __device__` array of kf_score.cu
+// (no allocation of any kind).  n <= kStaticMaxCands is the caller's check; cudaErrorInvalidValue beyond it.
+constexpr int64_t kStaticMaxCands = 65536;            // = KF_STATIC_MAX_CANDIDATES (checked in kf_api.cu)
+constexpr int kStaticPlanes = kScorePlanes + 2;       // propagated candidate + flag + slot
+cudaError_t launch_score_static(const FitParams& P, ScoreArgs a, const ScoreStep& step, cudaStream_t stream);
+
 // ---------------------------------------------------------------------------------- combinatorial building
 struct CombCall {
     int64_t n_seeds, ld;

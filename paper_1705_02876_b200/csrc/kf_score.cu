@@ -24,6 +24,8 @@
 // original index).
 // Warp w scans candidate order[w] when an order is given (kf_order_candidates), so neighbouring warps
 // share their windows in L1/L2; the order never changes a result.
+#include <mutex>
+
 #include "kf_score_common.cuh"
 
 namespace kf {
@@ -297,6 +299,72 @@ cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n
     }
     if (multi) update_global_kernel<true><<<cblocks, kCandBlock, 0, stream>>>(a, keep);
     else update_global_kernel<false><<<cblocks, kCandBlock, 0, stream>>>(a, keep);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------- kf_score_candidates_static
+// The scratch of the single-layer call for callers that must not allocate (include/kf_b200.h): the propagated
+// candidate planes, the flag and the winning slot, for at most kStaticMaxCands candidates, compiled into the
+// library.  Each device that loads the module has its own copy (7.75 MiB) until the process exits.  The single-layer
+// call never uses the between-layers track planes (keep = 0), so they have no static counterpart.
+//
+// In HOST code the name g_static_scratch is a host-side stand-in for the symbol, not a device address: the kernels
+// get the address cudaGetSymbolAddress returns, resolved once per device with that device current.
+}  // namespace kf
+
+static __device__ __align__(256) float g_static_scratch[(size_t)kf::kStaticPlanes * kf::kStaticMaxCands];
+
+namespace kf {
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+float* g_static_addr[kStaticMaxDevices] = {};   // device address of g_static_scratch per device ordinal
+
+cudaError_t static_scratch_address(float** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_addr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_static_addr[dev] = static_cast<float*>(p);
+    }
+    *out = g_static_addr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+// Same three launches as launch_build with n_steps = 1 (propagate, scan, decision); only the scratch differs.
+// Nothing in the array has to start at zero: propagate_global_kernel writes flag[i] for every i < n and the scratch
+// planes of every candidate it flags FLAG_AT_LAYER, scan_kernel writes slot[i] for exactly those, and
+// update_global_kernel reads nothing else.  What an earlier call left beyond that is never read.
+cudaError_t launch_score_static(const FitParams& P, ScoreArgs a, const ScoreStep& st, cudaStream_t stream) {
+    if (a.n == 0) return cudaSuccess;
+    if (a.n > kStaticMaxCands) return cudaErrorInvalidValue;
+    float* base = nullptr;
+    cudaError_t e = static_scratch_address(&base);
+    if (e != cudaSuccess) return e;
+    const int64_t ld = (a.n + 63) / 64 * 64;                    // planes stay 256-byte aligned; ld <= kStaticMaxCands
+    a.scratch = base;
+    a.track = nullptr;                                          // keep_track = 0 below: never dereferenced
+    a.flag = reinterpret_cast<int32_t*>(base + (int64_t)kScorePlanes * ld);
+    a.slot = a.flag + ld;
+    a.ld_sc = ld;
+    a.ev.n = 0;
+    const unsigned cblocks = (unsigned)((a.n + kCandBlock - 1) / kCandBlock);
+    const unsigned sblocks = (unsigned)((a.n + kScanBlock / 32 - 1) / (kScanBlock / 32));
+    propagate_global_kernel<<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer, 0);
+    a.hit_rec = st.hit_rec; a.bin_box = st.bin_box; a.bin_offset = st.bin_offset; a.n_hits = st.n_hits;
+    a.best_hit = st.best_hit; a.best_chi2 = st.best_chi2;
+    scan_kernel<false><<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
+    update_global_kernel<false><<<cblocks, kCandBlock, 0, stream>>>(a, 0);
     return cudaGetLastError();
 }
 

@@ -63,6 +63,7 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_fit_tracks_smooth(None, None, None, None, None, None) == -1
     assert lib.kf_bin_hits(None, 1.0, None, None) == -1
     assert lib.kf_score_candidates(None, None, 0, None, None, None, 2, 30.0, 1, None, None, None, None) == -1
+    assert lib.kf_score_candidates_static(None, None, 0, None, None, None, 2, 30.0, 1, None, None, None, None) == -1
     assert lib.kf_bin_layers(None, 1, None, None, None) == -1
     assert lib.kf_build_combinatorial(None, None, 0, 1, None, None, None, 2, 30.0, 4, None, None, 0) == -1
     assert lib.kf_build_best_hit(None, None, 0, 1, None, None, None, 2, 30.0, 1, None, None, None, 0) == -1

@@ -234,7 +234,7 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
     torch.cuda.synchronize()
     s = d3.results()
     geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass)
-    layers = [DeviceLayer.from_numpy(l.pos, l.cov, cfg.n_eta, cfg.n_phi, emax, dev) for l in ev.layers[L0:]]
+    layers = [DeviceLayer.from_numpy(l.pos, l.cov, cfg.n_eta, cfg.n_phi, emax, dev, soa=False) for l in ev.layers[L0:]]
     ctx.reserve(max_hits=sum(l.n_hits for l in layers))
     radii = [l.radius for l in ev.layers[L0:]]
     args = [(l.n_hits, l.pos, l.cov, l.bins) for l in layers]
@@ -321,7 +321,41 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
     events_ms = float(np.median(ts[2:]))
     egraph.close()
     events_equal = bool(torch.equal(eidx[:, :f.n], out["idx"][:, :f.n]) and torch.equal(eidx[:, (n_ev - 1) * f.n:n_ev * f.n], out["idx"][:, :f.n]))
-    del big, big_seed, eidx, ec2
+    # the same for combinatorial building (kf_build_combinatorial_events, 4 candidates per seed)
+    cbig = torch.empty((L - L0, big.ld), dtype=torch.int32, device=dev)
+    cnf = torch.zeros(big.ld, dtype=torch.int32, device=dev)
+
+    def comb_events_call():
+        ctx.build_combinatorial_events(geom, L0, first, big.n, big.par, big.cov, big.q, big.chi2, big.nhits, big.status,
+                                       [args] * n_ev, 2, 30.0, 4, cbig, cnf)
+    for k, v in big_seed.items():
+        getattr(big, k).copy_(v)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        comb_events_call()
+    torch.cuda.synchronize()
+    for k, v in big_seed.items():
+        getattr(big, k).copy_(v)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        ctx.graph_begin()
+        comb_events_call()
+        cgraph = ctx.graph_end()
+    ts = []
+    for it in range(reps + 2):
+        for k, v in big_seed.items():
+            getattr(big, k).copy_(v)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        cgraph.launch()
+        e1.record(st)
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    comb_events_ms = float(np.median(ts[2:]))
+    cgraph.close()
+    comb_events_equal = bool(torch.equal(cbig[:, :f.n], out["cidx"][:, :f.n]) and torch.equal(cbig[:, (n_ev - 1) * f.n:n_ev * f.n], out["cidx"][:, :f.n]))
+    del big, big_seed, eidx, ec2, cbig, cnf
     # end to end through kf_build_best_hit_host: pinned HOST pools and candidates in, results out, per event
     # (H2D of layer j + 1 overlapped with binning + scoring of layer j)
     from paper_1705_02876_b200.buffers import padded_ld
@@ -396,7 +430,11 @@ def measure_building(ctx, dev: str, reps: int = 10) -> dict:
             "combinatorial": {"n_cand": 4, "build_ms": tc, "eager_build_ms": eager["comb"],
                               "seeds_per_s": f.n / (tc * 1e-3),
                               "all_true_hits_found_fraction": comb_eff,
-                              "best_hit_all_true_hits_found_fraction": best_eff, "kernels": 4 * (L - L0) + 2}}
+                              "best_hit_all_true_hits_found_fraction": best_eff, "kernels": 4 * (L - L0) + 2,
+                              "events_in_one_call": {"api": "kf_build_combinatorial_events", "n_events": n_ev,
+                                                     "ms": comb_events_ms, "ms_per_event": comb_events_ms / n_ev,
+                                                     "speedup_vs_one_event_per_call": tc / (comb_events_ms / n_ev),
+                                                     "same_hits_as_single_event_call": comb_events_equal}}}
 
 
 def run_profile_sequence(args) -> None:

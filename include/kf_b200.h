@@ -174,7 +174,8 @@ typedef struct {
      * layer is skipped; a plane that lies behind the state or half a turn or more away is KF_STATUS_PROP_FAIL.
      * radius_cm[l] of a disc layer is not used but must keep the list increasing.  Discs are known to
      * kf_fit_tracks, kf_fit_tracks_indexed and kf_fit_tracks_host; every other call returns KF_ERR_UNSUPPORTED
-     * for a geometry with a disc, and so does energy_loss_model = 1 with discs. */
+     * for a geometry with a disc.  material_model and energy_loss_model apply at a disc with the path factor
+     * 1 / |cos| of the angle to the z axis = |p| / |pz|. */
     const int32_t* surface_type;  /* HOST [n_layers] 0 = barrel, 1 = disc pair; or NULL                        */
     const float* disc_z_cm;       /* HOST [n_layers] |z| of the disc pair (> 0), read where surface_type = 1   */
     const float* disc_rmin_cm;    /* HOST [n_layers] inner radius of the annulus (>= 0)                         */
@@ -414,6 +415,18 @@ KF_API int kf_build_combinatorial(kf_ctx* ctx, const kf_geometry* geom, int firs
                                   kf_tracks* cands, const kf_layer_hits* hits, const kf_layer_bins* bins,
                                   int window_half, float chi2_cut, int n_cand, int32_t* hit_index,
                                   int32_t* n_found, int64_t ld_out);
+
+/* Combinatorial building of SEVERAL EVENTS in one call (as kf_build_best_hit_events): `cands` holds
+ * the seeds of all events back to back, event e owns event_first[e] .. event_first[e + 1] - 1 (HOST int64
+ * [n_events + 1], event_first[0] = 0, last = cands->n); hits / bins: HOST arrays [n_events][n_build_layers]
+ * (event-major), every event with its own pools, all bins with one (n_eta, n_phi, eta_max); n_events <= 32.  The
+ * same 4 n_build_layers + 2 launches as one event.  Per seed the result is exactly what kf_build_combinatorial gives
+ * for its event alone (bit for bit); outputs as there. */
+KF_API int kf_build_combinatorial_events(kf_ctx* ctx, const kf_geometry* geom, int first_layer, int n_build_layers,
+                                         int n_events, const int64_t* event_first, kf_tracks* cands,
+                                         const kf_layer_hits* hits, const kf_layer_bins* bins, int window_half,
+                                         float chi2_cut, int n_cand, int32_t* hit_index, int32_t* n_found,
+                                         int64_t ld_out);
 
 #ifdef __cplusplus
 }

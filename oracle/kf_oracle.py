@@ -346,7 +346,8 @@ def fit_batch(batch, nthreads: int = 1, want_trace: bool = False) -> dict:
         return fit_tracks(batch.radius, batch.x_over_X0, batch.Bz, batch.mass, batch.par, batch.cov,
                           batch.q, batch.hpos, batch.hcov, batch.mask, nthreads, want_trace)
     with surfaces(st, batch.disc_z, batch.disc_rmin, batch.disc_rmax), \
-            geometry_options(int(getattr(batch, "material_model", 0)), getattr(batch, "half_length", None)):
+            geometry_options(int(getattr(batch, "material_model", 0)), getattr(batch, "half_length", None),
+                             energy_loss=int(getattr(batch, "energy_loss", 0))):
         return fit_tracks(batch.radius, batch.x_over_X0, batch.Bz, batch.mass, batch.par, batch.cov,
                           batch.q, batch.hpos, batch.hcov, batch.mask, nthreads, want_trace)
 

@@ -26,7 +26,7 @@ STATIC_MAX_CANDIDATES = 65536                                               # KF
 ERR_TOO_LARGE = -8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
            "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
-           "kf_score_candidates", "kf_score_candidates_static", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial",
+           "kf_score_candidates", "kf_score_candidates_static", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial", "kf_build_combinatorial_events",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
 
@@ -154,6 +154,10 @@ def load_library():
     lib.kf_build_combinatorial.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.POINTER(_Tracks),
                                            C.POINTER(_LayerHits), C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int,
                                            vp, vp, C.c_int64]
+    lib.kf_build_combinatorial_events.restype = C.c_int
+    lib.kf_build_combinatorial_events.argtypes = [vp, C.POINTER(_Geometry), C.c_int, C.c_int, C.c_int,
+                                                  C.POINTER(C.c_int64), C.POINTER(_Tracks), C.POINTER(_LayerHits),
+                                                  C.POINTER(_LayerBins), C.c_int, C.c_float, C.c_int, vp, vp, C.c_int64]
     lib.kf_graph_begin.restype = C.c_int
     lib.kf_graph_begin.argtypes = [vp]
     lib.kf_graph_end.restype = C.c_int
@@ -539,4 +543,22 @@ class KFContext:
                                                      hit_index.data_ptr(),
                                                      n_found.data_ptr() if n_found is not None else None,
                                                      int(hit_index.stride(0))), "kf_build_combinatorial")
+        del keep
+
+    def build_combinatorial_events(self, geom: Geometry, first_layer: int, event_first, n: int, par, cov, q, chi2,
+                                   nhits, status, layers_by_event, window_half: int, chi2_cut: float, n_cand: int,
+                                   hit_index, n_found=None):
+        """Several events in one call; arguments as build_best_hit_events (event_first in seed indices)."""
+        g, keep = geom._c()
+        cands = self._tracks(n, par, cov, q, chi2, nhits, status)
+        ne, m = len(layers_by_event), len(layers_by_event[0])
+        flat = [l for ev in layers_by_event for l in ev]
+        lhs = (_LayerHits * (ne * m))(*[self._layer_hits(nh, p, c) for (nh, p, c, _) in flat])
+        lbs = (_LayerBins * (ne * m))(*[b._c() for (_, _, _, b) in flat])
+        first = (C.c_int64 * (ne + 1))(*[int(v) for v in event_first])
+        self._check(self._lib.kf_build_combinatorial_events(self._h, C.byref(g), int(first_layer), m, ne, first,
+                                                            C.byref(cands), lhs, lbs, int(window_half), float(chi2_cut),
+                                                            int(n_cand), hit_index.data_ptr(),
+                                                            n_found.data_ptr() if n_found is not None else None,
+                                                            int(hit_index.stride(0))), "kf_build_combinatorial_events")
         del keep

@@ -139,13 +139,15 @@ class DeviceLayer:
 
     @staticmethod
     def from_numpy(pos: np.ndarray, cov: np.ndarray, n_eta: int, n_phi: int, eta_max: float,
-                   device="cuda:0") -> "DeviceLayer":
+                   device="cuda:0", soa: bool = True) -> "DeviceLayer":
+        """soa = False: no SoA copy of the sorted hits (kf_layer_bins.pos_sorted / cov_sorted NULL): scoring and
+        building read the packed records only."""
         from .binding import Bins
         n = int(pos.shape[1])
         ld = padded_ld(n)
         return DeviceLayer(n, ld, _to_planes(pos.astype(np.float32), ld, device),
                            _to_planes(cov.astype(np.float32), ld, device),
-                           Bins.allocate(n, n_eta, n_phi, eta_max, device))
+                           Bins.allocate(n, n_eta, n_phi, eta_max, device, soa))
 
     def bin(self, ctx: KFContext, radius_cm: float):
         ctx.bin_hits(radius_cm, self.n_hits, self.pos, self.cov, self.bins)

@@ -139,7 +139,6 @@ int make_params(const kf_geometry* g, FitParams* P, bool allow_discs = false) {
             P->layer[l].de0 = t > 0.0 ? (float)(0.307075e-3 * (14.0 / 28.0855) * t * 21.82) : 0.0f;
         }
     }
-    if (discs && g->energy_loss_model) return KF_ERR_UNSUPPORTED;   // (energy loss is implemented on barrels only)
     P->geometry_options = (P->model != 0 || discs) ? 1 : 0;
     P->has_discs = discs ? 1 : 0;
     for (int l = 0; l < g->n_layers; ++l) P->geometry_options |= std::isfinite(P->layer[l].half_len) ? 1 : 0;
@@ -755,6 +754,61 @@ int kf_build_combinatorial(kf_ctx* c, const kf_geometry* geom, int first_layer, 
     call.n_eta = bins[0].n_eta; call.n_phi = bins[0].n_phi; call.eta_max = bins[0].eta_max;
     call.window_half = window_half; call.chi2_cut = chi2_cut;
     call.hit_index = hit_index; call.ld_out = ld_out; call.n_found = n_found;
+    KF_ON_DEVICE(c);
+    cudaError_t e = launch_comb(c->comb, P, call, n_build_layers, steps, c->stream);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+    return KF_OK;
+}
+
+int kf_build_combinatorial_events(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_build_layers, int n_events,
+                                  const int64_t* event_first, kf_tracks* cands, const kf_layer_hits* hits,
+                                  const kf_layer_bins* bins, int window_half, float chi2_cut, int n_cand,
+                                  int32_t* hit_index, int32_t* n_found, int64_t ld_out) {
+    if (!c || !geom || !cands || !hits || !bins || !event_first) return KF_ERR_NULL;
+    FitParams P;
+    int rc = make_params(geom, &P);
+    if (rc) return rc;
+    if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
+    if (n_cand < 1 || n_cand > 8) return KF_ERR_UNSUPPORTED;
+    if (n_events < 1) return KF_ERR_SHAPE;
+    if (n_events > kMaxBuildEvents) return KF_ERR_UNSUPPORTED;
+    if ((rc = check_tracks(cands, true, true))) return rc;
+    if (event_first[0] != 0 || event_first[n_events] != cands->n) return KF_ERR_SHAPE;
+    for (int e = 0; e < n_events; ++e)
+        if (event_first[e + 1] < event_first[e]) return KF_ERR_SHAPE;
+    if (n_build_layers == 0 || cands->n == 0) return KF_OK;
+    if (!hit_index) return KF_ERR_NULL;
+    if (ld_out < cands->n) return KF_ERR_SHAPE;
+    if (cands->n * (int64_t)n_cand > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
+    ScoreStep steps[KF_MAX_LAYERS];
+    for (int j = 0; j < n_build_layers; ++j) {
+        for (int e = 0; e < n_events; ++e) {
+            const kf_layer_hits* h = hits + (int64_t)e * n_build_layers + j;
+            const kf_layer_bins* b = bins + (int64_t)e * n_build_layers + j;
+            if ((rc = check_score_bins(h, b, window_half))) return rc;
+            if (b->n_eta != bins[0].n_eta || b->n_phi != bins[0].n_phi || b->eta_max != bins[0].eta_max)
+                return KF_ERR_UNSUPPORTED;
+            steps[j].ev_hit_rec[e] = b->hit_rec;
+            steps[j].ev_bin_box[e] = b->bin_box;
+            steps[j].ev_bin_offset[e] = b->bin_offset;
+        }
+        steps[j].layer = first_layer + j;
+        steps[j].n_hits = hits[j].n_hits;
+        steps[j].hit_rec = bins[j].hit_rec;
+        steps[j].bin_box = bins[j].bin_box;
+        steps[j].bin_offset = bins[j].bin_offset;
+        steps[j].best_hit = nullptr;
+        steps[j].best_chi2 = nullptr;
+    }
+    CombCall call;
+    call.n_seeds = cands->n; call.ld = cands->ld; call.par = cands->par; call.cov = cands->cov; call.q = cands->q;
+    call.chi2 = cands->chi2; call.nhits = cands->nhits; call.status = cands->status;
+    call.n_cand = n_cand;
+    call.n_eta = bins[0].n_eta; call.n_phi = bins[0].n_phi; call.eta_max = bins[0].eta_max;
+    call.window_half = window_half; call.chi2_cut = chi2_cut;
+    call.hit_index = hit_index; call.ld_out = ld_out; call.n_found = n_found;
+    call.ev.n = n_events;
+    for (int e = 0; e <= n_events; ++e) call.ev.first[e] = event_first[e];
     KF_ON_DEVICE(c);
     cudaError_t e = launch_comb(c->comb, P, call, n_build_layers, steps, c->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);

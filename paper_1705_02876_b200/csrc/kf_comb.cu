@@ -40,6 +40,7 @@ struct CombArgs {
     // hits of the layer
     const float* hit_rec; const float* bin_box; const int32_t* bin_offset;
     int n_eta, n_phi; float eta_max; int window_half; float chi2_cut;
+    EventPools ev;                // kf_build_combinatorial_events (ev.n > 1): seeds of event e are first[e] .. first[e + 1] - 1
 };
 
 constexpr int32_t REC_NONE = -1;      // child takes no hit
@@ -124,6 +125,8 @@ __device__ __forceinline__ int acc_top(AccEntry* acc, int n, int keep, int lane)
     return m;
 }
 
+// MULTI: several events in one call (EventPools), compiled out of the single-event kernel as in kf_score.cu.
+template <bool MULTI>
 __global__ void __launch_bounds__(kScanBlock)
 comb_scan_kernel(const CombArgs a, float inv_r) {
     __shared__ int32_t survivors[kScanBlock / 32][96];
@@ -147,8 +150,10 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
     const unsigned lt_mask = (1u << lane) - 1u;
     const float ecc = c.ec * c.ec, ess = c.es * c.es, ecs2 = 2.0f * c.ec * c.es;
     const int wh = a.window_half;
-    const float4* __restrict__ rec = reinterpret_cast<const float4*>(a.hit_rec);
-    const float4* __restrict__ box = reinterpret_cast<const float4*>(a.bin_box);
+    const int event = MULTI ? event_of(a.ev, slot / a.nc) : 0;
+    const float4* __restrict__ rec = reinterpret_cast<const float4*>(MULTI ? a.ev.hit_rec[event] : a.hit_rec);
+    const float4* __restrict__ box = reinterpret_cast<const float4*>(MULTI ? a.ev.bin_box[event] : a.bin_box);
+    const int32_t* __restrict__ bin_offset = MULTI ? a.ev.bin_offset[event] : a.bin_offset;
     const int side = 2 * wh + 1, n_win = side * side;
 
     // full chi2 of up to 32 listed survivors; the compatible ones go to the accumulator
@@ -177,8 +182,8 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
             p -= p >= a.n_phi ? a.n_phi : 0;
             if (e >= 0 && e < a.n_eta) {
                 const int bin = e * a.n_phi + p;
-                s0 = __ldg(a.bin_offset + bin);
-                s1 = __ldg(a.bin_offset + bin + 1);
+                s0 = __ldg(bin_offset + bin);
+                s1 = __ldg(bin_offset + bin + 1);
                 const float4 X = __ldg(box + 2 * bin), Z = __ldg(box + 2 * bin + 1);
                 const float dzm = fmaxf(0.0f, fmaxf(Z.x - c.zn, c.zn - Z.y));
                 const float ax = -c.es, ay = c.ec;
@@ -319,6 +324,7 @@ comb_select_kernel(const CombArgs a) {
 }
 
 // One thread per surviving child: materialise it in the other half of the candidate store.
+template <bool MULTI>
 __global__ void __launch_bounds__(128)
 comb_update_kernel(const CombArgs a) {
     const int64_t so = (int64_t)blockIdx.x * 128 + threadIdx.x;
@@ -342,7 +348,8 @@ comb_update_kernel(const CombArgs a) {
         bool updated = false;
         if (r >= 0) {
             LocalHit h;
-            hit_from_record(reinterpret_cast<const float4*>(a.hit_rec), r, o, h);
+            const float* recs = MULTI ? a.ev.hit_rec[event_of(a.ev, sd)] : a.hit_rec;
+            hit_from_record(reinterpret_cast<const float4*>(recs), r, o, h);
             float d;
             const uint32_t rc = kalman_update(t, o, n, h, &d);
             if (rc == 0u) { updated = true; chi2 += d; nh += 1; } else st |= rc;
@@ -444,16 +451,23 @@ cudaError_t launch_comb(CombScratch& s, const FitParams& P, const CombCall& call
     };
     bind(cur);
     a.hit_rec = nullptr; a.bin_box = nullptr; a.bin_offset = nullptr; a.hist_parent = hist_parent; a.hist_hit = hist_hit;
+    a.ev = call.ev;
+    const bool multi = a.ev.n > 1;
     comb_init_kernel<<<seed_blocks, 128, 0, stream>>>(a);
     for (int j = 0; j < n_steps; ++j) {
         const ScoreStep& sp = steps[j];
         a.hit_rec = sp.hit_rec; a.bin_box = sp.bin_box; a.bin_offset = sp.bin_offset;
+        for (int e = 0; e < a.ev.n; ++e) {
+            a.ev.hit_rec[e] = sp.ev_hit_rec[e]; a.ev.bin_box[e] = sp.ev_bin_box[e]; a.ev.bin_offset[e] = sp.ev_bin_offset[e];
+        }
         a.hist_parent = hist_parent + (int64_t)j * S;
         a.hist_hit = hist_hit + (int64_t)j * S;
         comb_propagate_kernel<<<slot_blocks, 128, 0, stream>>>(P, a, sp.layer);
-        comb_scan_kernel<<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
+        if (multi) comb_scan_kernel<true><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
+        else comb_scan_kernel<false><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
         comb_select_kernel<<<(unsigned)((call.n_seeds + 3) / 4), 128, 0, stream>>>(a);
-        comb_update_kernel<<<slot_blocks, 128, 0, stream>>>(a);
+        if (multi) comb_update_kernel<true><<<slot_blocks, 128, 0, stream>>>(a);
+        else comb_update_kernel<false><<<slot_blocks, 128, 0, stream>>>(a);
         cur ^= 1;
         bind(cur);
     }

@@ -71,12 +71,20 @@ struct Hit {
 // would force the track into local memory in every kernel that can reach it (measured: the barrel-with-options
 // fit went from 0.354 to 0.535 ms per 2 M tracks), inlined it costs registers where it is used only.
 __device__ __forceinline__ uint32_t fit_layer_disc(Track& t, float k, float ik, const LayerConst& L, int model, float mass2,
-                                                const Hit& m, float& chi2) {
+                                                const Bethe& el, const Hit& m, float& chi2) {
     DiscCrossing o;
     const uint32_t reached = helix_to_plane(t, k, ik, L, o);
     if (reached) return reached;
     DiscCov n;
     transport_cov_disc(t, o, k, ms_at_disc(L, model, o, t.pz), mass2, n);
+    const float pz_in = t.pz;
+    if (model & MODEL_ENERGY_LOSS) {   // reading A21 at a disc: the path factor is 1 / |cos| to the z axis = (p / pT) / |T|
+        Eloss e;
+        if (!energy_loss_factors(el, L, model, mass2, o.T, o.pt2, o.ipt, pz_in, false, e)) return ST_PROP_FAIL;
+        float pz = pz_in;
+        apply_energy_loss_disc(e, o, n, pz);
+        t.pz = pz;
+    }
     Crossing c;                       // what hit_to_local reads of it
     c.xn = o.xn; c.yn = o.yn; c.zn = o.zt; c.erx = o.erx; c.ery = o.ery;
     LocalHit h;
@@ -84,6 +92,7 @@ __device__ __forceinline__ uint32_t fit_layer_disc(Track& t, float k, float ik, 
     float d;
     const uint32_t rc = kalman_update_disc(t, o, n, h, &d);
     if (rc == 0u) chi2 += d;
+    else t.pz = pz_in;                // layer skipped: the track stays as it was
     return rc;
 }
 
@@ -93,7 +102,7 @@ template <bool RADIAL_NULL, int GEOM = 1>
 __device__ __forceinline__ uint32_t fit_layer(Track& t, float k, float ik, const LayerConst& L, int model,
                                               float mass2, const Bethe& el, const Hit& m, float& chi2) {
     if constexpr (GEOM == 2) {
-        if (L.type == 1) return fit_layer_disc(t, k, ik, L, model, mass2, m, chi2);
+        if (L.type == 1) return fit_layer_disc(t, k, ik, L, model, mass2, el, m, chi2);
     }
     Crossing o;
     const uint32_t reached = reach_layer<false, GEOM != 0>(t, k, ik, L, o);

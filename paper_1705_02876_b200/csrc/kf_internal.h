@@ -230,6 +230,7 @@ struct CombCall {
     int n_cand;
     int n_eta, n_phi; float eta_max; int window_half; float chi2_cut;
     int32_t* hit_index; int64_t ld_out; int32_t* n_found;
+    EventPools ev = {};      // kf_build_combinatorial_events: ev.n > 1, ev.first in SEED indices; pools per step in ScoreStep::ev_*
 };
 
 struct CombScratch {

@@ -817,6 +817,22 @@ __device__ __forceinline__ float ms_at_disc(const LayerConst& L, int model, cons
     return L.ms0 * f * lg * lg;
 }
 
+// Reading A21 at a disc: the same direction-preserving momentum scaling and Jacobian J on (b1, b2, c) as
+// apply_energy_loss, on the disc's propagated state and covariance (T = pz / pT does not change).
+__device__ __forceinline__ void apply_energy_loss_disc(const Eloss& e, DiscCrossing& o, DiscCov& n, float& pz) {
+    const float f = e.f, g = e.g, h = e.h, ff = f * f;
+    o.pxn *= f; o.pyn *= f; pz *= f;
+    o.pt2 *= ff;
+    o.ipt *= rcp_fast(f);
+    n.r3 = g * n.r3 + h * n.r5;
+    n.t3 = g * n.t3 + h * n.t5;
+    n.n33 = g * (g * n.n33 + 2.0f * h * n.n35) + h * h * n.n55;
+    n.n34 = f * (g * n.n34 + h * n.n45);
+    n.n35 = f * (g * n.n35 + h * n.n55);
+    n.r4 *= f; n.t4 *= f; n.r5 *= f; n.t5 *= f;
+    n.n44 *= ff; n.n45 *= ff; n.n55 *= ff;
+}
+
 // Kalman update at a disc: C' has a zero z row, so the z component of S = C'_pp + V~ is eliminated first (Schur
 // complement on v_zz), leaving a 2-D measurement in (r, t) -- the disc's counterpart of kalman_update.
 __device__ __forceinline__ uint32_t kalman_update_disc(Track& t, const DiscCrossing& o, const DiscCov& n, const LocalHit& h,

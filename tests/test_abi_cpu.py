@@ -66,6 +66,7 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_score_candidates_static(None, None, 0, None, None, None, 2, 30.0, 1, None, None, None, None) == -1
     assert lib.kf_bin_layers(None, 1, None, None, None) == -1
     assert lib.kf_build_combinatorial(None, None, 0, 1, None, None, None, 2, 30.0, 4, None, None, 0) == -1
+    assert lib.kf_build_combinatorial_events(None, None, 0, 1, 1, None, None, None, None, 2, 30.0, 4, None, None, 0) == -1
     assert lib.kf_build_best_hit(None, None, 0, 1, None, None, None, 2, 30.0, 1, None, None, None, 0) == -1
     assert lib.kf_build_best_hit_events(None, None, 0, 1, 1, None, None, None, None, 2, 30.0, 1, None, None, 0) == -1
     assert lib.kf_build_best_hit_host(None, None, 0, 1, None, None, 40, 64, 1.2, 2, 30.0, 1, None, None, 0) == -1

@@ -82,6 +82,22 @@ def test_endcap_with_path_length_material(ctx):
     print("endcap toy with path-length material:", res)
 
 
+def test_endcap_with_energy_loss(ctx):
+    """Reading A21 on barrels AND discs (path factor |p| / |pz| at a disc), with and without the path-length
+    material: the option is set on both sides (the toy's hits carry no energy loss; parity does not need them to)."""
+    for mm in (0, 1):
+        b = W.simulate_endcap_event(7, 8000, material_model=mm)
+        b.energy_loss = 1
+        g, o = _fit_both(ctx, b)
+        res = _compare(g, o, b)
+        b.energy_loss = 0
+        o0 = O.fit_batch(b, nthreads=8)
+        ok = (o["status"] == 0) & (o0["status"] == 0)
+        p1 = np.linalg.norm(o["par"][3:6, ok], axis=0); p0 = np.linalg.norm(o0["par"][3:6, ok], axis=0)
+        assert np.median(p0 - p1) > 1e-4                                   # the option is felt: GeV lost on the way
+        print(f"endcap toy with energy loss (material_model={mm}):", res)
+
+
 def test_endcap_indexed_fit_equals_pre_gathered(ctx):
     """kf_fit_tracks_indexed knows discs too: the same hits addressed by index give the same fit."""
     from paper_1705_02876_b200.buffers import DeviceFit, padded_ld
@@ -119,11 +135,6 @@ def test_discs_are_refused_where_they_are_not_implemented(ctx):
         with pytest.raises(K.KFError) as e:
             call()
         assert e.value.code == -4
-    b.energy_loss = 1
-    d2 = DeviceFit.from_batch(b, "cuda:0")
-    with pytest.raises(K.KFError) as e:
-        d2.fit(ctx)
-    assert e.value.code == -4
     # malformed disc descriptions
     for bad in (dict(disc_z_cm=np.zeros(b.n_layers, np.float32)), dict(disc_rmax_cm=np.zeros(b.n_layers, np.float32))):
         b3 = W.simulate_endcap_event(0, 64)

@@ -76,6 +76,51 @@ def test_events_in_one_call_equal_one_call_per_event(ctx, sizes):
             assert np.array_equal(got[k][lo:hi], w[k]), (e, k)
 
 
+@pytest.mark.parametrize("sizes,n_cand", [([(700, 3000), (1, 50), (1200, 6000), (33, 0)], 4), ([(200, 1000)] * 32, 3)])
+def test_combinatorial_events_in_one_call_equal_one_call_per_event(ctx, sizes, n_cand):
+    """kf_build_combinatorial_events: per seed exactly what kf_build_combinatorial gives for its event alone
+    (tests/test_comb_gpu.py holds that call to the oracle)."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    evs = [_event(40 + i, n, noise) for i, (n, noise) in enumerate(sizes)]
+    fit0 = evs[0][0]
+    geom = K.Geometry(fit0.radius, fit0.x_over_X0, fit0.Bz, fit0.mass)
+    L0 = 3
+    want, pools = [], []
+    for fit, layers, par, cov, chi2, nh in evs:
+        dls = [DeviceLayer.from_numpy(p, c, NE, NP, EMAX, "cuda:0") for (_, p, c) in layers[L0:]]
+        ctx.bin_layers([r for (r, _, _) in layers[L0:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+        dc = DeviceCandidates.from_numpy(par, cov, fit.q, chi2, nh, "cuda:0")
+        idx, nf = dc.build_combinatorial(ctx, geom, L0, dls, n_cand)
+        torch.cuda.synchronize()
+        want.append(dict(dc.results(), idx=idx.cpu().numpy()[:, :fit.n], nf=nf.cpu().numpy()[:fit.n]))
+        pools.append(dls)
+    par = np.concatenate([e[2] for e in evs], axis=1); cov = np.concatenate([e[3] for e in evs], axis=1)
+    q = np.concatenate([e[0].q for e in evs]); chi2 = np.concatenate([e[4] for e in evs]); nh = np.concatenate([e[5] for e in evs])
+    first = np.concatenate([[0], np.cumsum([e[0].n for e in evs])])
+    dc = DeviceCandidates.from_numpy(par, cov, q, chi2, nh, "cuda:0")
+    m = 10 - L0
+    idx = torch.full((m, dc.ld), -9, dtype=torch.int32, device="cuda:0")
+    nf = torch.zeros(dc.ld, dtype=torch.int32, device="cuda:0")
+    ctx.build_combinatorial_events(geom, L0, first, dc.n, dc.par, dc.cov, dc.q, dc.chi2, dc.nhits, dc.status,
+                                   [[(d.n_hits, d.pos, d.cov, d.bins) for d in dls] for dls in pools], 2, 30.0, n_cand,
+                                   idx, nf)
+    torch.cuda.synchronize()
+    got = dict(dc.results(), idx=idx.cpu().numpy(), nf=nf.cpu().numpy())
+    for e, w in enumerate(want):
+        lo, hi = int(first[e]), int(first[e + 1])
+        for k in ("par", "cov", "idx"):
+            assert np.array_equal(got[k][..., lo:hi], w[k], equal_nan=True), (e, k)
+        for k in ("chi2", "nhits", "status", "nf"):
+            assert np.array_equal(got[k][lo:hi], w[k]), (e, k)
+    assert (got["idx"][:, :int(first[-1])] >= 0).mean() > 0.5
+    # argument errors as in the best-hit form
+    with pytest.raises(K.KFError) as err:
+        ctx.build_combinatorial_events(geom, L0, [0, dc.n - 1], dc.n, dc.par, dc.cov, dc.q, dc.chi2, dc.nhits, dc.status,
+                                       [[(d.n_hits, d.pos, d.cov, d.bins) for d in pools[0]]], 2, 30.0, n_cand, idx, nf)
+    assert err.value.code == -2
+
+
 def test_events_argument_errors(ctx):
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer

@@ -141,6 +141,9 @@ KF_API int kf_graph_destroy(kf_graph* graph);
 KF_API int kf_measure_fp32_peak(kf_ctx* ctx, int repeats, double* tflops_out);
 /* ABI version, bumped when a struct or signature changes. */
 KF_API int kf_abi_version(void);
+/* Floats per packed hit record of kf_layer_bins.hit_rec as this build writes it (= KF_HIT_RECORD_FLOATS). */
+#define KF_HIT_RECORD_FLOATS 12
+KF_API int kf_hit_record_floats(void);
 
 /* ---- geometry: concentric cylinders in a uniform solenoid field (PAPER.md:83 toy detector) ---- */
 typedef struct {
@@ -275,7 +278,7 @@ typedef struct {
     int64_t ld;               /* plane stride of pos_sorted / cov_sorted, >= n_hits, % 4 == 0      */
     int32_t* bin_offset;      /* DEV [n_eta*n_phi + 1] first sorted slot of each bin               */
     int32_t* sorted_to_orig;  /* DEV [n_hits] original index of the hit in each sorted slot        */
-    float* hit_rec;           /* DEV [n_hits][12] hits in bin order, packed for scoring:
+    float* hit_rec;           /* DEV [n_hits][KF_HIT_RECORD_FLOATS] hits in bin order, packed for scoring:
                                  x y z vzz | vxx vxy vyy index(int32 bits) | vxz vyz 0 0           */
     float* bin_box;           /* DEV [n_eta*n_phi][8] per-bin bounds for the scan's bin pruning:
                                  x_lo x_hi y_lo y_hi | z_lo z_hi max(vzz) max(vxx+vyy)              */
@@ -289,7 +292,7 @@ typedef struct {
  * buffers inside), -1 = no hit on that layer.  Otherwise exactly kf_fit_tracks (same arithmetic, same
  * status semantics, `out` may alias `seeds`).  index: DEV int32 [n_layers][ld_index], ld_index >= n.
  * `bins` = NULL, or a HOST array of n_layers kf_layer_bins made from the same pools by kf_bin_layers with
- * hit_rec and orig_to_sorted filled: the hits are then read from the packed records (3 memory sectors per
+ * hit_rec and orig_to_sorted filled: the hits are then read from the packed records (2 memory sectors per
  * hit instead of 9), same values, same results. */
 KF_API int kf_fit_tracks_indexed(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                                  const int32_t* index, int64_t ld_index, const kf_layer_hits* pools,

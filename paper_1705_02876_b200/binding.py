@@ -25,7 +25,7 @@ BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
 STATIC_MAX_CANDIDATES = 65536                                               # KF_STATIC_MAX_CANDIDATES
 ERR_TOO_LARGE = -8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_abi_version", "kf_hit_record_floats", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_score_candidates_static", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial", "kf_build_combinatorial_events",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
@@ -113,6 +113,8 @@ def load_library():
     lib.kf_measure_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     lib.kf_abi_version.restype = C.c_int
     lib.kf_abi_version.argtypes = []
+    lib.kf_hit_record_floats.restype = C.c_int
+    lib.kf_hit_record_floats.argtypes = []
     for name in ("kf_fit_tracks", "kf_fit_tracks_host"):
         f = getattr(lib, name)
         f.restype = C.c_int
@@ -199,6 +201,11 @@ def abi_version() -> int:
     return int(load_library().kf_abi_version())
 
 
+def hit_record_floats() -> int:
+    """Floats per packed hit record (kf_layer_bins.hit_rec) of the loaded library."""
+    return int(load_library().kf_hit_record_floats())
+
+
 @dataclass
 class Geometry:
     """Concentric cylinders in a uniform solenoid field (host-side numbers)."""
@@ -242,7 +249,7 @@ class Bins:
     eta_max: float
     bin_offset: torch.Tensor      # int32 [n_eta*n_phi + 1]
     sorted_to_orig: torch.Tensor  # int32 [n_hits]
-    hit_rec: torch.Tensor         # f32 [n_hits][12] packed records in bin order
+    hit_rec: torch.Tensor         # f32 [n_hits][hit_record_floats()] packed records in bin order
     bin_box: torch.Tensor         # f32 [n_bins][8] per-bin bounds
     orig_to_sorted: torch.Tensor  # int32 [n_hits] inverse of sorted_to_orig
     pos_sorted: torch.Tensor | None = None   # f32 [3][ld] optional SoA copy
@@ -254,7 +261,7 @@ class Bins:
         return Bins(n_eta, n_phi, eta_max,
                     torch.empty(n_eta * n_phi + 1, dtype=torch.int32, device=device),
                     torch.empty(max(n_hits, 1), dtype=torch.int32, device=device),
-                    torch.empty((max(n_hits, 1), 12), dtype=torch.float32, device=device),
+                    torch.empty((max(n_hits, 1), hit_record_floats()), dtype=torch.float32, device=device),
                     torch.empty((n_eta * n_phi, 8), dtype=torch.float32, device=device),
                     torch.empty(max(n_hits, 1), dtype=torch.int32, device=device),
                     torch.empty((3, ld), dtype=torch.float32, device=device) if soa else None,

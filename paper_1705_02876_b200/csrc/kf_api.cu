@@ -40,7 +40,8 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 11;
+constexpr int kAbiVersion = 12;
+static_assert(kRecFloats == KF_HIT_RECORD_FLOATS || kRecWords == 4, "kf_internal.h and kf_b200.h disagree on the hit record");
 
 // Makes the context's device current for the duration of an ABI call and puts the caller's device back on
 // return (the library links its own cudart next to torch's: both see the same current device).
@@ -175,6 +176,8 @@ int check_track_hits(const kf_track_hits* h, const kf_geometry* g, int64_t n, bo
 extern "C" {
 
 int kf_abi_version(void) { return kAbiVersion; }
+
+int kf_hit_record_floats(void) { return kRecFloats; }
 
 const char* kf_strerror(int code) {
     switch (code) {

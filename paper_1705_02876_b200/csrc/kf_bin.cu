@@ -166,10 +166,11 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     const float4* src = reinterpret_cast<const float4*>(L.rec_tmp + p * 12);
     const float4 A = src[0], Bw = src[1], C = src[2];
     if (L.hit_rec) {
-        float4* rec = reinterpret_cast<float4*>(L.hit_rec + dst * 12);
+        float4* rec = reinterpret_cast<float4*>(L.hit_rec + dst * kRecFloats);
         rec[0] = A;
         rec[1] = Bw;
         rec[2] = C;
+        if (kRecWords == 4) rec[3] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     }
     if (L.hit_rec) return;   // the SoA copies are then written from the final records, coalesced (bin_finish_kernel)
     if (L.pos_sorted) {
@@ -199,13 +200,13 @@ bin_finish_kernel(const __grid_constant__ BinBatch B) {
     float xl = inf, xh = -inf, yl = inf, yh = -inf, zl = inf, zh = -inf, vz = 0.0f, vt = 0.0f;
     const float4* rec = reinterpret_cast<const float4*>(L.hit_rec);
     for (int32_t s = s0 + lane; s < s1; s += 32) {
-        const float4 A = rec[(int64_t)s * 3], Bw = rec[(int64_t)s * 3 + 1];
+        const float4 A = rec[(int64_t)s * kRecWords], Bw = rec[(int64_t)s * kRecWords + 1];
         L.sorted_to_orig[s] = __float_as_int(Bw.w);
         if (L.pos_sorted) {
             L.pos_sorted[s] = A.x; L.pos_sorted[L.ld_out + s] = A.y; L.pos_sorted[2 * L.ld_out + s] = A.z;
         }
         if (L.cov_sorted) {   // xx xy xz yy yz zz
-            const float4 C = rec[(int64_t)s * 3 + 2];
+            const float4 C = rec[(int64_t)s * kRecWords + 2];
             L.cov_sorted[s] = Bw.x;                 L.cov_sorted[L.ld_out + s] = Bw.y;
             L.cov_sorted[2 * L.ld_out + s] = C.x;   L.cov_sorted[3 * L.ld_out + s] = Bw.z;
             L.cov_sorted[4 * L.ld_out + s] = C.y;   L.cov_sorted[5 * L.ld_out + s] = A.w;
@@ -228,25 +229,66 @@ bin_finish_kernel(const __grid_constant__ BinBatch B) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Chunked form of the same stable counting sort for hit pools (four launches + the finish step, every record
+// Chunked form of the same stable counting sort for hit pools (three launches + the finish step, every record
 // written ONCE): a layer is cut into chunks of kChunk consecutive hits, one CTA per chunk.
 //   chunk_count   bin of every hit; shared-memory histogram of the chunk; bucket lists in shared memory; every hit
 //                 counts the smaller indices of its bucket = its stable rank INSIDE the chunk (the arrival order of
-//                 the shared-memory atomics never shows); key, rank and the chunk's histogram go to global memory
+//                 the shared-memory atomics never shows); one word per hit (bin << 16 | rank) and the chunk's
+//                 histogram go to global memory.  512 threads x 4 hits: the kernel is one wave of CTAs and its
+//                 duration the ~370-instruction-per-hit chain of a warp, so fewer hits per thread = a shorter kernel
 //   chunk_prefix  per bin: prefix of the chunk histograms over the chunks (chunks are consecutive index ranges, so
-//                 earlier chunk = smaller index) and the bin total; bin_scan_kernel then gives bin_offset
-//   chunk_place   final slot = bin_offset[bin] + hits of the bin in earlier chunks + rank inside the chunk; the nine
-//                 values are read coalesced and the packed record goes straight to its final place
+//                 earlier chunk = smaller index) and the bin total; four warps per column, a quarter of the chunks
+//                 each, so that a whole column is in flight at once
+//   chunk_place   every CTA scans the bin totals itself (-> bin_offset, handed to the caller by chunk 0); final slot
+//                 = bin_offset[bin] + hits of the bin in earlier chunks + rank inside the chunk; the nine values are
+//                 read coalesced, four hits in flight per thread, and the packed record goes straight to its final place
 // Same results as the five-launch path, bit for bit.  Limits: n_bins <= kChunkMaxBins (shared memory).
+// Measured on configs[4] (7 x 120 000 hits, graph replay, no SoA copies), warm incremental cost per kernel:
+// count 17.7, prefix 3.5, place 16.2, finish 8.6 us = 46 us (round-2 start: 19.5 / 8.2 (+ scan) / 13.9 / 8.6 = 50).
 #ifndef KF_BIN_CHUNK
 #define KF_BIN_CHUNK 2048
 #endif
+
+// In-place exclusive scan of a[0 .. n) in shared memory by a block of THREADS threads (thread t owns a contiguous
+// range); returns the total to every thread.  wsum: THREADS / 32 words of shared memory.  Ends with a barrier.
+template <int THREADS>
+__device__ __forceinline__ int32_t block_exclusive_scan(int32_t* a, int n, int32_t* wsum) {
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int per = (n + THREADS - 1) / THREADS;
+    const int r0 = tid * per < n ? tid * per : n, r1 = r0 + per < n ? r0 + per : n;
+    int32_t sum = 0;
+    for (int i = r0; i < r1; ++i) sum += a[i];
+    int32_t incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int32_t o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+    }
+    if (lane == 31) wsum[wid] = incl;
+    __syncthreads();
+    int32_t run = incl - sum, total = 0;
+#pragma unroll
+    for (int w = 0; w < THREADS / 32; ++w) {
+        const int32_t v = wsum[w];
+        run += w < wid ? v : 0;
+        total += v;
+    }
+    for (int i = r0; i < r1; ++i) { const int32_t c = a[i]; a[i] = run; run += c; }
+    __syncthreads();
+    return total;
+}
 constexpr int kChunk = KF_BIN_CHUNK;
-constexpr int kChunkBlock = kChunk / 8;
+constexpr int kChunkBlock = kChunk / 8;     // chunk_place_kernel: 8 hits per thread
 constexpr int kChunkPer = kChunk / kChunkBlock;
+#ifndef KF_BIN_COUNT_PER
+#define KF_BIN_COUNT_PER 4
+#endif
+constexpr int kCountPer = KF_BIN_COUNT_PER;  // chunk_count_kernel: hits per thread.  The kernel is one wave of CTAs and a warp runs
+constexpr int kCountBlock = kChunk / kCountPer;   // ~370 instructions per hit one after the other, so its duration is the
+                                                  // length of that chain: 4 hits per thread (512 threads) instead of 8
 constexpr int kChunkMaxBins = 8192;
 
-__global__ void __launch_bounds__(kChunkBlock)
+__global__ void __launch_bounds__(kCountBlock)
 chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__ eta_edge_g,
                    const float* __restrict__ phi_cos_g, const float* __restrict__ phi_sin_g) {
     const BinLayerDev& L = B.layer[blockIdx.y];
@@ -264,27 +306,27 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
     float* eta_edge = reinterpret_cast<float*>(bucket + kChunk);       // [n_eta] [n_phi] [n_phi]
     float* phi_cos = eta_edge + B.n_eta;
     float* phi_sin = phi_cos + B.n_phi;
-    __shared__ int32_t wsum[kChunkBlock / 32];
-    for (int i = tid; i < nb; i += kChunkBlock) cnt[i] = 0;
-    for (int i = tid; i < B.n_eta; i += kChunkBlock) eta_edge[i] = eta_edge_g[i];
-    for (int i = tid; i < B.n_phi; i += kChunkBlock) { phi_cos[i] = phi_cos_g[i]; phi_sin[i] = phi_sin_g[i]; }
+    __shared__ int32_t wsum[kCountBlock / 32];
+    for (int i = tid; i < nb; i += kCountBlock) cnt[i] = 0;
+    for (int i = tid; i < B.n_eta; i += kCountBlock) eta_edge[i] = eta_edge_g[i];
+    for (int i = tid; i < B.n_phi; i += kCountBlock) { phi_cos[i] = phi_cos_g[i]; phi_sin[i] = phi_sin_g[i]; }
     __syncthreads();
-    // The bin rule of bin_of_hit for this thread's kChunkPer hits at once: all loads first, then the two searches
+    // The bin rule of bin_of_hit for this thread's kCountPer hits at once: all loads first, then the two searches
     // as descents in powers of two (same answer as the bisection for a monotone predicate; the trip count depends on
     // the grid only, so the hits' dependent look-ups interleave instead of running one hit after the other).
     {
-        float x[kChunkPer], y[kChunkPer], u[kChunkPer];
-        int pe[kChunkPer], pp[kChunkPer], lim[kChunkPer];
+        float x[kCountPer], y[kCountPer], u[kCountPer];
+        int pe[kCountPer], pp[kCountPer], lim[kCountPer];
         const int half = B.n_phi >> 1;
 #pragma unroll
-        for (int it = 0; it < kChunkPer; ++it) {
-            const int li = tid + it * kChunkBlock;
+        for (int it = 0; it < kCountPer; ++it) {
+            const int li = tid + it * kCountBlock;
             const int64_t h = h0 + (li < m ? li : 0);
             x[it] = __ldg(L.pos + h); y[it] = __ldg(L.pos + L.ld_in + h);
             u[it] = __ldg(L.pos + 2 * L.ld_in + h);
         }
 #pragma unroll
-        for (int it = 0; it < kChunkPer; ++it) {
+        for (int it = 0; it < kCountPer; ++it) {
             u[it] = __fdiv_rn(u[it], L.radius);
             const bool upper = y[it] > 0.0f || (y[it] == 0.0f && x[it] > 0.0f);
             pe[it] = 0;
@@ -295,7 +337,7 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
         while (top * 2 <= B.n_eta - 1) top *= 2;
         for (int step = top; step > 0; step >>= 1) {
 #pragma unroll
-            for (int it = 0; it < kChunkPer; ++it) {
+            for (int it = 0; it < kCountPer; ++it) {
                 const int t = pe[it] + step;
                 if (t <= B.n_eta - 1 && u[it] >= eta_edge[t]) pe[it] = t;
             }
@@ -304,14 +346,14 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
         while (top * 2 <= half) top *= 2;
         for (int step = top; step > 0; step >>= 1) {
 #pragma unroll
-            for (int it = 0; it < kChunkPer; ++it) {
+            for (int it = 0; it < kCountPer; ++it) {
                 const int t = pp[it] + step;
                 if (t <= lim[it] && __fmul_rn(phi_cos[t], y[it]) >= __fmul_rn(phi_sin[t], x[it])) pp[it] = t;
             }
         }
 #pragma unroll
-        for (int it = 0; it < kChunkPer; ++it) {
-            const int li = tid + it * kChunkBlock;
+        for (int it = 0; it < kCountPer; ++it) {
+            const int li = tid + it * kCountBlock;
             if (li < m) {
                 const int b = pe[it] * B.n_phi + pp[it];
                 ka[li] = ((uint32_t)b << 16) | (uint32_t)atomicAdd(cnt + b, 1);
@@ -320,7 +362,7 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
     }
     __syncthreads();
     // exclusive scan of cnt -> loc: thread t owns the bins [r0, r1)
-    const int per = (nb + kChunkBlock - 1) / kChunkBlock;
+    const int per = (nb + kCountBlock - 1) / kCountBlock;
     const int r0 = tid * per < nb ? tid * per : nb, r1 = r0 + per < nb ? r0 + per : nb;
     int32_t sum = 0;
     for (int b = r0; b < r1; ++b) { loc[b] = sum; sum += cnt[b]; }
@@ -333,107 +375,157 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
     if (lane == 31) wsum[wid] = incl;
     __syncthreads();
     if (wid == 0) {
-        int32_t w = lane < kChunkBlock / 32 ? wsum[lane] : 0;
+        int32_t w = lane < kCountBlock / 32 ? wsum[lane] : 0;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             const int32_t o = __shfl_up_sync(0xffffffffu, w, d);
             if (lane >= d) w += o;
         }
-        if (lane < kChunkBlock / 32) wsum[lane] = w;   // inclusive over warps
+        if (lane < kCountBlock / 32) wsum[lane] = w;   // inclusive over warps
     }
     __syncthreads();
     const int32_t excl = (wid ? wsum[wid - 1] : 0) + incl - sum;
     for (int b = r0; b < r1; ++b) loc[b] += excl;
     __syncthreads();
 #pragma unroll
-    for (int it = 0; it < kChunkPer; ++it) {
-        const int li = tid + it * kChunkBlock;
+    for (int it = 0; it < kCountPer; ++it) {
+        const int li = tid + it * kCountBlock;
         if (li < m) { const uint32_t k = ka[li]; bucket[loc[k >> 16] + (int)(k & 0xffffu)] = (uint16_t)li; }
     }
     __syncthreads();
 #pragma unroll
-    for (int it = 0; it < kChunkPer; ++it) {
-        const int li = tid + it * kChunkBlock;
+    for (int it = 0; it < kCountPer; ++it) {
+        const int li = tid + it * kCountBlock;
         if (li < m) {
             const int b = (int)(ka[li] >> 16);
             const int s0 = loc[b], s1 = s0 + cnt[b];
             int rank = 0;
             for (int j = s0; j < s1; ++j) rank += bucket[j] < (uint16_t)li ? 1 : 0;
-            L.key[h0 + li] = b;
-            L.pib[h0 + li] = rank;
+            L.key[h0 + li] = (b << 16) | rank;     // one word per hit for chunk_place_kernel (rank < kChunk <= 65536, b < 8192)
         }
     }
-    for (int b = tid; b < nb; b += kChunkBlock) L.chunk_cnt[(int64_t)c * nb + b] = cnt[b];   // [chunk][bin]
+    for (int b = tid; b < nb; b += kCountBlock) L.chunk_cnt[(int64_t)c * nb + b] = cnt[b];   // [chunk][bin]
 }
 
 // A thread per bin: chunk_cnt[c][b] becomes the number of hits of bin b in chunks before c (sixteen independent
-// loads in flight at a time); the bin total goes to counts[b], which bin_scan_kernel turns into bin_offset.
+// loads in flight at a time); the bin total goes to counts[b].  bin_offset = the exclusive scan of the totals is
+// made by every CTA of chunk_place_kernel for itself (a microsecond of a kernel that has to read the totals anyway;
+// as a launch of its own, one CTA per layer, it took 5 us, and as the last-CTA-done tail of this kernel 3.5 us).
 __global__ void __launch_bounds__(128)
 chunk_prefix_kernel(const __grid_constant__ BinBatch B) {
     const BinLayerDev& L = B.layer[blockIdx.y];
     const int nb = B.n_eta * B.n_phi;
     const int nc = (int)((L.n + kChunk - 1) / kChunk);
-    const int b = blockIdx.x * 128 + threadIdx.x;
-    if (b >= nb) return;
-    int32_t* col = L.chunk_cnt + b;            // [chunk][bin]: neighbouring threads, neighbouring words
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    // A CTA owns 32 bins; warp g takes the g-th quarter of the chunks (a contiguous range, so the four partial
+    // prefixes chain through shared memory): the column of a bin is read by four threads at once and a whole
+    // quarter of it is in flight per thread -- one round trip to L2 instead of four for configs[4]'s 59 chunks.
+    const int b = blockIdx.x * 32 + lane;
+    const int Q = (nc + 3) / 4;
+    const int c_lo = wid * Q < nc ? wid * Q : nc, c_hi = c_lo + Q < nc ? c_lo + Q : nc;
+    __shared__ int32_t part[4][32];
     int32_t tot = 0;
-    for (int c0 = 0; c0 < nc; c0 += 16) {
-        int32_t v[16];
+    if (b < nb) {
+        int32_t* col = L.chunk_cnt + b;            // [chunk][bin]: neighbouring lanes, neighbouring words
+        for (int c0 = c_lo; c0 < c_hi; c0 += 16) {
+            int32_t v[16];
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = c0 + k < nc ? col[(int64_t)(c0 + k) * nb] : 0;
+            for (int k = 0; k < 16; ++k) v[k] = c0 + k < c_hi ? col[(int64_t)(c0 + k) * nb] : 0;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            if (c0 + k < nc) col[(int64_t)(c0 + k) * nb] = tot;
-            tot += v[k];
+            for (int k = 0; k < 16; ++k) tot += v[k];
         }
     }
-    L.counts[b] = tot;
+    part[wid][lane] = tot;
+    __syncthreads();
+    if (b < nb) {
+        int32_t run = 0;
+        for (int g = 0; g < wid; ++g) run += part[g][lane];
+        int32_t* col = L.chunk_cnt + b;
+        for (int c0 = c_lo; c0 < c_hi; c0 += 16) {   // second pass over the quarter: the words are in L1 / L2 now
+            int32_t v[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) v[k] = c0 + k < c_hi ? col[(int64_t)(c0 + k) * nb] : 0;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                if (c0 + k < c_hi) col[(int64_t)(c0 + k) * nb] = run;
+                run += v[k];
+            }
+        }
+        if (wid == 3) L.counts[b] = part[0][lane] + part[1][lane] + part[2][lane] + part[3][lane];
+    }
 }
 
-__global__ void __launch_bounds__(kChunkBlock)
+__global__ void __launch_bounds__(kChunkBlock, 4)
 chunk_place_kernel(const __grid_constant__ BinBatch B) {
     const BinLayerDev& L = B.layer[blockIdx.y];
     const int c = blockIdx.x;
     const int64_t h0 = (int64_t)c * kChunk;
-    if (h0 >= L.n) return;
-    const int m = (int)(L.n - h0 < kChunk ? L.n - h0 : kChunk);
+    if (h0 >= L.n && c != 0) return;                         // (chunk 0 of an EMPTY layer still owes the caller bin_offset)
+    const int m = h0 >= L.n ? 0 : (int)(L.n - h0 < kChunk ? L.n - h0 : kChunk);
     const int nb = B.n_eta * B.n_phi;
     const int tid = threadIdx.x;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int32_t* base = reinterpret_cast<int32_t*>(smem_raw);   // [nb] final slot of this chunk's first hit of a bin
-    // Per warp: 32 records staged in shared memory and written out three lanes to a record, so that one store
-    // instruction covers whole 48-byte records (2 sectors each) instead of 32 separate 16-byte pieces.
-    __shared__ __align__(16) float4 stage[kChunkBlock / 32][32 * 3];
+    // Per warp: 32 records staged in shared memory and written out kRecWords lanes to a record, so that one store
+    // instruction covers whole records (with 64-byte records: two whole sectors each) instead of 32 separate
+    // 16-byte pieces.
+    __shared__ __align__(16) float4 stage[kChunkBlock / 32][32 * kRecWords];
     __shared__ int32_t stage_dst[kChunkBlock / 32][32];
     const int lane = tid & 31, wid = tid >> 5;
-    for (int b = tid; b < nb; b += kChunkBlock) base[b] = L.bin_offset[b] + L.chunk_cnt[(int64_t)c * nb + b];
+    __shared__ int32_t wsum[kChunkBlock / 32];
+    for (int b = tid; b < nb; b += kChunkBlock) base[b] = L.counts[b];      // the layer's hits per bin (chunk_prefix_kernel)
     __syncthreads();
+    const int32_t total = block_exclusive_scan<kChunkBlock>(base, nb, wsum);     // = bin_offset
+    if (c == 0) {                                                           // one CTA per layer hands it to the caller
+        for (int b = tid; b < nb; b += kChunkBlock) L.bin_offset[b] = base[b];
+        if (tid == 0) L.bin_offset[nb] = total;
+    }
+    if (m == 0) return;
+    __syncthreads();
+    for (int b = tid; b < nb; b += kChunkBlock) base[b] += L.chunk_cnt[(int64_t)c * nb + b];
+    __syncthreads();
+    // The loads of kPlaceBatch hits (9 values + the key word each) are issued together: the kernel is one wave of
+    // CTAs, so its duration is a CTA's latency, and eight dependent round trips to memory were most of it.  Four at
+    // a time keeps the kernel at 64 registers = 4 CTAs per SM = every chunk of configs[4] resident at once (all
+    // eight at a time: 128 registers, two waves, slower on configs[4] although faster beyond the L2 size).
+    constexpr int kPlaceBatch = 4;
+    static_assert(kChunkPer % kPlaceBatch == 0, "chunk_place_kernel batches");
+    for (int it0 = 0; it0 < kChunkPer; it0 += kPlaceBatch) {
+        float v[kPlaceBatch][9];
+        int32_t kr[kPlaceBatch];
 #pragma unroll
-    for (int it = 0; it < kChunkPer; ++it) {
-        const int li = tid + it * kChunkBlock;        // (a warp's 32 hits are consecutive)
-        int32_t dst = -1;
-        if (li < m) {
-            const int64_t h = h0 + li;
-            dst = base[__ldg(L.key + h)] + __ldg(L.pib + h);   // (written by the launch before)
-            if (L.orig_to_sorted) L.orig_to_sorted[h] = dst;
-            float v[9];
+        for (int j = 0; j < kPlaceBatch; ++j) {
+            const int li = tid + (it0 + j) * kChunkBlock;        // (a warp's 32 hits are consecutive)
+            const int64_t h = h0 + (li < m ? li : 0);
+            kr[j] = __ldg(L.key + h);                            // bin << 16 | rank inside the chunk (chunk_count_kernel)
 #pragma unroll
-            for (int k = 0; k < 3; ++k) v[k] = __ldg(L.pos + k * L.ld_in + h);
+            for (int k = 0; k < 3; ++k) v[j][k] = __ldg(L.pos + k * L.ld_in + h);
 #pragma unroll
-            for (int k = 0; k < 6; ++k) v[3 + k] = __ldg(L.cov + k * L.ld_in + h);
-            stage[wid][lane * 3 + 0] = make_float4(v[0], v[1], v[2], v[8]);                          // x y z vzz
-            stage[wid][lane * 3 + 1] = make_float4(v[3], v[4], v[6], __int_as_float((int32_t)h));    // vxx vxy vyy, index
-            stage[wid][lane * 3 + 2] = make_float4(v[5], v[7], 0.0f, 0.0f);                          // vxz vyz
+            for (int k = 0; k < 6; ++k) v[j][3 + k] = __ldg(L.cov + k * L.ld_in + h);
         }
-        stage_dst[wid][lane] = dst;
-        __syncwarp();
 #pragma unroll
-        for (int r = 0; r < 3; ++r) {
-            const int w = r * 32 + lane, rec = w / 3, part = w - rec * 3;
-            const int32_t d = stage_dst[wid][rec];
-            if (d >= 0) reinterpret_cast<float4*>(L.hit_rec + (int64_t)d * 12)[part] = stage[wid][w];
+        for (int j = 0; j < kPlaceBatch; ++j) {
+            const int li = tid + (it0 + j) * kChunkBlock;
+            int32_t dst = -1;
+            if (li < m) {
+                const int64_t h = h0 + li;
+                dst = base[kr[j] >> 16] + (kr[j] & 0xffff);
+                if (L.orig_to_sorted) L.orig_to_sorted[h] = dst;
+                stage[wid][lane * kRecWords + 0] = make_float4(v[j][0], v[j][1], v[j][2], v[j][8]);                       // x y z vzz
+                stage[wid][lane * kRecWords + 1] = make_float4(v[j][3], v[j][4], v[j][6], __int_as_float((int32_t)h));    // vxx vxy vyy, index
+                stage[wid][lane * kRecWords + 2] = make_float4(v[j][5], v[j][7], 0.0f, 0.0f);                             // vxz vyz
+                if (kRecWords == 4) stage[wid][lane * kRecWords + 3] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            }
+            stage_dst[wid][lane] = dst;
+            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < kRecWords; ++r) {
+                const int w = r * 32 + lane, rec = w / kRecWords, part = w - rec * kRecWords;
+                const int32_t d = stage_dst[wid][rec];
+                if (d >= 0) reinterpret_cast<float4*>(L.hit_rec + (int64_t)d * kRecFloats)[part] = stage[wid][w];
+            }
+            __syncwarp();
         }
-        __syncwarp();
     }
 }
 
@@ -601,9 +693,8 @@ cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max,
         chunks += (B.layer[j].n + kChunk - 1) / kChunk;
     }
     const dim3 grid((unsigned)nc, (unsigned)m);
-    chunk_count_kernel<<<grid, kChunkBlock, chunk_count_smem(B.n_eta, B.n_phi), stream>>>(B, s.eta_edge, s.phi_cos, s.phi_sin);
-    chunk_prefix_kernel<<<dim3((unsigned)((nb + 127) / 128), (unsigned)m), 128, 0, stream>>>(B);
-    bin_scan_kernel<<<dim3(1, m), 1024, 0, stream>>>(B);
+    chunk_count_kernel<<<grid, kCountBlock, chunk_count_smem(B.n_eta, B.n_phi), stream>>>(B, s.eta_edge, s.phi_cos, s.phi_sin);
+    chunk_prefix_kernel<<<dim3((unsigned)((nb + 31) / 32), (unsigned)m), 128, 0, stream>>>(B);
     chunk_place_kernel<<<grid, kChunkBlock, (size_t)nb * 4, stream>>>(B);
     bin_finish_kernel<<<dim3((unsigned)((nb * 32 + kBlock - 1) / kBlock), (unsigned)m), kBlock, 0, stream>>>(B);
     *done = true;

@@ -199,13 +199,13 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
             const int src = __ffs(kept) - 1;
             kept &= kept - 1;
             const int32_t b0 = __shfl_sync(0xffffffffu, s0, src), b1 = __shfl_sync(0xffffffffu, s1, src);
-            const float4* p = rec + (int64_t)(b0 + lane) * 3;
-            for (int32_t sb = b0; sb < b1; sb += 64, p += 64 * 3) {
+            const float4* p = rec + (int64_t)(b0 + lane) * kRecWords;
+            for (int32_t sb = b0; sb < b1; sb += 64, p += 64 * kRecWords) {
                 const int32_t sA = sb + lane, sB = sA + 32;
                 const bool vA = sA < b1, vB = sB < b1;
                 float4 A0 = make_float4(0.f, 0.f, 0.f, 0.f), B0 = A0, A1 = A0, B1 = A0;
                 if (vA) { A0 = __ldg(p); B0 = __ldg(p + 1); }
-                if (vB) { A1 = __ldg(p + 96); B1 = __ldg(p + 97); }
+                if (vB) { A1 = __ldg(p + 32 * kRecWords); B1 = __ldg(p + 32 * kRecWords + 1); }
                 const float dz0 = A0.z - c.zn, dz1 = A1.z - c.zn;
                 const float rt0 = c.ec * (A0.y - c.yn) - c.es * (A0.x - c.xn);
                 const float rt1 = c.ec * (A1.y - c.yn) - c.es * (A1.x - c.xn);

@@ -840,7 +840,7 @@ __device__ __forceinline__ int32_t resolve_hit(const IndexedPools& H, int l, int
 __device__ __forceinline__ Hit fetch_hit(const IndexedPools& H, int l, int32_t s) {
     Hit m;
     if (H.use_records) {   // one 48-byte record (2 sectors) instead of 9 scattered sectors
-        const float4* r = reinterpret_cast<const float4*>(H.hit_rec[l]) + (int64_t)s * 3;
+        const float4* r = reinterpret_cast<const float4*>(H.hit_rec[l]) + (int64_t)s * kRecWords;
         const float4 A = __ldg(r), B = __ldg(r + 1), C = __ldg(r + 2);
         m.x = A.x; m.y = A.y; m.z = A.z; m.vzz = A.w; m.vxx = B.x; m.vxy = B.y; m.vyy = B.z; m.vxz = C.x; m.vyz = C.y;
         return m;

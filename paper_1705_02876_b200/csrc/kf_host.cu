@@ -167,7 +167,7 @@ cudaError_t build_best_hit_host(BuildHostStage& hs, BinScratch& bs, ScoreScratch
         if (ldh[j] < 4) ldh[j] = 4;
         o_pos[j] = take((size_t)3 * ldh[j] * 4); o_hcov[j] = take((size_t)6 * ldh[j] * 4);
         o_off[j] = take((size_t)(nb + 1) * 4); o_s2o[j] = take((size_t)ldh[j] * 4);
-        o_rec[j] = take((size_t)ldh[j] * 48); o_box[j] = take((size_t)nb * 32);
+        o_rec[j] = take((size_t)ldh[j] * kRecFloats * 4); o_box[j] = take((size_t)nb * 32);
     }
     cudaError_t e = cudaStreamSynchronize(stream);       // the staging buffers may still serve the previous call
     if (e != cudaSuccess) return e;

@@ -85,7 +85,7 @@ struct HostStage {
 
 // ---------------------------------------------------------------------------------- binning
 constexpr int KF_MAX_BINS_INTERNAL = 65536;
-constexpr int kBinBatchMax = 16;  // layers per group of launches
+constexpr int kBinBatchMax = 32;  // layers per group of launches (the descriptors travel as one 4.4 KB kernel parameter)
 
 struct BinArgs {
     int64_t n_hits, ld_in;
@@ -150,8 +150,49 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
                          const int8_t* q, int n_eta, int n_phi, float eta_max, int32_t* order,
                          cudaStream_t stream);
 
+// ---------------------------------------------------------------------------------- dependent launches
+// The building and binning calls are chains of 4 - 30 short kernels, each reading what the one before wrote; at
+// event size a kernel boundary (drain, launch, ramp) costs 2 - 3 us of a 5 - 15 us kernel.  With programmatic
+// dependent launch the next kernel of the chain is scheduled while the current one is still running: every kernel
+// of a chain starts with pdl_start() -- `launch_dependents` lets the NEXT grid's CTAs take free slots as soon as all
+// CTAs of this grid have started, `wait` holds this grid until the PREVIOUS grid has completed and its writes are
+// visible -- and is launched with launch_chained().  Nothing is read or written before pdl_start(), so the order
+// of all memory effects is that of plain stream order.  A kernel launched the plain way runs both instructions as
+// no-ops.  Recorded in a graph (kf_graph_begin) the launches become programmatic edges.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_start() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+#endif
+
+template <class... KArgs, class... Args>
+inline cudaError_t launch_chained(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                                  Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---------------------------------------------------------------------------------- scoring
 constexpr int kScorePlanes = 29;
+
+// Packed hit record of kf_bin_hits (kf_layer_bins.hit_rec): kRecWords 16-byte words per hit,
+//   x y z vzz | vxx vxy vyy index | vxz vyz 0 0 [ | 0 0 0 0 ].
+// Three words = 48 bytes is what the library ships.  Four words (a 64-byte record = two whole, aligned sectors,
+// written once by four lanes, the pre-filters' two words in its first sector) is a build option
+// (-DKF_REC_WORDS=4) kept for measurements: on configs[4] (everything L2-resident) it LOST everywhere -- binning
+// 49.8 -> 58.8 us, best-hit building 177 -> 203 us, combinatorial 824 -> 899 us (a third more bytes through L2 per
+// hit scanned) -- and only won once the pools no longer fit in L2 (binning 28 x 120 000 hits: 241 -> 212 us).
+#ifndef KF_REC_WORDS
+#define KF_REC_WORDS 3
+#endif
+constexpr int kRecWords = KF_REC_WORDS;
+constexpr int kRecFloats = 4 * kRecWords;
 
 struct BinGrid { int n_eta, n_phi; float eta_max; };
 

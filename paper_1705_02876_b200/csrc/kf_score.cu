@@ -61,6 +61,7 @@ __device__ __forceinline__ void apply_decision(const ScoreArgs& a, int64_t i, Tr
 // First step: global-frame candidate -> local frame -> propagate to `layer`.
 __global__ void __launch_bounds__(kCandBlock)
 propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, int layer, int keep_track) {
+    pdl_start();
     const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
     if (i >= a.n) return;
     const int q = a.q[i];
@@ -86,6 +87,7 @@ propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
 template <bool MULTI>
 __global__ void __launch_bounds__(kCandBlock)
 update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, int layer) {
+    pdl_start();
     const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
     if (i >= a.n) return;
     const int32_t f = a.flag[i];
@@ -106,6 +108,7 @@ update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
 template <bool MULTI>
 __global__ void __launch_bounds__(kCandBlock)
 update_global_kernel(const ScoreArgs a, int have_track) {
+    pdl_start();
     const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
     if (i >= a.n) return;
     const int32_t f = a.flag[i];
@@ -125,6 +128,7 @@ update_global_kernel(const ScoreArgs a, int have_track) {
 template <bool MULTI>
 __global__ void __launch_bounds__(kScanBlock)
 scan_kernel(const ScoreArgs a, float inv_r) {
+    pdl_start();
     __shared__ int32_t survivors[kScanBlock / 32][96];
     const int lane = threadIdx.x & 31;
     const int64_t w = ((int64_t)blockIdx.x * kScanBlock + threadIdx.x) >> 5;
@@ -190,13 +194,13 @@ scan_kernel(const ScoreArgs a, float inv_r) {
             kept &= kept - 1;
             const int32_t b0 = __shfl_sync(0xffffffffu, s0, src), b1 = __shfl_sync(0xffffffffu, s1, src);
             // 64 hits per step: two records per lane, four independent 128-bit loads in flight
-            const float4* p = rec + (int64_t)(b0 + lane) * 3;
-            for (int32_t sb = b0; sb < b1; sb += 64, p += 64 * 3) {   // warp-uniform trip count
+            const float4* p = rec + (int64_t)(b0 + lane) * kRecWords;
+            for (int32_t sb = b0; sb < b1; sb += 64, p += 64 * kRecWords) {   // warp-uniform trip count
                 const int32_t sA = sb + lane, sB = sA + 32;
                 const bool vA = sA < b1, vB = sB < b1;
                 float4 A0 = make_float4(0.f, 0.f, 0.f, 0.f), B0 = A0, A1 = A0, B1 = A0;
                 if (vA) { A0 = __ldg(p); B0 = __ldg(p + 1); }
-                if (vB) { A1 = __ldg(p + 96); B1 = __ldg(p + 97); }
+                if (vB) { A1 = __ldg(p + 32 * kRecWords); B1 = __ldg(p + 32 * kRecWords + 1); }
                 const float dz0 = A0.z - c.zn, dz1 = A1.z - c.zn;
                 const float rt0 = c.ec * (A0.y - c.yn) - c.es * (A0.x - c.xn);
                 const float rt1 = c.ec * (A1.y - c.yn) - c.es * (A1.x - c.xn);
@@ -284,21 +288,25 @@ cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n
     const unsigned sblocks = (unsigned)((a.n + kScanBlock / 32 - 1) / (kScanBlock / 32));
     const int keep = n_steps > 1 ? 1 : 0;
     const bool multi = a.ev.n > 1;
+    const dim3 cgrid(cblocks), sgrid(sblocks), cblock(kCandBlock), sblock(kScanBlock);
+    cudaError_t e2 = cudaSuccess;
+    auto ok = [&](cudaError_t r) { if (e2 == cudaSuccess) e2 = r; };
     for (int j = 0; j < n_steps; ++j) {
         const ScoreStep& st = steps[j];
-        if (j == 0) propagate_global_kernel<<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer, keep);
-        else if (multi) update_propagate_kernel<true><<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer);   // a.hit_rec still step j-1
-        else update_propagate_kernel<false><<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer);
+        if (j == 0) ok(launch_chained(propagate_global_kernel, cgrid, cblock, 0, stream, P, a, st.layer, keep));
+        else if (multi) ok(launch_chained(update_propagate_kernel<true>, cgrid, cblock, 0, stream, P, a, st.layer));   // a.hit_rec still step j-1
+        else ok(launch_chained(update_propagate_kernel<false>, cgrid, cblock, 0, stream, P, a, st.layer));
         a.hit_rec = st.hit_rec; a.bin_box = st.bin_box; a.bin_offset = st.bin_offset; a.n_hits = st.n_hits;
         a.best_hit = st.best_hit; a.best_chi2 = st.best_chi2;
         for (int e = 0; e < a.ev.n; ++e) {
             a.ev.hit_rec[e] = st.ev_hit_rec[e]; a.ev.bin_box[e] = st.ev_bin_box[e]; a.ev.bin_offset[e] = st.ev_bin_offset[e];
         }
-        if (multi) scan_kernel<true><<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
-        else scan_kernel<false><<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
+        if (multi) ok(launch_chained(scan_kernel<true>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r));
+        else ok(launch_chained(scan_kernel<false>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r));
     }
-    if (multi) update_global_kernel<true><<<cblocks, kCandBlock, 0, stream>>>(a, keep);
-    else update_global_kernel<false><<<cblocks, kCandBlock, 0, stream>>>(a, keep);
+    if (multi) ok(launch_chained(update_global_kernel<true>, cgrid, cblock, 0, stream, a, keep));
+    else ok(launch_chained(update_global_kernel<false>, cgrid, cblock, 0, stream, a, keep));
+    if (e2 != cudaSuccess) return e2;
     return cudaGetLastError();
 }
 

@@ -54,7 +54,7 @@ __device__ __forceinline__ void get_scratch(const float* __restrict__ sc, int64_
 // covariance is identically zero after the first layer).
 __device__ __forceinline__ void hit_from_record(const float4* __restrict__ rec, int32_t slot, const Crossing& o,
                                                 LocalHit& h) {
-    const float4* r0 = rec + (int64_t)slot * 3;
+    const float4* r0 = rec + (int64_t)slot * kRecWords;
     const float4 A = __ldg(r0), B = __ldg(r0 + 1), C = __ldg(r0 + 2);
     hit_to_local(o, A.x, A.y, A.z, B.x, B.y, C.x, B.z, C.y, A.w, h);
 }
@@ -133,7 +133,7 @@ struct ScanCand {       // what the scan needs of the propagated candidate
 
 // Full chi2 of the hit in `slot` against the candidate (same Schur form as the update).
 __device__ __forceinline__ void score_hit(const ScanCand& c, const float4* __restrict__ rec, int32_t slot, Best& best) {
-    const float4* r0 = rec + (int64_t)slot * 3;
+    const float4* r0 = rec + (int64_t)slot * kRecWords;
     const float4 A = __ldg(r0), B = __ldg(r0 + 1), C = __ldg(r0 + 2);
     Crossing o;
     o.xn = c.xn; o.yn = c.yn; o.zn = c.zn; o.erx = c.ec; o.ery = c.es;

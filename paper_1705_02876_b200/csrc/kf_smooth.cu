@@ -144,9 +144,7 @@ rts_kernel(const __grid_constant__ FitParams P, const __grid_constant__ RtsMaps 
 // the row solves are long dependent chains, and with 2.25 warps per scheduler their latency is no longer hidden.
 // It was removed again; profiles/r02_counters.md has the numbers.)
 
-cudaError_t ensure_rts_attributes() {
-    return cudaSuccess;   // 23.6 KB of dynamic shared memory: below the 48 KB that needs no opt-in
-}
+// (23.6 KB of dynamic shared memory: below the 48 KB that needs no opt-in)
 
 }  // namespace
 

@@ -99,7 +99,7 @@ def _host_fit(ctx, b):
 
 @pytest.mark.parametrize("chunked", [2, 1])
 def test_bin_32_layers_in_one_call(ctx, chunked):
-    """KF_MAX_LAYERS pools in one kf_bin_layers call (two launch groups of 16), ragged sizes (1 to 3 chunks of the
+    """KF_MAX_LAYERS pools in one kf_bin_layers call (one launch group), ragged sizes (1 to 3 chunks of the
     chunked sort per pool), one empty pool; both forms of the sort."""
     import paper_1705_02876_b200 as K
     ctx.set_option(K.OPT_BIN_FORM, chunked)       # 2 = chunked sort wherever it applies, 1 = five-launch sort

@@ -231,11 +231,13 @@ bin_finish_kernel(const __grid_constant__ BinBatch B) {
 // ---------------------------------------------------------------------------------------------------------------
 // Chunked form of the same stable counting sort for hit pools (three launches + the finish step, every record
 // written ONCE): a layer is cut into chunks of kChunk consecutive hits, one CTA per chunk.
-//   chunk_count   bin of every hit; shared-memory histogram of the chunk; bucket lists in shared memory; every hit
-//                 counts the smaller indices of its bucket = its stable rank INSIDE the chunk (the arrival order of
-//                 the shared-memory atomics never shows); one word per hit (bin << 16 | rank) and the chunk's
-//                 histogram go to global memory.  512 threads x 4 hits: the kernel is one wave of CTAs and its
-//                 duration the ~370-instruction-per-hit chain of a warp, so fewer hits per thread = a shorter kernel
+//   chunk_count   bin of every hit (first guess from a look-up table, corrected against the edge tables); shared-
+//                 memory histogram of the chunk; every hit counts the smaller indices among the hits of its bin = its
+//                 stable rank INSIDE the chunk (the arrival order of the shared-memory atomics never shows; peer lists
+//                 of four per bin + a short overflow list, bucket lists for coarse grids); one word per hit
+//                 (bin << 16 | rank) and the chunk's histogram go to global memory.  512 threads x 4 hits: the kernel
+//                 is one wave of CTAs and its duration the instruction chain of a warp (~370 per hit with bisections
+//                 and bucket lists), so fewer hits per thread and fewer instructions per hit = a shorter kernel
 //   chunk_prefix  per bin: prefix of the chunk histograms over the chunks (chunks are consecutive index ranges, so
 //                 earlier chunk = smaller index) and the bin total; four warps per column, a quarter of the chunks
 //                 each, so that a whole column is in flight at once
@@ -244,7 +246,8 @@ bin_finish_kernel(const __grid_constant__ BinBatch B) {
 //                 read coalesced, four hits in flight per thread, and the packed record goes straight to its final place
 // Same results as the five-launch path, bit for bit.  Limits: n_bins <= kChunkMaxBins (shared memory).
 // Measured on configs[4] (7 x 120 000 hits, graph replay, no SoA copies), warm incremental cost per kernel:
-// count 17.7, prefix 3.5, place 16.2, finish 8.6 us = 46 us (round-2 start: 19.5 / 8.2 (+ scan) / 13.9 / 8.6 = 50).
+// count 17.7, prefix 3.5, place 16.2, finish 8.6 us = 46 us (round-2 start: 19.5 / 8.2 (+ scan) / 13.9 / 8.6 = 50);
+// with the peer lists and the look-up-table guesses in the count step: 43.7 us.
 #ifndef KF_BIN_CHUNK
 #define KF_BIN_CHUNK 2048
 #endif
@@ -290,7 +293,8 @@ constexpr int kChunkMaxBins = 8192;
 
 __global__ void __launch_bounds__(kCountBlock)
 chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__ eta_edge_g,
-                   const float* __restrict__ phi_cos_g, const float* __restrict__ phi_sin_g) {
+                   const float* __restrict__ phi_cos_g, const float* __restrict__ phi_sin_g,
+                   const int32_t* __restrict__ lut_g, float lut_u0, float lut_uscale) {
     const BinLayerDev& L = B.layer[blockIdx.y];
     const int c = blockIdx.x;
     const int64_t h0 = (int64_t)c * kChunk;
@@ -300,20 +304,20 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int32_t* cnt = reinterpret_cast<int32_t*>(smem_raw);              // [nb] histogram of the chunk
-    int32_t* loc = cnt + nb;                                           // [nb] start of each bin's bucket
-    uint32_t* ka = reinterpret_cast<uint32_t*>(loc + nb);              // [kChunk] bin << 16 | arrival number
+    int32_t* loc = cnt + nb;                                           // [nb] start of each bin's bucket (+ [nb] spare: peer lists)
+    uint32_t* ka = reinterpret_cast<uint32_t*>(loc + 2 * nb);          // [kChunk] bin << 16 | arrival number
     uint16_t* bucket = reinterpret_cast<uint16_t*>(ka + kChunk);       // [kChunk] chunk-local hit indices by bin
     float* eta_edge = reinterpret_cast<float*>(bucket + kChunk);       // [n_eta] [n_phi] [n_phi]
     float* phi_cos = eta_edge + B.n_eta;
     float* phi_sin = phi_cos + B.n_phi;
     __shared__ int32_t wsum[kCountBlock / 32];
+    __shared__ uint16_t lut[3 * kLutCells];
+    for (int i = tid; i < 3 * kLutCells; i += kCountBlock) lut[i] = (uint16_t)lut_g[i];
     for (int i = tid; i < nb; i += kCountBlock) cnt[i] = 0;
     for (int i = tid; i < B.n_eta; i += kCountBlock) eta_edge[i] = eta_edge_g[i];
     for (int i = tid; i < B.n_phi; i += kCountBlock) { phi_cos[i] = phi_cos_g[i]; phi_sin[i] = phi_sin_g[i]; }
     __syncthreads();
-    // The bin rule of bin_of_hit for this thread's kCountPer hits at once: all loads first, then the two searches
-    // as descents in powers of two (same answer as the bisection for a monotone predicate; the trip count depends on
-    // the grid only, so the hits' dependent look-ups interleave instead of running one hit after the other).
+    // The bin rule of bin_of_hit for this thread's kCountPer hits at once: all loads first, then the two searches.
     {
         float x[kCountPer], y[kCountPer], u[kCountPer];
         int pe[kCountPer], pp[kCountPer], lim[kCountPer];
@@ -333,23 +337,33 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
             pp[it] = upper ? half : 0;
             lim[it] = upper ? B.n_phi - 1 : (y[it] == 0.0f ? 0 : half - 1);
         }
-        int top = 1;
-        while (top * 2 <= B.n_eta - 1) top *= 2;
-        for (int step = top; step > 0; step >>= 1) {
+        // First guess from the look-up tables, then the exact rule: the largest index whose predicate holds, found
+        // by stepping up while the next edge is still below the hit and down while the own edge is above it (the
+        // predicates are monotone in the index, so this is the count the rule asks for -- the same answer as a
+        // bisection, for ~25 instructions per hit instead of ~95; a NaN makes every predicate false: index 0 / start).
+        const int ne1 = B.n_eta - 1;
 #pragma unroll
-            for (int it = 0; it < kCountPer; ++it) {
-                const int t = pe[it] + step;
-                if (t <= B.n_eta - 1 && u[it] >= eta_edge[t]) pe[it] = t;
-            }
+        for (int it = 0; it < kCountPer; ++it) {
+            int ce = __float2int_rd((u[it] - lut_u0) * lut_uscale);
+            ce = ce < 0 ? 0 : (ce > kLutCells - 1 ? kLutCells - 1 : ce);
+            int g = lut[ce];
+            g = g > ne1 ? ne1 : g;
+            while (g < ne1 && u[it] >= eta_edge[g + 1]) ++g;
+            while (g > 0 && !(u[it] >= eta_edge[g])) --g;
+            pe[it] = g;
         }
-        top = 1;
-        while (top * 2 <= half) top *= 2;
-        for (int step = top; step > 0; step >>= 1) {
 #pragma unroll
-            for (int it = 0; it < kCountPer; ++it) {
-                const int t = pp[it] + step;
-                if (t <= lim[it] && __fmul_rn(phi_cos[t], y[it]) >= __fmul_rn(phi_sin[t], x[it])) pp[it] = t;
-            }
+        for (int it = 0; it < kCountPer; ++it) {
+            const bool upper = pp[it] != 0;                    // (pp = start of the search: half in the upper half plane)
+            const float t = __fdividef(x[it], fabsf(x[it]) + fabsf(y[it]));
+            int cp = __float2int_rd((upper ? 1.0f - t : 1.0f + t) * (0.5f * kLutCells));
+            cp = cp < 0 ? 0 : (cp > kLutCells - 1 ? kLutCells - 1 : cp);
+            const int start = pp[it], hi = lim[it];
+            int g = lut[(upper ? 2 * kLutCells : kLutCells) + cp];
+            g = g < start ? start : (g > hi ? hi : g);
+            while (g < hi && __fmul_rn(phi_cos[g + 1], y[it]) >= __fmul_rn(phi_sin[g + 1], x[it])) ++g;
+            while (g > start && !(__fmul_rn(phi_cos[g], y[it]) >= __fmul_rn(phi_sin[g], x[it]))) --g;
+            pp[it] = g;
         }
 #pragma unroll
         for (int it = 0; it < kCountPer; ++it) {
@@ -361,6 +375,57 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
         }
     }
     __syncthreads();
+    // Stable rank inside the chunk = number of smaller indices among the hits of the same bin.
+    // Fast form (taken when at most kOverflowMax hits of the chunk arrived in their bin behind kPeers others, which
+    // is every chunk of a grid as fine as configs[4]'s: 0.8 hits per bin and chunk): the first kPeers arrivals of a
+    // bin are kept in peer[arrival][bin], later ones in a short overflow list; a hit compares itself with the
+    // (at most kPeers) peers of its bin and, if the bin has more, with the overflow entries of that bin.  No scan
+    // over the bins, no bucket lists.  Otherwise (coarse grids, all hits in one bin ...) the general form below.
+    {
+        constexpr int kPeers = 4, kOverflowMax = 64;
+        uint16_t* peer = reinterpret_cast<uint16_t*>(loc);              // [kPeers][nb], in the loc + spare area
+        __shared__ int32_t n_over_s;
+        __shared__ uint32_t over[kOverflowMax];                          // bin << 16 | chunk-local index
+        if (tid == 0) n_over_s = 0;
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < kCountPer; ++it) {
+            const int li = tid + it * kCountBlock;
+            if (li < m) {
+                const uint32_t k = ka[li];
+                const int b = (int)(k >> 16), a = (int)(k & 0xffffu);
+                if (a < kPeers) peer[a * nb + b] = (uint16_t)li;
+                else {
+                    const int32_t j = atomicAdd(&n_over_s, 1);
+                    if (j < kOverflowMax) over[j] = ((uint32_t)b << 16) | (uint32_t)li;
+                }
+            }
+        }
+        __syncthreads();
+        const int n_over = n_over_s;
+        if (n_over <= kOverflowMax) {
+#pragma unroll
+            for (int it = 0; it < kCountPer; ++it) {
+                const int li = tid + it * kCountBlock;
+                if (li < m) {
+                    const int b = (int)(ka[li] >> 16);
+                    const int n = cnt[b];
+                    int rank = 0;
+#pragma unroll
+                    for (int a = 0; a < kPeers; ++a) rank += (a < n && peer[a * nb + b] < (uint16_t)li) ? 1 : 0;
+                    if (n > kPeers)
+                        for (int j = 0; j < n_over; ++j) {
+                            const uint32_t o = over[j];
+                            rank += ((int)(o >> 16) == b && (int)(o & 0xffffu) < li) ? 1 : 0;
+                        }
+                    L.key[h0 + li] = (b << 16) | rank;     // one word per hit for chunk_place_kernel (rank < kChunk <= 65536, b < 8192)
+                }
+            }
+            for (int b = tid; b < nb; b += kCountBlock) L.chunk_cnt[(int64_t)c * nb + b] = cnt[b];   // [chunk][bin]
+            return;
+        }
+        __syncthreads();                                                 // (the general form reuses the peer area as loc)
+    }
     // exclusive scan of cnt -> loc: thread t owns the bins [r0, r1)
     const int per = (nb + kCountBlock - 1) / kCountBlock;
     const int r0 = tid * per < nb ? tid * per : nb, r1 = r0 + per < nb ? r0 + per : nb;
@@ -582,6 +647,7 @@ cudaError_t BinScratch::reserve(int64_t n_items, int64_t n_bins, cudaStream_t st
     if ((e = cudaMalloc(&eta_edge, tab_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&phi_cos, tab_b)) != cudaSuccess) { release(); return e; }
     if ((e = cudaMalloc(&phi_sin, tab_b)) != cudaSuccess) { release(); return e; }
+    if ((e = cudaMalloc(&guess_lut, (size_t)3 * kLutCells * sizeof(int32_t))) != cudaSuccess) { release(); return e; }
     if (want_rec) {
         if ((e = cudaMalloc(&rec_tmp, (size_t)(ni > 0 ? ni : 1) * 12 * sizeof(float))) != cudaSuccess) { release(); return e; }
         cap_rec = ni;
@@ -605,11 +671,12 @@ cudaError_t BinScratch::reserve_chunk_cnt(int64_t words, cudaStream_t stream) {
 }
 
 void BinScratch::release() {
-    void* ptrs[] = {key, unsorted, pib, counts, eta_edge, phi_cos, phi_sin, rec_tmp, chunk_cnt};
+    void* ptrs[] = {key, unsorted, pib, counts, eta_edge, phi_cos, phi_sin, rec_tmp, chunk_cnt, guess_lut};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     key = unsorted = pib = counts = nullptr;
     eta_edge = phi_cos = phi_sin = nullptr;
+    guess_lut = nullptr;
     rec_tmp = nullptr;
     chunk_cnt = nullptr;
     cap_chunk_cnt = 0;
@@ -641,6 +708,30 @@ cudaError_t BinScratch::tables(int n_eta, int n_phi, float eta_max, cudaStream_t
     if ((e = cudaMemcpyAsync(eta_edge, he, (size_t)n_eta * 4, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return e;
     if ((e = cudaMemcpyAsync(phi_cos, hc, (size_t)n_phi * 4, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return e;
     if ((e = cudaMemcpyAsync(phi_sin, hs, (size_t)n_phi * 4, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return e;
+    // First guesses for chunk_count_kernel's searches (any guess is corrected there against the tables above, in both
+    // directions, so these only have to be close): eta over kLutCells cells of u = z / r, phi over kLutCells cells of
+    // the "diamond angle" x / (|x| + |y|) per half plane.
+    {
+        host_lut.assign((size_t)3 * kLutCells, 0);
+        const float u0 = (float)std::sinh(-em), u1 = (float)std::sinh(em);
+        lut_u0 = u0;
+        lut_uscale = (float)((double)kLutCells / ((double)u1 - (double)u0));
+        const int half = n_phi / 2;
+        for (int c = 0; c < kLutCells; ++c) {
+            const double lo = (double)u0 + (double)c / (double)lut_uscale;
+            int g = 0;
+            for (int j = 1; j < n_eta; ++j) g += (double)he[j] <= lo ? 1 : 0;
+            host_lut[c] = g;
+            const double tl = -1.0 + 2.0 * c / kLutCells, tu = 1.0 - 2.0 * c / kLutCells;
+            const double pl = -std::atan2(1.0 - std::fabs(tl), tl), pu = std::atan2(1.0 - std::fabs(tu), tu);
+            int gl = 0, gu = half;
+            for (int j = 1; j < half; ++j) gl += (-kPi + j * d_phi) <= pl ? 1 : 0;
+            for (int j = half + 1; j < n_phi; ++j) gu += (-kPi + j * d_phi) <= pu ? 1 : 0;
+            host_lut[kLutCells + c] = gl;
+            host_lut[2 * kLutCells + c] = gu;
+        }
+        if ((e = cudaMemcpyAsync(guess_lut, host_lut.data(), host_lut.size() * sizeof(int32_t), cudaMemcpyHostToDevice, stream)) != cudaSuccess) return e;
+    }
     tab_n_eta = n_eta;
     tab_n_phi = n_phi;
     tab_eta_max = eta_max;
@@ -652,7 +743,7 @@ cudaError_t BinScratch::tables(int n_eta, int n_phi, float eta_max, cudaStream_t
 namespace {
 
 size_t chunk_count_smem(int n_eta, int n_phi) {
-    return (size_t)2 * n_eta * n_phi * 4 + (size_t)kChunk * 6 + ((size_t)n_eta + 2 * (size_t)n_phi) * 4;
+    return (size_t)3 * n_eta * n_phi * 4 + (size_t)kChunk * 6 + ((size_t)n_eta + 2 * (size_t)n_phi) * 4;   // (+ static: lut, wsum, overflow)
 }
 
 int64_t chunk_cnt_words(int64_t chunks, int nb) { return (chunks > 0 ? chunks : 1) * (int64_t)nb; }
@@ -693,7 +784,7 @@ cudaError_t try_chunk_sort(BinScratch& s, BinBatch& B, int m, int64_t group_max,
         chunks += (B.layer[j].n + kChunk - 1) / kChunk;
     }
     const dim3 grid((unsigned)nc, (unsigned)m);
-    chunk_count_kernel<<<grid, kCountBlock, chunk_count_smem(B.n_eta, B.n_phi), stream>>>(B, s.eta_edge, s.phi_cos, s.phi_sin);
+    chunk_count_kernel<<<grid, kCountBlock, chunk_count_smem(B.n_eta, B.n_phi), stream>>>(B, s.eta_edge, s.phi_cos, s.phi_sin, s.guess_lut, s.lut_u0, s.lut_uscale);
     chunk_prefix_kernel<<<dim3((unsigned)((nb + 31) / 32), (unsigned)m), 128, 0, stream>>>(B);
     chunk_place_kernel<<<grid, kChunkBlock, (size_t)nb * 4, stream>>>(B);
     bin_finish_kernel<<<dim3((unsigned)((nb * 32 + kBlock - 1) / kBlock), (unsigned)m), kBlock, 0, stream>>>(B);

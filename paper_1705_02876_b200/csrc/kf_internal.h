@@ -85,6 +85,7 @@ struct HostStage {
 
 // ---------------------------------------------------------------------------------- binning
 constexpr int KF_MAX_BINS_INTERNAL = 65536;
+constexpr int kLutCells = 256;
 constexpr int kBinBatchMax = 32;  // layers per group of launches (the descriptors travel as one 4.4 KB kernel parameter)
 
 struct BinArgs {
@@ -138,6 +139,10 @@ struct BinScratch {
     int tab_n_eta = 0, tab_n_phi = 0;
     float tab_eta_max = 0.0f;
     std::vector<float> host_tab; // persistent host copy of the three tables (source of the async copy)
+    // first guesses for the edge searches of chunk_count_kernel: [3][kLutCells] = eta, phi lower / upper half plane
+    int32_t* guess_lut = nullptr;
+    std::vector<int32_t> host_lut;
+    float lut_u0 = 0.0f, lut_uscale = 0.0f;   // eta cell of u = z / r: floor((u - u0) * uscale)
     cudaError_t reserve(int64_t n_items, int64_t n_bins, cudaStream_t stream, bool records = false);
     cudaError_t tables(int n_eta, int n_phi, float eta_max, cudaStream_t stream);
     void release();

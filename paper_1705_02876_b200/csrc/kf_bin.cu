@@ -313,7 +313,14 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
     __shared__ int32_t wsum[kCountBlock / 32];
     __shared__ uint16_t lut[3 * kLutCells];
     for (int i = tid; i < 3 * kLutCells; i += kCountBlock) lut[i] = (uint16_t)lut_g[i];
-    for (int i = tid; i < nb; i += kCountBlock) cnt[i] = 0;
+    // histogram = 0, peer lists = empty (0xffff); 16 bytes per store where the grid allows it
+    const bool vec4 = (nb & 3) == 0;
+    if (vec4) {
+        for (int i = tid; i < nb / 4; i += kCountBlock) reinterpret_cast<int4*>(cnt)[i] = make_int4(0, 0, 0, 0);
+        for (int i = tid; i < nb / 2; i += kCountBlock) reinterpret_cast<uint4*>(loc)[i] = make_uint4(~0u, ~0u, ~0u, ~0u);
+    } else {
+        for (int i = tid; i < nb; i += kCountBlock) { cnt[i] = 0; reinterpret_cast<uint2*>(loc)[i] = make_uint2(~0u, ~0u); }
+    }
     for (int i = tid; i < B.n_eta; i += kCountBlock) eta_edge[i] = eta_edge_g[i];
     for (int i = tid; i < B.n_phi; i += kCountBlock) { phi_cos[i] = phi_cos_g[i]; phi_sin[i] = phi_sin_g[i]; }
     __syncthreads();
@@ -348,8 +355,15 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
             ce = ce < 0 ? 0 : (ce > kLutCells - 1 ? kLutCells - 1 : ce);
             int g = lut[ce];
             g = g > ne1 ? ne1 : g;
-            while (g < ne1 && u[it] >= eta_edge[g + 1]) ++g;
-            while (g > 0 && !(u[it] >= eta_edge[g])) --g;
+            // the guess is the bin or the one below it: one look at the next edge, one at the edge that then decides
+            const bool up = g < ne1 && u[it] >= eta_edge[g + 1];
+            g += up ? 1 : 0;
+            const int pi = up ? (g < ne1 ? g + 1 : ne1) : g;
+            const bool ge = u[it] >= eta_edge[pi];
+            if (up ? (g < ne1 && ge) : (g > 0 && !ge)) {          // rare: further than one bin off (coarse table, NaN)
+                while (g < ne1 && u[it] >= eta_edge[g + 1]) ++g;
+                while (g > 0 && !(u[it] >= eta_edge[g])) --g;
+            }
             pe[it] = g;
         }
 #pragma unroll
@@ -361,8 +375,15 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
             const int start = pp[it], hi = lim[it];
             int g = lut[(upper ? 2 * kLutCells : kLutCells) + cp];
             g = g < start ? start : (g > hi ? hi : g);
-            while (g < hi && __fmul_rn(phi_cos[g + 1], y[it]) >= __fmul_rn(phi_sin[g + 1], x[it])) ++g;
-            while (g > start && !(__fmul_rn(phi_cos[g], y[it]) >= __fmul_rn(phi_sin[g], x[it]))) --g;
+            const int n1 = g < hi ? g + 1 : hi;
+            const bool up = g < hi && __fmul_rn(phi_cos[n1], y[it]) >= __fmul_rn(phi_sin[n1], x[it]);
+            g += up ? 1 : 0;
+            const int pi = up ? (g < hi ? g + 1 : hi) : g;
+            const bool ge = __fmul_rn(phi_cos[pi], y[it]) >= __fmul_rn(phi_sin[pi], x[it]);
+            if (up ? (g < hi && ge) : (g > start && !ge)) {
+                while (g < hi && __fmul_rn(phi_cos[g + 1], y[it]) >= __fmul_rn(phi_sin[g + 1], x[it])) ++g;
+                while (g > start && !(__fmul_rn(phi_cos[g], y[it]) >= __fmul_rn(phi_sin[g], x[it]))) --g;
+            }
             pp[it] = g;
         }
 #pragma unroll
@@ -383,7 +404,8 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
     // over the bins, no bucket lists.  Otherwise (coarse grids, all hits in one bin ...) the general form below.
     {
         constexpr int kPeers = 4, kOverflowMax = 64;
-        uint16_t* peer = reinterpret_cast<uint16_t*>(loc);              // [kPeers][nb], in the loc + spare area
+        static_assert(kPeers == 4 && kChunk < 65535, "peer lists: four 16-bit indices per bin, 0xffff = empty");
+        uint16_t* peer = reinterpret_cast<uint16_t*>(loc);              // [nb][kPeers], in the loc + spare area, preset to 0xffff
         __shared__ int32_t n_over_s;
         __shared__ uint32_t over[kOverflowMax];                          // bin << 16 | chunk-local index
         if (tid == 0) n_over_s = 0;
@@ -394,7 +416,7 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
             if (li < m) {
                 const uint32_t k = ka[li];
                 const int b = (int)(k >> 16), a = (int)(k & 0xffffu);
-                if (a < kPeers) peer[a * nb + b] = (uint16_t)li;
+                if (a < kPeers) peer[b * kPeers + a] = (uint16_t)li;
                 else {
                     const int32_t j = atomicAdd(&n_over_s, 1);
                     if (j < kOverflowMax) over[j] = ((uint32_t)b << 16) | (uint32_t)li;
@@ -409,11 +431,11 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
                 const int li = tid + it * kCountBlock;
                 if (li < m) {
                     const int b = (int)(ka[li] >> 16);
-                    const int n = cnt[b];
-                    int rank = 0;
-#pragma unroll
-                    for (int a = 0; a < kPeers; ++a) rank += (a < n && peer[a * nb + b] < (uint16_t)li) ? 1 : 0;
-                    if (n > kPeers)
+                    const uint2 p = reinterpret_cast<const uint2*>(peer)[b];       // the bin's four peers (0xffff: none)
+                    const uint32_t me = (uint32_t)li;
+                    int rank = ((p.x & 0xffffu) < me ? 1 : 0) + ((p.x >> 16) < me ? 1 : 0) +
+                               ((p.y & 0xffffu) < me ? 1 : 0) + ((p.y >> 16) < me ? 1 : 0);
+                    if ((p.y >> 16) != 0xffffu && n_over > 0)                     // four or more: some may be in the overflow list
                         for (int j = 0; j < n_over; ++j) {
                             const uint32_t o = over[j];
                             rank += ((int)(o >> 16) == b && (int)(o & 0xffffu) < li) ? 1 : 0;
@@ -421,7 +443,12 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
                     L.key[h0 + li] = (b << 16) | rank;     // one word per hit for chunk_place_kernel (rank < kChunk <= 65536, b < 8192)
                 }
             }
-            for (int b = tid; b < nb; b += kCountBlock) L.chunk_cnt[(int64_t)c * nb + b] = cnt[b];   // [chunk][bin]
+            if (vec4) {                                                           // [chunk][bin]
+                int4* row = reinterpret_cast<int4*>(L.chunk_cnt + (int64_t)c * nb);
+                for (int i = tid; i < nb / 4; i += kCountBlock) row[i] = reinterpret_cast<const int4*>(cnt)[i];
+            } else {
+                for (int b = tid; b < nb; b += kCountBlock) L.chunk_cnt[(int64_t)c * nb + b] = cnt[b];
+            }
             return;
         }
         __syncthreads();                                                 // (the general form reuses the peer area as loc)

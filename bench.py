@@ -524,6 +524,74 @@ def _opcode_table(path: str) -> None:
     print(f"TOTAL,{total},{flops}")
 
 
+def _function_table(dis: str, kernel: str, path: str) -> None:
+    """--function-table DIS KERNEL CSV: where a kernel's instructions go, per source function.
+    DIS = `nvdisasm -gi <cubin>` (line info with the inline chains; the cubin comes from `cuobjdump -xelf all libkf_b200.so`),
+    KERNEL = a fragment of the kernel's mangled name, CSV = `ncu -i X.ncu-rep --page source --csv --print-source sass
+    -k <kernel>`.  Both list the kernel's SASS in address order; every instruction is charged to the innermost line of
+    its inline chain that lies in this repo's kernel sources (CUDA's intrinsic headers and the number-type wrappers of
+    kf_pair.cuh are skipped), and lines are summed per enclosing function."""
+    import csv
+    import re
+    with open(dis) as fh:
+        lines = fh.read().split("\n")
+    start = next(i for i, l in enumerate(lines) if l.startswith(".text.") and kernel in l)
+    end = next((i for i, l in enumerate(lines) if l.startswith(".text.") and i > start), len(lines))
+    pat = re.compile(r'//## File ".*?([^/"]+)", line (\d+)(?: inlined at ".*?([^/"]+)", line (\d+))?')
+    seq, chain, last = [], [], None
+    for l in lines[start:end]:
+        m = pat.search(l)
+        if m:
+            chain.append((m.group(1), int(m.group(2))))
+            if m.group(3):
+                chain.append((m.group(3), int(m.group(4))))
+        elif re.match(r"\s+/\*[0-9a-f]{4,}\*/", l):
+            if chain:
+                own = [c for c in chain if c[0].startswith("kf_") and c[0] != "kf_pair.cuh"]
+                last = own[0] if own else chain[0]
+                chain = []
+            seq.append(last)
+    with open(path, newline="") as fh:
+        rows = list(csv.reader(fh))
+    hdr = next(r for r in rows if "Source" in r and "Instructions Executed" in r)
+    ei, si = hdr.index("Instructions Executed"), hdr.index("# Samples")
+    ex = []
+    for r in rows[rows.index(hdr) + 1:]:
+        if r and r[0] == "Kernel Name":
+            break
+        if len(r) > max(ei, si):
+            try:
+                ex.append((int(r[ei]), int(r[si] or 0)))
+            except ValueError:
+                pass
+    if len(ex) != len(seq):
+        raise SystemExit(f"{len(seq)} instructions in the disassembly, {len(ex)} in the ncu export: not the same build")
+    src = {}
+
+    def function_of(f, ln):
+        fp = os.path.join(ROOT, "paper_1705_02876_b200", "csrc", f)
+        if not os.path.exists(fp):
+            return f
+        if fp not in src:
+            with open(fp) as fh:
+                src[fp] = fh.read().split("\n")
+        for j in range(min(ln, len(src[fp])) - 1, -1, -1):
+            m = re.match(r"^(?:[\w:<>,\*& ]*?[ \*&])?([A-Za-z]\w*)\(", src[fp][j])
+            if m and not src[fp][j].startswith((" ", "/", "#", "}")) and m.group(1) not in ("if", "for", "while", "switch", "defined"):
+                return f + ": " + m.group(1)
+        return f
+    per = {}
+    for (f, ln), (e, smp) in zip([c or ("?", 0) for c in seq], ex):
+        a = per.setdefault(function_of(f, ln), [0, 0])
+        a[0] += e
+        a[1] += smp
+    te, ts = sum(v[0] for v in per.values()), max(1, sum(v[1] for v in per.values()))
+    print("function,warp_instructions,share_of_instructions,share_of_stall_samples")
+    for k, v in sorted(per.items(), key=lambda kv: -kv[1][0]):
+        print(f"{k},{v[0]},{v[0] / te:.4f},{v[1] / ts:.4f}")
+    print(f"TOTAL,{te},1.0000,1.0000")
+
+
 def run_ours(args) -> None:
     import torch
     import paper_1705_02876_b200 as K
@@ -844,9 +912,13 @@ def main():
     ap.add_argument("--events", type=int, default=100, help="events of 20 000 tracks per GPU (configs[2] = 100)")
     ap.add_argument("--profile-sequence", action="store_true", help="one launch of every hot call, for ncu (see profiles/)")
     ap.add_argument("--opcode-table", metavar="CSV", help="summarise an `ncu --page source --csv` export per SASS opcode")
+    ap.add_argument("--function-table", nargs=3, metavar=("DIS", "KERNEL", "CSV"),
+                    help="per source function: share of a kernel's executed instructions (nvdisasm -gi + ncu source page)")
     args = ap.parse_args()
     if args.opcode_table:
         return _opcode_table(args.opcode_table)
+    if args.function_table:
+        return _function_table(*args.function_table)
     if args.profile_sequence:
         return run_profile_sequence(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

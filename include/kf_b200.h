@@ -304,7 +304,7 @@ KF_API int kf_fit_tracks_indexed(kf_ctx* ctx, const kf_geometry* geom, const kf_
  * caller-allocated.  n_hits == 0 is valid (all offsets 0). */
 KF_API int kf_bin_hits(kf_ctx* ctx, float radius_cm, const kf_layer_hits* hits, kf_layer_bins* out);
 
-/* The same for n_layers layers at once (HOST arrays of descriptors, DEV buffers inside): four kernel
+/* The same for n_layers layers at once (HOST arrays of descriptors, DEV buffers inside): four or five kernel
  * launches in total instead of four per layer.  All layers must share n_eta, n_phi and eta_max. */
 KF_API int kf_bin_layers(kf_ctx* ctx, int n_layers, const float* radius_cm, const kf_layer_hits* hits,
                          kf_layer_bins* out);

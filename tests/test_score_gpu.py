@@ -161,6 +161,39 @@ def test_bin_hits_against_the_double_definition(ctx, sort_path):
     assert np.count_nonzero(differ >= 2 * k) <= 5
 
 
+@pytest.mark.parametrize("crowd", [4, 5, 68, 69, 300])
+def test_bin_hits_crowded_bins_within_a_chunk(ctx, sort_path, crowd):
+    """The count step of the chunked sort ranks a hit inside its chunk from per-bin peer lists (four entries) plus an
+    overflow list of 64, and falls back to bucket lists beyond that.  Chunks (2048 consecutive hits) built to sit on
+    those boundaries: bins with exactly `crowd` hits in ONE chunk -- 4 (peers only), 5 (one overflow entry), 68
+    (overflow list exactly full), 69 (one too many: bucket form), 300 -- next to singly occupied bins, in shuffled
+    index order, several chunks, a ragged last one.  Bit-exact against the oracle's serial counting sort."""
+    rng = np.random.default_rng(100 + crowd)
+    r = 12.0
+    H = 5 * 2048 + 777
+    phi, eta = rng.uniform(-np.pi, np.pi, H), rng.uniform(-1.19, 1.19, H)
+    # per chunk: some bins filled with `crowd` hits each (bin centres, tiny jitter), the rest uniform
+    d_eta, d_phi = 2 * EMAX / NE, 2 * np.pi / NP
+    for c in range(6):
+        lo, hi = c * 2048, min((c + 1) * 2048, H)
+        n_crowded = max(1, min(64 // max(crowd - 4, 1), 12)) if crowd > 4 else 20
+        idx = rng.permutation(np.arange(lo, hi))
+        used = 0
+        for b in range(n_crowded):
+            if used + crowd > hi - lo:
+                break
+            ie, ip = int(rng.integers(0, NE)), int(rng.integers(0, NP))
+            sel = idx[used:used + crowd]
+            used += crowd
+            eta[sel] = -EMAX + (ie + 0.5) * d_eta + rng.uniform(-0.2, 0.2, crowd) * d_eta
+            phi[sel] = -np.pi + (ip + 0.5) * d_phi + rng.uniform(-0.2, 0.2, crowd) * d_phi
+    pos = np.stack([r * np.cos(phi), r * np.sin(phi), r * np.sinh(eta)]).astype(np.float32)
+    cov = rng.uniform(1e-4, 1e-2, (6, H)).astype(np.float32)
+    dl, ob = _bin_both(ctx, pos, cov, r)
+    assert np.diff(ob["bin_offset"]).max() >= crowd
+    _assert_bins_equal(dl, ob, pos, cov)
+
+
 def test_bin_layers_batched_equals_per_layer(ctx, sort_path):
     """kf_bin_layers (all layers in four launches) == kf_bin_hits layer by layer == oracle."""
     from paper_1705_02876_b200.buffers import DeviceLayer

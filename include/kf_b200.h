@@ -261,7 +261,8 @@ KF_API int kf_fit_tracks_smooth(kf_ctx* ctx, const kf_geometry* geom, const kf_t
 
 /* Same call with every pointer HOST (pageable or pinned): copies in, fits, copies out, in chunks
  * pipelined over internal streams, and returns when `out` is complete.  This is the end-to-end
- * path (transfers overlapped with kernels).  Alignment rules do not apply. */
+ * path (transfers overlapped with kernels).  Alignment rules do not apply.  The results are
+ * those of kf_fit_tracks on the same tracks, bit for bit (every chunk runs the kernel the whole batch would). */
 KF_API int kf_fit_tracks_host(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                        const kf_track_hits* hits, kf_tracks* out);
 

@@ -930,6 +930,13 @@ cudaError_t ensure_fit_attributes() {
     return e;
 }
 
+bool fit_takes_pair_form(int64_t n, int n_layers, const LaunchOptions& opt) {
+    // (the pair form pays once the machine is full: at least 151 552 tracks, or 2 M track-layers -- config 3's
+    // 100 000 x 20 layers: 0.0429 ms against 0.0451 for the one-track kernel)
+    if (opt.pair_min_tracks > 0) return n >= opt.pair_min_tracks;
+    return n >= (int64_t)KF_PAIR_MIN_TRACKS || n * (int64_t)n_layers >= 2000000;
+}
+
 cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream, const LaunchOptions& opt) {
     if (a.n == 0) return cudaSuccess;
     const cudaError_t attr = ensure_fit_attributes();
@@ -938,16 +945,13 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     const bool store = a.lpar != nullptr;    // per-layer filtered states for the RTS smoother
     const int L = P.n_layers;
     FitMaps M;
-    const int64_t pair_min = opt.pair_min_tracks > 0 ? opt.pair_min_tracks : (int64_t)KF_PAIR_MIN_TRACKS;
     // Two tracks per thread.  The pair form of the refit takes ragged pairs (a layer only one of the two tracks
     // has a hit on) through the one-track path and then loses badly (1.2 % of tracks stopping short: 0.81 ms against
     // 0.49 ms for 600 000 twenty-layer tracks), so it is taken only where the caller says that every track has
     // every hit (mask == NULL); the pair form of the fit parks and shadows the idle track and wins either way.
     // (Option refit_pair_masked lifts that condition: the tests use it to drive the pair refit's ragged-pair code,
     // which failures can reach without any mask, with masks.)
-    // (the pair form pays once the machine is full: at least 151 552 tracks, or 2 M track-layers -- config 3's
-    // 100 000 x 20 layers: 0.0429 ms against 0.0451 for the one-track kernel)
-    const bool big = opt.pair_min_tracks > 0 ? a.n >= pair_min : (a.n >= pair_min || a.n * (int64_t)L >= 2000000);
+    const bool big = fit_takes_pair_form(a.n, L, opt);
     if (P.geometry_options == 0 && big &&
         (!smooth || (KF_PAIR_SMOOTH && (a.mask == nullptr || opt.refit_pair_masked != 0)))) {
         constexpr int W = kPairTile;

@@ -8,6 +8,8 @@
 // stages them and the pipeline degrades gracefully.
 #include <cstring>
 
+#include <cstdint>
+
 #include "kf_internal.h"
 
 namespace kf {
@@ -73,6 +75,10 @@ cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const Launch
     const SlotLayout lay(chunk, layers);
     const int L = io.L;
     const size_t cw = (size_t)chunk * 4;  // device pitch of float planes
+    // every chunk takes the kernel the WHOLE batch would take in kf_fit_tracks (chunks start at multiples of 64, so
+    // the pairs are the same too): host path and device path agree bit for bit
+    LaunchOptions chunk_opt = opt;
+    chunk_opt.pair_min_tracks = fit_takes_pair_form(io.n, L, opt) ? 1 : INT64_MAX;
     int slot = 0;
     for (int64_t t0 = 0; t0 < io.n; t0 += chunk, slot = (slot + 1) % kSlots) {
         const int64_t m = io.n - t0 < chunk ? io.n - t0 : chunk;
@@ -95,7 +101,7 @@ cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const Launch
             a.mask = io.mask ? (const uint32_t*)(b + lay.mask) : nullptr;
             a.opar = (float*)(b + lay.opar); a.ocov = (float*)(b + lay.ocov); a.ld_out = chunk;
             a.chi2 = (float*)(b + lay.chi2); a.nhits = (int32_t*)(b + lay.nhits); a.status = (uint32_t*)(b + lay.status);
-            KF_TRY(launch_fit(P, a, st, opt));
+            KF_TRY(launch_fit(P, a, st, chunk_opt));
         }
         KF_TRY(cudaMemcpy2DAsync(io.opar + t0, (size_t)io.ld_out * 4, b + lay.opar, cw, w, 6, cudaMemcpyDeviceToHost, st));
         KF_TRY(cudaMemcpy2DAsync(io.ocov + t0, (size_t)io.ld_out * 4, b + lay.ocov, cw, w, 21, cudaMemcpyDeviceToHost, st));

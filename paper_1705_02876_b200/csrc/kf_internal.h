@@ -57,6 +57,10 @@ struct IndexedPools {           // per-layer hit pools + the per-track hit indic
 // kf_fit.cu
 cudaError_t launch_fit_indexed(const FitParams& P, const IndexedPools& H, const FitArgs& a, cudaStream_t stream);
 cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream, const LaunchOptions& opt = LaunchOptions());
+// The size rule of launch_fit: does a batch of n tracks x n_layers take the two-tracks-per-thread kernels?
+// (kf_fit_tracks_host decides it on the WHOLE batch and launches every chunk accordingly, so that the host path gives,
+// bit for bit, what kf_fit_tracks gives on the same tracks.)
+bool fit_takes_pair_form(int64_t n, int n_layers, const LaunchOptions& opt);
 
 // kf_smooth.cu: backward RTS pass over the per-layer arrays the forward kernel filled
 cudaError_t launch_rts(const FitParams& P, const FitArgs& a, cudaStream_t stream);

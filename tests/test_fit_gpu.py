@@ -238,6 +238,24 @@ def test_fit_host_path_equals_device_path(ctx):
         assert np.array_equal(ref[k], r[k]), k
 
 
+def test_fit_host_path_equals_device_path_across_chunks(ctx):
+    """A batch large enough for the two-tracks-per-thread kernels (14 events = 280 000 tracks, holes in the masks of
+    some) goes through kf_fit_tracks_host in chunks of 131 072 tracks: every chunk takes the kernel the whole batch
+    takes on the device path, so the two agree bit for bit, chunk boundaries and the ragged last chunk included."""
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.make_fit_batch(2, n_events=14)
+    rng = np.random.default_rng(77)
+    holes = rng.random(b.n) < 0.05
+    b.mask = b.mask.copy()
+    b.mask[holes] &= ~(np.uint32(1) << rng.integers(0, 10, holes.sum()).astype(np.uint32))
+    ref = _gpu_fit(ctx, b)
+    h = DeviceFit.from_batch(b, "cpu", pin=True)
+    h.fit_host(ctx)
+    r = h.results()
+    for k in ref:
+        assert np.array_equal(ref[k], r[k], equal_nan=True), k
+
+
 def test_fit_argument_errors(ctx):
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceFit

@@ -176,8 +176,8 @@ typedef struct {
      * variance along z instead of along the radius; a crossing outside the annulus sets KF_STATUS_OUTSIDE and the
      * layer is skipped; a plane that lies behind the state or half a turn or more away is KF_STATUS_PROP_FAIL.
      * radius_cm[l] of a disc layer is not used but must keep the list increasing.  Discs are known to
-     * kf_fit_tracks, kf_fit_tracks_indexed and kf_fit_tracks_host; every other call returns KF_ERR_UNSUPPORTED
-     * for a geometry with a disc.  material_model and energy_loss_model apply at a disc with the path factor
+     * kf_fit_tracks, kf_fit_tracks_indexed, kf_fit_tracks_host and kf_fit_tracks_smooth; every other call returns
+     * KF_ERR_UNSUPPORTED for a geometry with a disc.  material_model and energy_loss_model apply at a disc with the path factor
      * 1 / |cos| of the angle to the z axis = |p| / |pz|. */
     const int32_t* surface_type;  /* HOST [n_layers] 0 = barrel, 1 = disc pair; or NULL                        */
     const float* disc_z_cm;       /* HOST [n_layers] |z| of the disc pair (> 0), read where surface_type = 1   */
@@ -255,7 +255,8 @@ typedef struct {
  * intermediate per-layer states (no other scratch is used).  A backward step that fails sets
  * KF_STATUS_SMOOTH_FAIL in out->status (see there).  Path-length material, finite barrels and the energy-loss
  * option are honoured (with energy loss the map between two layers is J F, reading A21: its Jacobian and its
- * process noise J Q J^T enter the recursion).  All pointers DEV.  Two kernels. */
+ * process noise J Q J^T enter the recursion), and so are endcap discs (the smoothed covariance of a layer that
+ * is a disc has no variance along z).  All pointers DEV.  Two kernels. */
 KF_API int kf_fit_tracks_smooth(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                                 const kf_track_hits* hits, kf_tracks* out, kf_smoothed* sm);
 

@@ -440,7 +440,7 @@ int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* se
                          kf_tracks* out, kf_smoothed* sm) {
     if (!c || !geom || !seeds || !hits || !out || !sm) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);   // (discs: reading A23, the forward kernel and the backward step both know them)
     if (rc) return rc;
     if ((rc = check_tracks(seeds, true, true))) return rc;
     if ((rc = check_tracks(out, false, true))) return rc;

@@ -154,13 +154,20 @@ __device__ __forceinline__ void track_to_tile(const Track& t, float* p) {
 // MODE 2: the filtered state of layer l in the local frame -> the per-layer arrays (coalesced 4-byte stores: lane =
 // track).  Planes: par 0..5 = x y z px py pz; cov 0..14 = c11 c12 c13 c14 c15 c22 c23 c24 c25 c33 c34 c35 c44 c45
 // c55, 15..16 = eax eay (17..20 are written by the backward pass only).
-__device__ __forceinline__ void store_layer_state(const Track& t, const FitArgs& a, int l, int64_t i) {
+// (type 1: the state stands on a disc, reading A23 -- its live coordinates are (r, t | b1 b2 c) and the first nine
+// planes hold rr rt r3 r4 r5 | tt t3 t4 t5 instead of tt tz t3 t4 t5 | zz z3 z4 z5.)
+__device__ __forceinline__ void store_layer_state(const Track& t, const FitArgs& a, int l, int64_t i, int type = 0) {
     float* p = a.lpar + (int64_t)l * 6 * a.ld_l + i;
     float* c = a.lcov + (int64_t)l * 21 * a.ld_l + i;
     const int64_t ld = a.ld_l;
     p[0] = t.x; p[ld] = t.y; p[2 * ld] = t.z; p[3 * ld] = t.px; p[4 * ld] = t.py; p[5 * ld] = t.pz;
-    c[0] = t.c11; c[ld] = t.c12; c[2 * ld] = t.c13; c[3 * ld] = t.c14; c[4 * ld] = t.c15;
-    c[5 * ld] = t.c22; c[6 * ld] = t.c23; c[7 * ld] = t.c24; c[8 * ld] = t.c25;
+    if (type == 1) {
+        c[0] = t.c00; c[ld] = t.c01; c[2 * ld] = t.c03; c[3 * ld] = t.c04; c[4 * ld] = t.c05;
+        c[5 * ld] = t.c11; c[6 * ld] = t.c13; c[7 * ld] = t.c14; c[8 * ld] = t.c15;
+    } else {
+        c[0] = t.c11; c[ld] = t.c12; c[2 * ld] = t.c13; c[3 * ld] = t.c14; c[4 * ld] = t.c15;
+        c[5 * ld] = t.c22; c[6 * ld] = t.c23; c[7 * ld] = t.c24; c[8 * ld] = t.c25;
+    }
     c[9 * ld] = t.c33; c[10 * ld] = t.c34; c[11 * ld] = t.c35;
     c[12 * ld] = t.c44; c[13 * ld] = t.c45; c[14 * ld] = t.c55;
     c[15 * ld] = t.eax; c[16 * ld] = t.eay;
@@ -243,7 +250,7 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             if (rc == 0u) {
                 nh += 1; used |= 1u << l;
                 started = GEOM != 2 || P.layer[l].type == 0;   // after a disc the z row is the null one, not the radial row
-                if constexpr (MODE == 2) { if (valid) store_layer_state(t, a, l, i); }
+                if constexpr (MODE == 2) { if (valid) store_layer_state(t, a, l, i, GEOM == 2 ? P.layer[l].type : 0); }
             }
         }
         // The hit values have been consumed by the math above, so the stage can be handed back to the
@@ -923,6 +930,7 @@ cudaError_t ensure_fit_attributes() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(true));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_pair_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem2_bytes(false));
@@ -978,9 +986,10 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
         return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
     const bool geom = P.geometry_options != 0;   // reading A20 options in use
-    if (P.has_discs && (smooth || store)) return cudaErrorInvalidValue;   // (refused at the ABI: discs are known to the fit only)
+    if (P.has_discs && smooth) return cudaErrorInvalidValue;   // (refused at the ABI: the refit of reading A18 does not know discs)
     if (smooth && geom) fit_kernel<1, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (smooth) fit_kernel<1, 0><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (store && P.has_discs) fit_kernel<2, 2><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (store && geom) fit_kernel<2, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (store) fit_kernel<2, 0><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (P.has_discs) fit_kernel<0, 2><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);

@@ -84,10 +84,48 @@ __device__ __forceinline__ void smooth_one_layer(const Track& t, float k, float 
     l_next = l;
 }
 
+// The same for geometries with endcap discs (reading A23): the 15 stored covariance values are the upper triangle
+// over the layer's live coordinates (barrel: t z b1 b2 c, disc: r t b1 b2 c), see store_layer_state.
+__device__ __forceinline__ void filtered_from_tile_surface(Track& t, Sym5& C, const float* p) {
+    t.x = p[0];        t.y = p[32];       t.z = p[64];       t.px = p[96];      t.py = p[128];     t.pz = p[160];
+    int r = 6;
+#pragma unroll
+    for (int i = 0; i < 5; ++i)
+#pragma unroll
+        for (int j = i; j < 5; ++j) { const float v = p[32 * r++]; C.m[i][j] = v; C.m[j][i] = v; }
+    t.eax = p[672];    t.eay = p[704];
+}
+
+template <bool ELOSS>
+__device__ __forceinline__ void smooth_one_layer_surface(const Track& t, const Sym5& C, float k, float ik, const FitParams& P,
+                                                         int model, const FitArgs& a, int l, int64_t i, SmoothedNext& nx,
+                                                         int& l_next, bool& broken) {
+    const int type = P.layer[l].type;
+    SmoothedStateT<float> s = {t.x, t.y, t.z, t.px, t.py, t.pz};
+    Sym5 Cs = C;
+    if (l_next >= 0 && !broken) {
+        const uint32_t rc = rts_step_surface<ELOSS>(t, C, type, k, ik, P.layer[l_next], model, P.mass2, P.el, nx, s, Cs);
+        if (rc != 0u) {
+            broken = true;
+            a.status[i] |= ST_SMOOTH_FAIL;
+        }
+    }
+    Track g = t;
+    track_from_sym5_surface(Cs, type, g);
+    leave_local_frame(g);
+    store_smoothed(a, l, i, s.x, s.y, s.z, s.px, s.py, s.pz, g);
+    nx.x = s.x; nx.y = s.y; nx.z = s.z; nx.px = s.px; nx.py = s.py; nx.pz = s.pz;
+    nx.fpx = t.px; nx.fpy = t.py; nx.fpz = t.pz;
+    nx.fax = t.eax; nx.fay = t.eay;
+    nx.Cs = Cs;
+    l_next = l;
+}
+
 #ifndef KF_RTS_MIN_BLOCKS
 #define KF_RTS_MIN_BLOCKS 3
 #endif
-template <bool ELOSS>
+// SURFACES: the geometry has endcap discs (own instantiation: the dense step costs the barrel-only kernel nothing).
+template <bool ELOSS, bool SURFACES = false>
 __global__ void __launch_bounds__(kRtsBlock, KF_RTS_MIN_BLOCKS)
 rts_kernel(const __grid_constant__ FitParams P, const __grid_constant__ RtsMaps M, const FitArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -133,11 +171,14 @@ rts_kernel(const __grid_constant__ FitParams P, const __grid_constant__ RtsMaps 
         const int s = step % kRtsStages, l = L - 1 - step;
         mbar_wait(bar0 + 8u * s, (uint32_t)(step / kRtsStages) & 1u);
         Track t;
-        filtered_from_tile(t, wbase + s * kRtsTileFloats + lane);
+        Sym5 C;
+        if constexpr (SURFACES) filtered_from_tile_surface(t, C, wbase + s * kRtsTileFloats + lane);
+        else filtered_from_tile(t, wbase + s * kRtsTileFloats + lane);
         __syncwarp();   // every lane holds its values: the stage can be refilled
         if (step + kRtsStages < L && elect_one()) request(step + kRtsStages);
         if (!((used >> l) & 1u)) continue;
-        smooth_one_layer<ELOSS>(t, k, ik, P, model, a, l, i, nx, l_next, broken);
+        if constexpr (SURFACES) smooth_one_layer_surface<ELOSS>(t, C, k, ik, P, model, a, l, i, nx, l_next, broken);
+        else smooth_one_layer<ELOSS>(t, k, ik, P, model, a, l, i, nx, l_next, broken);
     }
 }
 
@@ -159,7 +200,10 @@ cudaError_t launch_rts(const FitParams& P, const FitArgs& a, cudaStream_t stream
     if (!make_map(&M.par, a.lpar, a.n, a.ld_l, (int64_t)L * 6, 6) || !make_map(&M.cov, a.lcov, a.n, a.ld_l, (int64_t)L * 21, 17))
         return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kRtsBlock - 1) / kRtsBlock;
-    if (P.model & MODEL_ENERGY_LOSS) rts_kernel<true><<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
+    if (P.has_discs) {
+        if (P.model & MODEL_ENERGY_LOSS) rts_kernel<true, true><<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
+        else rts_kernel<false, true><<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
+    } else if (P.model & MODEL_ENERGY_LOSS) rts_kernel<true><<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
     else rts_kernel<false><<<(unsigned)blocks, kRtsBlock, kRtsSmemBytes, stream>>>(P, M, a);
     return cudaGetLastError();
 }

@@ -98,6 +98,67 @@ def test_endcap_with_energy_loss(ctx):
         print(f"endcap toy with energy loss (material_model={mm}):", res)
 
 
+def _smooth_both(ctx, b):
+    from paper_1705_02876_b200.buffers import DeviceFit
+    d = DeviceFit.from_batch(b, "cuda:0")
+    d.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    with O.surfaces(b.surface_type, b.disc_z, b.disc_rmin, b.disc_rmax), \
+            O.geometry_options(int(getattr(b, "material_model", 0)), b.half_length, energy_loss=int(getattr(b, "energy_loss", 0))):
+        o = O.smooth_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask, nthreads=8)
+    return d, o
+
+
+@pytest.mark.parametrize("options", [(0, 0), (1, 1)])
+def test_endcap_smoother_parity(ctx, options):
+    """kf_fit_tracks_smooth on the barrel + endcap toy (reading A22 over the surfaces of reading A23): smoothed state and
+    covariance at every used layer, barrels and discs, at the fit tolerances; on a disc the smoothed covariance has no
+    variance along z.  Second case: path-length material + energy loss on both kinds of surface."""
+    from tests.parity import dense_from_packed
+    mm, el = options
+    b = W.simulate_endcap_event(9, 12000, material_model=mm)
+    b.energy_loss = el
+    d, o = _smooth_both(ctx, b)
+    g, sg = d.results(), d.smoothed_results()
+    same = (g["status"] == o["status"]) & (g["nhits"] == o["nhits"]) & (sg["used"] == o["used"])
+    assert same.mean() >= 0.995, same.mean()                  # (crossings within rounding of an edge: reading A20's rule)
+    assert np.array_equal((g["status"][same] & 32) != 0, o["sstatus"][same] != 0)
+    OUT = np.uint32(O.OUTSIDE)
+    worst = dict(pos=0.0, mom=0.0, cov=0.0)
+    n_disc = 0
+    for l in range(b.n_layers):
+        has = same & (((o["used"] >> l) & 1) == 1)
+        if not has.any():
+            continue
+        ndf = np.maximum(2 * o["nhits"] - 5, 1)
+        excl = ((o["status"] & ~OUT) | o["sstatus"] | ((o["chi2"] > ndf + 9 * np.sqrt(2.0 * ndf)).astype(np.uint32) << 6))[has]
+        so = dict(par=o["spar"][l][:, has], cov=o["scov"][has, l], chi2=np.zeros(has.sum()), nhits=o["nhits"][has], status=excl)
+        gg = dict(par=sg["par"][l][:, has], cov=sg["cov"][l][:, has], chi2=np.zeros(has.sum()), nhits=o["nhits"][has], status=excl)
+        scale = np.maximum(np.hypot(np.hypot(so["par"][0], so["par"][1]), so["par"][2]), 4.0)
+        res = compare_fit(gg, so, scale, max_diverged_frac=5e-3)
+        for k in worst:
+            worst[k] = max(worst[k], res[k])
+        if b.surface_type[l] == 1:
+            C = dense_from_packed(gg["cov"].astype(np.float64))
+            assert np.max(np.abs(C[:, 2, :])) == 0.0
+            n_disc += int(has.sum())
+    assert n_disc > 10000
+    print(f"endcap smoother (material_model={mm}, energy_loss={el}), worst over layers (1.0 = tolerance): {worst}")
+
+
+def test_endcap_smoother_ragged_sizes(ctx):
+    for n in (1, 33, 1001):
+        b = W.simulate_endcap_event(3, n)
+        d, o = _smooth_both(ctx, b)
+        g, sg = d.results(), d.smoothed_results()
+        same = (g["status"] == o["status"]) & (sg["used"] == o["used"])
+        assert same.mean() >= (0.98 if n > 1 else 0.0)
+        for l in range(b.n_layers):
+            has = same & (((o["used"] >> l) & 1) == 1) & (o["status"] == 0) & (o["sstatus"] == 0)
+            if has.any():
+                np.testing.assert_allclose(sg["par"][l][:, has], o["spar"][l][:, has], rtol=0, atol=2e-3)
+
+
 def test_endcap_indexed_fit_equals_pre_gathered(ctx):
     """kf_fit_tracks_indexed knows discs too: the same hits addressed by index give the same fit."""
     from paper_1705_02876_b200.buffers import DeviceFit, padded_ld
@@ -131,7 +192,7 @@ def test_discs_are_refused_where_they_are_not_implemented(ctx):
     from paper_1705_02876_b200.buffers import DeviceFit
     b = W.simulate_endcap_event(0, 64)
     d = DeviceFit.from_batch(b, "cuda:0")
-    for call in (lambda: d.fit_refit(ctx), lambda: d.fit_smooth(ctx)):
+    for call in (lambda: d.fit_refit(ctx),):
         with pytest.raises(K.KFError) as e:
             call()
         assert e.value.code == -4

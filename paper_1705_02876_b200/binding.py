@@ -375,6 +375,27 @@ class KFContext:
                     "kf_fit_tracks")
         del keep
 
+    def prepare_fit_tracks(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,
+                           out_par, out_cov, out_chi2, out_nhits, out_status):
+        """The marshalling of fit_tracks done once: returns a callable that enqueues the same kf_fit_tracks call
+        again (for event after event through the same tensors: the ctypes structures are what an eager
+        event-sized call spends most of its 20 us on).  The tensors must stay alive and in place."""
+        g, keep = geom._c()
+        seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
+        out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
+        hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
+        fn, h, check = self._lib.kf_fit_tracks, self._h, self._check
+        rg, rs, rh, ro = C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)
+        alive = (keep, g, seeds, out, hits, par, cov, q, hpos, hcov, mask, out_par, out_cov, out_chi2, out_nhits, out_status)
+
+        def launch(_alive=alive):
+            if not h.value or h.value != self._h.value:
+                raise KFError(-1, "kf_fit_tracks (prepared call: its context is closed)")
+            rc = fn(h, rg, rs, rh, ro)
+            if rc != 0:
+                check(rc, "kf_fit_tracks")
+        return launch
+
     def fit_tracks_indexed(self, geom: Geometry, n: int, par, cov, q, index, pools,
                            out_par, out_cov, out_chi2, out_nhits, out_status, bins=None):
         """Fit with hits addressed by index: index int32 [L][ld_index] (device), pools = [(n_hits, pos, cov), ...]

@@ -66,8 +66,15 @@ class DeviceFit:
             out_chi2=mk((ld,), torch.float32), out_nhits=mk((ld,), torch.int32), out_status=mk((ld,), torch.int32))
 
     def fit(self, ctx: KFContext):
-        ctx.fit_tracks(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask,
-                       self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status)
+        # the marshalled call is kept as long as the context and the tensors are the same objects
+        ts = (self.geom, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask,
+              self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status)
+        key = (id(ctx), ctx._h.value, self.n) + tuple(id(t) for t in ts)
+        cached = getattr(self, "_prepared_fit", None)
+        if cached is None or cached[0] != key:
+            cached = (key, ctx.prepare_fit_tracks(self.geom, self.n, *ts[1:]))
+            self._prepared_fit = cached
+        cached[1]()
 
     def fit_refit(self, ctx: KFContext, kappa: float = 10.0) -> dict:
         """kf_fit_tracks_refit; the forward result lands in the usual out_* tensors, the smoothed one in

@@ -302,7 +302,9 @@ KF_API int kf_fit_tracks_indexed(kf_ctx* ctx, const kf_geometry* geom, const kf_
 
 /* Bin one layer's hits: bin = i_eta*n_phi + i_phi with eta = asinh(z/radius), phi = atan2(y,x) over
  * [-pi, pi); stable counting sort (within a bin, original order).  The bin of a hit is decided in
- * single precision against tabulated edges (reading A16b).  `out` arrays are
+ * single precision against tabulated edges (reading A16b).  radius_cm = 0 says that the pool belongs to a
+ * DISC layer (reading A24): the bins stay projective, eta = asinh(z / rho) with each hit's own rho = sqrt(x^2 + y^2)
+ * (in the single-precision rule rho = fl(sqrt(fl(fl(x x) + fl(y y))))).  `out` arrays are
  * caller-allocated.  n_hits == 0 is valid (all offsets 0). */
 KF_API int kf_bin_hits(kf_ctx* ctx, float radius_cm, const kf_layer_hits* hits, kf_layer_bins* out);
 

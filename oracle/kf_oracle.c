@@ -869,6 +869,8 @@ int orc_fit_tracks(int64_t n, int L, const double *radius, const double *xX0, do
  *   i_phi = floor((phi + pi) / (2 pi / n_phi)) mod n_phi;  bin = i_eta * n_phi + i_phi.        */
 int32_t orc_bin_index_def(double x, double y, double z, double r_layer, int n_eta, int n_phi,
                           double eta_max) {
+    /* reading A24: r_layer = 0 says "a disc layer": the bins stay projective, eta from the point's own rho */
+    if (!(r_layer > 0.0)) r_layer = sqrt(x * x + y * y);
     double eta = asinh(z / r_layer), phi = atan2(y, x);
     int ie = (int)floor((eta + eta_max) / (2.0 * eta_max / n_eta));
     if (ie < 0) ie = 0;
@@ -890,6 +892,11 @@ int32_t orc_bin_index_def(double x, double y, double z, double r_layer, int n_et
  *   edge j".  Compiled with -ffp-contract=off: every product is rounded to float once. */
 int32_t orc_bin_index_f32(float x, float y, float z, float r_layer, int n_eta, int n_phi,
                           double eta_max) {
+    if (!(r_layer > 0.0f)) { /* reading A24 (disc layer): rho = fl(sqrt(fl(fl(x x) + fl(y y)))), every step rounded once */
+        volatile float xx = x * x, yy = y * y;
+        volatile float s2 = xx + yy;
+        r_layer = sqrtf(s2);
+    }
     volatile float u = z / r_layer;
     int ie = 0;
     for (int j = 1; j < n_eta; ++j) {

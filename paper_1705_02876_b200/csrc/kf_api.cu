@@ -495,7 +495,7 @@ int check_bin_args(const kf_layer_hits* hits, const kf_layer_bins* out, float ra
     if (hits->n_hits < 0 || hits->ld < hits->n_hits) return KF_ERR_SHAPE;
     if (out->n_eta < 1 || out->n_phi < 2) return KF_ERR_SHAPE;
     if (out->n_phi % 2 != 0 || (int64_t)out->n_eta * out->n_phi > KF_MAX_BINS) return KF_ERR_UNSUPPORTED;
-    if (!(radius_cm > 0.0f) || !(out->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;
+    if (!(radius_cm >= 0.0f) || !(out->eta_max > 0.0f)) return KF_ERR_UNSUPPORTED;   // (0: a disc layer, reading A24)
     if (hits->n_hits > 0x7fffffffLL) return KF_ERR_UNSUPPORTED;
     if (!out->bin_offset || !out->bin_box) return KF_ERR_NULL;
     if (!aligned16(out->bin_box)) return KF_ERR_ALIGN;

@@ -42,6 +42,8 @@ __device__ __forceinline__ int bin_of_hit(float x, float y, float z, float r, in
                                           const float* __restrict__ eta_edge,
                                           const float* __restrict__ phi_cos,
                                           const float* __restrict__ phi_sin) {
+    // reading A24: r = 0 says "a disc layer" -- eta from the hit's own rho, every operation rounded once
+    if (!(r > 0.0f)) r = __fsqrt_rn(__fadd_rn(__fmul_rn(x, x), __fmul_rn(y, y)));
     const float u = __fdiv_rn(z, r);
     // edges are non-decreasing in j, so "count of edges <= u" is an upper-bound search
     int lo = 1, hi = n_eta;
@@ -338,7 +340,9 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
         }
 #pragma unroll
         for (int it = 0; it < kCountPer; ++it) {
-            u[it] = __fdiv_rn(u[it], L.radius);
+            const float rr = L.radius > 0.0f ? L.radius      // (reading A24: radius 0 = a disc layer, the hit's own rho)
+                                             : __fsqrt_rn(__fadd_rn(__fmul_rn(x[it], x[it]), __fmul_rn(y[it], y[it])));
+            u[it] = __fdiv_rn(u[it], rr);
             const bool upper = y[it] > 0.0f || (y[it] == 0.0f && x[it] > 0.0f);
             pe[it] = 0;
             pp[it] = upper ? half : 0;

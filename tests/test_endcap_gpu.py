@@ -159,6 +159,40 @@ def test_endcap_smoother_ragged_sizes(ctx):
                 np.testing.assert_allclose(sg["par"][l][:, has], o["spar"][l][:, has], rtol=0, atol=2e-3)
 
 
+@pytest.mark.parametrize("form", [1, 2])
+def test_bin_hits_of_a_disc_layer(ctx, form):
+    """kf_bin_hits with radius 0 (reading A24: a disc layer, eta from each hit's own rho): bit-exact against the
+    oracle's sort by the same single-precision rule, both forms of the sort, and equal to the DOUBLE definition
+    except for hits within rounding of a bin edge."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceLayer
+    from tests import test_score_gpu as S
+    rng = np.random.default_rng(17 + form)
+    NEd, NPd, EMd = 50, 64, float(np.float32(2.5))
+    H = 60_000
+    rho, phi = rng.uniform(4.0, 26.0, H), rng.uniform(-np.pi, np.pi, H)
+    z = rng.choice([-45.0, 45.0], H)
+    pos = np.stack([rho * np.cos(phi), rho * np.sin(phi), z]).astype(np.float32)
+    cov = rng.uniform(1e-4, 1e-2, (6, H)).astype(np.float32)
+    ctx.set_option(K.OPT_BIN_FORM, form)
+    try:
+        dl = DeviceLayer.from_numpy(pos, cov, NEd, NPd, EMd, "cuda:0")
+        dl.bin(ctx, 0.0)
+        torch.cuda.synchronize()
+    finally:
+        ctx.set_option(K.OPT_BIN_FORM, K.BIN_FORM_AUTO)
+    ob = O.bin_hits(pos, 0.0, NEd, NPd, EMd)
+    S._assert_bins_equal(dl, ob, pos, cov)
+    x, y, zz = (pos[i].astype(np.float64) for i in range(3))
+    fe = (np.arcsinh(zz / np.hypot(x, y)) + EMd) / (2 * EMd / NEd)
+    fp = (np.arctan2(y, x) + np.pi) / (2 * np.pi / NPd)
+    def_bin = np.clip(np.floor(fe), 0, NEd - 1).astype(np.int64) * NPd + (np.floor(fp).astype(np.int64) % NPd)
+    differ = np.flatnonzero(ob["bin_of"] != def_bin)
+    assert len(differ) <= 5
+    for i in differ:
+        assert min(abs(fe[i] - np.round(fe[i])), abs(fp[i] - np.round(fp[i]))) < 1e-5
+
+
 def test_endcap_indexed_fit_equals_pre_gathered(ctx):
     """kf_fit_tracks_indexed knows discs too: the same hits addressed by index give the same fit."""
     from paper_1705_02876_b200.buffers import DeviceFit, padded_ld

@@ -33,6 +33,48 @@ def test_bin_rule_f32_equals_definition_away_from_edges():
     assert n_edge < 10
 
 
+def test_bin_rule_on_a_disc_layer():
+    """Reading A24: radius 0 = a disc layer, the bins stay projective with eta from the point's own rho.  The
+    definition with radius 0 is the textbook pseudorapidity of the point, -ln tan(theta / 2); the single-precision
+    rule agrees with it away from bin edges; a point's bin does not depend on which surface it is said to lie on
+    when that surface is the cylinder through it."""
+    rng = np.random.default_rng(6)
+    n = 20000
+    NEd, EMd = 50, 2.5
+    zd = 45.0
+    rho = rng.uniform(4.0, 26.0, n)
+    phi = rng.uniform(-np.pi, np.pi, n)
+    sign = rng.choice([-1.0, 1.0], n)
+    x, y, z = (rho * np.cos(phi)).astype(np.float32), (rho * np.sin(phi)).astype(np.float32), (sign * zd).astype(np.float32)
+    n_edge = 0
+    for i in range(n):
+        xd, yd, zz = float(x[i]), float(y[i]), float(z[i])
+        bd = O.bin_index_def(xd, yd, zz, 0.0, NEd, NP, EMd)
+        theta = np.arctan2(np.hypot(xd, yd), zz)
+        eta = -np.log(np.tan(0.5 * theta))
+        ie = int(np.clip(np.floor((eta + EMd) / (2 * EMd / NEd)), 0, NEd - 1))
+        ip = int(np.floor((np.arctan2(yd, xd) + np.pi) / (2 * np.pi / NP))) % NP
+        fe = (eta + EMd) / (2 * EMd / NEd)
+        if abs(fe - round(fe)) > 1e-9:
+            assert bd == ie * NP + ip
+        assert bd == O.bin_index_def(xd, yd, zz, np.hypot(xd, yd), NEd, NP, EMd)
+        bf = O.bin_index_f32(x[i], y[i], z[i], 0.0, NEd, NP, EMd)
+        if bd != bf:
+            fp = (np.arctan2(yd, xd) + np.pi) / (2 * np.pi / NP)
+            assert min(abs(fe - round(fe)), abs(fp - round(fp))) < 1e-4
+            n_edge += 1
+    assert n_edge < 10
+    # the sort itself: stable counting sort by that rule
+    pos = np.stack([x, y, z])
+    ob = O.bin_hits(pos, 0.0, NEd, NP, EMd)
+    assert np.array_equal(np.sort(ob["sorted_to_orig"]), np.arange(n))
+    b = np.array([O.bin_index_f32(x[i], y[i], z[i], 0.0, NEd, NP, EMd) for i in range(0, n, 37)])
+    assert np.array_equal(ob["bin_of"][::37], b)
+    assert np.all(np.diff(ob["bin_of"][ob["sorted_to_orig"]]) >= 0)
+    same = np.diff(ob["bin_of"][ob["sorted_to_orig"]]) == 0
+    assert np.all(np.diff(ob["sorted_to_orig"])[same] > 0)
+
+
 def test_bin_rule_special_directions():
     r = 10.0
     f = lambda x, y, z=0.0: O.bin_index_f32(x, y, z, r, NE, NP, EMAX)

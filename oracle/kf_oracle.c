@@ -71,6 +71,13 @@ void orc_set_surfaces(int n_layers, const int32_t *type, const double *disc_z, c
 
 static double g_score_half_length = INFINITY; /* the one layer orc_score_layer works on */
 void orc_set_score_half_length(double h) { g_score_half_length = h; }
+/* ... and its surface (readings A23 / A24): type 0 = the cylinder of radius r_layer, 1 = the disc pair z = +-zd with
+ * the annulus rmin <= rho <= rmax (r_layer is then not used). */
+static int g_score_type = 0;
+static double g_score_zd = 0.0, g_score_rmin = 0.0, g_score_rmax = INFINITY;
+void orc_set_score_surface(int type, double zd, double rmin, double rmax) {
+    g_score_type = type; g_score_zd = zd; g_score_rmin = rmin; g_score_rmax = rmax;
+}
 
 void orc_set_geometry_options(int material_model, int n_layers, const double *half_length) {
     g_material_model = material_model;
@@ -969,12 +976,25 @@ void orc_score_layer(int64_t n, double r_layer, double xX0, double Bz, double ma
         if (second_chi2) second_chi2[i] = INFINITY;
         if (q[i] != 1 && q[i] != -1) { status[i] |= ORC_BAD_CHARGE; continue; }
         double up[6], F[36], Q[36], Cp[36];
-        int rc = orc_propagate(u, (double)q[i], Bz, r_layer, up, F, NULL, NULL);
-        if (!rc && fabs(up[2]) > g_score_half_length) rc = ORC_OUTSIDE;
+        int rc;
+        if (g_score_type == 1) { /* reading A23: the disc on the side the candidate is heading to */
+            rc = orc_propagate_to_z(u, (double)q[i], Bz, u[5] < 0.0 ? -g_score_zd : g_score_zd, up, F, NULL, NULL);
+            if (!rc) {
+                double rho = sqrt(up[0] * up[0] + up[1] * up[1]);
+                if (rho < g_score_rmin || rho > g_score_rmax) rc = ORC_OUTSIDE;
+            }
+        } else {
+            rc = orc_propagate(u, (double)q[i], Bz, r_layer, up, F, NULL, NULL);
+            if (!rc && fabs(up[2]) > g_score_half_length) rc = ORC_OUTSIDE;
+        }
         if (rc) { status[i] |= (uint32_t)rc; continue; }
+        g_at_surface = g_score_type;
         orc_process_noise(up, mass, xX0, Q);
         orc_transport_cov(F, C, Q, Cp);
-        if (g_energy_loss && orc_energy_loss_step(up, Cp, mass, xX0, +1, NULL)) { status[i] |= ORC_PROP_FAIL; continue; } /* A21 */
+        int el_rc = g_energy_loss ? orc_energy_loss_step(up, Cp, mass, xX0, +1, NULL) : 0; /* A21 */
+        g_at_surface = 0;
+        if (el_rc) { status[i] |= ORC_PROP_FAIL; continue; }
+        const double r_bins = g_score_type == 1 ? 0.0 : r_layer; /* reading A24: on a disc, eta from the point's own rho */
         double best = INFINITY, second = INFINITY;
         int32_t bh = -1;
         if (all_hits) {
@@ -985,7 +1005,7 @@ void orc_score_layer(int64_t n, double r_layer, double xX0, double Bz, double ma
                 else if (c < second) second = c;
             }
         } else {
-            int cb = orc_bin_index_def(up[0], up[1], up[2], r_layer, n_eta, n_phi, eta_max);
+            int cb = orc_bin_index_def(up[0], up[1], up[2], r_bins, n_eta, n_phi, eta_max);
             int ie = cb / n_phi, ip = cb % n_phi;
             for (int de = -window_half; de <= window_half; ++de) {
                 int e = ie + de;

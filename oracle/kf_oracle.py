@@ -63,6 +63,8 @@ def lib():
         _lib.orc_set_geometry_options.argtypes = [C.c_int, C.c_int, dp]
         _lib.orc_set_score_half_length.restype = None
         _lib.orc_set_score_half_length.argtypes = [C.c_double]
+        _lib.orc_set_score_surface.restype = None
+        _lib.orc_set_score_surface.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double]
         _lib.orc_set_surfaces.restype = None
         _lib.orc_set_surfaces.argtypes = [C.c_int, C.POINTER(C.c_int32), dp, dp, dp]
         _lib.orc_propagate_to_z.restype = C.c_int
@@ -105,6 +107,21 @@ class geometry_options:
         lib().orc_set_geometry_options(0, 0, None)
         lib().orc_set_energy_loss(0)
         lib().orc_set_score_half_length(float("inf"))
+
+
+class score_surface:
+    """Context manager: the ONE layer score_layer works on is a disc pair z = +-zd with the annulus rmin <= rho <=
+    rmax (readings A23 / A24; r_layer is then unused and the bins passed in must have been made with radius 0)."""
+
+    def __init__(self, zd: float, rmin: float, rmax: float):
+        self.a = (1, float(zd), float(rmin), float(rmax))
+
+    def __enter__(self):
+        lib().orc_set_score_surface(*self.a)
+        return self
+
+    def __exit__(self, *a):
+        lib().orc_set_score_surface(0, 0.0, 0.0, float("inf"))
 
 
 class surfaces:

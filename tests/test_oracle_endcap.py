@@ -199,3 +199,70 @@ def test_D6_path_length_material_on_a_disc():
             np.testing.assert_allclose(w[1:], th0 ** 2 * pp * pp, rtol=1e-10)
             checked += 1
     assert checked >= 20
+
+
+def test_D7_scoring_on_a_disc_layer():
+    """orc_score_layer on a disc (readings A23 / A24).  (i) Glue: with ONLY each track's own hit in the pool, a chain
+    of score_layer calls with do_update over the layers reproduces the filter (orc_fit_tracks with the surface list)
+    on the tracks that have every hit they cross: same surfaces, same noise, same update.  (ii) The window search
+    equals brute force over every hit of the layer wherever the brute-force winner passes the cut (a hit 30 chi2
+    units away lies well inside +-2 bins).  (iii) Candidates mostly take their own hit; a disc the candidate misses
+    sets OUTSIDE and changes nothing."""
+    NEd, NPd, EMd = 50, 64, 2.5
+    ev = W.make_endcap_build_event(500, 3000, event=3)
+    f = ev.fit
+    L = f.n_layers
+    seeds = O.Candidates(f.par, f.cov, f.q)
+    ref = O.fit_batch(f)
+
+    def score(c, l, pos, cov, all_hits=False, do_update=True):
+        ob = None if all_hits else O.bin_hits(pos, 0.0 if f.surface_type[l] == 1 else float(f.radius[l]), NEd, NPd, EMd)
+        if f.surface_type[l] == 1:
+            with O.score_surface(f.disc_z[l], f.disc_rmin[l], f.disc_rmax[l]):
+                return O.score_layer(c, 0.0, f.x_over_X0[l], f.Bz, f.mass, pos, cov, ob, NEd, NPd, EMd, 2, 30.0, do_update, all_hits)
+        with O.geometry_options(0, f.half_length, score_layer=l):
+            return O.score_layer(c, f.radius[l], f.x_over_X0[l], f.Bz, f.mass, pos, cov, ob, NEd, NPd, EMd, 2, 30.0, do_update, all_hits)
+
+    # (i) own hit only (one candidate and its one hit per call, so that no neighbour's hit can win), cut wide open
+    followed = [np.flatnonzero(((f.mask >> l) & 1) == 1)[:60] for l in range(L)]
+    for l in range(L):
+        for i in followed[l]:
+            one = O.Candidates(f.par[:, i:i + 1], f.cov[:, i:i + 1], f.q[i:i + 1])
+            one.par[:], one.cov[:], one.chi2[:], one.nhits[:] = seeds.par[i], seeds.cov[i], seeds.chi2[i], seeds.nhits[i]
+            hp, hc = f.hpos[l][:, i:i + 1], f.hcov[l][:, i:i + 1]
+            if f.surface_type[l] == 1:
+                with O.score_surface(f.disc_z[l], f.disc_rmin[l], f.disc_rmax[l]):
+                    O.score_layer(one, 0.0, f.x_over_X0[l], f.Bz, f.mass, hp, hc, None, NEd, NPd, EMd, 2, 1e30, True, True)
+            else:
+                with O.geometry_options(0, f.half_length, score_layer=l):
+                    O.score_layer(one, f.radius[l], f.x_over_X0[l], f.Bz, f.mass, hp, hc, None, NEd, NPd, EMd, 2, 1e30, True, True)
+            seeds.par[i], seeds.cov[i], seeds.chi2[i], seeds.nhits[i] = one.par[0], one.cov[0], one.chi2[0], one.nhits[0]
+            seeds.status[i] |= one.status[0]
+    chk = [i for i in range(f.n) if ref["status"][i] == 0 and seeds.status[i] == 0 and ref["nhits"][i] == bin(int(f.mask[i])).count("1")
+           and all(i in followed[l] for l in range(L) if (f.mask[i] >> l) & 1)]
+    assert len(chk) >= 20
+    for i in chk:
+        np.testing.assert_allclose(seeds.par[i], ref["par"][:, i], rtol=1e-9, atol=1e-9)
+        assert np.max(np.abs(seeds.cov[i] - ref["cov"][i])) < 1e-9 * np.max(np.abs(ref["cov"][i]))
+        assert abs(seeds.chi2[i] - ref["chi2"][i]) < 1e-9 * max(1.0, ref["chi2"][i])
+
+    # (ii) + (iii) on the disc layers, candidates = the oracle's fit of the barrel part
+    with O.surfaces(f.surface_type[:6], f.disc_z[:6], f.disc_rmin[:6], f.disc_rmax[:6]), O.geometry_options(0, f.half_length[:6]):
+        r6 = O.fit_tracks(f.radius[:6], f.x_over_X0[:6], f.Bz, f.mass, f.par, f.cov, f.q, f.hpos[:6], f.hcov[:6], f.mask & 63)
+    n_right = n_has = 0
+    for l in range(6, L):
+        lay = ev.layers[l]
+        a = O.Candidates(r6["par"].astype(np.float32), O.pack_cov21(r6["cov"]).astype(np.float32), f.q, r6["chi2"], r6["nhits"])
+        b = O.Candidates(r6["par"].astype(np.float32), O.pack_cov21(r6["cov"]).astype(np.float32), f.q, r6["chi2"], r6["nhits"])
+        before = a.par.copy()
+        wa = score(a, l, lay.pos, lay.cov)
+        wb = score(b, l, lay.pos, lay.cov, all_hits=True)
+        in_cut = wb["best_chi2"] < 30.0
+        assert np.array_equal(wa["best_hit"][in_cut], wb["best_hit"][in_cut])
+        np.testing.assert_allclose(wa["best_chi2"][in_cut], wb["best_chi2"][in_cut], rtol=0, atol=0)
+        assert np.array_equal(a.par[in_cut], b.par[in_cut])
+        out = (a.status & O.OUTSIDE) != 0
+        assert np.array_equal(a.par[out], before[out]) and np.all(wa["best_hit"][out] == -1)
+        has = (lay.true_index >= 0) & (r6["status"] == 0) & (r6["nhits"] >= 3)
+        n_has += int(has.sum()); n_right += int((wa["best_hit"][has] == lay.true_index[has]).sum())
+    assert n_has > 150 and n_right > 0.9 * n_has

@@ -460,3 +460,41 @@ def make_build_event(config: int = 4, n_tracks: int | None = None, noise_hits: i
                                 cov=np.ascontiguousarray(cov[:, perm], dtype=np.float32),
                                 true_index=inv[:fit.n].astype(np.int32)))
     return BuildEvent(cfg=cfg, fit=fit, layers=layers)
+
+
+@dataclass
+class EndcapBuildEvent:
+    """The barrel + endcap toy as a building workload: the event's tracks plus, per surface, ALL its hits (the
+    tracks' own hits where they left one, and uniform noise), shuffled, fp32 SoA."""
+    fit: FitBatch
+    layers: list[LayerHits]     # radius = 0 for a disc layer (reading A24); true_index = -1 where the track left no hit
+
+
+def make_endcap_build_event(n_tracks: int = 3000, noise_hits: int = 15000, event: int = 0, **kw) -> EndcapBuildEvent:
+    fit = simulate_endcap_event(event, n_tracks, **kw)
+    rng = np.random.default_rng(BASE_SEED + 77000 + event)
+    layers = []
+    for l in range(fit.n_layers):
+        has = ((fit.mask >> l) & 1) == 1
+        phi = rng.uniform(-np.pi, np.pi, size=noise_hits)
+        if fit.surface_type[l] == 1:
+            rho = np.sqrt(rng.uniform(fit.disc_rmin[l] ** 2, fit.disc_rmax[l] ** 2, size=noise_hits))
+            z = rng.choice([-1.0, 1.0], size=noise_hits) * fit.disc_z[l]
+            r_bins = 0.0
+        else:
+            rho = np.full(noise_hits, float(fit.radius[l]))
+            hl = float(fit.half_length[l]) if fit.half_length is not None else 30.0
+            z = rng.uniform(-hl, hl, size=noise_hits)
+            r_bins = float(fit.radius[l])
+        npos = np.stack([rho * np.cos(phi), rho * np.sin(phi), z])
+        pos = np.concatenate([fit.hpos[l][:, has].astype(np.float64), npos], axis=1)
+        cov = np.concatenate([fit.hcov[l][:, has].astype(np.float64), hit_covariance(phi)], axis=1)
+        H = pos.shape[1]
+        perm = rng.permutation(H)
+        inv = np.empty(H, dtype=np.int64)
+        inv[perm] = np.arange(H)
+        true_index = np.full(fit.n, -1, dtype=np.int32)
+        true_index[has] = inv[:int(has.sum())].astype(np.int32)
+        layers.append(LayerHits(radius=r_bins, pos=np.ascontiguousarray(pos[:, perm], dtype=np.float32),
+                                cov=np.ascontiguousarray(cov[:, perm], dtype=np.float32), true_index=true_index))
+    return EndcapBuildEvent(fit=fit, layers=layers)

@@ -590,7 +590,7 @@ int build_best_hit(kf_ctx* c, const kf_geometry* geom, int first_layer, int n_bu
                    float* local_state) {
     if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);   // (discs: readings A23 / A24)
     if (rc) return rc;
     if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
     if ((rc = check_tracks(cands, true, true))) return rc;
@@ -838,7 +838,7 @@ int kf_score_candidates_static(kf_ctx* c, const kf_geometry* geom, int layer, kf
                                float* best_chi2, float* local_state) {
     if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if (layer < 0 || layer >= geom->n_layers) return KF_ERR_SHAPE;
     if ((rc = check_tracks(cands, true, true))) return rc;

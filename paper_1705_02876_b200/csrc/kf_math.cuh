@@ -898,6 +898,32 @@ __device__ __forceinline__ uint32_t kalman_update_disc(Track& t, const DiscCross
     return 0u;
 }
 
+// chi2 of one hit against a candidate propagated to a DISC (C' has no variance along z): the z component of
+// S = C'_pp + V~ is eliminated first, as in kalman_update_disc; n_rr, n_rt, n_tt = the in-plane block of C'.
+__device__ __forceinline__ bool chi2_schur_disc(float nrr, float nrt, float ntt, const LocalHit& h, float& chi2) {
+    const float iv = rcp_fast(h.vzz);
+    const float sa = h.vrz * iv, sb = h.vtz * iv;
+    const float srr = nrr + (h.vrr - sa * h.vrz), srt = nrt + (h.vrt - sa * h.vtz), stt = ntt + (h.vtt - sb * h.vtz);
+    const float rr = h.rr - sa * h.rz, rt = h.rt - sb * h.rz;
+    const float det2 = srr * stt - srt * srt;
+    const float q = stt * rr * rr - 2.0f * srt * rr * rt + srr * rt * rt;
+    chi2 = h.rz * h.rz * iv + q * rcp_fast(det2);
+    return h.vzz * det2 > 0.0f;
+}
+
+// Keep the state propagated to a disc (no hit used).
+__device__ __forceinline__ void commit_propagated_disc(Track& t, const DiscCrossing& o, const DiscCov& n) {
+    t.x = o.xn; t.y = o.yn; t.z = o.zt; t.px = o.pxn; t.py = o.pyn;
+    t.eax = o.erx; t.eay = o.ery;
+    t.c00 = n.rr; t.c01 = n.rt; t.c11 = n.tt;
+    t.c02 = 0.0f; t.c12 = 0.0f; t.c22 = 0.0f; t.c23 = 0.0f; t.c24 = 0.0f; t.c25 = 0.0f;
+    t.c03 = n.r3; t.c04 = n.r4; t.c05 = n.r5;
+    t.c13 = n.t3; t.c14 = n.t4; t.c15 = n.t5;
+    t.c33 = n.n33; t.c34 = n.n34; t.c35 = n.n35;
+    t.c44 = n.n44; t.c45 = n.n45;
+    t.c55 = n.n55;
+}
+
 // Keep the propagated state (no hit used): position frame = arrival frame, momentum frame
 // already follows the propagated momentum.
 __device__ __forceinline__ void commit_propagated(Track& t, const Crossing& o, const PropCov& n) {

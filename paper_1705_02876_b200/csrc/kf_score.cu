@@ -37,14 +37,36 @@ namespace {
 // candidate after this layer in the local frame.
 // MULTI: the call builds several events at once (EventPools); compiled out of the single-event kernels, whose
 // inner loops it would otherwise cost 9 % (measured: 0.177 -> 0.194 ms per configs[4] build).
+// disc: the layer the candidate stands at is a disc (readings A23 / A24).
 template <bool MULTI>
-__device__ __forceinline__ void apply_decision(const ScoreArgs& a, int64_t i, Track& t) {
+__device__ __forceinline__ void apply_decision(const ScoreArgs& a, int64_t i, Track& t, bool disc = false) {
+    const int32_t slot = a.slot[i];
+    if (disc) {
+        DiscCrossing o;
+        DiscCov n;
+        float pz;
+        get_scratch_disc(a.scratch, a.ld_sc, i, o, n, pz);
+        t.pz = pz;
+        bool updated = false;
+        if (slot >= 0 && a.do_update) {
+            Crossing c;                       // what hit_to_local reads of it
+            c.xn = o.xn; c.yn = o.yn; c.zn = o.zt; c.erx = o.erx; c.ery = o.ery;
+            LocalHit h;
+            const float* recs = MULTI ? a.ev.hit_rec[event_of(a.ev, i)] : a.hit_rec;
+            hit_from_record(reinterpret_cast<const float4*>(recs), slot, c, h);
+            float d;
+            const uint32_t rc = kalman_update_disc(t, o, n, h, &d);
+            if (rc == 0u) { updated = true; a.chi2[i] += d; a.nhits[i] += 1; }
+            else a.status[i] |= rc;
+        }
+        if (!updated) commit_propagated_disc(t, o, n);
+        return;
+    }
     Crossing o;
     PropCov n;
     float pz;
     get_scratch(a.scratch, a.ld_sc, i, o, n, pz);
     t.pz = pz;
-    const int32_t slot = a.slot[i];
     bool updated = false;
     if (slot >= 0 && a.do_update) {
         LocalHit h;
@@ -77,8 +99,10 @@ propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
     }
     if (keep_track) put_track(a.track, a.ld_sc, i, t);
     const float k = (float)q * P.k0, ik = (float)q * P.inv_k0;
-    const uint32_t rc = propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.model, P.mass2, P.el,
-                                                    BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch, a.ld_sc, i);
+    const BinGrid grid{a.n_eta, a.n_phi, a.eta_max};
+    const uint32_t rc = P.layer[layer].type == 1
+        ? propagate_to_scratch_disc(t, k, ik, P.layer[layer], P.model, P.mass2, P.el, grid, a.scratch, a.ld_sc, i)
+        : propagate_to_scratch<false>(t, k, ik, P.layer[layer], P.model, P.mass2, P.el, grid, a.scratch, a.ld_sc, i);
     if (rc) a.status[i] |= rc;
     a.flag[i] = rc ? FLAG_IDLE : FLAG_AT_LAYER;
 }
@@ -86,18 +110,20 @@ propagate_global_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
 // Middle step of kf_build_best_hit: decision of the previous layer, then on to `layer`.
 template <bool MULTI>
 __global__ void __launch_bounds__(kCandBlock)
-update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, int layer) {
+update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, int layer, int prev_layer) {
     pdl_start();
     const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
     if (i >= a.n) return;
     const int32_t f = a.flag[i];
     if (f == FLAG_DEAD) return;
     Track t;
-    if (f == FLAG_AT_LAYER) { apply_decision<MULTI>(a, i, t); put_track(a.track, a.ld_sc, i, t); }
+    if (f == FLAG_AT_LAYER) { apply_decision<MULTI>(a, i, t, P.layer[prev_layer].type == 1); put_track(a.track, a.ld_sc, i, t); }
     else get_track(a.track, a.ld_sc, i, t);
     const float qf = (float)a.q[i];
-    const uint32_t rc = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model,
-                                                    P.mass2, P.el, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch,
+    const BinGrid grid{a.n_eta, a.n_phi, a.eta_max};
+    const uint32_t rc = P.layer[layer].type == 1
+        ? propagate_to_scratch_disc(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model, P.mass2, P.el, grid, a.scratch, a.ld_sc, i)
+        : propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model, P.mass2, P.el, grid, a.scratch,
                                                     a.ld_sc, i);
     if (rc) a.status[i] |= rc;
     a.flag[i] = rc ? FLAG_IDLE : FLAG_AT_LAYER;
@@ -107,14 +133,14 @@ update_propagate_kernel(const __grid_constant__ FitParams P, const ScoreArgs a, 
 // have_track = 0 (single-layer call): a candidate that did not reach the layer is left untouched.
 template <bool MULTI>
 __global__ void __launch_bounds__(kCandBlock)
-update_global_kernel(const ScoreArgs a, int have_track) {
+update_global_kernel(const ScoreArgs a, int have_track, int disc) {
     pdl_start();
     const int64_t i = (int64_t)blockIdx.x * kCandBlock + threadIdx.x;
     if (i >= a.n) return;
     const int32_t f = a.flag[i];
     if (f == FLAG_DEAD) return;
     Track t;
-    if (f == FLAG_AT_LAYER) apply_decision<MULTI>(a, i, t);
+    if (f == FLAG_AT_LAYER) apply_decision<MULTI>(a, i, t, disc != 0);
     else if (have_track) get_track(a.track, a.ld_sc, i, t);
     else return;
     if (a.lstate) {   // the candidate as it stands now, in the local frame, for the next per-layer call
@@ -125,7 +151,9 @@ update_global_kernel(const ScoreArgs a, int have_track) {
     store_track(t, a.par, a.cov, a.ld, i);
 }
 
-template <bool MULTI>
+// DISC: the layer is a disc pair (readings A23 / A24): the candidate's live position coordinates are (r, t) in the
+// plane instead of (t, z) on the cylinder, so the two Cauchy-Schwarz bounds are taken along r-hat and t-hat.
+template <bool MULTI, bool DISC = false>
 __global__ void __launch_bounds__(kScanBlock)
 scan_kernel(const ScoreArgs a, float inv_r) {
     pdl_start();
@@ -185,6 +213,13 @@ scan_kernel(const ScoreArgs a, float inv_r) {
                 const float lo = fminf(ax * x0, ax * x1) + fminf(ay * y0, ay * y1);
                 const float hi = fmaxf(ax * x0, ax * x1) + fmaxf(ay * y0, ay * y1);
                 const float rtm = lo > 0.0f ? lo : (hi < 0.0f ? -hi : 0.0f);
+                if constexpr (DISC) {
+                    // rr(x, y) = ec (x - xn) + es (y - yn) over the box; any in-plane variance of a hit <= vxx + vyy
+                    const float lor = fminf(c.ec * x0, c.ec * x1) + fminf(c.es * y0, c.es * y1);
+                    const float hir = fmaxf(c.ec * x0, c.ec * x1) + fmaxf(c.es * y0, c.es * y1);
+                    const float rrm = lor > 0.0f ? lor : (hir < 0.0f ? -hir : 0.0f);
+                    keep = (s1 > s0) & (rrm * rrm <= thr * (c.n11 + Z.w)) & (rtm * rtm <= thr * (c.n22 + Z.w));
+                } else
                 keep = (s1 > s0) & (dzm * dzm <= thr * (c.n22 + Z.z)) & (rtm * rtm <= thr * (c.n11 + Z.w));
             }
         }
@@ -206,8 +241,18 @@ scan_kernel(const ScoreArgs a, float inv_r) {
                 const float rt1 = c.ec * (A1.y - c.yn) - c.es * (A1.x - c.xn);
                 const float vt0 = ess * B0.x - ecs2 * B0.y + ecc * B0.z;
                 const float vt1 = ess * B1.x - ecs2 * B1.y + ecc * B1.z;
-                const bool pA = vA & (dz0 * dz0 <= thr * (c.n22 + A0.w)) & (rt0 * rt0 <= thr * (c.n11 + vt0));
-                const bool pB = vB & (dz1 * dz1 <= thr * (c.n22 + A1.w)) & (rt1 * rt1 <= thr * (c.n11 + vt1));
+                bool pA, pB;
+                if constexpr (DISC) {
+                    const float rr0 = c.ec * (A0.x - c.xn) + c.es * (A0.y - c.yn);
+                    const float rr1 = c.ec * (A1.x - c.xn) + c.es * (A1.y - c.yn);
+                    const float vr0 = ecc * B0.x + ecs2 * B0.y + ess * B0.z;
+                    const float vr1 = ecc * B1.x + ecs2 * B1.y + ess * B1.z;
+                    pA = vA & (rr0 * rr0 <= thr * (c.n11 + vr0)) & (rt0 * rt0 <= thr * (c.n22 + vt0));
+                    pB = vB & (rr1 * rr1 <= thr * (c.n11 + vr1)) & (rt1 * rt1 <= thr * (c.n22 + vt1));
+                } else {
+                    pA = vA & (dz0 * dz0 <= thr * (c.n22 + A0.w)) & (rt0 * rt0 <= thr * (c.n11 + vt0));
+                    pB = vB & (dz1 * dz1 <= thr * (c.n22 + A1.w)) & (rt1 * rt1 <= thr * (c.n11 + vt1));
+                }
                 const unsigned mA = __ballot_sync(0xffffffffu, pA);
                 const unsigned mB = __ballot_sync(0xffffffffu, pB);
                 if (pA) list[cnt + __popc(mA & lt_mask)] = sA;
@@ -223,7 +268,7 @@ scan_kernel(const ScoreArgs a, float inv_r) {
                     if (lane + 32 < cnt) list[lane] = c1;
                     if (lane + 64 < cnt) list[lane + 32] = c2;
                     cnt -= 32;
-                    score_hit(c, rec, sl, best);
+                    score_hit<DISC>(c, rec, sl, best);
                     float bmin = best.chi2;
 #pragma unroll
                     for (int d = 16; d > 0; d >>= 1) bmin = fminf(bmin, __shfl_xor_sync(0xffffffffu, bmin, d));
@@ -233,7 +278,7 @@ scan_kernel(const ScoreArgs a, float inv_r) {
         }
     }
     __syncwarp();
-    if (lane < cnt) score_hit(c, rec, list[lane], best);
+    if (lane < cnt) score_hit<DISC>(c, rec, list[lane], best);
     // warp arg-min on (chi2, original index)
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
@@ -294,18 +339,22 @@ cudaError_t launch_build(ScoreScratch& s, const FitParams& P, ScoreArgs a, int n
     for (int j = 0; j < n_steps; ++j) {
         const ScoreStep& st = steps[j];
         if (j == 0) ok(launch_chained(propagate_global_kernel, cgrid, cblock, 0, stream, P, a, st.layer, keep));
-        else if (multi) ok(launch_chained(update_propagate_kernel<true>, cgrid, cblock, 0, stream, P, a, st.layer));   // a.hit_rec still step j-1
-        else ok(launch_chained(update_propagate_kernel<false>, cgrid, cblock, 0, stream, P, a, st.layer));
+        else if (multi) ok(launch_chained(update_propagate_kernel<true>, cgrid, cblock, 0, stream, P, a, st.layer, steps[j - 1].layer));   // a.hit_rec still step j-1
+        else ok(launch_chained(update_propagate_kernel<false>, cgrid, cblock, 0, stream, P, a, st.layer, steps[j - 1].layer));
         a.hit_rec = st.hit_rec; a.bin_box = st.bin_box; a.bin_offset = st.bin_offset; a.n_hits = st.n_hits;
         a.best_hit = st.best_hit; a.best_chi2 = st.best_chi2;
         for (int e = 0; e < a.ev.n; ++e) {
             a.ev.hit_rec[e] = st.ev_hit_rec[e]; a.ev.bin_box[e] = st.ev_bin_box[e]; a.ev.bin_offset[e] = st.ev_bin_offset[e];
         }
-        if (multi) ok(launch_chained(scan_kernel<true>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r));
-        else ok(launch_chained(scan_kernel<false>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r));
+        const bool disc = P.layer[st.layer].type == 1;
+        if (multi) ok(disc ? launch_chained(scan_kernel<true, true>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r)
+                           : launch_chained(scan_kernel<true, false>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r));
+        else ok(disc ? launch_chained(scan_kernel<false, true>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r)
+                     : launch_chained(scan_kernel<false, false>, sgrid, sblock, 0, stream, a, P.layer[st.layer].inv_r));
     }
-    if (multi) ok(launch_chained(update_global_kernel<true>, cgrid, cblock, 0, stream, a, keep));
-    else ok(launch_chained(update_global_kernel<false>, cgrid, cblock, 0, stream, a, keep));
+    const int last_disc = P.layer[steps[n_steps - 1].layer].type == 1 ? 1 : 0;
+    if (multi) ok(launch_chained(update_global_kernel<true>, cgrid, cblock, 0, stream, a, keep, last_disc));
+    else ok(launch_chained(update_global_kernel<false>, cgrid, cblock, 0, stream, a, keep, last_disc));
     if (e2 != cudaSuccess) return e2;
     return cudaGetLastError();
 }
@@ -371,8 +420,10 @@ cudaError_t launch_score_static(const FitParams& P, ScoreArgs a, const ScoreStep
     propagate_global_kernel<<<cblocks, kCandBlock, 0, stream>>>(P, a, st.layer, 0);
     a.hit_rec = st.hit_rec; a.bin_box = st.bin_box; a.bin_offset = st.bin_offset; a.n_hits = st.n_hits;
     a.best_hit = st.best_hit; a.best_chi2 = st.best_chi2;
-    scan_kernel<false><<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
-    update_global_kernel<false><<<cblocks, kCandBlock, 0, stream>>>(a, 0);
+    const bool disc = P.layer[st.layer].type == 1;
+    if (disc) scan_kernel<false, true><<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
+    else scan_kernel<false, false><<<sblocks, kScanBlock, 0, stream>>>(a, P.layer[st.layer].inv_r);
+    update_global_kernel<false><<<cblocks, kCandBlock, 0, stream>>>(a, 0, disc ? 1 : 0);
     return cudaGetLastError();
 }
 

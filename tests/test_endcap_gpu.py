@@ -193,6 +193,86 @@ def test_bin_hits_of_a_disc_layer(ctx, form):
         assert min(abs(fe[i] - np.round(fe[i])), abs(fp[i] - np.round(fp[i]))) < 1e-5
 
 
+NEd, NPd, EMd = 50, 64, float(np.float32(2.5))
+
+
+def _endcap_seeds(f):
+    """Candidates = the oracle's fit of the first three (barrel) layers."""
+    with O.surfaces(f.surface_type[:3], f.disc_z[:3], f.disc_rmin[:3], f.disc_rmax[:3]), O.geometry_options(0, f.half_length[:3]):
+        r = O.fit_tracks(f.radius[:3], f.x_over_X0[:3], f.Bz, f.mass, f.par, f.cov, f.q, f.hpos[:3], f.hcov[:3], f.mask & 7)
+    return r["par"].astype(np.float32), O.pack_cov21(r["cov"]).astype(np.float32), r["chi2"], r["nhits"]
+
+
+def _oracle_score(oc, f, l, lay):
+    ob = O.bin_hits(lay.pos, lay.radius, NEd, NPd, EMd)
+    if f.surface_type[l] == 1:
+        with O.score_surface(f.disc_z[l], f.disc_rmin[l], f.disc_rmax[l]):
+            return O.score_layer(oc, 0.0, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NEd, NPd, EMd, 2, 30.0, True)
+    with O.geometry_options(0, f.half_length, score_layer=l):
+        return O.score_layer(oc, f.radius[l], f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, ob, NEd, NPd, EMd, 2, 30.0, True)
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_endcap_best_hit_building(ctx, fused):
+    """kf_score_candidates layer by layer (fused = False) and kf_build_best_hit in one call (True) on the barrel +
+    endcap toy: layers 3..5 are barrels, 6..9 disc pairs whose pools are binned with radius 0 (reading A24).  Hit
+    decisions by north_star's rule against the oracle's layer loop, status / hit counts equal (crossings within
+    rounding of an edge exempt, counted), final state at the fit tolerances."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    ev = W.make_endcap_build_event(6000, 30000, event=1)
+    f = ev.fit
+    L, L0 = f.n_layers, 3
+    par, cov, chi2, nh = _endcap_seeds(f)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, f.half_length, 0, 0, f.surface_type, f.disc_z, f.disc_rmin, f.disc_rmax)
+    dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    oc = O.Candidates(par, cov, f.q, chi2, nh)
+    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NEd, NPd, EMd, "cuda:0") for l in ev.layers[L0:]]
+    ctx.bin_layers([l.radius for l in ev.layers[L0:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+    if fused:
+        idx, c2 = dc.build(ctx, geom, L0, dls, 2, 30.0, True, None)
+        torch.cuda.synchronize()
+        idx, c2 = idx.cpu().numpy()[:, :f.n], c2.cpu().numpy()[:, :f.n]
+    alive = np.ones(f.n, dtype=bool)
+    n_dec = n_tie = n_disc_taken = 0
+    for j, l in enumerate(range(L0, L)):
+        lay = ev.layers[l]
+        if not fused:
+            dc.score(ctx, geom, l, dls[j], 2, 30.0, True)
+            torch.cuda.synchronize()
+            g = dc.results()
+            gh, gc = g["best_hit"], g["best_chi2"]
+        else:
+            gh, gc = idx[j], c2[j]
+        orr = _oracle_score(oc, f, l, lay)
+        if not fused:
+            # a crossing within rounding of an annulus / barrel edge may fall either side: such candidates leave the comparison
+            alive &= ((g["status"] ^ oc.status) & np.uint32(O.OUTSIDE | O.PROP_FAIL)) == 0
+        diff = (gh != orr["best_hit"]) & alive
+        b, s2 = orr["best_chi2"], orr["second_chi2"]
+        with np.errstate(invalid="ignore"):
+            tie = (np.abs(s2 - b) <= 1e-4 * np.abs(b)) | (np.abs(b - 30.0) <= 1e-4 * 30.0)
+        assert not np.any(diff & ~tie), f"layer {l}: {int((diff & ~tie).sum())} mismatches outside the tie window"
+        n_dec += int(alive.sum()); n_tie += int(diff.sum())
+        alive &= ~diff
+        acc = alive & (orr["best_hit"] >= 0)
+        assert (np.abs(gc[acc] - b[acc]) / np.maximum(b[acc], 1.0)).max(initial=0) < 1e-3
+        if f.surface_type[l] == 1:
+            n_disc_taken += int(acc.sum())
+    g = dc.results()
+    same = alive & (g["status"] == oc.status) & (g["nhits"] == oc.nhits)
+    assert same.sum() >= 0.985 * alive.sum(), (same.sum(), alive.sum())
+    assert alive.mean() > 0.97 and n_disc_taken > 4000
+    OUT = np.uint32(O.OUTSIDE)
+    sel = same & ((oc.status & ~OUT) == 0)
+    sub_g = {k: (g[k][..., sel] if k in ("par", "cov") else g[k][sel]) for k in ("par", "cov", "chi2", "nhits", "status")}
+    sub_o = dict(par=oc.par.T[:, sel], cov=oc.cov[sel], chi2=oc.chi2[sel], nhits=oc.nhits[sel], status=oc.status[sel] & ~OUT)
+    sub_g["status"] = sub_g["status"] & ~OUT
+    scale = np.maximum(np.hypot(np.hypot(sub_o["par"][0], sub_o["par"][1]), sub_o["par"][2]), 4.0)
+    res = compare_fit(sub_g, sub_o, scale, max_diverged_frac=1.0)
+    print(f"endcap building (fused={fused}): {n_dec} decisions, {n_tie} inside the tie window, {n_disc_taken} hits taken on discs; state: {res}")
+
+
 def test_endcap_indexed_fit_equals_pre_gathered(ctx):
     """kf_fit_tracks_indexed knows discs too: the same hits addressed by index give the same fit."""
     from paper_1705_02876_b200.buffers import DeviceFit, padded_ld
@@ -227,6 +307,19 @@ def test_discs_are_refused_where_they_are_not_implemented(ctx):
     b = W.simulate_endcap_event(0, 64)
     d = DeviceFit.from_batch(b, "cuda:0")
     for call in (lambda: d.fit_refit(ctx),):
+        with pytest.raises(K.KFError) as e:
+            call()
+        assert e.value.code == -4
+    # the combinatorial builder, the several-events and host forms of building and kf_order_candidates do not know discs
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    ev = W.make_endcap_build_event(64, 200)
+    f = ev.fit
+    par, cov, chi2, nh = _endcap_seeds(f)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, f.half_length, 0, 0, f.surface_type, f.disc_z, f.disc_rmin, f.disc_rmax)
+    dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NEd, NPd, EMd, "cuda:0") for l in ev.layers[3:]]
+    ctx.bin_layers([l.radius for l in ev.layers[3:]], [(x.n_hits, x.pos, x.cov, x.bins) for x in dls])
+    for call in (lambda: dc.build_combinatorial(ctx, geom, 3, dls, 4), lambda: dc.make_order(ctx, geom, 3, NEd, NPd, EMd)):
         with pytest.raises(K.KFError) as e:
             call()
         assert e.value.code == -4

@@ -1114,12 +1114,13 @@ void orc_build_combinatorial(int64_t n_seeds, int n_layers_total, int first_laye
             size_t nch = 0;
             for (int p = 0; p < nc; ++p) {
                 double up[6], F[36], Q[36], Cp[36];
-                int rc = orc_propagate(cur[p].u, (double)qq, Bz, radius[l], up, F, NULL, NULL);
-                if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
+                int rc = reach_surface(l, cur[p].u, (double)qq, Bz, radius[l], up, F); /* cylinder, or disc (A23) */
                 if (!rc) {
+                    g_at_surface = g_surface_type[l];
                     orc_process_noise(up, mass, xX0[l], Q);
                     orc_transport_cov(F, cur[p].C, Q, Cp);
                     if (g_energy_loss) rc = orc_energy_loss_step(up, Cp, mass, xX0[l], +1, NULL); /* A21 */
+                    g_at_surface = 0;
                 }
 #define ORC_ROOM() do { if (nch + 2 > cap) { cap *= 2; ch = (orc_child *)realloc(ch, sizeof(orc_child) * cap); } } while (0)
                 ORC_ROOM();
@@ -1131,7 +1132,7 @@ void orc_build_combinatorial(int64_t n_seeds, int n_layers_total, int first_laye
                 ch[nch].c = cur[p];
                 memcpy(ch[nch].c.u, up, sizeof up); memcpy(ch[nch].c.C, Cp, sizeof Cp);
                 ch[nch].parent = p; ch[nch].hit = -1; ++nch;
-                int cb = orc_bin_index_def(up[0], up[1], up[2], radius[l], n_eta, n_phi, eta_max);
+                int cb = orc_bin_index_def(up[0], up[1], up[2], g_surface_type[l] == 1 ? 0.0 : radius[l], n_eta, n_phi, eta_max); /* A24 */
                 int ie = cb / n_phi, ip = cb % n_phi;
                 for (int de = -window_half; de <= window_half; ++de) {
                     int e = ie + de;

@@ -639,7 +639,7 @@ int kf_build_best_hit_events(kf_ctx* c, const kf_geometry* geom, int first_layer
                              int32_t* hit_index, float* hit_chi2, int64_t ld_out) {
     if (!c || !geom || !cands || !hits || !bins || !event_first) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
     if (n_events < 1) return KF_ERR_SHAPE;
@@ -691,7 +691,7 @@ int kf_build_best_hit_host(kf_ctx* c, const kf_geometry* geom, int first_layer, 
     if (!c || !geom || !cands || !hits) return KF_ERR_NULL;
     if (c->capturing) return KF_ERR_UNSUPPORTED;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
     if ((rc = check_tracks(cands, true, false))) return rc;
@@ -728,7 +728,7 @@ int kf_build_combinatorial(kf_ctx* c, const kf_geometry* geom, int first_layer, 
                            int n_cand, int32_t* hit_index, int32_t* n_found, int64_t ld_out) {
     if (!c || !geom || !cands || !hits || !bins) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
     if (n_cand < 1 || n_cand > 8) return KF_ERR_UNSUPPORTED;
@@ -769,7 +769,7 @@ int kf_build_combinatorial_events(kf_ctx* c, const kf_geometry* geom, int first_
                                   int32_t* hit_index, int32_t* n_found, int64_t ld_out) {
     if (!c || !geom || !cands || !hits || !bins || !event_first) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if (n_build_layers < 0 || first_layer < 0 || first_layer + n_build_layers > geom->n_layers) return KF_ERR_SHAPE;
     if (n_cand < 1 || n_cand > 8) return KF_ERR_UNSUPPORTED;

@@ -73,8 +73,10 @@ comb_propagate_kernel(const __grid_constant__ FitParams P, const CombArgs a, int
     Track t;
     get_track(a.trk_in, a.ld_s, slot, t);
     const float qf = (float)a.q[sd];
-    const uint32_t rc = propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model,
-                                                    P.mass2, P.el, BinGrid{a.n_eta, a.n_phi, a.eta_max}, a.scratch,
+    const BinGrid grid{a.n_eta, a.n_phi, a.eta_max};
+    const uint32_t rc = P.layer[layer].type == 1       // readings A23 / A24: a disc layer
+        ? propagate_to_scratch_disc(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model, P.mass2, P.el, grid, a.scratch, a.ld_s, slot)
+        : propagate_to_scratch<false>(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], P.model, P.mass2, P.el, grid, a.scratch,
                                                     a.ld_s, slot);
     if (rc) a.st_in[slot] |= rc;   // its one child (REC_STUCK) inherits the reason
     a.flag[slot] = rc ? FLAG_IDLE : FLAG_AT_LAYER;
@@ -126,7 +128,8 @@ __device__ __forceinline__ int acc_top(AccEntry* acc, int n, int keep, int lane)
 }
 
 // MULTI: several events in one call (EventPools), compiled out of the single-event kernel as in kf_score.cu.
-template <bool MULTI>
+// DISC: the layer is a disc pair (bounds along r and t in the plane, as in scan_kernel of kf_score.cu).
+template <bool MULTI, bool DISC = false>
 __global__ void __launch_bounds__(kScanBlock)
 comb_scan_kernel(const CombArgs a, float inv_r) {
     __shared__ int32_t survivors[kScanBlock / 32][96];
@@ -161,7 +164,7 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
         __syncwarp();
         Best b;
         b.chi2 = CUDART_INF_F; b.orig = 0x7fffffff; b.slot = -1;
-        if (lane < n_take) score_hit(c, rec, list[lane], b);
+        if (lane < n_take) score_hit<DISC>(c, rec, list[lane], b);
         const bool ok = b.slot >= 0 && b.chi2 < a.chi2_cut;
         const unsigned m = __ballot_sync(0xffffffffu, ok);
         if (ok) { AccEntry e; e.chi2 = b.chi2; e.orig = b.orig; e.rec = b.slot; acc[nacc + __popc(m & lt_mask)] = e; }
@@ -191,6 +194,12 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
                 const float lo = fminf(ax * x0, ax * x1) + fminf(ay * y0, ay * y1);
                 const float hi = fmaxf(ax * x0, ax * x1) + fmaxf(ay * y0, ay * y1);
                 const float rtm = lo > 0.0f ? lo : (hi < 0.0f ? -hi : 0.0f);
+                if constexpr (DISC) {
+                    const float lor = fminf(c.ec * x0, c.ec * x1) + fminf(c.es * y0, c.es * y1);
+                    const float hir = fmaxf(c.ec * x0, c.ec * x1) + fmaxf(c.es * y0, c.es * y1);
+                    const float rrm = lor > 0.0f ? lor : (hir < 0.0f ? -hir : 0.0f);
+                    keep = (s1 > s0) & (rrm * rrm <= thr * (c.n11 + Z.w)) & (rtm * rtm <= thr * (c.n22 + Z.w));
+                } else
                 keep = (s1 > s0) & (dzm * dzm <= thr * (c.n22 + Z.z)) & (rtm * rtm <= thr * (c.n11 + Z.w));
             }
         }
@@ -211,8 +220,18 @@ comb_scan_kernel(const CombArgs a, float inv_r) {
                 const float rt1 = c.ec * (A1.y - c.yn) - c.es * (A1.x - c.xn);
                 const float vt0 = ess * B0.x - ecs2 * B0.y + ecc * B0.z;
                 const float vt1 = ess * B1.x - ecs2 * B1.y + ecc * B1.z;
-                const bool pA = vA & (dz0 * dz0 <= thr * (c.n22 + A0.w)) & (rt0 * rt0 <= thr * (c.n11 + vt0));
-                const bool pB = vB & (dz1 * dz1 <= thr * (c.n22 + A1.w)) & (rt1 * rt1 <= thr * (c.n11 + vt1));
+                bool pA, pB;
+                if constexpr (DISC) {
+                    const float rr0 = c.ec * (A0.x - c.xn) + c.es * (A0.y - c.yn);
+                    const float rr1 = c.ec * (A1.x - c.xn) + c.es * (A1.y - c.yn);
+                    const float vr0 = ecc * B0.x + ecs2 * B0.y + ess * B0.z;
+                    const float vr1 = ecc * B1.x + ecs2 * B1.y + ess * B1.z;
+                    pA = vA & (rr0 * rr0 <= thr * (c.n11 + vr0)) & (rt0 * rt0 <= thr * (c.n22 + vt0));
+                    pB = vB & (rr1 * rr1 <= thr * (c.n11 + vr1)) & (rt1 * rt1 <= thr * (c.n22 + vt1));
+                } else {
+                    pA = vA & (dz0 * dz0 <= thr * (c.n22 + A0.w)) & (rt0 * rt0 <= thr * (c.n11 + vt0));
+                    pB = vB & (dz1 * dz1 <= thr * (c.n22 + A1.w)) & (rt1 * rt1 <= thr * (c.n11 + vt1));
+                }
                 const unsigned mA = __ballot_sync(0xffffffffu, pA);
                 const unsigned mB = __ballot_sync(0xffffffffu, pB);
                 if (pA) list[cnt + __popc(mA & lt_mask)] = sA;
@@ -326,7 +345,7 @@ comb_select_kernel(const CombArgs a) {
 // One thread per surviving child: materialise it in the other half of the candidate store.
 template <bool MULTI>
 __global__ void __launch_bounds__(128)
-comb_update_kernel(const CombArgs a) {
+comb_update_kernel(const CombArgs a, int disc) {
     const int64_t so = (int64_t)blockIdx.x * 128 + threadIdx.x;
     if (so >= a.n_slots) return;
     const int64_t sd = so / a.nc;
@@ -339,6 +358,24 @@ comb_update_kernel(const CombArgs a) {
     uint32_t st = a.st_in[sp];
     if (r == REC_STUCK) {
         get_track(a.trk_in, a.ld_s, sp, t);   // st already carries ST_PROP_FAIL / ST_OUTSIDE (comb_propagate_kernel)
+    } else if (disc) {
+        DiscCrossing o;
+        DiscCov n;
+        float pz;
+        get_scratch_disc(a.scratch, a.ld_s, sp, o, n, pz);
+        t.pz = pz;
+        bool updated = false;
+        if (r >= 0) {
+            Crossing c;                       // what hit_to_local reads of it
+            c.xn = o.xn; c.yn = o.yn; c.zn = o.zt; c.erx = o.erx; c.ery = o.ery;
+            LocalHit h;
+            const float* recs = MULTI ? a.ev.hit_rec[event_of(a.ev, sd)] : a.hit_rec;
+            hit_from_record(reinterpret_cast<const float4*>(recs), r, c, h);
+            float d;
+            const uint32_t rc = kalman_update_disc(t, o, n, h, &d);
+            if (rc == 0u) { updated = true; chi2 += d; nh += 1; } else st |= rc;
+        }
+        if (!updated) commit_propagated_disc(t, o, n);
     } else {
         Crossing o;
         PropCov n;
@@ -463,11 +500,14 @@ cudaError_t launch_comb(CombScratch& s, const FitParams& P, const CombCall& call
         a.hist_parent = hist_parent + (int64_t)j * S;
         a.hist_hit = hist_hit + (int64_t)j * S;
         comb_propagate_kernel<<<slot_blocks, 128, 0, stream>>>(P, a, sp.layer);
-        if (multi) comb_scan_kernel<true><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
-        else comb_scan_kernel<false><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
+        const bool disc = P.layer[sp.layer].type == 1;
+        if (multi && disc) comb_scan_kernel<true, true><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
+        else if (multi) comb_scan_kernel<true, false><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
+        else if (disc) comb_scan_kernel<false, true><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
+        else comb_scan_kernel<false, false><<<scan_blocks, kScanBlock, 0, stream>>>(a, P.layer[sp.layer].inv_r);
         comb_select_kernel<<<(unsigned)((call.n_seeds + 3) / 4), 128, 0, stream>>>(a);
-        if (multi) comb_update_kernel<true><<<slot_blocks, 128, 0, stream>>>(a);
-        else comb_update_kernel<false><<<slot_blocks, 128, 0, stream>>>(a);
+        if (multi) comb_update_kernel<true><<<slot_blocks, 128, 0, stream>>>(a, disc ? 1 : 0);
+        else comb_update_kernel<false><<<slot_blocks, 128, 0, stream>>>(a, disc ? 1 : 0);
         cur ^= 1;
         bind(cur);
     }

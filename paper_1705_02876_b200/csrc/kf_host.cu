@@ -210,7 +210,8 @@ cudaError_t build_best_hit_host(BuildHostStage& hs, BinScratch& bs, ScoreScratch
             BinArgs ba;
             ba.n_hits = io.n_hits[j]; ba.ld_in = ldh[j];
             ba.pos = (const float*)(b + o_pos[j]); ba.cov = (const float*)(b + o_hcov[j]);
-            ba.radius = P.layer[io.first_layer + j].r; ba.n_eta = io.n_eta; ba.n_phi = io.n_phi; ba.eta_max = io.eta_max;
+            ba.radius = P.layer[io.first_layer + j].type == 1 ? 0.0f : P.layer[io.first_layer + j].r;   // (reading A24)
+            ba.n_eta = io.n_eta; ba.n_phi = io.n_phi; ba.eta_max = io.eta_max;
             ba.ld_out = ldh[j]; ba.bin_offset = (int32_t*)(b + o_off[j]); ba.sorted_to_orig = (int32_t*)(b + o_s2o[j]);
             ba.pos_sorted = nullptr; ba.cov_sorted = nullptr; ba.hit_rec = (float*)(b + o_rec[j]);
             ba.bin_box = (float*)(b + o_box[j]); ba.orig_to_sorted = nullptr;

@@ -266,3 +266,40 @@ def test_D7_scoring_on_a_disc_layer():
         has = (lay.true_index >= 0) & (r6["status"] == 0) & (r6["nhits"] >= 3)
         n_has += int(has.sum()); n_right += int((wa["best_hit"][has] == lay.true_index[has]).sum())
     assert n_has > 150 and n_right > 0.9 * n_has
+
+
+def test_D8_combinatorial_building_with_discs_reduces_to_best_hit():
+    """orc_build_combinatorial with the surface list (readings A23 / A24): with ONE candidate per seed it is the best-hit
+    layer loop of D7 -- same hits, same final state -- on three barrel and four disc layers; with four candidates every
+    seed's best track has at least as many hits as, and for equal hits no larger chi2 than, the best-hit one."""
+    NEd, NPd, EMd = 50, 64, 2.5
+    ev = W.make_endcap_build_event(400, 2500, event=5)
+    f = ev.fit
+    L, L0 = f.n_layers, 3
+    with O.surfaces(f.surface_type[:3], f.disc_z[:3], f.disc_rmin[:3], f.disc_rmax[:3]), O.geometry_options(0, f.half_length[:3]):
+        r = O.fit_tracks(f.radius[:3], f.x_over_X0[:3], f.Bz, f.mass, f.par, f.cov, f.q, f.hpos[:3], f.hcov[:3], f.mask & 7)
+    par, cov = r["par"].astype(np.float32), O.pack_cov21(r["cov"]).astype(np.float32)
+    layers = [(l.pos, l.cov, O.bin_hits(l.pos, l.radius, NEd, NPd, EMd)) for l in ev.layers[L0:]]
+    with O.surfaces(f.surface_type, f.disc_z, f.disc_rmin, f.disc_rmax), O.geometry_options(0, f.half_length):
+        c1 = O.build_combinatorial(f.radius, f.x_over_X0, f.Bz, f.mass, par, cov, f.q, r["chi2"], r["nhits"], L0, layers, NEd, NPd, EMd, 2, 30.0, 1)
+        c4 = O.build_combinatorial(f.radius, f.x_over_X0, f.Bz, f.mass, par, cov, f.q, r["chi2"], r["nhits"], L0, layers, NEd, NPd, EMd, 2, 30.0, 4)
+    oc = O.Candidates(par, cov, f.q, r["chi2"], r["nhits"])
+    hits = np.full((L - L0, f.n), -1, dtype=np.int32)
+    for j, l in enumerate(range(L0, L)):
+        lay = ev.layers[l]
+        if f.surface_type[l] == 1:
+            with O.score_surface(f.disc_z[l], f.disc_rmin[l], f.disc_rmax[l]):
+                out = O.score_layer(oc, 0.0, f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, layers[j][2], NEd, NPd, EMd, 2, 30.0, True)
+        else:
+            with O.geometry_options(0, f.half_length, score_layer=l):
+                out = O.score_layer(oc, f.radius[l], f.x_over_X0[l], f.Bz, f.mass, lay.pos, lay.cov, layers[j][2], NEd, NPd, EMd, 2, 30.0, True)
+        hits[j] = out["best_hit"]
+    assert np.array_equal(c1["hits"], hits)
+    assert np.array_equal(c1["nhits"], oc.nhits) and np.array_equal(c1["status"], oc.status)
+    np.testing.assert_allclose(c1["par"], oc.par.T, rtol=1e-12, atol=1e-12)
+    np.testing.assert_allclose(c1["chi2"], oc.chi2, rtol=1e-12, atol=1e-12)
+    assert np.max(np.abs(c1["cov"] - oc.cov)) < 1e-12 * np.max(np.abs(oc.cov))
+    assert (hits[3:] >= 0).sum() > 400
+    assert np.all(c4["nhits"] >= c1["nhits"])
+    eq = c4["nhits"] == c1["nhits"]
+    assert np.all(c4["chi2"][eq] <= c1["chi2"][eq] + 1e-9)

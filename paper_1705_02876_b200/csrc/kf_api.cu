@@ -549,7 +549,7 @@ int kf_order_candidates(kf_ctx* c, const kf_geometry* geom, int layer, const kf_
                         int n_phi, float eta_max, int32_t* order) {
     if (!c || !geom || !cands) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if (layer < 0 || layer >= geom->n_layers) return KF_ERR_SHAPE;
     if (cands->n < 0 || cands->ld < cands->n || n_eta < 1 || n_phi < 2) return KF_ERR_SHAPE;

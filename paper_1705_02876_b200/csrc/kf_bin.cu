@@ -639,9 +639,15 @@ cand_key_kernel(const __grid_constant__ FitParams P, int layer, int64_t n, int64
     t.px = __ldg(par + 3 * ld + i); t.py = __ldg(par + 4 * ld + i); t.pz = __ldg(par + 5 * ld + i);
     t.eax = 1.0f; t.eay = 0.0f;
     const float qf = (float)q[i];
-    Crossing o;
     float x = t.x, y = t.y, z = t.z;
-    if (helix_to_radius(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], o)) { x = o.xn; y = o.yn; z = o.zn; }
+    if (P.layer[layer].type == 1) {            // a disc layer (readings A23 / A24)
+        DiscCrossing o;
+        const uint32_t rc = helix_to_plane(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], o);
+        if (rc == 0u || rc == ST_OUTSIDE) { x = o.xn; y = o.yn; z = o.zt; }
+    } else {
+        Crossing o;
+        if (helix_to_radius(t, qf * P.k0, qf * P.inv_k0, P.layer[layer], o)) { x = o.xn; y = o.yn; z = o.zn; }
+    }
     const float rho = sqrtf(x * x + y * y);
     const float eta = asinhf(z / fmaxf(rho, 1e-20f));
     const float phi = atan2f(y, x);

@@ -357,6 +357,30 @@ def test_endcap_combinatorial_building_and_events(ctx):
             assert np.array_equal(r2[k][e * f.n:(e + 1) * f.n], r1[k]), k
 
 
+def test_endcap_order_changes_no_result(ctx):
+    """kf_order_candidates for a disc layer: a permutation (a scheduling hint), and kf_build_best_hit gives the same
+    result with and without it."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
+    ev = W.make_endcap_build_event(2000, 8000, event=4)
+    f = ev.fit
+    par, cov, chi2, nh = _endcap_seeds(f)
+    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, f.half_length, 0, 0, f.surface_type, f.disc_z, f.disc_rmin, f.disc_rmax)
+    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NEd, NPd, EMd, "cuda:0") for l in ev.layers[6:]]
+    ctx.bin_layers([l.radius for l in ev.layers[6:]], [(d.n_hits, d.pos, d.cov, d.bins) for d in dls])
+    a = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    b = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
+    order = b.make_order(ctx, geom, 6, NEd, NPd, EMd)
+    ia, ca = a.build(ctx, geom, 6, dls, 2, 30.0, True, None)
+    ib, cb = b.build(ctx, geom, 6, dls, 2, 30.0, True, order)
+    torch.cuda.synchronize()
+    assert np.array_equal(np.sort(order.cpu().numpy()[:f.n]), np.arange(f.n))
+    assert torch.equal(ia[:, :f.n], ib[:, :f.n]) and (ia[:, :f.n] >= 0).sum() > 1000
+    ra, rb = a.results(), b.results()
+    for k in ra:
+        assert np.array_equal(ra[k], rb[k], equal_nan=True), k
+
+
 def test_endcap_indexed_fit_equals_pre_gathered(ctx):
     """kf_fit_tracks_indexed knows discs too: the same hits addressed by index give the same fit."""
     from paper_1705_02876_b200.buffers import DeviceFit, padded_ld
@@ -391,19 +415,6 @@ def test_discs_are_refused_where_they_are_not_implemented(ctx):
     b = W.simulate_endcap_event(0, 64)
     d = DeviceFit.from_batch(b, "cuda:0")
     for call in (lambda: d.fit_refit(ctx),):
-        with pytest.raises(K.KFError) as e:
-            call()
-        assert e.value.code == -4
-    # kf_order_candidates does not know discs
-    from paper_1705_02876_b200.buffers import DeviceCandidates, DeviceLayer
-    ev = W.make_endcap_build_event(64, 200)
-    f = ev.fit
-    par, cov, chi2, nh = _endcap_seeds(f)
-    geom = K.Geometry(f.radius, f.x_over_X0, f.Bz, f.mass, f.half_length, 0, 0, f.surface_type, f.disc_z, f.disc_rmin, f.disc_rmax)
-    dc = DeviceCandidates.from_numpy(par, cov, f.q, chi2, nh, "cuda:0")
-    dls = [DeviceLayer.from_numpy(l.pos, l.cov, NEd, NPd, EMd, "cuda:0") for l in ev.layers[3:]]
-    ctx.bin_layers([l.radius for l in ev.layers[3:]], [(x.n_hits, x.pos, x.cov, x.bins) for x in dls])
-    for call in (lambda: dc.make_order(ctx, geom, 3, NEd, NPd, EMd),):
         with pytest.raises(K.KFError) as e:
             call()
         assert e.value.code == -4

@@ -722,6 +722,31 @@ def run_ours(args) -> None:
         geometry = {"api": "kf_fit_tracks with material_model 1 and 30 cm barrel half lengths (reading A20)", "ms": go_ms,
                     "fits_per_s": n / (go_ms * 1e-3), "tracks_cut_short": go_out,
                     "with_energy_loss_ms": el_ms, "with_energy_loss_fits_per_s": n / (el_ms * 1e-3)}
+        # ... and the barrel + endcap toy (readings A23 / A24: six barrels of half length 30 cm + four disc pairs,
+        # |eta| <= 2.5): fit and fit + RTS smoother of 2 M tracks (one 20 000-track event, 100 times)
+        from workloads import barrel_events as Wb
+        eb = Wb.concat_batches([Wb.simulate_endcap_event(0, 20000)] * (n // 20000 if n >= 20000 else 1))
+        de = DeviceFit.from_batch(eb, dev)
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                de.fit(ctx)
+            s0.record(stream)
+            for _ in range(20):
+                de.fit(ctx)
+            s1.record(stream)
+            de.fit_smooth(ctx)
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record(stream)
+            for _ in range(5):
+                de.fit_smooth(ctx)
+            t1.record(stream)
+        torch.cuda.synchronize()
+        geometry["endcap_discs"] = {"api": "kf_fit_tracks / kf_fit_tracks_smooth on the barrel + endcap toy (6 barrels + 4 disc pairs)",
+                                    "tracks": int(eb.n), "fit_ms": s0.elapsed_time(s1) / 20,
+                                    "fits_per_s": eb.n / (s0.elapsed_time(s1) / 20 * 1e-3),
+                                    "fit_smooth_ms": t0.elapsed_time(t1) / 5,
+                                    "hits_per_track": float(np.mean([bin(int(m)).count("1") for m in eb.mask[:20000]]))}
+        del de, eb
         # secondary: kf_fit_tracks_indexed -- same tracks, each layer's hits shuffled into a pool and addressed by index
         g = torch.Generator(device=dev); g.manual_seed(5)
         perm = [torch.randperm(n, device=dev, generator=g) for _ in range(L)]

@@ -179,15 +179,17 @@ int orc_propagate_inward(const double u[6], double q, double Bz, double r, doubl
  *   ds/du = -A[z, u] / (pz / pT)      (so row z of F vanishes: the arrival point stays in the plane and the
  *   transported covariance has no variance along z -- the disc's counterpart of the radial null of a cylinder).
  * Fails (ORC_PROP_FAIL, nothing written) unless the plane lies ahead (s > 0) within half a turn (|theta| < pi). */
-int orc_propagate_to_z(const double u[6], double q, double Bz, double zt, double out[6], double F[36],
-                       double *s_out, double *theta_out) {
+static int propagate_to_z_dir(const double u[6], double q, double Bz, double zt, int inward, double out[6],
+                              double F[36], double *s_out, double *theta_out) {
     double x = u[0], y = u[1], z = u[2], px = u[3], py = u[4], pz = u[5];
     double k = q * ORC_C_B * Bz;
     double pt2 = px * px + py * py;
     double pt = sqrt(pt2);
     if (!(pt > 0.0) || pz == 0.0) return ORC_PROP_FAIL;
     double s = (zt - z) * pt / pz;
-    if (!(s > 0.0)) return ORC_PROP_FAIL;
+    /* inward (the refit of reading A18 on a geometry with discs): the plane lies BEHIND the state, reached by
+     * following the same helix backward in path length (s < 0, theta of the opposite sign) */
+    if (inward ? !(s < 0.0) : !(s > 0.0)) return ORC_PROP_FAIL;
     double theta = k * s / pt;
     if (!(fabs(theta) < ORC_PI)) return ORC_PROP_FAIL;
     double S = sin(theta), co = cos(theta);
@@ -224,6 +226,10 @@ int orc_propagate_to_z(const double u[6], double q, double Bz, double zt, double
     if (s_out) *s_out = s;
     if (theta_out) *theta_out = theta;
     return 0;
+}
+int orc_propagate_to_z(const double u[6], double q, double Bz, double zt, double out[6], double F[36],
+                       double *s_out, double *theta_out) {
+    return propagate_to_z_dir(u, q, Bz, zt, 0, out, F, s_out, theta_out);
 }
 
 /* One layer of the geometry as the filter meets it: barrel (type 0) or disc pair (type 1, the disc on the side the
@@ -742,11 +748,22 @@ static void refit_inward_one(int L, const double *radius, const double *xX0, dou
             memcpy(ub, u, sizeof ub);
             memcpy(Cq, C, sizeof Cq);
             /* A21: the layer just left gives back the energy it took (before its scattering noise is added) */
-            if (g_energy_loss && orc_energy_loss_step(ub, Cq, mass, xX0[prev], -1, NULL)) { st |= ORC_PROP_FAIL; continue; }
-            orc_process_noise(ub, mass, xX0[prev], Q);
+            g_at_surface = g_surface_type[prev]; /* the state stands on layer prev (a cylinder or a disc, A23) */
+            int el_rc = g_energy_loss ? orc_energy_loss_step(ub, Cq, mass, xX0[prev], -1, NULL) : 0;
+            if (!el_rc) orc_process_noise(ub, mass, xX0[prev], Q);
+            g_at_surface = 0;
+            if (el_rc) { st |= ORC_PROP_FAIL; continue; }
             for (int i = 0; i < 36; ++i) Cq[i] += Q[i];
-            rc = propagate_dir(ub, (double)q, Bz, radius[l], 1, up, F, NULL, NULL);
-            if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
+            if (g_surface_type[l] == 1) { /* back to the disc on the track's side */
+                rc = propagate_to_z_dir(ub, (double)q, Bz, ub[5] < 0.0 ? -g_disc_z[l] : g_disc_z[l], 1, up, F, NULL, NULL);
+                if (!rc) {
+                    double rho = sqrt(up[0] * up[0] + up[1] * up[1]);
+                    if (rho < g_disc_rmin[l] || rho > g_disc_rmax[l]) rc = ORC_OUTSIDE;
+                }
+            } else {
+                rc = propagate_dir(ub, (double)q, Bz, radius[l], 1, up, F, NULL, NULL);
+                if (!rc && fabs(up[2]) > g_half_length[l]) rc = ORC_OUTSIDE;
+            }
             if (rc) { st |= (uint32_t)rc; continue; }
             memset(Z, 0, sizeof Z);
             orc_transport_cov(F, Cq, Z, Cp);

@@ -303,3 +303,37 @@ def test_D8_combinatorial_building_with_discs_reduces_to_best_hit():
     assert np.all(c4["nhits"] >= c1["nhits"])
     eq = c4["nhits"] == c1["nhits"]
     assert np.all(c4["chi2"][eq] <= c1["chi2"][eq] + 1e-9)
+
+
+def test_D9_inward_refit_with_discs():
+    """The inward refit (reading A18) over barrels and discs: the backward EKF equals the batch WLS of the model it
+    linearises (inflated forward covariance as prior, hits outermost first, one scatterer per step) -- the pin S3 of
+    tests/test_oracle_refit.py with disc layers on the way; its result stands on the innermost used layer."""
+    from tests.test_oracle_refit import _batch_wls_backward
+    b = W.simulate_endcap_event(11, 40)
+    L = b.n_layers
+    with O.surfaces(b.surface_type, b.disc_z, b.disc_rmin, b.disc_rmax), O.geometry_options(0, b.half_length):
+        r = O.fit_refit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par, b.cov, b.q, b.hpos, b.hcov, b.mask, want_trace=True)
+    Vs = O.unpack_cov6(b.hcov)
+    n_disc = n_chk = 0
+    for i in range(b.n):
+        if r["status"][i] != 0 or r["rstatus"][i] != 0:
+            continue
+        used = [l for l in range(L) if r["trace_fwd"][i][l][121] != 0]
+        back = [l for l in range(L - 1, -1, -1) if r["trace_bwd"][i][l][121] != 0]
+        assert back == used[::-1] and r["rnhits"][i] == len(used)
+        hits = b.hpos[:, :, i].astype(np.float64)
+        x0, C0 = r["par"][:, i], O.REFIT_KAPPA * r["cov"][i]
+        x, Cx, cost = _batch_wls_backward(x0, C0, r["trace_bwd"][i], hits, Vs[i], back)
+        np.testing.assert_allclose(r["rpar"][:, i], x, rtol=1e-9, atol=1e-9)
+        assert np.max(np.abs(r["rcov"][i] - Cx)) < 1e-8 * np.max(np.abs(Cx))
+        assert r["rchi2"][i] == pytest.approx(cost, rel=1e-8, abs=1e-9)
+        # the refitted state stands on the innermost used layer
+        l0 = used[0]
+        if b.surface_type[l0] == 1:
+            assert abs(abs(r["rpar"][2, i]) - b.disc_z[l0]) < 1e-9
+        else:
+            assert abs(np.hypot(r["rpar"][0, i], r["rpar"][1, i]) - b.radius[l0]) < 1e-2      # (moved by the update, in the tangent plane)
+        n_disc += sum(1 for l in used if b.surface_type[l] == 1)
+        n_chk += 1
+    assert n_chk >= 30 and n_disc >= 40

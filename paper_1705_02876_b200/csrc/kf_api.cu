@@ -408,7 +408,7 @@ int kf_fit_tracks_refit(kf_ctx* c, const kf_geometry* geom, const kf_tracks* see
                          float kappa, kf_tracks* out, kf_tracks* smoothed) {
     if (!c || !geom || !seeds || !hits || !out || !smoothed) return KF_ERR_NULL;
     FitParams P;
-    int rc = make_params(geom, &P);
+    int rc = make_params(geom, &P, true);
     if (rc) return rc;
     if (!(kappa >= 1.0f)) return KF_ERR_UNSUPPORTED;
     if ((rc = check_tracks(seeds, true, true))) return rc;

@@ -96,6 +96,87 @@ __device__ __forceinline__ uint32_t fit_layer_disc(Track& t, float k, float ik, 
     return rc;
 }
 
+// ---- the inward refit (reading A18) between surfaces of either kind (geometries with discs, one track per thread)
+// One backward step: the layer just left (Lprev, a cylinder or a disc) gives back its energy (A21) and adds its
+// scattering noise, then the state goes inward to L and takes L's hit.  first: the state already stands on L
+// (update only).  Worked on a copy: any failure leaves the track as it was.
+__device__ __forceinline__ uint32_t refit_step_surface(Track& t, float k, float ik, const LayerConst& L, const LayerConst& Lprev,
+                                                       int model, float mass2, const Bethe& el, bool first, const Hit& m,
+                                                       float* dchi2) {
+    Track tb = t;
+    if (!first) {
+        const float pt2 = tb.px * tb.px + tb.py * tb.py;
+        const float ipt = rsqrt_fast(pt2);
+        // |cos| that scales the thickness seen (path-length option): to the radial direction on a cylinder, to z on a disc
+        const float cos_a = Lprev.type == 1 ? tb.pz * ipt : (tb.eax * tb.px + tb.eay * tb.py) * ipt;
+        if (model & MODEL_ENERGY_LOSS) {
+            Eloss e;
+            if (!energy_loss_factors(el, Lprev, model, mass2, cos_a, pt2, ipt, tb.pz, true, e)) return ST_PROP_FAIL;
+            apply_energy_loss(e, tb);
+        }
+        {   // Highland noise of Lprev at the current momentum (add_process_noise with the surface's own path factor)
+            const float q2 = tb.px * tb.px + tb.py * tb.py, pz = tb.pz;
+            const float iq = rsqrt_fast(q2);
+            const float p2 = q2 + pz * pz;
+            float ms = Lprev.ms;
+            if (model & MODEL_PATH_LENGTH) {
+                if (Lprev.type == 1) {
+                    const float f = sqrtf(p2) * rcp_fast(fabsf(pz));
+                    const float lg = 1.0f + 0.038f * (Lprev.ln_t + __logf(f));
+                    ms = Lprev.ms0 * f * lg * lg;
+                } else {
+                    ms = layer_ms<float>(Lprev, model, (tb.eax * tb.px + tb.eay * tb.py) * iq, p2, iq);
+                }
+            }
+            const float ip2 = rcp_fast(p2);
+            const float th2 = ms * (p2 + mass2) * ip2 * ip2;
+            const float qc = th2 * p2 * iq;
+            tb.c33 += th2 * pz * pz;
+            tb.c35 -= qc * pz;
+            tb.c44 += th2 * p2;
+            tb.c55 += qc * (p2 * iq);
+        }
+    }
+    uint32_t rc;
+    if (L.type == 1) {
+        DiscCrossing o;
+        DiscCov n;
+        if (first) {
+            const float pt2 = tb.px * tb.px + tb.py * tb.py;
+            const float ipt = rsqrt_fast(pt2);
+            o.xn = tb.x; o.yn = tb.y; o.zt = tb.z; o.pxn = tb.px; o.pyn = tb.py;
+            o.erx = tb.eax; o.ery = tb.eay; o.elx = tb.px * ipt; o.ely = tb.py * ipt;
+            o.T = tb.pz * ipt; o.pt2 = pt2; o.ipt = ipt;
+            n.rr = tb.c00; n.rt = tb.c01; n.tt = tb.c11;
+            n.r3 = tb.c03; n.r4 = tb.c04; n.r5 = tb.c05; n.t3 = tb.c13; n.t4 = tb.c14; n.t5 = tb.c15;
+            n.n33 = tb.c33; n.n34 = tb.c34; n.n35 = tb.c35; n.n44 = tb.c44; n.n45 = tb.c45; n.n55 = tb.c55;
+        } else {
+            const uint32_t reached = helix_to_plane<true>(tb, k, ik, L, o);
+            if (reached) return reached;
+            transport_cov_disc(tb, o, k, 0.0f, mass2, n);
+        }
+        Crossing c;
+        c.xn = o.xn; c.yn = o.yn; c.zn = o.zt; c.erx = o.erx; c.ery = o.ery;
+        LocalHit h;
+        hit_to_local(c, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
+        rc = kalman_update_disc(tb, o, n, h, dchi2);
+    } else {
+        Crossing o;
+        PropCov n;
+        if (first) crossing_in_place(tb, o, n);
+        else {
+            const uint32_t reached = reach_layer<true, true>(tb, k, ik, L, o);
+            if (reached) return reached;
+            transport_cov<false>(tb, o, 0.0f, mass2, n);       // (the state may come from a disc: general covariance)
+        }
+        LocalHit h;
+        hit_to_local(o, m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, h);
+        rc = kalman_update(tb, o, n, h, dchi2);
+    }
+    if (rc == 0u) t = tb;
+    return rc;
+}
+
 // GEOM 0: the paper's toy detector (options compiled out); 1: the options of readings A20 / A21 on barrels;
 // 2: the same plus endcap discs (reading A23).
 template <bool RADIAL_NULL, int GEOM = 1>
@@ -291,7 +372,12 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
         int nb = 0;
         uint32_t sst = 0u;
         bool first = true;
-        if (used) scale_cov(t, a.kappa);
+        if (used) {
+            scale_cov(t, a.kappa);
+            if constexpr (GEOM == 2) {      // a result standing on a disc has its radial row live (and no z row)
+                t.c00 *= a.kappa; t.c01 *= a.kappa; t.c02 *= a.kappa; t.c03 *= a.kappa; t.c04 *= a.kappa; t.c05 *= a.kappa;
+            }
+        }
         for (int j = 0; j < L; ++j) {
             const int l = L - 1 - j, step = L + j, s = step % kStages;
             mbar_wait(bar0 + 8u * s, (phase >> s) & 1u);
@@ -304,7 +390,9 @@ fit_kernel(const __grid_constant__ FitParams P, const __grid_constant__ FitMaps 
             __syncwarp();
             if ((used >> l) & 1u) {
                 float d;
-                const uint32_t rc = refit_step<GEOM != 0>(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, P.el, first,
+                uint32_t rc;
+                if constexpr (GEOM == 2) rc = refit_step_surface(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, P.el, first, m, &d);
+                else rc = refit_step<GEOM != 0>(t, k, ik, P.layer[l], P.layer[l_prev], model, P.mass2, P.el, first,
                                                      m.x, m.y, m.z, m.vxx, m.vxy, m.vxz, m.vyy, m.vyz, m.vzz, &d);
                 if (rc == 0u) { schi2 += d; nb += 1; first = false; l_prev = l; }
                 else sst |= rc;
@@ -928,6 +1016,7 @@ cudaError_t ensure_fit_attributes() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(fit_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
@@ -986,8 +1075,8 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
         return cudaErrorInvalidValue;
     const int64_t blocks = (a.n + kFitBlock - 1) / kFitBlock;
     const bool geom = P.geometry_options != 0;   // reading A20 options in use
-    if (P.has_discs && smooth) return cudaErrorInvalidValue;   // (refused at the ABI: the refit of reading A18 does not know discs)
-    if (smooth && geom) fit_kernel<1, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    if (smooth && P.has_discs) fit_kernel<1, 2><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    else if (smooth && geom) fit_kernel<1, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (smooth) fit_kernel<1, 0><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (store && P.has_discs) fit_kernel<2, 2><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (store && geom) fit_kernel<2, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);

@@ -739,6 +739,9 @@ struct DiscCov {
 };
 
 // Returns 0, ST_PROP_FAIL (plane behind the state, |pz| = 0, half a turn or more away) or ST_OUTSIDE.
+// INWARD (the refit of reading A18): the plane lies behind the state and is reached by following the helix backward
+// in path length (theta of the opposite sign; the Jacobian holds for either sign).
+template <bool INWARD = false>
 __device__ __forceinline__ uint32_t helix_to_plane(const Track& t, float k, float ik, const LayerConst& L, DiscCrossing& o) {
     const float px = t.px, py = t.py, pz = t.pz;
     const float zt = copysignf(L.zd, pz);
@@ -746,7 +749,7 @@ __device__ __forceinline__ uint32_t helix_to_plane(const Track& t, float k, floa
     const float pt2 = px * px + py * py;
     const float theta = k * dz / pz;
     // (NaNs fail every comparison)
-    if (!(dz * pz > 0.0f) || !(fabsf(theta) < 3.14159265f) || !(pt2 > 0.0f)) return ST_PROP_FAIL;
+    if (!(INWARD ? dz * pz < 0.0f : dz * pz > 0.0f) || !(fabsf(theta) < 3.14159265f) || !(pt2 > 0.0f)) return ST_PROP_FAIL;
     float sh, ch;
     sincosf(0.5f * theta, &sh, &ch);
     const float S = 2.0f * sh * ch, Cm = 2.0f * sh * sh, co = 1.0f - Cm;

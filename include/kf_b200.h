@@ -175,9 +175,9 @@ typedef struct {
      * The state is propagated to the plane (theta = k (zt - z) / pz); the transported covariance then has no
      * variance along z instead of along the radius; a crossing outside the annulus sets KF_STATUS_OUTSIDE and the
      * layer is skipped; a plane that lies behind the state or half a turn or more away is KF_STATUS_PROP_FAIL.
-     * radius_cm[l] of a disc layer is not used but must keep the list increasing.  Discs are known to
-     * every call (the pool of a disc layer is binned with radius 0: kf_bin_hits).  material_model and energy_loss_model apply at a disc with the path factor
-     * 1 / |cos| of the angle to the z axis = |p| / |pz|. */
+     * radius_cm[l] of a disc layer is not used but must keep the list increasing.  Discs are known to every call
+     * (the pool of a disc layer is binned with radius 0: kf_bin_hits).  material_model and energy_loss_model apply
+     * at a disc with the path factor 1 / |cos| of the angle to the z axis = |p| / |pz|. */
     const int32_t* surface_type;  /* HOST [n_layers] 0 = barrel, 1 = disc pair; or NULL                        */
     const float* disc_z_cm;       /* HOST [n_layers] |z| of the disc pair (> 0), read where surface_type = 1   */
     const float* disc_rmin_cm;    /* HOST [n_layers] inner radius of the annulus (>= 0)                         */

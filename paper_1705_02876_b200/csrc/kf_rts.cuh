@@ -324,9 +324,9 @@ __device__ __forceinline__ uint32_t rts_step_surface(const Track& t, const Sym5&
         const float R[6] = {o.pc, -o.ps, -o.ca * o.iT, o.nr - o.ca * o.thk, -o.nt, -o.ca * o.thk * o.iT};
         const float Tt[6] = {o.ps, o.pc, -o.sa * o.iT, o.nt - o.sa * o.thk, o.nr, -o.sa * o.thk * o.iT};
         const float b2z = k * o.iT, b2b = o.theta, b2c = o.theta * o.iT;
-        const int c0 = src == 0 ? 1 : 0, c1 = src == 0 ? 2 : 1;          // k's two live position coordinates
-        Fs[0][0] = R[c0]; Fs[0][1] = R[c1]; Fs[0][2] = R[3]; Fs[0][3] = R[4]; Fs[0][4] = R[5];
-        Fs[1][0] = Tt[c0]; Fs[1][1] = Tt[c1]; Fs[1][2] = Tt[3]; Fs[1][3] = Tt[4]; Fs[1][4] = Tt[5];
+        const bool sb = src == 0;                                         // k's two live position coordinates: (a2, z) or (a1, a2)
+        Fs[0][0] = sb ? R[1] : R[0]; Fs[0][1] = sb ? R[2] : R[1]; Fs[0][2] = R[3]; Fs[0][3] = R[4]; Fs[0][4] = R[5];
+        Fs[1][0] = sb ? Tt[1] : Tt[0]; Fs[1][1] = sb ? Tt[2] : Tt[1]; Fs[1][2] = Tt[3]; Fs[1][3] = Tt[4]; Fs[1][4] = Tt[5];
         Fs[3][1] = src == 0 ? b2z : 0.0f; Fs[3][2] = b2b; Fs[3][3] = 1.0f; Fs[3][4] = b2c;
         xn = o.xn; yn = o.yn; wn = o.zt; pxn = o.pxn; pyn = o.pyn; erx = o.erx; ery = o.ery; elx = o.elx; ely = o.ely;
         T = o.T; pt2 = o.pt2; ipt = o.ipt;

@@ -650,6 +650,27 @@ def run_ours(args) -> None:
     d2h = n * (27 * 4 + 12)
     e2e = {"value": n_all * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
            "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "kf_fit_tracks_host, pinned host SoA buffers"}
+    # The seeds of configs[0-3] carry a DIAGONAL covariance (reading A13: what a seeding step hands over), and the
+    # path is bound by the host-to-device link: kf_fit_tracks_host_diag sends the six variances instead of the 21
+    # packed elements (24 instead of 84 of a track's 473 input bytes), same results bit for bit.  That call is the
+    # end-to-end number of this workload; the full-covariance call is kept beside it.
+    off_diag = [r for r in range(21) if r not in (0, 6, 11, 15, 18, 20)]
+    if bool(torch.all(h.cov[off_diag] == 0)):
+        full_res = h.results()
+        h.fit_host(ctx, cov_diagonal=True)
+        sharding.barrier(dev)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            h.fit_host(ctx, cov_diagonal=True)
+        torch.cuda.synchronize()
+        diag_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+        diag_res = h.results()
+        same = all(np.array_equal(full_res[k], diag_res[k], equal_nan=True) for k in full_res)
+        e2e = {"value": n_all * e2e_steps / diag_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d - n * 15 * 4),
+               "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "ms_per_step": 1e3 * diag_s / e2e_steps,
+               "api": "kf_fit_tracks_host_diag, pinned host SoA buffers (diagonal seed covariance: 6 planes instead of 21)",
+               "same_results_as_full_covariance_call": bool(same), "full_covariance_call": e2e}
     # the host path fits chunks with the one-track kernel, the resident path uses the pair kernel: same arithmetic,
     # different instruction selection, so the two agree to rounding, not bit for bit
     host_vs_dev, h_res = {}, h.results()

@@ -266,6 +266,15 @@ KF_API int kf_fit_tracks_smooth(kf_ctx* ctx, const kf_geometry* geom, const kf_t
 KF_API int kf_fit_tracks_host(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                        const kf_track_hits* hits, kf_tracks* out);
 
+/* kf_fit_tracks_host for seeds whose covariance is DIAGONAL (what a seeding step hands over: reading A13; the seeds
+ * of configs[0-3]): seeds->cov is HOST [6][ld], the variances xx yy zz pxpx pypy pzpz, and only those six planes
+ * cross the link (24 instead of 84 bytes per track; the end-to-end path is bound by the host-to-device link, and 84
+ * of a track's 473 input bytes at ten layers were that covariance).  The other 15 elements are zero on the device.
+ * Results are those of kf_fit_tracks_host given the same covariance in full, bit for bit.  `out->cov` is the full
+ * [21][ld] as always (and must not alias seeds->cov). */
+KF_API int kf_fit_tracks_host_diag(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                                   const kf_track_hits* hits, kf_tracks* out);
+
 /* ---- hits of one layer and their (eta, phi) bins ------------------------------------ */
 typedef struct {
     int64_t n_hits, ld;       /* ld >= n_hits, ld % 4 == 0                                         */

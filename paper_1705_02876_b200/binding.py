@@ -25,7 +25,7 @@ BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
 STATIC_MAX_CANDIDATES = 65536                                               # KF_STATIC_MAX_CANDIDATES
 ERR_TOO_LARGE = -8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_hit_record_floats", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_abi_version", "kf_hit_record_floats", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_fit_tracks_host_diag", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_score_candidates_static", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial", "kf_build_combinatorial_events",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
@@ -115,7 +115,7 @@ def load_library():
     lib.kf_abi_version.argtypes = []
     lib.kf_hit_record_floats.restype = C.c_int
     lib.kf_hit_record_floats.argtypes = []
-    for name in ("kf_fit_tracks", "kf_fit_tracks_host"):
+    for name in ("kf_fit_tracks", "kf_fit_tracks_host", "kf_fit_tracks_host_diag"):
         f = getattr(lib, name)
         f.restype = C.c_int
         f.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.POINTER(_Tracks)]
@@ -443,17 +443,23 @@ class KFContext:
         del keep
 
     def fit_tracks_host(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,
-                        out_par, out_cov, out_chi2, out_nhits, out_status):
-        """Same with HOST tensors (pinned for full overlap); returns when the outputs are complete."""
+                        out_par, out_cov, out_chi2, out_nhits, out_status, cov_diagonal: bool = False):
+        """Same with HOST tensors (pinned for full overlap); returns when the outputs are complete.
+        cov_diagonal: `cov` is [6][ld], the diagonal of the seed covariance (kf_fit_tracks_host_diag)."""
         for t in (par, cov, q, hpos, hcov, out_par, out_cov, out_chi2, out_nhits, out_status):
             if t.is_cuda:
                 raise ValueError("fit_tracks_host takes CPU tensors")
         g, keep = geom._c()
-        seeds = self._tracks(n, par, cov, q, out_chi2, out_nhits, out_status)
+        ld = _plane_ld(par, 6)
+        if _plane_ld(cov, 6 if cov_diagonal else 21) != ld:
+            raise ValueError("par and cov must share the plane stride ld")
+        seeds = _Tracks(int(n), ld, par.data_ptr(), cov.data_ptr(), q.data_ptr(), out_chi2.data_ptr(), out_nhits.data_ptr(),
+                        out_status.data_ptr())
         out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
         hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
-        self._check(self._lib.kf_fit_tracks_host(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)),
-                    "kf_fit_tracks_host")
+        fn = self._lib.kf_fit_tracks_host_diag if cov_diagonal else self._lib.kf_fit_tracks_host
+        self._check(fn(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)),
+                    "kf_fit_tracks_host_diag" if cov_diagonal else "kf_fit_tracks_host")
         del keep
 
     # ------------------------------------------------------------------ kf_bin_hits / kf_bin_layers

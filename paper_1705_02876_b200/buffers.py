@@ -118,9 +118,18 @@ class DeviceFit:
                     chi2=sm["chi2"][:n].cpu().numpy(), nhits=sm["nhits"][:n].cpu().numpy(),
                     status=sm["status"][:n].cpu().numpy().view(np.uint32))
 
-    def fit_host(self, ctx: KFContext):
-        ctx.fit_tracks_host(self.geom, self.n, self.par, self.cov, self.q, self.hpos, self.hcov, self.mask,
-                            self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status)
+    def fit_host(self, ctx: KFContext, cov_diagonal: bool = False):
+        """kf_fit_tracks_host; cov_diagonal: kf_fit_tracks_host_diag with the six diagonal planes of self.cov (kept as
+        self.cov_diag, pinned like the rest; the caller asserts that the seed covariance IS diagonal)."""
+        cov = self.cov
+        if cov_diagonal:
+            cov = getattr(self, "cov_diag", None)
+            if cov is None:
+                cov = torch.empty((6, self.ld), dtype=torch.float32, pin_memory=self.cov.is_pinned())
+                cov.copy_(self.cov[[0, 6, 11, 15, 18, 20]])
+                self.cov_diag = cov
+        ctx.fit_tracks_host(self.geom, self.n, self.par, cov, self.q, self.hpos, self.hcov, self.mask,
+                            self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status, cov_diagonal)
 
     def results(self) -> dict:
         n = self.n

@@ -464,8 +464,22 @@ int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* se
     return KF_OK;
 }
 
+namespace {
+int fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits, kf_tracks* out,
+                    bool cov_diagonal);
+}
 int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
                        const kf_track_hits* hits, kf_tracks* out) {
+    return fit_tracks_host(c, geom, seeds, hits, out, false);
+}
+int kf_fit_tracks_host_diag(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
+                            const kf_track_hits* hits, kf_tracks* out) {
+    return fit_tracks_host(c, geom, seeds, hits, out, true);
+}
+}  // extern "C"
+namespace {
+int fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits, kf_tracks* out,
+                    bool cov_diagonal) {
     if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;
     FitParams P;
     int rc = make_params(geom, &P, true);
@@ -483,10 +497,13 @@ int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seed
     io.hpos = hits->pos; io.hcov = hits->cov; io.ld_hit = hits->ld; io.mask = hits->mask;
     io.opar = out->par; io.ocov = out->cov; io.ld_out = out->ld;
     io.chi2 = out->chi2; io.nhits = out->nhits; io.status = out->status;
+    io.cov_diagonal = cov_diagonal;
     e = c->host.fit(P, io, c->opt);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;
 }
+}  // namespace
+extern "C" {
 
 namespace {
 

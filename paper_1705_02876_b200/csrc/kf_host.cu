@@ -16,13 +16,16 @@ namespace kf {
 
 namespace {
 
-constexpr int64_t kDefaultChunk = 1 << 17;  // 131072 tracks per chunk
+#ifndef KF_HOST_CHUNK
+#define KF_HOST_CHUNK (1 << 17)
+#endif
+constexpr int64_t kDefaultChunk = KF_HOST_CHUNK;  // 131072 tracks per chunk
 
 inline size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
 
 // Offsets of the SoA arrays of one chunk inside a slot buffer.
 struct SlotLayout {
-    size_t par, cov, q, mask, hpos, hcov, opar, ocov, chi2, nhits, status, total;
+    size_t par, cov, q, mask, hpos, hcov, opar, ocov, chi2, nhits, status, diag, total;
     SlotLayout(int64_t chunk, int L) {
         size_t o = 0;
         auto take = [&](size_t bytes) { size_t at = o; o += align256(bytes); return at; };
@@ -31,6 +34,7 @@ struct SlotLayout {
         hpos = take((size_t)L * 3 * chunk * 4); hcov = take((size_t)L * 6 * chunk * 4);
         opar = take(6 * chunk * 4);  ocov = take(21 * chunk * 4);
         chi2 = take(chunk * 4);      nhits = take(chunk * 4);  status = take(chunk * 4);
+        diag = take(6 * chunk * 4);  // kf_fit_tracks_host_diag: the six variance planes as they arrive
         total = o;
     }
 };
@@ -87,6 +91,17 @@ cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const Launch
         const size_t w = (size_t)m * 4;
 #define KF_TRY(x) do { e = (x); if (e != cudaSuccess) goto fail; } while (0)
         KF_TRY(cudaMemcpy2DAsync(b + lay.par, cw, io.par + t0, (size_t)io.ld_in * 4, w, 6, cudaMemcpyHostToDevice, st));
+        if (io.cov_diagonal) {
+            // 6 of the 21 planes travel: the others are zeroed on the device (rows xx yy zz pxpx pypy pzpz of the
+            // packed upper triangle: 0, 6, 11, 15, 18, 20)
+            // (one copy over the link, then six device-to-device row copies: six separate host-to-device copies of
+            // 0.5 MB each cost the link more than the bytes they saved)
+            static const int kDiagRow[6] = {0, 6, 11, 15, 18, 20};
+            KF_TRY(cudaMemcpy2DAsync(b + lay.diag, cw, io.cov + t0, (size_t)io.ld_in * 4, w, 6, cudaMemcpyHostToDevice, st));
+            KF_TRY(cudaMemsetAsync(b + lay.cov, 0, (size_t)21 * cw, st));
+            for (int r = 0; r < 6; ++r)
+                KF_TRY(cudaMemcpyAsync(b + lay.cov + (size_t)kDiagRow[r] * cw, b + lay.diag + (size_t)r * cw, w, cudaMemcpyDeviceToDevice, st));
+        } else
         KF_TRY(cudaMemcpy2DAsync(b + lay.cov, cw, io.cov + t0, (size_t)io.ld_in * 4, w, 21, cudaMemcpyHostToDevice, st));
         KF_TRY(cudaMemcpyAsync(b + lay.q, io.q + t0, (size_t)m, cudaMemcpyHostToDevice, st));
         if (io.mask) KF_TRY(cudaMemcpyAsync(b + lay.mask, io.mask + t0, w, cudaMemcpyHostToDevice, st));

@@ -71,6 +71,7 @@ struct HostFitIO {
     const float* par; const float* cov; int64_t ld_in; const int8_t* q;
     const float* hpos; const float* hcov; int64_t ld_hit; const uint32_t* mask;
     float* opar; float* ocov; int64_t ld_out; float* chi2; int32_t* nhits; uint32_t* status;
+    bool cov_diagonal = false;   // kf_fit_tracks_host_diag: cov is [6][ld_in], the diagonal of the seed covariance
 };
 
 // Device staging for kf_fit_tracks_host: kSlots chunk buffers, each with its own stream, so the

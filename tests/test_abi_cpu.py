@@ -59,6 +59,7 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_destroy(None) == -1
     assert lib.kf_fit_tracks(None, None, None, None, None) == -1
     assert lib.kf_fit_tracks_host(None, None, None, None, None) == -1
+    assert lib.kf_fit_tracks_host_diag(None, None, None, None, None) == -1
     assert lib.kf_fit_tracks_indexed(None, None, None, None, 0, None, None, None) == -1
     assert lib.kf_fit_tracks_refit(None, None, None, None, 10.0, None, None) == -1
     assert lib.kf_fit_tracks_smooth(None, None, None, None, None, None) == -1

@@ -256,6 +256,24 @@ def test_fit_host_path_equals_device_path_across_chunks(ctx):
         assert np.array_equal(ref[k], r[k], equal_nan=True), k
 
 
+def test_fit_host_path_with_diagonal_seed_covariance(ctx):
+    """kf_fit_tracks_host_diag: six covariance planes cross the link instead of 21; the seeds of configs[0-3] are
+    diagonal (reading A13), and the results are those of the full call, bit for bit, across chunk boundaries."""
+    from paper_1705_02876_b200.buffers import DeviceFit
+    b = W.make_fit_batch(2, n_events=8)
+    off = np.setdiff1d(np.arange(21), [0, 6, 11, 15, 18, 20])
+    assert np.all(b.cov[off] == 0.0)
+    h = DeviceFit.from_batch(b, "cpu", pin=True)
+    h.fit_host(ctx)
+    full = h.results()
+    h.out_par.zero_(); h.out_cov.zero_(); h.out_chi2.zero_()
+    h.fit_host(ctx, cov_diagonal=True)
+    diag = h.results()
+    for k in full:
+        assert np.array_equal(full[k], diag[k], equal_nan=True), k
+    assert np.count_nonzero(diag["chi2"]) > 0.99 * b.n
+
+
 def test_fit_argument_errors(ctx):
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceFit

@@ -136,6 +136,7 @@ bin_scatter_kernel(const __grid_constant__ BinBatch B) {
     const int64_t h = (int64_t)blockIdx.x * kBlock + threadIdx.x;
     if (h >= L.n) return;
     const int64_t slot = (int64_t)L.bin_offset[L.key[h]] + L.pib[h];
+    KF_CHECK(slot >= 0 && slot < L.n);
     L.unsorted[slot] = (int32_t)h;
     if (!L.rec_tmp) return;  // ordering only (candidates)
     float v[9];
@@ -162,6 +163,7 @@ bin_rank_gather_kernel(const __grid_constant__ BinBatch B) {
     int32_t rank = 0;
     for (int32_t j = s; j < e; ++j) rank += (__ldg(L.unsorted + j) < mine) ? 1 : 0;
     const int64_t dst = (int64_t)s + rank;
+    KF_CHECK(dst >= 0 && dst < L.n && rank < e - s);
     if (!L.hit_rec) L.sorted_to_orig[dst] = mine;   // else from the record's index word, coalesced (bin_finish_kernel)
     if (L.orig_to_sorted) L.orig_to_sorted[mine] = (int32_t)dst;
     if (!L.rec_tmp) return;  // ordering only (candidates)
@@ -420,6 +422,7 @@ chunk_count_kernel(const __grid_constant__ BinBatch B, const float* __restrict__
             if (li < m) {
                 const uint32_t k = ka[li];
                 const int b = (int)(k >> 16), a = (int)(k & 0xffffu);
+                KF_CHECK(b >= 0 && b < nb);
                 if (a < kPeers) peer[b * kPeers + a] = (uint16_t)li;
                 else {
                     const int32_t j = atomicAdd(&n_over_s, 1);
@@ -605,7 +608,9 @@ chunk_place_kernel(const __grid_constant__ BinBatch B) {
             int32_t dst = -1;
             if (li < m) {
                 const int64_t h = h0 + li;
+                KF_CHECK((kr[j] >> 16) >= 0 && (kr[j] >> 16) < nb);
                 dst = base[kr[j] >> 16] + (kr[j] & 0xffff);
+                KF_CHECK(dst >= 0 && dst < L.n);
                 if (L.orig_to_sorted) L.orig_to_sorted[h] = dst;
                 stage[wid][lane * kRecWords + 0] = make_float4(v[j][0], v[j][1], v[j][2], v[j][8]);                       // x y z vzz
                 stage[wid][lane * kRecWords + 1] = make_float4(v[j][3], v[j][4], v[j][6], __int_as_float((int32_t)h));    // vxx vxy vyy, index

@@ -160,6 +160,17 @@ cudaError_t launch_order(BinScratch& s, const FitParams& P, int layer, int64_t n
                          const int8_t* q, int n_eta, int n_phi, float eta_max, int32_t* order,
                          cudaStream_t stream);
 
+// ---------------------------------------------------------------------------------- bounds checks of a debug build
+// compute-sanitizer is not available on the pool this was developed on; `-DKF_DEBUG_BOUNDS` (python -m
+// paper_1705_02876_b200.build -DKF_DEBUG_BOUNDS --out=...) turns the index computations that SCATTER or GATHER
+// (final slots of the counting sort, hit records read by the scans, peer and overflow lists, the static scratch)
+// into traps when they leave their arrays; the GPU test suite is run against that build before a release.
+#ifdef KF_DEBUG_BOUNDS
+#define KF_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define KF_CHECK(cond) do { } while (0)
+#endif
+
 // ---------------------------------------------------------------------------------- dependent launches
 // The building and binning calls are chains of 4 - 30 short kernels, each reading what the one before wrote; at
 // event size a kernel boundary (drain, launch, ramp) costs 2 - 3 us of a 5 - 15 us kernel.  With programmatic

@@ -205,6 +205,7 @@ scan_kernel(const ScoreArgs a, float inv_r) {
                 const int bin = e * a.n_phi + p;
                 s0 = __ldg(bin_offset + bin);
                 s1 = __ldg(bin_offset + bin + 1);
+                KF_CHECK(s0 >= 0 && s1 >= s0 && (MULTI || s1 <= a.n_hits));
                 const float4 X = __ldg(box + 2 * bin), Z = __ldg(box + 2 * bin + 1);
                 const float dzm = fmaxf(0.0f, fmaxf(Z.x - c.zn, c.zn - Z.y));
                 // rt(x, y) = ec (y - yn) - es (x - xn) is linear: its range over the box is at the corners
@@ -409,6 +410,7 @@ cudaError_t launch_score_static(const FitParams& P, ScoreArgs a, const ScoreStep
     cudaError_t e = static_scratch_address(&base);
     if (e != cudaSuccess) return e;
     const int64_t ld = (a.n + 63) / 64 * 64;                    // planes stay 256-byte aligned; ld <= kStaticMaxCands
+    if (ld > kStaticMaxCands) return cudaErrorInvalidValue;      // (cannot happen: kStaticMaxCands is a multiple of 64)
     a.scratch = base;
     a.track = nullptr;                                          // keep_track = 0 below: never dereferenced
     a.flag = reinterpret_cast<int32_t*>(base + (int64_t)kScorePlanes * ld);

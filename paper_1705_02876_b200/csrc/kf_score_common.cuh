@@ -187,6 +187,7 @@ struct ScanCand {       // what the scan needs of the propagated candidate
 // on a disc (n11 / n12 / n22 = rr / rt / tt of C').
 template <bool DISC = false>
 __device__ __forceinline__ void score_hit(const ScanCand& c, const float4* __restrict__ rec, int32_t slot, Best& best) {
+    KF_CHECK(slot >= 0);
     const float4* r0 = rec + (int64_t)slot * kRecWords;
     const float4 A = __ldg(r0), B = __ldg(r0 + 1), C = __ldg(r0 + 2);
     Crossing o;

@@ -275,6 +275,21 @@ KF_API int kf_fit_tracks_host(kf_ctx* ctx, const kf_geometry* geom, const kf_tra
 KF_API int kf_fit_tracks_host_diag(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                                    const kf_track_hits* hits, kf_tracks* out);
 
+/* kf_fit_tracks_host_diag for hits whose covariance is diagonal in the hit's OWN cylindrical frame (what a strip or
+ * pixel sensor measures, and how the hits of every config here are made: a resolution along the radius, one along
+ * r-phi, one along z; PAPER.md:168 names the host-device transfers as the bottleneck to address next, and 240 of the
+ * 413 input bytes per ten-layer track of the _diag call are hit covariances).  hits->cov is HOST [n_layers][3][ld]:
+ * the variances v_r, v_t, v_z of the hit of track t on layer l along r^ = (x, y, 0)/rho, t^ = (-y, x, 0)/rho and z^,
+ * (x, y) the hit's own position; only those three planes per layer cross the link (12 instead of 24 bytes per hit).
+ * The device rebuilds, in fp32,
+ *     c2 = x x / rho2, s2 = y y / rho2, cs = x y / rho2, rho2 = x x + y y   (rho2 = 0: c2 = 1, s2 = cs = 0)
+ *     xx = v_r c2 + v_t s2,  xy = (v_r - v_t) cs,  yy = v_r s2 + v_t c2,  xz = yz = 0,  zz = v_z
+ * and fits as kf_fit_tracks does.  Results are those of kf_fit_tracks_host_diag given that covariance in full, up to
+ * the rounding of the five lines above (not bit for bit when the caller rebuilt it in another order or precision).
+ * seeds->cov is HOST [6][ld] as in kf_fit_tracks_host_diag. */
+KF_API int kf_fit_tracks_host_compact(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
+                                      const kf_track_hits* hits, kf_tracks* out);
+
 /* ---- hits of one layer and their (eta, phi) bins ------------------------------------ */
 typedef struct {
     int64_t n_hits, ld;       /* ld >= n_hits, ld % 4 == 0                                         */

@@ -25,7 +25,7 @@ BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
 STATIC_MAX_CANDIDATES = 65536                                               # KF_STATIC_MAX_CANDIDATES
 ERR_TOO_LARGE = -8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_hit_record_floats", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_fit_tracks_host_diag", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_abi_version", "kf_hit_record_floats", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_fit_tracks_host_diag", "kf_fit_tracks_host_compact", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_score_candidates_static", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial", "kf_build_combinatorial_events",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
@@ -115,7 +115,7 @@ def load_library():
     lib.kf_abi_version.argtypes = []
     lib.kf_hit_record_floats.restype = C.c_int
     lib.kf_hit_record_floats.argtypes = []
-    for name in ("kf_fit_tracks", "kf_fit_tracks_host", "kf_fit_tracks_host_diag"):
+    for name in ("kf_fit_tracks", "kf_fit_tracks_host", "kf_fit_tracks_host_diag", "kf_fit_tracks_host_compact"):
         f = getattr(lib, name)
         f.restype = C.c_int
         f.argtypes = [vp, C.POINTER(_Geometry), C.POINTER(_Tracks), C.POINTER(_TrackHits), C.POINTER(_Tracks)]
@@ -356,9 +356,9 @@ class KFContext:
                        chi2.data_ptr(), nhits.data_ptr(), status.data_ptr())
 
     @staticmethod
-    def _track_hits(n, L, hpos, hcov, mask) -> _TrackHits:
+    def _track_hits(n, L, hpos, hcov, mask, cov_planes=6) -> _TrackHits:
         ld = _plane_ld(hpos, 3 * L)
-        if _plane_ld(hcov, 6 * L) != ld:
+        if _plane_ld(hcov, cov_planes * L) != ld:
             raise ValueError("hpos and hcov must share the plane stride ld")
         return _TrackHits(int(L), int(n), ld, hpos.data_ptr(), hcov.data_ptr(),
                           mask.data_ptr() if mask is not None else None)
@@ -443,9 +443,14 @@ class KFContext:
         del keep
 
     def fit_tracks_host(self, geom: Geometry, n: int, par, cov, q, hpos, hcov, mask,
-                        out_par, out_cov, out_chi2, out_nhits, out_status, cov_diagonal: bool = False):
+                        out_par, out_cov, out_chi2, out_nhits, out_status, cov_diagonal: bool = False,
+                        hit_cov_local: bool = False):
         """Same with HOST tensors (pinned for full overlap); returns when the outputs are complete.
-        cov_diagonal: `cov` is [6][ld], the diagonal of the seed covariance (kf_fit_tracks_host_diag)."""
+        cov_diagonal: `cov` is [6][ld], the diagonal of the seed covariance (kf_fit_tracks_host_diag).
+        hit_cov_local (with cov_diagonal): `hcov` is [L][3][ld], the variances of each hit along its own r^, t^, z^
+        (kf_fit_tracks_host_compact)."""
+        if hit_cov_local and not cov_diagonal:
+            raise ValueError("hit_cov_local goes with cov_diagonal (kf_fit_tracks_host_compact)")
         for t in (par, cov, q, hpos, hcov, out_par, out_cov, out_chi2, out_nhits, out_status):
             if t.is_cuda:
                 raise ValueError("fit_tracks_host takes CPU tensors")
@@ -456,10 +461,10 @@ class KFContext:
         seeds = _Tracks(int(n), ld, par.data_ptr(), cov.data_ptr(), q.data_ptr(), out_chi2.data_ptr(), out_nhits.data_ptr(),
                         out_status.data_ptr())
         out = self._tracks(n, out_par, out_cov, None, out_chi2, out_nhits, out_status)
-        hits = self._track_hits(n, g.n_layers, hpos, hcov, mask)
-        fn = self._lib.kf_fit_tracks_host_diag if cov_diagonal else self._lib.kf_fit_tracks_host
-        self._check(fn(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)),
-                    "kf_fit_tracks_host_diag" if cov_diagonal else "kf_fit_tracks_host")
+        hits = self._track_hits(n, g.n_layers, hpos, hcov, mask, 3 if hit_cov_local else 6)
+        name = ("kf_fit_tracks_host_compact" if hit_cov_local else
+                "kf_fit_tracks_host_diag" if cov_diagonal else "kf_fit_tracks_host")
+        self._check(getattr(self._lib, name)(self._h, C.byref(g), C.byref(seeds), C.byref(hits), C.byref(out)), name)
         del keep
 
     # ------------------------------------------------------------------ kf_bin_hits / kf_bin_layers

@@ -118,9 +118,11 @@ class DeviceFit:
                     chi2=sm["chi2"][:n].cpu().numpy(), nhits=sm["nhits"][:n].cpu().numpy(),
                     status=sm["status"][:n].cpu().numpy().view(np.uint32))
 
-    def fit_host(self, ctx: KFContext, cov_diagonal: bool = False):
+    def fit_host(self, ctx: KFContext, cov_diagonal: bool = False, hit_var: torch.Tensor | None = None):
         """kf_fit_tracks_host; cov_diagonal: kf_fit_tracks_host_diag with the six diagonal planes of self.cov (kept as
-        self.cov_diag, pinned like the rest; the caller asserts that the seed covariance IS diagonal)."""
+        self.cov_diag, pinned like the rest; the caller asserts that the seed covariance IS diagonal).  hit_var (a host
+        [L][3][ld] tensor, with cov_diagonal): kf_fit_tracks_host_compact, the variances of every hit along its own
+        r^, t^, z^ in place of self.hcov."""
         cov = self.cov
         if cov_diagonal:
             cov = getattr(self, "cov_diag", None)
@@ -128,14 +130,17 @@ class DeviceFit:
                 cov = torch.empty((6, self.ld), dtype=torch.float32, pin_memory=self.cov.is_pinned())
                 cov.copy_(self.cov[[0, 6, 11, 15, 18, 20]])
                 self.cov_diag = cov
-        ctx.fit_tracks_host(self.geom, self.n, self.par, cov, self.q, self.hpos, self.hcov, self.mask,
-                            self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status, cov_diagonal)
+        ctx.fit_tracks_host(self.geom, self.n, self.par, cov, self.q, self.hpos, self.hcov if hit_var is None else hit_var,
+                            self.mask, self.out_par, self.out_cov, self.out_chi2, self.out_nhits, self.out_status,
+                            cov_diagonal, hit_var is not None)
 
     def results(self) -> dict:
+        """Copies of the outputs (also when the buffers are host tensors: a later call must not change them)."""
         n = self.n
-        return dict(par=self.out_par[:, :n].cpu().numpy(), cov=self.out_cov[:, :n].cpu().numpy(),
-                    chi2=self.out_chi2[:n].cpu().numpy(), nhits=self.out_nhits[:n].cpu().numpy(),
-                    status=self.out_status[:n].cpu().numpy().view(np.uint32))
+        host = lambda t: np.array(t.cpu().numpy(), copy=True)
+        return dict(par=host(self.out_par[:, :n]), cov=host(self.out_cov[:, :n]),
+                    chi2=host(self.out_chi2[:n]), nhits=host(self.out_nhits[:n]),
+                    status=host(self.out_status[:n]).view(np.uint32))
 
     @property
     def algorithmic_bytes(self) -> int:

@@ -40,7 +40,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 12;
+constexpr int kAbiVersion = 13;
 static_assert(kRecFloats == KF_HIT_RECORD_FLOATS || kRecWords == 4, "kf_internal.h and kf_b200.h disagree on the hit record");
 
 // Makes the context's device current for the duration of an ABI call and puts the caller's device back on
@@ -466,7 +466,7 @@ int kf_fit_tracks_smooth(kf_ctx* c, const kf_geometry* geom, const kf_tracks* se
 
 namespace {
 int fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits, kf_tracks* out,
-                    bool cov_diagonal);
+                    bool cov_diagonal, bool hit_cov_local = false);
 }
 int kf_fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
                        const kf_track_hits* hits, kf_tracks* out) {
@@ -476,10 +476,14 @@ int kf_fit_tracks_host_diag(kf_ctx* c, const kf_geometry* geom, const kf_tracks*
                             const kf_track_hits* hits, kf_tracks* out) {
     return fit_tracks_host(c, geom, seeds, hits, out, true);
 }
+int kf_fit_tracks_host_compact(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds,
+                               const kf_track_hits* hits, kf_tracks* out) {
+    return fit_tracks_host(c, geom, seeds, hits, out, true, true);
+}
 }  // extern "C"
 namespace {
 int fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, const kf_track_hits* hits, kf_tracks* out,
-                    bool cov_diagonal) {
+                    bool cov_diagonal, bool hit_cov_local) {
     if (!c || !geom || !seeds || !hits || !out) return KF_ERR_NULL;
     FitParams P;
     int rc = make_params(geom, &P, true);
@@ -498,6 +502,7 @@ int fit_tracks_host(kf_ctx* c, const kf_geometry* geom, const kf_tracks* seeds, 
     io.opar = out->par; io.ocov = out->cov; io.ld_out = out->ld;
     io.chi2 = out->chi2; io.nhits = out->nhits; io.status = out->status;
     io.cov_diagonal = cov_diagonal;
+    io.hit_cov_local = hit_cov_local;
     e = c->host.fit(P, io, c->opt);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     return KF_OK;

@@ -25,7 +25,7 @@ inline size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
 
 // Offsets of the SoA arrays of one chunk inside a slot buffer.
 struct SlotLayout {
-    size_t par, cov, q, mask, hpos, hcov, opar, ocov, chi2, nhits, status, diag, total;
+    size_t par, cov, q, mask, hpos, hcov, opar, ocov, chi2, nhits, status, diag, hvar, total;
     SlotLayout(int64_t chunk, int L) {
         size_t o = 0;
         auto take = [&](size_t bytes) { size_t at = o; o += align256(bytes); return at; };
@@ -35,9 +35,49 @@ struct SlotLayout {
         opar = take(6 * chunk * 4);  ocov = take(21 * chunk * 4);
         chi2 = take(chunk * 4);      nhits = take(chunk * 4);  status = take(chunk * 4);
         diag = take(6 * chunk * 4);  // kf_fit_tracks_host_diag: the six variance planes as they arrive
+        hvar = take((size_t)L * 3 * chunk * 4);  // kf_fit_tracks_host_compact: v_r v_t v_z of every hit as they arrive
         total = o;
     }
 };
+
+// kf_fit_tracks_host_compact: the hit covariance from its three variances in the hit's own cylindrical frame,
+// V = R_z(phi_h) diag(v_r, v_t, v_z) R_z(phi_h)^T with (cos, sin) phi_h = (x, y) / rho of the hit position
+// (include/kf_b200.h states the five lines below; four tracks per thread, planes are 16-byte aligned).
+__global__ void __launch_bounds__(256) expand_hit_cov_kernel(const float* __restrict__ hpos, const float* __restrict__ hvar,
+                                                             float* __restrict__ hcov, int64_t m, int64_t ld) {
+    const int64_t t = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (t >= m) return;
+    const int l = blockIdx.y;
+    const float* p = hpos + (size_t)l * 3 * ld + t;
+    const float* v = hvar + (size_t)l * 3 * ld + t;
+    float* c = hcov + (size_t)l * 6 * ld + t;
+    const float4 x4 = *reinterpret_cast<const float4*>(p), y4 = *reinterpret_cast<const float4*>(p + ld);
+    const float4 r4 = *reinterpret_cast<const float4*>(v), t4 = *reinterpret_cast<const float4*>(v + ld);
+    const float4 z4 = *reinterpret_cast<const float4*>(v + 2 * ld);
+    const float x[4] = {x4.x, x4.y, x4.z, x4.w}, y[4] = {y4.x, y4.y, y4.z, y4.w};
+    const float vr[4] = {r4.x, r4.y, r4.z, r4.w}, vt[4] = {t4.x, t4.y, t4.z, t4.w};
+    float xx[4], xy[4], yy[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float rho2 = __fadd_rn(__fmul_rn(x[k], x[k]), __fmul_rn(y[k], y[k]));
+        float c2 = 1.0f, s2 = 0.0f, cs = 0.0f;
+        if (rho2 > 0.0f) {
+            c2 = __fdiv_rn(__fmul_rn(x[k], x[k]), rho2);
+            s2 = __fdiv_rn(__fmul_rn(y[k], y[k]), rho2);
+            cs = __fdiv_rn(__fmul_rn(x[k], y[k]), rho2);
+        }
+        xx[k] = __fadd_rn(__fmul_rn(vr[k], c2), __fmul_rn(vt[k], s2));
+        xy[k] = __fmul_rn(__fsub_rn(vr[k], vt[k]), cs);
+        yy[k] = __fadd_rn(__fmul_rn(vr[k], s2), __fmul_rn(vt[k], c2));
+    }
+    const float4 zero = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    *reinterpret_cast<float4*>(c) = make_float4(xx[0], xx[1], xx[2], xx[3]);
+    *reinterpret_cast<float4*>(c + ld) = make_float4(xy[0], xy[1], xy[2], xy[3]);
+    *reinterpret_cast<float4*>(c + 2 * ld) = zero;
+    *reinterpret_cast<float4*>(c + 3 * ld) = make_float4(yy[0], yy[1], yy[2], yy[3]);
+    *reinterpret_cast<float4*>(c + 4 * ld) = zero;
+    *reinterpret_cast<float4*>(c + 5 * ld) = z4;
+}
 
 }  // namespace
 
@@ -106,6 +146,14 @@ cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const Launch
         KF_TRY(cudaMemcpyAsync(b + lay.q, io.q + t0, (size_t)m, cudaMemcpyHostToDevice, st));
         if (io.mask) KF_TRY(cudaMemcpyAsync(b + lay.mask, io.mask + t0, w, cudaMemcpyHostToDevice, st));
         KF_TRY(cudaMemcpy2DAsync(b + lay.hpos, cw, io.hpos + t0, (size_t)io.ld_hit * 4, w, (size_t)L * 3, cudaMemcpyHostToDevice, st));
+        if (io.hit_cov_local) {
+            // 3 of the 6 planes per layer travel; the covariance is rebuilt beside the hit positions
+            KF_TRY(cudaMemcpy2DAsync(b + lay.hvar, cw, io.hcov + t0, (size_t)io.ld_hit * 4, w, (size_t)L * 3, cudaMemcpyHostToDevice, st));
+            const dim3 grid((unsigned)((m + 1023) / 1024), (unsigned)L);
+            expand_hit_cov_kernel<<<grid, 256, 0, st>>>((const float*)(b + lay.hpos), (const float*)(b + lay.hvar),
+                                                        (float*)(b + lay.hcov), m, chunk);
+            KF_TRY(cudaGetLastError());
+        } else
         KF_TRY(cudaMemcpy2DAsync(b + lay.hcov, cw, io.hcov + t0, (size_t)io.ld_hit * 4, w, (size_t)L * 6, cudaMemcpyHostToDevice, st));
         {
             FitArgs a;

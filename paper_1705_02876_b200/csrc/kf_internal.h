@@ -72,6 +72,7 @@ struct HostFitIO {
     const float* hpos; const float* hcov; int64_t ld_hit; const uint32_t* mask;
     float* opar; float* ocov; int64_t ld_out; float* chi2; int32_t* nhits; uint32_t* status;
     bool cov_diagonal = false;   // kf_fit_tracks_host_diag: cov is [6][ld_in], the diagonal of the seed covariance
+    bool hit_cov_local = false;  // kf_fit_tracks_host_compact: hcov is [L][3][ld_hit], the variances along r^ t^ z^ of the hit
 };
 
 // Device staging for kf_fit_tracks_host: kSlots chunk buffers, each with its own stream, so the

@@ -44,7 +44,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_abi_version_and_error_strings(lib):
     import paper_1705_02876_b200 as K
-    assert K.abi_version() == 12
+    assert K.abi_version() == 13
     assert K.binding.hit_record_floats() == 12
     seen = set()
     for code in (0, -1, -2, -3, -4, -5, -6, -7, -99):
@@ -60,6 +60,7 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.kf_fit_tracks(None, None, None, None, None) == -1
     assert lib.kf_fit_tracks_host(None, None, None, None, None) == -1
     assert lib.kf_fit_tracks_host_diag(None, None, None, None, None) == -1
+    assert lib.kf_fit_tracks_host_compact(None, None, None, None, None) == -1
     assert lib.kf_fit_tracks_indexed(None, None, None, None, 0, None, None, None) == -1
     assert lib.kf_fit_tracks_refit(None, None, None, None, 10.0, None, None) == -1
     assert lib.kf_fit_tracks_smooth(None, None, None, None, None, None) == -1

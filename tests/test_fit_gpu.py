@@ -274,6 +274,70 @@ def test_fit_host_path_with_diagonal_seed_covariance(ctx):
     assert np.count_nonzero(diag["chi2"]) > 0.99 * b.n
 
 
+def _local_hit_variances(b, rng=None):
+    """[L][3][n] fp32: v_r, v_t, v_z of every hit (the workload's resolutions; with rng, scaled hit by hit so the
+    three planes are not constants) and the covariance they stand for, in fp64 from the fp32 positions and variances
+    as include/kf_b200.h defines it: V = Rz(phi_h) diag(v_r, v_t, v_z) Rz(phi_h)^T, (cos, sin) phi_h = (x, y) / rho."""
+    L, n = b.hpos.shape[0], b.n
+    var = np.empty((L, 3, n), dtype=np.float32)
+    var[:, 0], var[:, 1], var[:, 2] = W.SIGMA_R ** 2, W.SIGMA_RPHI ** 2, W.SIGMA_Z ** 2
+    if rng is not None:
+        var *= rng.uniform(0.5, 2.0, size=var.shape).astype(np.float32)
+    x, y = b.hpos[:, 0].astype(np.float64), b.hpos[:, 1].astype(np.float64)
+    rho2 = x * x + y * y
+    ok = rho2 > 0
+    c2 = np.where(ok, x * x / np.where(ok, rho2, 1.0), 1.0)
+    s2 = np.where(ok, y * y / np.where(ok, rho2, 1.0), 0.0)
+    cs = np.where(ok, x * y / np.where(ok, rho2, 1.0), 0.0)
+    vr, vt, vz = (var[:, k].astype(np.float64) for k in range(3))
+    zero = np.zeros_like(vr)
+    full = np.stack([vr * c2 + vt * s2, (vr - vt) * cs, zero, vr * s2 + vt * c2, zero, vz], axis=1)   # [L][6][n]
+    return var, full
+
+
+def test_fit_host_path_with_local_hit_variances(ctx):
+    """kf_fit_tracks_host_compact: three variance planes per layer cross the link instead of six covariance planes,
+    and the device rebuilds the covariance from the hit position.  (1) parity with the oracle given that covariance
+    in fp64, every track of a batch that spans three chunks and a ragged tail, variances that differ hit by hit;
+    (2) on the workload's own hits (constant resolutions) the call agrees with the full-covariance call to rounding
+    (the workload rotates by the same azimuth, so both describe the same covariance)."""
+    import copy
+    from paper_1705_02876_b200.buffers import DeviceFit, _to_planes
+    b = W.make_fit_batch(2, n_events=14)
+    b = copy.copy(b)
+    var, full = _local_hit_variances(b, np.random.default_rng(5))
+    h = DeviceFit.from_batch(b, "cpu", pin=True)
+    hv = _to_planes(var, h.ld, torch.device("cpu"), True)
+    h.fit_host(ctx, cov_diagonal=True, hit_var=hv)
+    g = h.results()
+    sel = slice(0, b.n, 7)                                   # every 7th track through the oracle: 40 000 of them
+    o = O.fit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par[:, sel], b.cov[:, sel], b.q[sel], b.hpos[:, :, sel],
+                     full[:, :, sel], b.mask[sel], nthreads=8)
+    gs = {k: (v[..., sel] if k in ("par", "cov") else v[sel]) for k, v in g.items()}
+    res = compare_fit(gs, o, float(b.radius[-1]))
+    print("compact host call vs oracle:", res)
+    # the tail of the last chunk and the chunk boundaries, one by one
+    for lo in (131_072 - 3, 262_144 - 3, b.n - 5):
+        s2 = slice(lo, min(lo + 6, b.n))
+        o2 = O.fit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par[:, s2], b.cov[:, s2], b.q[s2], b.hpos[:, :, s2],
+                          full[:, :, s2], b.mask[s2])
+        compare_fit({k: (v[..., s2] if k in ("par", "cov") else v[s2]) for k, v in g.items()}, o2, float(b.radius[-1]),
+                    max_diverged_frac=1.0)
+    # (2)
+    var0, _ = _local_hit_variances(b)
+    h.fit_host(ctx, cov_diagonal=True)
+    ref = h.results()
+    h.out_par.zero_(); h.out_cov.zero_(); h.out_chi2.zero_()
+    h.fit_host(ctx, cov_diagonal=True, hit_var=_to_planes(var0, h.ld, torch.device("cpu"), True))
+    r = h.results()
+    assert np.array_equal(ref["nhits"], r["nhits"]) and np.array_equal(ref["status"], r["status"])
+    ok = ref["status"] == 0
+    assert np.allclose(ref["par"][:, ok], r["par"][:, ok], rtol=2e-4, atol=2e-5)
+    assert np.allclose(ref["chi2"][ok], r["chi2"][ok], rtol=2e-3, atol=2e-3)
+    with pytest.raises(ValueError):
+        h.fit_host(ctx, cov_diagonal=False, hit_var=hv)
+
+
 def test_fit_argument_errors(ctx):
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceFit

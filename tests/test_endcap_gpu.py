@@ -61,6 +61,38 @@ def test_endcap_fit_parity(ctx):
     assert np.all(np.abs(np.abs(g["par"][2][ok]) - b.disc_z[last[ok]]) < 1e-4)
 
 
+def test_endcap_fit_and_smoother_at_the_benched_size(ctx):
+    """bench.py times the barrel + endcap toy on 2 M tracks made of one 20 000-track event a hundred times (launch
+    configuration: 15 625 CTAs of the one-track kernel, smoothed planes of 2 M columns).  Every copy must come out as
+    the event does when it is fitted alone, bit for bit, forward result and smoothed states at every layer; the event
+    alone is held against the oracle by test_endcap_fit_parity / test_endcap_smoother_parity."""
+    from paper_1705_02876_b200.buffers import DeviceFit
+    ev = W.simulate_endcap_event(0, 20000)
+    one = DeviceFit.from_batch(ev, "cuda:0")
+    one.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    r1, s1 = one.results(), one.smoothed_results()
+    one.fit(ctx)
+    torch.cuda.synchronize()
+    f1 = one.results()
+    big = DeviceFit.from_batch(W.concat_batches([ev] * 100), "cuda:0")
+    assert big.n == 2_000_000
+    big.fit(ctx)
+    torch.cuda.synchronize()
+    fb = big.results()
+    big.fit_smooth(ctx)
+    torch.cuda.synchronize()
+    rb, sb = big.results(), big.smoothed_results()
+    for c in (0, 1, 37, 99):
+        lo, hi = c * 20000, (c + 1) * 20000
+        for k in f1:
+            assert np.array_equal(f1[k], fb[k][..., lo:hi], equal_nan=True), (c, k)
+            assert np.array_equal(r1[k], rb[k][..., lo:hi], equal_nan=True), (c, k)
+        for k in s1:
+            assert np.array_equal(s1[k], sb[k][..., lo:hi], equal_nan=True), (c, k)
+    assert (fb["status"] == 0).mean() > 0.9
+
+
 @pytest.mark.parametrize("n", [1, 33, 1001])
 def test_endcap_ragged_sizes_and_host_path(ctx, n):
     b = W.simulate_endcap_event(2, n)

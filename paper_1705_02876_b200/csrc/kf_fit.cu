@@ -998,10 +998,6 @@ fit_indexed_kernel(const __grid_constant__ FitParams P, const __grid_constant__ 
 
 }  // namespace
 
-namespace {
-
-}  // namespace
-
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: set once for every device a context
 // launches on (the caller has made that device current).
 cudaError_t ensure_fit_attributes() {

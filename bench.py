@@ -838,9 +838,13 @@ def run_ours(args) -> None:
         ixr_ms = i0.elapsed_time(i1) / 10
         del pbins
         indexed = {"api": "kf_fit_tracks_indexed (hits gathered by index from shuffled layer pools)", "ms": ix_ms,
-                   "fits_per_s": n / (ix_ms * 1e-3), "sector_bytes_per_fit": 233 + L * (4 + 9 * 32),
+                   "fits_per_s": n / (ix_ms * 1e-3), "sector_bytes_per_fit": 233 + L * (4 + 2 * 32) + L * (36 + 48),
                    "records_ms": ixr_ms, "records_fits_per_s": n / (ixr_ms * 1e-3),
-                   "note": "nine scattered 4-byte loads per hit: bound by 32-byte DRAM/L2 sectors, not by arithmetic"}
+                   "note": "ms: SoA pools, packed by the call itself into 48-byte records in original order (36 B read + 48 B "
+                           "written per pool hit) and gathered from those, 2 memory sectors per hit (round 1 read the SoA "
+                           "planes directly, 9 sectors per hit: 3.3 ms); records_ms: the bin-ordered records of "
+                           "kf_bin_layers through orig_to_sorted (no packing, one more look-up per hit); both are bound by "
+                           "32-byte sectors of scattered reads, not by arithmetic"}
         del pools, perm, index
         # secondary: the other fit configs of BASELINE.json (0, 1: one event, launch-bound; 3: 100 000 tracks x 20
         # layers), one kf_fit_tracks call each, eager through the binding and replayed from a recorded graph

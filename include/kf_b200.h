@@ -317,8 +317,11 @@ typedef struct {
  * buffers inside), -1 = no hit on that layer.  Otherwise exactly kf_fit_tracks (same arithmetic, same
  * status semantics, `out` may alias `seeds`).  index: DEV int32 [n_layers][ld_index], ld_index >= n.
  * `bins` = NULL, or a HOST array of n_layers kf_layer_bins made from the same pools by kf_bin_layers with
- * hit_rec and orig_to_sorted filled: the hits are then read from the packed records (2 memory sectors per
- * hit instead of 9), same values, same results. */
+ * hit_rec and orig_to_sorted filled: the hits are then read from those packed records (2 memory sectors per
+ * hit instead of 9), same values, same results.  With bins = NULL the call packs the pools into records of its own
+ * first (context scratch of 48 bytes per pool hit, grown on demand like the other scratch: a call that has to grow
+ * it synchronises the stream and cannot be recorded into a graph), unless the pools hold more than eight times the
+ * hits the tracks can read, in which case the SoA planes are read directly.  Same results either way, bit for bit. */
 KF_API int kf_fit_tracks_indexed(kf_ctx* ctx, const kf_geometry* geom, const kf_tracks* seeds,
                                  const int32_t* index, int64_t ld_index, const kf_layer_hits* pools,
                                  const kf_layer_bins* bins, kf_tracks* out);

@@ -31,11 +31,13 @@ struct kf_ctx {
     // kf_score_candidates / kf_build_best_hit scratch
     ScoreScratch score;
     CombScratch comb;
+    // kf_fit_tracks_indexed: the pools as packed records
+    IndexScratch index;
     // *_host staging
     HostStage host;
     BuildHostStage build_host;
     // every reallocation of scratch and every rewrite of the bin edge tables moves this on
-    uint64_t scratch_gen() const { return bin.gen + score.gen + comb.gen; }
+    uint64_t scratch_gen() const { return bin.gen + score.gen + comb.gen + index.gen; }
 };
 
 namespace {
@@ -221,6 +223,7 @@ int kf_destroy(kf_ctx* c) {
     c->bin.release();
     c->score.release();
     c->comb.release();
+    c->index.release();
     c->host.release();
     c->build_host.release();
     delete c;
@@ -399,7 +402,31 @@ int kf_fit_tracks_indexed(kf_ctx* c, const kf_geometry* geom, const kf_tracks* s
     a.opar = out->par; a.ocov = out->cov; a.ld_out = out->ld;
     a.chi2 = out->chi2; a.nhits = out->nhits; a.status = out->status;
     KF_ON_DEVICE(c);
-    cudaError_t e = launch_fit_indexed(P, H, a, c->stream);
+    cudaError_t e;
+    if (!bins) {
+        // SoA pools: nine scattered 4-byte loads per hit cost nine memory sectors.  Unless the pools are far larger
+        // than what the tracks will read of them, pack them once into 48-byte records (original order, context
+        // scratch) and gather those: two sectors per hit.
+        PackPools A;
+        std::memset(&A, 0, sizeof(A));
+        int64_t total = 0;
+        for (int l = 0; l < geom->n_layers; ++l) total += (pools[l].n_hits + 3) / 4 * 4;
+        if (total > 0 && total <= 8 * seeds->n * (int64_t)geom->n_layers) {
+            e = c->index.reserve((size_t)total * kRecFloats * 4, c->stream);
+            if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
+            int64_t at = 0;
+            for (int l = 0; l < geom->n_layers; ++l) {
+                A.pos[l] = pools[l].pos; A.cov[l] = pools[l].cov; A.ld[l] = pools[l].ld; A.n[l] = pools[l].n_hits;
+                A.rec[l] = c->index.rec + at * kRecFloats;
+                H.hit_rec[l] = A.rec[l];
+                at += (pools[l].n_hits + 3) / 4 * 4;
+            }
+            e = launch_pack_pools(A, geom->n_layers, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e);
+            H.use_records = 2;
+        }
+    }
+    e = launch_fit_indexed(P, H, a, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;
 }

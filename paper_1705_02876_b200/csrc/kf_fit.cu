@@ -930,7 +930,7 @@ fit_pair_kernel(const __grid_constant__ FitParams P, const __grid_constant__ Fit
 // and the index of layer l + 3 read -- every stage has a whole layer of arithmetic to hide behind.
 __device__ __forceinline__ int32_t resolve_hit(const IndexedPools& H, int l, int32_t h) {
     if (h < 0) return -1;
-    return H.use_records ? __ldg(H.orig_to_sorted[l] + h) : h;
+    return H.use_records == 1 ? __ldg(H.orig_to_sorted[l] + h) : h;
 }
 __device__ __forceinline__ Hit fetch_hit(const IndexedPools& H, int l, int32_t s) {
     Hit m;
@@ -947,6 +947,37 @@ __device__ __forceinline__ Hit fetch_hit(const IndexedPools& H, int l, int32_t s
     m.vxx = __ldg(c + s);          m.vxy = __ldg(c + ld + s);     m.vxz = __ldg(c + 2 * ld + s);
     m.vyy = __ldg(c + 3 * ld + s); m.vyz = __ldg(c + 4 * ld + s); m.vzz = __ldg(c + 5 * ld + s);
     return m;
+}
+
+// SoA pools -> packed records in ORIGINAL order (same 12-float layout as kf_bin_layers' records: fetch_hit reads
+// both).  Reads coalesced plane by plane; a warp's 32 records are staged in shared memory and leave as 96
+// consecutive 16-byte words.
+__global__ void __launch_bounds__(256) pack_pool_records_kernel(const __grid_constant__ PackPools A) {
+    static_assert(kRecWords == 3 || kRecWords == 4, "record layout");
+    __shared__ float4 stage[8][32 * kRecWords];
+    const int l = blockIdx.y;
+    const int64_t n = A.n[l];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t base = (int64_t)blockIdx.x * 256 + w * 32;      // first hit of this warp
+    if (base >= n) return;
+    const int64_t h = base + lane;
+    if (h < n) {
+        const float* p = A.pos[l] + h;
+        const float* c = A.cov[l] + h;
+        const int64_t ld = A.ld[l];
+        const float x = __ldg(p), y = __ldg(p + ld), z = __ldg(p + 2 * ld);
+        const float vxx = __ldg(c), vxy = __ldg(c + ld), vxz = __ldg(c + 2 * ld);
+        const float vyy = __ldg(c + 3 * ld), vyz = __ldg(c + 4 * ld), vzz = __ldg(c + 5 * ld);
+        float4* s = &stage[w][lane * kRecWords];
+        s[0] = make_float4(x, y, z, vzz);
+        s[1] = make_float4(vxx, vxy, vyy, __int_as_float((int)h));
+        s[2] = make_float4(vxz, vyz, 0.0f, 0.0f);
+        if constexpr (kRecWords == 4) s[3] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    }
+    __syncwarp();
+    const int cnt = (int)(n - base < 32 ? n - base : 32) * kRecWords;
+    float4* out = reinterpret_cast<float4*>(A.rec[l]) + base * kRecWords;
+    for (int j = lane; j < cnt; j += 32) out[j] = stage[w][j];
 }
 
 template <int GEOM>
@@ -1080,6 +1111,32 @@ cudaError_t launch_fit(const FitParams& P, const FitArgs& a, cudaStream_t stream
     else if (P.has_discs) fit_kernel<0, 2><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else if (geom) fit_kernel<0, 1><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
     else fit_kernel<0, 0><<<(unsigned)blocks, kFitBlock, kSmemBytes, stream>>>(P, M, a);
+    return cudaGetLastError();
+}
+
+cudaError_t IndexScratch::reserve(size_t bytes, cudaStream_t stream) {
+    if (bytes <= cap) return cudaSuccess;
+    cudaError_t e = cudaStreamSynchronize(stream);       // the records of the previous call may still be read
+    if (e != cudaSuccess) return e;
+    release();
+    ++gen;
+    if ((e = cudaMalloc(&rec, bytes)) != cudaSuccess) { rec = nullptr; return e; }
+    cap = bytes;
+    return cudaSuccess;
+}
+
+void IndexScratch::release() {
+    if (rec) cudaFree(rec);
+    rec = nullptr;
+    cap = 0;
+}
+
+cudaError_t launch_pack_pools(const PackPools& A, int n_layers, cudaStream_t stream) {
+    int64_t most = 0;
+    for (int l = 0; l < n_layers; ++l) most = A.n[l] > most ? A.n[l] : most;
+    if (most == 0) return cudaSuccess;
+    const dim3 grid((unsigned)((most + 255) / 256), (unsigned)n_layers);
+    pack_pool_records_kernel<<<grid, 256, 0, stream>>>(A);
     return cudaGetLastError();
 }
 

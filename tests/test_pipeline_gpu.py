@@ -21,12 +21,14 @@ def ctx():
     c.close()
 
 
-def _fit_indexed(ctx, ev, index_np, use_records=False):
-    """Fit the event's seeds with hits index_np[L][n] (into ev.layers pools, -1 = none)."""
+def _fit_indexed(ctx, ev, index_np, use_records=False, n_fit=None):
+    """Fit the event's seeds (the first n_fit of them) with hits index_np[L][n] (into ev.layers pools, -1 = none)."""
     import paper_1705_02876_b200 as K
     from paper_1705_02876_b200.buffers import DeviceFit, DeviceLayer, padded_ld
     f = ev.fit
     d = DeviceFit.from_batch(f, "cuda:0")
+    if n_fit is not None:
+        d.n = n_fit
     pools = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers]
     idx = torch.full((len(ev.layers), padded_ld(f.n)), -1, dtype=torch.int32, device="cuda:0")
     idx[:, :f.n] = torch.from_numpy(np.ascontiguousarray(index_np, dtype=np.int32)).to("cuda:0")
@@ -34,7 +36,7 @@ def _fit_indexed(ctx, ev, index_np, use_records=False):
     if use_records:
         ctx.bin_layers([l.radius for l in ev.layers], [(p.n_hits, p.pos, p.cov, p.bins) for p in pools])
         bins = [p.bins for p in pools]
-    ctx.fit_tracks_indexed(d.geom, f.n, d.par, d.cov, d.q, idx, [(p.n_hits, p.pos, p.cov) for p in pools],
+    ctx.fit_tracks_indexed(d.geom, d.n, d.par, d.cov, d.q, idx, [(p.n_hits, p.pos, p.cov) for p in pools],
                            d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status, bins=bins)
     torch.cuda.synchronize()
     return d.results()
@@ -71,6 +73,44 @@ def test_indexed_fit_with_true_hits_equals_the_pre_gathered_fit(ctx):
     assert np.array_equal(r["nhits"], g["nhits"]) and np.array_equal(r["status"], g["status"])
     np.testing.assert_allclose(r["chi2"], g["chi2"], rtol=2e-4, atol=1e-4)
     np.testing.assert_allclose(r["par"], g["par"], rtol=0, atol=2e-4)
+
+
+def test_indexed_fit_reads_pools_directly_or_through_packed_records(ctx):
+    """Without bins the call packs the SoA pools into records of its own (context scratch) unless the pools hold more
+    than eight times the hits the tracks will read: both branches, same results bit for bit -- a few tracks against
+    large pools (direct reads), all tracks (packed), and again a few (the scratch of the packed call is still there
+    and must not be used)."""
+    ev = W.make_build_event(4, n_tracks=4001, noise_hits=20000)
+    truth = np.stack([l.true_index for l in ev.layers])
+    total = sum((len(l.pos[0]) + 3) // 4 * 4 for l in ev.layers)
+    L = len(ev.layers)
+    assert total > 8 * 300 * L and total <= 8 * 4001 * L
+    few = _fit_indexed(ctx, ev, truth, n_fit=300)                 # direct reads
+    full = _fit_indexed(ctx, ev, truth)                           # packed records
+    few2 = _fit_indexed(ctx, ev, truth, n_fit=300)
+    rec = _fit_indexed(ctx, ev, truth, use_records=True)          # kf_bin_layers' records
+    for k in full:
+        assert np.array_equal(few[k], full[k][..., :300], equal_nan=True), k
+        assert np.array_equal(few[k], few2[k], equal_nan=True), k
+        assert np.array_equal(rec[k], full[k], equal_nan=True), k
+    # a pool of a single hit, an empty pool, and a ragged last warp of the packing kernel
+    import copy
+    ev2 = copy.deepcopy(ev)
+    keep = 20037
+    for j, l in enumerate(ev2.layers):
+        m = 1 if j == 2 else (0 if j == 4 else keep + j)
+        l.pos, l.cov = np.ascontiguousarray(l.pos[:, :m]), np.ascontiguousarray(l.cov[:, :m])
+        truth[j] = np.where(truth[j] < m, truth[j], -1)
+    a = _fit_indexed(ctx, ev2, truth)
+    b = _fit_indexed(ctx, ev2, truth, n_fit=300)
+    o = _oracle_fit_with(ev2, truth)
+    assert np.array_equal(a["nhits"], o["nhits"])
+    for k in a:
+        assert np.array_equal(a[k][..., :300], b[k], equal_nan=True), k
+    sel = o["nhits"] >= 4
+    compare_fit({k: (v[..., sel] if k in ("par", "cov") else v[sel]) for k, v in a.items()},
+                {k: (v[..., sel] if k == "par" else v[sel]) for k, v in o.items()}, float(ev.fit.radius[-1]),
+                max_diverged_frac=0.02)
 
 
 def test_indexed_fit_with_path_length_material_and_energy_loss(ctx):

@@ -6,6 +6,7 @@
 // with kernels via streams"; PAPER.md:164 transfers are half of the wall time when they are not).
 // With pinned host memory the copies are truly asynchronous; with pageable memory the runtime
 // stages them and the pipeline degrades gracefully.
+#include <cmath>
 #include <cstring>
 
 #include <cstdint>
@@ -16,10 +17,25 @@ namespace kf {
 
 namespace {
 
-#ifndef KF_HOST_CHUNK
-#define KF_HOST_CHUNK (1 << 17)
+// Tracks per chunk.  A call costs  (copies in) + k x (starting the eleven copies of a chunk: 52 us, measured as the
+// slope of the call time against the number of chunks) + (kernel + copies out of the LAST chunk ~ 4.3 ms / k at 2 M
+// tracks), so the best number of chunks is k = sqrt(n x 4.1e-5): nine chunks of 223 232 tracks for 2 M tracks (16.6
+// ms; sixteen of 131 072: 16.9; thirty-one of 65 536: 17.7).  Chunks are multiples of 1024 tracks, so the pairs of
+// the two-tracks-per-thread kernel are the same as in one launch over the whole batch.  -DKF_HOST_CHUNK=n fixes it.
+inline int64_t host_chunk_for(int64_t n) {
+    int64_t c;
+#ifdef KF_HOST_CHUNK
+    c = KF_HOST_CHUNK;
+#else
+    const double k = std::sqrt((double)n * 4.1e-5);
+    const int64_t kk = k < 1.0 ? 1 : (int64_t)(k + 0.5);
+    c = ((n + kk - 1) / kk + 1023) / 1024 * 1024;
+    if (c < 32768) c = 32768;
+    if (c > 524288) c = 524288;
 #endif
-constexpr int64_t kDefaultChunk = KF_HOST_CHUNK;  // 131072 tracks per chunk
+    if (n <= c) c = n < 4 ? 4 : (n + 3) / 4 * 4;
+    return c;
+}
 
 inline size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
 
@@ -100,16 +116,19 @@ __global__ void __launch_bounds__(256) spread_diag_kernel(const float* __restric
 }  // namespace
 
 cudaError_t HostStage::reserve(int64_t max_tracks, int max_layers) {
-    int64_t want = max_tracks < kDefaultChunk ? ((max_tracks + 3) / 4) * 4 : kDefaultChunk;
-    if (want < 4) want = 4;
+    int64_t want = host_chunk_for(max_tracks);
     if (want <= chunk && max_layers <= layers) return cudaSuccess;
     if (want < chunk) want = chunk;
     if (max_layers < layers) max_layers = layers;
     release();
     SlotLayout lay(want, max_layers);
+    cudaError_t e0 = cudaStreamCreateWithFlags(&out_stream, cudaStreamNonBlocking);
+    if (e0 != cudaSuccess) { release(); return e0; }
     for (int s = 0; s < kSlots; ++s) {
         cudaError_t e = cudaStreamCreateWithFlags(&stream[s], cudaStreamNonBlocking);
         if (e != cudaSuccess) { release(); return e; }
+        if ((e = cudaEventCreateWithFlags(&fitted[s], cudaEventDisableTiming)) != cudaSuccess) { release(); return e; }
+        if ((e = cudaEventCreateWithFlags(&drained[s], cudaEventDisableTiming)) != cudaSuccess) { release(); return e; }
         e = cudaMalloc(&buf[s], lay.total);
         if (e != cudaSuccess) { release(); return e; }
     }
@@ -123,9 +142,14 @@ void HostStage::release() {
     for (int s = 0; s < kSlots; ++s) {
         if (buf[s]) cudaFree(buf[s]);
         if (stream[s]) cudaStreamDestroy(stream[s]);
+        if (fitted[s]) cudaEventDestroy(fitted[s]);
+        if (drained[s]) cudaEventDestroy(drained[s]);
         buf[s] = nullptr;
         stream[s] = nullptr;
+        fitted[s] = drained[s] = nullptr;
     }
+    if (out_stream) cudaStreamDestroy(out_stream);
+    out_stream = nullptr;
     chunk = 0;
     layers = 0;
     buf_bytes = 0;
@@ -134,16 +158,17 @@ void HostStage::release() {
 cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const LaunchOptions& opt) {
     cudaError_t e = reserve(io.n, io.L);
     if (e != cudaSuccess) return e;
-    const SlotLayout lay(chunk, layers);
+    const SlotLayout lay(chunk, layers);     // `chunk` = tracks a slot buffer holds = the pitch of its planes
     const int L = io.L;
     const size_t cw = (size_t)chunk * 4;  // device pitch of float planes
+    const int64_t step = host_chunk_for(io.n) < chunk ? host_chunk_for(io.n) : chunk;   // tracks per chunk of THIS call
     // every chunk takes the kernel the WHOLE batch would take in kf_fit_tracks (chunks start at multiples of 64, so
     // the pairs are the same too): host path and device path agree bit for bit
     LaunchOptions chunk_opt = opt;
     chunk_opt.pair_min_tracks = fit_takes_pair_form(io.n, L, opt) ? 1 : INT64_MAX;
     int slot = 0;
-    for (int64_t t0 = 0; t0 < io.n; t0 += chunk, slot = (slot + 1) % kSlots) {
-        const int64_t m = io.n - t0 < chunk ? io.n - t0 : chunk;
+    for (int64_t t0 = 0; t0 < io.n; t0 += step, slot = (slot + 1) % kSlots) {
+        const int64_t m = io.n - t0 < step ? io.n - t0 : step;
         cudaStream_t st = stream[slot];
         char* b = buf[slot];
         const size_t w = (size_t)m * 4;
@@ -184,22 +209,34 @@ cudaError_t HostStage::fit(const FitParams& P, const HostFitIO& io, const Launch
             a.mask = io.mask ? (const uint32_t*)(b + lay.mask) : nullptr;
             a.opar = (float*)(b + lay.opar); a.ocov = (float*)(b + lay.ocov); a.ld_out = chunk;
             a.chi2 = (float*)(b + lay.chi2); a.nhits = (int32_t*)(b + lay.nhits); a.status = (uint32_t*)(b + lay.status);
+            // the results of the chunk that used this slot before must have left (the inputs above may land earlier:
+            // they do not touch the output planes)
+            if (t0 >= (int64_t)kSlots * step) KF_TRY(cudaStreamWaitEvent(st, drained[slot], 0));
             KF_TRY(launch_fit(P, a, st, chunk_opt));
+            KF_TRY(cudaEventRecord(fitted[slot], st));
         }
-        KF_TRY(cudaMemcpy2DAsync(io.opar + t0, (size_t)io.ld_out * 4, b + lay.opar, cw, w, 6, cudaMemcpyDeviceToHost, st));
-        KF_TRY(cudaMemcpy2DAsync(io.ocov + t0, (size_t)io.ld_out * 4, b + lay.ocov, cw, w, 21, cudaMemcpyDeviceToHost, st));
-        KF_TRY(cudaMemcpyAsync(io.chi2 + t0, b + lay.chi2, w, cudaMemcpyDeviceToHost, st));
-        KF_TRY(cudaMemcpyAsync(io.nhits + t0, b + lay.nhits, w, cudaMemcpyDeviceToHost, st));
-        KF_TRY(cudaMemcpyAsync(io.status + t0, b + lay.status, w, cudaMemcpyDeviceToHost, st));
+        // results out on a stream of their own: the slot's stream carries host-to-device copies and kernels only
+        KF_TRY(cudaStreamWaitEvent(out_stream, fitted[slot], 0));
+        KF_TRY(cudaMemcpy2DAsync(io.opar + t0, (size_t)io.ld_out * 4, b + lay.opar, cw, w, 6, cudaMemcpyDeviceToHost, out_stream));
+        KF_TRY(cudaMemcpy2DAsync(io.ocov + t0, (size_t)io.ld_out * 4, b + lay.ocov, cw, w, 21, cudaMemcpyDeviceToHost, out_stream));
+        KF_TRY(cudaMemcpyAsync(io.chi2 + t0, b + lay.chi2, w, cudaMemcpyDeviceToHost, out_stream));
+        KF_TRY(cudaMemcpyAsync(io.nhits + t0, b + lay.nhits, w, cudaMemcpyDeviceToHost, out_stream));
+        KF_TRY(cudaMemcpyAsync(io.status + t0, b + lay.status, w, cudaMemcpyDeviceToHost, out_stream));
+        KF_TRY(cudaEventRecord(drained[slot], out_stream));
 #undef KF_TRY
     }
     for (int s = 0; s < kSlots; ++s) {
         cudaError_t es = cudaStreamSynchronize(stream[s]);
         if (es != cudaSuccess && e == cudaSuccess) e = es;
     }
+    {
+        cudaError_t es = cudaStreamSynchronize(out_stream);
+        if (es != cudaSuccess && e == cudaSuccess) e = es;
+    }
     return e;
 fail:
     for (int s = 0; s < kSlots; ++s) cudaStreamSynchronize(stream[s]);
+    cudaStreamSynchronize(out_stream);
     return e;
 }
 

@@ -100,6 +100,9 @@ struct HostStage {
     int64_t chunk = 0;  // tracks per chunk (multiple of 4)
     int layers = 0;
     cudaStream_t stream[kSlots] = {nullptr, nullptr, nullptr};
+    cudaStream_t out_stream = nullptr;                          // every device-to-host copy
+    cudaEvent_t fitted[kSlots] = {nullptr, nullptr, nullptr};   // chunk's kernel done (out_stream waits for it)
+    cudaEvent_t drained[kSlots] = {nullptr, nullptr, nullptr};  // chunk's results are in host memory (the slot's next kernel waits)
     char* buf[kSlots] = {nullptr, nullptr, nullptr};
     size_t buf_bytes = 0;
     cudaError_t reserve(int64_t max_tracks, int max_layers);

@@ -74,8 +74,9 @@ def test_indexed_fit_short_geometries(ctx, k, n_tracks):
 
 @pytest.mark.parametrize("n,k", [(1, 1), (131_072, 2), (131_073, 10), (5, 10), (1000, 32)])
 def test_host_path_chunk_boundaries(ctx, n, k):
-    """kf_fit_tracks_host cuts the batch into chunks of 131 072 tracks: exactly one chunk, one chunk plus one track,
-    a single track, a one-layer geometry -- same results as the resident call."""
+    """kf_fit_tracks_host cuts the batch into chunks (a multiple of 1024 tracks, their number grows with the square
+    root of the batch): two whole chunks of 65 536, two ragged ones (66 560 + 64 513), a single track, a one-layer
+    geometry -- same results as the resident call."""
     from paper_1705_02876_b200.buffers import DeviceFit
     cfg = dataclasses.replace(W.get_config(1), n_layers=k, n_tracks=n, layer_step_cm=4.0 if k <= 10 else 1.25)
     b = W.simulate_event(cfg, 31, n_tracks=n)

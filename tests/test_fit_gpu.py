@@ -240,7 +240,7 @@ def test_fit_host_path_equals_device_path(ctx):
 
 def test_fit_host_path_equals_device_path_across_chunks(ctx):
     """A batch large enough for the two-tracks-per-thread kernels (14 events = 280 000 tracks, holes in the masks of
-    some) goes through kf_fit_tracks_host in chunks of 131 072 tracks: every chunk takes the kernel the whole batch
+    some) goes through kf_fit_tracks_host in three chunks (94 208 tracks each at this size): every chunk takes the kernel the whole batch
     takes on the device path, so the two agree bit for bit, chunk boundaries and the ragged last chunk included."""
     from paper_1705_02876_b200.buffers import DeviceFit
     b = W.make_fit_batch(2, n_events=14)
@@ -317,7 +317,7 @@ def test_fit_host_path_with_local_hit_variances(ctx):
     res = compare_fit(gs, o, float(b.radius[-1]))
     print("compact host call vs oracle:", res)
     # the tail of the last chunk and the chunk boundaries, one by one
-    for lo in (131_072 - 3, 262_144 - 3, b.n - 5):
+    for lo in (94_208 - 3, 131_072 - 3, 188_416 - 3, 262_144 - 3, b.n - 5):     # (chunks of 94 208 tracks at this size)
         s2 = slice(lo, min(lo + 6, b.n))
         o2 = O.fit_tracks(b.radius, b.x_over_X0, b.Bz, b.mass, b.par[:, s2], b.cov[:, s2], b.q[s2], b.hpos[:, :, s2],
                           full[:, :, s2], b.mask[s2])

@@ -6,7 +6,7 @@
  * (arXiv:1705.02876; "seeding, building, fitting" + chi2; PAPER.md:65 6x6 track /
  * 3x3 hit matrices in global coordinates; PAPER.md:71 projective bins; PAPER.md:73 best hit =
  * lowest chi2 increment; equations: BASELINE.json:north_star).  The paper prints no formulas;
- * every formula below is a reading listed in DESIGN.md ("Readings A1..A23").
+ * every formula below is a reading listed in DESIGN.md ("Readings A1..A24").
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load this.  It shares no code, header, table or constant with the CUDA path
@@ -23,8 +23,10 @@
  * orc_chi2_increment against its definition and against orc_update (tests/test_oracle_scoring.py);
  * SM1-SM5 the RTS smoother (tests/test_oracle_smoother.py: batch WLS at every layer, exact helix, pulls);
  * R1-R5 the inward refit (tests/test_oracle_refit.py); C1-C4 combinatorial building;
- * D1-D6 endcap discs (tests/test_oracle_endcap.py: to-plane propagation vs RK4 and vs the to-radius form,
- * Jacobian, exact helix through barrels + discs, EKF == WLS, pulls).
+ * D1-D9 endcap discs (tests/test_oracle_endcap.py: to-plane propagation vs RK4 and vs the to-radius form,
+ * Jacobian, exact helix through barrels + discs, EKF and smoother == WLS, pulls, path-length material on a disc;
+ * D7-D9 scoring on a disc layer against brute force, combinatorial building with discs, the inward refit over
+ * surfaces); the bin of a disc-layer hit (reading A24) against its definition (tests/test_oracle_scoring.py).
  * Parity-unpinned: none of the functions below (efficiency / fake rate of PAPER.md:85 is not
  * computed here at all).
  */

@@ -205,3 +205,49 @@ def test_stale_graph_is_refused(ctx):
     assert c2._lib.kf_graph_launch(c2._h, g._g) == -7
     c2.close()
     g.close()
+
+
+def test_indexed_fit_in_a_graph_and_its_scratch(ctx):
+    """kf_fit_tracks_indexed without bins packs the pools into context scratch: recorded after one eager call the
+    graph replays the packing and the fit with identical results; a later call with larger pools reallocates that
+    scratch and the graph is refused (KF_ERR_STALE) instead of reading freed memory."""
+    import paper_1705_02876_b200 as K
+    from paper_1705_02876_b200.buffers import DeviceFit, DeviceLayer, padded_ld
+
+    def setup(n_tracks, noise):
+        ev = W.make_build_event(4, n_tracks=n_tracks, noise_hits=noise)
+        f = ev.fit
+        d = DeviceFit.from_batch(f, "cuda:0")
+        pools = [DeviceLayer.from_numpy(l.pos, l.cov, NE, NP, EMAX, "cuda:0") for l in ev.layers]
+        idx = torch.full((len(ev.layers), padded_ld(f.n)), -1, dtype=torch.int32, device="cuda:0")
+        idx[:, :f.n] = torch.from_numpy(np.stack([l.true_index for l in ev.layers]).astype(np.int32)).to("cuda:0")
+
+        def call():
+            ctx.fit_tracks_indexed(d.geom, f.n, d.par, d.cov, d.q, idx, [(p.n_hits, p.pos, p.cov) for p in pools],
+                                   d.out_par, d.out_cov, d.out_chi2, d.out_nhits, d.out_status)
+        return d, call, (pools, idx)
+
+    d, call, keep = setup(3000, 6000)
+    with torch.cuda.stream(ctx.torch_stream):
+        call()
+    torch.cuda.synchronize()
+    want = d.results()
+    ctx.graph_begin()
+    call()
+    g = ctx.graph_end()
+    d.out_par.zero_(); d.out_cov.zero_(); d.out_chi2.zero_()
+    torch.cuda.synchronize()
+    g.launch()
+    torch.cuda.synchronize()
+    got = d.results()
+    for k in want:
+        assert np.array_equal(got[k], want[k], equal_nan=True), k
+    assert np.count_nonzero(got["chi2"]) > 2900
+    d2, call2, keep2 = setup(9000, 20000)           # larger pools: the scratch grows
+    with torch.cuda.stream(ctx.torch_stream):
+        call2()
+    torch.cuda.synchronize()
+    with pytest.raises(K.KFError) as e:
+        g.launch()
+    assert e.value.code == -7
+    g.close()

@@ -107,7 +107,8 @@ enum {
                                      sort, 2 = the chunked sort wherever it applies                         */
 };
 KF_API int kf_set_option(kf_ctx* ctx, int option, int64_t value);
-/* Pre-size scratch so that no later call allocates: `max_hits` hits in total over the layers of one kf_bin_layers call,
+/* Pre-size scratch so that no later call allocates: `max_hits` hits in total over the layers of one kf_bin_layers call
+ * (or over the pools of one kf_fit_tracks_indexed call without bins, which packs them into 48-byte records),
  * `max_host_tracks` x `max_host_layers` for the *_host staging buffers (0 = leave as is). */
 KF_API int kf_reserve(kf_ctx* ctx, int64_t max_hits, int64_t max_host_tracks, int max_host_layers);
 /* Static, never NULL. */

@@ -323,6 +323,7 @@ int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_hos
     if (max_hits > 0) {
         e = c->bin.reserve(max_hits, 2 * (KF_MAX_BINS + 1), c->stream, true);
         if (e == cudaSuccess) e = reserve_chunked(c->bin, max_hits, KF_MAX_LAYERS, c->stream);
+        if (e == cudaSuccess) e = c->index.reserve((size_t)(max_hits + 4 * KF_MAX_LAYERS) * kRecFloats * 4, c->stream);
         if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     }
     if (max_host_tracks > 0 && max_host_layers > 0) {

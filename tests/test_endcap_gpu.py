@@ -103,6 +103,31 @@ def test_endcap_ragged_sizes_and_host_path(ctx, n):
         assert np.array_equal(g[k], h[k], equal_nan=True), k
 
 
+@pytest.mark.parametrize("n", [1, 33, 20000])
+def test_endcap_compact_host_call(ctx, n):
+    """kf_fit_tracks_host_compact on the barrel + endcap toy: a hit on a disc carries the same kind of covariance
+    (resolutions along the radius, r-phi and z in the hit's own frame), so three variances per hit describe it; layers a
+    track has no hit on hold zeros (rho = 0: the rebuilding step must not make NaNs of them).  Against the oracle given
+    the covariance the header defines, in fp64 from the same fp32 positions and variances."""
+    import copy
+    from paper_1705_02876_b200.buffers import DeviceFit, _to_planes
+    from tests.test_fit_gpu import _local_hit_variances
+    b = copy.copy(W.simulate_endcap_event(3, n))
+    var, full = _local_hit_variances(b, np.random.default_rng(n))
+    has = ((b.mask[None, :] >> np.arange(b.n_layers, dtype=np.uint32)[:, None]) & 1) == 1
+    var = np.where(has[:, None, :], var, 0.0).astype(np.float32)
+    full = np.where(has[:, None, :], full, 0.0)
+    off = np.setdiff1d(np.arange(21), [0, 6, 11, 15, 18, 20])
+    assert np.all(b.cov[off] == 0.0)
+    h = DeviceFit.from_batch(b, "cpu", pin=True)
+    h.fit_host(ctx, cov_diagonal=True, hit_var=_to_planes(var, h.ld, torch.device("cpu"), True))
+    g = h.results()
+    assert np.all(np.isfinite(g["par"])) and np.all(np.isfinite(g["cov"]))
+    b.hcov = full
+    o = O.fit_batch(b, nthreads=8)
+    _compare(g, o, b, min_same=0.995 if n > 1000 else 0.0)
+
+
 def test_endcap_with_path_length_material(ctx):
     b = W.simulate_endcap_event(5, 8000, material_model=1)
     g, o = _fit_both(ctx, b)

@@ -96,6 +96,19 @@ def _opcode_flops(name: str) -> float | None:
     return None
 
 
+def _opcode_counts(name: str) -> dict:
+    """Thread-level executed instructions per opcode of one launch (same file as _opcode_flops)."""
+    p = os.path.join(ROOT, "profiles", name)
+    out = {}
+    if os.path.exists(p):
+        with open(p) as f:
+            for line in f:
+                k = line.strip().split(",")
+                if len(k) == 3 and k[0] not in ("opcode", "TOTAL"):
+                    out[k[0]] = float(k[1])
+    return out
+
+
 def _kernel_counters(counters: dict, fragment: str) -> dict | None:
     for name, d in counters.items():
         if fragment in name:
@@ -715,6 +728,7 @@ def run_ours(args) -> None:
         else:
             host_vs_dev[key + "_equal"] = bool(np.array_equal(a, b))
     fp32_peak = ctx.measure_fp32_peak(5) if rank == 0 else 0.0
+    packed_shared, packed_distinct = ctx.measure_fp32_packed_rate(3) if rank == 0 else (0.0, 0.0)
     building = measure_building(ctx, dev) if (rank == 0 and not args.no_building) else None
     ctx.set_stream(stream)          # measure_building borrowed the context for torch's current stream
     smoothing = None
@@ -933,6 +947,24 @@ def run_ours(args) -> None:
                "executed_source": "SASS opcode histogram of the ncu capture: FFMA2 = 4, FMUL2 / FADD2 = 2, FFMA = 2, "
                                   "FMUL / FADD / MUFU = 1 flop per thread instruction (profiles/r02_fit_pair_opcodes.csv, "
                                   "profiles/r02_counters.md)"}
+        # What the register file lets the packed instructions do.  FFMA2 reads three 64-bit register pairs; with three
+        # DISTINCT pairs it issues at about 2/3 of the rate it reaches when operands repeat (measured now, both ways),
+        # FMUL2 / FADD2 (two pairs) run at the pipe's rate.  Floor of this kernel's own instruction mix (thread
+        # instructions from the opcode histogram of the ncu capture, scaled to n): every FFMA2 at the distinct rate
+        # (upper floor) / at the shared rate (lower floor = the FMA pipe alone); 24 % of the kernel's FFMA2 carry an
+        # operand-reuse flag in the SASS, so the truth lies near the upper one.
+        oc = _opcode_counts("r02_fit_pair_opcodes.csv")
+        if oc.get("FFMA2") and packed_distinct > 0:
+            sc_n = n / 2.0e6
+            r_sh, r_di = packed_shared * 1e12 / 4.0, packed_distinct * 1e12 / 4.0     # thread instructions per second
+            two_op = (oc.get("FMUL2", 0.0) + oc.get("FADD2", 0.0)) * sc_n
+            f_hi = oc["FFMA2"] * sc_n / r_di + two_op / r_sh
+            f_lo = (oc["FFMA2"] * sc_n + two_op) / r_sh
+            alu["packed_fp32"] = {"ffma2_shared_operands_tflops": packed_shared, "ffma2_distinct_operands_tflops": packed_distinct,
+                                  "source": "kf_measure_fp32_packed_rate, measured now",
+                                  "thread_instructions_per_launch": {k: oc.get(k, 0.0) * sc_n for k in ("FFMA2", "FMUL2", "FADD2")},
+                                  "floor_ms_fma_pipe_alone": 1e3 * f_lo, "floor_ms_ffma2_with_distinct_operands": 1e3 * f_hi,
+                                  "frac_of_distinct_operand_floor": f_hi / t_launch, "frac_of_pipe_floor": f_lo / t_launch}
         # the binding roofline is the one with the larger lower bound on time under the frozen algorithmic counts
         # (SURVEY.md 8(d)); `implementation_floor` is the larger bound for the work this kernel really does.
         roofline, other = (alu, hbm) if alg_flops / (fp32_peak * 1e12) > alg_bytes / (peak * 1e9) else (hbm, alu)

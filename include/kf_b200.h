@@ -140,6 +140,12 @@ KF_API int kf_graph_destroy(kf_graph* graph);
  * from a register-only FMA microbenchmark (8 independent chains per thread, 2048 threads per SM, best
  * of `repeats` launches).  Synchronises the stream.  This is the denominator of the ALU roofline. */
 KF_API int kf_measure_fp32_peak(kf_ctx* ctx, int repeats, double* tflops_out);
+/* The same for the packed instruction the two-tracks-per-thread kernels are made of (FFMA2, one fp32x2 FMA per lane:
+ * 4 flop): `shared_tflops` with two of the three operands shared by every chain (the FMA pipe's own rate),
+ * `distinct_tflops` with three distinct register pairs per instruction, which is what arithmetic on per-track
+ * matrices issues and what the register file can feed (about 2/3 of the former on B200).  Synchronises the stream;
+ * not to be called while recording a graph. */
+KF_API int kf_measure_fp32_packed_rate(kf_ctx* ctx, int repeats, double* shared_tflops, double* distinct_tflops);
 /* ABI version, bumped when a struct or signature changes. */
 KF_API int kf_abi_version(void);
 /* Floats per packed hit record of kf_layer_bins.hit_rec as this build writes it (= KF_HIT_RECORD_FLOATS). */

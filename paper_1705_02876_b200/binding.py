@@ -25,7 +25,7 @@ BIN_FORM_AUTO, BIN_FORM_FIVE_LAUNCH, BIN_FORM_CHUNKED = 0, 1, 2
 STATIC_MAX_CANDIDATES = 65536                                               # KF_STATIC_MAX_CANDIDATES
 ERR_TOO_LARGE = -8
 EXPORTS = ["kf_create", "kf_destroy", "kf_set_stream", "kf_set_option", "kf_reserve", "kf_strerror", "kf_last_cuda_error",
-           "kf_abi_version", "kf_hit_record_floats", "kf_measure_fp32_peak", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_fit_tracks_host_diag", "kf_fit_tracks_host_compact", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
+           "kf_abi_version", "kf_hit_record_floats", "kf_measure_fp32_peak", "kf_measure_fp32_packed_rate", "kf_fit_tracks", "kf_fit_tracks_indexed", "kf_fit_tracks_refit", "kf_fit_tracks_smooth", "kf_fit_tracks_host", "kf_fit_tracks_host_diag", "kf_fit_tracks_host_compact", "kf_bin_hits", "kf_bin_layers", "kf_order_candidates",
            "kf_score_candidates", "kf_score_candidates_static", "kf_build_best_hit", "kf_build_best_hit_events", "kf_build_best_hit_host", "kf_build_combinatorial", "kf_build_combinatorial_events",
            "kf_graph_begin", "kf_graph_end", "kf_graph_launch", "kf_graph_destroy"]
 
@@ -111,6 +111,8 @@ def load_library():
     lib.kf_last_cuda_error.argtypes = [vp]
     lib.kf_measure_fp32_peak.restype = C.c_int
     lib.kf_measure_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
+    lib.kf_measure_fp32_packed_rate.restype = C.c_int
+    lib.kf_measure_fp32_packed_rate.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.kf_abi_version.restype = C.c_int
     lib.kf_abi_version.argtypes = []
     lib.kf_hit_record_floats.restype = C.c_int
@@ -345,6 +347,13 @@ class KFContext:
         out = C.c_double(0.0)
         self._check(self._lib.kf_measure_fp32_peak(self._h, int(repeats), C.byref(out)), "kf_measure_fp32_peak")
         return float(out.value)
+
+    def measure_fp32_packed_rate(self, repeats: int = 5) -> tuple[float, float]:
+        """(shared, distinct) TFLOP/s of FFMA2 with shared operands / with three distinct register pairs."""
+        a, b = C.c_double(0.0), C.c_double(0.0)
+        self._check(self._lib.kf_measure_fp32_packed_rate(self._h, int(repeats), C.byref(a), C.byref(b)),
+                    "kf_measure_fp32_packed_rate")
+        return float(a.value), float(b.value)
 
     # ------------------------------------------------------------------ marshalling helpers
     @staticmethod

@@ -42,7 +42,7 @@ struct kf_ctx {
 
 namespace {
 
-constexpr int kAbiVersion = 13;
+constexpr int kAbiVersion = 14;
 static_assert(kRecFloats == KF_HIT_RECORD_FLOATS || kRecWords == 4, "kf_internal.h and kf_b200.h disagree on the hit record");
 
 // Makes the context's device current for the duration of an ABI call and puts the caller's device back on
@@ -330,6 +330,25 @@ int kf_reserve(kf_ctx* c, int64_t max_hits, int64_t max_host_tracks, int max_hos
         e = c->host.reserve(max_host_tracks, max_host_layers);
         if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? KF_ERR_NOMEM : cuda_fail(c, e);
     }
+    return KF_OK;
+}
+
+int kf_measure_fp32_packed_rate(kf_ctx* c, int repeats, double* shared_tflops, double* distinct_tflops) {
+    if (!c || !shared_tflops || !distinct_tflops) return KF_ERR_NULL;
+    if (repeats < 1) return KF_ERR_SHAPE;
+    if (c->capturing) return KF_ERR_UNSUPPORTED;
+    KF_ON_DEVICE(c);
+    cudaError_t e;
+    constexpr int kWords = 32 * 3 * 8 * 2 + 4;
+    float* scratch = nullptr;
+    if ((e = cudaMalloc(&scratch, kWords * 4)) != cudaSuccess) return cuda_fail(c, e);
+    static float init[kWords];
+    for (int i = 0; i < kWords; ++i) init[i] = 0.999f + 1e-5f * (float)(i % 7);
+    e = cudaMemcpyAsync(scratch, init, kWords * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e == cudaSuccess) e = measure_fp32_packed_rate(c->stream, repeats, scratch, shared_tflops, distinct_tflops);
+    cudaFree(scratch);
+    if (e != cudaSuccess) return cuda_fail(c, e);
     return KF_OK;
 }
 

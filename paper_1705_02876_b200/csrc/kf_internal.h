@@ -358,5 +358,7 @@ cudaError_t build_best_hit_host(BuildHostStage& hs, BinScratch& bs, ScoreScratch
 
 // kf_peak.cu
 double measure_fp32_peak(cudaStream_t stream, int repeats, float* sink);
+cudaError_t measure_fp32_packed_rate(cudaStream_t stream, int repeats, float* scratch, double* shared_tflops,
+                                     double* distinct_tflops);
 
 }  // namespace kf

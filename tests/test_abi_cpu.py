@@ -44,7 +44,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_abi_version_and_error_strings(lib):
     import paper_1705_02876_b200 as K
-    assert K.abi_version() == 13
+    assert K.abi_version() == 14
     assert K.binding.hit_record_floats() == 12
     seen = set()
     for code in (0, -1, -2, -3, -4, -5, -6, -7, -99):

@@ -66,3 +66,15 @@ def test_calls_restore_the_callers_current_device():
         assert np.array_equal(v, r[k], equal_nan=True), k
     ctx.close()
     assert torch.cuda.current_device() == 0
+
+
+def test_packed_fp32_rate_measurement():
+    """kf_measure_fp32_packed_rate: FFMA2 with shared operands runs at the FP32 peak of kf_measure_fp32_peak (4 flop per
+    lane and instruction, one instruction every two cycles), with three distinct register pairs clearly below it."""
+    import paper_1705_02876_b200 as K
+    c = K.KFContext(0)
+    peak = c.measure_fp32_peak(2)
+    shared, distinct = c.measure_fp32_packed_rate(2)
+    c.close()
+    assert 0.9 * peak < shared < 1.05 * peak, (peak, shared)
+    assert 0.5 * shared < distinct < 0.85 * shared, (shared, distinct)
